@@ -1,0 +1,669 @@
+/*
+ * kf_oracle.c -- CPU ORACLE (test infrastructure, see kf_oracle.h).
+ *
+ * Step-by-step restatement of the per-track Kalman fit, in the order and notation of
+ * SURVEY.md section 8(c) C.2 (the paper names the steps at PAPER.md:55-62 and 128 but prints no
+ * formula; the formulas below are derived from the definitions those passages name).
+ * Dense row-major matrices, plain loops, IEEE double, no blocking, no structure exploitation,
+ * no fused or reordered arithmetic.  Build: gcc -O2 -ffp-contract=off -fopenmp.
+ */
+#include "kf_oracle.h"
+
+#include <math.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ---- constants (the CUDA path carries its own copy) ------------- */
+static const double TESLA_TO_GEV_PER_MM = 2.99792458e-4; /* 1 T = 2.99792458e-4 GeV/(e mm) */
+static const double ME_GEV = 0.51099895e-3;              /* electron mass */
+static const double K_BETHE = 0.307075;                  /* MeV mol^-1 cm^2 */
+static const double NT_MIN = 1e-6;                       /* surface reachable if n.T > NT_MIN */
+static const double SIN_THETA_MIN = 1e-12;
+static const int MAX_SUBSTEPS = 1024;
+static const double PI = 3.14159265358979323846;
+
+/* ---- tiny dense helpers ------------------------------------------------------------------- */
+static void cross3(const double a[3], const double b[3], double c[3]) {
+  c[0] = a[1] * b[2] - a[2] * b[1];
+  c[1] = a[2] * b[0] - a[0] * b[2];
+  c[2] = a[0] * b[1] - a[1] * b[0];
+}
+static double dot3(const double a[3], const double b[3]) {
+  return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
+}
+/* C (n x m) = A (n x k) * B (k x m) */
+static void matmul(int n, int k, int m, const double* A, const double* B, double* C) {
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < m; ++j) {
+      double s = 0.0;
+      for (int l = 0; l < k; ++l) s += A[i * k + l] * B[l * m + j];
+      C[i * m + j] = s;
+    }
+}
+/* C (n x m) = A (n x k) * B^T, B is (m x k) */
+static void matmul_bt(int n, int k, int m, const double* A, const double* B, double* C) {
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < m; ++j) {
+      double s = 0.0;
+      for (int l = 0; l < k; ++l) s += A[i * k + l] * B[j * k + l];
+      C[i * m + j] = s;
+    }
+}
+static void symmetrise6(double C[36]) {
+  for (int i = 0; i < 6; ++i)
+    for (int j = i + 1; j < 6; ++j) {
+      double a = 0.5 * (C[i * 6 + j] + C[j * 6 + i]);
+      C[i * 6 + j] = a;
+      C[j * 6 + i] = a;
+    }
+}
+static int all_finite(const double* a, int n) {
+  for (int i = 0; i < n; ++i)
+    if (!isfinite(a[i])) return 0;
+  return 1;
+}
+static double wrap_pi(double a) { /* into (-pi, pi] */
+  while (a > PI) a -= 2.0 * PI;
+  while (a <= -PI) a += 2.0 * PI;
+  return a;
+}
+
+/* ---- field (C.2.2 "Field") ----------------------------------------------------------------- */
+void kfo_field_at(const kfo_field* fld, const double r[3], double b[3], int32_t* clamped) {
+  if (fld->kind == KFO_FIELD_CONST) {
+    b[0] = fld->b[0]; b[1] = fld->b[1]; b[2] = fld->b[2];
+    return;
+  }
+  /* trilinear: per axis f = (r_a - origin_a)/spacing_a, i = clamp(floor f, 0, n_a-2),
+     w = clamp(f - i, 0, 1); outside the grid the clamped value is used */
+  int idx[3];
+  double w[3];
+  for (int a = 0; a < 3; ++a) {
+    double f = (r[a] - fld->origin[a]) / fld->spacing[a];
+    double fl = floor(f);
+    if (fl < 0.0) fl = 0.0;
+    if (fl > (double)(fld->n[a] - 2)) fl = (double)(fld->n[a] - 2);
+    double ww = f - fl;
+    if (ww < 0.0) { ww = 0.0; if (clamped) *clamped |= 1; }
+    if (ww > 1.0) { ww = 1.0; if (clamped) *clamped |= 1; }
+    idx[a] = (int)fl;
+    w[a] = ww;
+  }
+  const int nx = fld->n[0], ny = fld->n[1];
+  b[0] = b[1] = b[2] = 0.0;
+  for (int dz = 0; dz < 2; ++dz)
+    for (int dy = 0; dy < 2; ++dy)
+      for (int dx = 0; dx < 2; ++dx) {
+        double wt = (dx ? w[0] : 1.0 - w[0]) * (dy ? w[1] : 1.0 - w[1]) * (dz ? w[2] : 1.0 - w[2]);
+        const double* node =
+            fld->grid + 3 * ((size_t)(idx[2] + dz) * ny * nx + (size_t)(idx[1] + dy) * nx + (idx[0] + dx));
+        b[0] += wt * node[0];
+        b[1] += wt * node[1];
+        b[2] += wt * node[2];
+      }
+}
+
+static void field_internal(const kfo_field* fld, const double r[3], double B[3], int32_t* clamped) {
+  double bt[3];
+  kfo_field_at(fld, r, bt, clamped);
+  for (int a = 0; a < 3; ++a) B[a] = bt[a] * TESLA_TO_GEV_PER_MM; /* dT/ds = lam T x B */
+}
+
+/* M(B) a := a x B */
+static void cross_matrix(const double B[3], double M[9]) {
+  M[0] = 0.0;   M[1] = B[2];  M[2] = -B[1];
+  M[3] = -B[2]; M[4] = 0.0;   M[5] = B[0];
+  M[6] = B[1];  M[7] = -B[0]; M[8] = 0.0;
+}
+
+/* ---- C.2.2: one RKN4 step with its step Jacobian -------------------------------------------- */
+void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double h, double fo[8],
+                   double Ds[64], double* eps, int32_t* clamped) {
+  const double* r = f;
+  const double t = f[3];
+  const double* T = f + 4;
+  const double lam = f[7];
+  double B1[3], B2[3], B3[3], k1[3], k2[3], k3[3], k4[3], tmp[3], rm[3], re[3];
+  double T2[3], T3[3], T4[3];
+
+  /* stages; the field is sampled at 3 points, stages 2 and 3 share the midpoint */
+  field_internal(fld, r, B1, clamped);
+  cross3(T, B1, tmp);
+  for (int a = 0; a < 3; ++a) k1[a] = lam * tmp[a];
+  for (int a = 0; a < 3; ++a) rm[a] = r[a] + 0.5 * h * T[a] + 0.125 * h * h * k1[a];
+  field_internal(fld, rm, B2, clamped);
+  for (int a = 0; a < 3; ++a) T2[a] = T[a] + 0.5 * h * k1[a];
+  cross3(T2, B2, tmp);
+  for (int a = 0; a < 3; ++a) k2[a] = lam * tmp[a];
+  for (int a = 0; a < 3; ++a) T3[a] = T[a] + 0.5 * h * k2[a];
+  cross3(T3, B2, tmp);
+  for (int a = 0; a < 3; ++a) k3[a] = lam * tmp[a];
+  for (int a = 0; a < 3; ++a) re[a] = r[a] + h * T[a] + 0.5 * h * h * k3[a];
+  field_internal(fld, re, B3, clamped);
+  for (int a = 0; a < 3; ++a) T4[a] = T[a] + h * k3[a];
+  cross3(T4, B3, tmp);
+  for (int a = 0; a < 3; ++a) k4[a] = lam * tmp[a];
+
+  /* state */
+  double Tn[3], norm = 0.0;
+  for (int a = 0; a < 3; ++a) {
+    fo[a] = r[a] + h * T[a] + h * h / 6.0 * (k1[a] + k2[a] + k3[a]);
+    Tn[a] = T[a] + h / 6.0 * (k1[a] + 2.0 * k2[a] + 2.0 * k3[a] + k4[a]);
+    norm += Tn[a] * Tn[a];
+  }
+  norm = sqrt(norm);
+  for (int a = 0; a < 3; ++a) fo[4 + a] = Tn[a] / norm;
+  const double dtds = sqrt(1.0 + mass * mass * lam * lam); /* dt/ds = 1/beta, |q| = 1 */
+  fo[3] = t + h * dtds;
+  fo[7] = lam;
+
+  /* embedded error estimate (diagnostic only) */
+  double e = 0.0;
+  for (int a = 0; a < 3; ++a) e += fabs(k1[a] - k2[a] - k3[a] + k4[a]);
+  if (eps) *eps = h * h * e;
+
+  if (!Ds) return;
+  /* step Jacobian, field gradient neglected (reading U4) */
+  double M1[9], M2[9], M3[9], d1[9], d2[9], d3[9], d4[9], P[9];
+  cross_matrix(B1, M1);
+  cross_matrix(B2, M2);
+  cross_matrix(B3, M3);
+  for (int i = 0; i < 9; ++i) d1[i] = lam * M1[i];
+  for (int i = 0; i < 9; ++i) P[i] = 0.5 * h * d1[i];
+  P[0] += 1.0; P[4] += 1.0; P[8] += 1.0;
+  matmul(3, 3, 3, M2, P, d2);
+  for (int i = 0; i < 9; ++i) d2[i] *= lam;
+  for (int i = 0; i < 9; ++i) P[i] = 0.5 * h * d2[i];
+  P[0] += 1.0; P[4] += 1.0; P[8] += 1.0;
+  matmul(3, 3, 3, M2, P, d3);
+  for (int i = 0; i < 9; ++i) d3[i] *= lam;
+  for (int i = 0; i < 9; ++i) P[i] = h * d3[i];
+  P[0] += 1.0; P[4] += 1.0; P[8] += 1.0;
+  matmul(3, 3, 3, M3, P, d4);
+  for (int i = 0; i < 9; ++i) d4[i] *= lam;
+
+  double l1[3], l2[3], l3[3], l4[3], q[3], c1[3], c2[3];
+  cross3(T, B1, l1);
+  cross3(T2, B2, c1);
+  for (int a = 0; a < 3; ++a) q[a] = 0.5 * h * l1[a];
+  cross3(q, B2, c2);
+  for (int a = 0; a < 3; ++a) l2[a] = c1[a] + lam * c2[a];
+  cross3(T3, B2, c1);
+  for (int a = 0; a < 3; ++a) q[a] = 0.5 * h * l2[a];
+  cross3(q, B2, c2);
+  for (int a = 0; a < 3; ++a) l3[a] = c1[a] + lam * c2[a];
+  cross3(T4, B3, c1);
+  for (int a = 0; a < 3; ++a) q[a] = h * l3[a];
+  cross3(q, B3, c2);
+  for (int a = 0; a < 3; ++a) l4[a] = c1[a] + lam * c2[a];
+
+  memset(Ds, 0, 64 * sizeof(double));
+  for (int i = 0; i < 8; ++i) Ds[i * 8 + i] = 1.0;
+  for (int i = 0; i < 3; ++i) {
+    for (int j = 0; j < 3; ++j) {
+      /* dr'/dT = h I + h^2/6 (d1+d2+d3);  dT'/dT = I + h/6 (d1+2d2+2d3+d4) */
+      Ds[i * 8 + (4 + j)] = (i == j ? h : 0.0) + h * h / 6.0 * (d1[i * 3 + j] + d2[i * 3 + j] + d3[i * 3 + j]);
+      Ds[(4 + i) * 8 + (4 + j)] =
+          (i == j ? 1.0 : 0.0) + h / 6.0 * (d1[i * 3 + j] + 2.0 * d2[i * 3 + j] + 2.0 * d3[i * 3 + j] + d4[i * 3 + j]);
+    }
+    Ds[i * 8 + 7] = h * h / 6.0 * (l1[i] + l2[i] + l3[i]);                        /* dr'/dlam */
+    Ds[(4 + i) * 8 + 7] = h / 6.0 * (l1[i] + 2.0 * l2[i] + 2.0 * l3[i] + l4[i]);  /* dT'/dlam */
+  }
+  Ds[3 * 8 + 7] = h * mass * mass * lam / dtds; /* dt'/dlam */
+}
+
+/* ---- C.2.1 - C.2.3: bound -> bound propagation with the 6x6 Jacobian ------------------------ */
+int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double x[6],
+                      const double* sf, const double* st, double xo[6], double J[36],
+                      double free_out[8], double* rk_err, int32_t* clamped) {
+  const double *cf = sf, *uf = sf + 3, *vf = sf + 6;
+  const double *ct = st, *ut = st + 3, *vt = st + 6, *nt = st + 9;
+  const double mass = opt->mass_gev;
+
+  /* C.2.1 bound -> free on the start surface */
+  const double sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
+  double f[8];
+  for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
+  f[3] = x[5];
+  f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
+  f[7] = x[4];
+  double Jb2f[48];
+  memset(Jb2f, 0, sizeof(Jb2f));
+  for (int a = 0; a < 3; ++a) {
+    Jb2f[a * 6 + 0] = uf[a];
+    Jb2f[a * 6 + 1] = vf[a];
+  }
+  Jb2f[3 * 6 + 5] = 1.0;
+  Jb2f[4 * 6 + 2] = -sphi * sth; Jb2f[4 * 6 + 3] = cphi * cth;
+  Jb2f[5 * 6 + 2] = cphi * sth;  Jb2f[5 * 6 + 3] = sphi * cth;
+  Jb2f[6 * 6 + 2] = 0.0;         Jb2f[6 * 6 + 3] = -sth;
+  Jb2f[7 * 6 + 4] = 1.0;
+
+  /* C.2.2 stepping: exactly n_sub + n_corr RKN4 steps, no tolerance test, no early exit */
+  double D[64], Ds[64], Dn[64];
+  memset(D, 0, sizeof(D));
+  for (int i = 0; i < 8; ++i) D[i * 8 + i] = 1.0;
+  double errmax = 0.0;
+  int n_sub = 1;
+  {
+    double nT = dot3(nt, f + 4);
+    if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
+    double dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
+    double s0 = dot3(nt, dr) / nT;
+    if (isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
+      double q = ceil(fabs(s0) / opt->max_step_mm * (1.0 - 1e-12));
+      if (!(q >= 1.0)) q = 1.0;
+      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      n_sub = (int)q;
+    }
+  }
+  const int n_steps = n_sub + opt->n_corr_steps;
+  for (int is = 0; is < n_steps; ++is) {
+    double nT = dot3(nt, f + 4);
+    if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
+    double dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
+    double h = dot3(nt, dr) / nT;
+    if (is < n_sub) h = h / (double)(n_sub - is); /* the last primary step aims at the plane */
+    double fn[8], e = 0.0;
+    kfo_rkn4_step(fld, mass, f, h, fn, Ds, &e, clamped);
+    if (e > errmax) errmax = e;
+    matmul(8, 8, 8, Ds, D, Dn);
+    memcpy(D, Dn, sizeof(D));
+    memcpy(f, fn, sizeof(f));
+    if (!all_finite(f, 8)) return KFO_ST_PROPAGATION;
+  }
+  if (rk_err) *rk_err = errmax;
+
+  /* C.2.3 free -> bound with the path-length correction */
+  const double* r = f;
+  const double* T = f + 4;
+  const double lam = f[7];
+  const double nT = dot3(nt, T);
+  if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
+  double B[3], TxB[3];
+  field_internal(fld, r, B, clamped);
+  cross3(T, B, TxB);
+  double fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
+                  lam * TxB[0], lam * TxB[1], lam * TxB[2], 0.0};
+  double w[8] = {nt[0] / nT, nt[1] / nT, nt[2] / nT, 0.0, 0.0, 0.0, 0.0, 0.0};
+  double Pm[64];
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 8; ++j) Pm[i * 8 + j] = (i == j ? 1.0 : 0.0) - fp[i] * w[j];
+  double Dt[64];
+  matmul(8, 8, 8, Pm, D, Dt);
+
+  const double thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
+  const double phn = atan2(T[1], T[0]);
+  const double s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
+  if (!(s2 > SIN_THETA_MIN)) return KFO_ST_THETA;
+  double dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
+  xo[0] = dot3(ut, dr);
+  xo[1] = dot3(vt, dr);
+  xo[2] = phn;
+  xo[3] = thn;
+  xo[4] = lam;
+  xo[5] = f[3];
+  double Jf2b[48];
+  memset(Jf2b, 0, sizeof(Jf2b));
+  for (int a = 0; a < 3; ++a) {
+    Jf2b[0 * 8 + a] = ut[a];
+    Jf2b[1 * 8 + a] = vt[a];
+  }
+  Jf2b[2 * 8 + 4] = -sp / s2; Jf2b[2 * 8 + 5] = cp / s2; Jf2b[2 * 8 + 6] = 0.0;
+  Jf2b[3 * 8 + 4] = cp * c2;  Jf2b[3 * 8 + 5] = sp * c2; Jf2b[3 * 8 + 6] = -s2;
+  Jf2b[4 * 8 + 7] = 1.0;
+  Jf2b[5 * 8 + 3] = 1.0;
+  double A68[48];
+  matmul(6, 8, 8, Jf2b, Dt, A68);
+  matmul(6, 8, 6, A68, Jb2f, J);
+  if (free_out) memcpy(free_out, f, sizeof(f));
+  if (!all_finite(xo, 6) || !all_finite(J, 36)) return KFO_ST_PROPAGATION;
+  return 0;
+}
+
+/* ---- C.2.4: gain-matrix update ------------------------------------------------ */
+int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], const double V[4],
+                   double xf[6], double Cf[36], double* chi2) {
+  /* H = first two rows of I6 */
+  const double r0 = m[0] - xp[0], r1 = m[1] - xp[1];
+  const double S00 = Cp[0] + V[0], S01 = Cp[1] + V[1], S10 = Cp[6] + V[2], S11 = Cp[7] + V[3];
+  const double det = S00 * S11 - S01 * S10;
+  if (!(S00 > 0.0 && det > 0.0)) return KFO_ST_NOT_POSITIVE; /* S must be positive definite */
+  const double Si00 = S11 / det, Si01 = -S01 / det, Si10 = -S10 / det, Si11 = S00 / det;
+  *chi2 = r0 * (Si00 * r0 + Si01 * r1) + r1 * (Si10 * r0 + Si11 * r1);
+  double K[12]; /* 6x2 = C H^T S^-1 */
+  for (int i = 0; i < 6; ++i) {
+    K[i * 2 + 0] = Cp[i * 6 + 0] * Si00 + Cp[i * 6 + 1] * Si10;
+    K[i * 2 + 1] = Cp[i * 6 + 0] * Si01 + Cp[i * 6 + 1] * Si11;
+  }
+  for (int i = 0; i < 6; ++i) xf[i] = xp[i] + K[i * 2 + 0] * r0 + K[i * 2 + 1] * r1;
+  /* C+ = (I - K H) C- */
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j)
+      Cf[i * 6 + j] = Cp[i * 6 + j] - (K[i * 2 + 0] * Cp[0 * 6 + j] + K[i * 2 + 1] * Cp[1 * 6 + j]);
+  symmetrise6(Cf);
+  return 0;
+}
+
+/* ---- C.2.5: material after the update -------------------------------------------------------- */
+int32_t kfo_material(const kfo_options* opt, const double* surf, const double xf[6],
+                     const double Cf[36], double xo[6], double Co[36], double* g_out,
+                     double* theta0_out, double* dE_out) {
+  const double* n = surf + 9;
+  const double xX0 = surf[14], thick = surf[15];
+  const double m = opt->mass_gev;
+  const double lam = xf[4];
+  const double sth = sin(xf[3]), cth = cos(xf[3]), sph = sin(xf[2]), cph = cos(xf[2]);
+  const double T[3] = {cph * sth, sph * sth, cth};
+  const double p = 1.0 / fabs(lam);
+  const double E = sqrt(p * p + m * m);
+  const double beta = p / E, gamma = E / m;
+  const double cfac = 1.0 / fabs(dot3(n, T)); /* path factor */
+
+  /* multiple scattering, Highland (PDG form) */
+  const double X = xX0 * cfac;
+  const double theta0 = 0.0136 / (beta * p) * sqrt(X) * (1.0 + 0.038 * log(X / (beta * beta)));
+
+  /* mean energy loss, Bethe with the asymptotic density correction */
+  const double bg = p / m;
+  const double I = opt->mat_I_eV * 1e-9; /* GeV */
+  const double ZA = opt->mat_Z / opt->mat_A;
+  const double Wmax = 2.0 * ME_GEV * bg * bg / (1.0 + 2.0 * gamma * ME_GEV / m + (ME_GEV / m) * (ME_GEV / m));
+  const double hwp = 28.816e-9 * sqrt(opt->mat_rho * ZA); /* GeV */
+  double dhalf = log(hwp / I) + log(bg) - 0.5;
+  if (dhalf < 0.0) dhalf = 0.0;
+  const double dedx_mass =
+      K_BETHE * ZA / (beta * beta) * (0.5 * log(2.0 * ME_GEV * bg * bg * Wmax / (I * I)) - beta * beta - dhalf);
+  /* MeV cm^2/g * g/cm^3 = MeV/cm -> GeV/mm: 1e-3 * 0.1 */
+  const double dE = dedx_mass * opt->mat_rho * 1e-3 * 0.1 * thick * cfac;
+  if (theta0_out) *theta0_out = theta0;
+  if (dE_out) *dE_out = dE;
+  const double E2 = E - dE;
+  if (!(E2 > m)) return KFO_ST_ENERGY;
+  const double p2 = sqrt(E2 * E2 - m * m);
+  const double lam2 = (lam < 0.0 ? -1.0 : 1.0) / p2;
+  const double g = (p * p * p * E2) / (p2 * p2 * p2 * E); /* dlam'/dlam, dE held constant */
+  if (g_out) *g_out = g;
+
+  for (int i = 0; i < 6; ++i) xo[i] = xf[i];
+  xo[4] = lam2;
+  double G[36], GC[36];
+  memset(G, 0, sizeof(G));
+  for (int i = 0; i < 6; ++i) G[i * 6 + i] = 1.0;
+  G[4 * 6 + 4] = g;
+  matmul(6, 6, 6, G, Cf, GC);
+  matmul_bt(6, 6, 6, GC, G, Co);
+  Co[2 * 6 + 2] += theta0 * theta0 / (sth * sth); /* Q_phiphi */
+  Co[3 * 6 + 3] += theta0 * theta0;               /* Q_thetatheta */
+  symmetrise6(Co);
+  return 0;
+}
+
+/* ---- inverse of an SPD 6x6 by Gauss-Jordan on the correlation-scaled matrix (reading U19) --- */
+static int32_t inverse_spd6(const double C[36], double Ci[36]) {
+  double s[6], R[36], Ri[36];
+  for (int i = 0; i < 6; ++i) {
+    if (!(C[i * 6 + i] > 0.0)) return KFO_ST_NOT_POSITIVE;
+    s[i] = sqrt(C[i * 6 + i]);
+  }
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) {
+      R[i * 6 + j] = C[i * 6 + j] / (s[i] * s[j]);
+      Ri[i * 6 + j] = (i == j) ? 1.0 : 0.0;
+    }
+  for (int k = 0; k < 6; ++k) { /* no pivoting: all pivots > 0 iff the matrix is SPD */
+    const double piv = R[k * 6 + k];
+    if (!(piv > 0.0)) return KFO_ST_NOT_POSITIVE;
+    for (int j = 0; j < 6; ++j) {
+      R[k * 6 + j] /= piv;
+      Ri[k * 6 + j] /= piv;
+    }
+    for (int i = 0; i < 6; ++i) {
+      if (i == k) continue;
+      const double fct = R[i * 6 + k];
+      for (int j = 0; j < 6; ++j) {
+        R[i * 6 + j] -= fct * R[k * 6 + j];
+        Ri[i * 6 + j] -= fct * Ri[k * 6 + j];
+      }
+    }
+  }
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) Ci[i * 6 + j] = Ri[i * 6 + j] / (s[i] * s[j]);
+  return 0;
+}
+
+/* ---- C.2.6: one RTS step ("stored Jacobians between states") ------------------- */
+int32_t kfo_rts_step(const double xf[6], const double Cf[36], const double F[36],
+                     const double xp1[6], const double Cp1[36], const double xs1[6],
+                     const double Cs1[36], double xs[6], double Cs[36]) {
+  double Cpi[36], CFt[36], A[36];
+  int32_t rc = inverse_spd6(Cp1, Cpi);
+  if (rc) return rc;
+  matmul_bt(6, 6, 6, Cf, F, CFt); /* C+_k F^T */
+  matmul(6, 6, 6, CFt, Cpi, A);   /* A_k = C+_k F^T (C-_{k+1})^-1 */
+  double dx[6];
+  for (int i = 0; i < 6; ++i) dx[i] = xs1[i] - xp1[i];
+  dx[2] = wrap_pi(dx[2]);
+  for (int i = 0; i < 6; ++i) {
+    double s = 0.0;
+    for (int j = 0; j < 6; ++j) s += A[i * 6 + j] * dx[j];
+    xs[i] = xf[i] + s;
+  }
+  double dC[36], AdC[36], AdCAt[36];
+  for (int i = 0; i < 36; ++i) dC[i] = Cs1[i] - Cp1[i];
+  matmul(6, 6, 6, A, dC, AdC);
+  matmul_bt(6, 6, 6, AdC, A, AdCAt);
+  for (int i = 0; i < 36; ++i) Cs[i] = Cf[i] + AdCAt[i];
+  symmetrise6(Cs);
+  if (!all_finite(xs, 6) || !all_finite(Cs, 36)) return KFO_ST_NOT_POSITIVE;
+  return 0;
+}
+
+/* ---- C.2: the per-track loop ----------------------------------------------------------------- */
+typedef struct {
+  double xp[6], Cp[36], F[36], xf[6], Cf[36];
+} leg_record;
+
+static void fill_nan(double* a, size_t n) {
+  for (size_t i = 0; i < n; ++i) a[i] = NAN;
+}
+
+int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int32_t start,
+                      const int32_t* offsets, const int32_t* surf_idx, const double* loc,
+                      const double* var, const double* cov01, int32_t n_surfaces,
+                      const double* geom, const kfo_field* fld, const kfo_options* opt,
+                      double* first_params, double* first_cov, double* last_params,
+                      double* last_cov, double* chi2_out, int32_t* ndf_out, uint32_t* status_out,
+                      int32_t* n_used_out, int32_t* n_out_out, int32_t* n_holes_out,
+                      double* sp_par, double* sp_cov, double* sf_par, double* sf_cov,
+                      double* ss_par, double* ss_cov, double* hit_chi2, uint8_t* hit_flags,
+                      double* rk_err_max, int32_t n_threads) {
+  if (N < 0 || !params0 || !cov0 || !offsets || !geom || !fld || !opt) return -1;
+  if (start < 0 || start >= n_surfaces) return -1;
+  const int Lmax = n_surfaces - 1 - start;
+  int used_threads = 1;
+#ifdef _OPENMP
+  if (n_threads > 0) omp_set_num_threads(n_threads);
+#pragma omp parallel
+  {
+#pragma omp single
+    used_threads = omp_get_num_threads();
+  }
+#endif
+
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t i = 0; i < N; ++i) {
+    const int32_t o0 = offsets[i], o1 = offsets[i + 1];
+    uint32_t status = 0;
+    double x[6], C[36];
+    for (int a = 0; a < 6; ++a) x[a] = params0[i * 6 + a];
+    for (int a = 0; a < 36; ++a) C[a] = opt->cov_inflation * cov0[i * 36 + a];
+    double first_x[6], first_C[36], last_x[6], last_C[36];
+    memcpy(first_x, x, sizeof(x)); memcpy(first_C, C, sizeof(C));
+    memcpy(last_x, x, sizeof(x));  memcpy(last_C, C, sizeof(C));
+    double chi2 = 0.0, errmax = 0.0;
+    int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0;
+
+    if (sp_par) fill_nan(sp_par + (size_t)i * Lmax * 6, (size_t)Lmax * 6);
+    if (sp_cov) fill_nan(sp_cov + (size_t)i * Lmax * 36, (size_t)Lmax * 36);
+    if (sf_par) fill_nan(sf_par + (size_t)i * Lmax * 6, (size_t)Lmax * 6);
+    if (sf_cov) fill_nan(sf_cov + (size_t)i * Lmax * 36, (size_t)Lmax * 36);
+    if (ss_par) fill_nan(ss_par + (size_t)i * Lmax * 6, (size_t)Lmax * 6);
+    if (ss_cov) fill_nan(ss_cov + (size_t)i * Lmax * 36, (size_t)Lmax * 36);
+    for (int32_t j = o0; j < o1; ++j) {
+      if (hit_chi2) hit_chi2[j] = 0.0;
+      if (hit_flags) hit_flags[j] = KFO_HIT_UNPROCESSED;
+    }
+
+    /* the hit list must be strictly ascending in surface index, inside (start, n_surfaces) */
+    int ok = 1;
+    {
+      int32_t prev_s = start;
+      for (int32_t j = o0; j < o1; ++j) {
+        if (!(surf_idx[j] > prev_s && surf_idx[j] < n_surfaces)) { ok = 0; break; }
+        prev_s = surf_idx[j];
+      }
+    }
+    leg_record* rec = NULL;
+    if (!ok) {
+      status |= KFO_ST_BAD_HITS;
+    } else if (o1 > o0) {
+      const int n_target = surf_idx[o1 - 1] - start; /* reading U7: visit every surface up to the last hit */
+      rec = (leg_record*)malloc(sizeof(leg_record) * (size_t)n_target);
+      double g_prev = 1.0;
+      int32_t hp = o0, prev = start;
+      for (int32_t s = start + 1; s <= start + n_target; ++s) {
+        const double* sf = geom + (size_t)prev * KFO_GEOM_STRIDE;
+        const double* st = geom + (size_t)s * KFO_GEOM_STRIDE;
+        leg_record* R = &rec[nleg];
+        double J[36], e = 0.0;
+        int32_t clamped = 0;
+        int32_t rc = kfo_propagate(fld, opt, x, sf, st, R->xp, J, NULL, &e, &clamped);
+        if (clamped) status |= KFO_ST_FIELD_CLAMPED;
+        if (rc) { status |= (uint32_t)rc; break; }
+        if (e > errmax) errmax = e;
+        /* F = J G_prev (G_prev = diag(1,1,1,1,g,1) of the previous surface's energy loss) */
+        double G[36], JC[36];
+        memset(G, 0, sizeof(G));
+        for (int a = 0; a < 6; ++a) G[a * 6 + a] = 1.0;
+        G[4 * 6 + 4] = g_prev;
+        matmul(6, 6, 6, J, G, R->F);
+        /* C- = J C J^T  (C already holds G C+ G^T + Q of the previous surface) */
+        matmul(6, 6, 6, J, C, JC);
+        matmul_bt(6, 6, 6, JC, J, R->Cp);
+        symmetrise6(R->Cp);
+
+        if (hp < o1 && surf_idx[hp] == s) {
+          double V[4];
+          if (var) {
+            V[0] = var[(size_t)hp * 2 + 0];
+            V[3] = var[(size_t)hp * 2 + 1];
+            V[1] = V[2] = cov01 ? cov01[hp] : 0.0;
+          } else {
+            V[0] = st[16]; V[3] = st[17]; V[1] = V[2] = 0.0;
+          }
+          double c2 = 0.0, xf[6], Cf[36];
+          rc = kfo_update(R->xp, R->Cp, loc + (size_t)hp * 2, V, xf, Cf, &c2);
+          if (rc) { status |= (uint32_t)rc; break; }
+          if (opt->outlier_chi2 > 0.0 && c2 > opt->outlier_chi2) { /* reading U9: strictly greater */
+            memcpy(R->xf, R->xp, sizeof(xf));
+            memcpy(R->Cf, R->Cp, sizeof(Cf));
+            n_outl++;
+            if (hit_flags) hit_flags[hp] = KFO_HIT_OUTLIER;
+          } else {
+            memcpy(R->xf, xf, sizeof(xf));
+            memcpy(R->Cf, Cf, sizeof(Cf));
+            chi2 += c2;
+            n_used++;
+            if (hit_flags) hit_flags[hp] = KFO_HIT_USED;
+          }
+          if (hit_chi2) hit_chi2[hp] = c2;
+          hp++;
+        } else { /* hole */
+          memcpy(R->xf, R->xp, sizeof(R->xf));
+          memcpy(R->Cf, R->Cp, sizeof(R->Cf));
+          n_holes++;
+        }
+        nleg++;
+        memcpy(last_x, R->xf, sizeof(last_x));
+        memcpy(last_C, R->Cf, sizeof(last_C));
+
+        if (opt->material && st[14] > 0.0) { /* reading U6: after the update, at every visited surface */
+          double g = 1.0;
+          rc = kfo_material(opt, st, R->xf, R->Cf, x, C, &g, NULL, NULL);
+          if (rc) { status |= (uint32_t)rc; break; }
+          g_prev = g;
+        } else {
+          memcpy(x, R->xf, sizeof(x));
+          memcpy(C, R->Cf, sizeof(C));
+          g_prev = 1.0;
+        }
+        prev = s;
+      }
+
+      if (nleg > 0) {
+        memcpy(first_x, rec[0].xf, sizeof(first_x));
+        memcpy(first_C, rec[0].Cf, sizeof(first_C));
+      }
+      for (int k = 0; k < nleg; ++k) {
+        size_t o = (size_t)i * Lmax + k;
+        if (sp_par) memcpy(sp_par + o * 6, rec[k].xp, 6 * sizeof(double));
+        if (sp_cov) memcpy(sp_cov + o * 36, rec[k].Cp, 36 * sizeof(double));
+        if (sf_par) memcpy(sf_par + o * 6, rec[k].xf, 6 * sizeof(double));
+        if (sf_cov) memcpy(sf_cov + o * 36, rec[k].Cf, 36 * sizeof(double));
+      }
+
+      /* C.2.6 RTS backward pass over the visited surfaces */
+      if (opt->smooth && nleg > 0) {
+        double xs[6], Cs[36];
+        memcpy(xs, rec[nleg - 1].xf, sizeof(xs));
+        memcpy(Cs, rec[nleg - 1].Cf, sizeof(Cs));
+        size_t o = (size_t)i * Lmax + (nleg - 1);
+        if (ss_par) memcpy(ss_par + o * 6, xs, sizeof(xs));
+        if (ss_cov) memcpy(ss_cov + o * 36, Cs, sizeof(Cs));
+        for (int k = nleg - 2; k >= 0; --k) {
+          double xn[6], Cn[36];
+          int32_t rc = kfo_rts_step(rec[k].xf, rec[k].Cf, rec[k + 1].F, rec[k + 1].xp,
+                                    rec[k + 1].Cp, xs, Cs, xn, Cn);
+          if (rc) { /* fall back to the filtered states for the remaining surfaces */
+            status |= (uint32_t)rc;
+            for (int kk = k; kk >= 0; --kk) {
+              size_t oo = (size_t)i * Lmax + kk;
+              if (ss_par) memcpy(ss_par + oo * 6, rec[kk].xf, 6 * sizeof(double));
+              if (ss_cov) memcpy(ss_cov + oo * 36, rec[kk].Cf, 36 * sizeof(double));
+            }
+            memcpy(xs, rec[0].xf, sizeof(xs));
+            memcpy(Cs, rec[0].Cf, sizeof(Cs));
+            break;
+          }
+          memcpy(xs, xn, sizeof(xs));
+          memcpy(Cs, Cn, sizeof(Cs));
+          o = (size_t)i * Lmax + k;
+          if (ss_par) memcpy(ss_par + o * 6, xs, sizeof(xs));
+          if (ss_cov) memcpy(ss_cov + o * 36, Cs, sizeof(Cs));
+        }
+        memcpy(first_x, xs, sizeof(first_x));
+        memcpy(first_C, Cs, sizeof(first_C));
+      }
+    }
+    free(rec);
+
+    const int ndf = 2 * n_used - 5; /* time is never measured: 5, not 6 (reading U10) */
+    if (ndf <= 0) status |= KFO_ST_NDF;
+    if (first_params) memcpy(first_params + i * 6, first_x, sizeof(first_x));
+    if (first_cov) memcpy(first_cov + i * 36, first_C, sizeof(first_C));
+    if (last_params) memcpy(last_params + i * 6, last_x, sizeof(last_x));
+    if (last_cov) memcpy(last_cov + i * 36, last_C, sizeof(last_C));
+    if (chi2_out) chi2_out[i] = chi2;
+    if (ndf_out) ndf_out[i] = ndf;
+    if (status_out) status_out[i] = status;
+    if (n_used_out) n_used_out[i] = n_used;
+    if (n_out_out) n_out_out[i] = n_outl;
+    if (n_holes_out) n_holes_out[i] = n_holes;
+    if (rk_err_max) rk_err_max[i] = errmax;
+  }
+  return used_threads;
+}
