@@ -1,0 +1,205 @@
+/*
+ * kf_fit.h -- C ABI of libkf_fit.so: batched per-track Kalman-filter track fit on one B200.
+ *
+ * What it computes (arxiv 2105.01796, "A GPU-based Kalman Filter for Track Fitting"):
+ *   for every track independently the Kalman step loop of PAPER.md:55-60 --
+ *   propagate the bound parameters (loc0, loc1, phi, theta, q/p, t) and their 6x6
+ *   covariance to the next measurement surface with a 4th-order Runge-Kutta-Nystrom stepper,
+ *   transporting the 8x8 free Jacobian alongside and applying the local<->global Jacobians at both
+ *   ends; combine the prediction with the surface's 2-D measurement in the
+ *   gain-matrix formalism; add the material effects of the surface;
+ *   then, optionally, the Rauch-Tung-Striebel smoother "with the stored Jacobians between states"
+ *   (PAPER.md:62, 75).  The four track-specific data sets of PAPER.md:174-180 (measurements,
+ *   starting parameters, fit configuration, results) are the four argument groups below; the
+ *   "global data shared by different tracks" (geometry, field) are kf_geometry / kf_field.
+ *   The exact arithmetic (the paper prints none) is stated in DESIGN.md "The algorithm".
+ *
+ * All of it runs in hand-written sm_100a CUDA kernels in IEEE double precision.  There is no CPU
+ * fallback: without a CUDA device every compute entry point returns KF_ERR_CUDA.
+ *
+ * Conventions
+ *   units      mm, GeV, e.  q/p in 1/GeV.  t is c*t in mm (1 ns = 299.792458 mm).  Field in tesla.
+ *   bound      x = (loc0, loc1, phi, theta, q/p, t) on a plane with centre c and orthonormal
+ *              u, v, n = u x v:  r = c + loc0 u + loc1 v,  T = (cos phi sin theta, sin phi sin theta, cos theta).
+ *   SoA        per-track arrays are component-major: element (component k, track i) of a
+ *              double[K][N] array lives at [k * N + i].
+ *   cov        6x6 symmetric, packed upper triangle row-major, 21 values:
+ *              (00 01 02 03 04 05 11 12 13 14 15 22 23 24 25 33 34 35 44 45 55).
+ *   pointers   every array pointer is a DEVICE pointer (8-byte aligned) unless the field says HOST;
+ *              the descriptor structs themselves are small HOST structs read during the call.
+ *
+ * Ownership and ordering
+ *   The caller owns every buffer including the workspace.  The library allocates nothing, keeps
+ *   no state between calls, never frees and never synchronises: kf_fit_batch validates the
+ *   descriptors on the host, enqueues its kernels on `cuda_stream` (a cudaStream_t; NULL = the
+ *   legacy default stream) and returns.  Inputs are read-only.  Buffers must stay valid until the
+ *   stream has run past the call.  Outputs of a rejected call (< 0) are untouched.
+ */
+#ifndef KF_FIT_H
+#define KF_FIT_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define KF_VERSION 100          /* major * 100 + minor */
+#define KF_GEOM_STRIDE 20       /* doubles per surface record */
+#define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
+
+/* return codes */
+enum {
+  KF_OK = 0,
+  KF_ERR_ARG = -1,        /* null / ill-formed descriptor */
+  KF_ERR_UNSUPPORTED = -2,/* unsupported option combination */
+  KF_ERR_WORKSPACE = -3,  /* workspace too small (see kf_workspace_bytes) */
+  KF_ERR_CUDA = -4        /* CUDA error at launch (text: kf_last_cuda_error) */
+};
+
+/* per-track status bits (never fail the call) */
+enum {
+  KF_ST_PROPAGATION = 1,   /* n.T <= 1e-6 or a non-finite state: next surface not reachable. Track stops. */
+  KF_ST_NOT_POSITIVE = 2,  /* S = H C H^T + V not positive definite (track stops), or a non-positive
+                              Cholesky pivot in the smoother (smoothed output falls back to filtered) */
+  KF_ST_ENERGY = 4,        /* E' <= m after the energy loss in a layer. Track stops after that layer. */
+  KF_ST_NDF = 8,           /* ndf = 2 n_used - 5 <= 0 */
+  KF_ST_THETA = 16,        /* sin(theta) <= 1e-12 on arrival: (phi, theta) chart singular. Track stops. */
+  KF_ST_FIELD_CLAMPED = 32,/* a field lookup fell outside the grid; the clamped value was used */
+  KF_ST_BAD_HITS = 64      /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces):
+                              track not fitted, outputs hold the start state */
+};
+
+/* per-hit flags */
+enum { KF_HIT_UNPROCESSED = 0, KF_HIT_USED = 1, KF_HIT_OUTLIER = 2 };
+
+/* field kinds */
+enum { KF_FIELD_CONST = 0, KF_FIELD_GRID3 = 1 };
+
+/* kernel variants (kf_options.variant) */
+enum { KF_VARIANT_AUTO = 0, KF_VARIANT_THREAD_PER_TRACK = 1, KF_VARIANT_LANES_PER_TRACK = 2 };
+
+/* kf_options.output_states bitmask: which per-leg states to write to kf_outputs.state_* */
+enum { KF_STATES_PRED = 1, KF_STATES_FILT = 2, KF_STATES_SMOOTH = 4 };
+
+/* (2) starting parameters -- PAPER.md:177 */
+typedef struct kf_tracks_in {
+  int64_t n_tracks;       /* N >= 0 */
+  const double* params;   /* double[6][N]  start parameters on the start surface */
+  const double* cov;      /* double[21][N] start covariance, packed upper triangle */
+  int32_t start_surface;  /* index into the geometry; one value for the batch */
+} kf_tracks_in;
+
+/* (1) input measurements -- PAPER.md:176; the geometry identifier that links a hit to its
+ * surface is surf_idx.  CSR over tracks. */
+typedef struct kf_measurements {
+  int64_t n_meas;          /* M = offsets[N] */
+  const int32_t* offsets;  /* int32[N+1], offsets[0] = 0, non-decreasing */
+  const int32_t* surf_idx; /* int32[M], strictly ascending within a track, in (start_surface, n_surfaces) */
+  const double* loc;       /* double[2][M] measured local position (loc0 row, then loc1 row) */
+  const double* var;       /* double[2][M] per-hit variances, or NULL: use the surface's meas_var */
+  const double* cov01;     /* double[M] per-hit covariance (needs var), or NULL: 0 */
+} kf_measurements;
+
+/* global data: detector geometry -- PAPER.md:168, 174, 182 (boundless planes).
+ * Surface record, KF_GEOM_STRIDE doubles:
+ *   [0..2] centre  [3..5] u  [6..8] v  [9..11] n = u x v (orthonormal)  [12..13] half lengths (informational)
+ *   [14] x/X0  [15] thickness in mm  [16..17] measurement variances (loc0, loc1)  [18..19] unused
+ * Navigation order = ascending surface index: a track visits start_surface+1, +2, ... up to the
+ * surface of its last hit. */
+typedef struct kf_geometry {
+  int32_t n_surfaces;
+  const double* surfaces;  /* double[n_surfaces][KF_GEOM_STRIDE] */
+  double mat_Z, mat_A;     /* one material for the batch: atomic number, mass (g/mol) */
+  double mat_rho;          /* density g/cm^3 */
+  double mat_I_eV;         /* mean excitation energy */
+} kf_geometry;
+
+/* global data: magnetic field -- PAPER.md:170 (constant 3x1 vector; inhomogeneous fields need
+ * "position-specific field information ... stored and retrieved") */
+typedef struct kf_field {
+  int32_t kind;        /* KF_FIELD_CONST | KF_FIELD_GRID3 */
+  double b[3];         /* CONST: tesla (HOST values) */
+  int32_t n[3];        /* GRID3: nodes along x, y, z (each >= 2) */
+  double origin[3];    /* GRID3: position of node (0,0,0), mm */
+  double spacing[3];   /* GRID3: mm, > 0 */
+  const double* grid;  /* GRID3: double[nz][ny][nx][3] tesla, x fastest, component innermost.
+                          Trilinear interpolation; outside the grid the clamped value is used. */
+} kf_field;
+
+/* (3) fit configuration -- PAPER.md:179 */
+typedef struct kf_options {
+  int32_t smooth;         /* 1: run the RTS backward pass */
+  int32_t material;       /* 1: Highland scattering noise + Bethe mean energy loss at surfaces with x/X0 > 0 */
+  double outlier_chi2;    /* <= 0: off.  Else a hit whose predicted chi2 (2 dof) is > this is flagged, not used */
+  int32_t n_corr_steps;   /* RKN correction steps after the primary ones, 0..8 (default 2) */
+  double max_step_mm;     /* cap on a primary step; +inf (or <= 0): one primary step per leg */
+  double mass_gev;        /* particle mass (> 0) */
+  double cov_inflation;   /* multiplies the start covariance (default 1) */
+  int32_t output_states;  /* KF_STATES_* bitmask */
+  int32_t variant;        /* KF_VARIANT_* */
+} kf_options;
+
+/* (4) results -- PAPER.md:180: status, track states, fitted parameters */
+typedef struct kf_outputs {
+  double* first_params;   /* double[6][N]  smoothed (or filtered if !smooth) state at the first visited surface */
+  double* first_cov;      /* double[21][N] */
+  double* last_params;    /* double[6][N]  filtered state at the last visited surface */
+  double* last_cov;       /* double[21][N] */
+  double* chi2;           /* double[N]     sum of predicted-residual chi2 over used hits */
+  int32_t* ndf;           /* int32[N]      2 n_used - 5 */
+  uint32_t* status;       /* uint32[N]     KF_ST_* bits */
+  int32_t* n_used;        /* int32[N] */
+  int32_t* n_outliers;    /* int32[N] */
+  int32_t* n_holes;       /* int32[N]      visited surfaces without a hit */
+  /* optional (NULL = skip).  Per-leg arrays are dense over (leg, track) with
+   * Lmax = n_surfaces - 1 - start_surface legs: element (leg l, component k, track i) at
+   * [(l * K + k) * N + i].  Legs a track did not visit are left untouched. */
+  double* state_params[3];/* double[Lmax][6][N]  for PRED, FILT, SMOOTH (index = log2 of the bit) */
+  double* state_cov[3];   /* double[Lmax][21][N] */
+  double* hit_chi2;       /* double[M]  predicted chi2 of every processed hit (0 if unprocessed) */
+  uint8_t* hit_flags;     /* uint8[M]   KF_HIT_* */
+  double* rk_err_max;     /* double[N]  largest embedded RKN error estimate h^2 |k1-k2-k3+k4|_1, mm */
+} kf_outputs;
+
+/* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
+ * muon mass, inflation 1, no per-leg states, variant AUTO. */
+void kf_default_options(kf_options* opt);
+
+/* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =
+ * n_surfaces - 1 - start_surface legs per track (RTS records; 0 extra when !smooth). */
+size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt);
+
+/* Enqueue the fit of one batch on `cuda_stream`.  Returns KF_OK or a negative KF_ERR_*. */
+int kf_fit_batch(const kf_tracks_in* tracks, const kf_measurements* meas, const kf_geometry* geom,
+                 const kf_field* field, const kf_options* opt, const kf_outputs* out,
+                 void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* End-to-end variant for HOST buffers (the paper's offload runtime):
+ * every array pointer in tracks/meas/geom/field/out is a HOST pointer (pinned memory for
+ * asynchronous copies).  The call copies the inputs into `device_arena` (caller-owned device
+ * memory of at least kf_host_arena_bytes), runs kf_fit_batch there and copies the requested
+ * outputs back, all enqueued on `cuda_stream`; it does not synchronise. */
+size_t kf_host_arena_bytes(int64_t n_tracks, int64_t n_meas, int32_t n_surfaces, int32_t start_surface,
+                           const kf_field* field, const kf_options* opt, int has_var, int has_cov01);
+int kf_fit_batch_host(const kf_tracks_in* tracks, const kf_measurements* meas, const kf_geometry* geom,
+                      const kf_field* field, const kf_options* opt, const kf_outputs* out,
+                      void* device_arena, size_t arena_bytes, void* cuda_stream);
+
+/* Number of kernels the last kf_fit_batch call of this thread enqueued (for launch accounting). */
+int kf_last_launch_count(void);
+
+/* Sustained FP64 FMA throughput probe (roofline denominator): runs a dependent-chain DFMA kernel
+ * `iters` long on every SM, on `cuda_stream`, synchronises, and returns TFLOP/s (2 flop per FMA),
+ * or a negative KF_ERR_*.  Not part of the fit. */
+double kf_probe_fp64_tflops(int iters, void* cuda_stream);
+
+const char* kf_status_string(int rc);
+const char* kf_last_cuda_error(void);
+int kf_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif

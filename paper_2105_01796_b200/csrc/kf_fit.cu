@@ -1,0 +1,396 @@
+// kf_fit.cu -- host side of libkf_fit.so: the C ABI declared in include/kf_fit.h.
+//
+// Validates the descriptors, lays out the workspace, and enqueues the sm_100a kernels of
+// kf_kernels.cuh on the caller's stream.  No allocation, no synchronisation, no global state
+// (apart from thread-local error text / launch counter).  There is no CPU fallback: every compute
+// entry point ends in a kernel launch and reports KF_ERR_CUDA if that fails.
+#include <cuda_runtime.h>
+
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+
+#include "kf_fit.h"
+#include "kf_kernels.cuh"
+
+namespace {
+
+thread_local char g_cuda_error[256] = "";
+thread_local int g_launches = 0;
+
+inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+struct WorkspaceLayout {
+  size_t rec_off, flag_off, nleg_off, total;
+  long long Np;
+};
+
+WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth) {
+  WorkspaceLayout w{};
+  w.Np = (long long)align_up((size_t)(N > 0 ? N : 0), 32);
+  if (!smooth || N <= 0 || n_legs_max <= 0) return w;
+  size_t off = 0;
+  w.rec_off = off;
+  off += align_up((size_t)n_legs_max * kf::kRecDoubles * (size_t)w.Np * sizeof(double), 256);
+  w.flag_off = off;
+  off += align_up((size_t)n_legs_max * (size_t)w.Np, 256);
+  w.nleg_off = off;
+  off += align_up((size_t)w.Np * sizeof(int), 256);
+  w.total = off;
+  return w;
+}
+
+bool set_cuda_error(cudaError_t e, const char* where) {
+  if (e == cudaSuccess) return false;
+  snprintf(g_cuda_error, sizeof(g_cuda_error), "%s: %s", where, cudaGetErrorString(e));
+  return true;
+}
+
+template <typename K>
+int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_t stream, const char* name) {
+  if (smem > 48 * 1024) {
+    if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name))
+      return KF_ERR_CUDA;
+  }
+  const unsigned grid = (unsigned)((P.N + block - 1) / block);
+  kernel<<<grid, block, smem, stream>>>(P);
+  if (set_cuda_error(cudaGetLastError(), name)) return KF_ERR_CUDA;
+  g_launches++;
+  return KF_OK;
+}
+
+int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
+             const kf_options* op, const kf_outputs* out) {
+  if (!tr || !ms || !ge || !fl || !op || !out) return KF_ERR_ARG;
+  if (tr->n_tracks < 0 || ms->n_meas < 0 || ms->n_meas > 2147483647LL) return KF_ERR_ARG;
+  if (ge->n_surfaces < 1 || !ge->surfaces) return KF_ERR_ARG;
+  if (tr->start_surface < 0 || tr->start_surface >= ge->n_surfaces) return KF_ERR_ARG;
+  if (tr->n_tracks > 0) {
+    if (!tr->params || !tr->cov || !ms->offsets) return KF_ERR_ARG;
+    if (ms->n_meas > 0 && (!ms->surf_idx || !ms->loc)) return KF_ERR_ARG;
+    if (ms->cov01 && !ms->var) return KF_ERR_ARG;
+    if (!out->first_params || !out->first_cov || !out->last_params || !out->last_cov || !out->chi2 ||
+        !out->ndf || !out->status || !out->n_used || !out->n_outliers || !out->n_holes)
+      return KF_ERR_ARG;
+  }
+  if (fl->kind == KF_FIELD_GRID3) {
+    if (!fl->grid) return KF_ERR_ARG;
+    for (int a = 0; a < 3; ++a)
+      if (fl->n[a] < 2 || !(fl->spacing[a] > 0.0)) return KF_ERR_ARG;
+  } else if (fl->kind != KF_FIELD_CONST) {
+    return KF_ERR_ARG;
+  }
+  if (op->n_corr_steps < 0 || op->n_corr_steps > 8) return KF_ERR_ARG;
+  if (!(op->mass_gev > 0.0) || !(op->cov_inflation > 0.0)) return KF_ERR_ARG;
+  if (op->output_states & ~7) return KF_ERR_ARG;
+  if (op->material && !(ge->mat_A > 0.0 && ge->mat_Z > 0.0 && ge->mat_rho > 0.0 && ge->mat_I_eV > 0.0))
+    return KF_ERR_ARG;
+  for (int b = 0; b < 3; ++b)
+    if ((op->output_states >> b) & 1)
+      if (tr->n_tracks > 0 && (!out->state_params[b] || !out->state_cov[b])) return KF_ERR_ARG;
+  if ((op->output_states & KF_STATES_SMOOTH) && !op->smooth) return KF_ERR_UNSUPPORTED;
+  if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK) return KF_ERR_UNSUPPORTED;
+  return KF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+void kf_default_options(kf_options* opt) {
+  if (!opt) return;
+  memset(opt, 0, sizeof(*opt));
+  opt->smooth = 1;
+  opt->material = 0;
+  opt->outlier_chi2 = 0.0;
+  opt->n_corr_steps = 2;
+  opt->max_step_mm = INFINITY;
+  opt->mass_gev = 0.1056583755;
+  opt->cov_inflation = 1.0;
+  opt->output_states = 0;
+  opt->variant = KF_VARIANT_AUTO;
+}
+
+size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt) {
+  const int smooth = opt ? opt->smooth : 1;
+  return workspace_layout(n_tracks, n_legs_max, smooth).total;
+}
+
+int kf_last_launch_count(void) { return g_launches; }
+const char* kf_last_cuda_error(void) { return g_cuda_error; }
+int kf_version(void) { return KF_VERSION; }
+
+const char* kf_status_string(int rc) {
+  switch (rc) {
+    case KF_OK: return "ok";
+    case KF_ERR_ARG: return "null or ill-formed descriptor";
+    case KF_ERR_UNSUPPORTED: return "unsupported option combination";
+    case KF_ERR_WORKSPACE: return "workspace too small";
+    case KF_ERR_CUDA: return "CUDA error (see kf_last_cuda_error)";
+    default: return "unknown return code";
+  }
+}
+
+int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
+                 const kf_field* fl, const kf_options* op, const kf_outputs* out, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+  g_launches = 0;
+  int rc = validate(tr, ms, ge, fl, op, out);
+  if (rc != KF_OK) return rc;
+  const long long N = tr->n_tracks;
+  if (N == 0) return KF_OK;
+  const int Lmax = ge->n_surfaces - 1 - tr->start_surface;
+  const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth);
+  if (w.total > 0 && (!workspace || workspace_bytes < w.total)) return KF_ERR_WORKSPACE;
+
+  kf::FitParams P{};
+  P.N = N; P.Np = w.Np; P.M = ms->n_meas;
+  P.params = tr->params; P.cov = tr->cov; P.start = tr->start_surface;
+  P.offsets = ms->offsets; P.surf_idx = ms->surf_idx; P.loc = ms->loc; P.var = ms->var; P.cov01 = ms->cov01;
+  P.n_surfaces = ge->n_surfaces; P.geom = ge->surfaces;
+  P.geom_in_smem = ge->n_surfaces <= 1024 ? 1 : 0;
+  if (fl->kind == KF_FIELD_CONST) {
+    for (int a = 0; a < 3; ++a) P.field.b[a] = fl->b[a] * 2.99792458e-4;  // tesla -> GeV/(e mm)
+  } else {
+    for (int a = 0; a < 3; ++a) {
+      P.field.n[a] = fl->n[a];
+      P.field.origin[a] = fl->origin[a];
+      P.field.spacing[a] = fl->spacing[a];
+    }
+    P.field.grid = fl->grid;
+  }
+  P.mat.mass = op->mass_gev;
+  if (op->material) {
+    P.mat.ZA = ge->mat_Z / ge->mat_A;
+    P.mat.rho = ge->mat_rho;
+    P.mat.I_gev = ge->mat_I_eV * 1e-9;
+    P.mat.log_hwp_I = log(28.816e-9 * sqrt(ge->mat_rho * P.mat.ZA) / P.mat.I_gev);
+  }
+  P.smooth = op->smooth ? 1 : 0;
+  P.n_corr = op->n_corr_steps;
+  P.output_states = op->output_states;
+  P.outlier_chi2 = op->outlier_chi2;
+  P.max_step = (op->max_step_mm > 0.0 && std::isfinite(op->max_step_mm)) ? op->max_step_mm : 0.0;
+  P.inflation = op->cov_inflation;
+  P.first_params = out->first_params; P.first_cov = out->first_cov;
+  P.last_params = out->last_params; P.last_cov = out->last_cov;
+  P.chi2 = out->chi2; P.ndf = out->ndf; P.status = out->status;
+  P.n_used = out->n_used; P.n_outliers = out->n_outliers; P.n_holes = out->n_holes;
+  for (int b = 0; b < 3; ++b) { P.state_params[b] = out->state_params[b]; P.state_cov[b] = out->state_cov[b]; }
+  P.hit_chi2 = out->hit_chi2; P.hit_flags = out->hit_flags; P.rk_err_max = out->rk_err_max;
+  if (w.total > 0) {
+    char* base = static_cast<char*>(workspace);
+    P.rec = reinterpret_cast<double*>(base + w.rec_off);
+    P.legflag = reinterpret_cast<unsigned char*>(base + w.flag_off);
+    P.nleg = reinterpret_cast<int*>(base + w.nleg_off);
+  } else {
+    P.smooth = 0;  // no legs to smooth (Lmax == 0)
+  }
+
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
+  const size_t fwd_smem = geom_smem + (size_t)KF_FWD_BLOCK * 9 * sizeof(double);
+  const bool grid3 = fl->kind == KF_FIELD_GRID3;
+  if (op->material) {
+    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel")
+               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
+  } else {
+    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, false>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel")
+               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, false>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
+  }
+  if (rc != KF_OK) return rc;
+  if (P.smooth) rc = launch(kf::kf_rts_kernel, P, KF_RTS_BLOCK, geom_smem, stream, "kf_rts_kernel");
+  return rc;
+}
+
+double kf_probe_fp64_tflops(int iters, void* cuda_stream) {
+  if (iters <= 0) return (double)KF_ERR_ARG;
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  int dev = 0, sms = 0;
+  if (set_cuda_error(cudaGetDevice(&dev), "cudaGetDevice")) return (double)KF_ERR_CUDA;
+  if (set_cuda_error(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
+    return (double)KF_ERR_CUDA;
+  const int block = 256, grid = sms * 8;
+  cudaEvent_t e0, e1;
+  if (set_cuda_error(cudaEventCreate(&e0), "cudaEventCreate")) return (double)KF_ERR_CUDA;
+  if (set_cuda_error(cudaEventCreate(&e1), "cudaEventCreate")) { cudaEventDestroy(e0); return (double)KF_ERR_CUDA; }
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {  // first repetition is the warm-up
+    cudaEventRecord(e0, stream);
+    kf::kf_dfma_probe_kernel<<<grid, block, 0, stream>>>(nullptr, iters, 1.0000001, 1e-9);
+    cudaEventRecord(e1, stream);
+    if (set_cuda_error(cudaEventSynchronize(e1), "kf_dfma_probe_kernel")) { best = (double)KF_ERR_CUDA; break; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double flops = 2.0 * 8.0 * (double)iters * (double)block * (double)grid;
+    const double tf = flops / ((double)ms * 1e-3) * 1e-12;
+    if (rep > 0 && tf > best) best = tf;
+  }
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  return best;
+}
+
+
+// ---- end-to-end variant for HOST buffers (pinned per-track blocks, H2D copy,
+// kernel, D2H copy) ------------------------------------------------------------------------
+namespace {
+struct Bump {
+  size_t off = 0;
+  size_t take(size_t bytes) {
+    const size_t o = off;
+    off += align_up(bytes, 256);
+    return o;
+  }
+};
+struct ArenaLayout {
+  size_t params, cov, offsets, surf_idx, loc, var, cov01, geom, grid;
+  size_t first_params, first_cov, last_params, last_cov, chi2, ndf, status, n_used, n_outliers, n_holes;
+  size_t state_params[3], state_cov[3], hit_chi2, hit_flags, rk_err, workspace, workspace_bytes, total;
+};
+ArenaLayout arena_layout(long long N, long long M, int nS, int start, const kf_field* fl, const kf_options* op,
+                         int has_var, int has_cov01) {
+  ArenaLayout a{};
+  Bump b;
+  const size_t D = sizeof(double), I = sizeof(int32_t);
+  const int Lmax = nS - 1 - start;
+  a.params = b.take(6 * N * D);
+  a.cov = b.take(21 * N * D);
+  a.offsets = b.take((N + 1) * I);
+  a.surf_idx = b.take(M * I);
+  a.loc = b.take(2 * M * D);
+  a.var = has_var ? b.take(2 * M * D) : 0;
+  a.cov01 = has_cov01 ? b.take(M * D) : 0;
+  a.geom = b.take((size_t)nS * KF_GEOM_STRIDE * D);
+  a.grid = 0;
+  if (fl && fl->kind == KF_FIELD_GRID3) a.grid = b.take((size_t)fl->n[0] * fl->n[1] * fl->n[2] * 3 * D);
+  a.first_params = b.take(6 * N * D);
+  a.first_cov = b.take(21 * N * D);
+  a.last_params = b.take(6 * N * D);
+  a.last_cov = b.take(21 * N * D);
+  a.chi2 = b.take(N * D);
+  a.ndf = b.take(N * I);
+  a.status = b.take(N * I);
+  a.n_used = b.take(N * I);
+  a.n_outliers = b.take(N * I);
+  a.n_holes = b.take(N * I);
+  for (int k = 0; k < 3; ++k) {
+    const bool on = op && ((op->output_states >> k) & 1);
+    a.state_params[k] = on ? b.take((size_t)Lmax * 6 * N * D) : 0;
+    a.state_cov[k] = on ? b.take((size_t)Lmax * 21 * N * D) : 0;
+  }
+  a.hit_chi2 = b.take(M * D);
+  a.hit_flags = b.take(M);
+  a.rk_err = b.take(N * D);
+  a.workspace_bytes = workspace_layout(N, Lmax, op ? op->smooth : 1).total;
+  a.workspace = b.take(a.workspace_bytes);
+  a.total = b.off;
+  return a;
+}
+}  // namespace
+
+size_t kf_host_arena_bytes(int64_t n_tracks, int64_t n_meas, int32_t n_surfaces, int32_t start_surface,
+                           const kf_field* field, const kf_options* opt, int has_var, int has_cov01) {
+  if (n_tracks < 0 || n_meas < 0 || n_surfaces < 1 || start_surface < 0 || start_surface >= n_surfaces) return 0;
+  return arena_layout(n_tracks, n_meas, n_surfaces, start_surface, field, opt, has_var, has_cov01).total;
+}
+
+int kf_fit_batch_host(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
+                      const kf_field* fl, const kf_options* op, const kf_outputs* out, void* device_arena,
+                      size_t arena_bytes, void* cuda_stream) {
+  g_launches = 0;
+  int rc = validate(tr, ms, ge, fl, op, out);
+  if (rc != KF_OK) return rc;
+  const long long N = tr->n_tracks, M = ms->n_meas;
+  if (N == 0) return KF_OK;
+  const int nS = ge->n_surfaces;
+  const ArenaLayout a = arena_layout(N, M, nS, tr->start_surface, fl, op, ms->var != nullptr, ms->cov01 != nullptr);
+  if (!device_arena || arena_bytes < a.total) return KF_ERR_WORKSPACE;
+  char* base = static_cast<char*>(device_arena);
+  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+  const size_t D = sizeof(double), I = sizeof(int32_t);
+  const int Lmax = nS - 1 - tr->start_surface;
+
+#define KF_H2D(dst_off, src, bytes)                                                                   \
+  do {                                                                                                \
+    if ((bytes) > 0 && set_cuda_error(cudaMemcpyAsync(base + (dst_off), (src), (bytes),               \
+                                                      cudaMemcpyHostToDevice, stream), "H2D copy"))   \
+      return KF_ERR_CUDA;                                                                             \
+  } while (0)
+#define KF_D2H(dst, src_off, bytes)                                                                   \
+  do {                                                                                                \
+    if ((dst) && (bytes) > 0 && set_cuda_error(cudaMemcpyAsync((dst), base + (src_off), (bytes),      \
+                                                      cudaMemcpyDeviceToHost, stream), "D2H copy"))   \
+      return KF_ERR_CUDA;                                                                             \
+  } while (0)
+
+  KF_H2D(a.params, tr->params, 6 * N * D);
+  KF_H2D(a.cov, tr->cov, 21 * N * D);
+  KF_H2D(a.offsets, ms->offsets, (N + 1) * I);
+  KF_H2D(a.surf_idx, ms->surf_idx, M * I);
+  KF_H2D(a.loc, ms->loc, 2 * M * D);
+  if (ms->var) KF_H2D(a.var, ms->var, 2 * M * D);
+  if (ms->cov01) KF_H2D(a.cov01, ms->cov01, M * D);
+  KF_H2D(a.geom, ge->surfaces, (size_t)nS * KF_GEOM_STRIDE * D);
+  if (fl->kind == KF_FIELD_GRID3) KF_H2D(a.grid, fl->grid, (size_t)fl->n[0] * fl->n[1] * fl->n[2] * 3 * D);
+
+  kf_tracks_in dtr = *tr;
+  dtr.params = reinterpret_cast<const double*>(base + a.params);
+  dtr.cov = reinterpret_cast<const double*>(base + a.cov);
+  kf_measurements dms = *ms;
+  dms.offsets = reinterpret_cast<const int32_t*>(base + a.offsets);
+  dms.surf_idx = reinterpret_cast<const int32_t*>(base + a.surf_idx);
+  dms.loc = reinterpret_cast<const double*>(base + a.loc);
+  dms.var = ms->var ? reinterpret_cast<const double*>(base + a.var) : nullptr;
+  dms.cov01 = ms->cov01 ? reinterpret_cast<const double*>(base + a.cov01) : nullptr;
+  kf_geometry dge = *ge;
+  dge.surfaces = reinterpret_cast<const double*>(base + a.geom);
+  kf_field dfl = *fl;
+  if (fl->kind == KF_FIELD_GRID3) dfl.grid = reinterpret_cast<const double*>(base + a.grid);
+  kf_outputs dout{};
+  dout.first_params = reinterpret_cast<double*>(base + a.first_params);
+  dout.first_cov = reinterpret_cast<double*>(base + a.first_cov);
+  dout.last_params = reinterpret_cast<double*>(base + a.last_params);
+  dout.last_cov = reinterpret_cast<double*>(base + a.last_cov);
+  dout.chi2 = reinterpret_cast<double*>(base + a.chi2);
+  dout.ndf = reinterpret_cast<int32_t*>(base + a.ndf);
+  dout.status = reinterpret_cast<uint32_t*>(base + a.status);
+  dout.n_used = reinterpret_cast<int32_t*>(base + a.n_used);
+  dout.n_outliers = reinterpret_cast<int32_t*>(base + a.n_outliers);
+  dout.n_holes = reinterpret_cast<int32_t*>(base + a.n_holes);
+  for (int k = 0; k < 3; ++k)
+    if ((op->output_states >> k) & 1) {
+      dout.state_params[k] = reinterpret_cast<double*>(base + a.state_params[k]);
+      dout.state_cov[k] = reinterpret_cast<double*>(base + a.state_cov[k]);
+    }
+  if (out->hit_chi2) dout.hit_chi2 = reinterpret_cast<double*>(base + a.hit_chi2);
+  if (out->hit_flags) dout.hit_flags = reinterpret_cast<uint8_t*>(base + a.hit_flags);
+  if (out->rk_err_max) dout.rk_err_max = reinterpret_cast<double*>(base + a.rk_err);
+
+  rc = kf_fit_batch(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, cuda_stream);
+  if (rc != KF_OK) return rc;
+
+  KF_D2H(out->first_params, a.first_params, 6 * N * D);
+  KF_D2H(out->first_cov, a.first_cov, 21 * N * D);
+  KF_D2H(out->last_params, a.last_params, 6 * N * D);
+  KF_D2H(out->last_cov, a.last_cov, 21 * N * D);
+  KF_D2H(out->chi2, a.chi2, N * D);
+  KF_D2H(out->ndf, a.ndf, N * I);
+  KF_D2H(out->status, a.status, N * I);
+  KF_D2H(out->n_used, a.n_used, N * I);
+  KF_D2H(out->n_outliers, a.n_outliers, N * I);
+  KF_D2H(out->n_holes, a.n_holes, N * I);
+  for (int k = 0; k < 3; ++k)
+    if ((op->output_states >> k) & 1) {
+      KF_D2H(out->state_params[k], a.state_params[k], (size_t)Lmax * 6 * N * D);
+      KF_D2H(out->state_cov[k], a.state_cov[k], (size_t)Lmax * 21 * N * D);
+    }
+  KF_D2H(out->hit_chi2, a.hit_chi2, M * D);
+  KF_D2H(out->hit_flags, a.hit_flags, (size_t)M);
+  KF_D2H(out->rk_err_max, a.rk_err, N * D);
+#undef KF_H2D
+#undef KF_D2H
+  return KF_OK;
+}
+
+}  // extern "C"
