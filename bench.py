@@ -1,0 +1,329 @@
+#!/usr/bin/env python
+"""bench.py -- fitted tracks/s of the batched Kalman track fit on B200 (BASELINE.json metric).
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--config C] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (forward filter + RTS smoother = one kf_fit_batch
+call) over one batch of synthetic tracks.  Default workload: BASELINE.json configs[2]
+(1,000,000 tracks x 30 layers with material, filter + smoother, seed 3) -- the configuration the
+north_star target is quoted on.  Inputs are resident in HBM for `value`; `e2e` goes through
+kf_fit_batch_host with pinned HOST buffers (H2D + fit + D2H inside the timed region).
+
+The path does not shard (north_star: one GPU, no collectives): with --gpus N > 1 (under torchrun)
+every rank fits its own replica of the batch ("replicas only"); value is
+the tracks all ranks fitted / max-over-ranks time.
+
+--impl reference times the CPU oracle (oracle/, as it stands) on the box's host cores on a
+bounded sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "fitted tracks/sec (device-timed, FP64)"
+UNIT = "tracks/s"
+
+# Algorithmic work per leg (one surface visited by one track), DESIGN.md "Rooflines":
+#   bytes: RTS record 53 doubles + 1 flag byte written by the forward kernel and read by the RTS
+#          kernel, the hit (2 doubles + int32) read by both; per track 27 doubles in, outputs out.
+#   flops: FP64 flop per leg counted from ncu instruction counters (DFMA = 2), see profiles/.
+REC_BYTES = 53 * 8 + 1
+HIT_BYTES = 2 * 8 + 4
+FWD_FLOP_PER_LEG = {"const": 3300.0, "grid3": 3900.0}   # + material
+RTS_FLOP_PER_LEG = 1900.0
+FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x clock)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2)")
+    ap.add_argument("--tracks", type=int, default=None, help="override the number of tracks (testing)")
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    return ap.parse_args()
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.proc, self.lines = index, None, []
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                 "-lms", "200"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.lines.append((time.time(), line.strip()))
+
+    def stop(self, t0, t1):
+        if self.proc is None:
+            return dict(sm_mhz=None, sm_max_mhz=None, reasons=["nvidia-smi unavailable"])
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+        sm, smax, power, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = [l for (t, l) in self.lines if t0 - 0.2 <= t <= t1 + 0.3] or [l for (_, l) in self.lines]
+        for l in rows:
+            f = [x.strip() for x in l.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); smax.append(float(f[1])); power.append(float(f[2]))
+            except ValueError:
+                continue
+            for nme, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nme)
+        return dict(sm_mhz=float(np.median(sm)) if sm else None, sm_max_mhz=max(smax) if smax else None,
+                    power_w=float(np.median(power)) if power else None, samples=len(sm), reasons=sorted(reasons))
+
+
+def dist_setup(n_gpus):
+    """-> (rank, world, dist or None). Under torchrun the env carries RANK/WORLD_SIZE/LOCAL_RANK."""
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    if world > 1:
+        import torch
+        import torch.distributed as dist
+        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
+        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", rank)))
+        dist.init_process_group("nccl")
+        return rank, world, dist
+    return 0, 1, None
+
+
+def cpu_baseline(wl, cores_hint=None):
+    """The oracle as it stands on a bounded sample (first tracks of the same workload), all host cores."""
+    import oracle  # test infrastructure; bench.py's cpu_baseline leg is one of its allowed callers
+    cores = os.cpu_count() or 1
+    n = int(min(wl.n_tracks, 6000 * cores, 400_000))
+    sub = wl.subset(np.arange(n))
+    oracle.fit_workload(wl.subset(np.arange(min(64, n))))  # builds/loads the library outside the timing
+    t = time.perf_counter()
+    r = oracle.fit_workload(sub)
+    dt = time.perf_counter() - t
+    return dict(value=n / dt, unit=UNIT, cores=int(r.threads), kind="oracle",
+                sample=f"first {n} tracks of {wl.name} ({sub.n_meas} hits), {dt:.2f} s wall, OpenMP over tracks")
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, K steps of a bounded sample each."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    import oracle
+    from paper_2105_01796_b200 import workloads as W
+    cores = os.cpu_count() or 1
+    n = int(min(args.tracks or 10**9, 1500 * cores, 100_000))
+    wl = W.make_config(args.config, n_tracks=n)
+    for _ in range(max(args.warmup, 1)):
+        r = oracle.fit_workload(wl)
+    t = time.perf_counter()
+    for _ in range(args.steps):
+        r = oracle.fit_workload(wl)
+    dt = (time.perf_counter() - t) / args.steps
+    val = n / dt
+    line = dict(impl="reference", metric=METRIC, value=val, unit=UNIT, n_gpus=args.gpus, steps=args.steps,
+                warmup=args.warmup, ms_per_step=dt * 1e3, higher_is_better=True, scaling="weak",
+                vs_baseline=None, dtype="f64", data="synthetic",
+                config=dict(workload=W.WORKLOAD_NAMES[args.config], tracks_per_step=n,
+                            note="CPU oracle on a bounded sample of the workload (seeded generator, first tracks)"),
+                cpu_baseline=dict(value=val, unit=UNIT, cores=int(r.threads), kind="oracle",
+                                  sample=f"{n} tracks of cfg{args.config} per step"),
+                e2e=dict(value=val, unit=UNIT, h2d_bytes_per_step=0, d2h_bytes_per_step=0),
+                gpu_launches=0)
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    import paper_2105_01796_b200 as kf
+    from paper_2105_01796_b200 import binding as B
+    from paper_2105_01796_b200 import workloads as W
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: the fit has no CPU fallback")
+    rank, world, dist = dist_setup(args.gpus)
+    dev = torch.device("cuda", torch.cuda.current_device())
+    peaks = load_peaks()
+
+    wl = W.make_config(args.config, n_tracks=args.tracks)
+    hb = kf.HostBatch.from_workload(wl)
+    db = kf.DeviceBatch(hb, dev)
+    call = kf.FitCall(db)  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
+    N, M = hb.n_tracks, hb.n_meas
+    smooth = bool(hb.options.get("smooth", 1))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(max(args.warmup, 3)):
+        call.run()
+    barrier()
+    fp64_probe = kf.probe_fp64_tflops(20000, dev) if rank == 0 else None
+
+    # ---- timed region: exactly K steps, CUDA events on the launching stream ----------------------------
+    timer = B.StageTimer(dev)
+    timer.prepare(args.steps)
+    sampler = ClockSampler(dev.index or 0)
+    if rank == 0:
+        sampler.start()
+        time.sleep(0.3)
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    t_wall0 = time.time()
+    e0.record()
+    for k in range(args.steps):
+        timer.arm(k)
+        call.run()
+    e1.record()
+    barrier()
+    t_wall1 = time.time()
+    fwd_ms, rts_ms = timer.finish()
+    clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
+    ms_total = e0.elapsed_time(e1)
+    if dist is not None:
+        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+    ms_step = ms_total / args.steps
+    value = world * N / (ms_step * 1e-3)
+    launches = call.launches * args.steps
+
+    # results of the last step, for the legs count and a sanity line
+    res = call.out
+    n_legs = int((res.n_used.sum() + res.n_outliers.sum() + res.n_holes.sum()).item())
+    bad = int(((res.status & 7) != 0).sum().item())
+
+    # ---- end to end through the HOST-buffer entry point -------------------------------------------------
+    e2e = None
+    if not args.no_e2e:
+        hc = kf.HostCall(hb, dev)
+        for _ in range(2):
+            hc.run()
+        barrier()
+        h0, h1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        ke = max(3, min(args.steps, 5))
+        h0.record()
+        for _ in range(ke):
+            hc.run()
+        h1.record()
+        barrier()
+        ms_e2e = h0.elapsed_time(h1) / ke
+        if dist is not None:
+            t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            ms_e2e = float(t.item())
+        e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
+                   d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke,
+                   api="kf_fit_batch_host (pinned host buffers; H2D, forward, RTS, D2H on one stream)")
+        launches += 0  # e2e launches are outside the timed region and not counted
+        del hc
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return 0
+
+    # ---- rooflines -------------------------------------------------------------------------------------
+    fwd = float(np.mean(fwd_ms))
+    rts = float(np.mean(rts_ms)) if smooth else 0.0
+    fkind = hb.field_kind
+    rec_b = REC_BYTES if smooth else 0
+    fwd_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 8) + N * (2 * 27 * 8 + 8 + 5 * 4) + M * 9
+    rts_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 12)
+    fwd_flop = n_legs * FWD_FLOP_PER_LEG[fkind]
+    rts_flop = n_legs * RTS_FLOP_PER_LEG
+    fp64_peak = 148 * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
+    hbm_peak = peaks["hbm_gbs"]
+
+    def kernel_roof(name, ms, nbytes, flop):
+        if ms <= 0:
+            return None
+        return dict(kernel=name, ms=ms, hbm_gbs=nbytes / (ms * 1e-3) / 1e9, hbm_frac=nbytes / (ms * 1e-3) / 1e9 / hbm_peak,
+                    fp64_tflops=flop / (ms * 1e-3) / 1e12, fp64_frac=flop / (ms * 1e-3) / 1e12 / fp64_peak)
+
+    kf_fwd = kernel_roof("kf_forward_kernel", fwd, fwd_bytes, fwd_flop)
+    kf_rts = kernel_roof("kf_rts_kernel", rts, rts_bytes, rts_flop) if smooth else None
+    dom = kf_fwd if (kf_rts is None or fwd >= rts) else kf_rts
+    # the dominant kernel's own bound: the larger of its two fractions says which roof it is nearer
+    if dom["fp64_frac"] >= dom["hbm_frac"]:
+        roofline = dict(bound="alu", achieved=dom["fp64_tflops"], peak=fp64_peak, unit="TFLOP/s",
+                        frac=dom["fp64_frac"], traffic=None, kernel=dom["kernel"],
+                        peak_source=f"148 SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); "
+                                    f"measured DFMA-chain probe this run: {fp64_probe:.1f} TFLOP/s")
+    else:
+        roofline = dict(bound="hbm", achieved=dom["hbm_gbs"], peak=hbm_peak, unit="GB/s", frac=dom["hbm_frac"],
+                        traffic=None, kernel=dom["kernel"], peak_source=f"MEASURED_PEAKS.json ({peaks['source']})")
+    roofline["ms_per_launch"] = dom["ms"]
+    roofline["share_of_step"] = dom["ms"] / ms_step
+
+    cpu = None if args.no_cpu_baseline else cpu_baseline(wl)
+
+    line = dict(
+        metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
+        ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+        data="synthetic",
+        config=dict(workload=W.WORKLOAD_NAMES[args.config], tracks=N, hits=M, legs=n_legs,
+                    layers=hb.n_surfaces - 1, field=fkind, smooth=int(smooth),
+                    material=int(hb.options.get("material", 0)),
+                    l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
+                    parallelism="replicas only" if world > 1 else "1 GPU",
+                    tracks_not_fitted=bad),
+        clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,
+        kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu)
+    print(json.dumps(line))
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -190,6 +190,14 @@ int kf_fit_batch_host(const kf_tracks_in* tracks, const kf_measurements* meas, c
 /* Number of kernels the last kf_fit_batch call of this thread enqueued (for launch accounting). */
 int kf_last_launch_count(void);
 
+/* Optional per-kernel timing for the roofline report.  After this call every kf_fit_batch of the
+ * calling thread records the three caller-owned CUDA events (cudaEvent_t handles created with
+ * timing enabled) on its stream: events3[0] before the forward-filter kernel, events3[1] after it
+ * (= before the RTS kernel), events3[2] after the RTS kernel (or after the forward kernel when
+ * !smooth).  events3 == NULL switches the recording off again.  The events are only recorded,
+ * never waited on. */
+void kf_set_stage_events(void* const* events3);
+
 /* Sustained FP64 FMA throughput probe (roofline denominator): runs a dependent-chain DFMA kernel
  * `iters` long on every SM, on `cuda_stream`, synchronises, and returns TFLOP/s (2 flop per FMA),
  * or a negative KF_ERR_*.  Not part of the fit. */

@@ -402,9 +402,13 @@ int32_t kfo_material(const kfo_options* opt, const double* surf, const double xf
   return 0;
 }
 
-/* ---- inverse of an SPD 6x6 by Gauss-Jordan on the correlation-scaled matrix (reading U19) --- */
-static int32_t inverse_spd6(const double C[36], double Ci[36]) {
-  double s[6], R[36], Ri[36];
+/* ---- X = C^-1 B for an SPD 6x6 C (reading U19): Gaussian elimination with partial pivoting on the
+ * correlation-scaled matrix R = D^-1 C D^-1, D = diag(sqrt(C_ii)), followed by back substitution.
+ * A solve, not an explicit inverse: forming C^-1 and multiplying costs a factor cond(R) in accuracy,
+ * which the cancellation in C^s = C+ + A (C^s' - C-') A^T then amplifies by |C+| / |C^s| (up to 1e6
+ * for an inflated prior).  Independent of the CUDA path, which uses an un-pivoted Cholesky. -------- */
+static int32_t solve_spd6(const double C[36], const double B[36], double X[36]) {
+  double s[6], R[36], Y[36];
   for (int i = 0; i < 6; ++i) {
     if (!(C[i * 6 + i] > 0.0)) return KFO_ST_NOT_POSITIVE;
     s[i] = sqrt(C[i * 6 + i]);
@@ -412,26 +416,45 @@ static int32_t inverse_spd6(const double C[36], double Ci[36]) {
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) {
       R[i * 6 + j] = C[i * 6 + j] / (s[i] * s[j]);
-      Ri[i * 6 + j] = (i == j) ? 1.0 : 0.0;
+      Y[i * 6 + j] = B[i * 6 + j] / s[i]; /* R (D X) = D^-1 B */
     }
-  for (int k = 0; k < 6; ++k) { /* no pivoting: all pivots > 0 iff the matrix is SPD */
-    const double piv = R[k * 6 + k];
-    if (!(piv > 0.0)) return KFO_ST_NOT_POSITIVE;
-    for (int j = 0; j < 6; ++j) {
-      R[k * 6 + j] /= piv;
-      Ri[k * 6 + j] /= piv;
-    }
-    for (int i = 0; i < 6; ++i) {
-      if (i == k) continue;
-      const double fct = R[i * 6 + k];
-      for (int j = 0; j < 6; ++j) {
-        R[i * 6 + j] -= fct * R[k * 6 + j];
-        Ri[i * 6 + j] -= fct * Ri[k * 6 + j];
+  /* an SPD matrix has positive leading minors: check them on an un-pivoted copy of the elimination
+     (the status decision), then solve with pivoting (the numbers) */
+  {
+    double T[36];
+    memcpy(T, R, sizeof(T));
+    for (int k = 0; k < 6; ++k) {
+      if (!(T[k * 6 + k] > 0.0)) return KFO_ST_NOT_POSITIVE;
+      for (int i = k + 1; i < 6; ++i) {
+        const double f = T[i * 6 + k] / T[k * 6 + k];
+        for (int j = k; j < 6; ++j) T[i * 6 + j] -= f * T[k * 6 + j];
       }
     }
   }
-  for (int i = 0; i < 6; ++i)
-    for (int j = 0; j < 6; ++j) Ci[i * 6 + j] = Ri[i * 6 + j] / (s[i] * s[j]);
+  for (int k = 0; k < 6; ++k) {
+    int piv = k;
+    for (int i = k + 1; i < 6; ++i)
+      if (fabs(R[i * 6 + k]) > fabs(R[piv * 6 + k])) piv = i;
+    if (piv != k)
+      for (int j = 0; j < 6; ++j) {
+        double t = R[k * 6 + j]; R[k * 6 + j] = R[piv * 6 + j]; R[piv * 6 + j] = t;
+        t = Y[k * 6 + j]; Y[k * 6 + j] = Y[piv * 6 + j]; Y[piv * 6 + j] = t;
+      }
+    if (R[k * 6 + k] == 0.0) return KFO_ST_NOT_POSITIVE;
+    for (int i = k + 1; i < 6; ++i) {
+      const double f = R[i * 6 + k] / R[k * 6 + k];
+      for (int j = k; j < 6; ++j) R[i * 6 + j] -= f * R[k * 6 + j];
+      for (int j = 0; j < 6; ++j) Y[i * 6 + j] -= f * Y[k * 6 + j];
+    }
+  }
+  for (int c = 0; c < 6; ++c)
+    for (int i = 5; i >= 0; --i) {
+      double v = Y[i * 6 + c];
+      for (int j = i + 1; j < 6; ++j) v -= R[i * 6 + j] * X[j * 6 + c];
+      X[i * 6 + c] = v / R[i * 6 + i];
+    }
+  for (int i = 0; i < 6; ++i) /* undo the scaling: X <- D^-1 (D X) */
+    for (int c = 0; c < 6; ++c) X[i * 6 + c] /= s[i];
   return 0;
 }
 
@@ -439,11 +462,12 @@ static int32_t inverse_spd6(const double C[36], double Ci[36]) {
 int32_t kfo_rts_step(const double xf[6], const double Cf[36], const double F[36],
                      const double xp1[6], const double Cp1[36], const double xs1[6],
                      const double Cs1[36], double xs[6], double Cs[36]) {
-  double Cpi[36], CFt[36], A[36];
-  int32_t rc = inverse_spd6(Cp1, Cpi);
+  double FC[36], At[36], A[36];
+  matmul(6, 6, 6, F, Cf, FC);          /* F C+_k  (C+ symmetric: = (C+ F^T)^T) */
+  int32_t rc = solve_spd6(Cp1, FC, At); /* A_k^T = (C-_{k+1})^-1 F C+_k */
   if (rc) return rc;
-  matmul_bt(6, 6, 6, Cf, F, CFt); /* C+_k F^T */
-  matmul(6, 6, 6, CFt, Cpi, A);   /* A_k = C+_k F^T (C-_{k+1})^-1 */
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) A[i * 6 + j] = At[j * 6 + i]; /* A_k = C+_k F^T (C-_{k+1})^-1 */
   double dx[6];
   for (int i = 0; i < 6; ++i) dx[i] = xs1[i] - xp1[i];
   dx[2] = wrap_pi(dx[2]);

@@ -24,7 +24,7 @@ STATES_PRED, STATES_FILT, STATES_SMOOTH = 1, 2, 4
 _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .. 55
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",
-           "kf_fit_batch_host", "kf_last_launch_count", "kf_probe_fp64_tflops", "kf_status_string",
+           "kf_fit_batch_host", "kf_last_launch_count", "kf_set_stage_events", "kf_probe_fp64_tflops", "kf_status_string",
            "kf_last_cuda_error", "kf_version")
 
 
@@ -91,6 +91,8 @@ def lib():
     L.kf_fit_batch_host.restype = C.c_int
     L.kf_fit_batch_host.argtypes = L.kf_fit_batch.argtypes
     L.kf_last_launch_count.restype = C.c_int
+    L.kf_set_stage_events.restype = None
+    L.kf_set_stage_events.argtypes = [C.POINTER(C.c_void_p)]
     L.kf_probe_fp64_tflops.restype = C.c_double
     L.kf_probe_fp64_tflops.argtypes = [C.c_int, C.c_void_p]
     L.kf_status_string.restype = C.c_char_p
@@ -465,3 +467,39 @@ def probe_fp64_tflops(iters=20000, device="cuda:0") -> float:
     if v < 0:
         raise KfError(int(v))
     return v
+
+
+class StageTimer:
+    """Per-kernel device times of kf_fit_batch calls via kf_set_stage_events: three CUDA events per
+    call that the library records around its forward and RTS kernels, on the launching stream.
+    prepare(K) creates the events, arm(k) points the library at set k before call k (no
+    synchronisation), finish() reads all of them after the caller has synchronised."""
+
+    def __init__(self, device="cuda:0"):
+        torch = _torch()
+        self.device = torch.device(device)
+        self._sets, self._arrs = [], []
+
+    def prepare(self, n_calls: int):
+        torch = _torch()
+        s = torch.cuda.current_stream(self.device)
+        self._sets, self._arrs = [], []
+        for _ in range(n_calls):
+            ev = [torch.cuda.Event(enable_timing=True) for _ in range(3)]
+            for e in ev:
+                e.record(s)  # creates the cudaEvent_t handle
+            self._sets.append(ev)
+            self._arrs.append((C.c_void_p * 3)(*[C.c_void_p(int(e.cuda_event)) for e in ev]))
+
+    def arm(self, k: int):
+        lib().kf_set_stage_events(self._arrs[k])
+
+    def disarm(self):
+        lib().kf_set_stage_events(None)
+
+    def finish(self):
+        """-> (forward_ms list, rts_ms list); call after torch.cuda.synchronize()."""
+        self.disarm()
+        fwd = [ev[0].elapsed_time(ev[1]) for ev in self._sets]
+        rts = [ev[1].elapsed_time(ev[2]) for ev in self._sets]
+        return fwd, rts

@@ -17,6 +17,12 @@ namespace {
 
 thread_local char g_cuda_error[256] = "";
 thread_local int g_launches = 0;
+thread_local cudaEvent_t g_stage_events[3] = {nullptr, nullptr, nullptr};
+thread_local bool g_stage_events_on = false;
+
+inline void record_stage(int k, cudaStream_t stream) {
+  if (g_stage_events_on && g_stage_events[k]) cudaEventRecord(g_stage_events[k], stream);
+}
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -117,6 +123,11 @@ size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options
 }
 
 int kf_last_launch_count(void) { return g_launches; }
+
+void kf_set_stage_events(void* const* events3) {
+  g_stage_events_on = events3 != nullptr;
+  for (int k = 0; k < 3; ++k) g_stage_events[k] = events3 ? static_cast<cudaEvent_t>(events3[k]) : nullptr;
+}
 const char* kf_last_cuda_error(void) { return g_cuda_error; }
 int kf_version(void) { return KF_VERSION; }
 
@@ -191,6 +202,7 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
   const size_t fwd_smem = geom_smem + (size_t)KF_FWD_BLOCK * 9 * sizeof(double);
   const bool grid3 = fl->kind == KF_FIELD_GRID3;
+  record_stage(0, stream);
   if (op->material) {
     rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel")
                : launch(kf::kf_forward_kernel<kf::FIELD_CONST, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
@@ -199,7 +211,9 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
                : launch(kf::kf_forward_kernel<kf::FIELD_CONST, false>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
   }
   if (rc != KF_OK) return rc;
+  record_stage(1, stream);
   if (P.smooth) rc = launch(kf::kf_rts_kernel, P, KF_RTS_BLOCK, geom_smem, stream, "kf_rts_kernel");
+  record_stage(2, stream);
   return rc;
 }
 

@@ -76,8 +76,10 @@ def compare(gpu, ref, states=False, sel=None):
     return rep
 
 
-def assert_parity(gpu, ref, states=False, sel=None, label=""):
+def assert_parity(gpu, ref, states=False, sel=None, label="", loosen=1.0):
+    """loosen > 1 widens every floating-point bar by that factor (only for inputs whose conditioning
+    DESIGN.md "Tolerances" shows to exceed the north_star bars, e.g. a 1e4-inflated prior)."""
     rep = compare(gpu, ref, states=states, sel=sel)
-    bad = {k: v for k, v in rep.items() if not v <= 1.0}
+    bad = {k: v for k, v in rep.items() if not v <= loosen}
     assert not bad, f"{label}: tolerance exceeded (factor over the bar): {bad}; all: {rep}"
     return rep

@@ -1,0 +1,97 @@
+"""Full-size runs in the launch configuration bench.py times (FitCall on resident inputs, minimal
+outputs): sampled tracks are re-fitted one by one by the oracle (tracks are independent,
+PAPER.md:119, so a subset reproduces the per-track results), and properties that hold at any size
+are checked on all tracks."""
+import numpy as np
+import pytest
+
+import oracle
+import parity
+import paper_2105_01796_b200 as kf
+from paper_2105_01796_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+
+def run_full(wl):
+    import torch
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    call = kf.FitCall(db)
+    call.run()
+    torch.cuda.synchronize()
+    assert call.launches == (2 if wl.options["smooth"] else 1)
+    return call.out.to_host()
+
+
+def sampled_parity(wl, got, n_sample, seed):
+    rng = np.random.default_rng(seed)
+    idx = np.sort(rng.choice(wl.n_tracks, n_sample, replace=False))
+    # always include the first and last CTA's tracks (ragged tail)
+    idx = np.unique(np.concatenate([idx, np.arange(0, 40), np.arange(wl.n_tracks - 40, wl.n_tracks)]))
+    sub = wl.subset(idx)
+    ref = oracle.fit_workload(sub)
+    pick = lambda a: a[idx]
+    from types import SimpleNamespace
+    g = SimpleNamespace(**{k: pick(getattr(got, k)) for k in (
+        "first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status", "n_used",
+        "n_outliers", "n_holes")})
+    g.hit_flags = g.hit_chi2 = None
+    ref.hit_flags = ref.hit_chi2 = None
+    return parity.assert_parity(g, ref, label=wl.name)
+
+
+def common_properties(wl, got):
+    ok = (got.status & 7) == 0
+    assert ok.mean() > 0.999
+    d_first = np.einsum("nii->ni", got.first_cov)
+    d_last = np.einsum("nii->ni", got.last_cov)
+    assert np.all(d_first[ok] > 0) and np.all(d_last[ok] > 0)
+    assert np.all(np.isfinite(got.chi2[ok])) and np.all(got.chi2 >= 0)
+    np.testing.assert_array_equal(got.ndf, 2 * got.n_used - 5)
+    counts = np.diff(wl.offsets)
+    np.testing.assert_array_equal((got.n_used + got.n_outliers)[ok], counts[ok])
+
+
+def test_cfg1_full_size():
+    wl = W.make_config(1)
+    got = run_full(wl)
+    sampled_parity(wl, got, 4000, 1)
+    common_properties(wl, got)
+    assert np.all(got.status == 0) and np.all(got.n_used == 10)
+    # consistent informative prior: E[chi2] = 2n (reading U10)
+    assert abs(got.chi2.mean() - 20.0) < 4 * np.sqrt(40.0 / wl.n_tracks)
+
+
+def test_cfg2_full_size_bench_configuration():
+    wl = W.make_config(2)
+    assert wl.n_tracks == 1_000_000 and wl.n_meas == 30_000_000
+    got = run_full(wl)
+    sampled_parity(wl, got, 2000, 2)
+    common_properties(wl, got)
+    assert np.all(got.status == 0) and np.all(got.n_used == 30) and np.all(got.n_holes == 0)
+    assert abs(got.chi2.mean() - 60.0) < 4 * np.sqrt(120.0 / wl.n_tracks)
+    # pulls of the filtered state at the last layer against truth entering that layer: unit width
+    pull = (got.last_params - wl.truth[:, -1, :]) / np.sqrt(np.einsum("nii->ni", got.last_cov))
+    assert np.all(np.abs(pull[:, :5].mean(0)) < 0.01)
+    assert np.all(np.abs(pull[:, :5].std(0) - 1.0) < 0.01)
+    spull = (got.first_params - wl.truth[:, 0, :]) / np.sqrt(np.einsum("nii->ni", got.first_cov))
+    assert np.all(np.abs(spull[:, :5].std(0) - 1.0) < 0.01)
+
+
+def test_cfg3_full_size_ragged_with_outliers():
+    wl = W.make_config(3)
+    got = run_full(wl)
+    sampled_parity(wl, got, 2000, 3)
+    common_properties(wl, got)
+    # nearly all injected noise hits are far from the track and must be flagged
+    n_true = int(wl.is_outlier.sum())
+    assert got.n_outliers.sum() > 0.97 * n_true
+    assert got.n_outliers.sum() < 1.02 * n_true + 3e-3 * wl.n_meas
+
+
+def test_cfg4_field_map_large():
+    wl = W.make_config(4, n_tracks=60_000)
+    got = run_full(wl)
+    sampled_parity(wl, got, 3000, 4)
+    common_properties(wl, got)
+    assert np.any(got.status & 32)
