@@ -134,12 +134,23 @@ def test_tilted_planes_general_field_direction_and_start_surface():
     cov0[:, range(6), range(6)] = np.array([0.5, 0.5, 5e-3, 5e-3, 0.05, 300.0]) ** 2
     cov0[:, 4, 4] = (0.05 * np.abs(params0[:, 4])) ** 2
     cov0[:, 0, 2] = cov0[:, 2, 0] = 0.3 * 0.5 * 5e-3  # a correlated start covariance
-    # hits: let the oracle itself not be the source -- plain random positions near the axis are fine
-    # for a parity test (chi2 is large; the arithmetic path is the same)
+    # hits: the start parameters transported plane to plane (step-level oracle call: an input
+    # generator here, never the CUDA path), smeared by the measurement resolution
     nh = L - start
     offsets = (np.arange(N + 1) * nh).astype(np.int32)
     surf_idx = np.tile(np.arange(start + 1, L + 1, dtype=np.int32), N)
-    loc = rng.uniform(-8, 8, (N * nh, 2))
+    fld = oracle.make_field("const", (0.3, -0.4, 1.7))
+    opt = oracle.make_options()
+    loc = np.zeros((N, nh, 2))
+    for i in range(N):
+        x = params0[i].copy()
+        for k in range(nh):
+            pr = oracle.propagate(fld, opt, x, geom[start + k], geom[start + k + 1])
+            assert pr.rc == 0
+            x = pr.x
+            loc[i, k] = x[:2]
+    loc = loc.reshape(-1, 2) + rng.standard_normal((N * nh, 2)) * np.array([0.01, 0.03])
+    params0 = params0 + rng.standard_normal((N, 6)) * np.sqrt(cov0[:, range(6), range(6)]) * 0.5
     got, ref = run_arrays(params0, cov0, start, offsets, surf_idx, loc, geom, field=("const", (0.3, -0.4, 1.7)),
                           material=1, smooth=1)
     parity.assert_parity(got, ref, states=True)
