@@ -36,10 +36,10 @@ METRIC = "fitted tracks/sec (device-timed, FP64)"
 UNIT = "tracks/s"
 
 # Algorithmic work per leg (one surface visited by one track), DESIGN.md "Rooflines":
-#   bytes: RTS record 53 doubles + 1 flag byte written by the forward kernel and read by the RTS
+#   bytes: RTS record 55 doubles + 1 flag byte written by the forward kernel and read by the RTS
 #          kernel, the hit (2 doubles + int32) read by both; per track 27 doubles in, outputs out.
 #   flops: FP64 flop per leg counted from ncu instruction counters (DFMA = 2), see profiles/.
-REC_BYTES = 53 * 8 + 1
+REC_BYTES = 55 * 8 + 1
 HIT_BYTES = 2 * 8 + 4
 FWD_FLOP_PER_LEG = {"const": 3300.0, "grid3": 3900.0}   # + material
 RTS_FLOP_PER_LEG = 1900.0

@@ -19,7 +19,8 @@ import numpy as np
 from . import build as _build
 
 GEOM_STRIDE = 20
-REC_DOUBLES = 53  # x-(6) C-(21) F(26): doubles per (leg, track) in the RTS workspace
+REC_DOUBLES = 55  # x-(6) C-(21) F(26) hit(2): doubles per (leg, track) in the RTS workspace
+TILE = 128         # tracks per workspace tile (= threads per CTA)
 STATES_PRED, STATES_FILT, STATES_SMOOTH = 1, 2, 4
 _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .. 55
 

@@ -13,6 +13,9 @@
 #pragma once
 
 #include <cstdint>
+#include <type_traits>
+
+#include "kf_math.cuh"
 
 namespace kf {
 
@@ -39,6 +42,8 @@ __host__ __device__ constexpr int SX(int i, int j) { return i <= j ? IX(i, j) : 
 
 struct FieldDesc {
   double b[3];        // CONST: field already in GeV/(e mm)
+  double b2;          // CONST: |b|^2
+  double inv_spacing[3];  // GRID3: 1 / spacing
   int n[3];           // GRID3 nodes
   double origin[3];
   double spacing[3];
@@ -47,6 +52,9 @@ struct FieldDesc {
 
 struct MaterialDesc {
   double mass;        // GeV
+  double inv_mass;    // 1 / mass
+  double rme;         // m_e / mass
+  double inv_I2;      // 1 / I^2, GeV^-2
   double ZA;          // Z / A
   double rho;         // g/cm^3
   double I_gev;       // mean excitation energy, GeV
@@ -75,7 +83,11 @@ __device__ __forceinline__ void field_at(const FieldDesc& F, const double r[3], 
     double w[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-      const double f = (r[a] - F.origin[a]) / F.spacing[a];
+      // correctly rounded quotient from the host-rounded reciprocal (Markstein): the cell index and the
+      // clamp flag must not depend on a last-bit difference from a true division
+      const double num = r[a] - F.origin[a];
+      double f = num * F.inv_spacing[a];
+      f = fma(fma(-f, F.spacing[a], num), F.inv_spacing[a], f);
       double fl = floor(f);
       fl = fmax(fl, 0.0);
       fl = fmin(fl, (double)(F.n[a] - 2));
@@ -120,7 +132,8 @@ __device__ __forceinline__ void cross_columns(const double X[9], const double B[
 // Advances (r, t, T) by a step of length h and returns the step-Jacobian blocks
 //   A = dr'/dT, a = dr'/dlam, Bm = dT'/dT, b = dT'/dlam, tau = dt'/dlam   (dr'/dr = I, dT'/dr = 0).
 template <int FIELD>
-__device__ __forceinline__ void rkn4_step(const FieldDesc& F, double mass, double r[3], double& t,
+// dtds = sqrt(1 + m^2 lam^2) and tfac = m^2 lam / dtds are constant along a leg (lam is).
+__device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, double tfac, double r[3], double& t,
                                           double T[3], double lam, double h, double A[9],
                                           double a[3], double Bm[9], double b[3], double& tau,
                                           double& eps, unsigned& status) {
@@ -208,15 +221,14 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double mass, doubl
   for (int i = 0; i < 3; ++i) sb[i] += l4[i];
 
   // Jacobian blocks
-  const double h6 = h / 6.0, h26 = h * h / 6.0;
+  const double h6 = h * (1.0 / 6.0), h26 = h * h6;
 #pragma unroll
   for (int i = 0; i < 9; ++i) { A[i] = h26 * SA[i]; Bm[i] = h6 * SB[i]; }
   A[0] += h; A[4] += h; A[8] += h;
   Bm[0] += 1.0; Bm[4] += 1.0; Bm[8] += 1.0;
 #pragma unroll
   for (int i = 0; i < 3; ++i) { a[i] = h26 * sa[i]; b[i] = h6 * sb[i]; }
-  const double dtds = sqrt(1.0 + mass * mass * lam * lam);
-  tau = h * mass * mass * lam / dtds;
+  tau = h * tfac;
 
   // error estimate (diagnostic)
   eps = h * h * (fabs(k1[0] - k2[0] - k3[0] + k4[0]) + fabs(k1[1] - k2[1] - k3[1] + k4[1]) +
@@ -229,13 +241,102 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double mass, doubl
     r[i] = r[i] + h * T[i] + h26 * (k1[i] + k2[i] + k3[i]);
     Tn[i] = T[i] + h6 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
   }
-  const double nrm = sqrt(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
+  const double inrm = rsqrt_nr(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) T[i] = Tn[i] / nrm;
+  for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
   t += h * dtds;
 }
 
-// 3x3 row-major helpers
+// ---- constant field: the RKN4 step in closed form ---------------------------------------------------
+// With B the same at the three field points, every stage derivative is a polynomial in
+// M = lam M_B (M_B v := v x B, M_B^3 = -|B|^2 M_B):  d1 = M, d2 = M + (h/2)M^2, d3 = d2 + (h^2/4)M^3,
+// d4 = M + hM^2 + (h^2/2)M^3 + (h^3/4)M^4, and k_i = d_i T.  The step of DESIGN.md A.2 therefore is,
+// with u = h lam, s = u^2 |B|^2, w1 = T x B, w2 = w1 x B:
+//   r' = r + hT + a1 w1 + a2 w2,   T' = normalise(T + c1 w1 + c2 w2),
+//   dr'/dT = hI + a1 M_B + a2 M_B^2,   dT'/dT = I + c1 M_B + c2 M_B^2,
+//   a1 = h u (1/2 - s/24), a2 = h u^2/6, c1 = u (1 - s/6), c2 = u^2 (1/2 - s/24),
+//   dr'/dlam = (da1) w1 + (da2) w2, dT'/dlam = (dc1) w1 + (dc2) w2  (derivatives of the coefficients),
+//   eps = h^2 |k1 - k2 - k3 + k4|_1 = h^2 |lam| (s/4) |w1 + u w2|_1.
+// Same discrete step, same Jacobian as the general code path: only the arithmetic is regrouped.  All
+// step Jacobians commute, so the accumulated D keeps the form  P = P0 I + P1 M_B + P2 M_B^2 (dr/dT0),
+// Q = I + Q1 M_B + Q2 M_B^2 (dT/dT0): six scalars instead of two 3x3 matrices.
+struct PolyJac {
+  double P0, P1, P2, Q1, Q2;  // Q0 == 1
+  double p[3], q[3], sigma;   // dr/dlam, dT/dlam, dt/dlam
+};
+
+// v -> c0 v + c1 (v x B) + c2 ((v x B) x B)
+__device__ __forceinline__ void poly_apply(const double B[3], double c0, double c1, double c2,
+                                           const double v[3], const double vx[3], const double vxx[3],
+                                           double out[3]) {
+#pragma unroll
+  for (int i = 0; i < 3; ++i) out[i] = fma(c2, vxx[i], fma(c1, vx[i], c0 * v[i]));
+}
+
+template <bool FIRST>
+__device__ __forceinline__ void const_field_step(const double B[3], double b2, double dtds, double tfac,
+                                                 double lam, double h, double r[3], double& t, double T[3],
+                                                 PolyJac& D, double& errmax) {
+  const double u = h * lam, uu = u * u, s = uu * b2;
+  const double e = fma(s, -1.0 / 24.0, 0.5);
+  const double c1 = u * fma(s, -1.0 / 6.0, 1.0);
+  const double c2 = uu * e;
+  const double a1 = h * u * e;
+  const double a2 = h * uu * (1.0 / 6.0);
+  const double hh = h * h;
+  const double dc1 = h * fma(s, -0.5, 1.0), dc2 = h * c1;
+  const double da1 = hh * fma(s, -0.125, 0.5), da2 = hh * u * (1.0 / 3.0);
+  double w1[3], w2[3];
+  cross(T, B, w1);
+  cross(w1, B, w2);
+  double av[3], bv[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    av[i] = fma(da2, w2[i], da1 * w1[i]);
+    bv[i] = fma(dc2, w2[i], dc1 * w1[i]);
+  }
+  const double eps = hh * fabs(lam) * 0.25 * s *
+                     (fabs(fma(u, w2[0], w1[0])) + fabs(fma(u, w2[1], w1[1])) + fabs(fma(u, w2[2], w1[2])));
+  errmax = fmax(errmax, eps);
+  // state
+  double Tn[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r[i] = fma(a2, w2[i], fma(a1, w1[i], fma(h, T[i], r[i])));
+    Tn[i] = fma(c2, w2[i], fma(c1, w1[i], T[i]));
+  }
+  const double inrm = rsqrt_nr(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
+  t = fma(h, dtds, t);
+  const double tau = h * tfac;
+  // D <- Dstep D
+  if constexpr (FIRST) {
+    D.P0 = h; D.P1 = a1; D.P2 = a2; D.Q1 = c1; D.Q2 = c2;
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { D.p[i] = av[i]; D.q[i] = bv[i]; }
+    D.sigma = tau;
+  } else {
+    double qx[3], qxx[3];
+    cross(D.q, B, qx);
+    cross(qx, B, qxx);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      D.p[i] += fma(a2, qxx[i], fma(a1, qx[i], fma(h, D.q[i], av[i])));
+      D.q[i] += fma(c2, qxx[i], fma(c1, qx[i], bv[i]));
+    }
+    // polynomial products modulo M_B^3 = -b2 M_B:  P += A Q,  Q = Bm Q   (A0 = h, Bm0 = Q0 = 1)
+    const double Q1 = D.Q1, Q2 = D.Q2;
+    D.P0 += h;
+    D.P1 += fma(h, Q1, a1) - b2 * fma(a1, Q2, a2 * Q1);
+    D.P2 += fma(h, Q2, fma(a1, Q1, a2)) - b2 * (a2 * Q2);
+    D.Q1 = (Q1 + c1) - b2 * fma(c1, Q2, c2 * Q1);
+    D.Q2 = fma(c1, Q1, Q2 + c2) - b2 * (c2 * Q2);
+    D.sigma += tau;
+  }
+}
+
+// 3x3 row-major helpers (general field path)
 __device__ __forceinline__ void mat3_mul(const double A[9], const double B[9], double C[9]) {
 #pragma unroll
   for (int i = 0; i < 3; ++i)
@@ -248,6 +349,10 @@ __device__ __forceinline__ void mat3_vec(const double A[9], const double x[3], d
   for (int i = 0; i < 3; ++i) y[i] = A[i * 3 + 0] * x[0] + A[i * 3 + 1] * x[1] + A[i * 3 + 2] * x[2];
 }
 
+struct MatJac {
+  double P[9], Q[9], p[3], q[3], sigma;
+};
+
 // The bound-to-bound Jacobian, non-trivial part: Ja rows (loc0, loc1, phi, theta) x columns
 // (loc0, loc1, phi, theta, qp); Jt = row t over the same columns.  Row qp = e_qp, column t = e_t.
 struct BoundJacobian {
@@ -256,89 +361,101 @@ struct BoundJacobian {
 };
 
 // ---- propagate a bound state from surface sf to surface st (A.1 - A.3) ---------------------------
-// trig = (sin phi, cos phi, sin theta, cos theta) of x.  Returns 0 or the stopping status bit.
+// trig = (sin phi, cos phi, sin theta, cos theta) of x on entry; on success it holds the values of
+// the predicted (phi, theta), taken from the direction vector itself.  Returns 0 or the stopping bit.
 template <int FIELD>
 __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, int n_corr,
                                               double max_step, const double* __restrict__ sf,
                                               const double* __restrict__ st, const double x[6],
-                                              const double trig[4], double xo[6], BoundJacobian& J,
+                                              double trig[4], double xo[6], BoundJacobian& J,
                                               double& errmax, unsigned& status) {
   const double sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
   // A.1 bound -> free
   double r[3], T[3];
 #pragma unroll
-  for (int i = 0; i < 3; ++i) r[i] = sf[i] + x[0] * sf[3 + i] + x[1] * sf[6 + i];
+  for (int i = 0; i < 3; ++i) r[i] = fma(x[1], sf[6 + i], fma(x[0], sf[3 + i], sf[i]));
   T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
   const double lam = x[4];
   double t = x[5];
-  const double Tphi[3] = {-sphi * sth, cphi * sth, 0.0};
+  const double Tphi[3] = {-T[1], T[0], 0.0};
   const double Tth[3] = {cphi * cth, sphi * cth, -sth};
   const double nt[3] = {st[9], st[10], st[11]};
   const double ct[3] = {st[0], st[1], st[2]};
+  const double ml = mass * lam;
+  double idtds;
+  const double dtds = sqrt_nr(fma(ml, ml, 1.0), idtds);  // dt/ds = sqrt(1 + m^2 lam^2)
+  const double tfac = mass * ml * idtds;                  // d(dt/ds)/dlam
 
   // A.2 stepping: n_sub primary steps + n_corr correction steps, no accept/reject
-  double P[9], Q[9], p[3], q[3], sigma = 0.0;
   int n_sub = 1;
-  {
-    const double nT = dot(nt, T);
-    if (!(nT > kNdotTMin)) return ST_PROPAGATION;
-    if (max_step > 0.0 && max_step < 1.0e300) {
-      const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-      const double s0 = dot(nt, dr) / nT;
-      double qn = ceil(fabs(s0) / max_step * (1.0 - 1e-12));
-      if (!(qn >= 1.0)) qn = 1.0;
-      if (qn > 1024.0) qn = 1024.0;
-      n_sub = (int)qn;
-    }
+  double nT = dot(nt, T);
+  if (!(nT > kNdotTMin)) return ST_PROPAGATION;
+  if (max_step > 0.0) {
+    const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+    const double s0 = dot(nt, dr) / nT;
+    double qn = ceil(fabs(s0) / max_step * (1.0 - 1e-12));
+    if (!(qn >= 1.0)) qn = 1.0;
+    if (qn > 1024.0) qn = 1024.0;
+    n_sub = (int)qn;
   }
   const int n_steps = n_sub + n_corr;
+  typename std::conditional<FIELD == FIELD_CONST, PolyJac, MatJac>::type D;
   for (int is = 0; is < n_steps; ++is) {
-    const double nT = dot(nt, T);
-    if (!(nT > kNdotTMin)) return ST_PROPAGATION;
+    if (is > 0) {
+      nT = dot(nt, T);
+      if (!(nT > kNdotTMin)) return ST_PROPAGATION;
+    }
     const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-    double h = dot(nt, dr) / nT;
-    if (is < n_sub) h = h / (double)(n_sub - is);
-    double A[9], a[3], Bm[9], b[3], tau, eps;
-    rkn4_step<FIELD>(F, mass, r, t, T, lam, h, A, a, Bm, b, tau, eps, status);
-    errmax = fmax(errmax, eps);
-    if (is == 0) {
-#pragma unroll
-      for (int i = 0; i < 9; ++i) { P[i] = A[i]; Q[i] = Bm[i]; }
-#pragma unroll
-      for (int i = 0; i < 3; ++i) { p[i] = a[i]; q[i] = b[i]; }
-      sigma = tau;
+    double h = dot(nt, dr) * rcp_nr(nT);
+    if (is < n_sub - 1) h = h / (double)(n_sub - is);
+    if constexpr (FIELD == FIELD_CONST) {
+      if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
+      else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
     } else {
-      // D <- Dstep D:  P += A Q,  p += A q + a,  Q = Bm Q,  q = Bm q + b,  sigma += tau
-      double AQ[9], Aq[3], BQ[9], Bq[3];
-      mat3_mul(A, Q, AQ);
-      mat3_vec(A, q, Aq);
-      mat3_mul(Bm, Q, BQ);
-      mat3_vec(Bm, q, Bq);
+      double A[9], a[3], Bm[9], b[3], tau, eps;
+      rkn4_step<FIELD>(F, dtds, tfac, r, t, T, lam, h, A, a, Bm, b, tau, eps, status);
+      errmax = fmax(errmax, eps);
+      if (is == 0) {
 #pragma unroll
-      for (int i = 0; i < 9; ++i) { P[i] += AQ[i]; Q[i] = BQ[i]; }
+        for (int i = 0; i < 9; ++i) { D.P[i] = A[i]; D.Q[i] = Bm[i]; }
 #pragma unroll
-      for (int i = 0; i < 3; ++i) { p[i] += Aq[i] + a[i]; q[i] = Bq[i] + b[i]; }
-      sigma += tau;
+        for (int i = 0; i < 3; ++i) { D.p[i] = a[i]; D.q[i] = b[i]; }
+        D.sigma = tau;
+      } else {
+        // D <- Dstep D:  P += A Q,  p += A q + a,  Q = Bm Q,  q = Bm q + b,  sigma += tau
+        double AQ[9], Aq[3], BQ[9], Bq[3];
+        mat3_mul(A, D.Q, AQ);
+        mat3_vec(A, D.q, Aq);
+        mat3_mul(Bm, D.Q, BQ);
+        mat3_vec(Bm, D.q, Bq);
+#pragma unroll
+        for (int i = 0; i < 9; ++i) { D.P[i] += AQ[i]; D.Q[i] = BQ[i]; }
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { D.p[i] += Aq[i] + a[i]; D.q[i] = Bq[i] + b[i]; }
+        D.sigma += tau;
+      }
     }
     const double fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
     if (!(fabs(fin) < 1.0e300)) return ST_PROPAGATION;  // catches NaN and Inf
   }
 
   // A.3 free -> bound with the path-length correction  D~ = (I - f' w^T) D
-  const double nT = dot(nt, T);
+  nT = dot(nt, T);
   if (!(nT > kNdotTMin)) return ST_PROPAGATION;
   double Bend[3], TxB[3];
   field_at<FIELD>(F, r, Bend, status);
   cross(T, Bend, TxB);
-  const double dtds = sqrt(1.0 + mass * mass * lam * lam);
   const double kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};  // dT/ds
-  const double w[3] = {nt[0] / nT, nt[1] / nT, nt[2] / nT};
+  const double inT = rcp_nr(nT);
+  const double w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
 
-  const double sth2 = sqrt(T[0] * T[0] + T[1] * T[1]);
-  if (!(sth2 > kSinThetaMin)) return ST_THETA;
+  const double st2 = fma(T[0], T[0], T[1] * T[1]);
+  if (!(st2 > kSinThetaMin * kSinThetaMin)) return ST_THETA;
+  double isth;
+  const double sth2 = sqrt_nr(st2, isth);
   const double cth2 = T[2];
-  const double cph2 = T[0] / sth2, sph2 = T[1] / sth2;
-  const double gphi[3] = {-sph2 / sth2, cph2 / sth2, 0.0};
+  const double cph2 = T[0] * isth, sph2 = T[1] * isth;
+  const double gphi[2] = {-sph2 * isth, cph2 * isth};
   const double gth[3] = {cph2 * cth2, sph2 * cth2, -sth2};
   const double* ut = st + 3;
   const double* vt = st + 6;
@@ -347,13 +464,12 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
   auto project = [&](int c, double cr[3], double ctime, double cT[3]) {
     const double wd = dot(w, cr);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) { cr[i] -= T[i] * wd; cT[i] -= kf_[i] * wd; }
-    ctime -= dtds * wd;
-    J.Ja[0][c] = ut[0] * cr[0] + ut[1] * cr[1] + ut[2] * cr[2];
-    J.Ja[1][c] = vt[0] * cr[0] + vt[1] * cr[1] + vt[2] * cr[2];
-    J.Ja[2][c] = gphi[0] * cT[0] + gphi[1] * cT[1];
-    J.Ja[3][c] = gth[0] * cT[0] + gth[1] * cT[1] + gth[2] * cT[2];
-    J.Jt[c] = ctime;
+    for (int i = 0; i < 3; ++i) { cr[i] = fma(-T[i], wd, cr[i]); cT[i] = fma(-kf_[i], wd, cT[i]); }
+    J.Ja[0][c] = dot(ut, cr);
+    J.Ja[1][c] = dot(vt, cr);
+    J.Ja[2][c] = fma(gphi[0], cT[0], gphi[1] * cT[1]);
+    J.Ja[3][c] = dot(gth, cT);
+    J.Jt[c] = fma(-dtds, wd, ctime);
   };
   {
     double cr[3] = {sf[3], sf[4], sf[5]}, cT[3] = {0.0, 0.0, 0.0};
@@ -363,21 +479,40 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
     double cr[3] = {sf[6], sf[7], sf[8]}, cT[3] = {0.0, 0.0, 0.0};
     project(1, cr, 0.0, cT);
   }
-  {
-    double cr[3], cT[3];
-    mat3_vec(P, Tphi, cr);
-    mat3_vec(Q, Tphi, cT);
-    project(2, cr, 0.0, cT);
+  if constexpr (FIELD == FIELD_CONST) {
+    {
+      double vx[3], vxx[3], cr[3], cT[3];
+      cross(Tphi, F.b, vx);
+      cross(vx, F.b, vxx);
+      poly_apply(F.b, D.P0, D.P1, D.P2, Tphi, vx, vxx, cr);
+      poly_apply(F.b, 1.0, D.Q1, D.Q2, Tphi, vx, vxx, cT);
+      project(2, cr, 0.0, cT);
+    }
+    {
+      double vx[3], vxx[3], cr[3], cT[3];
+      cross(Tth, F.b, vx);
+      cross(vx, F.b, vxx);
+      poly_apply(F.b, D.P0, D.P1, D.P2, Tth, vx, vxx, cr);
+      poly_apply(F.b, 1.0, D.Q1, D.Q2, Tth, vx, vxx, cT);
+      project(3, cr, 0.0, cT);
+    }
+  } else {
+    {
+      double cr[3], cT[3];
+      mat3_vec(D.P, Tphi, cr);
+      mat3_vec(D.Q, Tphi, cT);
+      project(2, cr, 0.0, cT);
+    }
+    {
+      double cr[3], cT[3];
+      mat3_vec(D.P, Tth, cr);
+      mat3_vec(D.Q, Tth, cT);
+      project(3, cr, 0.0, cT);
+    }
   }
   {
-    double cr[3], cT[3];
-    mat3_vec(P, Tth, cr);
-    mat3_vec(Q, Tth, cT);
-    project(3, cr, 0.0, cT);
-  }
-  {
-    double cr[3] = {p[0], p[1], p[2]}, cT[3] = {q[0], q[1], q[2]};
-    project(4, cr, sigma, cT);
+    double cr[3] = {D.p[0], D.p[1], D.p[2]}, cT[3] = {D.q[0], D.q[1], D.q[2]};
+    project(4, cr, D.sigma, cT);
   }
 
   const double dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
@@ -387,6 +522,7 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
   xo[3] = acos(fmin(fmax(T[2], -1.0), 1.0));
   xo[4] = lam;
   xo[5] = t;
+  trig[0] = sph2; trig[1] = cph2; trig[2] = sth2; trig[3] = cth2;
   double chk = xo[0] + xo[1] + xo[5];
 #pragma unroll
   for (int c = 0; c < 5; ++c) chk += J.Ja[0][c] + J.Ja[1][c] + J.Ja[2][c] + J.Ja[3][c] + J.Jt[c];
@@ -405,14 +541,14 @@ __device__ __forceinline__ void transport_covariance(const BoundJacobian& J, con
     for (int k = 0; k < 6; ++k) {
       double s = J.Ja[i][0] * C[SX(0, k)];
 #pragma unroll
-      for (int l = 1; l < 5; ++l) s += J.Ja[i][l] * C[SX(l, k)];
+      for (int l = 1; l < 5; ++l) s = fma(J.Ja[i][l], C[SX(l, k)], s);
       Ma[i][k] = s;
     }
 #pragma unroll
   for (int k = 0; k < 6; ++k) {
     double s = C[SX(5, k)];
 #pragma unroll
-    for (int l = 0; l < 5; ++l) s += J.Jt[l] * C[SX(l, k)];
+    for (int l = 0; l < 5; ++l) s = fma(J.Jt[l], C[SX(l, k)], s);
     Mt[k] = s;
   }
   // C- = M J^T, upper triangle
@@ -422,195 +558,246 @@ __device__ __forceinline__ void transport_covariance(const BoundJacobian& J, con
     for (int j = i; j < 4; ++j) {
       double s = Ma[i][0] * J.Ja[j][0];
 #pragma unroll
-      for (int l = 1; l < 5; ++l) s += Ma[i][l] * J.Ja[j][l];
+      for (int l = 1; l < 5; ++l) s = fma(Ma[i][l], J.Ja[j][l], s);
       Cp[IX(i, j)] = s;
     }
     Cp[IX(i, 4)] = Ma[i][4];
     double s = Ma[i][5];
 #pragma unroll
-    for (int l = 0; l < 5; ++l) s += Ma[i][l] * J.Jt[l];
+    for (int l = 0; l < 5; ++l) s = fma(Ma[i][l], J.Jt[l], s);
     Cp[IX(i, 5)] = s;
   }
   Cp[IX(4, 4)] = C[IX(4, 4)];
   {
     double s = C[IX(4, 5)];  // M[qp][t]
 #pragma unroll
-    for (int l = 0; l < 5; ++l) s += C[SX(4, l)] * J.Jt[l];
+    for (int l = 0; l < 5; ++l) s = fma(C[SX(4, l)], J.Jt[l], s);
     Cp[IX(4, 5)] = s;
   }
   {
     double s = Mt[5];
 #pragma unroll
-    for (int l = 0; l < 5; ++l) s += Mt[l] * J.Jt[l];
+    for (int l = 0; l < 5; ++l) s = fma(Mt[l], J.Jt[l], s);
     Cp[IX(5, 5)] = s;
   }
 }
 
 // ---- gain-matrix update with a 2-D hit (A.5) ----------------------------------------
-// Returns false when S is not positive definite.  xf/Cf may alias nothing of xp/Cp.
-__device__ __forceinline__ bool gain_update(const double xp[6], const double Cp[21], double m0,
-                                            double m1, double v00, double v01, double v11,
-                                            double xf[6], double Cf[21], double& chi2) {
-  const double r0 = m0 - xp[0], r1 = m1 - xp[1];
+// Split in two so that the outlier test (on chi2) comes before any state is written.
+struct Gain {
+  double r0, r1, i00, i01, i11;
+};
+// Returns false when S = H C- H^T + V is not positive definite.
+__device__ __forceinline__ bool gain_prepare(const double xp[6], const double Cp[21], double m0, double m1,
+                                             double v00, double v01, double v11, Gain& G, double& chi2) {
+  G.r0 = m0 - xp[0];
+  G.r1 = m1 - xp[1];
   const double S00 = Cp[IX(0, 0)] + v00, S01 = Cp[IX(0, 1)] + v01, S11 = Cp[IX(1, 1)] + v11;
-  const double det = S00 * S11 - S01 * S01;
+  const double det = fma(S00, S11, -S01 * S01);
   if (!(S00 > 0.0 && det > 0.0)) return false;
-  const double idet = 1.0 / det;
-  const double i00 = S11 * idet, i01 = -S01 * idet, i11 = S00 * idet;
-  chi2 = r0 * (i00 * r0 + i01 * r1) + r1 * (i01 * r0 + i11 * r1);
+  const double idet = rcp_nr(det);
+  G.i00 = S11 * idet;
+  G.i01 = -S01 * idet;
+  G.i11 = S00 * idet;
+  chi2 = G.r0 * fma(G.i00, G.r0, G.i01 * G.r1) + G.r1 * fma(G.i01, G.r0, G.i11 * G.r1);
+  return true;
+}
+// x+ = x- + K r, C+ = (I - K H) C-  with K = C- H^T S^-1.  xf/Cf must not alias xp/Cp.
+__device__ __forceinline__ void gain_apply(const Gain& G, const double xp[6], const double Cp[21],
+                                           double xf[6], double Cf[21]) {
   double K0[6], K1[6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
     const double c0 = Cp[SX(i, 0)], c1 = Cp[SX(i, 1)];
-    K0[i] = c0 * i00 + c1 * i01;
-    K1[i] = c0 * i01 + c1 * i11;
-    xf[i] = xp[i] + K0[i] * r0 + K1[i] * r1;
+    K0[i] = fma(c0, G.i00, c1 * G.i01);
+    K1[i] = fma(c0, G.i01, c1 * G.i11);
+    xf[i] = fma(K1[i], G.r1, fma(K0[i], G.r0, xp[i]));
   }
 #pragma unroll
   for (int i = 0; i < 6; ++i)
 #pragma unroll
     for (int j = i; j < 6; ++j)
-      Cf[IX(i, j)] = Cp[IX(i, j)] - (K0[i] * Cp[SX(0, j)] + K1[i] * Cp[SX(1, j)]);
-  return true;
+      Cf[IX(i, j)] = fma(-K1[i], Cp[SX(1, j)], fma(-K0[i], Cp[SX(0, j)], Cp[IX(i, j)]));
 }
 
 // ---- material at a surface, after the update (A.6) -----------------------------------
-// trig = sin/cos of the filtered phi, theta.  On success: lam -> lam', C -> G C G^T + Q in place.
-__device__ __forceinline__ bool apply_material(const MaterialDesc& Mt, const double* __restrict__ surf,
-                                               const double trig[4], double& lam, double C[21],
-                                               double& g) {
+// Highland theta0^2 and Bethe mean loss from the filtered state.  trig = sin/cos of the filtered
+// (phi, theta).  Returns false when the energy is exhausted (E' <= m).
+struct MaterialStep {
+  double lam_out, g, theta0sq_over_sin2, theta0sq;
+};
+__device__ __forceinline__ bool material_prepare(const MaterialDesc& Mt, const double* __restrict__ surf,
+                                                 const double trig[4], double lam, MaterialStep& S) {
   const double sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
-  const double T[3] = {cphi * sth, sphi * sth, cth};
   const double m = Mt.mass;
-  const double p = 1.0 / fabs(lam);
-  const double E = sqrt(p * p + m * m);
-  const double beta = p / E, gamma = E / m, bg = p / m;
-  const double cfac = 1.0 / fabs(surf[9] * T[0] + surf[10] * T[1] + surf[11] * T[2]);
-  // Highland
+  const double al = fabs(lam);
+  const double p = rcp_nr(al);
+  double iE;
+  const double E = sqrt_nr(fma(p, p, m * m), iE);
+  const double ib2 = (E * al) * (E * al);  // 1 / beta^2
+  const double bg = p * Mt.inv_mass, gamma = E * Mt.inv_mass;
+  const double nT = surf[9] * (cphi * sth) + surf[10] * (sphi * sth) + surf[11] * cth;
+  const double cfac = rcp_nr(fabs(nT));  // path factor 1/|n.T|
+  // Highland: theta0 = 0.0136/(beta p) sqrt(X) (1 + 0.038 ln(X/beta^2)),  1/(beta p) = E lam^2
   const double X = surf[14] * cfac;
-  const double b2 = beta * beta;
-  const double theta0 = 0.0136 / (beta * p) * sqrt(X) * (1.0 + 0.038 * log(X / b2));
+  const double theta0 = 0.0136 * (E * al * al) * sqrt_nr(X) * fma(0.038, log(X * ib2), 1.0);
   // Bethe, asymptotic density correction
   const double me = kElectronMass;
-  const double rme = me / m;
-  const double Wmax = 2.0 * me * bg * bg / (1.0 + 2.0 * gamma * rme + rme * rme);
+  const double Wmax = 2.0 * me * bg * bg * rcp_nr(1.0 + 2.0 * gamma * Mt.rme + Mt.rme * Mt.rme);
   const double dhalf = fmax(0.0, Mt.log_hwp_I + log(bg) - 0.5);
+  const double b2 = (p * iE) * (p * iE);
   const double dedx =
-      kBetheK * Mt.ZA / b2 * (0.5 * log(2.0 * me * bg * bg * Wmax / (Mt.I_gev * Mt.I_gev)) - b2 - dhalf);
+      kBetheK * Mt.ZA * ib2 * (0.5 * log(2.0 * me * bg * bg * Wmax * Mt.inv_I2) - b2 - dhalf);
   const double dE = dedx * Mt.rho * 1e-3 * 0.1 * surf[15] * cfac;
   const double E2 = E - dE;
   if (!(E2 > m)) return false;
-  const double p2 = sqrt(E2 * E2 - m * m);
-  g = (p * p * p * E2) / (p2 * p2 * p2 * E);
-  lam = (lam < 0.0 ? -1.0 : 1.0) / p2;
-  // C <- G C G^T + Q : row/column qp scaled by g
-#pragma unroll
-  for (int i = 0; i < 6; ++i)
-    if (i != 4) C[SX(i, 4)] *= g;
-  C[IX(4, 4)] *= g * g;
+  double ip2;
+  const double p2 = sqrt_nr(fma(E2, E2, -m * m), ip2);
+  (void)p2;
+  const double pr = p * ip2;
+  S.g = pr * pr * pr * E2 * iE;  // dlam'/dlam = p^3 E' / (p'^3 E)
+  S.lam_out = (lam < 0.0 ? -ip2 : ip2);
   const double t2 = theta0 * theta0;
-  C[IX(2, 2)] += t2 / (sth * sth);
-  C[IX(3, 3)] += t2;
+  S.theta0sq = t2;
+  S.theta0sq_over_sin2 = t2 * rcp_nr(sth * sth);
   return true;
 }
+// C <- G C G^T + Q : row/column qp scaled by g, Highland terms on the angle variances
+__device__ __forceinline__ void material_apply(const MaterialStep& S, double C[21]) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+    if (i != 4) C[SX(i, 4)] *= S.g;
+  C[IX(4, 4)] *= S.g * S.g;
+  C[IX(2, 2)] += S.theta0sq_over_sin2;
+  C[IX(3, 3)] += S.theta0sq;
+}
 
-// ---- one RTS step (A.7) --------------------------------------------------------------------
-// F = J G stored as 26 numbers: Fa[4][5], Ft[5] (column qp already scaled by g) and g.
-// In: filtered (xf, Cf) at k, record k+1 (xp1, Cp1, F), smoothed (xs, Cs) at k+1 (updated in place).
-__device__ __forceinline__ bool rts_step(const double xf[6], const double Cf[21],
-                                         const double Fa[4][5], const double Ft[5], double g,
-                                         const double xp1[6], const double Cp1[21], double xs[6],
-                                         double Cs[21]) {
-  // Cholesky C-_{k+1} = L L^T without pivoting; L[i][j] (i >= j) kept at packed (j, i)
-  double L[21], inv[6];
+// exact inverse of material_apply up to round-off (failure paths only)
+__device__ __forceinline__ void material_undo(const MaterialStep& S, double C[21]) {
+  const double ig = 1.0 / S.g;
+  C[IX(2, 2)] -= S.theta0sq_over_sin2;
+  C[IX(3, 3)] -= S.theta0sq;
 #pragma unroll
-  for (int j = 0; j < 6; ++j) {
-    double s = Cp1[IX(j, j)];
+  for (int i = 0; i < 6; ++i)
+    if (i != 4) C[SX(i, 4)] *= ig;
+  C[IX(4, 4)] *= ig * ig;
+}
+
+// ---- one RTS step (A.7), in two halves ---------------------------------------------------
+// R1 = this thread's column of record k+1 in shared memory (stride RS doubles): F = J G stored as
+// Fa[4][5], Ft[5] (column qp already scaled by g) and g, then x-_{k+1}, C-_{k+1}.
+// Head: everything that reads the record -- W = C+ F^T, Cholesky C-_{k+1} = L L^T (no pivoting; L[i][j],
+// i >= j, kept at packed (j, i); inv = 1/diag), dC = C^s_{k+1} - C-_{k+1} (in place in Cs),
+// dx = x^s_{k+1} - x-_{k+1} with the phi difference wrapped into (-pi, pi].  False on a non-positive pivot.
+template <int RS>
+__device__ __forceinline__ bool rts_gain_head(const double* __restrict__ R1, const double xf[6],
+                                              const double Cf[21], const double xs[6], double Cs[21],
+                                              double W[6][6], double L[21], double inv[6], double dx[6],
+                                              int oXp, int oCp, int oFa, int oFt, int oG) {
+  {
+    double Fa[4][5], Ft[5];
 #pragma unroll
-    for (int k = 0; k < j; ++k) s -= L[IX(k, j)] * L[IX(k, j)];
-    if (!(s > 0.0)) return false;
-    const double d = sqrt(s);
-    L[IX(j, j)] = d;
-    inv[j] = 1.0 / d;
+    for (int a = 0; a < 4; ++a)
 #pragma unroll
-    for (int i = j + 1; i < 6; ++i) {
-      double u = Cp1[IX(j, i)];
+      for (int c = 0; c < 5; ++c) Fa[a][c] = R1[(oFa + a * 5 + c) * RS];
 #pragma unroll
-      for (int k = 0; k < j; ++k) u -= L[IX(k, i)] * L[IX(k, j)];
-      L[IX(j, i)] = u * inv[j];
-    }
-  }
-  // A = C+ F^T (C-)^-1, one row at a time: w = row of C+ F^T, solve L L^T a = w
-  double A[6][6];
+    for (int c = 0; c < 5; ++c) Ft[c] = R1[(oFt + c) * RS];
+    const double g = R1[oG * RS];
 #pragma unroll
-  for (int i = 0; i < 6; ++i) {
-    double w[6];
+    for (int i = 0; i < 6; ++i) {
 #pragma unroll
-    for (int j = 0; j < 4; ++j) {
-      double s = Cf[SX(i, 0)] * Fa[j][0];
+      for (int j = 0; j < 4; ++j) {
+        double s = Cf[SX(i, 0)] * Fa[j][0];
 #pragma unroll
-      for (int k = 1; k < 5; ++k) s += Cf[SX(i, k)] * Fa[j][k];
-      w[j] = s;
-    }
-    w[4] = Cf[SX(i, 4)] * g;
-    {
+        for (int k = 1; k < 5; ++k) s = fma(Cf[SX(i, k)], Fa[j][k], s);
+        W[i][j] = s;
+      }
+      W[i][4] = Cf[SX(i, 4)] * g;
       double s = Cf[SX(i, 5)];
 #pragma unroll
-      for (int k = 0; k < 5; ++k) s += Cf[SX(i, k)] * Ft[k];
-      w[5] = s;
+      for (int k = 0; k < 5; ++k) s = fma(Cf[SX(i, k)], Ft[k], s);
+      W[i][5] = s;
+    }
+  }
+  bool ok = true;
+  {
+    double Cp1[21];
+#pragma unroll
+    for (int k = 0; k < 21; ++k) Cp1[k] = R1[(oCp + k) * RS];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      double s = Cp1[IX(j, j)];
+#pragma unroll
+      for (int k = 0; k < j; ++k) s = fma(-L[IX(k, j)], L[IX(k, j)], s);
+      if (!(s > 0.0)) { ok = false; s = 1.0; }
+      L[IX(j, j)] = sqrt_nr(s, inv[j]);
+#pragma unroll
+      for (int i = j + 1; i < 6; ++i) {
+        double u = Cp1[IX(j, i)];
+#pragma unroll
+        for (int k = 0; k < j; ++k) u = fma(-L[IX(k, i)], L[IX(k, j)], u);
+        L[IX(j, i)] = u * inv[j];
+      }
     }
 #pragma unroll
-    for (int r = 0; r < 6; ++r) {  // L y = w
-      double s = w[r];
+    for (int k = 0; k < 21; ++k) Cs[k] -= Cp1[k];
+  }
 #pragma unroll
-      for (int k = 0; k < r; ++k) s -= L[IX(k, r)] * w[k];
-      w[r] = s * inv[r];
+  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - R1[(oXp + j) * RS];
+  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
+  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+  return ok;
+}
+
+// Tail: A = W (L L^T)^-1 row by row (in place), x^s_k = x+_k + A dx, C^s_k = C+_k + A dC A^T.
+// On entry Cs holds dC; on exit (xs, Cs) is the smoothed state at k.  False if the result is not finite.
+__device__ __forceinline__ bool rts_gain_tail(const double xf[6], double Cf[21], double W[6][6],
+                                              const double L[21], const double inv[6], const double dx[6],
+                                              double xs[6], double Cs[21]) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {  // L y = w
+      double s = W[i][r];
+#pragma unroll
+      for (int k = 0; k < r; ++k) s = fma(-L[IX(k, r)], W[i][k], s);
+      W[i][r] = s * inv[r];
     }
 #pragma unroll
     for (int r = 5; r >= 0; --r) {  // L^T a = y
-      double s = w[r];
+      double s = W[i][r];
 #pragma unroll
-      for (int k = r + 1; k < 6; ++k) s -= L[IX(r, k)] * w[k];
-      w[r] = s * inv[r];
+      for (int k = r + 1; k < 6; ++k) s = fma(-L[IX(r, k)], W[i][k], s);
+      W[i][r] = s * inv[r];
     }
-#pragma unroll
-    for (int j = 0; j < 6; ++j) A[i][j] = w[j];
   }
-  // x^s_k = x+_k + A (x^s_{k+1} - x-_{k+1}),  phi difference wrapped into (-pi, pi]
-  double dx[6];
-#pragma unroll
-  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - xp1[j];
-  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
-  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
-  // C^s_k = C+_k + A (C^s_{k+1} - C-_{k+1}) A^T
-  double dC[21];
-#pragma unroll
-  for (int k = 0; k < 21; ++k) dC[k] = Cs[k] - Cp1[k];
   double chk = 0.0;
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
     double s = xf[i];
 #pragma unroll
-    for (int j = 0; j < 6; ++j) s += A[i][j] * dx[j];
+    for (int j = 0; j < 6; ++j) s = fma(W[i][j], dx[j], s);
     xs[i] = s;
     chk += s;
     double AdC[6];
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-      double u = A[i][0] * dC[SX(0, j)];
+      double u = W[i][0] * Cs[SX(0, j)];
 #pragma unroll
-      for (int k = 1; k < 6; ++k) u += A[i][k] * dC[SX(k, j)];
+      for (int k = 1; k < 6; ++k) u = fma(W[i][k], Cs[SX(k, j)], u);
       AdC[j] = u;
     }
 #pragma unroll
     for (int j = i; j < 6; ++j) {
       double u = Cf[IX(i, j)];
 #pragma unroll
-      for (int k = 0; k < 6; ++k) u += AdC[k] * A[j][k];
-      Cs[IX(i, j)] = u;
+      for (int k = 0; k < 6; ++k) u = fma(AdC[k], W[j][k], u);
+      Cf[IX(i, j)] = u;  // each C+ entry is consumed exactly here: reuse its register
       chk += u;
     }
   }
+#pragma unroll
+  for (int k = 0; k < 21; ++k) Cs[k] = Cf[k];
   return fabs(chk) < 1.0e300;
 }
 

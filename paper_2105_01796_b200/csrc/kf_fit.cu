@@ -26,22 +26,23 @@ inline void record_stage(int k, cudaStream_t stream) {
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Workspace: tile-major RTS records, then the per-track leg counts.
 struct WorkspaceLayout {
-  size_t rec_off, flag_off, nleg_off, total;
-  long long Np;
+  size_t rec_off, nleg_off, total;
+  size_t tile_stride;
+  long long n_tiles;
 };
 
 WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth) {
   WorkspaceLayout w{};
-  w.Np = (long long)align_up((size_t)(N > 0 ? N : 0), 32);
+  w.n_tiles = N > 0 ? (N + KF_TILE - 1) / KF_TILE : 0;
   if (!smooth || N <= 0 || n_legs_max <= 0) return w;
   size_t off = 0;
   w.rec_off = off;
-  off += align_up((size_t)n_legs_max * kf::kRecDoubles * (size_t)w.Np * sizeof(double), 256);
-  w.flag_off = off;
-  off += align_up((size_t)n_legs_max * (size_t)w.Np, 256);
+  w.tile_stride = (size_t)n_legs_max * kf::kLegBytes;
+  off += align_up((size_t)w.n_tiles * w.tile_stride, 256);
   w.nleg_off = off;
-  off += align_up((size_t)w.Np * sizeof(int), 256);
+  off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
   w.total = off;
   return w;
 }
@@ -58,7 +59,7 @@ int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_
     if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name))
       return KF_ERR_CUDA;
   }
-  const unsigned grid = (unsigned)((P.N + block - 1) / block);
+  const unsigned grid = (unsigned)((P.N + block - 1) / block);  // block == KF_TILE: one CTA per tile
   kernel<<<grid, block, smem, stream>>>(P);
   if (set_cuda_error(cudaGetLastError(), name)) return KF_ERR_CUDA;
   g_launches++;
@@ -155,26 +156,31 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (w.total > 0 && (!workspace || workspace_bytes < w.total)) return KF_ERR_WORKSPACE;
 
   kf::FitParams P{};
-  P.N = N; P.Np = w.Np; P.M = ms->n_meas;
+  P.N = N; P.M = ms->n_meas;
   P.params = tr->params; P.cov = tr->cov; P.start = tr->start_surface;
   P.offsets = ms->offsets; P.surf_idx = ms->surf_idx; P.loc = ms->loc; P.var = ms->var; P.cov01 = ms->cov01;
   P.n_surfaces = ge->n_surfaces; P.geom = ge->surfaces;
   P.geom_in_smem = ge->n_surfaces <= 1024 ? 1 : 0;
   if (fl->kind == KF_FIELD_CONST) {
     for (int a = 0; a < 3; ++a) P.field.b[a] = fl->b[a] * 2.99792458e-4;  // tesla -> GeV/(e mm)
+    P.field.b2 = P.field.b[0] * P.field.b[0] + P.field.b[1] * P.field.b[1] + P.field.b[2] * P.field.b[2];
   } else {
     for (int a = 0; a < 3; ++a) {
       P.field.n[a] = fl->n[a];
       P.field.origin[a] = fl->origin[a];
       P.field.spacing[a] = fl->spacing[a];
+      P.field.inv_spacing[a] = 1.0 / fl->spacing[a];
     }
     P.field.grid = fl->grid;
   }
   P.mat.mass = op->mass_gev;
+  P.mat.inv_mass = 1.0 / op->mass_gev;
+  P.mat.rme = 0.51099895e-3 / op->mass_gev;
   if (op->material) {
     P.mat.ZA = ge->mat_Z / ge->mat_A;
     P.mat.rho = ge->mat_rho;
     P.mat.I_gev = ge->mat_I_eV * 1e-9;
+    P.mat.inv_I2 = 1.0 / (P.mat.I_gev * P.mat.I_gev);
     P.mat.log_hwp_I = log(28.816e-9 * sqrt(ge->mat_rho * P.mat.ZA) / P.mat.I_gev);
   }
   P.smooth = op->smooth ? 1 : 0;
@@ -191,8 +197,9 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   P.hit_chi2 = out->hit_chi2; P.hit_flags = out->hit_flags; P.rk_err_max = out->rk_err_max;
   if (w.total > 0) {
     char* base = static_cast<char*>(workspace);
-    P.rec = reinterpret_cast<double*>(base + w.rec_off);
-    P.legflag = reinterpret_cast<unsigned char*>(base + w.flag_off);
+    P.rec = base + w.rec_off;
+    P.leg_stride = kf::kLegBytes;
+    P.tile_stride = w.tile_stride;
     P.nleg = reinterpret_cast<int*>(base + w.nleg_off);
   } else {
     P.smooth = 0;  // no legs to smooth (Lmax == 0)
@@ -200,19 +207,20 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
 
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
-  const size_t fwd_smem = geom_smem + (size_t)KF_FWD_BLOCK * 9 * sizeof(double);
+  const size_t fwd_smem = geom_smem;
+  const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
   const bool grid3 = fl->kind == KF_FIELD_GRID3;
   record_stage(0, stream);
   if (op->material) {
-    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel")
-               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, true>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
+    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, true>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel")
+               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, true>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel");
   } else {
-    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, false>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel")
-               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, false>, P, KF_FWD_BLOCK, fwd_smem, stream, "kf_forward_kernel");
+    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, false>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel")
+               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, false>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel");
   }
   if (rc != KF_OK) return rc;
   record_stage(1, stream);
-  if (P.smooth) rc = launch(kf::kf_rts_kernel, P, KF_RTS_BLOCK, geom_smem, stream, "kf_rts_kernel");
+  if (P.smooth) rc = launch(kf::kf_rts_kernel, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
   record_stage(2, stream);
   return rc;
 }

@@ -11,26 +11,26 @@
 //                       trades ~170 flops per leg for 27 doubles of HBM traffic each way
 //                       (DESIGN.md "RTS record").
 //
-// Workspace layout, Np = N rounded up to 32:
-//   rec   double[Lmax][kRecDoubles][Np]   component-major within a leg: a warp's 32 tracks write
-//                                         32 consecutive doubles per component (256 B, coalesced)
-//   flag  uint8 [Lmax][Np]                0 hole, 1 used, 2 outlier
-//   nleg  int32 [Np]                      number of legs the forward pass completed
+// Workspace layout: tile-major, one tile = KF_TILE tracks = one CTA.
+//   rec   [tile][leg]{ double[kRecDoubles][KF_TILE]; uint8 flag[KF_TILE] }   (kLegBytes per tile-leg)
+//         a warp's 32 tracks write 32 consecutive doubles per component (256 B, coalesced); the component
+//         stride is a compile-time constant (immediate offsets); the RTS kernel fetches one tile-leg with
+//         one bulk async copy.  flag: 0 hole, 1 used, 2 outlier.
+//   nleg  int32 [tiles * KF_TILE]   number of legs the forward pass completed
 #pragma once
 
 #include "kf_device.cuh"
 
 namespace kf {
 
-constexpr int kRecDoubles = 53;  // x-(6) C-(21) Fa(20) Ft(5) g(1)
-constexpr int kRecXp = 0, kRecCp = 6, kRecFa = 27, kRecFt = 47, kRecG = 52;
+constexpr int kRecDoubles = 55;  // x-(6) C-(21) Fa(20) Ft(5) g(1) hit(2)
+constexpr int kRecXp = 0, kRecCp = 6, kRecFa = 27, kRecFt = 47, kRecG = 52, kRecM = 53;
 
-#ifndef KF_FWD_BLOCK
-#define KF_FWD_BLOCK 128
+// tracks per tile = threads per CTA of both kernels (the record layout is tiled by it)
+#ifndef KF_TILE
+#define KF_TILE 128
 #endif
-#ifndef KF_RTS_BLOCK
-#define KF_RTS_BLOCK 128
-#endif
+constexpr size_t kLegBytes = (size_t)kRecDoubles * KF_TILE * sizeof(double) + KF_TILE;  // record + flags
 #ifndef KF_FWD_MIN_BLOCKS
 #define KF_FWD_MIN_BLOCKS 1
 #endif
@@ -42,7 +42,7 @@ enum : int { OUT_PRED = 1, OUT_FILT = 2, OUT_SMOOTH = 4 };
 
 struct FitParams {
   // inputs
-  long long N, Np, M;
+  long long N, M;
   const double* params;   // [6][N]
   const double* cov;      // [21][N]
   int start;
@@ -69,8 +69,9 @@ struct FitParams {
   unsigned char* hit_flags;
   double* rk_err_max;
   // workspace
-  double* rec;
-  unsigned char* legflag;
+  char* rec;            // [tile][leg]{ double[kRecDoubles][KF_TILE]; uint8 flag[KF_TILE] }
+  size_t leg_stride;    // = kLegBytes
+  size_t tile_stride;   // = Lmax * kLegBytes
   int* nleg;
 };
 
@@ -93,34 +94,19 @@ __device__ __forceinline__ const double* stage_geometry(const FitParams& P, doub
 }
 
 
-// indices of the 9 numbers the material step changes: q/p, C(i,4) for i = 0..5, C(2,2), C(3,3)
-__device__ __forceinline__ void stash_save(double* s, int stride, const double x[6], const double C[21]) {
-  s[0] = x[4];
-#pragma unroll
-  for (int k = 0; k < 6; ++k) s[(1 + k) * stride] = C[SX(k, 4)];
-  s[7 * stride] = C[IX(2, 2)];
-  s[8 * stride] = C[IX(3, 3)];
-}
-__device__ __forceinline__ void stash_restore(const double* s, int stride, double x[6], double C[21]) {
-  x[4] = s[0];
-#pragma unroll
-  for (int k = 0; k < 6; ++k) C[SX(k, 4)] = s[(1 + k) * stride];
-  C[IX(2, 2)] = s[7 * stride];
-  C[IX(3, 3)] = s[8 * stride];
-}
-
 // =====================================================================================================
-// Forward filter.  Dynamic shared memory: [geometry table if geom_in_smem][9 doubles per thread].
+// Forward filter.  Dynamic shared memory: [geometry table if geom_in_smem].
+// Material is applied lazily, at the top of the next leg, so that on exit (x, C) is the filtered
+// state of the last completed leg before that layer's material (= last_*); the material step of the
+// last surface is still evaluated for its status bit (energy exhausted), as in DESIGN.md A.6.
 template <int FIELD, bool MATERIAL>
-__global__ void __launch_bounds__(KF_FWD_BLOCK, KF_FWD_MIN_BLOCKS)
+__global__ void __launch_bounds__(KF_TILE, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   extern __shared__ double s_dyn[];
   const double* __restrict__ G = stage_geometry(P, s_dyn);
-  double* stash = s_dyn + (P.geom_in_smem ? P.n_surfaces * 20 : 0) + threadIdx.x;
-  const int sstride = blockDim.x;
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  const long long i = (long long)blockIdx.x * KF_TILE + threadIdx.x;
   if (i >= P.N) return;
-  const long long N = P.N, Np = P.Np;
+  const long long N = P.N;
 
   const int o0 = P.offsets[i], o1 = P.offsets[i + 1];
   double x[6], C[21];
@@ -144,51 +130,75 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     else n_target = prev_s - P.start;  // visit every surface up to the one of the last hit (U7)
   }
 
-  double chi2 = 0.0, errmax = 0.0, g_prev = 1.0;
+  double chi2 = 0.0, errmax = 0.0;
   int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0, hp = o0;
-  bool mat_applied = false;
   double trig[4];
   sincos(x[2], &trig[0], &trig[1]);
   sincos(x[3], &trig[2], &trig[3]);
+  // this tile's records: [leg][kRecDoubles][KF_TILE] doubles + [KF_TILE] flag bytes per leg
+  char* __restrict__ tile_base = P.rec + (size_t)blockIdx.x * P.tile_stride;
+  char* __restrict__ tile_rec = tile_base + (size_t)threadIdx.x * sizeof(double);
+  unsigned char* __restrict__ tile_flag =
+      reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(double) + threadIdx.x;
 
   for (int l = 0; l < n_target; ++l) {
     const int s = P.start + 1 + l;
     const double* __restrict__ sf = G + (s - 1) * 20;
     const double* __restrict__ st = G + s * 20;
+    // material of the previous surface, from its filtered state (U6, U16).  C is advanced through
+    // the layer only after the propagation succeeded, so that a failed leg leaves (x, C) = last_*.
+    double g_prev = 1.0;
+    const double lam_filtered = x[4];
+    MaterialStep ms;
+    const bool mat_here = MATERIAL && l > 0 && sf[14] > 0.0;
+    if (mat_here) {
+      if (!material_prepare(P.mat, sf, trig, x[4], ms)) { status |= ST_ENERGY; break; }
+      x[4] = ms.lam_out;
+      g_prev = ms.g;
+    }
     double xp[6];
     BoundJacobian J;
-    double e = 0.0;
     const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, sf, st, x, trig,
-                                         xp, J, e, status);
-    if (rc) { status |= rc; break; }
-    errmax = fmax(errmax, e);
+                                         xp, J, errmax, status);
+    if (rc) {
+      status |= rc;
+      x[4] = lam_filtered;
+      break;
+    }
+    if (mat_here) material_apply(ms, C);
     double Cp[21];
     transport_covariance(J, C, Cp);
 
-    // RTS record: x-, C-, F = J G_prev, g_prev ("stored Jacobians")
+    // hit of this surface, if any
+    const bool has_hit = (hp < o1) && (P.surf_idx[hp] == s);
+    double m0 = 0.0, m1 = 0.0;
+    if (has_hit) { m0 = P.loc[hp]; m1 = P.loc[P.M + hp]; }
+
+    // RTS record: x-, C-, F = J G_prev, g_prev, hit ("stored Jacobians")
+    double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth) {
-      double* __restrict__ R = P.rec + (size_t)l * kRecDoubles * Np + i;
 #pragma unroll
-      for (int k = 0; k < 6; ++k) R[(kRecXp + k) * Np] = xp[k];
+      for (int k = 0; k < 6; ++k) R[(kRecXp + k) * KF_TILE] = xp[k];
 #pragma unroll
-      for (int k = 0; k < 21; ++k) R[(kRecCp + k) * Np] = Cp[k];
+      for (int k = 0; k < 21; ++k) R[(kRecCp + k) * KF_TILE] = Cp[k];
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) R[(kRecFa + a * 5 + c) * Np] = J.Ja[a][c];
-        R[(kRecFa + a * 5 + 4) * Np] = J.Ja[a][4] * g_prev;
+        for (int c = 0; c < 4; ++c) R[(kRecFa + a * 5 + c) * KF_TILE] = J.Ja[a][c];
+        R[(kRecFa + a * 5 + 4) * KF_TILE] = J.Ja[a][4] * g_prev;
       }
 #pragma unroll
-      for (int c = 0; c < 4; ++c) R[(kRecFt + c) * Np] = J.Jt[c];
-      R[(kRecFt + 4) * Np] = J.Jt[4] * g_prev;
-      R[kRecG * Np] = g_prev;
+      for (int c = 0; c < 4; ++c) R[(kRecFt + c) * KF_TILE] = J.Jt[c];
+      R[(kRecFt + 4) * KF_TILE] = J.Jt[4] * g_prev;
+      R[kRecG * KF_TILE] = g_prev;
+      R[kRecM * KF_TILE] = m0;
+      R[(kRecM + 1) * KF_TILE] = m1;
     }
 
     // gain-matrix update with the surface's hit, or hole
     unsigned char flag = 0;
-    const bool has_hit = (hp < o1) && (P.surf_idx[hp] == s);
+    bool updated = false;
     if (has_hit) {
-      const double m0 = P.loc[hp], m1 = P.loc[P.M + hp];
       double v00, v11, v01 = 0.0;
       if (P.var) {
         v00 = P.var[hp];
@@ -198,16 +208,20 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
         v00 = st[16];
         v11 = st[17];
       }
+      Gain gn;
       double c2 = 0.0;
-      if (!gain_update(xp, Cp, m0, m1, v00, v01, v11, x, C, c2)) { status |= ST_NOT_POSITIVE; break; }
+      if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
+        status |= ST_NOT_POSITIVE;
+        if (mat_here) material_undo(ms, C);
+        x[4] = lam_filtered;
+        break;
+      }
       if (P.outlier_chi2 > 0.0 && c2 > P.outlier_chi2) {  // strictly greater: flagged, not used (U9)
-#pragma unroll
-        for (int k = 0; k < 6; ++k) x[k] = xp[k];
-#pragma unroll
-        for (int k = 0; k < 21; ++k) C[k] = Cp[k];
         n_outl++;
         flag = 2;
       } else {
+        gain_apply(gn, xp, Cp, x, C);
+        updated = true;
         chi2 += c2;
         n_used++;
         flag = 1;
@@ -216,13 +230,18 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       if (P.hit_flags) P.hit_flags[hp] = flag;
       hp++;
     } else {
+      n_holes++;
+    }
+    if (updated) {
+      sincos(x[2], &trig[0], &trig[1]);
+      sincos(x[3], &trig[2], &trig[3]);
+    } else {  // hole or outlier: the filtered state is the predicted one (trig already holds its angles)
 #pragma unroll
       for (int k = 0; k < 6; ++k) x[k] = xp[k];
 #pragma unroll
       for (int k = 0; k < 21; ++k) C[k] = Cp[k];
-      n_holes++;
     }
-    if (P.smooth) P.legflag[(size_t)l * Np + i] = flag;
+    if (P.smooth) tile_flag[(size_t)l * P.leg_stride] = flag;
     if (P.output_states & OUT_PRED) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
       store21(P.state_cov[0] + (size_t)l * 21 * N, N, i, Cp);
@@ -236,25 +255,14 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       store21(P.first_cov, N, i, C);
     }
     nleg++;
-
-    // material after the update, at every visited surface (U6).  The 9 numbers it changes are
-    // stashed in shared memory so that last_* can be the pre-material filtered state.
-    sincos(x[2], &trig[0], &trig[1]);
-    sincos(x[3], &trig[2], &trig[3]);
-    g_prev = 1.0;
-    mat_applied = false;
-    if (MATERIAL && st[14] > 0.0) {
-      stash_save(stash, sstride, x, C);
-      double lam = x[4], g = 1.0;
-      if (!apply_material(P.mat, st, trig, lam, C, g)) { status |= ST_ENERGY; break; }
-      x[4] = lam;
-      g_prev = g;
-      mat_applied = true;
-    }
   }
 
-  // x, C = state after the last completed leg (start state if none); undo its material step
-  if (MATERIAL && mat_applied) stash_restore(stash, sstride, x, C);
+  // (x, C) = filtered state of the last completed leg, before that layer's material (start state if none)
+  if (MATERIAL && nleg == n_target && nleg > 0) {  // the last surface's material: status bit only
+    const double* __restrict__ sl = G + (P.start + nleg) * 20;
+    MaterialStep ms;
+    if (sl[14] > 0.0 && !material_prepare(P.mat, sl, trig, x[4], ms)) status |= ST_ENERGY;
+  }
   store6(P.last_params, N, i, x);
   store21(P.last_cov, N, i, C);
   if (nleg == 0) {
@@ -279,49 +287,73 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 }
 
 // =====================================================================================================
-// RTS backward pass.  Record k holds x-_k, C-_k, F_k = dx-_k/dx+_{k-1}.
+// RTS backward pass.  Record k holds x-_k, C-_k, F_k = dx-_k/dx+_{k-1}, the hit.
 //   A_k = C+_k F_{k+1}^T (C-_{k+1})^-1,  x^s_k = x+_k + A_k (x^s_{k+1} - x-_{k+1}),
 //   C^s_k = C+_k + A_k (C^s_{k+1} - C-_{k+1}) A_k^T.
-__device__ __forceinline__ void load_record(const FitParams& P, int l, long long i, double xp[6],
-                                            double Cp[21], double Fa[4][5], double Ft[5], double& g) {
-  const double* __restrict__ R = P.rec + (size_t)l * kRecDoubles * P.Np + i;
-  const long long Np = P.Np;
-#pragma unroll
-  for (int k = 0; k < 6; ++k) xp[k] = R[(kRecXp + k) * Np];
-#pragma unroll
-  for (int k = 0; k < 21; ++k) Cp[k] = R[(kRecCp + k) * Np];
-#pragma unroll
-  for (int a = 0; a < 4; ++a)
-#pragma unroll
-    for (int c = 0; c < 5; ++c) Fa[a][c] = R[(kRecFa + a * 5 + c) * Np];
-#pragma unroll
-  for (int c = 0; c < 5; ++c) Ft[c] = R[(kRecFt + c) * Np];
-  g = R[kRecG * Np];
+//
+// One CTA = one tile of KF_TILE tracks.  The tile's records are contiguous per leg (kLegBytes), so
+// one bulk async copy (TMA, cp.async.bulk) per leg brings a record into shared memory while the
+// threads compute; two stages hold records k and k+1, and the stage of record k+1 is re-armed with
+// record k-1 as soon as every thread has consumed it (before the solves and the triple product).
+// Threads read their own column (stride KF_TILE doubles: conflict-free), each value exactly once.
+
+__device__ __forceinline__ unsigned smem_u32(const void* p) {
+  return static_cast<unsigned>(__cvta_generic_to_shared(p));
+}
+__device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
+  asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
+}
+__device__ __forceinline__ void mbar_expect_tx(unsigned long long* bar, unsigned bytes) {
+  asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes)
+               : "memory");
+}
+__device__ __forceinline__ void mbar_wait(unsigned long long* bar, unsigned parity) {
+  asm volatile(
+      "{\n"
+      ".reg .pred p;\n"
+      "KF_WAIT_%=:\n"
+      "mbarrier.try_wait.parity.shared::cta.b64 p, [%0], %1;\n"
+      "@p bra KF_DONE_%=;\n"
+      "bra KF_WAIT_%=;\n"
+      "KF_DONE_%=:\n"
+      "}\n" ::"r"(smem_u32(bar)), "r"(parity)
+      : "memory");
+}
+__device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, unsigned bytes,
+                                          unsigned long long* bar) {
+  asm volatile(
+      "cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+          smem_u32(smem_dst)),
+      "l"(gmem_src), "r"(bytes), "r"(smem_u32(bar))
+      : "memory");
 }
 
-// filtered state of leg l, recomputed from its record and hit exactly as the forward pass did
-__device__ __forceinline__ void refilter(const FitParams& P, const double* __restrict__ G, int l,
-                                         long long i, int& hp, const double xp[6], const double Cp[21],
-                                         double xf[6], double Cf[21]) {
-  const unsigned char flag = P.legflag[(size_t)l * P.Np + i];
+// filtered state of a leg from its record column R (stride KF_TILE) exactly as the forward pass did
+__device__ __forceinline__ void refilter(const FitParams& P, const double* __restrict__ R, unsigned char flag,
+                                         int surface, int hp, double xf[6], double Cf[21]) {
+  double xp[6], Cp[21];
+#pragma unroll
+  for (int k = 0; k < 6; ++k) xp[k] = R[(kRecXp + k) * KF_TILE];
+#pragma unroll
+  for (int k = 0; k < 21; ++k) Cp[k] = R[(kRecCp + k) * KF_TILE];
   bool copied = true;
-  if (flag != 0) {  // the leg consumed hit hp
-    if (flag == 1) {
-      const double m0 = P.loc[hp], m1 = P.loc[P.M + hp];
-      double v00, v11, v01 = 0.0;
-      if (P.var) {
-        v00 = P.var[hp];
-        v11 = P.var[P.M + hp];
-        if (P.cov01) v01 = P.cov01[hp];
-      } else {
-        const double* st = G + (P.start + 1 + l) * 20;
-        v00 = st[16];
-        v11 = st[17];
-      }
-      double c2;
-      copied = !gain_update(xp, Cp, m0, m1, v00, v01, v11, xf, Cf, c2);
+  if (flag == 1) {
+    const double m0 = R[kRecM * KF_TILE], m1 = R[(kRecM + 1) * KF_TILE];
+    double v00, v11, v01 = 0.0;
+    if (P.var) {
+      v00 = P.var[hp];
+      v11 = P.var[P.M + hp];
+      if (P.cov01) v01 = P.cov01[hp];
+    } else {
+      v00 = __ldg(P.geom + surface * 20 + 16);
+      v11 = __ldg(P.geom + surface * 20 + 17);
     }
-    hp--;
+    Gain gn;
+    double c2;
+    if (gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
+      gain_apply(gn, xp, Cp, xf, Cf);
+      copied = false;
+    }
   }
   if (copied) {
 #pragma unroll
@@ -331,61 +363,101 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* __res
   }
 }
 
-__global__ void __launch_bounds__(KF_RTS_BLOCK, KF_RTS_MIN_BLOCKS)
+__global__ void __launch_bounds__(KF_TILE, KF_RTS_MIN_BLOCKS)
 kf_rts_kernel(const __grid_constant__ FitParams P) {
-  extern __shared__ double s_dyn[];
-  const double* __restrict__ G = stage_geometry(P, s_dyn);
-  const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (i >= P.N) return;
+  extern __shared__ __align__(128) unsigned char s_raw[];
+  unsigned char* stage[2] = {s_raw, s_raw + kLegBytes};
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_raw + 2 * kLegBytes);
+  __shared__ int s_nmax;
+  const int tid = threadIdx.x;
+  const long long i = (long long)blockIdx.x * KF_TILE + tid;
   const long long N = P.N;
-  const int nleg = P.nleg[i];
-  if (nleg <= 0) return;  // first_* already holds the start state
+  const bool in_range = i < N;
+  const int nleg = in_range ? P.nleg[i] : 0;
+  if (tid == 0) {
+    s_nmax = 0;
+    mbar_init(&bar[0], 1);
+    mbar_init(&bar[1], 1);
+    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  }
+  __syncthreads();
+  if (nleg > 0) atomicMax(&s_nmax, nleg);
+  __syncthreads();
+  const int n = s_nmax;
+  if (n <= 0) return;  // no track of the tile completed a leg: first_* already holds the start state
 
-  // last hit consumed by the forward pass (it may have stopped early)
-  const int o0 = P.offsets[i];
-  int hp = P.offsets[i + 1] - 1;
-  while (hp >= o0 && P.surf_idx[hp] > P.start + nleg) hp--;
+  const char* __restrict__ tile_base = P.rec + (size_t)blockIdx.x * P.tile_stride;
+  if (tid == 0) {
+    mbar_expect_tx(&bar[(n - 1) & 1], (unsigned)kLegBytes);
+    bulk_load(stage[(n - 1) & 1], tile_base + (size_t)(n - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[(n - 1) & 1]);
+    if (n >= 2) {
+      mbar_expect_tx(&bar[(n - 2) & 1], (unsigned)kLegBytes);
+      bulk_load(stage[(n - 2) & 1], tile_base + (size_t)(n - 2) * P.leg_stride, (unsigned)kLegBytes, &bar[(n - 2) & 1]);
+    }
+  }
 
-  double xp1[6], Cp1[21], Fa1[4][5], Ft1[5], g1;
+  // per-hit variances (optional input) are looked up by hit index: start from the last consumed hit
+  int hp = 0;
+  if (P.var && nleg > 0) {
+    const int o0 = P.offsets[i];
+    hp = P.offsets[i + 1] - 1;
+    while (hp >= o0 && P.surf_idx[hp] > P.start + nleg) hp--;
+  }
+
   double xs[6], Cs[21];
-  load_record(P, nleg - 1, i, xp1, Cp1, Fa1, Ft1, g1);
-  refilter(P, G, nleg - 1, i, hp, xp1, Cp1, xs, Cs);  // x^s_n = x+_n
-  if (P.output_states & OUT_SMOOTH) {
-    store6(P.state_params[2] + (size_t)(nleg - 1) * 6 * N, N, i, xs);
-    store21(P.state_cov[2] + (size_t)(nleg - 1) * 21 * N, N, i, Cs);
-  }
   bool failed = false;
-  for (int k = nleg - 2; k >= 0; --k) {
-    double xpk[6], Cpk[21], Fak[4][5], Ftk[5], gk;
-    load_record(P, k, i, xpk, Cpk, Fak, Ftk, gk);
+  unsigned phase = 0u;
+  for (int k = n - 1; k >= 0; --k) {
+    const int sc = k & 1, sn = sc ^ 1;
+    mbar_wait(&bar[sc], (phase >> sc) & 1u);
+    phase ^= 1u << sc;
+    const bool active = k < nleg;
+    const bool top = k == nleg - 1;
+    const double* __restrict__ Rc = reinterpret_cast<const double*>(stage[sc]) + tid;
+    const double* __restrict__ Rn = reinterpret_cast<const double*>(stage[sn]) + tid;
     double xf[6], Cf[21];
-    refilter(P, G, k, i, hp, xpk, Cpk, xf, Cf);
-    if (!failed) failed = !rts_step(xf, Cf, Fa1, Ft1, g1, xp1, Cp1, xs, Cs);
-    if (failed) {  // fall back to the filtered states for the remaining surfaces
-#pragma unroll
-      for (int c = 0; c < 6; ++c) xs[c] = xf[c];
-#pragma unroll
-      for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
+    double W[6][6], L[21], inv[6], dx[6];
+    bool ok = true;
+    if (active) {
+      const unsigned char flag = stage[sc][(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
+      refilter(P, Rc, flag, P.start + 1 + k, hp, xf, Cf);
+      if (flag != 0) hp--;
+      if (!top) ok = rts_gain_head<KF_TILE>(Rn, xf, Cf, xs, Cs, W, L, inv, dx, kRecXp, kRecCp, kRecFa, kRecFt, kRecG);
     }
-    if (P.output_states & OUT_SMOOTH) {
-      store6(P.state_params[2] + (size_t)k * 6 * N, N, i, xs);
-      store21(P.state_cov[2] + (size_t)k * 21 * N, N, i, Cs);
+    if (k < n - 1) {
+      __syncthreads();  // every thread has consumed record k+1: re-arm its stage with record k-1
+      if (tid == 0 && k >= 1) {
+        mbar_expect_tx(&bar[sn], (unsigned)kLegBytes);
+        bulk_load(stage[sn], tile_base + (size_t)(k - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[sn]);
+      }
     }
+    if (active) {
+      if (top) {
 #pragma unroll
-    for (int c = 0; c < 6; ++c) xp1[c] = xpk[c];
+        for (int c = 0; c < 6; ++c) xs[c] = xf[c];
 #pragma unroll
-    for (int c = 0; c < 21; ++c) Cp1[c] = Cpk[c];
+        for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
+      } else {
+        if (!failed && ok) ok = rts_gain_tail(xf, Cf, W, L, inv, dx, xs, Cs);
+        if (failed || !ok) {  // fall back to the filtered states for the remaining surfaces (U25)
+          failed = true;
 #pragma unroll
-    for (int a = 0; a < 4; ++a)
+          for (int c = 0; c < 6; ++c) xs[c] = xf[c];
 #pragma unroll
-      for (int c = 0; c < 5; ++c) Fa1[a][c] = Fak[a][c];
-#pragma unroll
-    for (int c = 0; c < 5; ++c) Ft1[c] = Ftk[c];
-    g1 = gk;
+          for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
+        }
+      }
+      if (P.output_states & OUT_SMOOTH) {
+        store6(P.state_params[2] + (size_t)k * 6 * N, N, i, xs);
+        store21(P.state_cov[2] + (size_t)k * 21 * N, N, i, Cs);
+      }
+    }
   }
-  store6(P.first_params, N, i, xs);
-  store21(P.first_cov, N, i, Cs);
-  if (failed) P.status[i] |= ST_NOT_POSITIVE;
+  if (nleg > 0) {
+    store6(P.first_params, N, i, xs);
+    store21(P.first_cov, N, i, Cs);
+    if (failed) P.status[i] |= ST_NOT_POSITIVE;
+  }
 }
 
 // ---- sustained FP64 FMA throughput probe (roofline denominator; not part of the fit) -----------------

@@ -54,17 +54,18 @@ def test_defaults_and_version():
 
 def test_workspace_bytes():
     o = B.default_options()
-    # records: Lmax * 53 doubles * Np, flags Lmax * Np bytes, nleg Np int32, each rounded to 256 B
+    # tile-major records: tiles * Lmax * (55 doubles + 1 flag byte) * TILE, then nleg int32 per slot,
+    # each block rounded to 256 B (include/kf_fit.h "workspace")
     n, L = 1000, 6
-    Np = 1024
+    tiles = (n + B.TILE - 1) // B.TILE
     up = lambda v: (v + 255) // 256 * 256
-    assert B.workspace_bytes(n, L, o) == up(L * 53 * Np * 8) + up(L * Np) + up(Np * 4)
+    assert B.workspace_bytes(n, L, o) == up(tiles * L * (B.REC_DOUBLES * 8 + 1) * B.TILE) + up(tiles * B.TILE * 4)
     o.smooth = 0
     assert B.workspace_bytes(n, L, o) == 0
     o.smooth = 1
     assert B.workspace_bytes(0, L, o) == 0
     # 1e6 tracks x 30 legs fits comfortably in 180 GB
-    assert B.workspace_bytes(1_000_000, 30, o) < 13e9
+    assert B.workspace_bytes(1_000_000, 30, o) < 14e9
 
 
 def _dummy_call(**over):
