@@ -44,6 +44,12 @@ HIT_BYTES = 2 * 8 + 4
 FWD_FLOP_PER_LEG = {"const": 3300.0, "grid3": 3900.0}   # + material
 RTS_FLOP_PER_LEG = 1900.0
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x clock)
+# DRAM traffic per leg measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one launch
+# over 262,144 tracks x 30 legs of this workload, divided by the legs), from the committed capture below.
+# bench.py scales it to the launch it times; it is not re-measured live (never time under a profiler).
+NCU_TRAFFIC = dict(source="profiles/r01b_ncu_summary.md",
+                   bytes_per_leg={"kf_forward_kernel": (0.381929e9 + 3.617632e9) / 7864320,
+                                  "kf_rts_kernel": (3.470334e9 + 0.093517e9) / 7864320})
 
 
 def parse_args():
@@ -120,15 +126,12 @@ class ClockSampler:
 
 def dist_setup(n_gpus):
     """-> (rank, world, dist or None). Under torchrun the env carries RANK/WORLD_SIZE/LOCAL_RANK."""
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
+    from paper_2105_01796_b200 import replicas
+    rank, local, world = replicas.rank_world()
     if world > 1:
         import torch
-        import torch.distributed as dist
-        os.environ.setdefault("MASTER_ADDR", "127.0.0.1")
-        torch.cuda.set_device(int(os.environ.get("LOCAL_RANK", rank)))
-        dist.init_process_group("nccl")
-        return rank, world, dist
+        torch.cuda.set_device(local)
+        return rank, world, replicas.init("nccl")
     return 0, 1, None
 
 
@@ -184,6 +187,7 @@ def main():
     import torch
     import paper_2105_01796_b200 as kf
     from paper_2105_01796_b200 import binding as B
+    from paper_2105_01796_b200 import replicas
     from paper_2105_01796_b200 import workloads as W
 
     if not torch.cuda.is_available():
@@ -228,13 +232,8 @@ def main():
     t_wall1 = time.time()
     fwd_ms, rts_ms = timer.finish()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    ms_total = e0.elapsed_time(e1)
-    if dist is not None:
-        t = torch.tensor([ms_total], device=dev, dtype=torch.float64)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        ms_total = float(t.item())
+    value, ms_total, n_job = replicas.job_throughput(N * args.steps, e0.elapsed_time(e1), dist, dev)
     ms_step = ms_total / args.steps
-    value = world * N / (ms_step * 1e-3)
     launches = call.launches * args.steps
 
     # results of the last step, for the legs count and a sanity line
@@ -256,11 +255,7 @@ def main():
             hc.run()
         h1.record()
         barrier()
-        ms_e2e = h0.elapsed_time(h1) / ke
-        if dist is not None:
-            t = torch.tensor([ms_e2e], device=dev, dtype=torch.float64)
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            ms_e2e = float(t.item())
+        ms_e2e = replicas.max_over_ranks(h0.elapsed_time(h1), dist, dev) / ke
         e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
                    d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke,
                    api="kf_fit_batch_host (pinned host buffers; H2D, forward, RTS, D2H on one stream)")
@@ -302,6 +297,11 @@ def main():
     else:
         roofline = dict(bound="hbm", achieved=dom["hbm_gbs"], peak=hbm_peak, unit="GB/s", frac=dom["hbm_frac"],
                         traffic=None, kernel=dom["kernel"], peak_source=f"MEASURED_PEAKS.json ({peaks['source']})")
+    if args.config == 2 and smooth:  # the capture is of this workload; other configs report null
+        roofline["traffic"] = NCU_TRAFFIC["bytes_per_leg"][dom["kernel"]] * n_legs
+        roofline["traffic_unit"] = "bytes per launch (ncu dram read+write per leg x legs of this launch)"
+        roofline["traffic_source"] = NCU_TRAFFIC["source"]
+        roofline["algorithmic_bytes"] = fwd_bytes if dom["kernel"] == "kf_forward_kernel" else rts_bytes
     roofline["ms_per_launch"] = dom["ms"]
     roofline["share_of_step"] = dom["ms"] / ms_step
 
