@@ -518,8 +518,23 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
   const double dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
   xo[0] = dot(ut, dr);
   xo[1] = dot(vt, dr);
-  xo[2] = atan2(T[1], T[0]);
-  xo[3] = acos(fmin(fmax(T[2], -1.0), 1.0));
+  // phi' = atan2(Ty, Tx) and theta' = acos(Tz), taken as the input angle plus the rotation over the leg
+  // (sin of the difference from the two direction vectors) whenever that rotation is small
+  {
+    const double sdp = fma(sph2, cphi, -cph2 * sphi), cdp = fma(cph2, cphi, sph2 * sphi);
+    const double sdt = fma(sth2, cth, -cth2 * sth), cdt = fma(cth2, cth, sth2 * sth);
+    if (fabs(sdp) <= kSmallSine && cdp > 0.0 && fabs(sdt) <= kSmallSine && cdt > 0.0 && fabs(x[2]) <= kPi &&
+        x[3] > 0.0 && x[3] < kPi) {
+      double ph = x[2] + asin_small(sdp);
+      if (ph > kPi) ph -= 2.0 * kPi;
+      else if (ph <= -kPi) ph += 2.0 * kPi;
+      xo[2] = ph;
+      xo[3] = x[3] + asin_small(sdt);
+    } else {
+      xo[2] = atan2(T[1], T[0]);
+      xo[3] = acos(fmin(fmax(T[2], -1.0), 1.0));
+    }
+  }
   xo[4] = lam;
   xo[5] = t;
   trig[0] = sph2; trig[1] = cph2; trig[2] = sth2; trig[3] = cth2;

@@ -121,13 +121,22 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   {
     bool ok = true;
     int prev_s = P.start;
-    for (int j = o0; j < o1; ++j) {
-      const int s = P.surf_idx[j];
-      if (!(s > prev_s && s < P.n_surfaces)) { ok = false; break; }
+#pragma unroll 4
+    for (int j = o0; j < o1; ++j) {  // no early exit: the loads of a track's list stay independent
+      const int s = __ldg(P.surf_idx + j);
+      ok = ok && (s > prev_s) && (s < P.n_surfaces);
       prev_s = s;
     }
     if (!ok) status |= ST_BAD_HITS;
     else n_target = prev_s - P.start;  // visit every surface up to the one of the last hit (U7)
+  }
+  // the next unconsumed hit is held in registers one leg ahead of its use
+  int hit_s = -1;
+  double hit_m0 = 0.0, hit_m1 = 0.0;
+  if (o0 < o1) {
+    hit_s = __ldg(P.surf_idx + o0);
+    hit_m0 = __ldg(P.loc + o0);
+    hit_m1 = __ldg(P.loc + P.M + o0);
   }
 
   double chi2 = 0.0, errmax = 0.0;
@@ -169,10 +178,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     double Cp[21];
     transport_covariance(J, C, Cp);
 
-    // hit of this surface, if any
-    const bool has_hit = (hp < o1) && (P.surf_idx[hp] == s);
-    double m0 = 0.0, m1 = 0.0;
-    if (has_hit) { m0 = P.loc[hp]; m1 = P.loc[P.M + hp]; }
+    // hit of this surface, if any (prefetched)
+    const bool has_hit = hit_s == s;
+    const double m0 = has_hit ? hit_m0 : 0.0, m1 = has_hit ? hit_m1 : 0.0;
 
     // RTS record: x-, C-, F = J G_prev, g_prev, hit ("stored Jacobians")
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
@@ -195,9 +203,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       R[(kRecM + 1) * KF_TILE] = m1;
     }
 
-    // gain-matrix update with the surface's hit, or hole
+    // gain-matrix update with the surface's hit.  A hole or a flagged outlier runs the
+    // same arithmetic with a zero gain (x+ = x-, C+ = C- exactly), so the leg has one code path.
     unsigned char flag = 0;
-    bool updated = false;
+    Gain gn;
+    gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
     if (has_hit) {
       double v00, v11, v01 = 0.0;
       if (P.var) {
@@ -208,7 +218,6 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
         v00 = st[16];
         v11 = st[17];
       }
-      Gain gn;
       double c2 = 0.0;
       if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
         status |= ST_NOT_POSITIVE;
@@ -219,9 +228,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       if (P.outlier_chi2 > 0.0 && c2 > P.outlier_chi2) {  // strictly greater: flagged, not used (U9)
         n_outl++;
         flag = 2;
+        gn.i00 = gn.i01 = gn.i11 = 0.0;
       } else {
-        gain_apply(gn, xp, Cp, x, C);
-        updated = true;
         chi2 += c2;
         n_used++;
         flag = 1;
@@ -229,18 +237,19 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       if (P.hit_chi2) P.hit_chi2[hp] = c2;
       if (P.hit_flags) P.hit_flags[hp] = flag;
       hp++;
+      hit_s = -1;
+      if (hp < o1) {  // fetch the next hit now: it is used after the next propagation
+        hit_s = __ldg(P.surf_idx + hp);
+        hit_m0 = __ldg(P.loc + hp);
+        hit_m1 = __ldg(P.loc + P.M + hp);
+      }
     } else {
       n_holes++;
     }
-    if (updated) {
-      sincos(x[2], &trig[0], &trig[1]);
-      sincos(x[3], &trig[2], &trig[3]);
-    } else {  // hole or outlier: the filtered state is the predicted one (trig already holds its angles)
-#pragma unroll
-      for (int k = 0; k < 6; ++k) x[k] = xp[k];
-#pragma unroll
-      for (int k = 0; k < 21; ++k) C[k] = Cp[k];
-    }
+    gain_apply(gn, xp, Cp, x, C);
+    // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
+    rotate_sincos(trig[0], trig[1], x[2], x[2] - xp[2]);
+    rotate_sincos(trig[2], trig[3], x[3], x[3] - xp[3]);
     if (P.smooth) tile_flag[(size_t)l * P.leg_stride] = flag;
     if (P.output_states & OUT_PRED) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
