@@ -698,122 +698,4 @@ __device__ __forceinline__ void material_undo(const MaterialStep& S, double C[21
   C[IX(4, 4)] *= ig * ig;
 }
 
-// ---- one RTS step (A.7), in two halves ---------------------------------------------------
-// R1 = this thread's column of record k+1 in shared memory (stride RS doubles): F = J G stored as
-// Fa[4][5], Ft[5] (column qp already scaled by g) and g, then x-_{k+1}, C-_{k+1}.
-// Head: everything that reads the record -- W = C+ F^T, Cholesky C-_{k+1} = L L^T (no pivoting; L[i][j],
-// i >= j, kept at packed (j, i); inv = 1/diag), dC = C^s_{k+1} - C-_{k+1} (in place in Cs),
-// dx = x^s_{k+1} - x-_{k+1} with the phi difference wrapped into (-pi, pi].  False on a non-positive pivot.
-template <int RS>
-__device__ __forceinline__ bool rts_gain_head(const double* __restrict__ R1, const double xf[6],
-                                              const double Cf[21], const double xs[6], double Cs[21],
-                                              double W[6][6], double L[21], double inv[6], double dx[6],
-                                              int oXp, int oCp, int oFa, int oFt, int oG) {
-  {
-    double Fa[4][5], Ft[5];
-#pragma unroll
-    for (int a = 0; a < 4; ++a)
-#pragma unroll
-      for (int c = 0; c < 5; ++c) Fa[a][c] = R1[(oFa + a * 5 + c) * RS];
-#pragma unroll
-    for (int c = 0; c < 5; ++c) Ft[c] = R1[(oFt + c) * RS];
-    const double g = R1[oG * RS];
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-#pragma unroll
-      for (int j = 0; j < 4; ++j) {
-        double s = Cf[SX(i, 0)] * Fa[j][0];
-#pragma unroll
-        for (int k = 1; k < 5; ++k) s = fma(Cf[SX(i, k)], Fa[j][k], s);
-        W[i][j] = s;
-      }
-      W[i][4] = Cf[SX(i, 4)] * g;
-      double s = Cf[SX(i, 5)];
-#pragma unroll
-      for (int k = 0; k < 5; ++k) s = fma(Cf[SX(i, k)], Ft[k], s);
-      W[i][5] = s;
-    }
-  }
-  bool ok = true;
-  {
-    double Cp1[21];
-#pragma unroll
-    for (int k = 0; k < 21; ++k) Cp1[k] = R1[(oCp + k) * RS];
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-      double s = Cp1[IX(j, j)];
-#pragma unroll
-      for (int k = 0; k < j; ++k) s = fma(-L[IX(k, j)], L[IX(k, j)], s);
-      if (!(s > 0.0)) { ok = false; s = 1.0; }
-      L[IX(j, j)] = sqrt_nr(s, inv[j]);
-#pragma unroll
-      for (int i = j + 1; i < 6; ++i) {
-        double u = Cp1[IX(j, i)];
-#pragma unroll
-        for (int k = 0; k < j; ++k) u = fma(-L[IX(k, i)], L[IX(k, j)], u);
-        L[IX(j, i)] = u * inv[j];
-      }
-    }
-#pragma unroll
-    for (int k = 0; k < 21; ++k) Cs[k] -= Cp1[k];
-  }
-#pragma unroll
-  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - R1[(oXp + j) * RS];
-  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
-  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
-  return ok;
-}
-
-// Tail: A = W (L L^T)^-1 row by row (in place), x^s_k = x+_k + A dx, C^s_k = C+_k + A dC A^T.
-// On entry Cs holds dC; on exit (xs, Cs) is the smoothed state at k.  False if the result is not finite.
-__device__ __forceinline__ bool rts_gain_tail(const double xf[6], double Cf[21], double W[6][6],
-                                              const double L[21], const double inv[6], const double dx[6],
-                                              double xs[6], double Cs[21]) {
-#pragma unroll
-  for (int i = 0; i < 6; ++i) {
-#pragma unroll
-    for (int r = 0; r < 6; ++r) {  // L y = w
-      double s = W[i][r];
-#pragma unroll
-      for (int k = 0; k < r; ++k) s = fma(-L[IX(k, r)], W[i][k], s);
-      W[i][r] = s * inv[r];
-    }
-#pragma unroll
-    for (int r = 5; r >= 0; --r) {  // L^T a = y
-      double s = W[i][r];
-#pragma unroll
-      for (int k = r + 1; k < 6; ++k) s = fma(-L[IX(r, k)], W[i][k], s);
-      W[i][r] = s * inv[r];
-    }
-  }
-  double chk = 0.0;
-#pragma unroll
-  for (int i = 0; i < 6; ++i) {
-    double s = xf[i];
-#pragma unroll
-    for (int j = 0; j < 6; ++j) s = fma(W[i][j], dx[j], s);
-    xs[i] = s;
-    chk += s;
-    double AdC[6];
-#pragma unroll
-    for (int j = 0; j < 6; ++j) {
-      double u = W[i][0] * Cs[SX(0, j)];
-#pragma unroll
-      for (int k = 1; k < 6; ++k) u = fma(W[i][k], Cs[SX(k, j)], u);
-      AdC[j] = u;
-    }
-#pragma unroll
-    for (int j = i; j < 6; ++j) {
-      double u = Cf[IX(i, j)];
-#pragma unroll
-      for (int k = 0; k < 6; ++k) u = fma(AdC[k], W[j][k], u);
-      Cf[IX(i, j)] = u;  // each C+ entry is consumed exactly here: reuse its register
-      chk += u;
-    }
-  }
-#pragma unroll
-  for (int k = 0; k < 21; ++k) Cs[k] = Cf[k];
-  return fabs(chk) < 1.0e300;
-}
-
 }  // namespace kf

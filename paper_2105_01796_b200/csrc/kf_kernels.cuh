@@ -337,17 +337,28 @@ __device__ __forceinline__ void bulk_load(void* smem_dst, const void* gmem_src, 
       : "memory");
 }
 
-// filtered state of a leg from its record column R (stride KF_TILE) exactly as the forward pass did
-__device__ __forceinline__ void refilter(const FitParams& P, const double* __restrict__ R, unsigned char flag,
-                                         int surface, int hp, double xf[6], double Cf[21]) {
+__device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
+}
+
+constexpr int kStageDoubles = (int)(kLegBytes / sizeof(double));
+static_assert(kLegBytes % 16 == 0, "a tile-leg must be a whole number of 16-byte units (bulk copy)");
+// record column of one thread inside a stage: component c at R[c * KF_TILE]
+#define KF_R(R, c) (R)[(c) * KF_TILE]
+
+// filtered state of a leg from its record column R exactly as the forward pass computed it:
+// the same gain routine on (x-, C-, hit); a hole or flagged outlier has x+ = x-, C+ = C-.
+__device__ __forceinline__ void refilter(const FitParams& P, const double* R, unsigned char flag, int surface,
+                                         int hp, double xf[6], double Cf[21]) {
   double xp[6], Cp[21];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) xp[k] = R[(kRecXp + k) * KF_TILE];
+  for (int k = 0; k < 6; ++k) xp[k] = KF_R(R, kRecXp + k);
 #pragma unroll
-  for (int k = 0; k < 21; ++k) Cp[k] = R[(kRecCp + k) * KF_TILE];
-  bool copied = true;
+  for (int k = 0; k < 21; ++k) Cp[k] = KF_R(R, kRecCp + k);
+  Gain gn;
+  gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
   if (flag == 1) {
-    const double m0 = R[kRecM * KF_TILE], m1 = R[(kRecM + 1) * KF_TILE];
+    const double m0 = KF_R(R, kRecM), m1 = KF_R(R, kRecM + 1);
     double v00, v11, v01 = 0.0;
     if (P.var) {
       v00 = P.var[hp];
@@ -357,26 +368,138 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* __res
       v00 = __ldg(P.geom + surface * 20 + 16);
       v11 = __ldg(P.geom + surface * 20 + 17);
     }
-    Gain gn;
     double c2;
-    if (gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
-      gain_apply(gn, xp, Cp, xf, Cf);
-      copied = false;
+    if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) gn.i00 = gn.i01 = gn.i11 = 0.0;
+  }
+  gain_apply(gn, xp, Cp, xf, Cf);
+}
+
+// One RTS step (DESIGN.md A.7).  In: (xf, Cf) = filtered state at k, (xs, Cs) = smoothed state at k+1,
+// R1 = this thread's column of record k+1 in shared memory (x-, C-, F = J G, g).  Out: (xs, Cs) =
+// smoothed state at k.  The record column is dead after its single read, so it doubles as scratch:
+// C+ goes to the F slots and dC = C^s - C- to the C- slots while the 6x6 solve owns the registers.
+// Returns false (xs, Cs untouched apart from being overwritten by the caller) on a non-positive
+// Cholesky pivot or a non-finite result.
+__device__ __forceinline__ bool rts_step(double* R1, const double xf[6], const double Cf[21], double xs[6],
+                                         double Cs[21]) {
+  // W = C+ F^T, streaming F (rows loc0, loc1, phi, theta over columns loc0..qp; row t; row qp = g e_qp)
+  double W[6][6];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    double f[5];
+#pragma unroll
+    for (int c = 0; c < 5; ++c) f[c] = KF_R(R1, kRecFa + j * 5 + c);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      double s = Cf[SX(i, 0)] * f[0];
+#pragma unroll
+      for (int c = 1; c < 5; ++c) s = fma(Cf[SX(i, c)], f[c], s);
+      W[i][j] = s;
     }
   }
-  if (copied) {
+  {
+    double f[5];
 #pragma unroll
-    for (int k = 0; k < 6; ++k) xf[k] = xp[k];
+    for (int c = 0; c < 5; ++c) f[c] = KF_R(R1, kRecFt + c);
+    const double g = KF_R(R1, kRecG);
 #pragma unroll
-    for (int k = 0; k < 21; ++k) Cf[k] = Cp[k];
+    for (int i = 0; i < 6; ++i) {
+      W[i][4] = Cf[SX(i, 4)] * g;
+      double s = Cf[SX(i, 5)];
+#pragma unroll
+      for (int c = 0; c < 5; ++c) s = fma(Cf[SX(i, c)], f[c], s);
+      W[i][5] = s;
+    }
   }
+  // C+ -> scratch (the F slots are consumed)
+#pragma unroll
+  for (int c = 0; c < 21; ++c) KF_R(R1, kRecFa + c) = Cf[c];
+
+  // dC = C^s_{k+1} - C-_{k+1} -> scratch; Cholesky C-_{k+1} = L L^T without pivoting (scale-invariant),
+  // L[i][j] (i >= j) kept at packed (j, i), inv = 1 / diag
+  double L[21], inv[6];
+  bool ok = true;
+#pragma unroll
+  for (int c = 0; c < 21; ++c) {
+    L[c] = KF_R(R1, kRecCp + c);
+    KF_R(R1, kRecCp + c) = Cs[c] - L[c];
+  }
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    double s = L[IX(j, j)];
+#pragma unroll
+    for (int k = 0; k < j; ++k) s = fma(-L[IX(k, j)], L[IX(k, j)], s);
+    if (!(s > 0.0)) { ok = false; s = 1.0; }
+    L[IX(j, j)] = sqrt_nr(s, inv[j]);
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i) {
+      double u = L[IX(j, i)];
+#pragma unroll
+      for (int k = 0; k < j; ++k) u = fma(-L[IX(k, i)], L[IX(k, j)], u);
+      L[IX(j, i)] = u * inv[j];
+    }
+  }
+  // dx = x^s_{k+1} - x-_{k+1}, phi difference wrapped into (-pi, pi]
+  double dx[6];
+#pragma unroll
+  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - KF_R(R1, kRecXp + j);
+  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
+  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+
+  // A = W (L L^T)^-1 row by row in place, x^s_k = x+_k + A dx
+  double chk = 0.0;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+#pragma unroll
+    for (int r = 0; r < 6; ++r) {  // L y = w
+      double s = W[i][r];
+#pragma unroll
+      for (int k = 0; k < r; ++k) s = fma(-L[IX(k, r)], W[i][k], s);
+      W[i][r] = s * inv[r];
+    }
+#pragma unroll
+    for (int r = 5; r >= 0; --r) {  // L^T a = y
+      double s = W[i][r];
+#pragma unroll
+      for (int k = r + 1; k < 6; ++k) s = fma(-L[IX(r, k)], W[i][k], s);
+      W[i][r] = s * inv[r];
+    }
+    double s = xf[i];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) s = fma(W[i][j], dx[j], s);
+    xs[i] = s;
+    chk += s;
+  }
+  // C^s_k = C+_k + A dC A^T  (dC and C+ back from scratch)
+  double dC[21];
+#pragma unroll
+  for (int c = 0; c < 21; ++c) dC[c] = KF_R(R1, kRecCp + c);
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    double T[6];
+#pragma unroll
+    for (int j = 0; j < 6; ++j) {
+      double u = W[i][0] * dC[SX(0, j)];
+#pragma unroll
+      for (int k = 1; k < 6; ++k) u = fma(W[i][k], dC[SX(k, j)], u);
+      T[j] = u;
+    }
+#pragma unroll
+    for (int j = i; j < 6; ++j) {
+      double u = KF_R(R1, kRecFa + IX(i, j));
+#pragma unroll
+      for (int k = 0; k < 6; ++k) u = fma(T[k], W[j][k], u);
+      Cs[IX(i, j)] = u;
+      chk += u;
+    }
+  }
+  return ok && fabs(chk) < 1.0e300;
 }
 
 __global__ void __launch_bounds__(KF_TILE, KF_RTS_MIN_BLOCKS)
 kf_rts_kernel(const __grid_constant__ FitParams P) {
-  extern __shared__ __align__(128) unsigned char s_raw[];
-  unsigned char* stage[2] = {s_raw, s_raw + kLegBytes};
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_raw + 2 * kLegBytes);
+  extern __shared__ __align__(128) double s_rec[];  // two stages of kStageDoubles, then two mbarriers
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_rec + 2 * kStageDoubles);
   __shared__ int s_nmax;
   const int tid = threadIdx.x;
   const long long i = (long long)blockIdx.x * KF_TILE + tid;
@@ -398,10 +521,12 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
   const char* __restrict__ tile_base = P.rec + (size_t)blockIdx.x * P.tile_stride;
   if (tid == 0) {
     mbar_expect_tx(&bar[(n - 1) & 1], (unsigned)kLegBytes);
-    bulk_load(stage[(n - 1) & 1], tile_base + (size_t)(n - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[(n - 1) & 1]);
+    bulk_load(s_rec + ((n - 1) & 1) * kStageDoubles, tile_base + (size_t)(n - 1) * P.leg_stride, (unsigned)kLegBytes,
+              &bar[(n - 1) & 1]);
     if (n >= 2) {
       mbar_expect_tx(&bar[(n - 2) & 1], (unsigned)kLegBytes);
-      bulk_load(stage[(n - 2) & 1], tile_base + (size_t)(n - 2) * P.leg_stride, (unsigned)kLegBytes, &bar[(n - 2) & 1]);
+      bulk_load(s_rec + ((n - 2) & 1) * kStageDoubles, tile_base + (size_t)(n - 2) * P.leg_stride, (unsigned)kLegBytes,
+                &bar[(n - 2) & 1]);
     }
   }
 
@@ -418,47 +543,46 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
   unsigned phase = 0u;
   for (int k = n - 1; k >= 0; --k) {
     const int sc = k & 1, sn = sc ^ 1;
+    // record k-2 is fetched at the end of the next iteration: start it towards L2 now
+    if (tid == 0 && k >= 2) bulk_prefetch_l2(tile_base + (size_t)(k - 2) * P.leg_stride, (unsigned)kLegBytes);
     mbar_wait(&bar[sc], (phase >> sc) & 1u);
     phase ^= 1u << sc;
-    const bool active = k < nleg;
-    const bool top = k == nleg - 1;
-    const double* __restrict__ Rc = reinterpret_cast<const double*>(stage[sc]) + tid;
-    const double* __restrict__ Rn = reinterpret_cast<const double*>(stage[sn]) + tid;
-    double xf[6], Cf[21];
-    double W[6][6], L[21], inv[6], dx[6];
-    bool ok = true;
-    if (active) {
-      const unsigned char flag = stage[sc][(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
+    const double* Rc = s_rec + sc * kStageDoubles + tid;
+    double* Rn = s_rec + sn * kStageDoubles + tid;
+    if (k < nleg) {
+      const unsigned char flag =
+          reinterpret_cast<const unsigned char*>(s_rec + sc * kStageDoubles)[(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
+      double xf[6], Cf[21];
       refilter(P, Rc, flag, P.start + 1 + k, hp, xf, Cf);
       if (flag != 0) hp--;
-      if (!top) ok = rts_gain_head<KF_TILE>(Rn, xf, Cf, xs, Cs, W, L, inv, dx, kRecXp, kRecCp, kRecFa, kRecFt, kRecG);
-    }
-    if (k < n - 1) {
-      __syncthreads();  // every thread has consumed record k+1: re-arm its stage with record k-1
-      if (tid == 0 && k >= 1) {
-        mbar_expect_tx(&bar[sn], (unsigned)kLegBytes);
-        bulk_load(stage[sn], tile_base + (size_t)(k - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[sn]);
+      bool smoothed = false;
+      if (k < nleg - 1 && !failed) {
+        smoothed = rts_step(Rn, xf, Cf, xs, Cs);
+        if (!smoothed) {  // U25: this and all earlier surfaces fall back to the filtered states
+          failed = true;
+#pragma unroll
+          for (int c = 0; c < 21; ++c) Cf[c] = KF_R(Rn, kRecFa + c);
+        }
       }
-    }
-    if (active) {
-      if (top) {
+      if (!smoothed) {  // top of the track, or fallback
 #pragma unroll
         for (int c = 0; c < 6; ++c) xs[c] = xf[c];
 #pragma unroll
         for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
-      } else {
-        if (!failed && ok) ok = rts_gain_tail(xf, Cf, W, L, inv, dx, xs, Cs);
-        if (failed || !ok) {  // fall back to the filtered states for the remaining surfaces (U25)
-          failed = true;
-#pragma unroll
-          for (int c = 0; c < 6; ++c) xs[c] = xf[c];
-#pragma unroll
-          for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
-        }
       }
       if (P.output_states & OUT_SMOOTH) {
         store6(P.state_params[2] + (size_t)k * 6 * N, N, i, xs);
         store21(P.state_cov[2] + (size_t)k * 21 * N, N, i, Cs);
+      }
+    }
+    if (k < n - 1) {
+      // every thread is done with record k+1 and its scratch (generic-proxy writes ordered before the
+      // async-proxy write of the next bulk copy): fetch record k-1 into that stage
+      asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+      __syncthreads();
+      if (tid == 0 && k >= 1) {
+        mbar_expect_tx(&bar[sn], (unsigned)kLegBytes);
+        bulk_load(s_rec + sn * kStageDoubles, tile_base + (size_t)(k - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[sn]);
       }
     }
   }
