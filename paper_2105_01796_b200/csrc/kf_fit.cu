@@ -211,12 +211,21 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
   const bool grid3 = fl->kind == KF_FIELD_GRID3;
   record_stage(0, stream);
-  if (op->material) {
-    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, true>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel")
-               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, true>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel");
-  } else {
-    rc = grid3 ? launch(kf::kf_forward_kernel<kf::FIELD_GRID3, false>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel")
-               : launch(kf::kf_forward_kernel<kf::FIELD_CONST, false>, P, KF_TILE, fwd_smem, stream, "kf_forward_kernel");
+  {
+    using kf::FIELD_CONST;
+    using kf::FIELD_GRID3;
+    const int sel = (grid3 ? 4 : 0) | (op->material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
+    const char* nm = "kf_forward_kernel";
+    switch (sel) {
+      case 0: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, false>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 1: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, true>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 2: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, false>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 3: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, true>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 4: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, false>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 5: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, true>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 6: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, false>, P, KF_TILE, fwd_smem, stream, nm); break;
+      default: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, true>, P, KF_TILE, fwd_smem, stream, nm); break;
+    }
   }
   if (rc != KF_OK) return rc;
   record_stage(1, stream);

@@ -85,25 +85,31 @@ __device__ __forceinline__ void store21(double* base, long long stride, long lon
 }
 
 // stage the geometry table in shared memory once per CTA (5 KB for 31 planes)
-__device__ __forceinline__ const double* stage_geometry(const FitParams& P, double* smem) {
-  if (!P.geom_in_smem) return P.geom;
+__device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem) {
   const int n = P.n_surfaces * 20;
   for (int k = threadIdx.x; k < n; k += blockDim.x) smem[k] = P.geom[k];
   __syncthreads();
-  return smem;
 }
 
 
 // =====================================================================================================
-// Forward filter.  Dynamic shared memory: [geometry table if geom_in_smem].
+// Forward filter.  Dynamic shared memory: [geometry table if GEOM_SMEM].
 // Material is applied lazily, at the top of the next leg, so that on exit (x, C) is the filtered
 // state of the last completed leg before that layer's material (= last_*); the material step of the
 // last surface is still evaluated for its status bit (energy exhausted), as in DESIGN.md A.6.
-template <int FIELD, bool MATERIAL>
+// GEOM_SMEM: the geometry table is read from shared memory (shared-space loads, their own scoreboard)
+// or, for tables too large to stage, from global memory.
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM>
 __global__ void __launch_bounds__(KF_TILE, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   extern __shared__ double s_dyn[];
-  const double* __restrict__ G = stage_geometry(P, s_dyn);
+  const double* __restrict__ G;
+  if constexpr (GEOM_SMEM) {
+    stage_geometry(P, s_dyn);
+    G = s_dyn;
+  } else {
+    G = P.geom;
+  }
   const long long i = (long long)blockIdx.x * KF_TILE + threadIdx.x;
   if (i >= P.N) return;
   const long long N = P.N;
@@ -348,8 +354,8 @@ static_assert(kLegBytes % 16 == 0, "a tile-leg must be a whole number of 16-byte
 
 // filtered state of a leg from its record column R exactly as the forward pass computed it:
 // the same gain routine on (x-, C-, hit); a hole or flagged outlier has x+ = x-, C+ = C-.
-__device__ __forceinline__ void refilter(const FitParams& P, const double* R, unsigned char flag, int surface,
-                                         int hp, double xf[6], double Cf[21]) {
+__device__ __forceinline__ void refilter(const FitParams& P, const double* R, unsigned char flag, double gv0,
+                                         double gv1, int hp, double xf[6], double Cf[21]) {
   double xp[6], Cp[21];
 #pragma unroll
   for (int k = 0; k < 6; ++k) xp[k] = KF_R(R, kRecXp + k);
@@ -365,8 +371,8 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* R, un
       v11 = P.var[P.M + hp];
       if (P.cov01) v01 = P.cov01[hp];
     } else {
-      v00 = __ldg(P.geom + surface * 20 + 16);
-      v11 = __ldg(P.geom + surface * 20 + 17);
+      v00 = gv0;  // the surface's resolution (geometry table), fetched by the caller
+      v11 = gv1;
     }
     double c2;
     if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) gn.i00 = gn.i01 = gn.i11 = 0.0;
@@ -424,19 +430,24 @@ __device__ __forceinline__ bool rts_step(double* R1, const double xf[6], const d
     L[c] = KF_R(R1, kRecCp + c);
     KF_R(R1, kRecCp + c) = Cs[c] - L[c];
   }
+  // (fixed trip counts with compile-time guards: every index is a constant after unrolling)
 #pragma unroll
   for (int j = 0; j < 6; ++j) {
     double s = L[IX(j, j)];
 #pragma unroll
-    for (int k = 0; k < j; ++k) s = fma(-L[IX(k, j)], L[IX(k, j)], s);
+    for (int k = 0; k < 6; ++k)
+      if (k < j) s = fma(-L[SX(k, j)], L[SX(k, j)], s);
     if (!(s > 0.0)) { ok = false; s = 1.0; }
     L[IX(j, j)] = sqrt_nr(s, inv[j]);
 #pragma unroll
-    for (int i = j + 1; i < 6; ++i) {
-      double u = L[IX(j, i)];
+    for (int i = 0; i < 6; ++i) {
+      if (i > j) {
+        double u = L[SX(j, i)];
 #pragma unroll
-      for (int k = 0; k < j; ++k) u = fma(-L[IX(k, i)], L[IX(k, j)], u);
-      L[IX(j, i)] = u * inv[j];
+        for (int k = 0; k < 6; ++k)
+          if (k < j) u = fma(-L[SX(k, i)], L[SX(k, j)], u);
+        L[SX(j, i)] = u * inv[j];
+      }
     }
   }
   // dx = x^s_{k+1} - x-_{k+1}, phi difference wrapped into (-pi, pi]
@@ -545,6 +556,12 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
     const int sc = k & 1, sn = sc ^ 1;
     // record k-2 is fetched at the end of the next iteration: start it towards L2 now
     if (tid == 0 && k >= 2) bulk_prefetch_l2(tile_base + (size_t)(k - 2) * P.leg_stride, (unsigned)kLegBytes);
+    // the surface's measurement variances come from L2: ask for them before waiting on the record
+    double gv0 = 0.0, gv1 = 0.0;
+    if (!P.var) {
+      gv0 = __ldg(P.geom + (P.start + 1 + k) * 20 + 16);
+      gv1 = __ldg(P.geom + (P.start + 1 + k) * 20 + 17);
+    }
     mbar_wait(&bar[sc], (phase >> sc) & 1u);
     phase ^= 1u << sc;
     const double* Rc = s_rec + sc * kStageDoubles + tid;
@@ -553,7 +570,7 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
       const unsigned char flag =
           reinterpret_cast<const unsigned char*>(s_rec + sc * kStageDoubles)[(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
       double xf[6], Cf[21];
-      refilter(P, Rc, flag, P.start + 1 + k, hp, xf, Cf);
+      refilter(P, Rc, flag, gv0, gv1, hp, xf, Cf);
       if (flag != 0) hp--;
       bool smoothed = false;
       if (k < nleg - 1 && !failed) {
