@@ -84,6 +84,23 @@ __device__ __forceinline__ void store21(double* base, long long stride, long lon
   for (int k = 0; k < 21; ++k) base[k * stride + i] = v[k];
 }
 
+__device__ __forceinline__ unsigned smem_u32(const void* p) {
+  return static_cast<unsigned>(__cvta_generic_to_shared(p));
+}
+// per-thread asynchronous global -> shared copies (LDGSTS): completion is tracked by copy groups, not by
+// the register scoreboards, so a fetch in flight never holds up an unrelated load of the same thread
+__device__ __forceinline__ void cp_async4(void* smem_dst, const void* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 4;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* smem_dst, const void* gmem_src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(smem_u32(smem_dst)), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// bytes of the forward kernel's hit staging area: two alternating slots of (loc0, loc1, surface) per thread
+constexpr size_t kHitStageBytes = (size_t)KF_TILE * (2 * 2 * sizeof(double) + 2 * sizeof(int));
+
 // stage the geometry table in shared memory once per CTA (5 KB for 31 planes)
 __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem) {
   const int n = P.n_surfaces * 20;
@@ -93,7 +110,7 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 
 
 // =====================================================================================================
-// Forward filter.  Dynamic shared memory: [geometry table if GEOM_SMEM].
+// Forward filter.  Dynamic shared memory: [geometry table if GEOM_SMEM][hit staging, kHitStageBytes].
 // Material is applied lazily, at the top of the next leg, so that on exit (x, C) is the filtered
 // state of the last completed leg before that layer's material (= last_*); the material step of the
 // last surface is still evaluated for its status bit (energy exhausted), as in DESIGN.md A.6.
@@ -136,14 +153,18 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     if (!ok) status |= ST_BAD_HITS;
     else n_target = prev_s - P.start;  // visit every surface up to the one of the last hit (U7)
   }
-  // the next unconsumed hit is held in registers one leg ahead of its use
-  int hit_s = -1;
-  double hit_m0 = 0.0, hit_m1 = 0.0;
-  if (o0 < o1) {
-    hit_s = __ldg(P.surf_idx + o0);
-    hit_m0 = __ldg(P.loc + o0);
-    hit_m1 = __ldg(P.loc + P.M + o0);
-  }
+  // the next unconsumed hit is fetched one leg ahead of its use into this thread's own shared-memory
+  // slot (two alternating slots), asynchronously
+  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][KF_TILE]
+  int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * KF_TILE) + threadIdx.x;  // [slot][KF_TILE]
+  int slot = 0;
+  auto fetch_hit = [&](int j, int sl) {
+    cp_async4(s_hs + sl * KF_TILE, P.surf_idx + j);
+    cp_async8(s_hm + (sl * 2 + 0) * KF_TILE, P.loc + j);
+    cp_async8(s_hm + (sl * 2 + 1) * KF_TILE, P.loc + P.M + j);
+    cp_async_commit();
+  };
+  if (o0 < o1) fetch_hit(o0, 0);
 
   double chi2 = 0.0, errmax = 0.0;
   int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0, hp = o0;
@@ -184,9 +205,12 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     double Cp[21];
     transport_covariance(J, C, Cp);
 
-    // hit of this surface, if any (prefetched)
-    const bool has_hit = hit_s == s;
-    const double m0 = has_hit ? hit_m0 : 0.0, m1 = has_hit ? hit_m1 : 0.0;
+    // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
+    cp_async_wait_all();
+    const bool has_hit = hp < o1 && s_hs[slot * KF_TILE] == s;
+    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * KF_TILE] : 0.0;
+    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_TILE] : 0.0;
+    if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     // RTS record: x-, C-, F = J G_prev, g_prev, hit ("stored Jacobians")
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
@@ -243,12 +267,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       if (P.hit_chi2) P.hit_chi2[hp] = c2;
       if (P.hit_flags) P.hit_flags[hp] = flag;
       hp++;
-      hit_s = -1;
-      if (hp < o1) {  // fetch the next hit now: it is used after the next propagation
-        hit_s = __ldg(P.surf_idx + hp);
-        hit_m0 = __ldg(P.loc + hp);
-        hit_m1 = __ldg(P.loc + P.M + hp);
-      }
+      slot ^= 1;
     } else {
       n_holes++;
     }
@@ -312,9 +331,6 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 // record k-1 as soon as every thread has consumed it (before the solves and the triple product).
 // Threads read their own column (stride KF_TILE doubles: conflict-free), each value exactly once.
 
-__device__ __forceinline__ unsigned smem_u32(const void* p) {
-  return static_cast<unsigned>(__cvta_generic_to_shared(p));
-}
 __device__ __forceinline__ void mbar_init(unsigned long long* bar, unsigned count) {
   asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(smem_u32(bar)), "r"(count) : "memory");
 }
