@@ -241,7 +241,7 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
     r[i] = r[i] + h * T[i] + h26 * (k1[i] + k2[i] + k3[i]);
     Tn[i] = T[i] + h6 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
   }
-  const double inrm = rsqrt_nr(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
+  const double inrm = rsqrt_near_one(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
 #pragma unroll
   for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
   t += h * dtds;
@@ -305,7 +305,7 @@ __device__ __forceinline__ void const_field_step(const double B[3], double b2, d
     r[i] = fma(a2, w2[i], fma(a1, w1[i], fma(h, T[i], r[i])));
     Tn[i] = fma(c2, w2[i], fma(c1, w1[i], T[i]));
   }
-  const double inrm = rsqrt_nr(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+  const double inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
 #pragma unroll
   for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
   t = fma(h, dtds, t);
@@ -400,7 +400,29 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
   }
   const int n_steps = n_sub + n_corr;
   typename std::conditional<FIELD == FIELD_CONST, PolyJac, MatJac>::type D;
-  for (int is = 0; is < n_steps; ++is) {
+  bool fast = false;
+  if constexpr (FIELD == FIELD_CONST) {
+    // default policy (one primary + two correction steps) in a constant field: the three steps as one
+    // straight-line instruction stream, failure tests collected and taken once at the end
+    fast = n_sub == 1 && n_corr == 2;
+    if (fast) {
+      bool bad = false;
+#pragma unroll
+      for (int is = 0; is < 3; ++is) {
+        if (is > 0) {
+          nT = dot(nt, T);
+          bad = bad || !(nT > kNdotTMin);
+        }
+        const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+        const double h = dot(nt, dr) * rcp_nr(nT);
+        if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
+        else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
+      }
+      const double fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
+      if (bad || !(fabs(fin) < 1.0e300)) return ST_PROPAGATION;  // non-finite values persist through the steps
+    }
+  }
+  for (int is = 0; !fast && is < n_steps; ++is) {
     if (is > 0) {
       nT = dot(nt, T);
       if (!(nT > kNdotTMin)) return ST_PROPAGATION;
@@ -655,14 +677,14 @@ __device__ __forceinline__ bool material_prepare(const MaterialDesc& Mt, const d
   const double cfac = rcp_nr(fabs(nT));  // path factor 1/|n.T|
   // Highland: theta0 = 0.0136/(beta p) sqrt(X) (1 + 0.038 ln(X/beta^2)),  1/(beta p) = E lam^2
   const double X = surf[14] * cfac;
-  const double theta0 = 0.0136 * (E * al * al) * sqrt_nr(X) * fma(0.038, log(X * ib2), 1.0);
+  const double theta0 = 0.0136 * (E * al * al) * sqrt_nr(X) * fma(0.038, log_pos(X * ib2), 1.0);
   // Bethe, asymptotic density correction
   const double me = kElectronMass;
   const double Wmax = 2.0 * me * bg * bg * rcp_nr(1.0 + 2.0 * gamma * Mt.rme + Mt.rme * Mt.rme);
-  const double dhalf = fmax(0.0, Mt.log_hwp_I + log(bg) - 0.5);
+  const double dhalf = fmax(0.0, Mt.log_hwp_I + log_pos(bg) - 0.5);
   const double b2 = (p * iE) * (p * iE);
   const double dedx =
-      kBetheK * Mt.ZA * ib2 * (0.5 * log(2.0 * me * bg * bg * Wmax * Mt.inv_I2) - b2 - dhalf);
+      kBetheK * Mt.ZA * ib2 * (0.5 * log_pos(2.0 * me * bg * bg * Wmax * Mt.inv_I2) - b2 - dhalf);
   const double dE = dedx * Mt.rho * 1e-3 * 0.1 * surf[15] * cfac;
   const double E2 = E - dE;
   if (!(E2 > m)) return false;

@@ -207,7 +207,10 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
 
   cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
-  const size_t fwd_smem = geom_smem + kf::kHitStageBytes;
+  size_t fwd_smem = geom_smem + kf::kHitStageBytes;
+#ifdef KF_FWD_EXTRA_SMEM
+  fwd_smem += KF_FWD_EXTRA_SMEM;
+#endif
   const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
   const bool grid3 = fl->kind == KF_FIELD_GRID3;
   record_stage(0, stream);

@@ -273,8 +273,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     }
     gain_apply(gn, xp, Cp, x, C);
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
-    rotate_sincos(trig[0], trig[1], x[2], x[2] - xp[2]);
-    rotate_sincos(trig[2], trig[3], x[3], x[3] - xp[3]);
+    rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
     if (P.smooth) tile_flag[(size_t)l * P.leg_stride] = flag;
     if (P.output_states & OUT_PRED) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
