@@ -144,7 +144,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   {
     bool ok = true;
     int prev_s = P.start;
-#pragma unroll 4
+#pragma unroll 8
     for (int j = o0; j < o1; ++j) {  // no early exit: the loads of a track's list stay independent
       const int s = __ldg(P.surf_idx + j);
       ok = ok && (s > prev_s) && (s < P.n_surfaces);
@@ -201,6 +201,23 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       x[4] = lam_filtered;
       break;
     }
+    // RTS record ("stored Jacobians"): x-, F = J G_prev, g_prev go out right away so that the
+    // stores drain under the covariance transport; C- and the hit follow it
+    double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
+    if (P.smooth) {
+#pragma unroll
+      for (int k = 0; k < 6; ++k) R[(kRecXp + k) * KF_TILE] = xp[k];
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+#pragma unroll
+        for (int c = 0; c < 4; ++c) R[(kRecFa + a * 5 + c) * KF_TILE] = J.Ja[a][c];
+        R[(kRecFa + a * 5 + 4) * KF_TILE] = J.Ja[a][4] * g_prev;
+      }
+#pragma unroll
+      for (int c = 0; c < 4; ++c) R[(kRecFt + c) * KF_TILE] = J.Jt[c];
+      R[(kRecFt + 4) * KF_TILE] = J.Jt[4] * g_prev;
+      R[kRecG * KF_TILE] = g_prev;
+    }
     if (mat_here) material_apply(ms, C);
     double Cp[21];
     transport_covariance(J, C, Cp);
@@ -212,23 +229,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_TILE] : 0.0;
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
-    // RTS record: x-, C-, F = J G_prev, g_prev, hit ("stored Jacobians")
-    double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth) {
 #pragma unroll
-      for (int k = 0; k < 6; ++k) R[(kRecXp + k) * KF_TILE] = xp[k];
-#pragma unroll
       for (int k = 0; k < 21; ++k) R[(kRecCp + k) * KF_TILE] = Cp[k];
-#pragma unroll
-      for (int a = 0; a < 4; ++a) {
-#pragma unroll
-        for (int c = 0; c < 4; ++c) R[(kRecFa + a * 5 + c) * KF_TILE] = J.Ja[a][c];
-        R[(kRecFa + a * 5 + 4) * KF_TILE] = J.Ja[a][4] * g_prev;
-      }
-#pragma unroll
-      for (int c = 0; c < 4; ++c) R[(kRecFt + c) * KF_TILE] = J.Jt[c];
-      R[(kRecFt + 4) * KF_TILE] = J.Jt[4] * g_prev;
-      R[kRecG * KF_TILE] = g_prev;
       R[kRecM * KF_TILE] = m0;
       R[(kRecM + 1) * KF_TILE] = m1;
     }
@@ -395,14 +398,55 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* R, un
   gain_apply(gn, xp, Cp, xf, Cf);
 }
 
-// One RTS step (DESIGN.md A.7).  In: (xf, Cf) = filtered state at k, (xs, Cs) = smoothed state at k+1,
-// R1 = this thread's column of record k+1 in shared memory (x-, C-, F = J G, g).  Out: (xs, Cs) =
-// smoothed state at k.  The record column is dead after its single read, so it doubles as scratch:
-// C+ goes to the F slots and dC = C^s - C- to the C- slots while the 6x6 solve owns the registers.
-// Returns false (xs, Cs untouched apart from being overwritten by the caller) on a non-positive
-// Cholesky pivot or a non-finite result.
-__device__ __forceinline__ bool rts_step(double* R1, const double xf[6], const double Cf[21], double xs[6],
-                                         double Cs[21]) {
+// One RTS step (DESIGN.md A.7), in two parts.  In: (xf, Cf) = filtered state at k, (xs, Cs) = smoothed state
+// at k+1, R1 = this thread's column of record k+1 in shared memory (x-, C-, F = J G, g).  Out: (xs, Cs) =
+// smoothed state at k.  The record column is dead after its single read, so it doubles as scratch: C+
+// goes to the F slots and dC = C^s - C- to the C- slots while the 6x6 solve owns the registers.
+//
+// Part 1 needs record k+1 only, so it runs BEFORE the wait for record k (it covers the bulk copy's latency):
+// dx = x^s_{k+1} - x-_{k+1} (phi wrapped into (-pi, pi]), dC -> scratch, Cholesky C-_{k+1} = L L^T without
+// pivoting (scale-invariant), L[i][j] (i >= j) kept at packed (j, i), inv = 1 / diag.
+// Returns false on a non-positive pivot.
+__device__ __forceinline__ bool rts_step_pre(double* R1, const double xs[6], const double Cs[21], double dx[6],
+                                             double L[21], double inv[6]) {
+  bool ok = true;
+#pragma unroll
+  for (int c = 0; c < 21; ++c) {
+    L[c] = KF_R(R1, kRecCp + c);
+    KF_R(R1, kRecCp + c) = Cs[c] - L[c];
+  }
+  // (fixed trip counts with compile-time guards: every index is a constant after unrolling)
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    double s = L[IX(j, j)];
+#pragma unroll
+    for (int k = 0; k < 6; ++k)
+      if (k < j) s = fma(-L[SX(k, j)], L[SX(k, j)], s);
+    if (!(s > 0.0)) { ok = false; s = 1.0; }
+    L[IX(j, j)] = sqrt_nr(s, inv[j]);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      if (i > j) {
+        double u = L[SX(j, i)];
+#pragma unroll
+        for (int k = 0; k < 6; ++k)
+          if (k < j) u = fma(-L[SX(k, i)], L[SX(k, j)], u);
+        L[SX(j, i)] = u * inv[j];
+      }
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - KF_R(R1, kRecXp + j);
+  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
+  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+  return ok;
+}
+
+// Part 2: W = C+ F^T, A = W (L L^T)^-1, x^s_k = x+_k + A dx, C^s_k = C+_k + A dC A^T.
+// Returns false on a non-finite result (C+ is then still in the scratch F slots).
+__device__ __forceinline__ bool rts_step_post(double* R1, const double xf[6], const double Cf[21],
+                                              const double dx[6], const double L[21], const double inv[6],
+                                              double xs[6], double Cs[21]) {
   // W = C+ F^T, streaming F (rows loc0, loc1, phi, theta over columns loc0..qp; row t; row qp = g e_qp)
   double W[6][6];
 #pragma unroll
@@ -435,42 +479,6 @@ __device__ __forceinline__ bool rts_step(double* R1, const double xf[6], const d
   // C+ -> scratch (the F slots are consumed)
 #pragma unroll
   for (int c = 0; c < 21; ++c) KF_R(R1, kRecFa + c) = Cf[c];
-
-  // dC = C^s_{k+1} - C-_{k+1} -> scratch; Cholesky C-_{k+1} = L L^T without pivoting (scale-invariant),
-  // L[i][j] (i >= j) kept at packed (j, i), inv = 1 / diag
-  double L[21], inv[6];
-  bool ok = true;
-#pragma unroll
-  for (int c = 0; c < 21; ++c) {
-    L[c] = KF_R(R1, kRecCp + c);
-    KF_R(R1, kRecCp + c) = Cs[c] - L[c];
-  }
-  // (fixed trip counts with compile-time guards: every index is a constant after unrolling)
-#pragma unroll
-  for (int j = 0; j < 6; ++j) {
-    double s = L[IX(j, j)];
-#pragma unroll
-    for (int k = 0; k < 6; ++k)
-      if (k < j) s = fma(-L[SX(k, j)], L[SX(k, j)], s);
-    if (!(s > 0.0)) { ok = false; s = 1.0; }
-    L[IX(j, j)] = sqrt_nr(s, inv[j]);
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-      if (i > j) {
-        double u = L[SX(j, i)];
-#pragma unroll
-        for (int k = 0; k < 6; ++k)
-          if (k < j) u = fma(-L[SX(k, i)], L[SX(k, j)], u);
-        L[SX(j, i)] = u * inv[j];
-      }
-    }
-  }
-  // dx = x^s_{k+1} - x-_{k+1}, phi difference wrapped into (-pi, pi]
-  double dx[6];
-#pragma unroll
-  for (int j = 0; j < 6; ++j) dx[j] = xs[j] - KF_R(R1, kRecXp + j);
-  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
-  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
 
   // A = W (L L^T)^-1 row by row in place, x^s_k = x+_k + A dx
   double chk = 0.0;
@@ -519,7 +527,7 @@ __device__ __forceinline__ bool rts_step(double* R1, const double xf[6], const d
       chk += u;
     }
   }
-  return ok && fabs(chk) < 1.0e300;
+  return fabs(chk) < 1.0e300;
 }
 
 __global__ void __launch_bounds__(KF_TILE, KF_RTS_MIN_BLOCKS)
@@ -577,10 +585,15 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
       gv0 = __ldg(P.geom + (P.start + 1 + k) * 20 + 16);
       gv1 = __ldg(P.geom + (P.start + 1 + k) * 20 + 17);
     }
-    mbar_wait(&bar[sc], (phase >> sc) & 1u);
-    phase ^= 1u << sc;
     const double* Rc = s_rec + sc * kStageDoubles + tid;
     double* Rn = s_rec + sn * kStageDoubles + tid;
+    // everything that needs record k+1 only comes before the wait for record k
+    const bool step = k < nleg - 1 && !failed;
+    double dx[6], L[21], inv[6];
+    bool ok = true;
+    if (step) ok = rts_step_pre(Rn, xs, Cs, dx, L, inv);
+    mbar_wait(&bar[sc], (phase >> sc) & 1u);
+    phase ^= 1u << sc;
     if (k < nleg) {
       const unsigned char flag =
           reinterpret_cast<const unsigned char*>(s_rec + sc * kStageDoubles)[(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
@@ -588,13 +601,15 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
       refilter(P, Rc, flag, gv0, gv1, hp, xf, Cf);
       if (flag != 0) hp--;
       bool smoothed = false;
-      if (k < nleg - 1 && !failed) {
-        smoothed = rts_step(Rn, xf, Cf, xs, Cs);
-        if (!smoothed) {  // U25: this and all earlier surfaces fall back to the filtered states
-          failed = true;
+      if (step) {
+        if (ok) {
+          smoothed = rts_step_post(Rn, xf, Cf, dx, L, inv, xs, Cs);
+          if (!smoothed) {
 #pragma unroll
-          for (int c = 0; c < 21; ++c) Cf[c] = KF_R(Rn, kRecFa + c);
+            for (int c = 0; c < 21; ++c) Cf[c] = KF_R(Rn, kRecFa + c);
+          }
         }
+        if (!smoothed) failed = true;  // U25: this and all earlier surfaces fall back to the filtered states
       }
       if (!smoothed) {  // top of the track, or fallback
 #pragma unroll
