@@ -59,7 +59,7 @@ int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_
     if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name))
       return KF_ERR_CUDA;
   }
-  const unsigned grid = (unsigned)((P.N + block - 1) / block);  // block == KF_TILE: one CTA per tile
+  const unsigned grid = (unsigned)((P.N + block - 1) / block);  // forward: KF_FWD_BLOCK tracks per CTA; RTS: one CTA per tile
   kernel<<<grid, block, smem, stream>>>(P);
   if (set_cuda_error(cudaGetLastError(), name)) return KF_ERR_CUDA;
   g_launches++;
@@ -220,14 +220,14 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
     const int sel = (grid3 ? 4 : 0) | (op->material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
     const char* nm = "kf_forward_kernel";
     switch (sel) {
-      case 0: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, false>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 1: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, true>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 2: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, false>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 3: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, true>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 4: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, false>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 5: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, true>, P, KF_TILE, fwd_smem, stream, nm); break;
-      case 6: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, false>, P, KF_TILE, fwd_smem, stream, nm); break;
-      default: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, true>, P, KF_TILE, fwd_smem, stream, nm); break;
+      case 0: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, false>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 1: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, true>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 2: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, false>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 3: rc = launch(kf::kf_forward_kernel<FIELD_CONST, true, true>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 4: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, false>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 5: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, false, true>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      case 6: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, false>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
+      default: rc = launch(kf::kf_forward_kernel<FIELD_GRID3, true, true>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
     }
   }
   if (rc != KF_OK) return rc;

@@ -26,10 +26,15 @@ namespace kf {
 constexpr int kRecDoubles = 55;  // x-(6) C-(21) Fa(20) Ft(5) g(1) hit(2)
 constexpr int kRecXp = 0, kRecCp = 6, kRecFa = 27, kRecFt = 47, kRecG = 52, kRecM = 53;
 
-// tracks per tile = threads per CTA of both kernels (the record layout is tiled by it)
+// tracks per tile of the record layout = threads per CTA of the RTS kernel (one bulk copy per tile-leg);
+// the forward kernel's CTA covers KF_FWD_BLOCK / KF_TILE whole tiles
 #ifndef KF_TILE
-#define KF_TILE 128
+#define KF_TILE 64
 #endif
+#ifndef KF_FWD_BLOCK
+#define KF_FWD_BLOCK 128
+#endif
+static_assert(KF_FWD_BLOCK % KF_TILE == 0 && KF_TILE % 32 == 0, "a forward CTA covers whole tiles; a tile covers whole warps");
 constexpr size_t kLegBytes = (size_t)kRecDoubles * KF_TILE * sizeof(double) + KF_TILE;  // record + flags
 #ifndef KF_FWD_MIN_BLOCKS
 #define KF_FWD_MIN_BLOCKS 1
@@ -99,7 +104,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // bytes of the forward kernel's hit staging area: two alternating slots of (loc0, loc1, surface) per thread
-constexpr size_t kHitStageBytes = (size_t)KF_TILE * (2 * 2 * sizeof(double) + 2 * sizeof(int));
+constexpr size_t kHitStageBytes = (size_t)KF_FWD_BLOCK * (2 * 2 * sizeof(double) + 2 * sizeof(int));
 
 // stage the geometry table in shared memory once per CTA (5 KB for 31 planes)
 __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem) {
@@ -117,7 +122,7 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // GEOM_SMEM: the geometry table is read from shared memory (shared-space loads, their own scoreboard)
 // or, for tables too large to stage, from global memory.
 template <int FIELD, bool MATERIAL, bool GEOM_SMEM>
-__global__ void __launch_bounds__(KF_TILE, KF_FWD_MIN_BLOCKS)
+__global__ void __launch_bounds__(KF_FWD_BLOCK, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   extern __shared__ double s_dyn[];
   const double* __restrict__ G;
@@ -127,7 +132,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   } else {
     G = P.geom;
   }
-  const long long i = (long long)blockIdx.x * KF_TILE + threadIdx.x;
+  const long long i = (long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x;
   if (i >= P.N) return;
   const long long N = P.N;
 
@@ -155,13 +160,13 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   }
   // the next unconsumed hit is fetched one leg ahead of its use into this thread's own shared-memory
   // slot (two alternating slots), asynchronously
-  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][KF_TILE]
-  int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * KF_TILE) + threadIdx.x;  // [slot][KF_TILE]
+  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][KF_FWD_BLOCK]
+  int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * KF_FWD_BLOCK) + threadIdx.x;  // [slot][KF_FWD_BLOCK]
   int slot = 0;
   auto fetch_hit = [&](int j, int sl) {
-    cp_async4(s_hs + sl * KF_TILE, P.surf_idx + j);
-    cp_async8(s_hm + (sl * 2 + 0) * KF_TILE, P.loc + j);
-    cp_async8(s_hm + (sl * 2 + 1) * KF_TILE, P.loc + P.M + j);
+    cp_async4(s_hs + sl * KF_FWD_BLOCK, P.surf_idx + j);
+    cp_async8(s_hm + (sl * 2 + 0) * KF_FWD_BLOCK, P.loc + j);
+    cp_async8(s_hm + (sl * 2 + 1) * KF_FWD_BLOCK, P.loc + P.M + j);
     cp_async_commit();
   };
   if (o0 < o1) fetch_hit(o0, 0);
@@ -172,10 +177,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   sincos(x[2], &trig[0], &trig[1]);
   sincos(x[3], &trig[2], &trig[3]);
   // this tile's records: [leg][kRecDoubles][KF_TILE] doubles + [KF_TILE] flag bytes per leg
-  char* __restrict__ tile_base = P.rec + (size_t)blockIdx.x * P.tile_stride;
-  char* __restrict__ tile_rec = tile_base + (size_t)threadIdx.x * sizeof(double);
+  const int lane_in_tile = threadIdx.x % KF_TILE;
+  char* __restrict__ tile_base = P.rec + (size_t)(i / KF_TILE) * P.tile_stride;
+  char* __restrict__ tile_rec = tile_base + (size_t)lane_in_tile * sizeof(double);
   unsigned char* __restrict__ tile_flag =
-      reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(double) + threadIdx.x;
+      reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(double) + lane_in_tile;
 
   for (int l = 0; l < n_target; ++l) {
     const int s = P.start + 1 + l;
@@ -224,9 +230,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 
     // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
     cp_async_wait_all();
-    const bool has_hit = hp < o1 && s_hs[slot * KF_TILE] == s;
-    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * KF_TILE] : 0.0;
-    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_TILE] : 0.0;
+    const bool has_hit = hp < o1 && s_hs[slot * KF_FWD_BLOCK] == s;
+    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * KF_FWD_BLOCK] : 0.0;
+    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_FWD_BLOCK] : 0.0;
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth) {
