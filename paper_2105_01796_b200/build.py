@@ -16,7 +16,7 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB_PATH = os.path.join(_HERE, "libkf_fit.so")
 SOURCES = [os.path.join(CSRC, "kf_fit.cu")]
-HEADERS = [os.path.join(CSRC, "kf_device.cuh"), os.path.join(CSRC, "kf_kernels.cuh"),
+HEADERS = [os.path.join(CSRC, "kf_device.cuh"), os.path.join(CSRC, "kf_kernels.cuh"), os.path.join(CSRC, "kf_math.cuh"),
            os.path.join(INCLUDE, "kf_fit.h")]
 
 NVCC_FLAGS = [
