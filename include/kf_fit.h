@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 100          /* major * 100 + minor */
+#define KF_VERSION 101          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -187,7 +187,26 @@ int kf_fit_batch_host(const kf_tracks_in* tracks, const kf_measurements* meas, c
                       const kf_field* field, const kf_options* opt, const kf_outputs* out,
                       void* device_arena, size_t arena_bytes, void* cuda_stream);
 
-/* Number of kernels the last kf_fit_batch call of this thread enqueued (for launch accounting). */
+/* The same with the copies and the fit of different track ranges overlapped (the paper's multi-stream
+ * offload): the tracks are cut into chunks of `chunk_tracks` (rounded up to whole
+ * 128-track CTAs; 0 = max(16384, N / (4 n_streams))); chunk c runs its H2D copies, its forward and RTS
+ * kernels and its D2H copies in order on streams[c % n_streams].  The whole call is ordered after the work
+ * already enqueued on `cuda_stream`, and `cuda_stream` continues only after every chunk has finished
+ * (fork/join through the caller-owned events, which need no timing).  All handles are caller-owned;
+ * meas->offsets is read on the host during the call.  Returns like kf_fit_batch_host. */
+#define KF_MAX_STREAMS 8
+typedef struct kf_pipeline {
+  int32_t n_streams;                 /* 1..KF_MAX_STREAMS */
+  void* streams[KF_MAX_STREAMS];     /* cudaStream_t handles */
+  void* events[KF_MAX_STREAMS + 1];  /* cudaEvent_t handles, n_streams + 1 of them */
+  int64_t chunk_tracks;              /* >= 0 */
+} kf_pipeline;
+int kf_fit_batch_host_pipelined(const kf_tracks_in* tracks, const kf_measurements* meas, const kf_geometry* geom,
+                                const kf_field* field, const kf_options* opt, const kf_outputs* out,
+                                void* device_arena, size_t arena_bytes, void* cuda_stream,
+                                const kf_pipeline* pipe);
+
+/* Number of kernels the last kf_fit_batch* call of this thread enqueued (for launch accounting). */
 int kf_last_launch_count(void);
 
 /* Optional per-kernel timing for the roofline report.  After this call every kf_fit_batch of the

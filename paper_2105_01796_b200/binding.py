@@ -20,12 +20,12 @@ from . import build as _build
 
 GEOM_STRIDE = 20
 REC_DOUBLES = 55  # x-(6) C-(21) F(26) hit(2): doubles per (leg, track) in the RTS workspace
-TILE = 128         # tracks per workspace tile (= threads per CTA)
+TILE = 64          # tracks per workspace tile (= threads per RTS CTA)
 STATES_PRED, STATES_FILT, STATES_SMOOTH = 1, 2, 4
 _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .. 55
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",
-           "kf_fit_batch_host", "kf_last_launch_count", "kf_set_stage_events", "kf_probe_fp64_tflops", "kf_status_string",
+           "kf_fit_batch_host", "kf_fit_batch_host_pipelined", "kf_last_launch_count", "kf_set_stage_events", "kf_probe_fp64_tflops", "kf_status_string",
            "kf_last_cuda_error", "kf_version")
 
 
@@ -53,6 +53,14 @@ class KfOptions(C.Structure):
     _fields_ = [("smooth", C.c_int32), ("material", C.c_int32), ("outlier_chi2", C.c_double),
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
                 ("cov_inflation", C.c_double), ("output_states", C.c_int32), ("variant", C.c_int32)]
+
+
+KF_MAX_STREAMS = 8
+
+
+class KfPipeline(C.Structure):
+    _fields_ = [("n_streams", C.c_int32), ("streams", C.c_void_p * KF_MAX_STREAMS),
+                ("events", C.c_void_p * (KF_MAX_STREAMS + 1)), ("chunk_tracks", C.c_int64)]
 
 
 class KfOutputs(C.Structure):
@@ -91,6 +99,8 @@ def lib():
                                       C.POINTER(KfOptions), C.c_int, C.c_int]
     L.kf_fit_batch_host.restype = C.c_int
     L.kf_fit_batch_host.argtypes = L.kf_fit_batch.argtypes
+    L.kf_fit_batch_host_pipelined.restype = C.c_int
+    L.kf_fit_batch_host_pipelined.argtypes = L.kf_fit_batch.argtypes + [C.POINTER(KfPipeline)]
     L.kf_last_launch_count.restype = C.c_int
     L.kf_set_stage_events.restype = None
     L.kf_set_stage_events.argtypes = [C.POINTER(C.c_void_p)]
@@ -395,10 +405,26 @@ class HostCall:
     all enqueued on one stream by the library.  Pinned tensors are allocated once here; `run()` only
     enqueues.  h2d_bytes / d2h_bytes count the tensors the library copies per call."""
 
-    def __init__(self, hb: HostBatch, device="cuda:0", per_hit=False, **opt_over):
+    def __init__(self, hb: HostBatch, device="cuda:0", per_hit=False, n_streams=0, chunk_tracks=0, **opt_over):
         torch = _torch()
         self.hb, self.device = hb, torch.device(device)
         self.opt = _options_for(hb, opt_over)
+        # n_streams >= 1: kf_fit_batch_host_pipelined over that many caller-owned streams (+ fork/join events)
+        self.pipe = None
+        if n_streams:
+            if not 1 <= n_streams <= KF_MAX_STREAMS:
+                raise ValueError("n_streams must be in 1..%d" % KF_MAX_STREAMS)
+            self.streams = [torch.cuda.Stream(self.device) for _ in range(n_streams)]
+            self.events = [torch.cuda.Event(enable_timing=False) for _ in range(n_streams + 1)]
+            with torch.cuda.device(self.device):
+                for e in self.events:
+                    e.record()  # torch creates the handle lazily: make it exist
+            self.pipe = KfPipeline()
+            self.pipe.n_streams, self.pipe.chunk_tracks = n_streams, int(chunk_tracks)
+            for k, st in enumerate(self.streams):
+                self.pipe.streams[k] = st.cuda_stream
+            for k, e in enumerate(self.events):
+                self.pipe.events[k] = e.cuda_event
         if self.opt.output_states:
             raise ValueError("HostCall returns the per-track results only (output_states must be 0)")
         pin = lambda a: None if a is None else torch.from_numpy(a).pin_memory()
@@ -441,9 +467,12 @@ class HostCall:
     def run(self, stream=None):
         torch = _torch()
         s = stream if stream is not None else torch.cuda.current_stream(self.device)
-        rc = lib().kf_fit_batch_host(C.byref(self.tracks), C.byref(self.meas), C.byref(self.geom),
-                                     C.byref(self.field), C.byref(self.opt), C.byref(self.outs),
-                                     _ptr(self.arena), self.arena.numel(), C.c_void_p(s.cuda_stream))
+        args = (C.byref(self.tracks), C.byref(self.meas), C.byref(self.geom), C.byref(self.field), C.byref(self.opt),
+                C.byref(self.outs), _ptr(self.arena), self.arena.numel(), C.c_void_p(s.cuda_stream))
+        if self.pipe is not None:
+            rc = lib().kf_fit_batch_host_pipelined(*args, C.byref(self.pipe))
+        else:
+            rc = lib().kf_fit_batch_host(*args)
         if rc != 0:
             raise KfError(rc)
         self.launches = lib().kf_last_launch_count()

@@ -6,6 +6,7 @@
 // entry point ends in a kernel launch and reports KF_ERR_CUDA if that fails.
 #include <cuda_runtime.h>
 
+#include <algorithm>
 #include <cmath>
 #include <cstdio>
 #include <cstring>
@@ -143,20 +144,21 @@ const char* kf_status_string(int rc) {
   }
 }
 
-int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
-                 const kf_field* fl, const kf_options* op, const kf_outputs* out, void* workspace,
-                 size_t workspace_bytes, void* cuda_stream) {
-  g_launches = 0;
-  int rc = validate(tr, ms, ge, fl, op, out);
-  if (rc != KF_OK) return rc;
+}  // extern "C"
+
+namespace {
+
+// Kernel parameter block of the whole batch (host-side descriptor -> device-side view).
+int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
+                 const kf_options* op, const kf_outputs* out, void* workspace, size_t workspace_bytes,
+                 kf::FitParams& P) {
   const long long N = tr->n_tracks;
-  if (N == 0) return KF_OK;
   const int Lmax = ge->n_surfaces - 1 - tr->start_surface;
   const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth);
   if (w.total > 0 && (!workspace || workspace_bytes < w.total)) return KF_ERR_WORKSPACE;
 
-  kf::FitParams P{};
-  P.N = N; P.M = ms->n_meas;
+  P = kf::FitParams{};
+  P.N = N; P.M = ms->n_meas; P.ldn = N; P.ldm = ms->n_meas;
   P.params = tr->params; P.cov = tr->cov; P.start = tr->start_surface;
   P.offsets = ms->offsets; P.surf_idx = ms->surf_idx; P.loc = ms->loc; P.var = ms->var; P.cov01 = ms->cov01;
   P.n_surfaces = ge->n_surfaces; P.geom = ge->surfaces;
@@ -204,20 +206,43 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   } else {
     P.smooth = 0;  // no legs to smooth (Lmax == 0)
   }
+  return KF_OK;
+}
 
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
+// The same block restricted to tracks [t0, t0 + n): every per-track base pointer advances by t0 (t0 is a
+// multiple of KF_FWD_BLOCK, so tiles stay whole); hit arrays keep their absolute indexing through `offsets`.
+kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
+  kf::FitParams P = F;
+  P.N = n;
+  P.params += t0; P.cov += t0; P.offsets += t0;
+  P.first_params += t0; P.first_cov += t0; P.last_params += t0; P.last_cov += t0;
+  P.chi2 += t0; P.ndf += t0; P.status += t0; P.n_used += t0; P.n_outliers += t0; P.n_holes += t0;
+  for (int b = 0; b < 3; ++b) {
+    if (P.state_params[b]) P.state_params[b] += t0;
+    if (P.state_cov[b]) P.state_cov[b] += t0;
+  }
+  if (P.rk_err_max) P.rk_err_max += t0;
+  if (P.rec) {
+    P.rec += (size_t)(t0 / KF_TILE) * P.tile_stride;
+    P.nleg += t0;
+  }
+  return P;
+}
+
+// Enqueue the forward filter and, if asked for, the RTS pass over the tracks of P on `stream`.
+int enqueue_fit(const kf::FitParams& P, bool grid3, bool material, cudaStream_t stream) {
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
   size_t fwd_smem = geom_smem + kf::kHitStageBytes;
 #ifdef KF_FWD_EXTRA_SMEM
   fwd_smem += KF_FWD_EXTRA_SMEM;
 #endif
   const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
-  const bool grid3 = fl->kind == KF_FIELD_GRID3;
+  int rc;
   record_stage(0, stream);
   {
     using kf::FIELD_CONST;
     using kf::FIELD_GRID3;
-    const int sel = (grid3 ? 4 : 0) | (op->material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
+    const int sel = (grid3 ? 4 : 0) | (material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
     const char* nm = "kf_forward_kernel";
     switch (sel) {
       case 0: rc = launch(kf::kf_forward_kernel<FIELD_CONST, false, false>, P, KF_FWD_BLOCK, fwd_smem, stream, nm); break;
@@ -235,6 +260,23 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (P.smooth) rc = launch(kf::kf_rts_kernel, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
   record_stage(2, stream);
   return rc;
+}
+
+}  // namespace
+
+extern "C" {
+
+int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
+                 const kf_field* fl, const kf_options* op, const kf_outputs* out, void* workspace,
+                 size_t workspace_bytes, void* cuda_stream) {
+  g_launches = 0;
+  int rc = validate(tr, ms, ge, fl, op, out);
+  if (rc != KF_OK) return rc;
+  if (tr->n_tracks == 0) return KF_OK;
+  kf::FitParams P;
+  rc = build_params(tr, ms, ge, fl, op, out, workspace, workspace_bytes, P);
+  if (rc != KF_OK) return rc;
+  return enqueue_fit(P, fl->kind == KF_FIELD_GRID3, op->material != 0, static_cast<cudaStream_t>(cuda_stream));
 }
 
 double kf_probe_fp64_tflops(int iters, void* cuda_stream) {
@@ -329,45 +371,37 @@ size_t kf_host_arena_bytes(int64_t n_tracks, int64_t n_meas, int32_t n_surfaces,
   return arena_layout(n_tracks, n_meas, n_surfaces, start_surface, field, opt, has_var, has_cov01).total;
 }
 
-int kf_fit_batch_host(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
-                      const kf_field* fl, const kf_options* op, const kf_outputs* out, void* device_arena,
-                      size_t arena_bytes, void* cuda_stream) {
+}  // extern "C"
+
+namespace {
+
+// Host-buffer path.  With pipe == nullptr: one chunk on `main` (H2D, forward, RTS, D2H in
+// order).  With a pipeline: the tracks are cut into chunks of whole tiles; chunk c runs H2D -> fit -> D2H on
+// pipe->streams[c % n_streams], so that the copy engines and the SMs work on different chunks at the same time
+// (the paper's multi-stream offload).  Chunks address slices of the same full-size arena arrays.
+int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
+              const kf_options* op, const kf_outputs* out, void* device_arena, size_t arena_bytes,
+              cudaStream_t main, const kf_pipeline* pipe) {
   g_launches = 0;
   int rc = validate(tr, ms, ge, fl, op, out);
   if (rc != KF_OK) return rc;
+  int S = 0;
+  if (pipe) {
+    S = pipe->n_streams;
+    if (S < 1 || S > KF_MAX_STREAMS || pipe->chunk_tracks < 0 || !pipe->events[S]) return KF_ERR_ARG;
+    for (int k = 0; k < S; ++k)
+      if (!pipe->events[k]) return KF_ERR_ARG;
+  }
   const long long N = tr->n_tracks, M = ms->n_meas;
   if (N == 0) return KF_OK;
   const int nS = ge->n_surfaces;
   const ArenaLayout a = arena_layout(N, M, nS, tr->start_surface, fl, op, ms->var != nullptr, ms->cov01 != nullptr);
   if (!device_arena || arena_bytes < a.total) return KF_ERR_WORKSPACE;
   char* base = static_cast<char*>(device_arena);
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
   const size_t D = sizeof(double), I = sizeof(int32_t);
   const int Lmax = nS - 1 - tr->start_surface;
 
-#define KF_H2D(dst_off, src, bytes)                                                                   \
-  do {                                                                                                \
-    if ((bytes) > 0 && set_cuda_error(cudaMemcpyAsync(base + (dst_off), (src), (bytes),               \
-                                                      cudaMemcpyHostToDevice, stream), "H2D copy"))   \
-      return KF_ERR_CUDA;                                                                             \
-  } while (0)
-#define KF_D2H(dst, src_off, bytes)                                                                   \
-  do {                                                                                                \
-    if ((dst) && (bytes) > 0 && set_cuda_error(cudaMemcpyAsync((dst), base + (src_off), (bytes),      \
-                                                      cudaMemcpyDeviceToHost, stream), "D2H copy"))   \
-      return KF_ERR_CUDA;                                                                             \
-  } while (0)
-
-  KF_H2D(a.params, tr->params, 6 * N * D);
-  KF_H2D(a.cov, tr->cov, 21 * N * D);
-  KF_H2D(a.offsets, ms->offsets, (N + 1) * I);
-  KF_H2D(a.surf_idx, ms->surf_idx, M * I);
-  KF_H2D(a.loc, ms->loc, 2 * M * D);
-  if (ms->var) KF_H2D(a.var, ms->var, 2 * M * D);
-  if (ms->cov01) KF_H2D(a.cov01, ms->cov01, M * D);
-  KF_H2D(a.geom, ge->surfaces, (size_t)nS * KF_GEOM_STRIDE * D);
-  if (fl->kind == KF_FIELD_GRID3) KF_H2D(a.grid, fl->grid, (size_t)fl->n[0] * fl->n[1] * fl->n[2] * 3 * D);
-
+  // device-side descriptors: the arena's arrays
   kf_tracks_in dtr = *tr;
   dtr.params = reinterpret_cast<const double*>(base + a.params);
   dtr.cov = reinterpret_cast<const double*>(base + a.cov);
@@ -400,31 +434,108 @@ int kf_fit_batch_host(const kf_tracks_in* tr, const kf_measurements* ms, const k
   if (out->hit_chi2) dout.hit_chi2 = reinterpret_cast<double*>(base + a.hit_chi2);
   if (out->hit_flags) dout.hit_flags = reinterpret_cast<uint8_t*>(base + a.hit_flags);
   if (out->rk_err_max) dout.rk_err_max = reinterpret_cast<double*>(base + a.rk_err);
-
-  rc = kf_fit_batch(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, cuda_stream);
+  kf::FitParams F;
+  rc = build_params(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, F);
   if (rc != KF_OK) return rc;
 
-  KF_D2H(out->first_params, a.first_params, 6 * N * D);
-  KF_D2H(out->first_cov, a.first_cov, 21 * N * D);
-  KF_D2H(out->last_params, a.last_params, 6 * N * D);
-  KF_D2H(out->last_cov, a.last_cov, 21 * N * D);
-  KF_D2H(out->chi2, a.chi2, N * D);
-  KF_D2H(out->ndf, a.ndf, N * I);
-  KF_D2H(out->status, a.status, N * I);
-  KF_D2H(out->n_used, a.n_used, N * I);
-  KF_D2H(out->n_outliers, a.n_outliers, N * I);
-  KF_D2H(out->n_holes, a.n_holes, N * I);
-  for (int k = 0; k < 3; ++k)
-    if ((op->output_states >> k) & 1) {
-      KF_D2H(out->state_params[k], a.state_params[k], (size_t)Lmax * 6 * N * D);
-      KF_D2H(out->state_cov[k], a.state_cov[k], (size_t)Lmax * 21 * N * D);
+#define KF_TRY(call, what)                                 \
+  do {                                                     \
+    if (set_cuda_error((call), (what))) return KF_ERR_CUDA; \
+  } while (0)
+  // `rows` rows of `n` elements of `elem` bytes starting at element e0 of every row; row pitch `ld` elements
+  auto h2d = [&](size_t dst_off, const void* src, size_t ld, size_t e0, size_t n, size_t rows, size_t elem,
+                 cudaStream_t st) -> cudaError_t {
+    if (!src || n == 0 || rows == 0) return cudaSuccess;
+    return cudaMemcpy2DAsync(base + dst_off + e0 * elem, ld * elem, static_cast<const char*>(src) + e0 * elem,
+                             ld * elem, n * elem, rows, cudaMemcpyHostToDevice, st);
+  };
+  auto d2h = [&](void* dst, size_t src_off, size_t ld, size_t e0, size_t n, size_t rows, size_t elem,
+                 cudaStream_t st) -> cudaError_t {
+    if (!dst || n == 0 || rows == 0) return cudaSuccess;
+    return cudaMemcpy2DAsync(static_cast<char*>(dst) + e0 * elem, ld * elem, base + src_off + e0 * elem, ld * elem,
+                             n * elem, rows, cudaMemcpyDeviceToHost, st);
+  };
+
+  // shared global data first, on the caller's stream
+  KF_TRY(h2d(a.geom, ge->surfaces, (size_t)nS * KF_GEOM_STRIDE, 0, (size_t)nS * KF_GEOM_STRIDE, 1, D, main), "H2D geometry");
+  if (fl->kind == KF_FIELD_GRID3) {
+    const size_t g = (size_t)fl->n[0] * fl->n[1] * fl->n[2] * 3;
+    KF_TRY(h2d(a.grid, fl->grid, g, 0, g, 1, D, main), "H2D field grid");
+  }
+
+  long long chunk = N;
+  if (pipe) {
+    chunk = pipe->chunk_tracks > 0 ? pipe->chunk_tracks : std::max<long long>(16384, N / (4LL * S));
+    chunk = (chunk + KF_FWD_BLOCK - 1) / KF_FWD_BLOCK * KF_FWD_BLOCK;  // whole forward CTAs (and record tiles)
+    KF_TRY(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[S]), main), "pipeline fork");
+    for (int k = 0; k < S; ++k)
+      KF_TRY(cudaStreamWaitEvent(static_cast<cudaStream_t>(pipe->streams[k]), static_cast<cudaEvent_t>(pipe->events[S]), 0),
+             "pipeline fork");
+  }
+  const bool grid3 = fl->kind == KF_FIELD_GRID3;
+  int c = 0;
+  for (long long t0 = 0; t0 < N; t0 += chunk, ++c) {
+    const long long n = std::min(chunk, N - t0);
+    cudaStream_t st = pipe ? static_cast<cudaStream_t>(pipe->streams[c % S]) : main;
+    const long long m0 = ms->offsets[t0], m1 = ms->offsets[t0 + n];  // HOST array in this entry point
+    if (m0 < 0 || m1 < m0 || m1 > M) return KF_ERR_ARG;
+    const size_t nm = (size_t)(m1 - m0);
+    KF_TRY(h2d(a.params, tr->params, N, t0, n, 6, D, st), "H2D params");
+    KF_TRY(h2d(a.cov, tr->cov, N, t0, n, 21, D, st), "H2D cov");
+    KF_TRY(h2d(a.offsets, ms->offsets, N + 1, t0, n + 1, 1, I, st), "H2D offsets");
+    KF_TRY(h2d(a.surf_idx, ms->surf_idx, M, m0, nm, 1, I, st), "H2D surf_idx");
+    KF_TRY(h2d(a.loc, ms->loc, M, m0, nm, 2, D, st), "H2D loc");
+    KF_TRY(h2d(a.var, ms->var, M, m0, nm, 2, D, st), "H2D var");
+    KF_TRY(h2d(a.cov01, ms->cov01, M, m0, nm, 1, D, st), "H2D cov01");
+
+    rc = enqueue_fit(sub_range(F, t0, n), grid3, op->material != 0, st);
+    if (rc != KF_OK) return rc;
+
+    KF_TRY(d2h(out->first_params, a.first_params, N, t0, n, 6, D, st), "D2H first_params");
+    KF_TRY(d2h(out->first_cov, a.first_cov, N, t0, n, 21, D, st), "D2H first_cov");
+    KF_TRY(d2h(out->last_params, a.last_params, N, t0, n, 6, D, st), "D2H last_params");
+    KF_TRY(d2h(out->last_cov, a.last_cov, N, t0, n, 21, D, st), "D2H last_cov");
+    KF_TRY(d2h(out->chi2, a.chi2, N, t0, n, 1, D, st), "D2H chi2");
+    KF_TRY(d2h(out->ndf, a.ndf, N, t0, n, 1, I, st), "D2H ndf");
+    KF_TRY(d2h(out->status, a.status, N, t0, n, 1, I, st), "D2H status");
+    KF_TRY(d2h(out->n_used, a.n_used, N, t0, n, 1, I, st), "D2H n_used");
+    KF_TRY(d2h(out->n_outliers, a.n_outliers, N, t0, n, 1, I, st), "D2H n_outliers");
+    KF_TRY(d2h(out->n_holes, a.n_holes, N, t0, n, 1, I, st), "D2H n_holes");
+    for (int k = 0; k < 3; ++k)
+      if ((op->output_states >> k) & 1) {
+        KF_TRY(d2h(out->state_params[k], a.state_params[k], N, t0, n, (size_t)Lmax * 6, D, st), "D2H state_params");
+        KF_TRY(d2h(out->state_cov[k], a.state_cov[k], N, t0, n, (size_t)Lmax * 21, D, st), "D2H state_cov");
+      }
+    KF_TRY(d2h(out->hit_chi2, a.hit_chi2, M, m0, nm, 1, D, st), "D2H hit_chi2");
+    KF_TRY(d2h(out->hit_flags, a.hit_flags, M, m0, nm, 1, 1, st), "D2H hit_flags");
+    KF_TRY(d2h(out->rk_err_max, a.rk_err, N, t0, n, 1, D, st), "D2H rk_err_max");
+  }
+  if (pipe) {  // join: the caller's stream continues after every chunk stream
+    for (int k = 0; k < S && k < c; ++k) {
+      KF_TRY(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[k]), static_cast<cudaStream_t>(pipe->streams[k])),
+             "pipeline join");
+      KF_TRY(cudaStreamWaitEvent(main, static_cast<cudaEvent_t>(pipe->events[k]), 0), "pipeline join");
     }
-  KF_D2H(out->hit_chi2, a.hit_chi2, M * D);
-  KF_D2H(out->hit_flags, a.hit_flags, (size_t)M);
-  KF_D2H(out->rk_err_max, a.rk_err, N * D);
-#undef KF_H2D
-#undef KF_D2H
+  }
+#undef KF_TRY
   return KF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int kf_fit_batch_host(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
+                      const kf_field* fl, const kf_options* op, const kf_outputs* out, void* device_arena,
+                      size_t arena_bytes, void* cuda_stream) {
+  return host_impl(tr, ms, ge, fl, op, out, device_arena, arena_bytes, static_cast<cudaStream_t>(cuda_stream), nullptr);
+}
+
+int kf_fit_batch_host_pipelined(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge,
+                                const kf_field* fl, const kf_options* op, const kf_outputs* out, void* device_arena,
+                                size_t arena_bytes, void* cuda_stream, const kf_pipeline* pipe) {
+  if (!pipe) return KF_ERR_ARG;
+  return host_impl(tr, ms, ge, fl, op, out, device_arena, arena_bytes, static_cast<cudaStream_t>(cuda_stream), pipe);
 }
 
 }  // extern "C"

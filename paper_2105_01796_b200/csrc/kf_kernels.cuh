@@ -47,7 +47,9 @@ enum : int { OUT_PRED = 1, OUT_FILT = 2, OUT_SMOOTH = 4 };
 
 struct FitParams {
   // inputs
-  long long N, M;
+  long long N, M;       // tracks of this launch; hits of the batch
+  long long ldn, ldm;   // leading dimensions of the SoA track arrays / hit arrays (>= N, >= M): a launch over a
+                        // sub-range of a batch gets base pointers advanced by its first track and ldn = batch size
   const double* params;   // [6][N]
   const double* cov;      // [21][N]
   int start;
@@ -134,7 +136,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   }
   const long long i = (long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x;
   if (i >= P.N) return;
-  const long long N = P.N;
+  const long long N = P.ldn;  // SoA stride
 
   const int o0 = P.offsets[i], o1 = P.offsets[i + 1];
   double x[6], C[21];
@@ -166,7 +168,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   auto fetch_hit = [&](int j, int sl) {
     cp_async4(s_hs + sl * KF_FWD_BLOCK, P.surf_idx + j);
     cp_async8(s_hm + (sl * 2 + 0) * KF_FWD_BLOCK, P.loc + j);
-    cp_async8(s_hm + (sl * 2 + 1) * KF_FWD_BLOCK, P.loc + P.M + j);
+    cp_async8(s_hm + (sl * 2 + 1) * KF_FWD_BLOCK, P.loc + P.ldm + j);
     cp_async_commit();
   };
   if (o0 < o1) fetch_hit(o0, 0);
@@ -251,7 +253,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       double v00, v11, v01 = 0.0;
       if (P.var) {
         v00 = P.var[hp];
-        v11 = P.var[P.M + hp];
+        v11 = P.var[P.ldm + hp];
         if (P.cov01) v01 = P.cov01[hp];
       } else {
         v00 = st[16];
@@ -392,7 +394,7 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* R, un
     double v00, v11, v01 = 0.0;
     if (P.var) {
       v00 = P.var[hp];
-      v11 = P.var[P.M + hp];
+      v11 = P.var[P.ldm + hp];
       if (P.cov01) v01 = P.cov01[hp];
     } else {
       v00 = gv0;  // the surface's resolution (geometry table), fetched by the caller
@@ -543,8 +545,8 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
   __shared__ int s_nmax;
   const int tid = threadIdx.x;
   const long long i = (long long)blockIdx.x * KF_TILE + tid;
-  const long long N = P.N;
-  const bool in_range = i < N;
+  const long long N = P.ldn;  // SoA stride
+  const bool in_range = i < P.N;
   const int nleg = in_range ? P.nleg[i] : 0;
   if (tid == 0) {
     s_nmax = 0;

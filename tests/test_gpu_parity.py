@@ -250,3 +250,26 @@ def test_host_buffer_entry_point_matches_oracle():
         parity.assert_parity(got, ref, label=f"host cfg{cfg}")
         assert call.h2d_bytes > 0 and call.d2h_bytes >= n * (54 * 8 + 8 + 20)
         assert call.launches == 2
+
+
+@pytest.mark.parametrize("n_streams,chunk", [(1, 0), (3, 256), (4, 1000), (8, 128)])
+def test_pipelined_host_entry_point_matches_oracle(n_streams, chunk):
+    """kf_fit_batch_host_pipelined: chunks of whole 128-track CTAs over several streams, ragged
+    hit lists (CFG3) and a ragged last chunk; every chunk writes its slice of the same host arrays."""
+    import torch
+    for cfg, n in ((3, 3001), (4, 1501)):
+        wl = W.make_config(cfg, n_tracks=n, seed=43)
+        ref = oracle.fit_workload(wl)
+        call = kf.HostCall(kf.HostBatch.from_workload(wl), per_hit=True, n_streams=n_streams, chunk_tracks=chunk)
+        call.run()
+        torch.cuda.synchronize()
+        got = call.to_host()
+        got.rk_err_max = None
+        parity.assert_parity(got, ref, label=f"pipelined host cfg{cfg} S={n_streams}")
+        step = n if chunk == 0 and n <= 16384 else ((chunk or max(16384, n // (4 * n_streams))) + 127) // 128 * 128
+        assert call.launches == 2 * ((n + step - 1) // step)
+        # a second call on the same buffers is ordered after the first (fork/join on the caller's stream)
+        call.run()
+        torch.cuda.synchronize()
+        again = call.to_host()
+        assert np.array_equal(again.chi2, got.chi2) and np.array_equal(again.first_cov, got.first_cov)
