@@ -60,6 +60,8 @@ def parse_args():
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2)")
     ap.add_argument("--tracks", type=int, default=None, help="override the number of tracks (testing)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--variant", default="auto", choices=["auto", "thread", "lanes"],
+                    help="kernel variant (kf_options.variant): thread per track or 8 lanes per track")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -199,7 +201,8 @@ def main():
     wl = W.make_config(args.config, n_tracks=args.tracks)
     hb = kf.HostBatch.from_workload(wl)
     db = kf.DeviceBatch(hb, dev)
-    call = kf.FitCall(db)  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
+    variant = {"auto": 0, "thread": 1, "lanes": 2}[args.variant]
+    call = kf.FitCall(db, variant=variant)  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -322,7 +325,7 @@ def main():
                     layers=hb.n_surfaces - 1, field=fkind, smooth=int(smooth),
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
-                    parallelism="replicas only" if world > 1 else "1 GPU",
+                    parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,
         kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu)

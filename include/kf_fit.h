@@ -77,8 +77,14 @@ enum { KF_HIT_UNPROCESSED = 0, KF_HIT_USED = 1, KF_HIT_OUTLIER = 2 };
 /* field kinds */
 enum { KF_FIELD_CONST = 0, KF_FIELD_GRID3 = 1 };
 
-/* kernel variants (kf_options.variant) */
+/* kernel variants (kf_options.variant); results agree to round-off.
+ *   THREAD_PER_TRACK  one CUDA thread fits one track ("track-level parallelisation")
+ *   LANES_PER_TRACK   8 adjacent lanes of a warp fit one track, the 6x6 products split by row and exchanged
+ *                     with warp shuffles ("intra-track parallelisation")
+ *   AUTO              the measured choice: LANES for batches (or pipeline chunks) of at most
+ *                     KF_AUTO_LANES_MAX_TRACKS tracks, THREAD above */
 enum { KF_VARIANT_AUTO = 0, KF_VARIANT_THREAD_PER_TRACK = 1, KF_VARIANT_LANES_PER_TRACK = 2 };
+#define KF_AUTO_LANES_MAX_TRACKS 2048
 
 /* kf_options.output_states bitmask: which per-leg states to write to kf_outputs.state_* */
 enum { KF_STATES_PRED = 1, KF_STATES_FILT = 2, KF_STATES_SMOOTH = 4 };

@@ -22,6 +22,7 @@ GEOM_STRIDE = 20
 REC_DOUBLES = 55  # x-(6) C-(21) F(26) hit(2): doubles per (leg, track) in the RTS workspace
 TILE = 64          # tracks per workspace tile (= threads per RTS CTA)
 STATES_PRED, STATES_FILT, STATES_SMOOTH = 1, 2, 4
+VARIANT_AUTO, VARIANT_THREAD_PER_TRACK, VARIANT_LANES_PER_TRACK = 0, 1, 2
 _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .. 55
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",

@@ -20,6 +20,7 @@
 #pragma once
 
 #include "kf_device.cuh"
+#include "kf_lanes.cuh"
 
 namespace kf {
 
@@ -123,7 +124,12 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // last surface is still evaluated for its status bit (energy exhausted), as in DESIGN.md A.6.
 // GEOM_SMEM: the geometry table is read from shared memory (shared-space loads, their own scoreboard)
 // or, for tables too large to stage, from global memory.
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM>
+//
+// LPT = lanes per track.  1: one thread owns one track (the default).  kLanes (8): the lanes-per-track
+// variant ("intra-track parallelisation", NS "warp-cooperative lanes-per-track"): the 8 lanes
+// of a group run the scalar part of the leg redundantly (identical values, identical branches) and share the
+// 6x6 covariance transport row by row, exchanging the rows with warp shuffles; lane 0 of the group stores.
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT>
 __global__ void __launch_bounds__(KF_FWD_BLOCK, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   extern __shared__ double s_dyn[];
@@ -134,9 +140,13 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   } else {
     G = P.geom;
   }
-  const long long i = (long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x;
-  if (i >= P.N) return;
+  const long long i = ((long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x) / LPT;
+  if (i >= P.N) return;       // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
   const long long N = P.ldn;  // SoA stride
+  const int q = LPT > 1 ? (int)(threadIdx.x % LPT) : 0;           // lane within the group
+  const int gbase = LPT > 1 ? (int)((threadIdx.x & 31) & ~(LPT - 1)) : 0;  // first lane of the group in its warp
+  const unsigned gmask = LPT > 1 ? ((1u << LPT) - 1u) << gbase : 0u;
+  const bool lead = LPT == 1 || q == 0;  // the lane that writes the track's results
 
   const int o0 = P.offsets[i], o1 = P.offsets[i + 1];
   double x[6], C[21];
@@ -179,7 +189,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   sincos(x[2], &trig[0], &trig[1]);
   sincos(x[3], &trig[2], &trig[3]);
   // this tile's records: [leg][kRecDoubles][KF_TILE] doubles + [KF_TILE] flag bytes per leg
-  const int lane_in_tile = threadIdx.x % KF_TILE;
+  const int lane_in_tile = LPT == 1 ? threadIdx.x % KF_TILE : (int)(i % KF_TILE);
   char* __restrict__ tile_base = P.rec + (size_t)(i / KF_TILE) * P.tile_stride;
   char* __restrict__ tile_rec = tile_base + (size_t)lane_in_tile * sizeof(double);
   unsigned char* __restrict__ tile_flag =
@@ -212,7 +222,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     // RTS record ("stored Jacobians"): x-, F = J G_prev, g_prev go out right away so that the
     // stores drain under the covariance transport; C- and the hit follow it
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
-    if (P.smooth) {
+    if (P.smooth && lead) {
 #pragma unroll
       for (int k = 0; k < 6; ++k) R[(kRecXp + k) * KF_TILE] = xp[k];
 #pragma unroll
@@ -228,7 +238,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     }
     if (mat_here) material_apply(ms, C);
     double Cp[21];
-    transport_covariance(J, C, Cp);
+    if constexpr (LPT == 1) transport_covariance(J, C, Cp);
+    else transport_covariance_lanes(J, C, Cp, q, gbase, gmask);
 
     // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
     cp_async_wait_all();
@@ -237,7 +248,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_FWD_BLOCK] : 0.0;
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
-    if (P.smooth) {
+    if (P.smooth && lead) {
 #pragma unroll
       for (int k = 0; k < 21; ++k) R[(kRecCp + k) * KF_TILE] = Cp[k];
       R[kRecM * KF_TILE] = m0;
@@ -275,8 +286,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
         n_used++;
         flag = 1;
       }
-      if (P.hit_chi2) P.hit_chi2[hp] = c2;
-      if (P.hit_flags) P.hit_flags[hp] = flag;
+      if (P.hit_chi2 && lead) P.hit_chi2[hp] = c2;
+      if (P.hit_flags && lead) P.hit_flags[hp] = flag;
       hp++;
       slot ^= 1;
     } else {
@@ -285,16 +296,16 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     gain_apply(gn, xp, Cp, x, C);
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
     rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
-    if (P.smooth) tile_flag[(size_t)l * P.leg_stride] = flag;
-    if (P.output_states & OUT_PRED) {
+    if (P.smooth && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
+    if ((P.output_states & OUT_PRED) && lead) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
       store21(P.state_cov[0] + (size_t)l * 21 * N, N, i, Cp);
     }
-    if (P.output_states & OUT_FILT) {
+    if ((P.output_states & OUT_FILT) && lead) {
       store6(P.state_params[1] + (size_t)l * 6 * N, N, i, x);
       store21(P.state_cov[1] + (size_t)l * 21 * N, N, i, C);
     }
-    if (l == 0) {
+    if (l == 0 && lead) {
       store6(P.first_params, N, i, x);
       store21(P.first_cov, N, i, C);
     }
@@ -307,6 +318,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     MaterialStep ms;
     if (sl[14] > 0.0 && !material_prepare(P.mat, sl, trig, x[4], ms)) status |= ST_ENERGY;
   }
+  if (!lead) return;
   store6(P.last_params, N, i, x);
   store21(P.last_cov, N, i, C);
   if (nleg == 0) {
@@ -642,6 +654,223 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
     }
   }
   if (nleg > 0) {
+    store6(P.first_params, N, i, xs);
+    store21(P.first_cov, N, i, Cs);
+    if (failed) P.status[i] |= ST_NOT_POSITIVE;
+  }
+}
+
+// =====================================================================================================
+// RTS backward pass, lanes-per-track variant (kf_lanes.cuh): a group of kLanes lanes owns one track.
+// The record of a leg (kRecDoubles doubles of the track's column) is brought into the group's own
+// shared-memory slot by per-lane asynchronous copies (lane q fetches components q, q+8, ...), three
+// slots deep: records k and k+1 in use, record k-1 in flight.  Re-filtering and the Cholesky factor
+// run redundantly in every lane; the rows of W = C+ F^T, of the gain A (two triangular solves per row),
+// of A dC and of C^s are one per lane, exchanged with shuffles.  Same arithmetic per element as
+// kf_rts_kernel, same fallback rule (U25).
+constexpr int kLaneSlotDoubles = 56;                       // kRecDoubles rounded up to an even count
+constexpr int kRtsLanesBlock = 128;                        // 16 tracks per CTA
+constexpr size_t kRtsLanesSmem = (size_t)(kRtsLanesBlock / kLanes) * 3 * kLaneSlotDoubles * sizeof(double);
+
+__global__ void __launch_bounds__(kRtsLanesBlock)
+kf_rts_lanes_kernel(const __grid_constant__ FitParams P) {
+  extern __shared__ __align__(16) double s_slots[];
+  const long long i = ((long long)blockIdx.x * kRtsLanesBlock + threadIdx.x) / kLanes;
+  if (i >= P.N) return;
+  const long long N = P.ldn;
+  const int q = threadIdx.x % kLanes, row = q < 6 ? q : 5;
+  const int gbase = (threadIdx.x & 31) & ~(kLanes - 1);
+  const unsigned gmask = ((1u << kLanes) - 1u) << gbase;
+  const bool lead = q == 0;
+  const int nleg = P.nleg[i];
+  if (nleg <= 0) return;  // first_* already holds the start state
+
+  double* const slots = s_slots + (size_t)(threadIdx.x / kLanes) * 3 * kLaneSlotDoubles;
+  const char* __restrict__ tile_base = P.rec + (size_t)(i / KF_TILE) * P.tile_stride;
+  const int col = (int)(i % KF_TILE);
+  auto fetch = [&](int k) {  // record k -> slot k % 3 (this lane's share), one copy group
+    if (k >= 0) {
+      const double* src = reinterpret_cast<const double*>(tile_base + (size_t)k * P.leg_stride) + col;
+      double* dst = slots + (k % 3) * kLaneSlotDoubles;
+      for (int c = q; c < kRecDoubles; c += kLanes) cp_async8(dst + c, src + (size_t)c * KF_TILE);
+    }
+    cp_async_commit();
+  };
+  auto load_flag = [&](int k) -> unsigned char {
+    if (k < 0) return 0;
+    return reinterpret_cast<const unsigned char*>(tile_base + (size_t)k * P.leg_stride)[(size_t)kRecDoubles * KF_TILE * sizeof(double) + col];
+  };
+  fetch(nleg - 1);
+  fetch(nleg - 2);
+  unsigned char f_cur = load_flag(nleg - 1), f_n1 = load_flag(nleg - 2);
+
+  int hp = 0;
+  if (P.var) {
+    const int o0 = P.offsets[i];
+    hp = P.offsets[i + 1] - 1;
+    while (hp >= o0 && P.surf_idx[hp] > P.start + nleg) hp--;
+  }
+
+  double xs[6], Cs[21];
+  bool failed = false;
+  for (int k = nleg - 1; k >= 0; --k) {
+    const unsigned char f_n2 = load_flag(k - 2);
+    asm volatile("cp.async.wait_group 1;" ::: "memory");  // everything but the newest group: record k is here
+    __syncwarp(gmask);
+    const double* Rc = slots + (k % 3) * kLaneSlotDoubles;
+    const double* R1 = slots + ((k + 1) % 3) * kLaneSlotDoubles;
+
+    // filtered state of leg k, as the forward pass computed it (same gain routine)
+    double xf[6], Cf[21];
+    {
+      double xp[6], Cp[21];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) xp[c] = Rc[kRecXp + c];
+#pragma unroll
+      for (int c = 0; c < 21; ++c) Cp[c] = Rc[kRecCp + c];
+      Gain gn;
+      gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
+      if (f_cur == 1) {
+        double v00, v11, v01 = 0.0;
+        if (P.var) {
+          v00 = P.var[hp];
+          v11 = P.var[P.ldm + hp];
+          if (P.cov01) v01 = P.cov01[hp];
+        } else {
+          v00 = __ldg(P.geom + (P.start + 1 + k) * 20 + 16);
+          v11 = __ldg(P.geom + (P.start + 1 + k) * 20 + 17);
+        }
+        double c2;
+        if (!gain_prepare(xp, Cp, Rc[kRecM], Rc[kRecM + 1], v00, v01, v11, gn, c2)) gn.i00 = gn.i01 = gn.i11 = 0.0;
+      }
+      gain_apply(gn, xp, Cp, xf, Cf);
+      if (f_cur != 0) hp--;
+    }
+
+    bool smoothed = false;
+    if (k < nleg - 1 && !failed) {
+      // Cholesky C-_{k+1} = L L^T (every lane), L[i][j] (i >= j) at packed (j, i)
+      double L[21], inv[6], dC[21];
+      bool ok = true;
+#pragma unroll
+      for (int c = 0; c < 21; ++c) {
+        L[c] = R1[kRecCp + c];
+        dC[c] = Cs[c] - L[c];
+      }
+#pragma unroll
+      for (int j = 0; j < 6; ++j) {
+        double s = L[IX(j, j)];
+#pragma unroll
+        for (int m = 0; m < 6; ++m)
+          if (m < j) s = fma(-L[SX(m, j)], L[SX(m, j)], s);
+        if (!(s > 0.0)) { ok = false; s = 1.0; }
+        L[IX(j, j)] = sqrt_nr(s, inv[j]);
+#pragma unroll
+        for (int r = 0; r < 6; ++r) {
+          if (r > j) {
+            double u = L[SX(j, r)];
+#pragma unroll
+            for (int m = 0; m < 6; ++m)
+              if (m < j) u = fma(-L[SX(m, r)], L[SX(m, j)], u);
+            L[SX(j, r)] = u * inv[j];
+          }
+        }
+      }
+      double dx[6];
+#pragma unroll
+      for (int j = 0; j < 6; ++j) dx[j] = xs[j] - R1[kRecXp + j];
+      if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
+      else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+
+      // this lane's row of C+ and of W = C+ F^T
+      double cr[6], W[6];
+#pragma unroll
+      for (int c = 0; c < 6; ++c) cr[c] = sym_row(Cf, row, c);
+#pragma unroll
+      for (int j = 0; j < 4; ++j) {
+        double s = cr[0] * R1[kRecFa + j * 5];
+#pragma unroll
+        for (int c = 1; c < 5; ++c) s = fma(cr[c], R1[kRecFa + j * 5 + c], s);
+        W[j] = s;
+      }
+      W[4] = cr[4] * R1[kRecG];
+      {
+        double s = cr[5];
+#pragma unroll
+        for (int c = 0; c < 5; ++c) s = fma(cr[c], R1[kRecFt + c], s);
+        W[5] = s;
+      }
+      // row of A = W (L L^T)^-1
+#pragma unroll
+      for (int r = 0; r < 6; ++r) {
+        double s = W[r];
+#pragma unroll
+        for (int m = 0; m < r; ++m) s = fma(-L[IX(m, r)], W[m], s);
+        W[r] = s * inv[r];
+      }
+#pragma unroll
+      for (int r = 5; r >= 0; --r) {
+        double s = W[r];
+#pragma unroll
+        for (int m = r + 1; m < 6; ++m) s = fma(-L[IX(r, m)], W[m], s);
+        W[r] = s * inv[r];
+      }
+      // x^s component and the row of A dC
+      double xq = vec_sel(xf, row);
+#pragma unroll
+      for (int j = 0; j < 6; ++j) xq = fma(W[j], dx[j], xq);
+      double T[6];
+#pragma unroll
+      for (int j = 0; j < 6; ++j) {
+        double u = W[0] * dC[SX(0, j)];
+#pragma unroll
+        for (int m = 1; m < 6; ++m) u = fma(W[m], dC[SX(m, j)], u);
+        T[j] = u;
+      }
+      // row of C^s = C+ + (A dC) A^T: the other lanes' rows of A arrive by shuffle
+      double Rw[6];
+#pragma unroll
+      for (int j = 0; j < 6; ++j) {
+        double u = cr[j];
+#pragma unroll
+        for (int m = 0; m < 6; ++m) u = fma(T[m], __shfl_sync(gmask, W[m], gbase + j), u);
+        Rw[j] = u;
+      }
+      double xn[6], Cn[21];
+#pragma unroll
+      for (int j = 0; j < 6; ++j) xn[j] = __shfl_sync(gmask, xq, gbase + j);
+      gather_sym(Rw, Cn, gbase, gmask);
+      double chk = 0.0;
+#pragma unroll
+      for (int j = 0; j < 6; ++j) chk += xn[j];
+#pragma unroll
+      for (int c = 0; c < 21; ++c) chk += Cn[c];
+      smoothed = ok && fabs(chk) < 1.0e300;
+      if (smoothed) {
+#pragma unroll
+        for (int j = 0; j < 6; ++j) xs[j] = xn[j];
+#pragma unroll
+        for (int c = 0; c < 21; ++c) Cs[c] = Cn[c];
+      } else {
+        failed = true;  // U25
+      }
+    }
+    if (!smoothed) {  // top of the track, or fallback to the filtered state
+#pragma unroll
+      for (int c = 0; c < 6; ++c) xs[c] = xf[c];
+#pragma unroll
+      for (int c = 0; c < 21; ++c) Cs[c] = Cf[c];
+    }
+    if ((P.output_states & OUT_SMOOTH) && lead) {
+      store6(P.state_params[2] + (size_t)k * 6 * N, N, i, xs);
+      store21(P.state_cov[2] + (size_t)k * 21 * N, N, i, Cs);
+    }
+    __syncwarp(gmask);  // every lane is done with record k+1: its slot takes record k-2
+    fetch(k - 2);
+    f_cur = f_n1;
+    f_n1 = f_n2;
+  }
+  if (lead) {
     store6(P.first_params, N, i, xs);
     store21(P.first_cov, N, i, Cs);
     if (failed) P.status[i] |= ST_NOT_POSITIVE;

@@ -20,7 +20,7 @@ def both(wl, states=True, **over):
 
 
 # ---- the five configs at sizes the oracle finishes in seconds: several CTAs and a ragged tail ----------
-@pytest.mark.parametrize("cfg,n", [(0, 1000), (1, 20003), (2, 5003), (3, 5003), (4, 5003)])
+@pytest.mark.parametrize("cfg,n", [(0, 1000), (0, 3001), (1, 20003), (2, 5003), (3, 5003), (4, 5003)])
 def test_config_parity_all_states(cfg, n):
     wl = W.make_config(cfg, n_tracks=n)
     got, ref = both(wl, states=True)
@@ -31,11 +31,41 @@ def test_config_parity_all_states(cfg, n):
     np.testing.assert_allclose(got.rk_err_max, ref.rk_err_max, rtol=1e-6, atol=1e-18)
 
 
+# ---- lanes-per-track variant (8 lanes of a warp per track): same results ------------------
+@pytest.mark.parametrize("cfg,n", [(0, 1000), (1, 3001), (2, 2003), (3, 2003), (4, 2003)])
+def test_lanes_per_track_variant_parity(cfg, n):
+    wl = W.make_config(cfg, n_tracks=n, seed=60 + cfg)
+    ref = oracle.fit_workload(wl, states=True)
+    got = kf.fit_workload(wl, states=True, variant=B.VARIANT_LANES_PER_TRACK)
+    rep = parity.assert_parity(got, ref, states=True, label=f"lanes cfg{cfg}")
+    assert max(rep.values()) < 0.02, rep
+    assert B.lib().kf_last_launch_count() == (2 if wl.options.get("smooth", 1) else 1)
+
+
+@pytest.mark.parametrize("n", [1, 3, 4, 5, 15, 16, 17, 67])
+def test_lanes_per_track_ragged_group_counts(n):
+    """Group counts that leave warps and CTAs partly filled (4 groups per warp, 16 per CTA), failing tracks included."""
+    wl = W.make_config(3, n_tracks=n, seed=200 + n)
+    ref = oracle.fit_workload(wl, states=True)
+    got = kf.fit_workload(wl, states=True, variant=B.VARIANT_LANES_PER_TRACK)
+    parity.assert_parity(got, ref, states=True, label=f"lanes n={n}")
+
+
+def test_lanes_variant_with_inflated_prior_and_options():
+    wl = W.make_config(3, n_tracks=1031, seed=78)
+    for over in (dict(outlier_chi2=6.0), dict(max_step_mm=7.0, n_corr_steps=1), dict(smooth=0)):
+        ref = oracle.fit_workload(wl, states=True, **over)
+        got = kf.fit_workload(wl, states=True, variant=B.VARIANT_LANES_PER_TRACK, **over)
+        parity.assert_parity(got, ref, states=True, label=f"lanes {over}")
+
+
 @pytest.mark.parametrize("n", [1, 31, 32, 33, 127, 128, 129, 257])
 def test_ragged_tail_sizes(n):
     wl = W.make_config(3, n_tracks=n, seed=100 + n)
-    got, ref = both(wl, states=True)
-    parity.assert_parity(got, ref, states=True, label=f"n={n}")
+    ref = oracle.fit_workload(wl, states=True)
+    for variant in (B.VARIANT_THREAD_PER_TRACK, B.VARIANT_AUTO):  # AUTO takes the lanes variant at these sizes
+        got = kf.fit_workload(wl, states=True, variant=variant)
+        parity.assert_parity(got, ref, states=True, label=f"n={n} variant={variant}")
 
 
 def test_runs_are_bitwise_deterministic():
@@ -77,7 +107,17 @@ def test_filter_only_with_material_and_grid_field():
     assert got.smooth_params is None
 
 
-# ---- custom inputs ----------------------------------------------------------------------------------------
+# ---- custom inputs (each test runs once per kernel variant) ----------------------------------------------------
+_VARIANT = [B.VARIANT_AUTO]
+
+
+@pytest.fixture(params=[B.VARIANT_THREAD_PER_TRACK, B.VARIANT_LANES_PER_TRACK], ids=["thread", "lanes"])
+def variant(request):
+    _VARIANT[0] = request.param
+    yield request.param
+    _VARIANT[0] = B.VARIANT_AUTO
+
+
 def run_arrays(params0, cov0, start, offsets, surf_idx, loc, geom, var=None, cov01=None, field=("const", (0, 0, 2.0)),
                states=True, **opts):
     fld = oracle.make_field(field[0], field[1]) if field[0] == "const" else oracle.make_field(*field)
@@ -89,13 +129,13 @@ def run_arrays(params0, cov0, start, offsets, surf_idx, loc, geom, var=None, cov
                                   options=opts)
     smooth = opts.get("smooth", 1)
     os_ = (B.STATES_PRED | B.STATES_FILT | (B.STATES_SMOOTH if smooth else 0)) if states else 0
-    out = kf.fit_batch(hb, output_states=os_)
+    out = kf.fit_batch(hb, output_states=os_, variant=_VARIANT[0])
     import torch
     torch.cuda.synchronize()
     return out.to_host(), ref
 
 
-def test_per_hit_variances_and_correlation():
+def test_per_hit_variances_and_correlation(variant):
     wl = W.make_config(2, n_tracks=1500, seed=5)
     rng = np.random.default_rng(3)
     M = wl.n_meas
@@ -121,7 +161,7 @@ def tilted_geometry(L):
     return g
 
 
-def test_tilted_planes_general_field_direction_and_start_surface():
+def test_tilted_planes_general_field_direction_and_start_surface(variant):
     L, N = 12, 1200
     geom = tilted_geometry(L)
     rng = np.random.default_rng(12)
@@ -157,7 +197,7 @@ def test_tilted_planes_general_field_direction_and_start_surface():
     assert got.pred_params.shape == (N, L - start, 6)
 
 
-def test_status_bits_and_degenerate_tracks():
+def test_status_bits_and_degenerate_tracks(variant):
     """empty hit lists, malformed lists, unreachable surfaces, exhausted energy, NaN input,
     one-hit tracks -- all in one batch, next to healthy tracks."""
     wl = W.make_config(2, n_tracks=600, seed=31)
@@ -196,7 +236,7 @@ def test_status_bits_and_degenerate_tracks():
     np.testing.assert_array_equal(got.hit_flags, ref.hit_flags)
 
 
-def test_energy_exhausted_in_material():
+def test_energy_exhausted_in_material(variant):
     """slow muons in zero field lose all their kinetic energy in the silicon: status bit 4, track stops,
     last_* holds the filtered state of the layer where it stopped."""
     L, N = 30, 257

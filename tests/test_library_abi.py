@@ -128,7 +128,7 @@ def test_argument_validation_rejects_before_any_launch():
     assert _call(d) == -2
     d = _dummy_call()
     d["op"].variant = 99
-    assert _call(d) == -2
+    assert _call(d) == -1
     # null descriptor
     assert B.lib().kf_fit_batch(None, None, None, None, None, None, None, 0, None) == -1
     # zero tracks: accepted, nothing enqueued
