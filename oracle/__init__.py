@@ -58,6 +58,8 @@ def lib():
         _lib.kfo_material.restype = C.c_int32
         _lib.kfo_rts_step.restype = C.c_int32
         _lib.kfo_field_at.restype = None
+        _lib.kfo_to_line.restype = C.c_int32
+        _lib.kfo_perigee_batch.restype = C.c_int32
         _lib.kfo_rkn4_step.restype = None
     return _lib
 
@@ -156,6 +158,31 @@ def rts_step(xf, Cf, F1, xp1, Cp1, xs1, Cs1):
     return rc, xs, Cs
 
 
+def to_line(fld, opt, x, Cm, surf_from, line_c=(0.0, 0.0, 0.0), line_a=(0.0, 0.0, 1.0)):
+    """bound state on a plane -> perigee parameters on the line surface (kfo_to_line)."""
+    xo, Co, J = np.zeros(6), np.zeros((6, 6)), np.zeros((6, 6))
+    cl = C.c_int32(0)
+    rc = lib().kfo_to_line(C.byref(fld), C.byref(opt), _d(_arr(x)), _d(_arr(Cm)), _d(_arr(surf_from)),
+                           _d(_arr(line_c)), _d(_arr(line_a)), _d(xo), _d(Co), _d(J), C.byref(cl))
+    return SimpleNamespace(rc=rc, x=xo, C=Co, J=J, clamped=cl.value)
+
+
+def perigee_batch(res, geometry, start_surface, fld, opt, line_c=(0.0, 0.0, 0.0), line_a=(0.0, 0.0, 1.0)):
+    """Adds perigee_params (N,6), perigee_cov (N,6,6) to a fit result (and KFO_ST_PERIGEE = 128 to its
+    status where the extrapolation stopped): first_* taken to the line surface."""
+    N = res.first_params.shape[0]
+    nleg = (res.n_used + res.n_outliers + res.n_holes).astype(np.int32)
+    on = (int(start_surface) + (nleg > 0)).astype(np.int32)
+    res.perigee_params, res.perigee_cov = np.zeros((N, 6)), np.zeros((N, 6, 6))
+    rc = lib().kfo_perigee_batch(C.c_int64(N), _d(_arr(res.first_params)), _d(_arr(res.first_cov)),
+                                 on.ctypes.data_as(_ip), _d(_arr(geometry)), C.byref(fld), C.byref(opt),
+                                 _d(_arr(line_c)), _d(_arr(line_a)), _d(res.perigee_params), _d(res.perigee_cov),
+                                 res.status.ctypes.data_as(C.POINTER(C.c_uint32)))
+    if rc < 0:
+        raise ValueError("kfo_perigee_batch rejected the call")
+    return res
+
+
 # ---- the batch fit ----------------------------------------------------------------------------
 def fit_batch(params0, cov0, start_surface, offsets, surf_idx, loc, geometry, fld, opt, var=None,
               cov01=None, states=False, n_threads=0):
@@ -195,7 +222,12 @@ def fit_batch(params0, cov0, start_surface, offsets, surf_idx, loc, geometry, fl
     return r
 
 
-def fit_workload(wl, states=False, n_threads=0, **opt_over):
-    return fit_batch(wl.params0, wl.cov0, wl.start_surface, wl.offsets, wl.surf_idx, wl.loc,
-                     wl.geometry, field_of(wl), options_of(wl, **opt_over), states=states,
-                     n_threads=n_threads)
+def fit_workload(wl, states=False, n_threads=0, perigee=None, **opt_over):
+    """perigee = (line_centre, line_direction) adds perigee_params / perigee_cov (perigee_batch)."""
+    opt_over.pop("variant", None)  # a kernel-variant choice of the CUDA path means nothing here
+    fld, opt = field_of(wl), options_of(wl, **opt_over)
+    res = fit_batch(wl.params0, wl.cov0, wl.start_surface, wl.offsets, wl.surf_idx, wl.loc,
+                    wl.geometry, fld, opt, states=states, n_threads=n_threads)
+    if perigee is not None:
+        perigee_batch(res, wl.geometry, wl.start_surface, fld, opt, perigee[0], perigee[1])
+    return res

@@ -324,6 +324,135 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
   return 0;
 }
 
+/* ---- perigee: bound state on a plane -> bound state on a LINE surface --------
+ * The perigee surface of the paper is "defined at the point of closest approach to a reference
+ * point"; there loc0, loc1 "become the transverse and longitudinal impact parameters d0 and z0".
+ * Here (readings U27-U30) the surface is a straight line through c with unit direction
+ * a (the beam axis).  With D = r - c and D_perp = D - (D.a) a, the state is ON the surface when
+ *     g(r, T) = D_perp . T = 0            (closest approach of the tangent to the axis),
+ * and its local coordinates are  d0 = D . e_d,  e_d = (a x T)/|a x T|,   z0 = D . a.
+ * Stepping: the same fixed policy as for planes (n_sub + n_corr RKN4 steps, no accept/reject), each
+ * step aimed with the Newton root of g along the track:  h = -g / (dg/ds),
+ * dg/ds = 1 - (a.T)^2 + lam D_perp . (T x B)  (the curvature term keeps the convergence quadratic when the
+ * track passes the axis at a distance); h may be negative (the perigee lies behind the first plane).
+ * Jacobian: J = J_f2b (I - f' w^T) D J_b2f with w = grad g / (dg/ds),
+ *   grad_r g = T - (a.T) a,  grad_T g = D_perp,  dg/ds = 1 - (a.T)^2 + lam D_perp . (T x B);
+ *   J_f2b rows: d0: e_d on r (its T-derivative vanishes on the surface, where D_perp || e_d),
+ *   z0: a on r, angles / q/p / t as for planes.
+ * C_out = J C J^T.  No material is crossed.  Returns 0 or the status bit that stopped it. */
+int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x[6], const double C[36],
+                    const double* sf, const double lc[3], const double la[3], double xo[6], double Co[36],
+                    double J[36], int32_t* clamped) {
+  const double *cf = sf, *uf = sf + 3, *vf = sf + 6;
+  const double mass = opt->mass_gev;
+  const double sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
+  double f[8];
+  for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
+  f[3] = x[5];
+  f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
+  f[7] = x[4];
+  double Jb2f[48];
+  memset(Jb2f, 0, sizeof(Jb2f));
+  for (int a = 0; a < 3; ++a) {
+    Jb2f[a * 6 + 0] = uf[a];
+    Jb2f[a * 6 + 1] = vf[a];
+  }
+  Jb2f[3 * 6 + 5] = 1.0;
+  Jb2f[4 * 6 + 2] = -sphi * sth; Jb2f[4 * 6 + 3] = cphi * cth;
+  Jb2f[5 * 6 + 2] = cphi * sth;  Jb2f[5 * 6 + 3] = sphi * cth;
+  Jb2f[6 * 6 + 2] = 0.0;         Jb2f[6 * 6 + 3] = -sth;
+  Jb2f[7 * 6 + 4] = 1.0;
+
+  double D[64], Ds[64], Dn[64];
+  memset(D, 0, sizeof(D));
+  for (int i = 0; i < 8; ++i) D[i * 8 + i] = 1.0;
+  int n_sub = 1;
+  for (int is = 0;; ++is) {
+    const double* T = f + 4;
+    const double aT = dot3(la, T);
+    const double den = 1.0 - aT * aT;
+    if (!(den > 1e-12)) return KFO_ST_PROPAGATION; /* moving along the axis: no closest approach */
+    double dl[3] = {f[0] - lc[0], f[1] - lc[1], f[2] - lc[2]};
+    const double da = dot3(dl, la);
+    double dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
+    /* Newton step on g along the track: dg/ds = 1 - (a.T)^2 + lam D_perp . (T x B) */
+    double Bs[3], TxBs[3];
+    field_internal(fld, f, Bs, clamped);
+    cross3(T, Bs, TxBs);
+    const double slope = den + f[7] * dot3(dperp, TxBs);
+    if (!(fabs(slope) > 1e-12)) return KFO_ST_PROPAGATION;
+    double h = -dot3(dperp, T) / slope;
+    if (is == 0 && isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
+      double q = ceil(fabs(h) / opt->max_step_mm * (1.0 - 1e-12));
+      if (!(q >= 1.0)) q = 1.0;
+      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      n_sub = (int)q;
+    }
+    if (is >= n_sub + opt->n_corr_steps) break;
+    if (is < n_sub) h = h / (double)(n_sub - is);
+    double fn[8], e = 0.0;
+    kfo_rkn4_step(fld, mass, f, h, fn, Ds, &e, clamped);
+    matmul(8, 8, 8, Ds, D, Dn);
+    memcpy(D, Dn, sizeof(D));
+    memcpy(f, fn, sizeof(f));
+    if (!all_finite(f, 8)) return KFO_ST_PROPAGATION;
+  }
+
+  const double* r = f;
+  const double* T = f + 4;
+  const double lam = f[7];
+  const double aT = dot3(la, T);
+  double dl[3] = {r[0] - lc[0], r[1] - lc[1], r[2] - lc[2]};
+  const double da = dot3(dl, la);
+  double dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
+  double B[3], TxB[3];
+  field_internal(fld, r, B, clamped);
+  cross3(T, B, TxB);
+  double fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
+                  lam * TxB[0], lam * TxB[1], lam * TxB[2], 0.0};
+  const double dgds = 1.0 - aT * aT + lam * dot3(dperp, TxB);
+  if (!(fabs(dgds) > 1e-12)) return KFO_ST_PROPAGATION;
+  double w[8] = {(T[0] - aT * la[0]) / dgds, (T[1] - aT * la[1]) / dgds, (T[2] - aT * la[2]) / dgds, 0.0,
+                 dperp[0] / dgds, dperp[1] / dgds, dperp[2] / dgds, 0.0};
+  double Pm[64], Dt[64];
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 8; ++j) Pm[i * 8 + j] = (i == j ? 1.0 : 0.0) - fp[i] * w[j];
+  matmul(8, 8, 8, Pm, D, Dt);
+
+  const double thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
+  const double phn = atan2(T[1], T[0]);
+  const double s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
+  if (!(s2 > SIN_THETA_MIN)) return KFO_ST_THETA;
+  double ed[3];
+  cross3(la, T, ed);
+  const double edn = sqrt(dot3(ed, ed));
+  for (int a = 0; a < 3; ++a) ed[a] /= edn;
+  xo[0] = dot3(dl, ed);
+  xo[1] = da;
+  xo[2] = phn;
+  xo[3] = thn;
+  xo[4] = lam;
+  xo[5] = f[3];
+  double Jf2b[48];
+  memset(Jf2b, 0, sizeof(Jf2b));
+  for (int a = 0; a < 3; ++a) {
+    Jf2b[0 * 8 + a] = ed[a];
+    Jf2b[1 * 8 + a] = la[a];
+  }
+  Jf2b[2 * 8 + 4] = -sp / s2; Jf2b[2 * 8 + 5] = cp / s2; Jf2b[2 * 8 + 6] = 0.0;
+  Jf2b[3 * 8 + 4] = cp * c2;  Jf2b[3 * 8 + 5] = sp * c2; Jf2b[3 * 8 + 6] = -s2;
+  Jf2b[4 * 8 + 7] = 1.0;
+  Jf2b[5 * 8 + 3] = 1.0;
+  double A68[48], JC[36];
+  matmul(6, 8, 8, Jf2b, Dt, A68);
+  matmul(6, 8, 6, A68, Jb2f, J);
+  matmul(6, 6, 6, J, C, JC);
+  matmul_bt(6, 6, 6, JC, J, Co);
+  symmetrise6(Co);
+  if (!all_finite(xo, 6) || !all_finite(J, 36) || !all_finite(Co, 36)) return KFO_ST_PROPAGATION;
+  return 0;
+}
+
 /* ---- C.2.4: gain-matrix update ------------------------------------------------ */
 int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], const double V[4],
                    double xf[6], double Cf[36], double* chi2) {
@@ -691,3 +820,31 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
   }
   return used_threads;
 }
+
+/* ---- perigee of every fitted track: first_* (on the first visited surface, or on the start surface for a
+ * track that completed no leg) extrapolated to the line surface.  on_surface[i] = geometry index of the
+ * surface first_* of track i lives on.  A track whose extrapolation stops gets KFO_ST_PERIGEE OR-ed into
+ * status[i] (plus FIELD_CLAMPED when a lookup was clamped) and NaN outputs. */
+int32_t kfo_perigee_batch(int64_t N, const double* first_params, const double* first_cov,
+                          const int32_t* on_surface, const double* geometry, const kfo_field* fld,
+                          const kfo_options* opt, const double line_c[3], const double line_a[3],
+                          double* out_params, double* out_cov, uint32_t* status) {
+  if (N < 0 || !first_params || !first_cov || !on_surface || !geometry || !fld || !opt || !out_params || !out_cov)
+    return -1;
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < N; ++i) {
+    double J[36];
+    int32_t clamped = 0;
+    const int32_t rc = kfo_to_line(fld, opt, first_params + i * 6, first_cov + i * 36,
+                                   geometry + (size_t)on_surface[i] * KFO_GEOM_STRIDE, line_c, line_a,
+                                   out_params + i * 6, out_cov + i * 36, J, &clamped);
+    if (rc != 0) {
+      fill_nan(out_params + i * 6, 6);
+      fill_nan(out_cov + i * 36, 36);
+      if (status) status[i] |= KFO_ST_PERIGEE;
+    }
+    if (status && clamped) status[i] |= KFO_ST_FIELD_CLAMPED;
+  }
+  return 0;
+}
+

@@ -45,7 +45,8 @@ enum {
   KFO_ST_NDF = 8,           /* ndf <= 0                                                        */
   KFO_ST_THETA = 16,        /* sin(theta) <= 1e-12: (phi, theta) chart singular                */
   KFO_ST_FIELD_CLAMPED = 32,/* a field lookup fell outside the grid (clamped value used)       */
-  KFO_ST_BAD_HITS = 64      /* hit list not strictly ascending / outside (start, n_surfaces)   */
+  KFO_ST_BAD_HITS = 64,     /* hit list not strictly ascending / outside (start, n_surfaces)   */
+  KFO_ST_PERIGEE = 128      /* the extrapolation to the perigee (line) surface stopped          */
 };
 
 /* hit flags */
@@ -87,6 +88,13 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
                       const double* surf_from, const double* surf_to, double x_out[6],
                       double J[36], double free_out[8], double* rk_err, int32_t* clamped);
 
+/* bound state (x, C) on plane `surf_from` -> bound state (d0, z0, phi, theta, q/p, t) with covariance on
+ * the line surface through line_c with unit direction line_a: the perigee surface of PAPER.md:70, 85
+ * (closest approach to the axis); J is the 6x6 Jacobian.  Returns 0 or the stopping status bit. */
+int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x[6], const double C[36],
+                    const double* surf_from, const double line_c[3], const double line_a[3],
+                    double x_out[6], double C_out[36], double J[36], int32_t* clamped);
+
 /* gain-matrix update with a 2-D hit: returns 0, or KFO_ST_NOT_POSITIVE. */
 int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], const double V[4],
                    double xf[6], double Cf[36], double* chi2);
@@ -123,6 +131,14 @@ int32_t kfo_fit_batch(int64_t n_tracks, const double* params0, const double* cov
                       double* st_filt_cov, double* st_smooth_params, double* st_smooth_cov,
                       double* hit_chi2, uint8_t* hit_flags, double* rk_err_max,
                       int32_t n_threads);
+
+/* perigee parameters (d0, z0, phi, theta, q/p, t) and covariance of N fitted tracks: kfo_to_line applied to
+ * first_params [N][6] / first_cov [N][6][6], which live on geometry surface on_surface[i].  out_* as the
+ * inputs; a stopped extrapolation sets KFO_ST_PERIGEE in status[i] and NaN outputs.  Returns 0, or < 0. */
+int32_t kfo_perigee_batch(int64_t n_tracks, const double* first_params, const double* first_cov,
+                          const int32_t* on_surface, const double* geometry, const kfo_field* fld,
+                          const kfo_options* opt, const double line_c[3], const double line_a[3],
+                          double* out_params, double* out_cov, uint32_t* status);
 
 #ifdef __cplusplus
 }
