@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 101          /* major * 100 + minor */
+#define KF_VERSION 102          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -67,8 +67,10 @@ enum {
   KF_ST_NDF = 8,           /* ndf = 2 n_used - 5 <= 0 */
   KF_ST_THETA = 16,        /* sin(theta) <= 1e-12 on arrival: (phi, theta) chart singular. Track stops. */
   KF_ST_FIELD_CLAMPED = 32,/* a field lookup fell outside the grid; the clamped value was used */
-  KF_ST_BAD_HITS = 64      /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces):
+  KF_ST_BAD_HITS = 64,     /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces):
                               track not fitted, outputs hold the start state */
+  KF_ST_PERIGEE = 128      /* the extrapolation of first_* to the perigee surface stopped (moving along the axis,
+                              non-finite state, theta chart singular): perigee_* hold NaN */
 };
 
 /* per-hit flags */
@@ -145,6 +147,10 @@ typedef struct kf_options {
   double cov_inflation;   /* multiplies the start covariance (default 1) */
   int32_t output_states;  /* KF_STATES_* bitmask */
   int32_t variant;        /* KF_VARIANT_* */
+  /* perigee surface (used only when kf_outputs.perigee_params is given): the straight line
+   * through perigee_center with UNIT direction perigee_axis (the beam axis; default origin, +z) */
+  double perigee_center[3];
+  double perigee_axis[3];
 } kf_options;
 
 /* (4) results -- PAPER.md:180: status, track states, fitted parameters */
@@ -167,10 +173,16 @@ typedef struct kf_outputs {
   double* hit_chi2;       /* double[M]  predicted chi2 of every processed hit (0 if unprocessed) */
   uint8_t* hit_flags;     /* uint8[M]   KF_HIT_* */
   double* rk_err_max;     /* double[N]  largest embedded RKN error estimate h^2 |k1-k2-k3+k4|_1, mm */
+  /* optional, both or neither: the fitted parameters on the perigee surface:
+   * first_* extrapolated (backwards, no material) to the point of closest approach to the line of
+   * kf_options.perigee_*, as (d0, z0, phi, theta, q/p, t) with d0 = D.(a x T)/|a x T|, z0 = D.a, D = r - centre,
+   * and their covariance J first_cov J^T.  One more kernel after the fit.  DESIGN.md U27-U30. */
+  double* perigee_params; /* double[6][N] */
+  double* perigee_cov;    /* double[21][N] */
 } kf_outputs;
 
 /* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
- * muon mass, inflation 1, no per-leg states, variant AUTO. */
+ * muon mass, inflation 1, no per-leg states, variant AUTO, perigee line = the z axis through the origin. */
 void kf_default_options(kf_options* opt);
 
 /* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =

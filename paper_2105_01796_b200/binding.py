@@ -53,7 +53,8 @@ class KfField(C.Structure):
 class KfOptions(C.Structure):
     _fields_ = [("smooth", C.c_int32), ("material", C.c_int32), ("outlier_chi2", C.c_double),
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
-                ("cov_inflation", C.c_double), ("output_states", C.c_int32), ("variant", C.c_int32)]
+                ("cov_inflation", C.c_double), ("output_states", C.c_int32), ("variant", C.c_int32),
+                ("perigee_center", C.c_double * 3), ("perigee_axis", C.c_double * 3)]
 
 
 KF_MAX_STREAMS = 8
@@ -70,7 +71,7 @@ class KfOutputs(C.Structure):
                 ("status", C.c_void_p), ("n_used", C.c_void_p), ("n_outliers", C.c_void_p),
                 ("n_holes", C.c_void_p), ("state_params", C.c_void_p * 3),
                 ("state_cov", C.c_void_p * 3), ("hit_chi2", C.c_void_p), ("hit_flags", C.c_void_p),
-                ("rk_err_max", C.c_void_p)]
+                ("rk_err_max", C.c_void_p), ("perigee_params", C.c_void_p), ("perigee_cov", C.c_void_p)]
 
 
 _lib = None
@@ -132,8 +133,11 @@ def default_options() -> KfOptions:
 
 
 def make_options(smooth=1, material=0, outlier_chi2=0.0, n_corr_steps=2, max_step_mm=float("inf"),
-                 mass_gev=0.1056583755, cov_inflation=1.0, output_states=0, variant=0, **_ignored) -> KfOptions:
+                 mass_gev=0.1056583755, cov_inflation=1.0, output_states=0, variant=0,
+                 perigee_center=(0.0, 0.0, 0.0), perigee_axis=(0.0, 0.0, 1.0), **_ignored) -> KfOptions:
     o = KfOptions()
+    for k in range(3):
+        o.perigee_center[k], o.perigee_axis[k] = float(perigee_center[k]), float(perigee_axis[k])
     o.smooth, o.material, o.outlier_chi2 = int(smooth), int(material), float(outlier_chi2)
     o.n_corr_steps, o.max_step_mm, o.mass_gev = int(n_corr_steps), float(max_step_mm), float(mass_gev)
     o.cov_inflation, o.output_states, o.variant = float(cov_inflation), int(output_states), int(variant)
@@ -281,7 +285,7 @@ class DeviceOutputs:
     """Output buffers of one kf_fit_batch call, allocated once and reusable across calls."""
 
     def __init__(self, n_tracks, n_meas, n_legs_max, output_states=0, per_hit=True, rk_err=True,
-                 device="cuda:0"):
+                 device="cuda:0", perigee=False):
         torch = _torch()
         N, M, L = int(n_tracks), int(n_meas), int(n_legs_max)
         dev = torch.device(device)
@@ -301,11 +305,14 @@ class DeviceOutputs:
         self.hit_chi2 = torch.zeros(M, **f64) if per_hit else None
         self.hit_flags = torch.zeros(M, dtype=torch.uint8, device=dev) if per_hit else None
         self.rk_err_max = torch.zeros(N, **f64) if rk_err else None
+        self.perigee_params = torch.zeros((6, N), **f64) if perigee else None
+        self.perigee_cov = torch.zeros((21, N), **f64) if perigee else None
 
     def struct(self) -> KfOutputs:
         o = KfOutputs()
         for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status",
-                     "n_used", "n_outliers", "n_holes", "hit_chi2", "hit_flags", "rk_err_max"):
+                     "n_used", "n_outliers", "n_holes", "hit_chi2", "hit_flags", "rk_err_max", "perigee_params",
+                     "perigee_cov"):
             setattr(o, name, _ptr(getattr(self, name)) or None)
         for b in range(3):
             o.state_params[b] = _ptr(self.state_params[b]) or None
@@ -324,7 +331,9 @@ class DeviceOutputs:
             last_params=cpu(self.last_params).T.copy(), last_cov=unpack_cov(cpu(self.last_cov)),
             chi2=cpu(self.chi2), ndf=cpu(self.ndf), status=cpu(self.status).astype(np.uint32),
             n_used=cpu(self.n_used), n_outliers=cpu(self.n_outliers), n_holes=cpu(self.n_holes),
-            hit_chi2=cpu(self.hit_chi2), hit_flags=cpu(self.hit_flags), rk_err_max=cpu(self.rk_err_max))
+            hit_chi2=cpu(self.hit_chi2), hit_flags=cpu(self.hit_flags), rk_err_max=cpu(self.rk_err_max),
+            perigee_params=None if self.perigee_params is None else cpu(self.perigee_params).T.copy(),
+            perigee_cov=None if self.perigee_cov is None else unpack_cov(cpu(self.perigee_cov)))
         for b, name in enumerate(("pred", "filt", "smooth")):
             sp, sc = cpu(self.state_params[b]), cpu(self.state_cov[b])
             if sp is None:
@@ -352,12 +361,16 @@ class FitCall:
     """A prepared kf_fit_batch call: descriptors built once, `run()` only enqueues.
     This is what bench.py times; `fit_batch` below is the one-shot convenience."""
 
-    def __init__(self, batch: DeviceBatch, out: Optional[DeviceOutputs] = None, workspace=None, **opt_over):
+    def __init__(self, batch: DeviceBatch, out: Optional[DeviceOutputs] = None, workspace=None, perigee=None,
+                 **opt_over):
+        """perigee = (centre, unit axis): also return the fitted parameters on that line surface."""
         hb = batch.host
         self.batch = batch
+        if perigee is not None:
+            opt_over = dict(opt_over, perigee_center=perigee[0], perigee_axis=perigee[1])
         self.opt = _options_for(hb, opt_over)
         self.out = out or DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, self.opt.output_states,
-                                        device=batch.device)
+                                        device=batch.device, perigee=perigee is not None)
         self.workspace = workspace if workspace is not None else alloc_workspace(
             hb.n_tracks, hb.n_legs_max, self.opt, batch.device)
         self.tracks = KfTracksIn(hb.n_tracks, _ptr(batch.params), _ptr(batch.cov), hb.start_surface)
@@ -390,7 +403,8 @@ def fit_batch(batch, device="cuda:0", **opt_over) -> DeviceOutputs:
 
 
 def fit_workload(wl, device="cuda:0", states=False, **opt_over) -> SimpleNamespace:
-    """Fit a Workload and return host arrays in the oracle's natural layouts (for the parity tests)."""
+    """Fit a Workload and return host arrays in the oracle's natural layouts (for the parity tests).
+    perigee=(centre, unit axis) adds perigee_params / perigee_cov."""
     torch = _torch()
     if states:
         smooth = opt_over.get("smooth", wl.options.get("smooth", 1))
@@ -406,9 +420,12 @@ class HostCall:
     all enqueued on one stream by the library.  Pinned tensors are allocated once here; `run()` only
     enqueues.  h2d_bytes / d2h_bytes count the tensors the library copies per call."""
 
-    def __init__(self, hb: HostBatch, device="cuda:0", per_hit=False, n_streams=0, chunk_tracks=0, **opt_over):
+    def __init__(self, hb: HostBatch, device="cuda:0", per_hit=False, n_streams=0, chunk_tracks=0, perigee=None,
+                 **opt_over):
         torch = _torch()
         self.hb, self.device = hb, torch.device(device)
+        if perigee is not None:
+            opt_over = dict(opt_over, perigee_center=perigee[0], perigee_axis=perigee[1])
         self.opt = _options_for(hb, opt_over)
         # n_streams >= 1: kf_fit_batch_host_pipelined over that many caller-owned streams (+ fork/join events)
         self.pipe = None
@@ -443,6 +460,8 @@ class HostCall:
         self.n_used, self.n_outliers, self.n_holes = (hz(N, torch.int32) for _ in range(3))
         self.hit_chi2 = hz(M, torch.float64) if per_hit else None
         self.hit_flags = hz(M, torch.uint8) if per_hit else None
+        self.perigee_params = hz((6, N), torch.float64) if perigee is not None else None
+        self.perigee_cov = hz((21, N), torch.float64) if perigee is not None else None
         self.tracks = KfTracksIn(N, _ptr(self.h_params), _ptr(self.h_cov), hb.start_surface)
         self.meas = KfMeasurements(M, _ptr(self.h_offsets), _ptr(self.h_surf_idx), _ptr(self.h_loc),
                                    _ptr(self.h_var) or None, _ptr(self.h_cov01) or None)
@@ -450,7 +469,7 @@ class HostCall:
         self.field = _field_struct(hb, _ptr(self.h_grid))
         o = KfOutputs()
         for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status",
-                     "n_used", "n_outliers", "n_holes", "hit_chi2", "hit_flags"):
+                     "n_used", "n_outliers", "n_holes", "hit_chi2", "hit_flags", "perigee_params", "perigee_cov"):
             setattr(o, name, _ptr(getattr(self, name)) or None)
         self.outs = o
         nbytes = int(lib().kf_host_arena_bytes(N, M, hb.n_surfaces, hb.start_surface, C.byref(self.field),
@@ -462,7 +481,8 @@ class HostCall:
                                              self.h_loc, self.h_var, self.h_cov01, self.h_geometry, self.h_grid))
         self.d2h_bytes = sum(nb(t) for t in (self.first_params, self.first_cov, self.last_params,
                                              self.last_cov, self.chi2, self.ndf, self.status, self.n_used,
-                                             self.n_outliers, self.n_holes, self.hit_chi2, self.hit_flags))
+                                             self.n_outliers, self.n_holes, self.hit_chi2, self.hit_flags,
+                                             self.perigee_params, self.perigee_cov))
         self.launches = 0
 
     def run(self, stream=None):
@@ -487,7 +507,9 @@ class HostCall:
             chi2=n(self.chi2).copy(), ndf=n(self.ndf).copy(), status=n(self.status).astype(np.uint32),
             n_used=n(self.n_used).copy(), n_outliers=n(self.n_outliers).copy(), n_holes=n(self.n_holes).copy(),
             hit_chi2=None if self.hit_chi2 is None else n(self.hit_chi2).copy(),
-            hit_flags=None if self.hit_flags is None else n(self.hit_flags).copy())
+            hit_flags=None if self.hit_flags is None else n(self.hit_flags).copy(),
+            perigee_params=None if self.perigee_params is None else n(self.perigee_params).T.copy(),
+            perigee_cov=None if self.perigee_cov is None else unpack_cov(n(self.perigee_cov)))
 
 
 def probe_fp64_tflops(iters=20000, device="cuda:0") -> float:

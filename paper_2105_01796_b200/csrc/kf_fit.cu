@@ -13,6 +13,7 @@
 
 #include "kf_fit.h"
 #include "kf_kernels.cuh"
+#include "kf_perigee.cuh"
 
 namespace {
 
@@ -99,6 +100,12 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
     if ((op->output_states >> b) & 1)
       if (tr->n_tracks > 0 && (!out->state_params[b] || !out->state_cov[b])) return KF_ERR_ARG;
   if ((op->output_states & KF_STATES_SMOOTH) && !op->smooth) return KF_ERR_UNSUPPORTED;
+  if ((out->perigee_params != nullptr) != (out->perigee_cov != nullptr)) return KF_ERR_ARG;
+  if (out->perigee_params) {
+    const double* a = op->perigee_axis;
+    const double n2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
+    if (!(std::fabs(n2 - 1.0) < 1e-9)) return KF_ERR_ARG;
+  }
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)
     return KF_ERR_ARG;
@@ -121,6 +128,7 @@ void kf_default_options(kf_options* opt) {
   opt->cov_inflation = 1.0;
   opt->output_states = 0;
   opt->variant = KF_VARIANT_AUTO;
+  opt->perigee_axis[2] = 1.0;
 }
 
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt) {
@@ -255,7 +263,8 @@ int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t sme
 // variant: KF_VARIANT_*.  AUTO is the measured choice: 8 lanes
 // per track while the batch is so small that every warp of either variant has an SM sub-partition to itself
 // (<= KF_AUTO_LANES_MAX_TRACKS: 6-9 % shorter latency), one thread per track above (up to 6.5x the throughput).
-int enqueue_fit(const kf::FitParams& P, bool grid3, bool material, int variant, cudaStream_t stream) {
+int enqueue_fit(const kf::FitParams& P, const kf::PerigeeParams& G, bool grid3, bool material, int variant,
+                cudaStream_t stream) {
   const bool lanes = variant == KF_VARIANT_LANES_PER_TRACK || (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS);
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
   size_t fwd_smem = geom_smem + kf::kHitStageBytes;
@@ -275,7 +284,22 @@ int enqueue_fit(const kf::FitParams& P, bool grid3, bool material, int variant, 
                : launch(kf::kf_rts_kernel, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
   }
   record_stage(2, stream);
+  if (rc == KF_OK && G.params) {  // fitted parameters on the perigee surface: one more (small) kernel
+    const unsigned grid = (unsigned)((P.N + kf::kPerigeeBlock - 1) / kf::kPerigeeBlock);
+    if (grid3) kf::kf_perigee_kernel<kf::FIELD_GRID3><<<grid, kf::kPerigeeBlock, 0, stream>>>(P, G);
+    else kf::kf_perigee_kernel<kf::FIELD_CONST><<<grid, kf::kPerigeeBlock, 0, stream>>>(P, G);
+    if (set_cuda_error(cudaGetLastError(), "kf_perigee_kernel")) return KF_ERR_CUDA;
+    g_launches++;
+  }
   return rc;
+}
+
+kf::PerigeeParams perigee_params(const kf_options* op, const kf_outputs* out, long long t0) {
+  kf::PerigeeParams G{};
+  for (int a = 0; a < 3; ++a) { G.line.c[a] = op->perigee_center[a]; G.line.a[a] = op->perigee_axis[a]; }
+  G.params = out->perigee_params ? out->perigee_params + t0 : nullptr;
+  G.cov = out->perigee_cov ? out->perigee_cov + t0 : nullptr;
+  return G;
 }
 
 }  // namespace
@@ -292,7 +316,8 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   kf::FitParams P;
   rc = build_params(tr, ms, ge, fl, op, out, workspace, workspace_bytes, P);
   if (rc != KF_OK) return rc;
-  return enqueue_fit(P, fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant, static_cast<cudaStream_t>(cuda_stream));
+  return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
+                     static_cast<cudaStream_t>(cuda_stream));
 }
 
 double kf_probe_fp64_tflops(int iters, void* cuda_stream) {
@@ -338,7 +363,7 @@ struct Bump {
 struct ArenaLayout {
   size_t params, cov, offsets, surf_idx, loc, var, cov01, geom, grid;
   size_t first_params, first_cov, last_params, last_cov, chi2, ndf, status, n_used, n_outliers, n_holes;
-  size_t state_params[3], state_cov[3], hit_chi2, hit_flags, rk_err, workspace, workspace_bytes, total;
+  size_t state_params[3], state_cov[3], hit_chi2, hit_flags, rk_err, perigee_params, perigee_cov, workspace, workspace_bytes, total;
 };
 ArenaLayout arena_layout(long long N, long long M, int nS, int start, const kf_field* fl, const kf_options* op,
                          int has_var, int has_cov01) {
@@ -374,6 +399,8 @@ ArenaLayout arena_layout(long long N, long long M, int nS, int start, const kf_f
   a.hit_chi2 = b.take(M * D);
   a.hit_flags = b.take(M);
   a.rk_err = b.take(N * D);
+  a.perigee_params = b.take(6 * N * D);
+  a.perigee_cov = b.take(21 * N * D);
   a.workspace_bytes = workspace_layout(N, Lmax, op ? op->smooth : 1).total;
   a.workspace = b.take(a.workspace_bytes);
   a.total = b.off;
@@ -450,6 +477,10 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
   if (out->hit_chi2) dout.hit_chi2 = reinterpret_cast<double*>(base + a.hit_chi2);
   if (out->hit_flags) dout.hit_flags = reinterpret_cast<uint8_t*>(base + a.hit_flags);
   if (out->rk_err_max) dout.rk_err_max = reinterpret_cast<double*>(base + a.rk_err);
+  if (out->perigee_params) {
+    dout.perigee_params = reinterpret_cast<double*>(base + a.perigee_params);
+    dout.perigee_cov = reinterpret_cast<double*>(base + a.perigee_cov);
+  }
   kf::FitParams F;
   rc = build_params(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, F);
   if (rc != KF_OK) return rc;
@@ -504,7 +535,7 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     KF_TRY(h2d(a.var, ms->var, M, m0, nm, 2, D, st), "H2D var");
     KF_TRY(h2d(a.cov01, ms->cov01, M, m0, nm, 1, D, st), "H2D cov01");
 
-    rc = enqueue_fit(sub_range(F, t0, n), grid3, op->material != 0, op->variant, st);
+    rc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant, st);
     if (rc != KF_OK) return rc;
 
     KF_TRY(d2h(out->first_params, a.first_params, N, t0, n, 6, D, st), "D2H first_params");
@@ -525,6 +556,8 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     KF_TRY(d2h(out->hit_chi2, a.hit_chi2, M, m0, nm, 1, D, st), "D2H hit_chi2");
     KF_TRY(d2h(out->hit_flags, a.hit_flags, M, m0, nm, 1, 1, st), "D2H hit_flags");
     KF_TRY(d2h(out->rk_err_max, a.rk_err, N, t0, n, 1, D, st), "D2H rk_err_max");
+    KF_TRY(d2h(out->perigee_params, a.perigee_params, N, t0, n, 6, D, st), "D2H perigee_params");
+    KF_TRY(d2h(out->perigee_cov, a.perigee_cov, N, t0, n, 21, D, st), "D2H perigee_cov");
   }
   if (pipe) {  // join: the caller's stream continues after every chunk stream
     for (int k = 0; k < S && k < c; ++k) {

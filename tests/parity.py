@@ -66,6 +66,10 @@ def compare(gpu, ref, states=False, sel=None):
     if sel is None and gpu.hit_flags is not None and ref.hit_flags is not None:
         np.testing.assert_array_equal(gpu.hit_flags, ref.hit_flags, err_msg="hit_flags")
         rep["hit_chi2"] = chi2_excess(gpu.hit_chi2, ref.hit_chi2)
+    gp, rp = getattr(gpu, "perigee_params", None), getattr(ref, "perigee_params", None)
+    if gp is not None and rp is not None:  # fitted parameters on the perigee surface (NaN where bit 128 is set)
+        rep["perigee_params"] = param_excess(pick(gp), pick(rp))
+        rep["perigee_cov"] = cov_excess(pick(gpu.perigee_cov), pick(ref.perigee_cov))
     if states:
         for kind in ("pred", "filt", "smooth"):
             g, r = getattr(gpu, kind + "_params", None), getattr(ref, kind + "_params", None)

@@ -31,6 +31,79 @@ def test_config_parity_all_states(cfg, n):
     np.testing.assert_allclose(got.rk_err_max, ref.rk_err_max, rtol=1e-6, atol=1e-18)
 
 
+# ---- fitted parameters on the perigee surface -------------------------------
+Z_AXIS = ((0.0, 0.0, 0.0), (0.0, 0.0, 1.0))
+_ax = np.array([0.12, -0.2, 1.0])
+TILTED_AXIS = ((1.5, -2.0, 4.0), tuple(_ax / np.linalg.norm(_ax)))
+
+
+@pytest.mark.parametrize("cfg,n,line", [(1, 6001, Z_AXIS), (2, 3001, Z_AXIS), (3, 3001, TILTED_AXIS), (4, 3001, Z_AXIS),
+                                        (4, 1001, TILTED_AXIS), (0, 1000, Z_AXIS)])
+def test_perigee_parameters_parity(cfg, n, line):
+    wl = W.make_config(cfg, n_tracks=n, seed=80 + cfg)
+    ref = oracle.fit_workload(wl, perigee=line)
+    got = kf.fit_workload(wl, perigee=line)
+    rep = parity.assert_parity(got, ref, label=f"perigee cfg{cfg}")
+    assert rep["perigee_params"] < 0.05 and rep["perigee_cov"] < 0.05, rep
+    smooth = wl.options.get("smooth", 1)
+    assert B.lib().kf_last_launch_count() == (3 if smooth else 2)
+    ok = (got.status & 128) == 0
+    assert ok.mean() > 0.99 and np.all(np.isfinite(got.perigee_params[ok]))
+    if line is Z_AXIS and cfg in (1, 2):
+        # the truth starts ON the axis: its perigee is (0, 0, phi, theta, q/p, 0); Fig. 5 pulls
+        truth = wl.truth_start.copy()
+        truth[:, [0, 1, 5]] = 0.0
+        pull = (got.perigee_params - truth) / np.sqrt(np.diagonal(got.perigee_cov, axis1=1, axis2=2))
+        assert np.all(np.abs(pull.mean(axis=0)) < 4.5 / np.sqrt(n)) and np.all(np.abs(pull.std(axis=0) - 1.0) < 0.05)
+
+
+def test_perigee_failing_tracks_and_options(variant):
+    """tracks that never start (bad hit lists, NaN input), moving along the axis, stepping options."""
+    wl = W.make_config(2, n_tracks=400, seed=33)
+    params0 = wl.params0.copy()
+    params0[5, 0] = np.nan                       # NaN input: perigee NaN, bit 128
+    params0[6, 3] = 1e-13                        # along +z = along the axis: never reaches the planes, no closest approach
+    surf_idx = wl.surf_idx.copy()
+    surf_idx[wl.offsets[7] + 2] = 99             # malformed list: not fitted; perigee of the start state
+    for over in (dict(), dict(max_step_mm=6.0, n_corr_steps=1), dict(smooth=0), dict(material=0, n_corr_steps=3)):
+        hb = kf.HostBatch.from_arrays(params0, wl.cov0, 0, wl.offsets, surf_idx, wl.loc, wl.geometry, field_kind="const",
+                                      field_b=(0, 0, 2.0), options=dict(wl.options, **over))
+        db = kf.DeviceBatch(hb)
+        call = kf.FitCall(db, perigee=Z_AXIS, variant=variant)
+        got = call.run().to_host()
+        fld, opt = oracle.make_field("const", (0, 0, 2.0)), oracle.make_options(**dict(wl.options, **over))
+        ref = oracle.fit_batch(params0, wl.cov0, 0, wl.offsets, surf_idx, wl.loc, wl.geometry, fld, opt)
+        oracle.perigee_batch(ref, wl.geometry, 0, fld, opt, *Z_AXIS)
+        assert ref.status[5] & 128 and ref.status[6] & 128 and ref.status[7] & 64 and not (ref.status[7] & 128)
+        healthy = np.ones(400, bool)
+        healthy[5] = False
+        parity.assert_parity(got, ref, sel=healthy, label=f"perigee {over}")
+        np.testing.assert_array_equal(got.status, ref.status)
+        assert np.all(np.isnan(got.perigee_params[5])) and np.all(np.isnan(got.perigee_cov[6]))
+
+
+def test_perigee_through_the_host_entry_points():
+    import torch
+    wl = W.make_config(3, n_tracks=2501, seed=47)
+    ref = oracle.fit_workload(wl, perigee=TILTED_AXIS)
+    for ns in (0, 3):
+        call = kf.HostCall(kf.HostBatch.from_workload(wl), per_hit=True, n_streams=ns, chunk_tracks=512, perigee=TILTED_AXIS)
+        call.run()
+        torch.cuda.synchronize()
+        got = call.to_host()
+        got.rk_err_max = None
+        rep = parity.assert_parity(got, ref, label=f"host perigee S={ns}")
+        assert "perigee_cov" in rep
+
+
+def test_perigee_axis_must_be_a_unit_vector():
+    wl = W.make_config(1, n_tracks=64)
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    with pytest.raises(kf.KfError) as e:
+        kf.FitCall(db, perigee=((0, 0, 0), (0, 0, 2.0))).run()
+    assert e.value.rc == -1
+
+
 # ---- lanes-per-track variant (8 lanes of a warp per track, PAPER.md:126-128): same results ------------------
 @pytest.mark.parametrize("cfg,n", [(0, 1000), (1, 3001), (2, 2003), (3, 2003), (4, 2003)])
 def test_lanes_per_track_variant_parity(cfg, n):
