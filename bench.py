@@ -138,12 +138,16 @@ def dist_setup(n_gpus):
 
 
 def cpu_baseline(wl, cores_hint=None):
-    """The oracle as it stands on a bounded sample (first tracks of the same workload), all host cores."""
+    """The oracle as it stands on a bounded sample (first tracks of the same workload), all host cores.
+    A short probe sets the sample so that the timed run is about 10 s of wall clock (capped at the workload)."""
     import oracle  # test infrastructure; bench.py's cpu_baseline leg is one of its allowed callers
-    cores = os.cpu_count() or 1
-    n = int(min(wl.n_tracks, 6000 * cores, 400_000))
+    n0 = int(min(wl.n_tracks, 20_000))
+    oracle.fit_workload(wl.subset(np.arange(min(64, n0))))  # builds/loads the library outside the timing
+    t = time.perf_counter()
+    oracle.fit_workload(wl.subset(np.arange(n0)))
+    rate = n0 / max(time.perf_counter() - t, 1e-6)
+    n = int(min(wl.n_tracks, max(n0, rate * 10.0)))
     sub = wl.subset(np.arange(n))
-    oracle.fit_workload(wl.subset(np.arange(min(64, n))))  # builds/loads the library outside the timing
     t = time.perf_counter()
     r = oracle.fit_workload(sub)
     dt = time.perf_counter() - t
