@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 102          /* major * 100 + minor */
+#define KF_VERSION 103          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -87,6 +87,16 @@ enum { KF_FIELD_CONST = 0, KF_FIELD_GRID3 = 1 };
  *                     KF_AUTO_LANES_MAX_TRACKS tracks, THREAD above */
 enum { KF_VARIANT_AUTO = 0, KF_VARIANT_THREAD_PER_TRACK = 1, KF_VARIANT_LANES_PER_TRACK = 2 };
 #define KF_AUTO_LANES_MAX_TRACKS 2048
+
+/* kf_options.length_sort: ragged batches (tracks whose last hit lies on different surfaces) are fitted in
+ * order of decreasing leg count, so that the threads of a warp and the tracks of a record tile finish
+ * together; results do not depend on it.  AUTO: considered for a batch (or pipeline chunk) of at least
+ * KF_AUTO_SORT_MIN_TRACKS tracks whose hit lists are not dense (n_meas != n_tracks * legs) when the
+ * workspace holds the sort's arrays (it does when sized by kf_workspace_bytes); the device then keeps the
+ * batch's own order if the mean leg count is within 15 % of the longest track's (nothing to win).
+ * ON: always sorted. */
+enum { KF_SORT_AUTO = 0, KF_SORT_OFF = 1, KF_SORT_ON = 2 };
+#define KF_AUTO_SORT_MIN_TRACKS 8192
 
 /* kf_options.output_states bitmask: which per-leg states to write to kf_outputs.state_* */
 enum { KF_STATES_PRED = 1, KF_STATES_FILT = 2, KF_STATES_SMOOTH = 4 };
@@ -147,6 +157,8 @@ typedef struct kf_options {
   double cov_inflation;   /* multiplies the start covariance (default 1) */
   int32_t output_states;  /* KF_STATES_* bitmask */
   int32_t variant;        /* KF_VARIANT_* */
+  int32_t length_sort;    /* KF_SORT_* */
+  int32_t reserved0;      /* 0 */
   /* perigee surface (used only when kf_outputs.perigee_params is given): the straight line
    * through perigee_center with UNIT direction perigee_axis (the beam axis; default origin, +z) */
   double perigee_center[3];
@@ -182,11 +194,13 @@ typedef struct kf_outputs {
 } kf_outputs;
 
 /* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
- * muon mass, inflation 1, no per-leg states, variant AUTO, perigee line = the z axis through the origin. */
+ * muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis through the origin. */
 void kf_default_options(kf_options* opt);
 
 /* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =
- * n_surfaces - 1 - start_surface legs per track (RTS records; 0 extra when !smooth). */
+ * n_surfaces - 1 - start_surface legs per track: the RTS records and leg counts (only when smooth), then the
+ * length sort's permutation and counters (4.5 B per track).  A workspace that holds only the first part is
+ * accepted: the batch is then fitted unsorted (KF_SORT_ON: KF_ERR_WORKSPACE). */
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt);
 
 /* Enqueue the fit of one batch on `cuda_stream`.  Returns KF_OK or a negative KF_ERR_*. */

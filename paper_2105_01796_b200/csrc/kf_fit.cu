@@ -14,6 +14,7 @@
 #include "kf_fit.h"
 #include "kf_kernels.cuh"
 #include "kf_perigee.cuh"
+#include "kf_sort.cuh"
 
 namespace {
 
@@ -28,9 +29,12 @@ inline void record_stage(int k, cudaStream_t stream) {
 
 inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
-// Workspace: tile-major RTS records, then the per-track leg counts.
+// Workspace: tile-major RTS records and the per-slot leg counts (both only
+// when smoothing), then the length sort's slot -> track permutation and its bin counters (one set of
+// kSortBins counters per 128 tracks, so that every pipeline chunk has its own).
 struct WorkspaceLayout {
-  size_t rec_off, nleg_off, total;
+  size_t rec_off, nleg_off, perm_off, bins_off, total;
+  size_t rec_total;   // bytes up to the end of the leg counts: what the fit cannot run without
   size_t tile_stride;
   long long n_tiles;
 };
@@ -38,16 +42,30 @@ struct WorkspaceLayout {
 WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth) {
   WorkspaceLayout w{};
   w.n_tiles = N > 0 ? (N + KF_TILE - 1) / KF_TILE : 0;
-  if (!smooth || N <= 0 || n_legs_max <= 0) return w;
+  if (N <= 0 || n_legs_max <= 0) return w;
   size_t off = 0;
-  w.rec_off = off;
-  w.tile_stride = (size_t)n_legs_max * kf::kLegBytes;
-  off += align_up((size_t)w.n_tiles * w.tile_stride, 256);
-  w.nleg_off = off;
+  if (smooth) {
+    w.rec_off = off;
+    w.tile_stride = (size_t)n_legs_max * kf::kLegBytes;
+    off += align_up((size_t)w.n_tiles * w.tile_stride, 256);
+    w.nleg_off = off;
+    off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
+  }
+  w.rec_total = off;
+  w.perm_off = off;
   off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
+  w.bins_off = off;
+  off += align_up((size_t)((N + KF_FWD_BLOCK - 1) / KF_FWD_BLOCK) * kf::kSortBins * sizeof(int), 256);
   w.total = off;
   return w;
 }
+
+// where the length sort of a launch keeps its permutation and counters; perm == nullptr: no sort
+struct SortPlan {
+  int* perm;
+  int* bins;
+  int force;  // KF_SORT_ON: sort even when the lengths hardly differ
+};
 
 bool set_cuda_error(cudaError_t e, const char* where) {
   if (e == cudaSuccess) return false;
@@ -106,6 +124,7 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
     const double n2 = a[0] * a[0] + a[1] * a[1] + a[2] * a[2];
     if (!(std::fabs(n2 - 1.0) < 1e-9)) return KF_ERR_ARG;
   }
+  if (op->length_sort < KF_SORT_AUTO || op->length_sort > KF_SORT_ON) return KF_ERR_ARG;
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)
     return KF_ERR_ARG;
@@ -129,6 +148,7 @@ void kf_default_options(kf_options* opt) {
   opt->output_states = 0;
   opt->variant = KF_VARIANT_AUTO;
   opt->perigee_axis[2] = 1.0;
+  opt->length_sort = KF_SORT_AUTO;
 }
 
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt) {
@@ -163,11 +183,21 @@ namespace {
 // Kernel parameter block of the whole batch (host-side descriptor -> device-side view).
 int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
                  const kf_options* op, const kf_outputs* out, void* workspace, size_t workspace_bytes,
-                 kf::FitParams& P) {
+                 kf::FitParams& P, SortPlan& sort) {
   const long long N = tr->n_tracks;
   const int Lmax = ge->n_surfaces - 1 - tr->start_surface;
   const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth);
-  if (w.total > 0 && (!workspace || workspace_bytes < w.total)) return KF_ERR_WORKSPACE;
+  if (w.rec_total > 0 && (!workspace || workspace_bytes < w.rec_total)) return KF_ERR_WORKSPACE;
+  // the sort's arrays come after the records: a workspace sized by kf_workspace_bytes always holds them; a
+  // shorter one (records only) runs unsorted under AUTO and is refused under ON
+  const bool sort_room = w.total > 0 && workspace && workspace_bytes >= w.total;
+  sort = SortPlan{nullptr, nullptr, 0};
+  if (op->length_sort == KF_SORT_ON && !sort_room && w.total > 0) return KF_ERR_WORKSPACE;
+  if (op->length_sort != KF_SORT_OFF && sort_room) {
+    char* base = static_cast<char*>(workspace);
+    sort.perm = reinterpret_cast<int*>(base + w.perm_off);
+    sort.bins = reinterpret_cast<int*>(base + w.bins_off);
+  }
 
   P = kf::FitParams{};
   P.N = N; P.M = ms->n_meas; P.ldn = N; P.ldm = ms->n_meas;
@@ -209,7 +239,7 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   P.n_used = out->n_used; P.n_outliers = out->n_outliers; P.n_holes = out->n_holes;
   for (int b = 0; b < 3; ++b) { P.state_params[b] = out->state_params[b]; P.state_cov[b] = out->state_cov[b]; }
   P.hit_chi2 = out->hit_chi2; P.hit_flags = out->hit_flags; P.rk_err_max = out->rk_err_max;
-  if (w.total > 0) {
+  if (w.rec_total > 0) {
     char* base = static_cast<char*>(workspace);
     P.rec = base + w.rec_off;
     P.leg_stride = kf::kLegBytes;
@@ -263,8 +293,27 @@ int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t sme
 // variant: KF_VARIANT_*.  AUTO is the measured choice: 8 lanes
 // per track while the batch is so small that every warp of either variant has an SM sub-partition to itself
 // (<= KF_AUTO_LANES_MAX_TRACKS: 6-9 % shorter latency), one thread per track above (up to 6.5x the throughput).
-int enqueue_fit(const kf::FitParams& P, const kf::PerigeeParams& G, bool grid3, bool material, int variant,
-                cudaStream_t stream) {
+//
+// sort.perm != nullptr: first the length sort of the range (kf_sort.cuh: zero the bin counters, histogram, scan,
+// scatter), then both kernels go through the slot -> track permutation.
+int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3, bool material, int variant,
+                SortPlan sort, cudaStream_t stream) {
+  kf::FitParams P = P0;
+  P.perm = nullptr;
+  if (sort.perm) {
+    kf::SortParams S{};
+    S.N = P.N; S.offsets = P.offsets; S.surf_idx = P.surf_idx; S.start = P.start;
+    S.lmax = P.n_surfaces - 1 - P.start;
+    S.bins = sort.bins; S.perm = sort.perm; S.force = sort.force;
+    if (set_cuda_error(cudaMemsetAsync(sort.bins, 0, kf::kSortBins * sizeof(int), stream), "length sort")) return KF_ERR_CUDA;
+    const unsigned grid = (unsigned)((P.N + kf::kSortBlock - 1) / kf::kSortBlock);
+    kf::kf_sort_hist_kernel<<<grid, kf::kSortBlock, 0, stream>>>(S);
+    kf::kf_sort_scan_kernel<<<1, 32, 0, stream>>>(sort.bins, S.lmax, S.force);
+    kf::kf_sort_scatter_kernel<<<grid, kf::kSortBlock, 0, stream>>>(S);
+    if (set_cuda_error(cudaGetLastError(), "length sort")) return KF_ERR_CUDA;
+    g_launches += 3;
+    P.perm = sort.perm;
+  }
   const bool lanes = variant == KF_VARIANT_LANES_PER_TRACK || (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS);
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
   size_t fwd_smem = geom_smem + kf::kHitStageBytes;
@@ -294,6 +343,21 @@ int enqueue_fit(const kf::FitParams& P, const kf::PerigeeParams& G, bool grid3, 
   return rc;
 }
 
+// Does the range [t0, t0 + n) with n_hits hits get the length sort?  ON: yes.  AUTO: when its hit lists are not
+// dense (some track has fewer hits than there are surfaces, so leg counts may differ) and it is large enough for
+// the three extra launches not to matter.
+SortPlan sort_for_range(const SortPlan& whole, const kf_options* op, long long t0, long long n, long long n_hits,
+                        int lmax) {
+  SortPlan r{nullptr, nullptr, op->length_sort == KF_SORT_ON ? 1 : 0};
+  if (!whole.perm) return r;
+  const bool ragged = n_hits != n * (long long)lmax;
+  if (op->length_sort == KF_SORT_ON || (op->length_sort == KF_SORT_AUTO && ragged && n >= KF_AUTO_SORT_MIN_TRACKS)) {
+    r.perm = whole.perm + t0;
+    r.bins = whole.bins + (t0 / KF_FWD_BLOCK) * kf::kSortBins;
+  }
+  return r;
+}
+
 kf::PerigeeParams perigee_params(const kf_options* op, const kf_outputs* out, long long t0) {
   kf::PerigeeParams G{};
   for (int a = 0; a < 3; ++a) { G.line.c[a] = op->perigee_center[a]; G.line.a[a] = op->perigee_axis[a]; }
@@ -314,10 +378,12 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (rc != KF_OK) return rc;
   if (tr->n_tracks == 0) return KF_OK;
   kf::FitParams P;
-  rc = build_params(tr, ms, ge, fl, op, out, workspace, workspace_bytes, P);
+  SortPlan sort;
+  rc = build_params(tr, ms, ge, fl, op, out, workspace, workspace_bytes, P, sort);
   if (rc != KF_OK) return rc;
+  const int lmax = ge->n_surfaces - 1 - tr->start_surface;
   return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
-                     static_cast<cudaStream_t>(cuda_stream));
+                     sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream));
 }
 
 double kf_probe_fp64_tflops(int iters, void* cuda_stream) {
@@ -482,7 +548,8 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     dout.perigee_cov = reinterpret_cast<double*>(base + a.perigee_cov);
   }
   kf::FitParams F;
-  rc = build_params(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, F);
+  SortPlan sort;
+  rc = build_params(&dtr, &dms, &dge, &dfl, op, &dout, base + a.workspace, a.workspace_bytes, F, sort);
   if (rc != KF_OK) return rc;
 
 #define KF_TRY(call, what)                                 \
@@ -535,7 +602,8 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     KF_TRY(h2d(a.var, ms->var, M, m0, nm, 2, D, st), "H2D var");
     KF_TRY(h2d(a.cov01, ms->cov01, M, m0, nm, 1, D, st), "H2D cov01");
 
-    rc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant, st);
+    rc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant,
+                     sort_for_range(sort, op, t0, n, (long long)nm, Lmax), st);
     if (rc != KF_OK) return rc;
 
     KF_TRY(d2h(out->first_params, a.first_params, N, t0, n, 6, D, st), "D2H first_params");

@@ -80,7 +80,10 @@ struct FitParams {
   char* rec;            // [tile][leg]{ double[kRecDoubles][KF_TILE]; uint8 flag[KF_TILE] }
   size_t leg_stride;    // = kLegBytes
   size_t tile_stride;   // = Lmax * kLegBytes
-  int* nleg;
+  int* nleg;            // [slots] legs the forward pass completed, by SLOT
+  // length sort of ragged batches (kf_sort.cuh): slot -> track.  Records and nleg are indexed by slot (the
+  // position in launch order), every caller-visible array by track.  nullptr: slot == track.
+  const int* perm;
 };
 
 __device__ __forceinline__ void store6(double* base, long long stride, long long i, const double v[6]) {
@@ -140,8 +143,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   } else {
     G = P.geom;
   }
-  const long long i = ((long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x) / LPT;
-  if (i >= P.N) return;       // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
+  const long long tslot = ((long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x) / LPT;
+  if (tslot >= P.N) return;    // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
+  const long long i = P.perm ? (long long)P.perm[tslot] : tslot;  // the track this slot fits
   const long long N = P.ldn;  // SoA stride
   const int q = LPT > 1 ? (int)(threadIdx.x % LPT) : 0;           // lane within the group
   const int gbase = LPT > 1 ? (int)((threadIdx.x & 31) & ~(LPT - 1)) : 0;  // first lane of the group in its warp
@@ -189,8 +193,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   sincos(x[2], &trig[0], &trig[1]);
   sincos(x[3], &trig[2], &trig[3]);
   // this tile's records: [leg][kRecDoubles][KF_TILE] doubles + [KF_TILE] flag bytes per leg
-  const int lane_in_tile = LPT == 1 ? threadIdx.x % KF_TILE : (int)(i % KF_TILE);
-  char* __restrict__ tile_base = P.rec + (size_t)(i / KF_TILE) * P.tile_stride;
+  const int lane_in_tile = LPT == 1 ? threadIdx.x % KF_TILE : (int)(tslot % KF_TILE);
+  char* __restrict__ tile_base = P.rec + (size_t)(tslot / KF_TILE) * P.tile_stride;
   char* __restrict__ tile_rec = tile_base + (size_t)lane_in_tile * sizeof(double);
   unsigned char* __restrict__ tile_flag =
       reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(double) + lane_in_tile;
@@ -335,7 +339,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   P.n_outliers[i] = n_outl;
   P.n_holes[i] = n_holes;
   if (P.rk_err_max) P.rk_err_max[i] = errmax;
-  if (P.smooth) P.nleg[i] = nleg;
+  if (P.smooth) P.nleg[tslot] = nleg;
   for (int j = hp; j < o1; ++j) {  // hits never reached
     if (P.hit_chi2) P.hit_chi2[j] = 0.0;
     if (P.hit_flags) P.hit_flags[j] = 0;
@@ -556,10 +560,11 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
   unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_rec + 2 * kStageDoubles);
   __shared__ int s_nmax;
   const int tid = threadIdx.x;
-  const long long i = (long long)blockIdx.x * KF_TILE + tid;
+  const long long tslot = (long long)blockIdx.x * KF_TILE + tid;
   const long long N = P.ldn;  // SoA stride
-  const bool in_range = i < P.N;
-  const int nleg = in_range ? P.nleg[i] : 0;
+  const bool in_range = tslot < P.N;
+  const long long i = in_range && P.perm ? (long long)P.perm[tslot] : tslot;  // the track this slot fitted
+  const int nleg = in_range ? P.nleg[tslot] : 0;
   if (tid == 0) {
     s_nmax = 0;
     mbar_init(&bar[0], 1);
@@ -675,19 +680,20 @@ constexpr size_t kRtsLanesSmem = (size_t)(kRtsLanesBlock / kLanes) * 3 * kLaneSl
 __global__ void __launch_bounds__(kRtsLanesBlock)
 kf_rts_lanes_kernel(const __grid_constant__ FitParams P) {
   extern __shared__ __align__(16) double s_slots[];
-  const long long i = ((long long)blockIdx.x * kRtsLanesBlock + threadIdx.x) / kLanes;
-  if (i >= P.N) return;
+  const long long tslot = ((long long)blockIdx.x * kRtsLanesBlock + threadIdx.x) / kLanes;
+  if (tslot >= P.N) return;
+  const long long i = P.perm ? (long long)P.perm[tslot] : tslot;
   const long long N = P.ldn;
   const int q = threadIdx.x % kLanes, row = q < 6 ? q : 5;
   const int gbase = (threadIdx.x & 31) & ~(kLanes - 1);
   const unsigned gmask = ((1u << kLanes) - 1u) << gbase;
   const bool lead = q == 0;
-  const int nleg = P.nleg[i];
+  const int nleg = P.nleg[tslot];
   if (nleg <= 0) return;  // first_* already holds the start state
 
   double* const slots = s_slots + (size_t)(threadIdx.x / kLanes) * 3 * kLaneSlotDoubles;
-  const char* __restrict__ tile_base = P.rec + (size_t)(i / KF_TILE) * P.tile_stride;
-  const int col = (int)(i % KF_TILE);
+  const char* __restrict__ tile_base = P.rec + (size_t)(tslot / KF_TILE) * P.tile_stride;
+  const int col = (int)(tslot % KF_TILE);
   auto fetch = [&](int k) {  // record k -> slot k % 3 (this lane's share), one copy group
     if (k >= 0) {
       const double* src = reinterpret_cast<const double*>(tile_base + (size_t)k * P.leg_stride) + col;

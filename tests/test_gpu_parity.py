@@ -104,6 +104,42 @@ def test_perigee_axis_must_be_a_unit_vector():
     assert e.value.rc == -1
 
 
+# ---- length sort of ragged batches (kf_sort.cuh): same results, track by track -------------------------------
+@pytest.mark.parametrize("cfg,n", [(3, 5003), (4, 5003), (4, 129), (2, 1000), (4, 9001)])
+def test_length_sort_parity_all_states(cfg, n, variant):
+    wl = W.make_config(cfg, n_tracks=n, seed=90 + cfg)
+    ref = oracle.fit_workload(wl, states=True, perigee=Z_AXIS)
+    sort = B.SORT_AUTO if n == 9001 else B.SORT_ON   # 9001 ragged tracks: AUTO sorts on its own
+    got = kf.fit_workload(wl, states=True, perigee=Z_AXIS, length_sort=sort, variant=variant)
+    parity.assert_parity(got, ref, states=True, label=f"sorted cfg{cfg}")
+    smooth = wl.options.get("smooth", 1)
+    assert B.lib().kf_last_launch_count() == 3 + (2 if smooth else 1) + 1
+    off = kf.fit_workload(wl, states=True, perigee=Z_AXIS, length_sort=B.SORT_OFF, variant=variant)
+    assert B.lib().kf_last_launch_count() == (2 if smooth else 1) + 1
+    # a track's fit does not depend on the slot it ran in: bit for bit the unsorted run
+    for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "smooth_params", "smooth_cov",
+                 "perigee_params", "status", "hit_flags"):
+        np.testing.assert_array_equal(getattr(got, name), getattr(off, name), err_msg=name)
+
+
+def test_length_sort_degenerate_lists_and_host_chunks():
+    """pipeline chunks sort independently (each has its own counters); malformed and empty lists are covered by
+    test_status_bits_and_degenerate_tracks, which runs sorted."""
+    import torch
+    wl = W.make_config(4, n_tracks=2600, seed=12)
+    ref = oracle.fit_workload(wl)
+    for ns, chunk in ((0, 0), (3, 384), (2, 128)):
+        call = kf.HostCall(kf.HostBatch.from_workload(wl), per_hit=True, n_streams=ns, chunk_tracks=chunk,
+                           length_sort=B.SORT_ON)
+        call.run()
+        torch.cuda.synchronize()
+        got = call.to_host()
+        got.rk_err_max = None
+        parity.assert_parity(got, ref, label=f"sorted host S={ns}")
+        n_chunks = 1 if ns == 0 else (2600 + chunk - 1) // chunk
+        assert call.launches == 5 * n_chunks
+
+
 # ---- lanes-per-track variant (8 lanes of a warp per track, PAPER.md:126-128): same results ------------------
 @pytest.mark.parametrize("cfg,n", [(0, 1000), (1, 3001), (2, 2003), (3, 2003), (4, 2003)])
 def test_lanes_per_track_variant_parity(cfg, n):
@@ -297,7 +333,7 @@ def test_status_bits_and_degenerate_tracks(variant):
     surf_idx = np.concatenate(surf).astype(np.int32)
     loc = np.concatenate(locs)
     got, ref = run_arrays(params0, cov0, 0, offsets, surf_idx, loc, wl.geometry, material=1, smooth=1,
-                          outlier_chi2=15.0)
+                          outlier_chi2=15.0, length_sort=B.SORT_ON)
     assert ref.status[3] == 8 and ref.status[4] & 8
     assert ref.status[5] & 64 and ref.status[6] & 64 and ref.status[7] & 64
     assert ref.status[8] & 1 and ref.status[10] & 1 and ref.status[11] & 1

@@ -37,16 +37,16 @@ def test_struct_sizes_match_the_header_layout():
     assert C.sizeof(B.KfMeasurements) == 48
     assert C.sizeof(B.KfGeometry) == 48
     assert C.sizeof(B.KfField) == 4 + 4 + 24 + 12 + 4 + 24 + 24 + 8
-    assert C.sizeof(B.KfOptions) == 56 + 48
+    assert C.sizeof(B.KfOptions) == 56 + 8 + 48
     assert C.sizeof(B.KfOutputs) == 10 * 8 + 6 * 8 + 3 * 8 + 2 * 8
     assert C.sizeof(B.KfPipeline) == 8 + 8 * 8 + 9 * 8 + 8
 
 
 def test_defaults_and_version():
     L = B.lib()
-    assert L.kf_version() == 102
+    assert L.kf_version() == 103
     o = B.default_options()
-    assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant) == (1, 0, 2, 0, 0)
+    assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort) == (1, 0, 2, 0, 0, 0)
     assert o.outlier_chi2 == 0.0 and np.isinf(o.max_step_mm) and o.cov_inflation == 1.0
     assert o.mass_gev == pytest.approx(0.1056583755)
     assert L.kf_status_string(0) == b"ok"
@@ -58,12 +58,15 @@ def test_workspace_bytes():
     # tile-major records: tiles * Lmax * (55 doubles + 1 flag byte) * TILE, then nleg int32 per slot,
     # each block rounded to 256 B (include/kf_fit.h "workspace")
     up = lambda v: (v + 255) // 256 * 256
+    # then the length sort's arrays: slot -> track permutation (int32 per slot), 64 counters per 128 tracks
+    sort = lambda n: up((n + B.TILE - 1) // B.TILE * B.TILE * 4) + up((n + 127) // 128 * 64 * 4)
     for n, L in ((1000, 6), (50, 3), (65, 30)):
         tiles = (n + B.TILE - 1) // B.TILE
-        assert B.workspace_bytes(n, L, o) == up(tiles * L * (B.REC_DOUBLES * 8 + 1) * B.TILE) + up(tiles * B.TILE * 4)
+        assert B.workspace_bytes(n, L, o) == (up(tiles * L * (B.REC_DOUBLES * 8 + 1) * B.TILE) + up(tiles * B.TILE * 4)
+                                              + sort(n))
     n, L = 1000, 6
     o.smooth = 0
-    assert B.workspace_bytes(n, L, o) == 0
+    assert B.workspace_bytes(n, L, o) == sort(n)
     o.smooth = 1
     assert B.workspace_bytes(0, L, o) == 0
     # 1e6 tracks x 30 legs fits comfortably in 180 GB
