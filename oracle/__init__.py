@@ -40,7 +40,7 @@ class _Options(C.Structure):
     _fields_ = [("smooth", C.c_int32), ("material", C.c_int32), ("outlier_chi2", C.c_double),
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
                 ("cov_inflation", C.c_double), ("mat_Z", C.c_double), ("mat_A", C.c_double),
-                ("mat_rho", C.c_double), ("mat_I_eV", C.c_double)]
+                ("mat_rho", C.c_double), ("mat_I_eV", C.c_double), ("step_tolerance_mm", C.c_double)]
 
 
 _lib = None
@@ -92,8 +92,9 @@ def make_field(kind="const", b=(0.0, 0.0, 2.0), grid_n=None, grid_origin=None, g
 
 def make_options(smooth=1, material=0, outlier_chi2=0.0, n_corr_steps=2, max_step_mm=float("inf"),
                  mass_gev=0.1056583755, cov_inflation=1.0, Z=14.0, A=28.0855, rho=2.329,
-                 I_eV=173.0, **_ignored):
+                 I_eV=173.0, step_tolerance_mm=0.0, **_ignored):
     o = _Options()
+    o.step_tolerance_mm = float(step_tolerance_mm)
     o.smooth, o.material, o.outlier_chi2 = int(smooth), int(material), float(outlier_chi2)
     o.n_corr_steps, o.max_step_mm, o.mass_gev = int(n_corr_steps), float(max_step_mm), float(mass_gev)
     o.cov_inflation = float(cov_inflation)

@@ -259,6 +259,19 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
       if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
       n_sub = (int)q;
     }
+    /* Adaptive step count ("adaptive Runge-Kutta-Nystrom"; reading U31): the embedded
+     * error estimate eps0 of ONE trial step over the whole leg (the step itself is discarded) fixes the number of
+     * primary steps.  eps = h^2 |k1-k2-k3+k4|_1 falls with the fourth power of the step, so
+     * n = ceil((eps0 / tol)^(1/4)) steps bring the estimate of each to about tol.  A rule on a number, decided once
+     * per leg before any step is taken: no accept/reject loop. */
+    if (isfinite(opt->step_tolerance_mm) && opt->step_tolerance_mm > 0.0) {
+      double ft[8], Dt_[64], e0 = 0.0;
+      kfo_rkn4_step(fld, mass, f, s0, ft, Dt_, &e0, clamped);
+      double q = ceil(sqrt(sqrt(e0 / opt->step_tolerance_mm)) * (1.0 - 1e-12));
+      if (!(q >= 1.0)) q = 1.0;
+      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      if ((int)q > n_sub) n_sub = (int)q;
+    }
   }
   const int n_steps = n_sub + opt->n_corr_steps;
   for (int is = 0; is < n_steps; ++is) {

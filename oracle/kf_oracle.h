@@ -70,6 +70,7 @@ typedef struct {
   double mass_gev;
   double cov_inflation;  /* multiplies the whole start covariance */
   double mat_Z, mat_A, mat_rho, mat_I_eV; /* one material for the batch (silicon in the configs) */
+  double step_tolerance_mm; /* > 0: adaptive step count per leg (U31); <= 0 or inf: off */
 } kfo_options;
 
 /* --- step-level entry points (pinned one by one in tests/test_oracle_steps.py) ------------- */
