@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 103          /* major * 100 + minor */
+#define KF_VERSION 104          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -159,6 +159,11 @@ typedef struct kf_options {
   int32_t variant;        /* KF_VARIANT_* */
   int32_t length_sort;    /* KF_SORT_* */
   int32_t reserved0;      /* 0 */
+  double step_tolerance_mm; /* > 0: adaptive number of primary RKN steps per leg ("adaptive"): the
+                             embedded error estimate eps0 = h^2 |k1-k2-k3+k4|_1 of one trial step over the whole leg
+                             gives n = ceil((eps0 / tolerance)^(1/4)) primary steps (at least what max_step_mm asks
+                             for, at most KF_MAX_SUBSTEPS), decided once per leg, no accept/reject loop.
+                             <= 0 or inf (default 0): off */
   /* perigee surface (used only when kf_outputs.perigee_params is given): the straight line
    * through perigee_center with UNIT direction perigee_axis (the beam axis; default origin, +z) */
   double perigee_center[3];
@@ -194,7 +199,7 @@ typedef struct kf_outputs {
 } kf_outputs;
 
 /* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
- * muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis through the origin. */
+ * no step tolerance, muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis through the origin. */
 void kf_default_options(kf_options* opt);
 
 /* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =

@@ -365,7 +365,7 @@ struct BoundJacobian {
 // the predicted (phi, theta), taken from the direction vector itself.  Returns 0 or the stopping bit.
 template <int FIELD>
 __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, int n_corr,
-                                              double max_step, const double* __restrict__ sf,
+                                              double max_step, double step_tol, const double* __restrict__ sf,
                                               const double* __restrict__ st, const double x[6],
                                               double trig[4], double xo[6], BoundJacobian& J,
                                               double& errmax, unsigned& status) {
@@ -390,13 +390,37 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
   int n_sub = 1;
   double nT = dot(nt, T);
   if (!(nT > kNdotTMin)) return ST_PROPAGATION;
-  if (max_step > 0.0) {
+  if (max_step > 0.0 || step_tol > 0.0) {
     const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
     const double s0 = dot(nt, dr) / nT;
-    double qn = ceil(fabs(s0) / max_step * (1.0 - 1e-12));
-    if (!(qn >= 1.0)) qn = 1.0;
-    if (qn > 1024.0) qn = 1024.0;
-    n_sub = (int)qn;
+    if (max_step > 0.0) {
+      double qn = ceil(fabs(s0) / max_step * (1.0 - 1e-12));
+      if (!(qn >= 1.0)) qn = 1.0;
+      if (qn > 1024.0) qn = 1024.0;
+      n_sub = (int)qn;
+    }
+    if (step_tol > 0.0) {
+      // adaptive step count (U31): the embedded error estimate of ONE trial step over the
+      // whole leg fixes the number of primary steps, n = ceil((eps0 / tol)^(1/4)); the trial step is discarded
+      double e0;
+      if constexpr (FIELD == FIELD_CONST) {
+        // closed form of h^2 |k1 - k2 - k3 + k4|_1 in a constant field (const_field_step)
+        const double u = s0 * lam, sq = u * u * F.b2;
+        double w1[3], w2[3];
+        cross(T, F.b, w1);
+        cross(w1, F.b, w2);
+        e0 = s0 * s0 * fabs(lam) * 0.25 * sq *
+             (fabs(fma(u, w2[0], w1[0])) + fabs(fma(u, w2[1], w1[1])) + fabs(fma(u, w2[2], w1[2])));
+      } else {
+        double rr[3] = {r[0], r[1], r[2]}, TT[3] = {T[0], T[1], T[2]}, tt = t;
+        double A[9], a[3], Bm[9], b[3], tau;
+        rkn4_step<FIELD>(F, dtds, tfac, rr, tt, TT, lam, s0, A, a, Bm, b, tau, e0, status);
+      }
+      double qn = ceil(sqrt(sqrt(e0 / step_tol)) * (1.0 - 1e-12));
+      if (!(qn >= 1.0)) qn = 1.0;
+      if (qn > 1024.0) qn = 1024.0;
+      if ((int)qn > n_sub) n_sub = (int)qn;
+    }
   }
   const int n_steps = n_sub + n_corr;
   typename std::conditional<FIELD == FIELD_CONST, PolyJac, MatJac>::type D;

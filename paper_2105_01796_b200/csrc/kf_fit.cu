@@ -232,6 +232,7 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   P.output_states = op->output_states;
   P.outlier_chi2 = op->outlier_chi2;
   P.max_step = (op->max_step_mm > 0.0 && std::isfinite(op->max_step_mm)) ? op->max_step_mm : 0.0;
+  P.step_tol = (op->step_tolerance_mm > 0.0 && std::isfinite(op->step_tolerance_mm)) ? op->step_tolerance_mm : 0.0;
   P.inflation = op->cov_inflation;
   P.first_params = out->first_params; P.first_cov = out->first_cov;
   P.last_params = out->last_params; P.last_cov = out->last_cov;

@@ -66,7 +66,7 @@ struct FitParams {
   MaterialDesc mat;
   // options
   int smooth, n_corr, output_states;
-  double outlier_chi2, max_step, inflation;
+  double outlier_chi2, max_step, step_tol, inflation;
   // outputs
   double *first_params, *first_cov, *last_params, *last_cov, *chi2;
   int *ndf, *n_used, *n_outliers, *n_holes;
@@ -216,7 +216,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     }
     double xp[6];
     BoundJacobian J;
-    const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, sf, st, x, trig,
+    const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, P.step_tol, sf, st, x, trig,
                                          xp, J, errmax, status);
     if (rc) {
       status |= rc;

@@ -104,6 +104,20 @@ def test_perigee_axis_must_be_a_unit_vector():
     assert e.value.rc == -1
 
 
+# ---- adaptive step count (kf_options.step_tolerance_mm, U31) ----------------------------------------
+@pytest.mark.parametrize("cfg,n,tol", [(1, 4001, 1e-5), (1, 4001, 1e-8), (4, 3001, 1e-6), (2, 2001, 1e-9)])
+def test_adaptive_step_count_parity(cfg, n, tol, variant):
+    """tracks of one warp take different numbers of primary steps (0.5-10 GeV: 1 to 4 at 1e-5); constant field
+    (closed-form estimate in the kernel) and grid field (trial step), both variants."""
+    wl = W.make_config(cfg, n_tracks=n, seed=70 + cfg)
+    ref = oracle.fit_workload(wl, states=True, step_tolerance_mm=tol)
+    got = kf.fit_workload(wl, states=True, step_tolerance_mm=tol, variant=variant)
+    parity.assert_parity(got, ref, states=True, label=f"adaptive cfg{cfg} tol={tol}")
+    np.testing.assert_allclose(got.rk_err_max, ref.rk_err_max, rtol=1e-6, atol=1e-18)
+    base = oracle.fit_workload(wl)
+    assert ref.rk_err_max.max() < 0.2 * base.rk_err_max.max()  # the option did change the stepping
+
+
 # ---- length sort of ragged batches (kf_sort.cuh): same results, track by track -------------------------------
 @pytest.mark.parametrize("cfg,n", [(3, 5003), (4, 5003), (4, 129), (2, 1000), (4, 9001)])
 def test_length_sort_parity_all_states(cfg, n, variant):
@@ -189,7 +203,8 @@ def test_runs_are_bitwise_deterministic():
 @pytest.mark.parametrize("over", [
     dict(n_corr_steps=0), dict(n_corr_steps=1), dict(n_corr_steps=3), dict(max_step_mm=7.0),
     dict(max_step_mm=11.0, n_corr_steps=1), dict(cov_inflation=10.0), dict(smooth=0), dict(material=0),
-    dict(outlier_chi2=6.0), dict(mass_gev=0.13957), dict(outlier_chi2=0.0),
+    dict(outlier_chi2=6.0), dict(mass_gev=0.13957), dict(outlier_chi2=0.0), dict(step_tolerance_mm=1e-7),
+    dict(step_tolerance_mm=1e-5, max_step_mm=20.0, n_corr_steps=1),
 ])
 def test_options_parity(over):
     wl = W.make_config(3, n_tracks=2051, seed=77)
