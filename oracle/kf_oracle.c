@@ -65,9 +65,8 @@ static int all_finite(const double* a, int n) {
     if (!isfinite(a[i])) return 0;
   return 1;
 }
-static double wrap_pi(double a) { /* into (-pi, pi] */
-  while (a > PI) a -= 2.0 * PI;
-  while (a <= -PI) a += 2.0 * PI;
+static double wrap_pi(double a) { /* into (-pi, pi]: a - 2 pi ceil((a - pi) / (2 pi)); NaN for a non-finite a */
+  if (a > PI || a <= -PI) a = a - (2.0 * PI) * ceil((a - PI) / (2.0 * PI));
   return a;
 }
 

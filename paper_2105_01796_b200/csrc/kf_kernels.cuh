@@ -461,8 +461,7 @@ __device__ __forceinline__ bool rts_step_pre(double* R1, const double xs[6], con
   }
 #pragma unroll
   for (int j = 0; j < 6; ++j) dx[j] = xs[j] - KF_R(R1, kRecXp + j);
-  if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
-  else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+  dx[2] = wrap_pi(dx[2]);
   return ok;
 }
 
@@ -785,8 +784,7 @@ kf_rts_lanes_kernel(const __grid_constant__ FitParams P) {
       double dx[6];
 #pragma unroll
       for (int j = 0; j < 6; ++j) dx[j] = xs[j] - R1[kRecXp + j];
-      if (dx[2] > kPi) dx[2] -= 2.0 * kPi;
-      else if (dx[2] <= -kPi) dx[2] += 2.0 * kPi;
+      dx[2] = wrap_pi(dx[2]);
 
       // this lane's row of C+ and of W = C+ F^T
       double cr[6], W[6];

@@ -1,0 +1,155 @@
+"""Randomised parity of the CUDA path with the oracle: random telescopes (spacing, tilt, material per plane),
+field directions and strengths (and a random 3-D grid), momenta, hole patterns, outliers, per-hit covariances,
+every option of kf_options, both kernel variants, sorted and unsorted, with the perigee on a random axis.
+Each seed is one configuration; the bars are those of tests/parity.py.  `pytest -m gpu`."""
+import numpy as np
+import pytest
+
+import oracle
+import parity
+import paper_2105_01796_b200 as kf
+from paper_2105_01796_b200 import binding as B
+
+pytestmark = pytest.mark.gpu
+
+
+def random_geometry(rng, L):
+    g = np.zeros((L + 1, 20))
+    x = 0.0
+    for k in range(L + 1):
+        a, b = rng.uniform(-0.15, 0.15, 2) if k else (0.0, 0.0)
+        u = np.array([-np.sin(a), np.cos(a), 0.0])
+        v = np.array([-np.sin(b) * np.cos(a), -np.sin(b) * np.sin(a), np.cos(b)])
+        v -= u * (u @ v)
+        v /= np.linalg.norm(v)
+        g[k, 0:3] = (x, rng.uniform(-2, 2), rng.uniform(-2, 2))
+        g[k, 3:6], g[k, 6:9], g[k, 9:12] = u, v, np.cross(u, v)
+        g[k, 12:14] = 50.0
+        if k and rng.random() < 0.7:
+            g[k, 14] = rng.uniform(5e-4, 1e-2)
+            g[k, 15] = g[k, 14] * 93.7
+        g[k, 16:18] = rng.uniform(0.005, 0.05, 2) ** 2
+        x += rng.uniform(12.0, 55.0)
+    return g
+
+
+def random_case(seed):
+    rng = np.random.default_rng(1000 + seed)
+    L = int(rng.integers(3, 36))
+    N = int(rng.integers(40, 700))
+    geom = random_geometry(rng, L)
+    start = int(rng.integers(0, min(3, L - 2)))
+    kind = rng.choice(["const", "zero", "grid3"], p=[0.55, 0.15, 0.3])
+    if kind == "grid3":
+        n = np.array([int(rng.integers(8, 20)), int(rng.integers(5, 9)), int(rng.integers(5, 9))])
+        origin = np.array([-20.0, -60.0, -60.0])
+        spacing = np.array([(geom[-1, 0] * rng.uniform(0.5, 1.1) + 40.0) / (n[0] - 1), 120.0 / (n[1] - 1), 120.0 / (n[2] - 1)])
+        grid = rng.uniform(-0.3, 0.3, (n[2], n[1], n[0], 3))
+        grid[..., 2] += rng.uniform(1.0, 2.5)
+        field = dict(field_kind="grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+        fld = oracle.make_field("grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+    else:
+        b = (0.0, 0.0, 0.0) if kind == "zero" else tuple(rng.uniform(-0.5, 0.5, 2)) + (rng.choice([-1, 1]) * rng.uniform(0.5, 3.0),)
+        field = dict(field_kind="const", field_b=b)
+        fld = oracle.make_field("const", b)
+    p = np.exp(rng.uniform(np.log(0.4), np.log(60.0), N))
+    x0 = np.stack([rng.uniform(-4, 4, N), rng.uniform(-4, 4, N), rng.uniform(-0.12, 0.12, N),
+                   np.pi / 2 + rng.uniform(-0.12, 0.12, N), rng.choice([-1.0, 1.0], N) / p, rng.uniform(0, 50, N)], axis=1)
+    sig = np.array([0.1, 0.1, 2e-3, 2e-3, 0.0, 300.0])[None, :].repeat(N, 0)
+    sig[:, 4] = 0.03 * np.abs(x0[:, 4])
+    R = rng.uniform(-0.3, 0.3, (6, 6))
+    corr = R @ R.T * 0.2 + np.eye(6)
+    d = np.sqrt(np.diag(corr))
+    corr = corr / np.outer(d, d)
+    cov0 = corr[None] * sig[:, :, None] * sig[:, None, :]
+    opts = dict(smooth=int(rng.random() < 0.8), material=int(rng.random() < 0.7),
+                outlier_chi2=float(rng.choice([0.0, 9.0, 15.0, 30.0])), n_corr_steps=int(rng.integers(0, 4)),
+                max_step_mm=float(rng.choice([np.inf, np.inf, 25.0, 9.0])),
+                step_tolerance_mm=float(rng.choice([0.0, 0.0, 1e-5, 1e-8])), mass_gev=float(rng.choice([0.1056583755, 0.13957, 0.4937])),
+                cov_inflation=float(rng.choice([1.0, 1.0, 4.0, 100.0])))
+    # noise hits far from the track only when the cut that is there to catch them is on: a 40 mm mistake taken at
+    # 15 um resolution throws the extended filter into a regime where round-off is amplified without bound
+    p_noise = 0.03 if opts["outlier_chi2"] > 0.0 else 0.0
+    # truth hits: the start state taken plane to plane by the step-level oracle (input generation only)
+    opt0 = oracle.make_options()
+    offsets, surf, loc, lens = [0], [], [], []
+    eff = rng.uniform(0.75, 1.0)
+    for i in range(N):
+        x = x0[i].copy()
+        stop = int(rng.integers(start + 1, L + 1)) if rng.random() < 0.4 else L
+        for k in range(start, stop):
+            pr = oracle.propagate(fld, opt0, x, geom[k], geom[k + 1])
+            if pr.rc != 0:
+                break
+            x = pr.x
+            if rng.random() < eff:
+                m = x[:2] + rng.standard_normal(2) * np.sqrt(geom[k + 1, 16:18])
+                if rng.random() < p_noise:
+                    m = rng.uniform(-40, 40, 2)
+                surf.append(k + 1)
+                loc.append(m)
+        offsets.append(len(surf))
+    M = len(surf)
+    var = cov01 = None
+    if rng.random() < 0.35:
+        var = rng.uniform(0.005, 0.05, (M, 2)) ** 2
+        if rng.random() < 0.5:
+            cov01 = rng.uniform(-0.5, 0.5, M) * np.sqrt(var[:, 0] * var[:, 1])
+    params0 = x0 + rng.standard_normal((N, 6)) * sig * 0.7
+    ax = np.array([rng.uniform(-0.2, 0.2), rng.uniform(-0.2, 0.2), 1.0])
+    line = (tuple(rng.uniform(-3, 3, 3)), tuple(ax / np.linalg.norm(ax)))
+    return dict(params0=params0, cov0=cov0, start=start, offsets=np.array(offsets, np.int32), surf_idx=np.array(surf, np.int32),
+                loc=np.array(loc).reshape(-1, 2), geom=geom, var=var, cov01=cov01, field=field, fld=fld, opts=opts, line=line)
+
+
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("KF_FUZZ_SEEDS", "48"))))
+def test_random_configuration_parity(seed):
+    c = random_case(seed)
+    opt = oracle.make_options(**c["opts"])
+    ref = oracle.fit_batch(c["params0"], c["cov0"], c["start"], c["offsets"], c["surf_idx"], c["loc"], c["geom"], c["fld"],
+                           opt, var=c["var"], cov01=c["cov01"], states=True)
+    oracle.perigee_batch(ref, c["geom"], c["start"], c["fld"], opt, *c["line"])
+    hb = kf.HostBatch.from_arrays(c["params0"], c["cov0"], c["start"], c["offsets"], c["surf_idx"], c["loc"], c["geom"],
+                                  var=c["var"], cov01=c["cov01"], options=c["opts"], **c["field"])
+    smooth = c["opts"]["smooth"]
+    states = B.STATES_PRED | B.STATES_FILT | (B.STATES_SMOOTH if smooth else 0)
+    # a 100x inflated prior makes the first legs' covariances ill-conditioned: wider bars there
+    loosen = 1.0 if c["opts"]["cov_inflation"] <= 4.0 else 50.0
+    # The gain form C+ = (I - K H) C- (reading U18) cancels kappa = C-_ii / C+_ii leading digits: a precise hit after a
+    # long blind extrapolation (holes + material at low momentum: sigma 40 mm against 15 um, kappa 7e6) leaves a
+    # rounding difference of ~30 eps kappa between any two orderings of the same formula.  Tracks with kappa > 1e5
+    # are compared with bars widened in proportion; everything else keeps the north_star bars.
+    with np.errstate(invalid="ignore", divide="ignore"):
+        dP = np.einsum("nlii->nli", ref.pred_cov)[..., :2] / np.einsum("nlii->nli", ref.filt_cov)[..., :2]
+    kappa = np.nan_to_num(np.nanmax(np.where(np.isfinite(dP), dP, 0.0), axis=(1, 2)), nan=0.0)
+    # a fit that ran away (predicted positions or their errors of metres on +-50 mm planes: a low-momentum track that
+    # the hits stopped constraining) has no digits to compare
+    with np.errstate(invalid="ignore"):
+        far = np.nan_to_num(np.abs(ref.pred_params[..., :2]), nan=0.0, posinf=1e99).max(axis=(1, 2)) > 200.0
+        wide = np.nan_to_num(np.einsum("nlii->nli", ref.pred_cov)[..., :2], nan=0.0, posinf=1e99).max(axis=(1, 2)) > 1e4
+        odd = ~np.all(np.isfinite(np.nan_to_num(ref.last_params, nan=0.0)), axis=1)
+    runaway = far | wide | odd
+    for variant in (B.VARIANT_THREAD_PER_TRACK, B.VARIANT_LANES_PER_TRACK):
+        for sort in (B.SORT_OFF, B.SORT_ON):
+            db = kf.DeviceBatch(hb)
+            out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, states, perigee=True)
+            call = kf.FitCall(db, out=out, perigee=c["line"], variant=variant, length_sort=sort, output_states=states)
+            got = call.run().to_host()
+            label = f"seed {seed} variant {variant} sort {sort} opts {c['opts']}"
+            # integers, flags and status: exact on every track that stayed a track.  On a runaway track the stopping
+            # reason is the sign of det S or of a pivot of a numerically singular matrix (a last leg with sigma(loc) of
+            # 280 m and smallest correlation eigenvalue -5e-17 was seen): the one discrete decision that round-off may
+            # flip (SURVEY.md 8(c) C.5 lists such flips instead of hiding them)
+            keep_hits = np.repeat(~runaway, np.diff(c["offsets"]))
+            for name in ("ndf", "n_used", "n_outliers", "n_holes"):
+                np.testing.assert_array_equal(getattr(got, name)[~runaway], getattr(ref, name)[~runaway], err_msg=label + " " + name)
+            np.testing.assert_array_equal(got.hit_flags[keep_hits], ref.hit_flags[keep_hits], err_msg=label + " hit_flags")
+            np.testing.assert_array_equal(got.status[~runaway], ref.status[~runaway], err_msg=label)
+            np.testing.assert_array_equal(got.status[runaway] & np.uint32(64), ref.status[runaway] & np.uint32(64), err_msg=label)
+            # values: every track that stayed a track, with the north_star bars where the updates are well conditioned
+            well = ~runaway & (kappa <= 1e5)
+            parity.assert_parity(got, ref, states=True, sel=well, loosen=loosen, label=label)
+            ill = ~runaway & ~(kappa <= 1e5)
+            if np.any(ill):
+                parity.assert_parity(got, ref, states=True, sel=ill, loosen=loosen * 1e3 * kappa[ill].max() / 1e5,
+                                     label=label + " (ill-conditioned updates)")

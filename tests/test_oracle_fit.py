@@ -343,3 +343,32 @@ def test_subset_reproduces_per_track_results():
     np.testing.assert_array_equal(a.first_params[idx], b.first_params)
     np.testing.assert_array_equal(a.chi2[idx], b.chi2)
     np.testing.assert_array_equal(a.status[idx], b.status)
+
+
+def test_rts_phi_difference_is_wrapped_over_any_number_of_turns():
+    """x^s_{k+1} - x^-_{k+1} in phi is an angle difference: taken into (-pi, pi] (DESIGN.md A.7), whatever the number
+    of turns between the two representations (a far-off hit that is not cut can turn the filtered phi by more than
+    one), and a non-finite state ends the step instead of hanging it."""
+    rng = np.random.default_rng(3)
+    A = rng.standard_normal((6, 6)) * 0.1
+    Cf = A @ A.T + np.eye(6) * 0.05
+    F = np.eye(6) + rng.standard_normal((6, 6)) * 0.05
+    Cp1 = F @ Cf @ F.T + np.eye(6) * 0.01
+    xf, xp1 = rng.standard_normal(6), rng.standard_normal(6)
+    xs1 = xp1 + rng.standard_normal(6) * 0.1
+    Cs1 = Cp1 * 0.9
+    rc0, x0, C0 = oracle.rts_step(xf, Cf, F, xp1, Cp1, xs1, Cs1)
+    assert rc0 == 0
+    for turns in (1, -1, 3, -5, 1000):
+        shifted = xs1.copy()
+        shifted[2] += 2 * np.pi * turns
+        rc, x, C = oracle.rts_step(xf, Cf, F, xp1, Cp1, shifted, Cs1)
+        assert rc == 0
+        np.testing.assert_allclose(x, x0, rtol=0, atol=1e-9 * abs(turns))
+        np.testing.assert_array_equal(C, C0)
+    bad = xs1.copy()
+    bad[2] = np.inf
+    rc, x, C = oracle.rts_step(xf, Cf, F, xp1, Cp1, bad, Cs1)
+    assert rc != 0
+    bad[2] = 1e300
+    rc, x, C = oracle.rts_step(xf, Cf, F, xp1, Cp1, bad, Cs1)  # returns (the loop form never did)
