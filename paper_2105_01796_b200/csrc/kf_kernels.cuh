@@ -44,6 +44,13 @@ constexpr size_t kLegBytes = (size_t)kRecDoubles * KF_TILE * sizeof(double) + KF
 #define KF_RTS_MIN_BLOCKS 1
 #endif
 
+// record stores: written once, read much later by the RTS kernel -> streaming stores (evict-first in L2), so that
+// 13 GB of records passing through do not push the field grid and the hit lists out of L2
+#ifdef KF_REC_PLAIN_STORES
+#define KF_REC_STORE(ptr, v) (*(ptr) = (v))
+#else
+#define KF_REC_STORE(ptr, v) __stcs((ptr), (v))
+#endif
 enum : int { OUT_PRED = 1, OUT_FILT = 2, OUT_SMOOTH = 4 };
 
 struct FitParams {
@@ -228,17 +235,17 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth && lead) {
 #pragma unroll
-      for (int k = 0; k < 6; ++k) R[(kRecXp + k) * KF_TILE] = xp[k];
+      for (int k = 0; k < 6; ++k) KF_REC_STORE(&R[(kRecXp + k) * KF_TILE], xp[k]);
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) R[(kRecFa + a * 5 + c) * KF_TILE] = J.Ja[a][c];
-        R[(kRecFa + a * 5 + 4) * KF_TILE] = J.Ja[a][4] * g_prev;
+        for (int c = 0; c < 4; ++c) KF_REC_STORE(&R[(kRecFa + a * 5 + c) * KF_TILE], J.Ja[a][c]);
+        KF_REC_STORE(&R[(kRecFa + a * 5 + 4) * KF_TILE], J.Ja[a][4] * g_prev);
       }
 #pragma unroll
-      for (int c = 0; c < 4; ++c) R[(kRecFt + c) * KF_TILE] = J.Jt[c];
-      R[(kRecFt + 4) * KF_TILE] = J.Jt[4] * g_prev;
-      R[kRecG * KF_TILE] = g_prev;
+      for (int c = 0; c < 4; ++c) KF_REC_STORE(&R[(kRecFt + c) * KF_TILE], J.Jt[c]);
+      KF_REC_STORE(&R[(kRecFt + 4) * KF_TILE], J.Jt[4] * g_prev);
+      KF_REC_STORE(&R[kRecG * KF_TILE], g_prev);
     }
     if (mat_here) material_apply(ms, C);
     double Cp[21];
@@ -254,9 +261,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 
     if (P.smooth && lead) {
 #pragma unroll
-      for (int k = 0; k < 21; ++k) R[(kRecCp + k) * KF_TILE] = Cp[k];
-      R[kRecM * KF_TILE] = m0;
-      R[(kRecM + 1) * KF_TILE] = m1;
+      for (int k = 0; k < 21; ++k) KF_REC_STORE(&R[(kRecCp + k) * KF_TILE], Cp[k]);
+      KF_REC_STORE(&R[kRecM * KF_TILE], m0);
+      KF_REC_STORE(&R[(kRecM + 1) * KF_TILE], m1);
     }
 
     // gain-matrix update with the surface's hit.  A hole or a flagged outlier runs the
