@@ -225,8 +225,8 @@ int kf_fit_batch_host(const kf_tracks_in* tracks, const kf_measurements* meas, c
                       void* device_arena, size_t arena_bytes, void* cuda_stream);
 
 /* The same with the copies and the fit of different track ranges overlapped (the paper's multi-stream
- * offload): the tracks are cut into chunks of `chunk_tracks` (rounded up to whole
- * 128-track CTAs; 0 = max(16384, N / (4 n_streams))); chunk c runs its H2D copies, its forward and RTS
+ * offload): the tracks are cut into chunks of `chunk_tracks` (rounded up to a multiple of
+ * 128 tracks; 0 = max(16384, N / (4 n_streams))); chunk c runs its H2D copies, its forward and RTS
  * kernels and its D2H copies in order on streams[c % n_streams].  The whole call is ordered after the work
  * already enqueued on `cuda_stream`, and `cuda_stream` continues only after every chunk has finished
  * (fork/join through the caller-owned events, which need no timing).  All handles are caller-owned;

@@ -18,6 +18,9 @@
 
 namespace {
 
+// batches of more tracks than this take the 256-thread forward CTA (148 SMs x 2 CTAs x 128 threads = one wave)
+constexpr long long KF_FWD_BIG_MIN_TRACKS = 148LL * 2 * 128;
+
 thread_local char g_cuda_error[256] = "";
 thread_local int g_launches = 0;
 thread_local cudaEvent_t g_stage_events[3] = {nullptr, nullptr, nullptr};
@@ -32,6 +35,10 @@ inline size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // Workspace: tile-major RTS records and the per-slot leg counts (both only
 // when smoothing), then the length sort's slot -> track permutation and its bin counters (one set of
 // kSortBins counters per 128 tracks, so that every pipeline chunk has its own).
+// pipeline chunks are whole multiples of this many tracks (two record tiles); one set of sort counters per unit
+constexpr int kChunkTracks = 128;
+static_assert(kChunkTracks % KF_TILE == 0, "a chunk covers whole record tiles");
+
 struct WorkspaceLayout {
   size_t rec_off, nleg_off, perm_off, bins_off, total;
   size_t rec_total;   // bytes up to the end of the leg counts: what the fit cannot run without
@@ -55,7 +62,7 @@ WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth) {
   w.perm_off = off;
   off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
   w.bins_off = off;
-  off += align_up((size_t)((N + KF_FWD_BLOCK - 1) / KF_FWD_BLOCK) * kf::kSortBins * sizeof(int), 256);
+  off += align_up((size_t)((N + kChunkTracks - 1) / kChunkTracks) * kf::kSortBins * sizeof(int), 256);
   w.total = off;
   return w;
 }
@@ -253,7 +260,7 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
 }
 
 // The same block restricted to tracks [t0, t0 + n): every per-track base pointer advances by t0 (t0 is a
-// multiple of KF_FWD_BLOCK, so tiles stay whole); hit arrays keep their absolute indexing through `offsets`.
+// multiple of kChunkTracks, so tiles stay whole); hit arrays keep their absolute indexing through `offsets`.
 kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
   kf::FitParams P = F;
   P.N = n;
@@ -273,21 +280,25 @@ kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
 }
 
 // Enqueue the forward filter and, if asked for, the RTS pass over the tracks of P on `stream`.
-template <int LPT>
-int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t smem, cudaStream_t stream) {
+template <int LPT, int BLOCK>
+int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geom_smem, cudaStream_t stream) {
   using kf::FIELD_CONST;
   using kf::FIELD_GRID3;
+  size_t smem = geom_smem + kf::hit_stage_bytes(BLOCK);
+#ifdef KF_FWD_EXTRA_SMEM
+  smem += KF_FWD_EXTRA_SMEM;
+#endif
   const int sel = (grid3 ? 4 : 0) | (material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
   const char* nm = "kf_forward_kernel";
   switch (sel) {
-    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, false, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 2: return launch(kf::kf_forward_kernel<FIELD_CONST, true, false, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 3: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 4: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, false, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
-    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT>, P, KF_FWD_BLOCK, smem, stream, nm, LPT);
+    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, false, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 2: return launch(kf::kf_forward_kernel<FIELD_CONST, true, false, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 3: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 4: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, false, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
+    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT, BLOCK>, P, BLOCK, smem, stream, nm, LPT);
   }
 }
 
@@ -317,15 +328,14 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   }
   const bool lanes = variant == KF_VARIANT_LANES_PER_TRACK || (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS);
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
-  size_t fwd_smem = geom_smem + kf::kHitStageBytes;
-#ifdef KF_FWD_EXTRA_SMEM
-  fwd_smem += KF_FWD_EXTRA_SMEM;
-#endif
   const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
   int rc;
   record_stage(0, stream);
-  rc = lanes ? launch_forward<kf::kLanes>(P, grid3, material, fwd_smem, stream)
-             : launch_forward<1>(P, grid3, material, fwd_smem, stream);
+  // 256-thread forward CTAs once a constant-field batch is more than one wave of 128-thread CTAs at two per SM
+  // (CFG2 3.47 -> 3.40 ms; the grid-field kernel, at 255 registers with spills, is slower that way: CFG4 5.87 -> 6.11 ms)
+  if (lanes) rc = launch_forward<kf::kLanes, KF_FWD_BLOCK_SMALL>(P, grid3, material, geom_smem, stream);
+  else if (!grid3 && P.N > KF_FWD_BIG_MIN_TRACKS) rc = launch_forward<1, KF_FWD_BLOCK>(P, grid3, material, geom_smem, stream);
+  else rc = launch_forward<1, KF_FWD_BLOCK_SMALL>(P, grid3, material, geom_smem, stream);
   if (rc != KF_OK) return rc;
   record_stage(1, stream);
   if (P.smooth) {
@@ -354,7 +364,7 @@ SortPlan sort_for_range(const SortPlan& whole, const kf_options* op, long long t
   const bool ragged = n_hits != n * (long long)lmax;
   if (op->length_sort == KF_SORT_ON || (op->length_sort == KF_SORT_AUTO && ragged && n >= KF_AUTO_SORT_MIN_TRACKS)) {
     r.perm = whole.perm + t0;
-    r.bins = whole.bins + (t0 / KF_FWD_BLOCK) * kf::kSortBins;
+    r.bins = whole.bins + (t0 / kChunkTracks) * kf::kSortBins;
   }
   return r;
 }
@@ -581,7 +591,7 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
   long long chunk = N;
   if (pipe) {
     chunk = pipe->chunk_tracks > 0 ? pipe->chunk_tracks : std::max<long long>(16384, N / (4LL * S));
-    chunk = (chunk + KF_FWD_BLOCK - 1) / KF_FWD_BLOCK * KF_FWD_BLOCK;  // whole forward CTAs (and record tiles)
+    chunk = (chunk + kChunkTracks - 1) / kChunkTracks * kChunkTracks;  // whole record tiles
     KF_TRY(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[S]), main), "pipeline fork");
     for (int k = 0; k < S; ++k)
       KF_TRY(cudaStreamWaitEvent(static_cast<cudaStream_t>(pipe->streams[k]), static_cast<cudaEvent_t>(pipe->events[S]), 0),

@@ -32,10 +32,16 @@ constexpr int kRecXp = 0, kRecCp = 6, kRecFa = 27, kRecFt = 47, kRecG = 52, kRec
 #ifndef KF_TILE
 #define KF_TILE 64
 #endif
+// threads per forward CTA: KF_FWD_BLOCK for batches that fill the chip more than once (measured on CFG2: 256
+// threads 3.38-3.40 ms, 128 threads 3.46-3.48 ms), KF_FWD_BLOCK_SMALL for smaller ones and for the lanes variant
+// (more CTAs, so more SMs take part while a batch is latency-bound)
 #ifndef KF_FWD_BLOCK
-#define KF_FWD_BLOCK 128
+#define KF_FWD_BLOCK 256
 #endif
-static_assert(KF_FWD_BLOCK % KF_TILE == 0 && KF_TILE % 32 == 0, "a forward CTA covers whole tiles; a tile covers whole warps");
+#ifndef KF_FWD_BLOCK_SMALL
+#define KF_FWD_BLOCK_SMALL 128
+#endif
+static_assert(KF_FWD_BLOCK % KF_TILE == 0 && KF_FWD_BLOCK_SMALL % KF_TILE == 0 && KF_TILE % 32 == 0, "a forward CTA covers whole tiles; a tile covers whole warps");
 constexpr size_t kLegBytes = (size_t)kRecDoubles * KF_TILE * sizeof(double) + KF_TILE;  // record + flags
 #ifndef KF_FWD_MIN_BLOCKS
 #define KF_FWD_MIN_BLOCKS 1
@@ -117,7 +123,7 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // bytes of the forward kernel's hit staging area: two alternating slots of (loc0, loc1, surface) per thread
-constexpr size_t kHitStageBytes = (size_t)KF_FWD_BLOCK * (2 * 2 * sizeof(double) + 2 * sizeof(int));
+constexpr size_t hit_stage_bytes(int block) { return (size_t)block * (2 * 2 * sizeof(double) + 2 * sizeof(int)); }
 
 // stage the geometry table in shared memory once per CTA (5 KB for 31 planes)
 __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem) {
@@ -139,9 +145,10 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // variant ("intra-track parallelisation", NS "warp-cooperative lanes-per-track"): the 8 lanes
 // of a group run the scalar part of the leg redundantly (identical values, identical branches) and share the
 // 6x6 covariance transport row by row, exchanging the rows with warp shuffles; lane 0 of the group stores.
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT>
-__global__ void __launch_bounds__(KF_FWD_BLOCK, KF_FWD_MIN_BLOCKS)
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK>
+__global__ void __launch_bounds__(BLOCK, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
+  static_assert(BLOCK % KF_TILE == 0, "a forward CTA covers whole tiles");
   extern __shared__ double s_dyn[];
   const double* __restrict__ G;
   if constexpr (GEOM_SMEM) {
@@ -150,7 +157,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   } else {
     G = P.geom;
   }
-  const long long tslot = ((long long)blockIdx.x * KF_FWD_BLOCK + threadIdx.x) / LPT;
+  const long long tslot = ((long long)blockIdx.x * BLOCK + threadIdx.x) / LPT;
   if (tslot >= P.N) return;    // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
   const long long i = P.perm ? (long long)P.perm[tslot] : tslot;  // the track this slot fits
   const long long N = P.ldn;  // SoA stride
@@ -183,13 +190,13 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   }
   // the next unconsumed hit is fetched one leg ahead of its use into this thread's own shared-memory
   // slot (two alternating slots), asynchronously
-  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][KF_FWD_BLOCK]
-  int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * KF_FWD_BLOCK) + threadIdx.x;  // [slot][KF_FWD_BLOCK]
+  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][BLOCK]
+  int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * BLOCK) + threadIdx.x;  // [slot][BLOCK]
   int slot = 0;
   auto fetch_hit = [&](int j, int sl) {
-    cp_async4(s_hs + sl * KF_FWD_BLOCK, P.surf_idx + j);
-    cp_async8(s_hm + (sl * 2 + 0) * KF_FWD_BLOCK, P.loc + j);
-    cp_async8(s_hm + (sl * 2 + 1) * KF_FWD_BLOCK, P.loc + P.ldm + j);
+    cp_async4(s_hs + sl * BLOCK, P.surf_idx + j);
+    cp_async8(s_hm + (sl * 2 + 0) * BLOCK, P.loc + j);
+    cp_async8(s_hm + (sl * 2 + 1) * BLOCK, P.loc + P.ldm + j);
     cp_async_commit();
   };
   if (o0 < o1) fetch_hit(o0, 0);
@@ -254,9 +261,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 
     // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
     cp_async_wait_all();
-    const bool has_hit = hp < o1 && s_hs[slot * KF_FWD_BLOCK] == s;
-    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * KF_FWD_BLOCK] : 0.0;
-    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * KF_FWD_BLOCK] : 0.0;
+    const bool has_hit = hp < o1 && s_hs[slot * BLOCK] == s;
+    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * BLOCK] : 0.0;
+    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * BLOCK] : 0.0;
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth && lead) {
