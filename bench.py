@@ -62,6 +62,9 @@ def parse_args():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", default="auto", choices=["auto", "thread", "lanes"],
                     help="kernel variant (kf_options.variant): thread per track or 8 lanes per track")
+    ap.add_argument("--smoother", default="rts", choices=["rts", "bf"],
+                    help="backward pass (kf_options.smoother): Rauch-Tung-Striebel (default, the north_star's) or the "
+                         "Bryson-Frazier form of the same smoothed state (42-double records, no 6x6 solve)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -206,7 +209,8 @@ def main():
     hb = kf.HostBatch.from_workload(wl)
     db = kf.DeviceBatch(hb, dev)
     variant = {"auto": 0, "thread": 1, "lanes": 2}[args.variant]
-    call = kf.FitCall(db, variant=variant)  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
+    bf = args.smoother == "bf"
+    call = kf.FitCall(db, variant=variant, smoother=int(bf))  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -264,17 +268,35 @@ def main():
             barrier()
             return replicas.max_over_ranks(h0.elapsed_time(h1), dist, dev) / ke, ke
         # the public host-buffer call: chunks of 65,536 tracks over 3 streams (H2D, fit and D2H of different chunks overlap)
-        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536)
+        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf))
         ms_e2e, ke = time_host(hc)
         e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
                    d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke, launches_per_step=int(hc.launches),
                    api="kf_fit_batch_host_pipelined (pinned host buffers; chunks of 65536 tracks on 3 streams: "
                        "H2D, forward, RTS, D2H per chunk)")
         del hc
-        hc = kf.HostCall(hb, dev)  # context: the same through kf_fit_batch_host, everything in order on one stream
+        hc = kf.HostCall(hb, dev, smoother=int(bf))  # context: the same through kf_fit_batch_host, everything in order on one stream
         ms_one, _ = time_host(hc)
         e2e["single_stream_ms_per_step"] = ms_one
         del hc
+
+    # ---- context: the same step with the backward pass in Bryson-Frazier form (kf_options.smoother) --------------------
+    alt = None
+    if smooth and not bf and args.config == 2 and not args.no_e2e:
+        call2 = kf.FitCall(db, variant=variant, smoother=1)
+        for _ in range(3):
+            call2.run()
+        barrier()
+        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a0.record()
+        for _ in range(args.steps):
+            call2.run()
+        a1.record()
+        barrier()
+        v2, ms2, _ = replicas.job_throughput(N * args.steps, a0.elapsed_time(a1), dist, dev)
+        alt = dict(smoother="bryson-frazier (same smoothed first state, 42-double records, no 6x6 solve; an option, "
+                            "not the north_star's RTS form)", value=v2, unit=UNIT, ms_per_step=ms2 / args.steps)
+        del call2
 
     if rank != 0:
         if dist is not None:
@@ -285,9 +307,12 @@ def main():
     fwd = float(np.mean(fwd_ms))
     rts = float(np.mean(rts_ms)) if smooth else 0.0
     fkind = hb.field_kind
-    rec_b = REC_BYTES if smooth else 0
+    rec_b = (42 * 8 if bf else REC_BYTES) if smooth else 0   # Bryson-Frazier record: 42 doubles, no flag byte
     fwd_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 8) + N * (2 * 27 * 8 + 8 + 5 * 4) + M * 9
     rts_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 12)
+    if bf:  # no hits re-read; the first-leg block (27 doubles) read, first_* written
+        rts_bytes = n_legs * rec_b + N * (27 * 8 + 27 * 8 + 8)
+        fwd_bytes += N * 27 * 8
     fwd_flop = n_legs * FWD_FLOP_PER_LEG[fkind]
     rts_flop = n_legs * RTS_FLOP_PER_LEG
     fp64_peak = 148 * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
@@ -300,7 +325,7 @@ def main():
                     fp64_tflops=flop / (ms * 1e-3) / 1e12, fp64_frac=flop / (ms * 1e-3) / 1e12 / fp64_peak)
 
     kf_fwd = kernel_roof("kf_forward_kernel", fwd, fwd_bytes, fwd_flop)
-    kf_rts = kernel_roof("kf_rts_kernel", rts, rts_bytes, rts_flop) if smooth else None
+    kf_rts = kernel_roof("kf_mbf_kernel" if bf else "kf_rts_kernel", rts, rts_bytes, rts_flop) if smooth else None
     dom = kf_fwd if (kf_rts is None or fwd >= rts) else kf_rts
     # the dominant kernel's own bound: the larger of its two fractions says which roof it is nearer
     if dom["fp64_frac"] >= dom["hbm_frac"]:
@@ -311,7 +336,7 @@ def main():
     else:
         roofline = dict(bound="hbm", achieved=dom["hbm_gbs"], peak=hbm_peak, unit="GB/s", frac=dom["hbm_frac"],
                         traffic=None, kernel=dom["kernel"], peak_source=f"MEASURED_PEAKS.json ({peaks['source']})")
-    if args.config == 2 and smooth:  # the capture is of this workload; other configs report null
+    if args.config == 2 and smooth and not bf:  # the capture is of this workload and of the RTS kernels; else null
         roofline["traffic"] = NCU_TRAFFIC["bytes_per_leg"][dom["kernel"]] * n_legs
         roofline["traffic_unit"] = "bytes per launch (ncu dram read+write per leg x legs of this launch)"
         roofline["traffic_source"] = NCU_TRAFFIC["source"]
@@ -329,10 +354,11 @@ def main():
                     layers=hb.n_surfaces - 1, field=fkind, smooth=int(smooth),
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
-                    parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant,
+                    parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant, smoother=args.smoother,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,
-        kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu)
+        kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu,
+        alt_smoother=alt)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

@@ -45,7 +45,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 104          /* major * 100 + minor */
+#define KF_VERSION 105          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -97,6 +97,16 @@ enum { KF_VARIANT_AUTO = 0, KF_VARIANT_THREAD_PER_TRACK = 1, KF_VARIANT_LANES_PE
  * ON: always sorted. */
 enum { KF_SORT_AUTO = 0, KF_SORT_OFF = 1, KF_SORT_ON = 2 };
 #define KF_AUTO_SORT_MIN_TRACKS 8192
+
+/* kf_options.smoother: how the backward pass reaches the smoothed state.
+ *   RTS  (default) the Rauch-Tung-Striebel recursion of PAPER.md:62, 75 with the stored Jacobians: one 6x6 SPD solve
+ *        per state; every per-leg smoothed state available (KF_STATES_SMOOTH).
+ *   BRYSON_FRAZIER  the same smoothed state at the first surface (first_*) from the adjoint recursion of the modified
+ *        Bryson-Frazier smoother: no 6x6 solve, 42-double records instead of 55, thread-per-track kernels only.
+ *        Agrees with RTS to round-off while kappa = C-_ii / C^s_ii stays moderate (1.6e3 on the configs); loses
+ *        kappa * 1e-16 relative to it (an inflated prior), so it is an option, not the default.  Not with
+ *        KF_STATES_SMOOTH, not with KF_VARIANT_LANES_PER_TRACK (KF_ERR_UNSUPPORTED). */
+enum { KF_SMOOTHER_RTS = 0, KF_SMOOTHER_BRYSON_FRAZIER = 1 };
 
 /* kf_options.output_states bitmask: which per-leg states to write to kf_outputs.state_* */
 enum { KF_STATES_PRED = 1, KF_STATES_FILT = 2, KF_STATES_SMOOTH = 4 };
@@ -158,7 +168,7 @@ typedef struct kf_options {
   int32_t output_states;  /* KF_STATES_* bitmask */
   int32_t variant;        /* KF_VARIANT_* */
   int32_t length_sort;    /* KF_SORT_* */
-  int32_t reserved0;      /* 0 */
+  int32_t smoother;       /* KF_SMOOTHER_* (used when smooth) */
   double step_tolerance_mm; /* > 0: adaptive number of primary RKN steps per leg ("adaptive"): the
                              embedded error estimate eps0 = h^2 |k1-k2-k3+k4|_1 of one trial step over the whole leg
                              gives n = ceil((eps0 / tolerance)^(1/4)) primary steps (at least what max_step_mm asks

@@ -15,6 +15,7 @@
 #include "kf_kernels.cuh"
 #include "kf_perigee.cuh"
 #include "kf_sort.cuh"
+#include "kf_mbf.cuh"
 
 namespace {
 
@@ -46,14 +47,16 @@ struct WorkspaceLayout {
   long long n_tiles;
 };
 
-WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth) {
+WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth, int mbf = 0) {
   WorkspaceLayout w{};
   w.n_tiles = N > 0 ? (N + KF_TILE - 1) / KF_TILE : 0;
   if (N <= 0 || n_legs_max <= 0) return w;
   size_t off = 0;
   if (smooth) {
     w.rec_off = off;
-    w.tile_stride = (size_t)n_legs_max * kf::kLegBytes;
+    // RTS: Lmax tile-legs of kLegBytes; Bryson-Frazier: Lmax tile-legs of kMbfLegBytes + the first-leg block
+    w.tile_stride = mbf ? (size_t)n_legs_max * kf::kMbfLegBytes + (size_t)kf::kMbfFirstDoubles * KF_TILE * sizeof(double)
+                        : (size_t)n_legs_max * kf::kLegBytes;
     off += align_up((size_t)w.n_tiles * w.tile_stride, 256);
     w.nleg_off = off;
     off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
@@ -132,6 +135,10 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
     if (!(std::fabs(n2 - 1.0) < 1e-9)) return KF_ERR_ARG;
   }
   if (op->length_sort < KF_SORT_AUTO || op->length_sort > KF_SORT_ON) return KF_ERR_ARG;
+  if (op->smoother != KF_SMOOTHER_RTS && op->smoother != KF_SMOOTHER_BRYSON_FRAZIER) return KF_ERR_ARG;
+  if (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER &&
+      ((op->output_states & KF_STATES_SMOOTH) || op->variant == KF_VARIANT_LANES_PER_TRACK))
+    return KF_ERR_UNSUPPORTED;
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)
     return KF_ERR_ARG;
@@ -156,11 +163,13 @@ void kf_default_options(kf_options* opt) {
   opt->variant = KF_VARIANT_AUTO;
   opt->perigee_axis[2] = 1.0;
   opt->length_sort = KF_SORT_AUTO;
+  opt->smoother = KF_SMOOTHER_RTS;
 }
 
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt) {
   const int smooth = opt ? opt->smooth : 1;
-  return workspace_layout(n_tracks, n_legs_max, smooth).total;
+  const int mbf = smooth && opt && opt->smoother == KF_SMOOTHER_BRYSON_FRAZIER;
+  return workspace_layout(n_tracks, n_legs_max, smooth, mbf).total;
 }
 
 int kf_last_launch_count(void) { return g_launches; }
@@ -193,7 +202,8 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
                  kf::FitParams& P, SortPlan& sort) {
   const long long N = tr->n_tracks;
   const int Lmax = ge->n_surfaces - 1 - tr->start_surface;
-  const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth);
+  const int mbf = op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER;
+  const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth, mbf);
   if (w.rec_total > 0 && (!workspace || workspace_bytes < w.rec_total)) return KF_ERR_WORKSPACE;
   // the sort's arrays come after the records: a workspace sized by kf_workspace_bytes always holds them; a
   // shorter one (records only) runs unsorted under AUTO and is refused under ON
@@ -250,8 +260,10 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (w.rec_total > 0) {
     char* base = static_cast<char*>(workspace);
     P.rec = base + w.rec_off;
-    P.leg_stride = kf::kLegBytes;
+    P.leg_stride = mbf ? kf::kMbfLegBytes : kf::kLegBytes;
     P.tile_stride = w.tile_stride;
+    P.mbf = mbf;
+    P.first_off = (size_t)Lmax * kf::kMbfLegBytes;
     P.nleg = reinterpret_cast<int*>(base + w.nleg_off);
   } else {
     P.smooth = 0;  // no legs to smooth (Lmax == 0)
@@ -326,7 +338,8 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
     g_launches += 3;
     P.perm = sort.perm;
   }
-  const bool lanes = variant == KF_VARIANT_LANES_PER_TRACK || (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS);
+  const bool lanes = !P.mbf && (variant == KF_VARIANT_LANES_PER_TRACK ||
+                                (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS));
   const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
   const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
   int rc;
@@ -338,7 +351,9 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   else rc = launch_forward<1, KF_FWD_BLOCK_SMALL>(P, grid3, material, geom_smem, stream);
   if (rc != KF_OK) return rc;
   record_stage(1, stream);
-  if (P.smooth) {
+  if (P.smooth && P.mbf) {
+    rc = launch(kf::kf_mbf_kernel, P, KF_TILE, kf::kMbfSmem, stream, "kf_mbf_kernel");
+  } else if (P.smooth) {
     rc = lanes ? launch(kf::kf_rts_lanes_kernel, P, kf::kRtsLanesBlock, kf::kRtsLanesSmem, stream, "kf_rts_lanes_kernel",
                         kf::kLanes)
                : launch(kf::kf_rts_kernel, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
@@ -478,7 +493,8 @@ ArenaLayout arena_layout(long long N, long long M, int nS, int start, const kf_f
   a.rk_err = b.take(N * D);
   a.perigee_params = b.take(6 * N * D);
   a.perigee_cov = b.take(21 * N * D);
-  a.workspace_bytes = workspace_layout(N, Lmax, op ? op->smooth : 1).total;
+  a.workspace_bytes = workspace_layout(N, Lmax, op ? op->smooth : 1,
+                                       op && op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER).total;
   a.workspace = b.take(a.workspace_bytes);
   a.total = b.off;
   return a;

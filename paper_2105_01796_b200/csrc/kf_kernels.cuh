@@ -26,6 +26,12 @@ namespace kf {
 
 constexpr int kRecDoubles = 55;  // x-(6) C-(21) Fa(20) Ft(5) g(1) hit(2)
 constexpr int kRecXp = 0, kRecCp = 6, kRecFa = 27, kRecFt = 47, kRecG = 52, kRecM = 53;
+// record of the Bryson-Frazier backward pass (kf_options.smoother, kf_mbf.cuh): gain (r0 r1 S^-1_00 S^-1_01 S^-1_11;
+// zero gain = hole or outlier), the two leading columns of C- (00 01 .. 05 11 .. 15), then F = J G and g as above.
+// x- and C- of the FIRST leg only go to a per-tile block behind the tile's legs.
+constexpr int kMbfDoubles = 42;
+constexpr int kMbfGain = 0, kMbfCcol = 5, kMbfFa = 16, kMbfFt = 36, kMbfG = 41;
+constexpr int kMbfFirstDoubles = 27;  // x-(6) C-(21) of leg 0
 
 // tracks per tile of the record layout = threads per CTA of the RTS kernel (one bulk copy per tile-leg);
 // the forward kernel's CTA covers KF_FWD_BLOCK / KF_TILE whole tiles
@@ -94,6 +100,8 @@ struct FitParams {
   size_t leg_stride;    // = kLegBytes
   size_t tile_stride;   // = Lmax * kLegBytes
   int* nleg;            // [slots] legs the forward pass completed, by SLOT
+  int mbf;              // 1: Bryson-Frazier records (kMbf*), 0: RTS records (kRec*)
+  size_t first_off;     // mbf: byte offset of a tile's first-leg block [kMbfFirstDoubles][KF_TILE] from its base
   // length sort of ragged batches (kf_sort.cuh): slot -> track.  Records and nleg are indexed by slot (the
   // position in launch order), every caller-visible array by track.  nullptr: slot == track.
   const int* perm;
@@ -241,18 +249,26 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     // stores drain under the covariance transport; C- and the hit follow it
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth && lead) {
+      // the F block sits at kRecFa (RTS record) or kMbfFa (Bryson-Frazier record); Ft and g follow it in both
+      double* __restrict__ RF = R + (size_t)(P.mbf ? kMbfFa : kRecFa) * KF_TILE;
+      if (!P.mbf) {
 #pragma unroll
-      for (int k = 0; k < 6; ++k) KF_REC_STORE(&R[(kRecXp + k) * KF_TILE], xp[k]);
+        for (int k = 0; k < 6; ++k) KF_REC_STORE(&R[(kRecXp + k) * KF_TILE], xp[k]);
+      } else if (l == 0) {
+        double* __restrict__ FB = reinterpret_cast<double*>(tile_rec + P.first_off);
+#pragma unroll
+        for (int k = 0; k < 6; ++k) KF_REC_STORE(&FB[k * KF_TILE], xp[k]);
+      }
 #pragma unroll
       for (int a = 0; a < 4; ++a) {
 #pragma unroll
-        for (int c = 0; c < 4; ++c) KF_REC_STORE(&R[(kRecFa + a * 5 + c) * KF_TILE], J.Ja[a][c]);
-        KF_REC_STORE(&R[(kRecFa + a * 5 + 4) * KF_TILE], J.Ja[a][4] * g_prev);
+        for (int c = 0; c < 4; ++c) KF_REC_STORE(&RF[(a * 5 + c) * KF_TILE], J.Ja[a][c]);
+        KF_REC_STORE(&RF[(a * 5 + 4) * KF_TILE], J.Ja[a][4] * g_prev);
       }
 #pragma unroll
-      for (int c = 0; c < 4; ++c) KF_REC_STORE(&R[(kRecFt + c) * KF_TILE], J.Jt[c]);
-      KF_REC_STORE(&R[(kRecFt + 4) * KF_TILE], J.Jt[4] * g_prev);
-      KF_REC_STORE(&R[kRecG * KF_TILE], g_prev);
+      for (int c = 0; c < 4; ++c) KF_REC_STORE(&RF[(kRecFt - kRecFa + c) * KF_TILE], J.Jt[c]);
+      KF_REC_STORE(&RF[(kRecFt - kRecFa + 4) * KF_TILE], J.Jt[4] * g_prev);
+      KF_REC_STORE(&RF[(kRecG - kRecFa) * KF_TILE], g_prev);
     }
     if (mat_here) material_apply(ms, C);
     double Cp[21];
@@ -267,10 +283,20 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth && lead) {
+      if (!P.mbf) {
 #pragma unroll
-      for (int k = 0; k < 21; ++k) KF_REC_STORE(&R[(kRecCp + k) * KF_TILE], Cp[k]);
-      KF_REC_STORE(&R[kRecM * KF_TILE], m0);
-      KF_REC_STORE(&R[(kRecM + 1) * KF_TILE], m1);
+        for (int k = 0; k < 21; ++k) KF_REC_STORE(&R[(kRecCp + k) * KF_TILE], Cp[k]);
+        KF_REC_STORE(&R[kRecM * KF_TILE], m0);
+        KF_REC_STORE(&R[(kRecM + 1) * KF_TILE], m1);
+      } else {
+#pragma unroll
+        for (int k = 0; k < 11; ++k) KF_REC_STORE(&R[(kMbfCcol + k) * KF_TILE], Cp[k]);  // (0,0..5), (1,1..5)
+        if (l == 0) {
+          double* __restrict__ FB = reinterpret_cast<double*>(tile_rec + P.first_off);
+#pragma unroll
+          for (int k = 0; k < 21; ++k) KF_REC_STORE(&FB[(6 + k) * KF_TILE], Cp[k]);
+        }
+      }
     }
 
     // gain-matrix update with the surface's hit.  A hole or a flagged outlier runs the
@@ -311,10 +337,17 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     } else {
       n_holes++;
     }
+    if (P.smooth && P.mbf && lead) {  // the gain as applied: zero for a hole or a flagged outlier
+      KF_REC_STORE(&R[(kMbfGain + 0) * KF_TILE], gn.r0);
+      KF_REC_STORE(&R[(kMbfGain + 1) * KF_TILE], gn.r1);
+      KF_REC_STORE(&R[(kMbfGain + 2) * KF_TILE], gn.i00);
+      KF_REC_STORE(&R[(kMbfGain + 3) * KF_TILE], gn.i01);
+      KF_REC_STORE(&R[(kMbfGain + 4) * KF_TILE], gn.i11);
+    }
     gain_apply(gn, xp, Cp, x, C);
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
     rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
-    if (P.smooth && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
+    if (P.smooth && !P.mbf && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
     if ((P.output_states & OUT_PRED) && lead) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
       store21(P.state_cov[0] + (size_t)l * 21 * N, N, i, Cp);

@@ -118,6 +118,43 @@ def test_adaptive_step_count_parity(cfg, n, tol, variant):
     assert ref.rk_err_max.max() < 0.2 * base.rk_err_max.max()  # the option did change the stepping
 
 
+# ---- backward pass in Bryson-Frazier form (kf_options.smoother): the RTS result at the first surface ----------
+@pytest.mark.parametrize("cfg,n,sort", [(1, 6001, 1), (2, 3001, 1), (3, 3001, 2), (4, 3001, 2), (3, 129, 1), (2, 40000, 0)])
+def test_bryson_frazier_backward_pass_matches_the_rts_oracle(cfg, n, sort):
+    wl = W.make_config(cfg, n_tracks=n, seed=95 + cfg)
+    ref = oracle.fit_workload(wl, perigee=Z_AXIS)
+    got = kf.fit_workload(wl, perigee=Z_AXIS, smoother=B.SMOOTHER_BRYSON_FRAZIER, length_sort=sort)
+    rep = parity.assert_parity(got, ref, label=f"bryson-frazier cfg{cfg}")
+    assert rep["first_params"] < 0.1 and rep["first_cov"] < 0.1, rep
+    # the forward pass is the same code: last_*, chi2 and flags are bit-identical to the RTS run
+    rts = kf.fit_workload(wl, perigee=Z_AXIS, length_sort=sort, variant=B.VARIANT_THREAD_PER_TRACK)
+    for name in ("last_params", "last_cov", "chi2", "hit_flags", "status"):
+        np.testing.assert_array_equal(getattr(got, name), getattr(rts, name), err_msg=name)
+
+
+def test_bryson_frazier_option_rules():
+    wl = W.make_config(1, n_tracks=300)
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    for over in (dict(output_states=B.STATES_SMOOTH), dict(variant=B.VARIANT_LANES_PER_TRACK)):
+        with pytest.raises(kf.KfError) as e:
+            kf.FitCall(db, smoother=B.SMOOTHER_BRYSON_FRAZIER, **over).run()
+        assert e.value.rc == -2
+    # filter only: the option is ignored; one leg: the first-leg block still fits the workspace
+    a = kf.fit_workload(wl, smooth=0, smoother=B.SMOOTHER_BRYSON_FRAZIER)
+    b = kf.fit_workload(wl, smooth=0)
+    np.testing.assert_array_equal(a.first_cov, b.first_cov)
+    short = W.make_config(0, n_tracks=200)
+    geom1 = short.geometry[:2].copy()
+    keep = short.surf_idx == 1
+    offs = np.arange(201, dtype=np.int32)
+    hb = kf.HostBatch.from_arrays(short.params0, short.cov0, 0, offs, short.surf_idx[keep], short.loc[keep], geom1,
+                                  options=dict(smooth=1, smoother=B.SMOOTHER_BRYSON_FRAZIER))
+    got = kf.fit_batch(hb).to_host()
+    fld, opt = oracle.make_field("const", (0, 0, 2.0)), oracle.make_options(smooth=1)
+    ref = oracle.fit_batch(short.params0, short.cov0, 0, offs, short.surf_idx[keep], short.loc[keep], geom1, fld, opt)
+    parity.assert_parity(got, ref, label="one leg")
+
+
 # ---- length sort of ragged batches (kf_sort.cuh): same results, track by track -------------------------------
 @pytest.mark.parametrize("cfg,n", [(3, 5003), (4, 5003), (4, 129), (2, 1000), (4, 9001)])
 def test_length_sort_parity_all_states(cfg, n, variant):
