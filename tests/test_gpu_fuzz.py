@@ -153,3 +153,22 @@ def test_random_configuration_parity(seed):
             if np.any(ill):
                 parity.assert_parity(got, ref, states=True, sel=ill, loosen=loosen * 1e3 * kappa[ill].max() / 1e5,
                                      label=label + " (ill-conditioned updates)")
+    # the Bryson-Frazier backward pass (kf_options.smoother) reaches the same first_*: its final step
+    # C- - C- Lam C- cancels kappa_s = C-_ii / C^s_ii digits at the first leg, so the bars scale with kappa_s / 1e4
+    if smooth:
+        first = c["start"]  # per-leg arrays are indexed from the start surface: leg 0
+        with np.errstate(invalid="ignore", divide="ignore"):
+            ks = np.einsum("nii->ni", ref.pred_cov[:, 0]) / np.einsum("nii->ni", ref.smooth_cov[:, 0])
+        kappa_s = np.nan_to_num(np.where(np.isfinite(ks), ks, 0.0).max(axis=1), nan=0.0)
+        call = kf.FitCall(kf.DeviceBatch(hb), perigee=c["line"], smoother=B.SMOOTHER_BRYSON_FRAZIER,
+                          variant=B.VARIANT_THREAD_PER_TRACK)
+        got = call.run().to_host()
+        ok = ~runaway & (kappa <= 1e5) & (ref.status == 0) & (got.status == 0)
+        if np.any(ok):
+            from types import SimpleNamespace
+            pick = lambda r: SimpleNamespace(**{k: getattr(r, k) for k in (
+                "first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status", "n_used", "n_outliers",
+                "n_holes", "perigee_params", "perigee_cov")}, hit_flags=None, hit_chi2=None)
+            parity.assert_parity(pick(got), pick(ref), sel=ok, loosen=loosen * max(1.0, kappa_s[ok].max() / 1e4),
+                                 label=f"seed {seed} bryson-frazier opts {c['opts']}")
+
