@@ -69,8 +69,11 @@ enum {
   KF_ST_FIELD_CLAMPED = 32,/* a field lookup fell outside the grid; the clamped value was used */
   KF_ST_BAD_HITS = 64,     /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces):
                               track not fitted, outputs hold the start state */
-  KF_ST_PERIGEE = 128      /* the extrapolation of first_* to the perigee surface stopped (moving along the axis,
+  KF_ST_PERIGEE = 128,     /* the extrapolation of first_* to the perigee surface stopped (moving along the axis,
                               non-finite state, theta chart singular): perigee_* hold NaN */
+  KF_ST_CANCELLATION = 256 /* Bryson-Frazier backward pass only: first_cov = C- - C- Lam C- cancelled more than 1e6 (an
+                              uninformative prior): first_* are valid but may miss the 1e-8 covariance bar; the RTS
+                              form (the default) does not have this */
 };
 
 /* per-hit flags */

@@ -29,7 +29,7 @@ __device__ constexpr double kPi = 3.14159265358979323846;
 
 enum : unsigned {
   ST_PROPAGATION = 1u, ST_NOT_POSITIVE = 2u, ST_ENERGY = 4u, ST_NDF = 8u, ST_THETA = 16u,
-  ST_FIELD_CLAMPED = 32u, ST_BAD_HITS = 64u, ST_PERIGEE = 128u
+  ST_FIELD_CLAMPED = 32u, ST_BAD_HITS = 64u, ST_PERIGEE = 128u, ST_CANCELLATION = 256u
 };
 
 constexpr int FIELD_CONST = 0;

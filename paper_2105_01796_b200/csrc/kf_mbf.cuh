@@ -21,6 +21,7 @@
 namespace kf {
 
 constexpr size_t kMbfLegBytes = (size_t)kMbfDoubles * KF_TILE * sizeof(double);
+constexpr double kMbfKappaMax = 1.0e6;  // ~30 eps kappa against the 1e-8 covariance bar
 constexpr int kMbfStages = 2;  // 43 KB per CTA: five CTAs (ten warps) per SM
 constexpr size_t kMbfSmem = kMbfStages * kMbfLegBytes + kMbfStages * sizeof(unsigned long long);
 static_assert(kMbfLegBytes % 16 == 0, "a tile-leg must be a whole number of 16-byte units (bulk copy)");
@@ -217,6 +218,12 @@ kf_mbf_kernel(const __grid_constant__ FitParams P) {
     if (fabs(chk) < 1.0e300) {
       store6(P.first_params, N, i, xs);
       store21(P.first_cov, N, i, Cs);
+      // the subtraction above loses kappa = C-_ii / C^s_ii leading digits: tell the caller when that is more than the
+      // covariance bar of the parity contract can absorb (an uninformative prior; the RTS form does not have this)
+      double kappa = 0.0;
+#pragma unroll
+      for (int a = 0; a < 6; ++a) kappa = fmax(kappa, Cs[IX(a, a)] > 0.0 ? Cp[IX(a, a)] / Cs[IX(a, a)] : 1.0e300);
+      if (kappa > kMbfKappaMax) P.status[i] |= ST_CANCELLATION;
     } else {
       P.status[i] |= ST_NOT_POSITIVE;  // first_* keeps the filtered state the forward pass wrote (U25)
     }

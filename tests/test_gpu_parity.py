@@ -132,6 +132,18 @@ def test_bryson_frazier_backward_pass_matches_the_rts_oracle(cfg, n, sort):
         np.testing.assert_array_equal(getattr(got, name), getattr(rts, name), err_msg=name)
 
 
+def test_bryson_frazier_flags_a_cancelling_first_state():
+    """a 1e4-inflated prior: C- at the first leg is ~1e7 times the smoothed covariance, the subtraction
+    C- - C- Lam C- cannot hold the 1e-8 bar, and the kernel says so (status bit 256) instead of staying silent."""
+    wl = W.make_config(1, n_tracks=2000, seed=17)
+    got = kf.fit_workload(wl, smoother=B.SMOOTHER_BRYSON_FRAZIER, cov_inflation=1e4)
+    ref = oracle.fit_workload(wl, cov_inflation=1e4)
+    assert np.mean((got.status & 256) != 0) > 0.9 and np.all((got.status & ~np.uint32(256)) == ref.status)
+    np.testing.assert_allclose(got.first_params, ref.first_params, rtol=1e-6, atol=1e-6)  # still the same state
+    plain = kf.fit_workload(wl, smoother=B.SMOOTHER_BRYSON_FRAZIER)
+    assert not np.any(plain.status & 256)
+
+
 def test_bryson_frazier_option_rules():
     wl = W.make_config(1, n_tracks=300)
     db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
