@@ -144,6 +144,20 @@ def test_bryson_frazier_flags_a_cancelling_first_state():
     assert not np.any(plain.status & 256)
 
 
+def test_bryson_frazier_through_the_host_entry_points():
+    import torch
+    wl = W.make_config(3, n_tracks=2501, seed=48)
+    ref = oracle.fit_workload(wl, perigee=TILTED_AXIS)
+    for ns, sort in ((0, B.SORT_OFF), (3, B.SORT_ON)):
+        call = kf.HostCall(kf.HostBatch.from_workload(wl), per_hit=True, n_streams=ns, chunk_tracks=512, perigee=TILTED_AXIS,
+                           smoother=B.SMOOTHER_BRYSON_FRAZIER, length_sort=sort, variant=B.VARIANT_THREAD_PER_TRACK)
+        call.run()
+        torch.cuda.synchronize()
+        got = call.to_host()
+        got.rk_err_max = None
+        parity.assert_parity(got, ref, label=f"host bryson-frazier S={ns}")
+
+
 def test_bryson_frazier_option_rules():
     wl = W.make_config(1, n_tracks=300)
     db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
