@@ -153,7 +153,9 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // variant ("intra-track parallelisation", NS "warp-cooperative lanes-per-track"): the 8 lanes
 // of a group run the scalar part of the leg redundantly (identical values, identical branches) and share the
 // 6x6 covariance transport row by row, exchanging the rows with warp shuffles; lane 0 of the group stores.
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK>
+// MBF: the record written is the Bryson-Frazier one (kMbf*, kf_mbf.cuh) instead of the RTS one (kRec*); a template
+// parameter because a run-time flag cost the RTS path 2.7 % (3.41 -> 3.51 ms on CFG2: five more registers).
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF>
 __global__ void __launch_bounds__(BLOCK, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   static_assert(BLOCK % KF_TILE == 0, "a forward CTA covers whole tiles");
@@ -250,8 +252,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth && lead) {
       // the F block sits at kRecFa (RTS record) or kMbfFa (Bryson-Frazier record); Ft and g follow it in both
-      double* __restrict__ RF = R + (size_t)(P.mbf ? kMbfFa : kRecFa) * KF_TILE;
-      if (!P.mbf) {
+      double* __restrict__ RF = R + (size_t)(MBF ? kMbfFa : kRecFa) * KF_TILE;
+      if (!MBF) {
 #pragma unroll
         for (int k = 0; k < 6; ++k) KF_REC_STORE(&R[(kRecXp + k) * KF_TILE], xp[k]);
       } else if (l == 0) {
@@ -283,7 +285,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth && lead) {
-      if (!P.mbf) {
+      if (!MBF) {
 #pragma unroll
         for (int k = 0; k < 21; ++k) KF_REC_STORE(&R[(kRecCp + k) * KF_TILE], Cp[k]);
         KF_REC_STORE(&R[kRecM * KF_TILE], m0);
@@ -337,7 +339,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     } else {
       n_holes++;
     }
-    if (P.smooth && P.mbf && lead) {  // the gain as applied: zero for a hole or a flagged outlier
+    if (P.smooth && MBF && lead) {  // the gain as applied: zero for a hole or a flagged outlier
       KF_REC_STORE(&R[(kMbfGain + 0) * KF_TILE], gn.r0);
       KF_REC_STORE(&R[(kMbfGain + 1) * KF_TILE], gn.r1);
       KF_REC_STORE(&R[(kMbfGain + 2) * KF_TILE], gn.i00);
@@ -347,7 +349,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     gain_apply(gn, xp, Cp, x, C);
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
     rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
-    if (P.smooth && !P.mbf && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
+    if (P.smooth && !MBF && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
     if ((P.output_states & OUT_PRED) && lead) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
       store21(P.state_cov[0] + (size_t)l * 21 * N, N, i, Cp);
