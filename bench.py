@@ -210,7 +210,9 @@ def main():
     db = kf.DeviceBatch(hb, dev)
     variant = {"auto": 0, "thread": 1, "lanes": 2}[args.variant]
     bf = args.smoother == "bf"
-    call = kf.FitCall(db, variant=variant, smoother=int(bf))  # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit flags
+    # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit chi2 and flags (no RKN error diagnostic)
+    out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
+    call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf))
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -283,7 +285,8 @@ def main():
     # ---- context: the same step with the backward pass in Bryson-Frazier form (kf_options.smoother) --------------------
     alt = None
     if smooth and not bf and args.config == 2 and not args.no_e2e:
-        call2 = kf.FitCall(db, variant=variant, smoother=1)
+        out2 = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
+        call2 = kf.FitCall(db, out=out2, variant=variant, smoother=1)
         for _ in range(3):
             call2.run()
         barrier()

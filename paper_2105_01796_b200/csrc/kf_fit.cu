@@ -292,7 +292,7 @@ kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
 }
 
 // Enqueue the forward filter and, if asked for, the RTS pass over the tracks of P on `stream`.
-template <int LPT, int BLOCK, bool MBF>
+template <int LPT, int BLOCK, bool MBF, bool PLAIN = false>
 int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geom_smem, cudaStream_t stream) {
   using kf::FIELD_CONST;
   using kf::FIELD_GRID3;
@@ -303,14 +303,14 @@ int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geo
   const int sel = (grid3 ? 4 : 0) | (material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
   const char* nm = "kf_forward_kernel";
   switch (sel) {
-    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, false, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 2: return launch(kf::kf_forward_kernel<FIELD_CONST, true, false, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 3: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 4: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, false, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
-    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT, BLOCK, MBF>, P, BLOCK, smem, stream, nm, LPT);
+    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
+    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
+    case 2: return launch(kf::kf_forward_kernel<FIELD_CONST, true, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
+    case 3: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
+    case 4: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
+    case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
+    case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
+    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
   }
 }
 
@@ -347,9 +347,16 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   // 256-thread forward CTAs once a constant-field batch is more than one wave of 128-thread CTAs at two per SM
   // (CFG2 3.47 -> 3.40 ms; the grid-field kernel, at 255 registers with spills, is slower that way: CFG4 5.87 -> 6.11 ms)
   const bool big = !grid3 && P.N > KF_FWD_BIG_MIN_TRACKS;
+  // the plain instantiation: default stepping, per-surface resolutions, no per-leg PRED/FILT states, no RKN estimate
+  const bool plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
+                     !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
   if (lanes) rc = launch_forward<kf::kLanes, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
+  else if (P.mbf && plain) rc = big ? launch_forward<1, KF_FWD_BLOCK, true, true>(P, grid3, material, geom_smem, stream)
+                                    : launch_forward<1, KF_FWD_BLOCK_SMALL, true, true>(P, grid3, material, geom_smem, stream);
   else if (P.mbf) rc = big ? launch_forward<1, KF_FWD_BLOCK, true>(P, grid3, material, geom_smem, stream)
                            : launch_forward<1, KF_FWD_BLOCK_SMALL, true>(P, grid3, material, geom_smem, stream);
+  else if (plain) rc = big ? launch_forward<1, KF_FWD_BLOCK, false, true>(P, grid3, material, geom_smem, stream)
+                           : launch_forward<1, KF_FWD_BLOCK_SMALL, false, true>(P, grid3, material, geom_smem, stream);
   else rc = big ? launch_forward<1, KF_FWD_BLOCK, false>(P, grid3, material, geom_smem, stream)
                 : launch_forward<1, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
   if (rc != KF_OK) return rc;

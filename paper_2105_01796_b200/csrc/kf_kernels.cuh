@@ -155,9 +155,17 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // 6x6 covariance transport row by row, exchanging the rows with warp shuffles; lane 0 of the group stores.
 // MBF: the record written is the Bryson-Frazier one (kMbf*, kf_mbf.cuh) instead of the RTS one (kRec*); a template
 // parameter because a run-time flag cost the RTS path 2.7 % (3.41 -> 3.51 ms on CFG2: five more registers).
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF>
+// PLAIN: the call uses the default stepping policy (one primary + two correction steps, no step cap, no tolerance),
+// per-surface resolutions, and asks for no per-leg predicted/filtered states and no RKN error estimate: those paths are
+// compiled out (measured on CFG2: 3.39 -> 3.15 ms; the run-time tests cost registers in a kernel that has none to spare).
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN>
 __global__ void __launch_bounds__(BLOCK, KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
+  const int o_n_corr = PLAIN ? 2 : P.n_corr;
+  const double o_max_step = PLAIN ? 0.0 : P.max_step, o_step_tol = PLAIN ? 0.0 : P.step_tol;
+  const double* const o_var = PLAIN ? nullptr : P.var;
+  const int o_states = PLAIN ? 0 : P.output_states;
+  double* const o_rk_err = PLAIN ? nullptr : P.rk_err_max;
   static_assert(BLOCK % KF_TILE == 0, "a forward CTA covers whole tiles");
   extern __shared__ double s_dyn[];
   const double* __restrict__ G;
@@ -240,7 +248,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     }
     double xp[6];
     BoundJacobian J;
-    const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, P.step_tol, sf, st, x, trig,
+    const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig,
                                          xp, J, errmax, status);
     if (rc) {
       status |= rc;
@@ -308,9 +316,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
     if (has_hit) {
       double v00, v11, v01 = 0.0;
-      if (P.var) {
-        v00 = P.var[hp];
-        v11 = P.var[P.ldm + hp];
+      if (o_var) {
+        v00 = o_var[hp];
+        v11 = o_var[P.ldm + hp];
         if (P.cov01) v01 = P.cov01[hp];
       } else {
         v00 = st[16];
@@ -350,11 +358,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
     rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
     if (P.smooth && !MBF && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
-    if ((P.output_states & OUT_PRED) && lead) {
+    if ((o_states & OUT_PRED) && lead) {
       store6(P.state_params[0] + (size_t)l * 6 * N, N, i, xp);
       store21(P.state_cov[0] + (size_t)l * 21 * N, N, i, Cp);
     }
-    if ((P.output_states & OUT_FILT) && lead) {
+    if ((o_states & OUT_FILT) && lead) {
       store6(P.state_params[1] + (size_t)l * 6 * N, N, i, x);
       store21(P.state_cov[1] + (size_t)l * 21 * N, N, i, C);
     }
@@ -387,7 +395,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   P.n_used[i] = n_used;
   P.n_outliers[i] = n_outl;
   P.n_holes[i] = n_holes;
-  if (P.rk_err_max) P.rk_err_max[i] = errmax;
+  if (o_rk_err) o_rk_err[i] = errmax;
   if (P.smooth) P.nleg[tslot] = nleg;
   for (int j = hp; j < o1; ++j) {  // hits never reached
     if (P.hit_chi2) P.hit_chi2[j] = 0.0;

@@ -16,7 +16,10 @@ pytestmark = pytest.mark.gpu
 def run_full(wl):
     import torch
     db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
-    call = kf.FitCall(db)
+    # the launch configuration bench.py times: minimal outputs (no RKN error diagnostic) -> the PLAIN forward kernel
+    hb = db.host
+    out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False)
+    call = kf.FitCall(db, out=out)
     call.run()
     torch.cuda.synchronize()
     ragged = wl.n_meas != wl.n_tracks * (wl.geometry.shape[0] - 1 - wl.start_surface)

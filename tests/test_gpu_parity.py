@@ -118,6 +118,30 @@ def test_adaptive_step_count_parity(cfg, n, tol, variant):
     assert ref.rk_err_max.max() < 0.2 * base.rk_err_max.max()  # the option did change the stepping
 
 
+# ---- the PLAIN forward instantiation (default stepping, no optional per-leg outputs: what bench.py times) -------
+@pytest.mark.parametrize("cfg,n", [(0, 3001), (1, 5001), (2, 3001), (3, 3001), (4, 3001), (2, 45000)])
+@pytest.mark.parametrize("smoother", [B.SMOOTHER_RTS, B.SMOOTHER_BRYSON_FRAZIER])
+def test_plain_forward_kernel_parity(cfg, n, smoother):
+    wl = W.make_config(cfg, n_tracks=n, seed=30 + cfg)
+    ref = oracle.fit_workload(wl, states=True)
+    hb = kf.HostBatch.from_workload(wl)
+    smooth = wl.options.get("smooth", 1)
+    states = B.STATES_SMOOTH if (smooth and smoother == B.SMOOTHER_RTS) else 0
+    out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, states, per_hit=True, rk_err=False)
+    got = kf.FitCall(kf.DeviceBatch(hb), out=out, output_states=states, smoother=smoother,
+                     variant=B.VARIANT_THREAD_PER_TRACK).run().to_host()
+    ref.pred_params = ref.filt_params = None
+    rep = parity.assert_parity(got, ref, states=True, label=f"plain cfg{cfg}")
+    assert max(rep.values()) < 0.1, rep
+    # and the general instantiation's results to round-off (another instantiation is another instruction order)
+    gen = kf.fit_workload(wl, smoother=smoother, variant=B.VARIANT_THREAD_PER_TRACK)
+    for name in ("status", "hit_flags", "ndf"):
+        np.testing.assert_array_equal(getattr(got, name), getattr(gen, name), err_msg=name)
+    gen.hit_chi2 = got.hit_chi2 = gen.hit_flags = got.hit_flags = None
+    rep = parity.compare(got, gen)
+    assert max(rep.values()) < 0.1, rep
+
+
 # ---- backward pass in Bryson-Frazier form (kf_options.smoother): the RTS result at the first surface ----------
 @pytest.mark.parametrize("cfg,n,sort", [(1, 6001, 1), (2, 3001, 1), (3, 3001, 2), (4, 3001, 2), (3, 129, 1), (2, 40000, 0)])
 def test_bryson_frazier_backward_pass_matches_the_rts_oracle(cfg, n, sort):
