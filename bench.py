@@ -47,9 +47,9 @@ FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x
 # DRAM traffic per leg measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one launch
 # over 262,144 tracks x 30 legs of this workload, divided by the legs), from the committed capture below.
 # bench.py scales it to the launch it times; it is not re-measured live (never time under a profiler).
-NCU_TRAFFIC = dict(source="profiles/r01j_ncu_summary.md",
-                   bytes_per_leg={"kf_forward_kernel": (0.254369e9 + 3.625990e9) / 7864320,
-                                  "kf_rts_kernel": (3.475758e9 + 0.060069e9) / 7864320})
+NCU_TRAFFIC = dict(source="profiles/r01p_ncu_summary.md",
+                   bytes_per_leg={"kf_forward_kernel": (0.250662e9 + 3.624204e9) / 7864320,
+                                  "kf_rts_kernel": (3.475152e9 + 0.058937e9) / 7864320})
 
 
 def parse_args():
