@@ -366,7 +366,9 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   } else if (P.smooth) {
     rc = lanes ? launch(kf::kf_rts_lanes_kernel, P, kf::kRtsLanesBlock, kf::kRtsLanesSmem, stream, "kf_rts_lanes_kernel",
                         kf::kLanes)
-               : launch(kf::kf_rts_kernel, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
+               : (!P.var && !(P.output_states & kf::OUT_SMOOTH))
+                     ? launch(kf::kf_rts_kernel<true>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel")
+                     : launch(kf::kf_rts_kernel<false>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
   }
   record_stage(2, stream);
   if (rc == KF_OK && G.params) {  // fitted parameters on the perigee surface: one more (small) kernel
