@@ -221,8 +221,18 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    t_warm = time.time()
     for _ in range(max(args.warmup, 3)):
         call.run()
+    barrier()
+    # a fresh box ramps its clocks over the first few hundred milliseconds of load (a cold first run measured 1916 MHz
+    # and 6.0 ms per step against 1965 MHz and 5.8 ms): keep warming up, untimed, until half a second has passed
+    extra_warmup = 0
+    while time.time() - t_warm < 0.5 and extra_warmup < 200:
+        call.run()
+        extra_warmup += 1
+        if extra_warmup % 8 == 0:
+            torch.cuda.synchronize()
     barrier()
     fp64_probe = kf.probe_fp64_tflops(20000, dev) if rank == 0 else None
 
@@ -358,6 +368,7 @@ def main():
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
                     parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant, smoother=args.smoother,
+                    extra_untimed_warmup_steps=extra_warmup,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,
         kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu,
