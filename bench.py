@@ -35,14 +35,28 @@ if ROOT not in sys.path:
 METRIC = "fitted tracks/sec (device-timed, FP64)"
 UNIT = "tracks/s"
 
-# Algorithmic work per leg (one surface visited by one track), DESIGN.md "Rooflines":
+# Work per leg (one surface visited by one track), DESIGN.md "Rooflines".
 #   bytes: RTS record 55 doubles + 1 flag byte written by the forward kernel and read by the RTS
 #          kernel, the hit (2 doubles + int32) read by both; per track 27 doubles in, outputs out.
-#   flops: FP64 flop per leg counted from ncu instruction counters (DFMA = 2), see profiles/.
+#   flops, two clearly separate counts (DFMA = 2, DMUL/DADD = 1):
+#     ALGORITHMIC  SURVEY.md 8(d) D.3: the hand count of the method as stated (dense 3x3 stage chains, three
+#                  RKN4 steps, library transcendentals as FP64-instruction equivalents).  A property of the method.
+#     EXECUTED     what the kernels issue, from the opcode table of the committed ncu capture named below
+#                  (warp-level DFMA/DMUL/DADD of one launch x 32 / legs of that launch).  The closed-form
+#                  constant-field step and the structured products make it 1.8x smaller than the hand count, so
+#                  only THIS count may be divided by a measured FP64 peak.  FP64_PIPE = FP64-pipe instructions
+#                  (DFMA + DMUL + DADD + DSETP) per leg and thread from the same table: the issue-slot view.
 REC_BYTES = 55 * 8 + 1
 HIT_BYTES = 2 * 8 + 4
-FWD_FLOP_PER_LEG = {"const": 3300.0, "grid3": 3900.0}   # + material
-RTS_FLOP_PER_LEG = 1900.0
+ALGORITHMIC_FLOP_PER_LEG = dict(source="SURVEY.md 8(d) D.3 (hand count of the method)",
+                                forward={"const": 3450.0, "const_nomat": 3200.0, "grid3": 4000.0}, rts=1650.0 + 170.0)
+EXECUTED_PER_LEG = dict(source="profiles/r01p_ncu_summary.md (opcode table; 262,144 tracks x 30 legs = 7,864,320 legs per launch)",
+                        flop=dict(kf_forward_kernel=(181.7e6 * 2 + 85.0e6 + 24.3e6) * 32 / 7864320,
+                                  kf_rts_kernel=(183.7e6 * 2 + 44.6e6 + 14.1e6) * 32 / 7864320),
+                        fp64_pipe_instr=dict(kf_forward_kernel=(181.7e6 + 85.0e6 + 24.3e6 + 7.1e6) * 32 / 7864320,
+                                             kf_rts_kernel=(183.7e6 + 44.6e6 + 14.1e6 + 3.8e6) * 32 / 7864320),
+                        fp64_pipe_pct_ncu=dict(kf_forward_kernel=63.7, kf_rts_kernel=60.0),
+                        workload="cfg2 (constant field, material, RTS)")
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x clock)
 # DRAM traffic per leg measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one launch
 # over 262,144 tracks x 30 legs of this workload, divided by the legs), from the committed capture below.
@@ -141,8 +155,9 @@ def dist_setup(n_gpus):
 
 
 def cpu_baseline(wl, cores_hint=None):
-    """The oracle as it stands on a bounded sample (first tracks of the same workload), all host cores.
-    A short probe sets the sample so that the timed run is about 10 s of wall clock (capped at the workload)."""
+    """The oracle as it stands on a bounded sample (first tracks of the same workload): all host cores (OpenMP over
+    tracks, the paper's CPU parallelisation) and, beside it, one thread.  A short
+    probe sets the samples so that the two timed runs are about 10 s and 4 s of wall clock (capped at the workload)."""
     import oracle  # test infrastructure; bench.py's cpu_baseline leg is one of its allowed callers
     n0 = int(min(wl.n_tracks, 20_000))
     oracle.fit_workload(wl.subset(np.arange(min(64, n0))))  # builds/loads the library outside the timing
@@ -154,8 +169,17 @@ def cpu_baseline(wl, cores_hint=None):
     t = time.perf_counter()
     r = oracle.fit_workload(sub)
     dt = time.perf_counter() - t
-    return dict(value=n / dt, unit=UNIT, cores=int(r.threads), kind="oracle",
-                sample=f"first {n} tracks of {wl.name} ({sub.n_meas} hits), {dt:.2f} s wall, OpenMP over tracks")
+    cores = int(r.threads)
+    n1 = int(min(n, max(2000, rate / max(cores, 1) * 4.0)))
+    sub1 = wl.subset(np.arange(n1))
+    t = time.perf_counter()
+    r1 = oracle.fit_workload(sub1, n_threads=1)
+    dt1 = time.perf_counter() - t
+    assert int(r1.threads) == 1
+    return dict(value=n / dt, unit=UNIT, cores=cores, kind="oracle",
+                sample=f"first {n} tracks of {wl.name} ({sub.n_meas} hits), {dt:.2f} s wall, OpenMP over tracks",
+                one_thread=dict(value=n1 / dt1, unit=UNIT, cores=1,
+                                sample=f"first {n1} tracks of {wl.name}, {dt1:.2f} s wall, 1 thread"))
 
 
 def run_reference(args):
@@ -244,19 +268,26 @@ def main():
         sampler.start()
         time.sleep(0.3)
     barrier()
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    # one event before every step and one after the last: the whole region (value) and every step (statistics)
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
     t_wall0 = time.time()
-    e0.record()
     for k in range(args.steps):
+        ev[k].record()
         timer.arm(k)
         call.run()
-    e1.record()
+    ev[args.steps].record()
     barrier()
     t_wall1 = time.time()
     fwd_ms, rts_ms = timer.finish()
     clocks = sampler.stop(t_wall0, t_wall1) if rank == 0 else None
-    value, ms_total, n_job = replicas.job_throughput(N * args.steps, e0.elapsed_time(e1), dist, dev)
+    value, ms_total, n_job = replicas.job_throughput(N * args.steps, ev[0].elapsed_time(ev[args.steps]), dist, dev)
     ms_step = ms_total / args.steps
+    # SURVEY.md 8(d) D.4 / PAPER.md:268: median, and the paper-style mean +- RMS deviation over the timed calls (this rank)
+    per_step = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
+    step_stats = dict(n=int(per_step.size), median_ms=float(np.median(per_step)), mean_ms=float(per_step.mean()),
+                      rms_ms=float(np.sqrt(np.mean((per_step - per_step.mean()) ** 2))),
+                      min_ms=float(per_step.min()), max_ms=float(per_step.max()),
+                      note="per-step CUDA-event times on the launching stream; rms = sqrt(mean squared deviation) as PAPER.md:268")
     launches = call.launches * args.steps
 
     # results of the last step, for the legs count and a sanity line
@@ -292,25 +323,6 @@ def main():
         e2e["single_stream_ms_per_step"] = ms_one
         del hc
 
-    # ---- context: the same step with the backward pass in Bryson-Frazier form (kf_options.smoother) --------------------
-    alt = None
-    if smooth and not bf and args.config == 2 and not args.no_e2e:
-        out2 = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
-        call2 = kf.FitCall(db, out=out2, variant=variant, smoother=1)
-        for _ in range(3):
-            call2.run()
-        barrier()
-        a0, a1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        a0.record()
-        for _ in range(args.steps):
-            call2.run()
-        a1.record()
-        barrier()
-        v2, ms2, _ = replicas.job_throughput(N * args.steps, a0.elapsed_time(a1), dist, dev)
-        alt = dict(smoother="bryson-frazier (same smoothed first state, 42-double records, no 6x6 solve; an option, "
-                            "not the north_star's RTS form)", value=v2, unit=UNIT, ms_per_step=ms2 / args.steps)
-        del call2
-
     if rank != 0:
         if dist is not None:
             dist.destroy_process_group()
@@ -326,36 +338,68 @@ def main():
     if bf:  # no hits re-read; the first-leg block (27 doubles) read, first_* written
         rts_bytes = n_legs * rec_b + N * (27 * 8 + 27 * 8 + 8)
         fwd_bytes += N * 27 * 8
-    fwd_flop = n_legs * FWD_FLOP_PER_LEG[fkind]
-    rts_flop = n_legs * RTS_FLOP_PER_LEG
-    fp64_peak = 148 * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
+    material = int(hb.options.get("material", 0))
+    akey = "grid3" if fkind == "grid3" else ("const" if material else "const_nomat")
+    alg = dict(kf_forward_kernel=ALGORITHMIC_FLOP_PER_LEG["forward"][akey], kf_rts_kernel=ALGORITHMIC_FLOP_PER_LEG["rts"])
+    # the executed counts are of the capture's workload (constant field, material, RTS); other configs: null
+    exe_ok = fkind == "const" and material == 1 and smooth and not bf
+    fp64_nominal = 148 * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
+    fp64_peak = float(fp64_probe)   # the DFMA-chain probe of THIS run (same box, same clocks, same power cap)
     hbm_peak = peaks["hbm_gbs"]
 
-    def kernel_roof(name, ms, nbytes, flop):
+    def kernel_roof(name, key, ms, nbytes):
         if ms <= 0:
             return None
-        return dict(kernel=name, ms=ms, hbm_gbs=nbytes / (ms * 1e-3) / 1e9, hbm_frac=nbytes / (ms * 1e-3) / 1e9 / hbm_peak,
-                    fp64_tflops=flop / (ms * 1e-3) / 1e12, fp64_frac=flop / (ms * 1e-3) / 1e12 / fp64_peak)
+        sec = ms * 1e-3
+        k = dict(kernel=name, ms=ms, hbm_gbs=nbytes / sec / 1e9, hbm_frac=nbytes / sec / 1e9 / hbm_peak,
+                 algorithmic_flop_per_leg=alg[key], algorithmic_tflops=alg[key] * n_legs / sec / 1e12)
+        if exe_ok:
+            ex = EXECUTED_PER_LEG["flop"][key] * n_legs / sec / 1e12
+            k.update(executed_flop_per_leg=EXECUTED_PER_LEG["flop"][key], executed_tflops=ex,
+                     fp64_frac=ex / fp64_peak, fp64_frac_of_nominal=ex / fp64_nominal,
+                     # issue-slot view: FP64-pipe instructions per second over the probe's DFMA rate (one slot each)
+                     fp64_pipe_frac=EXECUTED_PER_LEG["fp64_pipe_instr"][key] * n_legs / sec / (fp64_peak * 1e12 / 2.0),
+                     fp64_pipe_pct_ncu=EXECUTED_PER_LEG["fp64_pipe_pct_ncu"][key])
+        return k
 
-    kf_fwd = kernel_roof("kf_forward_kernel", fwd, fwd_bytes, fwd_flop)
-    kf_rts = kernel_roof("kf_mbf_kernel" if bf else "kf_rts_kernel", rts, rts_bytes, rts_flop) if smooth else None
+    kf_fwd = kernel_roof("kf_forward_kernel", "kf_forward_kernel", fwd, fwd_bytes)
+    kf_rts = kernel_roof("kf_mbf_kernel" if bf else "kf_rts_kernel", "kf_rts_kernel", rts, rts_bytes) if smooth else None
     dom = kf_fwd if (kf_rts is None or fwd >= rts) else kf_rts
-    # the dominant kernel's own bound: the larger of its two fractions says which roof it is nearer
-    if dom["fp64_frac"] >= dom["hbm_frac"]:
-        roofline = dict(bound="alu", achieved=dom["fp64_tflops"], peak=fp64_peak, unit="TFLOP/s",
+    dkey = "kf_forward_kernel" if dom is kf_fwd else "kf_rts_kernel"
+    # the dominant kernel's own bound: whichever roof it is nearer to (FP64 issue slots or HBM bytes)
+    if exe_ok and dom["fp64_pipe_frac"] >= dom["hbm_frac"]:
+        roofline = dict(bound="alu", achieved=dom["executed_tflops"], peak=fp64_peak, unit="TFLOP/s",
                         frac=dom["fp64_frac"], traffic=None, kernel=dom["kernel"],
-                        peak_source=f"148 SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md); "
-                                    f"measured DFMA-chain probe this run: {fp64_probe:.1f} TFLOP/s")
+                        what="EXECUTED FP64 flop (ncu opcode counts: " + EXECUTED_PER_LEG["source"] + ") / CUDA-event time, over the "
+                             "DFMA-chain probe of the same run",
+                        peak_source="kf_probe_fp64_tflops this run (8 independent DFMA chains per thread, all SMs)",
+                        peak_nominal=fp64_nominal,
+                        peak_nominal_source=f"148 SMs x {FP64_LANES_PER_SM} FP64 FMA lanes x 2 x {peaks['sm_max_mhz']:.0f} MHz (DESIGN.md)",
+                        frac_of_nominal=dom["fp64_frac_of_nominal"], fp64_pipe_frac=dom["fp64_pipe_frac"],
+                        fp64_pipe_pct_ncu=dom["fp64_pipe_pct_ncu"], hbm_frac=dom["hbm_frac"],
+                        algorithmic=dict(flop_per_leg=alg[dkey], tflops=dom["algorithmic_tflops"],
+                                         source=ALGORITHMIC_FLOP_PER_LEG["source"],
+                                         note="the method's hand count; not comparable with a measured peak (the kernels "
+                                              "execute fewer flop than the method states)"))
     else:
         roofline = dict(bound="hbm", achieved=dom["hbm_gbs"], peak=hbm_peak, unit="GB/s", frac=dom["hbm_frac"],
-                        traffic=None, kernel=dom["kernel"], peak_source=f"MEASURED_PEAKS.json ({peaks['source']})")
+                        traffic=None, kernel=dom["kernel"], peak_source=f"MEASURED_PEAKS.json ({peaks['source']})",
+                        what="ALGORITHMIC bytes (records + hits + per-track in/out of this launch) / CUDA-event time",
+                        fp64_pipe_frac=dom.get("fp64_pipe_frac"), fp64_pipe_pct_ncu=dom.get("fp64_pipe_pct_ncu"),
+                        fp64_probe_tflops=fp64_peak, fp64_nominal_tflops=fp64_nominal)
     if args.config == 2 and smooth and not bf:  # the capture is of this workload and of the RTS kernels; else null
-        roofline["traffic"] = NCU_TRAFFIC["bytes_per_leg"][dom["kernel"]] * n_legs
+        roofline["traffic"] = NCU_TRAFFIC["bytes_per_leg"][dkey] * n_legs
         roofline["traffic_unit"] = "bytes per launch (ncu dram read+write per leg x legs of this launch)"
         roofline["traffic_source"] = NCU_TRAFFIC["source"]
-        roofline["algorithmic_bytes"] = fwd_bytes if dom["kernel"] == "kf_forward_kernel" else rts_bytes
+    roofline["algorithmic_bytes"] = fwd_bytes if dom is kf_fwd else rts_bytes
     roofline["ms_per_launch"] = dom["ms"]
     roofline["share_of_step"] = dom["ms"] / ms_step
+    # whole step against its two floors (kernels run back to back): executed flop / probe, algorithmic bytes / HBM peak
+    if exe_ok:
+        roofline["step_floors_ms"] = dict(
+            fp64=(EXECUTED_PER_LEG["flop"]["kf_forward_kernel"] + EXECUTED_PER_LEG["flop"]["kf_rts_kernel"]) * n_legs
+                 / (fp64_peak * 1e12) * 1e3,
+            hbm=(fwd_bytes + rts_bytes) / (hbm_peak * 1e9) * 1e3, measured=ms_step)
 
     cpu = None if args.no_cpu_baseline else cpu_baseline(wl)
 
@@ -372,7 +416,7 @@ def main():
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,
         kernels=[k for k in (kf_fwd, kf_rts) if k], fp64_probe_tflops=fp64_probe, cpu_baseline=cpu,
-        alt_smoother=alt)
+        step_stats=step_stats)
     print(json.dumps(line))
     if dist is not None:
         dist.destroy_process_group()

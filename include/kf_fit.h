@@ -29,11 +29,22 @@
  *              the descriptor structs themselves are small HOST structs read during the call.
  *
  * Ownership and ordering
- *   The caller owns every buffer including the workspace.  The library allocates nothing, keeps
- *   no state between calls, never frees and never synchronises: kf_fit_batch validates the
- *   descriptors on the host, enqueues its kernels on `cuda_stream` (a cudaStream_t; NULL = the
- *   legacy default stream) and returns.  Inputs are read-only.  Buffers must stay valid until the
- *   stream has run past the call.  Outputs of a rejected call (< 0) are untouched.
+ *   The caller owns every buffer including the workspace.  The library allocates no device or
+ *   pinned memory, never frees and never synchronises: kf_fit_batch validates the descriptors on
+ *   the host, enqueues its kernels on `cuda_stream` (a cudaStream_t; NULL = the legacy default
+ *   stream) and returns.  Inputs are read-only.  Buffers must stay valid until the stream has run
+ *   past the call.  No state of a fit survives the call; what the library does keep is bookkeeping
+ *   only: per calling thread, the text of the last CUDA error, the launch count of the last call
+ *   (kf_last_launch_count) and the stage-event hook (kf_set_stage_events); per process, the list of
+ *   kernels whose dynamic shared-memory limit has been raised (a one-time cudaFuncSetAttribute).
+ *
+ * Errors
+ *   0 = everything enqueued.  KF_ERR_ARG / KF_ERR_UNSUPPORTED / KF_ERR_WORKSPACE are decided on the
+ *   host before anything is enqueued: outputs are untouched.  KF_ERR_CUDA means a CUDA call failed
+ *   while enqueuing: kernels and copies enqueued before the failure still run (outputs may be
+ *   partly written); in kf_fit_batch_host_pipelined the worker streams are joined back onto
+ *   `cuda_stream` before the call returns, so the caller's stream remains an ordering point for
+ *   reusing the buffers.  Per-track problems never fail a call: they set KF_ST_* bits.
  */
 #ifndef KF_FIT_H
 #define KF_FIT_H
@@ -67,8 +78,9 @@ enum {
   KF_ST_NDF = 8,           /* ndf = 2 n_used - 5 <= 0 */
   KF_ST_THETA = 16,        /* sin(theta) <= 1e-12 on arrival: (phi, theta) chart singular. Track stops. */
   KF_ST_FIELD_CLAMPED = 32,/* a field lookup fell outside the grid; the clamped value was used */
-  KF_ST_BAD_HITS = 64,     /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces):
-                              track not fitted, outputs hold the start state */
+  KF_ST_BAD_HITS = 64,     /* hit list not strictly ascending in surf_idx or outside (start, n_surfaces), or CSR
+                              offsets of the track outside 0 <= offsets[i] <= offsets[i+1] <= n_meas: track not
+                              fitted, outputs hold the start state, its per-hit outputs are left untouched */
   KF_ST_PERIGEE = 128,     /* the extrapolation of first_* to the perigee surface stopped (moving along the axis,
                               non-finite state, theta chart singular): perigee_* hold NaN */
   KF_ST_CANCELLATION = 256 /* Bryson-Frazier backward pass only: first_cov = C- - C- Lam C- cancelled more than 1e6 (an

@@ -5,6 +5,7 @@ The built library is git-ignored but travels to the GPU box with the gpurun snap
 """
 from __future__ import annotations
 
+import glob
 import os
 import shutil
 import subprocess
@@ -16,8 +17,12 @@ CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB_PATH = os.path.join(_HERE, "libkf_fit.so")
 SOURCES = [os.path.join(CSRC, "kf_fit.cu")]
-HEADERS = [os.path.join(CSRC, "kf_device.cuh"), os.path.join(CSRC, "kf_kernels.cuh"), os.path.join(CSRC, "kf_math.cuh"),
-           os.path.join(INCLUDE, "kf_fit.h")]
+
+
+def headers() -> list:
+    """Every header the translation unit can include: csrc/*.cuh and include/*.h (globbed, so a new file is watched)."""
+    return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(INCLUDE, "*.h")))
+
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
@@ -38,7 +43,7 @@ def is_stale() -> bool:
     if not os.path.exists(LIB_PATH):
         return True
     t = os.path.getmtime(LIB_PATH)
-    return any(os.path.getmtime(p) > t for p in SOURCES + HEADERS)
+    return any(os.path.getmtime(p) > t for p in SOURCES + headers())
 
 
 def build_library(force: bool = False, verbose: bool = False, extra_flags=()) -> str:

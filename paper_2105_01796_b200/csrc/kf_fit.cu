@@ -10,6 +10,8 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
+#include <mutex>
+#include <vector>
 
 #include "kf_fit.h"
 #include "kf_kernels.cuh"
@@ -83,13 +85,31 @@ bool set_cuda_error(cudaError_t e, const char* where) {
   return true;
 }
 
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel): set it the first time a kernel
+// asks for more than 48 KB on a device (or for more than it asked before), not on every launch
+bool raise_smem_limit(const void* kernel, size_t smem, const char* name) {
+  struct Entry { const void* fn; int dev; size_t bytes; };
+  static std::mutex mu;
+  static std::vector<Entry> seen;
+  int dev = 0;
+  if (set_cuda_error(cudaGetDevice(&dev), name)) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  for (Entry& e : seen)
+    if (e.fn == kernel && e.dev == dev) {
+      if (e.bytes >= smem) return true;
+      if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
+      e.bytes = smem;
+      return true;
+    }
+  if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
+  seen.push_back(Entry{kernel, dev, smem});
+  return true;
+}
+
 template <typename K>
 int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_t stream, const char* name,
            int lanes_per_track = 1) {
-  if (smem > 48 * 1024) {
-    if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name))
-      return KF_ERR_CUDA;
-  }
+  if (smem > 48 * 1024 && !raise_smem_limit(reinterpret_cast<const void*>(kernel), smem, name)) return KF_ERR_CUDA;
   // thread per track: forward KF_FWD_BLOCK tracks per CTA, RTS one CTA per tile; lanes per track: block / lanes tracks per CTA
   const unsigned grid = (unsigned)((P.N * lanes_per_track + block - 1) / block);
   kernel<<<grid, block, smem, stream>>>(P);
@@ -326,7 +346,7 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   P.perm = nullptr;
   if (sort.perm) {
     kf::SortParams S{};
-    S.N = P.N; S.offsets = P.offsets; S.surf_idx = P.surf_idx; S.start = P.start;
+    S.N = P.N; S.M = P.M; S.offsets = P.offsets; S.surf_idx = P.surf_idx; S.start = P.start;
     S.lmax = P.n_surfaces - 1 - P.start;
     S.bins = sort.bins; S.perm = sort.perm; S.force = sort.force;
     if (set_cuda_error(cudaMemsetAsync(sort.bins, 0, kf::kSortBins * sizeof(int), stream), "length sort")) return KF_ERR_CUDA;
@@ -620,6 +640,16 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
   if (pipe) {
     chunk = pipe->chunk_tracks > 0 ? pipe->chunk_tracks : std::max<long long>(16384, N / (4LL * S));
     chunk = (chunk + kChunkTracks - 1) / kChunkTracks * kChunkTracks;  // whole record tiles
+  }
+  // every chunk boundary of the HOST offsets array is checked before anything of the chunks is enqueued
+  for (long long t0 = 0; t0 < N; t0 += chunk) {
+    const long long m0 = ms->offsets[t0], m1 = ms->offsets[std::min(t0 + chunk, N)];
+    if (m0 < 0 || m1 < m0 || m1 > M) return KF_ERR_ARG;
+  }
+  // the whole CSR offsets array goes over once, on the caller's stream, ahead of the fork (chunks share their
+  // boundary elements)
+  KF_TRY(h2d(a.offsets, ms->offsets, N + 1, 0, N + 1, 1, I, main), "H2D offsets");
+  if (pipe) {
     KF_TRY(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[S]), main), "pipeline fork");
     for (int k = 0; k < S; ++k)
       KF_TRY(cudaStreamWaitEvent(static_cast<cudaStream_t>(pipe->streams[k]), static_cast<cudaEvent_t>(pipe->events[S]), 0),
@@ -627,23 +657,21 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
   }
   const bool grid3 = fl->kind == KF_FIELD_GRID3;
   int c = 0;
-  for (long long t0 = 0; t0 < N; t0 += chunk, ++c) {
-    const long long n = std::min(chunk, N - t0);
-    cudaStream_t st = pipe ? static_cast<cudaStream_t>(pipe->streams[c % S]) : main;
+  // From here on an error must not leave the worker streams un-joined: the loop body reports through `rc`, and the
+  // join below runs whatever it says (chunks enqueued before the failure still run; see kf_fit.h "Errors").
+  auto enqueue_chunk = [&](long long t0, long long n, cudaStream_t st) -> int {
     const long long m0 = ms->offsets[t0], m1 = ms->offsets[t0 + n];  // HOST array in this entry point
-    if (m0 < 0 || m1 < m0 || m1 > M) return KF_ERR_ARG;
     const size_t nm = (size_t)(m1 - m0);
     KF_TRY(h2d(a.params, tr->params, N, t0, n, 6, D, st), "H2D params");
     KF_TRY(h2d(a.cov, tr->cov, N, t0, n, 21, D, st), "H2D cov");
-    KF_TRY(h2d(a.offsets, ms->offsets, N + 1, t0, n + 1, 1, I, st), "H2D offsets");
     KF_TRY(h2d(a.surf_idx, ms->surf_idx, M, m0, nm, 1, I, st), "H2D surf_idx");
     KF_TRY(h2d(a.loc, ms->loc, M, m0, nm, 2, D, st), "H2D loc");
     KF_TRY(h2d(a.var, ms->var, M, m0, nm, 2, D, st), "H2D var");
     KF_TRY(h2d(a.cov01, ms->cov01, M, m0, nm, 1, D, st), "H2D cov01");
 
-    rc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant,
-                     sort_for_range(sort, op, t0, n, (long long)nm, Lmax), st);
-    if (rc != KF_OK) return rc;
+    const int frc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant,
+                                sort_for_range(sort, op, t0, n, (long long)nm, Lmax), st);
+    if (frc != KF_OK) return frc;
 
     KF_TRY(d2h(out->first_params, a.first_params, N, t0, n, 6, D, st), "D2H first_params");
     KF_TRY(d2h(out->first_cov, a.first_cov, N, t0, n, 21, D, st), "D2H first_cov");
@@ -665,14 +693,20 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     KF_TRY(d2h(out->rk_err_max, a.rk_err, N, t0, n, 1, D, st), "D2H rk_err_max");
     KF_TRY(d2h(out->perigee_params, a.perigee_params, N, t0, n, 6, D, st), "D2H perigee_params");
     KF_TRY(d2h(out->perigee_cov, a.perigee_cov, N, t0, n, 21, D, st), "D2H perigee_cov");
-  }
-  if (pipe) {  // join: the caller's stream continues after every chunk stream
+    return KF_OK;
+  };
+  rc = KF_OK;
+  for (long long t0 = 0; t0 < N && rc == KF_OK; t0 += chunk, ++c)
+    rc = enqueue_chunk(t0, std::min(chunk, N - t0), pipe ? static_cast<cudaStream_t>(pipe->streams[c % S]) : main);
+  if (pipe) {  // join: the caller's stream continues after every chunk stream, also when a chunk failed to enqueue
     for (int k = 0; k < S && k < c; ++k) {
-      KF_TRY(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[k]), static_cast<cudaStream_t>(pipe->streams[k])),
-             "pipeline join");
-      KF_TRY(cudaStreamWaitEvent(main, static_cast<cudaEvent_t>(pipe->events[k]), 0), "pipeline join");
+      const bool bad = set_cuda_error(cudaEventRecord(static_cast<cudaEvent_t>(pipe->events[k]),
+                                                      static_cast<cudaStream_t>(pipe->streams[k])), "pipeline join") ||
+                       set_cuda_error(cudaStreamWaitEvent(main, static_cast<cudaEvent_t>(pipe->events[k]), 0), "pipeline join");
+      if (bad && rc == KF_OK) rc = KF_ERR_CUDA;
     }
   }
+  if (rc != KF_OK) return rc;
 #undef KF_TRY
   return KF_OK;
 }

@@ -184,7 +184,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   const unsigned gmask = LPT > 1 ? ((1u << LPT) - 1u) << gbase : 0u;
   const bool lead = LPT == 1 || q == 0;  // the lane that writes the track's results
 
-  const int o0 = P.offsets[i], o1 = P.offsets[i + 1];
+  int o0 = P.offsets[i], o1 = P.offsets[i + 1];
+  // the CSR offsets live in device memory, out of the host validation's sight: a range outside [0, M] or running
+  // backwards is a malformed hit list (the track is not fitted and none of its per-hit outputs is touched)
+  const bool offsets_ok = o0 >= 0 && o0 <= o1 && (long long)o1 <= P.M;
+  if (!offsets_ok) o0 = o1 = 0;
   double x[6], C[21];
 #pragma unroll
   for (int k = 0; k < 6; ++k) x[k] = P.params[k * N + i];
@@ -203,7 +207,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       ok = ok && (s > prev_s) && (s < P.n_surfaces);
       prev_s = s;
     }
-    if (!ok) status |= ST_BAD_HITS;
+    if (!ok || !offsets_ok) status |= ST_BAD_HITS;
     else n_target = prev_s - P.start;  // visit every surface up to the one of the last hit (U7)
   }
   // the next unconsumed hit is fetched one leg ahead of its use into this thread's own shared-memory

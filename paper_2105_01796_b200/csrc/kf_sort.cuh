@@ -20,7 +20,7 @@ constexpr int kSortBins = 64;    // lengths are quantised into at most this many
 constexpr int kSortBlock = 256;
 
 struct SortParams {
-  long long N;
+  long long N, M;      // tracks of the launch; hits of the batch
   const int* offsets;   // [N+1]
   const int* surf_idx;  // [M]
   int start, lmax;      // legs of a track = surface of its last hit - start, clamped to [0, lmax]
@@ -32,7 +32,7 @@ struct SortParams {
 __device__ __forceinline__ int sort_bin_of(const SortParams& S, long long i) {
   const int o0 = S.offsets[i], o1 = S.offsets[i + 1];
   int len = 0;
-  if (o1 > o0) len = __ldg(S.surf_idx + (o1 - 1)) - S.start;
+  if (o1 > o0 && o0 >= 0 && (long long)o1 <= S.M) len = __ldg(S.surf_idx + (o1 - 1)) - S.start;  // else: malformed, not fitted
   len = max(0, min(len, S.lmax));
   // longest first: bin 0 holds the longest tracks
   const int b = S.lmax < kSortBins ? len : (int)(((long long)len * (kSortBins - 1)) / S.lmax);

@@ -8,7 +8,6 @@ tests)."""
 from __future__ import annotations
 
 import os
-from typing import Optional
 
 
 def rank_world() -> tuple:
@@ -53,14 +52,3 @@ def job_throughput(n_tracks_per_rank: int, ms_local: float, dist, device=None) -
         dist.all_reduce(c, op=dist.ReduceOp.SUM)
         total = int(c.item())
     return total / (ms * 1e-3), ms, total
-
-
-def replica_slice(n_total: int, rank: int, world: int) -> Optional[range]:
-    """Contiguous track range of `rank` when one batch is split over replicas (CSR offsets are rebased
-    by the caller).  Not used by bench.py (weak scaling: every rank fits a full batch); provided for
-    callers that feed one event to several devices, as the paper's host thread team does."""
-    if world <= 0 or not 0 <= rank < world:
-        raise ValueError("bad rank/world")
-    base, rem = divmod(int(n_total), world)
-    lo = rank * base + min(rank, rem)
-    return range(lo, lo + base + (1 if rank < rem else 0))

@@ -48,9 +48,10 @@ def chi2_excess(got, ref):
     return float(ex.max()) if ex.size else 0.0
 
 
-def compare(gpu, ref, states=False, sel=None):
+def compare(gpu, ref, states=False, sel=None, offsets=None):
     """Returns a dict of excess factors (<= 1 passes) and asserts the exact fields.
-    `sel`: optional boolean/index selection of tracks."""
+    `sel`: optional boolean/index selection of tracks; with `offsets` (the batch's CSR offsets) the per-hit
+    arrays are compared on the selected tracks' hits too."""
     def pick(a):
         return a if sel is None else a[sel]
     rep = {}
@@ -63,9 +64,14 @@ def compare(gpu, ref, states=False, sel=None):
     rep["first_cov"] = cov_excess(pick(gpu.first_cov), pick(ref.first_cov))
     rep["last_cov"] = cov_excess(pick(gpu.last_cov), pick(ref.last_cov))
     rep["chi2"] = chi2_excess(pick(gpu.chi2), pick(ref.chi2))
-    if sel is None and gpu.hit_flags is not None and ref.hit_flags is not None:
-        np.testing.assert_array_equal(gpu.hit_flags, ref.hit_flags, err_msg="hit_flags")
-        rep["hit_chi2"] = chi2_excess(gpu.hit_chi2, ref.hit_chi2)
+    if gpu.hit_flags is not None and ref.hit_flags is not None and (sel is None or offsets is not None):
+        hsel = slice(None)
+        if sel is not None:  # the hits of the selected tracks (CSR offsets of the batch)
+            keep = np.zeros(len(offsets) - 1, bool)
+            keep[sel] = True
+            hsel = np.repeat(keep, np.diff(offsets))
+        np.testing.assert_array_equal(gpu.hit_flags[hsel], ref.hit_flags[hsel], err_msg="hit_flags")
+        rep["hit_chi2"] = chi2_excess(gpu.hit_chi2[hsel], ref.hit_chi2[hsel])
     gp, rp = getattr(gpu, "perigee_params", None), getattr(ref, "perigee_params", None)
     if gp is not None and rp is not None:  # fitted parameters on the perigee surface (NaN where bit 128 is set)
         rep["perigee_params"] = param_excess(pick(gp), pick(rp))
@@ -80,10 +86,10 @@ def compare(gpu, ref, states=False, sel=None):
     return rep
 
 
-def assert_parity(gpu, ref, states=False, sel=None, label="", loosen=1.0):
+def assert_parity(gpu, ref, states=False, sel=None, label="", loosen=1.0, offsets=None):
     """loosen > 1 widens every floating-point bar by that factor (only for inputs whose conditioning
     DESIGN.md "Tolerances" shows to exceed the north_star bars, e.g. a 1e4-inflated prior)."""
-    rep = compare(gpu, ref, states=states, sel=sel)
+    rep = compare(gpu, ref, states=states, sel=sel, offsets=offsets)
     bad = {k: v for k, v in rep.items() if not v <= loosen}
     assert not bad, f"{label}: tolerance exceeded (factor over the bar): {bad}; all: {rep}"
     return rep

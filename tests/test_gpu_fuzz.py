@@ -148,11 +148,11 @@ def test_random_configuration_parity(seed):
             np.testing.assert_array_equal(got.status[runaway] & np.uint32(64), ref.status[runaway] & np.uint32(64), err_msg=label)
             # values: every track that stayed a track, with the north_star bars where the updates are well conditioned
             well = ~runaway & (kappa <= 1e5)
-            parity.assert_parity(got, ref, states=True, sel=well, loosen=loosen, label=label)
+            parity.assert_parity(got, ref, states=True, sel=well, loosen=loosen, label=label, offsets=c["offsets"])
             ill = ~runaway & ~(kappa <= 1e5)
             if np.any(ill):
                 parity.assert_parity(got, ref, states=True, sel=ill, loosen=loosen * 1e3 * kappa[ill].max() / 1e5,
-                                     label=label + " (ill-conditioned updates)")
+                                     label=label + " (ill-conditioned updates)", offsets=c["offsets"])
     # the Bryson-Frazier backward pass (kf_options.smoother) reaches the same first_*: its final step
     # C- - C- Lam C- cancels kappa_s = C-_ii / C^s_ii digits at the first leg, so the bars scale with kappa_s / 1e4
     if smooth:

@@ -447,6 +447,43 @@ def test_status_bits_and_degenerate_tracks(variant):
     np.testing.assert_array_equal(got.hit_flags, ref.hit_flags)
 
 
+def test_corrupted_csr_offsets_in_device_memory(variant):
+    """The CSR offsets are device data the host validation cannot see: a range that runs backwards or past n_meas
+    must not be dereferenced.  Such a track gets status bit 64, keeps its start state and none of its per-hit outputs
+    is written; its neighbours are fitted as if nothing had happened."""
+    import torch
+    wl = W.make_config(3, n_tracks=700, seed=21)
+    hb = kf.HostBatch.from_workload(wl)
+    for sort in (B.SORT_OFF, B.SORT_ON):
+        good = kf.FitCall(kf.DeviceBatch(hb), variant=variant, length_sort=sort).run().to_host()
+        db = kf.DeviceBatch(hb)
+        off = hb.offsets.copy()
+        off[11] = off[10] - 3             # track 10 runs backwards; track 11 starts inside track 10's hits
+        off[20] = hb.n_meas + 1000        # track 19 ends past the hit arrays; track 20 starts there
+        off[300] = -7                     # track 299 ends below zero; track 300 starts there
+        db.offsets.copy_(torch.from_numpy(off))
+        call = kf.FitCall(db, variant=variant, length_sort=sort)
+        call.out.hit_chi2.fill_(-1.0)
+        call.out.hit_flags.fill_(77)
+        got = call.run().to_host()
+        bad = np.array([10, 19, 20, 299, 300])
+        assert np.all(got.status[bad] == 64 | 8), got.status[bad]
+        np.testing.assert_array_equal(got.first_params[bad], wl.params0[bad])
+        np.testing.assert_array_equal(got.last_cov[bad], wl.cov0[bad])
+        assert np.all(got.n_used[bad] == 0)
+        ok = np.ones(700, bool)
+        ok[[10, 11, 19, 20, 299, 300]] = False   # track 11's list is valid CSR but not its own hits any more
+        for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "status", "ndf"):
+            np.testing.assert_array_equal(getattr(got, name)[ok], getattr(good, name)[ok], err_msg=name)
+        ok[9] = False                            # track 11's range now overlaps track 9's last hits (their per-hit outputs)
+        hits_ok = np.repeat(ok, np.diff(hb.offsets))
+        np.testing.assert_array_equal(got.hit_flags[hits_ok], good.hit_flags[hits_ok])
+        np.testing.assert_array_equal(got.hit_chi2[hits_ok], good.hit_chi2[hits_ok])
+        for t in (19, 20, 299, 300):             # hits that belong to no well-formed range: never written
+            assert np.all(got.hit_flags[hb.offsets[t]:hb.offsets[t + 1]] == 77)
+            assert np.all(got.hit_chi2[hb.offsets[t]:hb.offsets[t + 1]] == -1.0)
+
+
 def test_energy_exhausted_in_material(variant):
     """slow muons in zero field lose all their kinetic energy in the silicon: status bit 4, track stops,
     last_* holds the filtered state of the layer where it stopped."""
