@@ -12,66 +12,102 @@
 #include <math.h>
 #include <stdlib.h>
 #include <string.h>
+#include <tgmath.h> /* sin, cos, sqrt, fabs, ... follow the type of their argument */
+
+/* ---- the arithmetic type -------------------------------------------------------------------
+ * Every quantity of the fit is a `real`; the interface (kf_oracle.h) stays in double and converts
+ * at the door.  Three builds of this one file (oracle/__init__.py):
+ *   real = double       the oracle proper (BASELINE.json metric: FP64)
+ *   real = long double  the ARBITER: the same algorithm in x87 80-bit arithmetic (64-bit mantissa), used by the
+ *                       tests to tell which of two double-precision results is nearer the exact one where the
+ *                       conditioning of the inputs exceeds the parity bars
+ *   real = float        the paper's operating point ("All the tests use single precision ...
+ *                       with the exception of the matrix inversion"): every operand float, the 6x6 solve of the
+ *                       smoother in double (`sreal`).  Built with -fsingle-precision-constant so that literals
+ *                       do not promote an expression to double.
+ * Constants are written once as double literals: the long-double build uses the same (double-rounded) values,
+ * so that it differs from the double build by arithmetic round-off only. */
+#ifndef KFO_REAL
+#define KFO_REAL double
+#endif
+#ifndef KFO_SOLVE_REAL
+#define KFO_SOLVE_REAL double
+#endif
+typedef KFO_REAL real;
+typedef KFO_SOLVE_REAL sreal; /* type of the smoother's 6x6 solve */
 #ifdef _OPENMP
 #include <omp.h>
 #endif
 
 /* ---- constants (the CUDA path carries its own copy) ------------- */
-static const double TESLA_TO_GEV_PER_MM = 2.99792458e-4; /* 1 T = 2.99792458e-4 GeV/(e mm) */
-static const double ME_GEV = 0.51099895e-3;              /* electron mass */
-static const double K_BETHE = 0.307075;                  /* MeV mol^-1 cm^2 */
-static const double NT_MIN = 1e-6;                       /* surface reachable if n.T > NT_MIN */
-static const double SIN_THETA_MIN = 1e-12;
+static const real TESLA_TO_GEV_PER_MM = 2.99792458e-4; /* 1 T = 2.99792458e-4 GeV/(e mm) */
+static const real ME_GEV = 0.51099895e-3;              /* electron mass */
+static const real K_BETHE = 0.307075;                  /* MeV mol^-1 cm^2 */
+static const real NT_MIN = 1e-6;                       /* surface reachable if n.T > NT_MIN */
+static const real SIN_THETA_MIN = 1e-12;
 static const int MAX_SUBSTEPS = 1024;
-static const double PI = 3.14159265358979323846;
+static const real PI = 3.14159265358979323846;
+
+/* ---- the descriptors of kf_oracle.h with their numbers as `real` (converted once per call) ---- */
+typedef struct {
+  int32_t kind;
+  real b[3];
+  int32_t n[3];
+  real origin[3], spacing[3];
+  const double* grid; /* the table itself stays as given; every node value read is converted to real */
+} field_r;
+typedef struct {
+  int32_t smooth, material, n_corr_steps;
+  real outlier_chi2, max_step_mm, mass_gev, cov_inflation, mat_Z, mat_A, mat_rho, mat_I_eV, step_tolerance_mm;
+} options_r;
 
 /* ---- tiny dense helpers ------------------------------------------------------------------- */
-static void cross3(const double a[3], const double b[3], double c[3]) {
+static void cross3(const real a[3], const real b[3], real c[3]) {
   c[0] = a[1] * b[2] - a[2] * b[1];
   c[1] = a[2] * b[0] - a[0] * b[2];
   c[2] = a[0] * b[1] - a[1] * b[0];
 }
-static double dot3(const double a[3], const double b[3]) {
+static real dot3(const real a[3], const real b[3]) {
   return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
 }
 /* C (n x m) = A (n x k) * B (k x m) */
-static void matmul(int n, int k, int m, const double* A, const double* B, double* C) {
+static void matmul(int n, int k, int m, const real* A, const real* B, real* C) {
   for (int i = 0; i < n; ++i)
     for (int j = 0; j < m; ++j) {
-      double s = 0.0;
+      real s = 0.0;
       for (int l = 0; l < k; ++l) s += A[i * k + l] * B[l * m + j];
       C[i * m + j] = s;
     }
 }
 /* C (n x m) = A (n x k) * B^T, B is (m x k) */
-static void matmul_bt(int n, int k, int m, const double* A, const double* B, double* C) {
+static void matmul_bt(int n, int k, int m, const real* A, const real* B, real* C) {
   for (int i = 0; i < n; ++i)
     for (int j = 0; j < m; ++j) {
-      double s = 0.0;
+      real s = 0.0;
       for (int l = 0; l < k; ++l) s += A[i * k + l] * B[j * k + l];
       C[i * m + j] = s;
     }
 }
-static void symmetrise6(double C[36]) {
+static void symmetrise6(real C[36]) {
   for (int i = 0; i < 6; ++i)
     for (int j = i + 1; j < 6; ++j) {
-      double a = 0.5 * (C[i * 6 + j] + C[j * 6 + i]);
+      real a = 0.5 * (C[i * 6 + j] + C[j * 6 + i]);
       C[i * 6 + j] = a;
       C[j * 6 + i] = a;
     }
 }
-static int all_finite(const double* a, int n) {
+static int all_finite(const real* a, int n) {
   for (int i = 0; i < n; ++i)
     if (!isfinite(a[i])) return 0;
   return 1;
 }
-static double wrap_pi(double a) { /* into (-pi, pi]: a - 2 pi ceil((a - pi) / (2 pi)); NaN for a non-finite a */
+static real wrap_pi(real a) { /* into (-pi, pi]: a - 2 pi ceil((a - pi) / (2 pi)); NaN for a non-finite a */
   if (a > PI || a <= -PI) a = a - (2.0 * PI) * ceil((a - PI) / (2.0 * PI));
   return a;
 }
 
 /* ---- field (C.2.2 "Field") ----------------------------------------------------------------- */
-void kfo_field_at(const kfo_field* fld, const double r[3], double b[3], int32_t* clamped) {
+static void field_at_r(const field_r* fld, const real r[3], real b[3], int32_t* clamped) {
   if (fld->kind == KFO_FIELD_CONST) {
     b[0] = fld->b[0]; b[1] = fld->b[1]; b[2] = fld->b[2];
     return;
@@ -79,13 +115,13 @@ void kfo_field_at(const kfo_field* fld, const double r[3], double b[3], int32_t*
   /* trilinear: per axis f = (r_a - origin_a)/spacing_a, i = clamp(floor f, 0, n_a-2),
      w = clamp(f - i, 0, 1); outside the grid the clamped value is used */
   int idx[3];
-  double w[3];
+  real w[3];
   for (int a = 0; a < 3; ++a) {
-    double f = (r[a] - fld->origin[a]) / fld->spacing[a];
-    double fl = floor(f);
+    real f = (r[a] - fld->origin[a]) / fld->spacing[a];
+    real fl = floor(f);
     if (fl < 0.0) fl = 0.0;
-    if (fl > (double)(fld->n[a] - 2)) fl = (double)(fld->n[a] - 2);
-    double ww = f - fl;
+    if (fl > (real)(fld->n[a] - 2)) fl = (real)(fld->n[a] - 2);
+    real ww = f - fl;
     if (ww < 0.0) { ww = 0.0; if (clamped) *clamped |= 1; }
     if (ww > 1.0) { ww = 1.0; if (clamped) *clamped |= 1; }
     idx[a] = (int)fl;
@@ -96,37 +132,37 @@ void kfo_field_at(const kfo_field* fld, const double r[3], double b[3], int32_t*
   for (int dz = 0; dz < 2; ++dz)
     for (int dy = 0; dy < 2; ++dy)
       for (int dx = 0; dx < 2; ++dx) {
-        double wt = (dx ? w[0] : 1.0 - w[0]) * (dy ? w[1] : 1.0 - w[1]) * (dz ? w[2] : 1.0 - w[2]);
+        real wt = (dx ? w[0] : 1.0 - w[0]) * (dy ? w[1] : 1.0 - w[1]) * (dz ? w[2] : 1.0 - w[2]);
         const double* node =
             fld->grid + 3 * ((size_t)(idx[2] + dz) * ny * nx + (size_t)(idx[1] + dy) * nx + (idx[0] + dx));
-        b[0] += wt * node[0];
-        b[1] += wt * node[1];
-        b[2] += wt * node[2];
+        b[0] += wt * (real)node[0];
+        b[1] += wt * (real)node[1];
+        b[2] += wt * (real)node[2];
       }
 }
 
-static void field_internal(const kfo_field* fld, const double r[3], double B[3], int32_t* clamped) {
-  double bt[3];
-  kfo_field_at(fld, r, bt, clamped);
+static void field_internal(const field_r* fld, const real r[3], real B[3], int32_t* clamped) {
+  real bt[3];
+  field_at_r(fld, r, bt, clamped);
   for (int a = 0; a < 3; ++a) B[a] = bt[a] * TESLA_TO_GEV_PER_MM; /* dT/ds = lam T x B */
 }
 
 /* M(B) a := a x B */
-static void cross_matrix(const double B[3], double M[9]) {
+static void cross_matrix(const real B[3], real M[9]) {
   M[0] = 0.0;   M[1] = B[2];  M[2] = -B[1];
   M[3] = -B[2]; M[4] = 0.0;   M[5] = B[0];
   M[6] = B[1];  M[7] = -B[0]; M[8] = 0.0;
 }
 
 /* ---- C.2.2: one RKN4 step with its step Jacobian -------------------------------------------- */
-void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double h, double fo[8],
-                   double Ds[64], double* eps, int32_t* clamped) {
-  const double* r = f;
-  const double t = f[3];
-  const double* T = f + 4;
-  const double lam = f[7];
-  double B1[3], B2[3], B3[3], k1[3], k2[3], k3[3], k4[3], tmp[3], rm[3], re[3];
-  double T2[3], T3[3], T4[3];
+static void rkn4_step_r(const field_r* fld, real mass, const real f[8], real h, real fo[8],
+                   real Ds[64], real* eps, int32_t* clamped) {
+  const real* r = f;
+  const real t = f[3];
+  const real* T = f + 4;
+  const real lam = f[7];
+  real B1[3], B2[3], B3[3], k1[3], k2[3], k3[3], k4[3], tmp[3], rm[3], re[3];
+  real T2[3], T3[3], T4[3];
 
   /* stages; the field is sampled at 3 points, stages 2 and 3 share the midpoint */
   field_internal(fld, r, B1, clamped);
@@ -147,7 +183,7 @@ void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double 
   for (int a = 0; a < 3; ++a) k4[a] = lam * tmp[a];
 
   /* state */
-  double Tn[3], norm = 0.0;
+  real Tn[3], norm = 0.0;
   for (int a = 0; a < 3; ++a) {
     fo[a] = r[a] + h * T[a] + h * h / 6.0 * (k1[a] + k2[a] + k3[a]);
     Tn[a] = T[a] + h / 6.0 * (k1[a] + 2.0 * k2[a] + 2.0 * k3[a] + k4[a]);
@@ -155,18 +191,18 @@ void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double 
   }
   norm = sqrt(norm);
   for (int a = 0; a < 3; ++a) fo[4 + a] = Tn[a] / norm;
-  const double dtds = sqrt(1.0 + mass * mass * lam * lam); /* dt/ds = 1/beta, |q| = 1 */
+  const real dtds = sqrt(1.0 + mass * mass * lam * lam); /* dt/ds = 1/beta, |q| = 1 */
   fo[3] = t + h * dtds;
   fo[7] = lam;
 
   /* embedded error estimate (diagnostic only) */
-  double e = 0.0;
+  real e = 0.0;
   for (int a = 0; a < 3; ++a) e += fabs(k1[a] - k2[a] - k3[a] + k4[a]);
   if (eps) *eps = h * h * e;
 
   if (!Ds) return;
   /* step Jacobian, field gradient neglected (reading U4) */
-  double M1[9], M2[9], M3[9], d1[9], d2[9], d3[9], d4[9], P[9];
+  real M1[9], M2[9], M3[9], d1[9], d2[9], d3[9], d4[9], P[9];
   cross_matrix(B1, M1);
   cross_matrix(B2, M2);
   cross_matrix(B3, M3);
@@ -184,7 +220,7 @@ void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double 
   matmul(3, 3, 3, M3, P, d4);
   for (int i = 0; i < 9; ++i) d4[i] *= lam;
 
-  double l1[3], l2[3], l3[3], l4[3], q[3], c1[3], c2[3];
+  real l1[3], l2[3], l3[3], l4[3], q[3], c1[3], c2[3];
   cross3(T, B1, l1);
   cross3(T2, B2, c1);
   for (int a = 0; a < 3; ++a) q[a] = 0.5 * h * l1[a];
@@ -199,7 +235,7 @@ void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double 
   cross3(q, B3, c2);
   for (int a = 0; a < 3; ++a) l4[a] = c1[a] + lam * c2[a];
 
-  memset(Ds, 0, 64 * sizeof(double));
+  memset(Ds, 0, 64 * sizeof(real));
   for (int i = 0; i < 8; ++i) Ds[i * 8 + i] = 1.0;
   for (int i = 0; i < 3; ++i) {
     for (int j = 0; j < 3; ++j) {
@@ -215,21 +251,21 @@ void kfo_rkn4_step(const kfo_field* fld, double mass, const double f[8], double 
 }
 
 /* ---- C.2.1 - C.2.3: bound -> bound propagation with the 6x6 Jacobian ------------------------ */
-int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double x[6],
-                      const double* sf, const double* st, double xo[6], double J[36],
-                      double free_out[8], double* rk_err, int32_t* clamped) {
-  const double *cf = sf, *uf = sf + 3, *vf = sf + 6;
-  const double *ct = st, *ut = st + 3, *vt = st + 6, *nt = st + 9;
-  const double mass = opt->mass_gev;
+static int32_t propagate_r(const field_r* fld, const options_r* opt, const real x[6],
+                      const real* sf, const real* st, real xo[6], real J[36],
+                      real free_out[8], real* rk_err, int32_t* clamped) {
+  const real *cf = sf, *uf = sf + 3, *vf = sf + 6;
+  const real *ct = st, *ut = st + 3, *vt = st + 6, *nt = st + 9;
+  const real mass = opt->mass_gev;
 
   /* C.2.1 bound -> free on the start surface */
-  const double sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
-  double f[8];
+  const real sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
+  real f[8];
   for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
   f[3] = x[5];
   f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
   f[7] = x[4];
-  double Jb2f[48];
+  real Jb2f[48];
   memset(Jb2f, 0, sizeof(Jb2f));
   for (int a = 0; a < 3; ++a) {
     Jb2f[a * 6 + 0] = uf[a];
@@ -242,20 +278,20 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
   Jb2f[7 * 6 + 4] = 1.0;
 
   /* C.2.2 stepping: exactly n_sub + n_corr RKN4 steps, no tolerance test, no early exit */
-  double D[64], Ds[64], Dn[64];
+  real D[64], Ds[64], Dn[64];
   memset(D, 0, sizeof(D));
   for (int i = 0; i < 8; ++i) D[i * 8 + i] = 1.0;
-  double errmax = 0.0;
+  real errmax = 0.0;
   int n_sub = 1;
   {
-    double nT = dot3(nt, f + 4);
+    real nT = dot3(nt, f + 4);
     if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
-    double dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
-    double s0 = dot3(nt, dr) / nT;
+    real dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
+    real s0 = dot3(nt, dr) / nT;
     if (isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
-      double q = ceil(fabs(s0) / opt->max_step_mm * (1.0 - 1e-12));
+      real q = ceil(fabs(s0) / opt->max_step_mm * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;
-      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      if (q > (real)MAX_SUBSTEPS) q = (real)MAX_SUBSTEPS;
       n_sub = (int)q;
     }
     /* Adaptive step count ("adaptive Runge-Kutta-Nystrom"; reading U31): the embedded
@@ -264,23 +300,23 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
      * n = ceil((eps0 / tol)^(1/4)) steps bring the estimate of each to about tol.  A rule on a number, decided once
      * per leg before any step is taken: no accept/reject loop. */
     if (isfinite(opt->step_tolerance_mm) && opt->step_tolerance_mm > 0.0) {
-      double ft[8], Dt_[64], e0 = 0.0;
-      kfo_rkn4_step(fld, mass, f, s0, ft, Dt_, &e0, clamped);
-      double q = ceil(sqrt(sqrt(e0 / opt->step_tolerance_mm)) * (1.0 - 1e-12));
+      real ft[8], Dt_[64], e0 = 0.0;
+      rkn4_step_r(fld, mass, f, s0, ft, Dt_, &e0, clamped);
+      real q = ceil(sqrt(sqrt(e0 / opt->step_tolerance_mm)) * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;
-      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      if (q > (real)MAX_SUBSTEPS) q = (real)MAX_SUBSTEPS;
       if ((int)q > n_sub) n_sub = (int)q;
     }
   }
   const int n_steps = n_sub + opt->n_corr_steps;
   for (int is = 0; is < n_steps; ++is) {
-    double nT = dot3(nt, f + 4);
+    real nT = dot3(nt, f + 4);
     if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
-    double dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
-    double h = dot3(nt, dr) / nT;
-    if (is < n_sub) h = h / (double)(n_sub - is); /* the last primary step aims at the plane */
-    double fn[8], e = 0.0;
-    kfo_rkn4_step(fld, mass, f, h, fn, Ds, &e, clamped);
+    real dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
+    real h = dot3(nt, dr) / nT;
+    if (is < n_sub) h = h / (real)(n_sub - is); /* the last primary step aims at the plane */
+    real fn[8], e = 0.0;
+    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped);
     if (e > errmax) errmax = e;
     matmul(8, 8, 8, Ds, D, Dn);
     memcpy(D, Dn, sizeof(D));
@@ -290,35 +326,35 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
   if (rk_err) *rk_err = errmax;
 
   /* C.2.3 free -> bound with the path-length correction */
-  const double* r = f;
-  const double* T = f + 4;
-  const double lam = f[7];
-  const double nT = dot3(nt, T);
+  const real* r = f;
+  const real* T = f + 4;
+  const real lam = f[7];
+  const real nT = dot3(nt, T);
   if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
-  double B[3], TxB[3];
+  real B[3], TxB[3];
   field_internal(fld, r, B, clamped);
   cross3(T, B, TxB);
-  double fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
+  real fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
                   lam * TxB[0], lam * TxB[1], lam * TxB[2], 0.0};
-  double w[8] = {nt[0] / nT, nt[1] / nT, nt[2] / nT, 0.0, 0.0, 0.0, 0.0, 0.0};
-  double Pm[64];
+  real w[8] = {nt[0] / nT, nt[1] / nT, nt[2] / nT, 0.0, 0.0, 0.0, 0.0, 0.0};
+  real Pm[64];
   for (int i = 0; i < 8; ++i)
     for (int j = 0; j < 8; ++j) Pm[i * 8 + j] = (i == j ? 1.0 : 0.0) - fp[i] * w[j];
-  double Dt[64];
+  real Dt[64];
   matmul(8, 8, 8, Pm, D, Dt);
 
-  const double thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
-  const double phn = atan2(T[1], T[0]);
-  const double s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
+  const real thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
+  const real phn = atan2(T[1], T[0]);
+  const real s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
   if (!(s2 > SIN_THETA_MIN)) return KFO_ST_THETA;
-  double dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
+  real dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
   xo[0] = dot3(ut, dr);
   xo[1] = dot3(vt, dr);
   xo[2] = phn;
   xo[3] = thn;
   xo[4] = lam;
   xo[5] = f[3];
-  double Jf2b[48];
+  real Jf2b[48];
   memset(Jf2b, 0, sizeof(Jf2b));
   for (int a = 0; a < 3; ++a) {
     Jf2b[0 * 8 + a] = ut[a];
@@ -328,7 +364,7 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
   Jf2b[3 * 8 + 4] = cp * c2;  Jf2b[3 * 8 + 5] = sp * c2; Jf2b[3 * 8 + 6] = -s2;
   Jf2b[4 * 8 + 7] = 1.0;
   Jf2b[5 * 8 + 3] = 1.0;
-  double A68[48];
+  real A68[48];
   matmul(6, 8, 8, Jf2b, Dt, A68);
   matmul(6, 8, 6, A68, Jb2f, J);
   if (free_out) memcpy(free_out, f, sizeof(f));
@@ -352,18 +388,18 @@ int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double
  *   J_f2b rows: d0: e_d on r (its T-derivative vanishes on the surface, where D_perp || e_d),
  *   z0: a on r, angles / q/p / t as for planes.
  * C_out = J C J^T.  No material is crossed.  Returns 0 or the status bit that stopped it. */
-int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x[6], const double C[36],
-                    const double* sf, const double lc[3], const double la[3], double xo[6], double Co[36],
-                    double J[36], int32_t* clamped) {
-  const double *cf = sf, *uf = sf + 3, *vf = sf + 6;
-  const double mass = opt->mass_gev;
-  const double sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
-  double f[8];
+static int32_t to_line_r(const field_r* fld, const options_r* opt, const real x[6], const real C[36],
+                    const real* sf, const real lc[3], const real la[3], real xo[6], real Co[36],
+                    real J[36], int32_t* clamped) {
+  const real *cf = sf, *uf = sf + 3, *vf = sf + 6;
+  const real mass = opt->mass_gev;
+  const real sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
+  real f[8];
   for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
   f[3] = x[5];
   f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
   f[7] = x[4];
-  double Jb2f[48];
+  real Jb2f[48];
   memset(Jb2f, 0, sizeof(Jb2f));
   for (int a = 0; a < 3; ++a) {
     Jb2f[a * 6 + 0] = uf[a];
@@ -375,69 +411,69 @@ int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x
   Jb2f[6 * 6 + 2] = 0.0;         Jb2f[6 * 6 + 3] = -sth;
   Jb2f[7 * 6 + 4] = 1.0;
 
-  double D[64], Ds[64], Dn[64];
+  real D[64], Ds[64], Dn[64];
   memset(D, 0, sizeof(D));
   for (int i = 0; i < 8; ++i) D[i * 8 + i] = 1.0;
   int n_sub = 1;
   for (int is = 0;; ++is) {
-    const double* T = f + 4;
-    const double aT = dot3(la, T);
-    const double den = 1.0 - aT * aT;
+    const real* T = f + 4;
+    const real aT = dot3(la, T);
+    const real den = 1.0 - aT * aT;
     if (!(den > 1e-12)) return KFO_ST_PROPAGATION; /* moving along the axis: no closest approach */
-    double dl[3] = {f[0] - lc[0], f[1] - lc[1], f[2] - lc[2]};
-    const double da = dot3(dl, la);
-    double dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
+    real dl[3] = {f[0] - lc[0], f[1] - lc[1], f[2] - lc[2]};
+    const real da = dot3(dl, la);
+    real dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
     /* Newton step on g along the track: dg/ds = 1 - (a.T)^2 + lam D_perp . (T x B) */
-    double Bs[3], TxBs[3];
+    real Bs[3], TxBs[3];
     field_internal(fld, f, Bs, clamped);
     cross3(T, Bs, TxBs);
-    const double slope = den + f[7] * dot3(dperp, TxBs);
+    const real slope = den + f[7] * dot3(dperp, TxBs);
     if (!(fabs(slope) > 1e-12)) return KFO_ST_PROPAGATION;
-    double h = -dot3(dperp, T) / slope;
+    real h = -dot3(dperp, T) / slope;
     if (is == 0 && isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
-      double q = ceil(fabs(h) / opt->max_step_mm * (1.0 - 1e-12));
+      real q = ceil(fabs(h) / opt->max_step_mm * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;
-      if (q > (double)MAX_SUBSTEPS) q = (double)MAX_SUBSTEPS;
+      if (q > (real)MAX_SUBSTEPS) q = (real)MAX_SUBSTEPS;
       n_sub = (int)q;
     }
     if (is >= n_sub + opt->n_corr_steps) break;
-    if (is < n_sub) h = h / (double)(n_sub - is);
-    double fn[8], e = 0.0;
-    kfo_rkn4_step(fld, mass, f, h, fn, Ds, &e, clamped);
+    if (is < n_sub) h = h / (real)(n_sub - is);
+    real fn[8], e = 0.0;
+    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped);
     matmul(8, 8, 8, Ds, D, Dn);
     memcpy(D, Dn, sizeof(D));
     memcpy(f, fn, sizeof(f));
     if (!all_finite(f, 8)) return KFO_ST_PROPAGATION;
   }
 
-  const double* r = f;
-  const double* T = f + 4;
-  const double lam = f[7];
-  const double aT = dot3(la, T);
-  double dl[3] = {r[0] - lc[0], r[1] - lc[1], r[2] - lc[2]};
-  const double da = dot3(dl, la);
-  double dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
-  double B[3], TxB[3];
+  const real* r = f;
+  const real* T = f + 4;
+  const real lam = f[7];
+  const real aT = dot3(la, T);
+  real dl[3] = {r[0] - lc[0], r[1] - lc[1], r[2] - lc[2]};
+  const real da = dot3(dl, la);
+  real dperp[3] = {dl[0] - da * la[0], dl[1] - da * la[1], dl[2] - da * la[2]};
+  real B[3], TxB[3];
   field_internal(fld, r, B, clamped);
   cross3(T, B, TxB);
-  double fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
+  real fp[8] = {T[0], T[1], T[2], sqrt(1.0 + mass * mass * lam * lam),
                   lam * TxB[0], lam * TxB[1], lam * TxB[2], 0.0};
-  const double dgds = 1.0 - aT * aT + lam * dot3(dperp, TxB);
+  const real dgds = 1.0 - aT * aT + lam * dot3(dperp, TxB);
   if (!(fabs(dgds) > 1e-12)) return KFO_ST_PROPAGATION;
-  double w[8] = {(T[0] - aT * la[0]) / dgds, (T[1] - aT * la[1]) / dgds, (T[2] - aT * la[2]) / dgds, 0.0,
+  real w[8] = {(T[0] - aT * la[0]) / dgds, (T[1] - aT * la[1]) / dgds, (T[2] - aT * la[2]) / dgds, 0.0,
                  dperp[0] / dgds, dperp[1] / dgds, dperp[2] / dgds, 0.0};
-  double Pm[64], Dt[64];
+  real Pm[64], Dt[64];
   for (int i = 0; i < 8; ++i)
     for (int j = 0; j < 8; ++j) Pm[i * 8 + j] = (i == j ? 1.0 : 0.0) - fp[i] * w[j];
   matmul(8, 8, 8, Pm, D, Dt);
 
-  const double thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
-  const double phn = atan2(T[1], T[0]);
-  const double s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
+  const real thn = acos(T[2] > 1.0 ? 1.0 : (T[2] < -1.0 ? -1.0 : T[2]));
+  const real phn = atan2(T[1], T[0]);
+  const real s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
   if (!(s2 > SIN_THETA_MIN)) return KFO_ST_THETA;
-  double ed[3];
+  real ed[3];
   cross3(la, T, ed);
-  const double edn = sqrt(dot3(ed, ed));
+  const real edn = sqrt(dot3(ed, ed));
   for (int a = 0; a < 3; ++a) ed[a] /= edn;
   xo[0] = dot3(dl, ed);
   xo[1] = da;
@@ -445,7 +481,7 @@ int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x
   xo[3] = thn;
   xo[4] = lam;
   xo[5] = f[3];
-  double Jf2b[48];
+  real Jf2b[48];
   memset(Jf2b, 0, sizeof(Jf2b));
   for (int a = 0; a < 3; ++a) {
     Jf2b[0 * 8 + a] = ed[a];
@@ -455,7 +491,7 @@ int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x
   Jf2b[3 * 8 + 4] = cp * c2;  Jf2b[3 * 8 + 5] = sp * c2; Jf2b[3 * 8 + 6] = -s2;
   Jf2b[4 * 8 + 7] = 1.0;
   Jf2b[5 * 8 + 3] = 1.0;
-  double A68[48], JC[36];
+  real A68[48], JC[36];
   matmul(6, 8, 8, Jf2b, Dt, A68);
   matmul(6, 8, 6, A68, Jb2f, J);
   matmul(6, 6, 6, J, C, JC);
@@ -466,16 +502,16 @@ int32_t kfo_to_line(const kfo_field* fld, const kfo_options* opt, const double x
 }
 
 /* ---- C.2.4: gain-matrix update ------------------------------------------------ */
-int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], const double V[4],
-                   double xf[6], double Cf[36], double* chi2) {
+static int32_t update_r(const real xp[6], const real Cp[36], const real m[2], const real V[4],
+                   real xf[6], real Cf[36], real* chi2) {
   /* H = first two rows of I6 */
-  const double r0 = m[0] - xp[0], r1 = m[1] - xp[1];
-  const double S00 = Cp[0] + V[0], S01 = Cp[1] + V[1], S10 = Cp[6] + V[2], S11 = Cp[7] + V[3];
-  const double det = S00 * S11 - S01 * S10;
+  const real r0 = m[0] - xp[0], r1 = m[1] - xp[1];
+  const real S00 = Cp[0] + V[0], S01 = Cp[1] + V[1], S10 = Cp[6] + V[2], S11 = Cp[7] + V[3];
+  const real det = S00 * S11 - S01 * S10;
   if (!(S00 > 0.0 && det > 0.0)) return KFO_ST_NOT_POSITIVE; /* S must be positive definite */
-  const double Si00 = S11 / det, Si01 = -S01 / det, Si10 = -S10 / det, Si11 = S00 / det;
+  const real Si00 = S11 / det, Si01 = -S01 / det, Si10 = -S10 / det, Si11 = S00 / det;
   *chi2 = r0 * (Si00 * r0 + Si01 * r1) + r1 * (Si10 * r0 + Si11 * r1);
-  double K[12]; /* 6x2 = C H^T S^-1 */
+  real K[12]; /* 6x2 = C H^T S^-1 */
   for (int i = 0; i < 6; ++i) {
     K[i * 2 + 0] = Cp[i * 6 + 0] * Si00 + Cp[i * 6 + 1] * Si10;
     K[i * 2 + 1] = Cp[i * 6 + 0] * Si01 + Cp[i * 6 + 1] * Si11;
@@ -490,48 +526,48 @@ int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], c
 }
 
 /* ---- C.2.5: material after the update -------------------------------------------------------- */
-int32_t kfo_material(const kfo_options* opt, const double* surf, const double xf[6],
-                     const double Cf[36], double xo[6], double Co[36], double* g_out,
-                     double* theta0_out, double* dE_out) {
-  const double* n = surf + 9;
-  const double xX0 = surf[14], thick = surf[15];
-  const double m = opt->mass_gev;
-  const double lam = xf[4];
-  const double sth = sin(xf[3]), cth = cos(xf[3]), sph = sin(xf[2]), cph = cos(xf[2]);
-  const double T[3] = {cph * sth, sph * sth, cth};
-  const double p = 1.0 / fabs(lam);
-  const double E = sqrt(p * p + m * m);
-  const double beta = p / E, gamma = E / m;
-  const double cfac = 1.0 / fabs(dot3(n, T)); /* path factor */
+static int32_t material_r(const options_r* opt, const real* surf, const real xf[6],
+                     const real Cf[36], real xo[6], real Co[36], real* g_out,
+                     real* theta0_out, real* dE_out) {
+  const real* n = surf + 9;
+  const real xX0 = surf[14], thick = surf[15];
+  const real m = opt->mass_gev;
+  const real lam = xf[4];
+  const real sth = sin(xf[3]), cth = cos(xf[3]), sph = sin(xf[2]), cph = cos(xf[2]);
+  const real T[3] = {cph * sth, sph * sth, cth};
+  const real p = 1.0 / fabs(lam);
+  const real E = sqrt(p * p + m * m);
+  const real beta = p / E, gamma = E / m;
+  const real cfac = 1.0 / fabs(dot3(n, T)); /* path factor */
 
   /* multiple scattering, Highland (PDG form) */
-  const double X = xX0 * cfac;
-  const double theta0 = 0.0136 / (beta * p) * sqrt(X) * (1.0 + 0.038 * log(X / (beta * beta)));
+  const real X = xX0 * cfac;
+  const real theta0 = 0.0136 / (beta * p) * sqrt(X) * (1.0 + 0.038 * log(X / (beta * beta)));
 
   /* mean energy loss, Bethe with the asymptotic density correction */
-  const double bg = p / m;
-  const double I = opt->mat_I_eV * 1e-9; /* GeV */
-  const double ZA = opt->mat_Z / opt->mat_A;
-  const double Wmax = 2.0 * ME_GEV * bg * bg / (1.0 + 2.0 * gamma * ME_GEV / m + (ME_GEV / m) * (ME_GEV / m));
-  const double hwp = 28.816e-9 * sqrt(opt->mat_rho * ZA); /* GeV */
-  double dhalf = log(hwp / I) + log(bg) - 0.5;
+  const real bg = p / m;
+  const real I_exc = opt->mat_I_eV * 1e-9; /* GeV */
+  const real ZA = opt->mat_Z / opt->mat_A;
+  const real Wmax = 2.0 * ME_GEV * bg * bg / (1.0 + 2.0 * gamma * ME_GEV / m + (ME_GEV / m) * (ME_GEV / m));
+  const real hwp = 28.816e-9 * sqrt(opt->mat_rho * ZA); /* GeV */
+  real dhalf = log(hwp / I_exc) + log(bg) - 0.5;
   if (dhalf < 0.0) dhalf = 0.0;
-  const double dedx_mass =
-      K_BETHE * ZA / (beta * beta) * (0.5 * log(2.0 * ME_GEV * bg * bg * Wmax / (I * I)) - beta * beta - dhalf);
+  const real dedx_mass =
+      K_BETHE * ZA / (beta * beta) * (0.5 * log(2.0 * ME_GEV * bg * bg * Wmax / (I_exc * I_exc)) - beta * beta - dhalf);
   /* MeV cm^2/g * g/cm^3 = MeV/cm -> GeV/mm: 1e-3 * 0.1 */
-  const double dE = dedx_mass * opt->mat_rho * 1e-3 * 0.1 * thick * cfac;
+  const real dE = dedx_mass * opt->mat_rho * 1e-3 * 0.1 * thick * cfac;
   if (theta0_out) *theta0_out = theta0;
   if (dE_out) *dE_out = dE;
-  const double E2 = E - dE;
+  const real E2 = E - dE;
   if (!(E2 > m)) return KFO_ST_ENERGY;
-  const double p2 = sqrt(E2 * E2 - m * m);
-  const double lam2 = (lam < 0.0 ? -1.0 : 1.0) / p2;
-  const double g = (p * p * p * E2) / (p2 * p2 * p2 * E); /* dlam'/dlam, dE held constant */
+  const real p2 = sqrt(E2 * E2 - m * m);
+  const real lam2 = (lam < 0.0 ? -1.0 : 1.0) / p2;
+  const real g = (p * p * p * E2) / (p2 * p2 * p2 * E); /* dlam'/dlam, dE held constant */
   if (g_out) *g_out = g;
 
   for (int i = 0; i < 6; ++i) xo[i] = xf[i];
   xo[4] = lam2;
-  double G[36], GC[36];
+  real G[36], GC[36];
   memset(G, 0, sizeof(G));
   for (int i = 0; i < 6; ++i) G[i * 6 + i] = 1.0;
   G[4 * 6 + 4] = g;
@@ -547,9 +583,38 @@ int32_t kfo_material(const kfo_options* opt, const double* surf, const double xf
  * correlation-scaled matrix R = D^-1 C D^-1, D = diag(sqrt(C_ii)), followed by back substitution.
  * A solve, not an explicit inverse: forming C^-1 and multiplying costs a factor cond(R) in accuracy,
  * which the cancellation in C^s = C+ + A (C^s' - C-') A^T then amplifies by |C+| / |C^s| (up to 1e6
- * for an inflated prior).  Independent of the CUDA path, which uses an un-pivoted Cholesky. -------- */
-static int32_t solve_spd6(const double C[36], const double B[36], double X[36]) {
-  double s[6], R[36], Y[36];
+ * for an inflated prior; pinned against the long-double build in tests/test_oracle_precision.py).
+ * Independent of the CUDA path, which uses an un-pivoted Cholesky.
+ * The whole routine runs in `sreal`: the paper keeps its matrix inversion in double whatever the
+ * operand type, so the float build converts in and out here. -------- */
+
+/* determinant of the leading k x k block of the 6x6 matrix R, by pivoted elimination */
+static sreal leading_minor6(const sreal R[36], int k) {
+  sreal T[36], det = 1.0;
+  for (int i = 0; i < k; ++i)
+    for (int j = 0; j < k; ++j) T[i * k + j] = R[i * 6 + j];
+  for (int c = 0; c < k; ++c) {
+    int piv = c;
+    for (int i = c + 1; i < k; ++i)
+      if (fabs(T[i * k + c]) > fabs(T[piv * k + c])) piv = i;
+    if (T[piv * k + c] == 0.0) return 0.0;
+    if (piv != c) {
+      for (int j = 0; j < k; ++j) { sreal t = T[c * k + j]; T[c * k + j] = T[piv * k + j]; T[piv * k + j] = t; }
+      det = -det;
+    }
+    det *= T[c * k + c];
+    for (int i = c + 1; i < k; ++i) {
+      const sreal f = T[i * k + c] / T[c * k + c];
+      for (int j = c; j < k; ++j) T[i * k + j] -= f * T[c * k + j];
+    }
+  }
+  return det;
+}
+
+static int32_t solve_spd6(const real Cin[36], const real Bin[36], real Xout[36]) {
+  sreal C[36], B[36], X[36];
+  for (int i = 0; i < 36; ++i) { C[i] = (sreal)Cin[i]; B[i] = (sreal)Bin[i]; }
+  sreal s[6], R[36], Y[36];
   for (int i = 0; i < 6; ++i) {
     if (!(C[i * 6 + i] > 0.0)) return KFO_ST_NOT_POSITIVE;
     s[i] = sqrt(C[i * 6 + i]);
@@ -559,65 +624,56 @@ static int32_t solve_spd6(const double C[36], const double B[36], double X[36]) 
       R[i * 6 + j] = C[i * 6 + j] / (s[i] * s[j]);
       Y[i * 6 + j] = B[i * 6 + j] / s[i]; /* R (D X) = D^-1 B */
     }
-  /* an SPD matrix has positive leading minors: check them on an un-pivoted copy of the elimination
-     (the status decision), then solve with pivoting (the numbers) */
-  {
-    double T[36];
-    memcpy(T, R, sizeof(T));
-    for (int k = 0; k < 6; ++k) {
-      if (!(T[k * 6 + k] > 0.0)) return KFO_ST_NOT_POSITIVE;
-      for (int i = k + 1; i < 6; ++i) {
-        const double f = T[i * 6 + k] / T[k * 6 + k];
-        for (int j = k; j < 6; ++j) T[i * 6 + j] -= f * T[k * 6 + j];
-      }
-    }
-  }
+  /* the status decision is the definition: a symmetric matrix is positive definite iff its six leading
+     principal minors are positive (Sylvester's criterion) */
+  for (int k = 1; k <= 6; ++k)
+    if (!(leading_minor6(R, k) > 0.0)) return KFO_ST_NOT_POSITIVE;
   for (int k = 0; k < 6; ++k) {
     int piv = k;
     for (int i = k + 1; i < 6; ++i)
       if (fabs(R[i * 6 + k]) > fabs(R[piv * 6 + k])) piv = i;
     if (piv != k)
       for (int j = 0; j < 6; ++j) {
-        double t = R[k * 6 + j]; R[k * 6 + j] = R[piv * 6 + j]; R[piv * 6 + j] = t;
+        sreal t = R[k * 6 + j]; R[k * 6 + j] = R[piv * 6 + j]; R[piv * 6 + j] = t;
         t = Y[k * 6 + j]; Y[k * 6 + j] = Y[piv * 6 + j]; Y[piv * 6 + j] = t;
       }
     if (R[k * 6 + k] == 0.0) return KFO_ST_NOT_POSITIVE;
     for (int i = k + 1; i < 6; ++i) {
-      const double f = R[i * 6 + k] / R[k * 6 + k];
+      const sreal f = R[i * 6 + k] / R[k * 6 + k];
       for (int j = k; j < 6; ++j) R[i * 6 + j] -= f * R[k * 6 + j];
       for (int j = 0; j < 6; ++j) Y[i * 6 + j] -= f * Y[k * 6 + j];
     }
   }
   for (int c = 0; c < 6; ++c)
     for (int i = 5; i >= 0; --i) {
-      double v = Y[i * 6 + c];
+      sreal v = Y[i * 6 + c];
       for (int j = i + 1; j < 6; ++j) v -= R[i * 6 + j] * X[j * 6 + c];
       X[i * 6 + c] = v / R[i * 6 + i];
     }
   for (int i = 0; i < 6; ++i) /* undo the scaling: X <- D^-1 (D X) */
-    for (int c = 0; c < 6; ++c) X[i * 6 + c] /= s[i];
+    for (int c = 0; c < 6; ++c) Xout[i * 6 + c] = (real)(X[i * 6 + c] / s[i]);
   return 0;
 }
 
 /* ---- C.2.6: one RTS step ("stored Jacobians between states") ------------------- */
-int32_t kfo_rts_step(const double xf[6], const double Cf[36], const double F[36],
-                     const double xp1[6], const double Cp1[36], const double xs1[6],
-                     const double Cs1[36], double xs[6], double Cs[36]) {
-  double FC[36], At[36], A[36];
+static int32_t rts_step_r(const real xf[6], const real Cf[36], const real F[36],
+                     const real xp1[6], const real Cp1[36], const real xs1[6],
+                     const real Cs1[36], real xs[6], real Cs[36]) {
+  real FC[36], At[36], A[36];
   matmul(6, 6, 6, F, Cf, FC);          /* F C+_k  (C+ symmetric: = (C+ F^T)^T) */
   int32_t rc = solve_spd6(Cp1, FC, At); /* A_k^T = (C-_{k+1})^-1 F C+_k */
   if (rc) return rc;
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) A[i * 6 + j] = At[j * 6 + i]; /* A_k = C+_k F^T (C-_{k+1})^-1 */
-  double dx[6];
+  real dx[6];
   for (int i = 0; i < 6; ++i) dx[i] = xs1[i] - xp1[i];
   dx[2] = wrap_pi(dx[2]);
   for (int i = 0; i < 6; ++i) {
-    double s = 0.0;
+    real s = 0.0;
     for (int j = 0; j < 6; ++j) s += A[i * 6 + j] * dx[j];
     xs[i] = xf[i] + s;
   }
-  double dC[36], AdC[36], AdCAt[36];
+  real dC[36], AdC[36], AdCAt[36];
   for (int i = 0; i < 36; ++i) dC[i] = Cs1[i] - Cp1[i];
   matmul(6, 6, 6, A, dC, AdC);
   matmul_bt(6, 6, 6, AdC, A, AdCAt);
@@ -627,9 +683,37 @@ int32_t kfo_rts_step(const double xf[6], const double Cf[36], const double F[36]
   return 0;
 }
 
+/* ---- double <-> real at the interface ------------------------------------------------------------------- */
+static void get(real* dst, const double* src, int n) {
+  for (int i = 0; i < n; ++i) dst[i] = (real)src[i];
+}
+static void put(double* dst, const real* src, int n) {
+  for (int i = 0; i < n; ++i) dst[i] = (double)src[i];
+}
+static field_r field_to_real(const kfo_field* f) {
+  field_r o;
+  o.kind = f->kind;
+  for (int a = 0; a < 3; ++a) {
+    o.b[a] = (real)f->b[a];
+    o.n[a] = f->n[a];
+    o.origin[a] = (real)f->origin[a];
+    o.spacing[a] = (real)f->spacing[a];
+  }
+  o.grid = f->grid;
+  return o;
+}
+static options_r options_to_real(const kfo_options* p) {
+  options_r o;
+  o.smooth = p->smooth; o.material = p->material; o.n_corr_steps = p->n_corr_steps;
+  o.outlier_chi2 = (real)p->outlier_chi2; o.max_step_mm = (real)p->max_step_mm; o.mass_gev = (real)p->mass_gev;
+  o.cov_inflation = (real)p->cov_inflation; o.mat_Z = (real)p->mat_Z; o.mat_A = (real)p->mat_A;
+  o.mat_rho = (real)p->mat_rho; o.mat_I_eV = (real)p->mat_I_eV; o.step_tolerance_mm = (real)p->step_tolerance_mm;
+  return o;
+}
+
 /* ---- C.2: the per-track loop ----------------------------------------------------------------- */
 typedef struct {
-  double xp[6], Cp[36], F[36], xf[6], Cf[36];
+  real xp[6], Cp[36], F[36], xf[6], Cf[36];
 } leg_record;
 
 static void fill_nan(double* a, size_t n) {
@@ -639,16 +723,24 @@ static void fill_nan(double* a, size_t n) {
 int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int32_t start,
                       const int32_t* offsets, const int32_t* surf_idx, const double* loc,
                       const double* var, const double* cov01, int32_t n_surfaces,
-                      const double* geom, const kfo_field* fld, const kfo_options* opt,
+                      const double* geom_in, const kfo_field* fld_in, const kfo_options* opt_in,
                       double* first_params, double* first_cov, double* last_params,
                       double* last_cov, double* chi2_out, int32_t* ndf_out, uint32_t* status_out,
                       int32_t* n_used_out, int32_t* n_out_out, int32_t* n_holes_out,
                       double* sp_par, double* sp_cov, double* sf_par, double* sf_cov,
                       double* ss_par, double* ss_cov, double* hit_chi2, uint8_t* hit_flags,
                       double* rk_err_max, int32_t n_threads) {
-  if (N < 0 || !params0 || !cov0 || !offsets || !geom || !fld || !opt) return -1;
+  if (N < 0 || !params0 || !cov0 || !offsets || !geom_in || !fld_in || !opt_in) return -1;
   if (start < 0 || start >= n_surfaces) return -1;
   const int Lmax = n_surfaces - 1 - start;
+  /* the shared global data (geometry, field, options) as `real`, once */
+  const field_r fld_v = field_to_real(fld_in);
+  const options_r opt_v = options_to_real(opt_in);
+  const field_r* fld = &fld_v;
+  const options_r* opt = &opt_v;
+  real* geom = (real*)malloc(sizeof(real) * (size_t)n_surfaces * KFO_GEOM_STRIDE);
+  if (!geom) return -1;
+  for (size_t a = 0; a < (size_t)n_surfaces * KFO_GEOM_STRIDE; ++a) geom[a] = (real)geom_in[a];
   int used_threads = 1;
 #ifdef _OPENMP
   if (n_threads > 0) omp_set_num_threads(n_threads);
@@ -663,13 +755,13 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
   for (int64_t i = 0; i < N; ++i) {
     const int32_t o0 = offsets[i], o1 = offsets[i + 1];
     uint32_t status = 0;
-    double x[6], C[36];
-    for (int a = 0; a < 6; ++a) x[a] = params0[i * 6 + a];
-    for (int a = 0; a < 36; ++a) C[a] = opt->cov_inflation * cov0[i * 36 + a];
-    double first_x[6], first_C[36], last_x[6], last_C[36];
+    real x[6], C[36];
+    for (int a = 0; a < 6; ++a) x[a] = (real)params0[i * 6 + a];
+    for (int a = 0; a < 36; ++a) C[a] = opt->cov_inflation * (real)cov0[i * 36 + a];
+    real first_x[6], first_C[36], last_x[6], last_C[36];
     memcpy(first_x, x, sizeof(x)); memcpy(first_C, C, sizeof(C));
     memcpy(last_x, x, sizeof(x));  memcpy(last_C, C, sizeof(C));
-    double chi2 = 0.0, errmax = 0.0;
+    real chi2 = 0.0, errmax = 0.0;
     int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0;
 
     if (sp_par) fill_nan(sp_par + (size_t)i * Lmax * 6, (size_t)Lmax * 6);
@@ -698,20 +790,20 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
     } else if (o1 > o0) {
       const int n_target = surf_idx[o1 - 1] - start; /* reading U7: visit every surface up to the last hit */
       rec = (leg_record*)malloc(sizeof(leg_record) * (size_t)n_target);
-      double g_prev = 1.0;
+      real g_prev = 1.0;
       int32_t hp = o0, prev = start;
       for (int32_t s = start + 1; s <= start + n_target; ++s) {
-        const double* sf = geom + (size_t)prev * KFO_GEOM_STRIDE;
-        const double* st = geom + (size_t)s * KFO_GEOM_STRIDE;
+        const real* sf = geom + (size_t)prev * KFO_GEOM_STRIDE;
+        const real* st = geom + (size_t)s * KFO_GEOM_STRIDE;
         leg_record* R = &rec[nleg];
-        double J[36], e = 0.0;
+        real J[36], e = 0.0;
         int32_t clamped = 0;
-        int32_t rc = kfo_propagate(fld, opt, x, sf, st, R->xp, J, NULL, &e, &clamped);
+        int32_t rc = propagate_r(fld, opt, x, sf, st, R->xp, J, NULL, &e, &clamped);
         if (clamped) status |= KFO_ST_FIELD_CLAMPED;
         if (rc) { status |= (uint32_t)rc; break; }
         if (e > errmax) errmax = e;
         /* F = J G_prev (G_prev = diag(1,1,1,1,g,1) of the previous surface's energy loss) */
-        double G[36], JC[36];
+        real G[36], JC[36];
         memset(G, 0, sizeof(G));
         for (int a = 0; a < 6; ++a) G[a * 6 + a] = 1.0;
         G[4 * 6 + 4] = g_prev;
@@ -722,16 +814,17 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
         symmetrise6(R->Cp);
 
         if (hp < o1 && surf_idx[hp] == s) {
-          double V[4];
+          real V[4];
           if (var) {
-            V[0] = var[(size_t)hp * 2 + 0];
-            V[3] = var[(size_t)hp * 2 + 1];
-            V[1] = V[2] = cov01 ? cov01[hp] : 0.0;
+            V[0] = (real)var[(size_t)hp * 2 + 0];
+            V[3] = (real)var[(size_t)hp * 2 + 1];
+            V[1] = V[2] = cov01 ? (real)cov01[hp] : 0.0;
           } else {
             V[0] = st[16]; V[3] = st[17]; V[1] = V[2] = 0.0;
           }
-          double c2 = 0.0, xf[6], Cf[36];
-          rc = kfo_update(R->xp, R->Cp, loc + (size_t)hp * 2, V, xf, Cf, &c2);
+          real c2 = 0.0, xf[6], Cf[36];
+          const real m[2] = {(real)loc[(size_t)hp * 2 + 0], (real)loc[(size_t)hp * 2 + 1]};
+          rc = update_r(R->xp, R->Cp, m, V, xf, Cf, &c2);
           if (rc) { status |= (uint32_t)rc; break; }
           if (opt->outlier_chi2 > 0.0 && c2 > opt->outlier_chi2) { /* reading U9: strictly greater */
             memcpy(R->xf, R->xp, sizeof(xf));
@@ -745,7 +838,7 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
             n_used++;
             if (hit_flags) hit_flags[hp] = KFO_HIT_USED;
           }
-          if (hit_chi2) hit_chi2[hp] = c2;
+          if (hit_chi2) hit_chi2[hp] = (double)c2;
           hp++;
         } else { /* hole */
           memcpy(R->xf, R->xp, sizeof(R->xf));
@@ -757,8 +850,8 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
         memcpy(last_C, R->Cf, sizeof(last_C));
 
         if (opt->material && st[14] > 0.0) { /* reading U6: after the update, at every visited surface */
-          double g = 1.0;
-          rc = kfo_material(opt, st, R->xf, R->Cf, x, C, &g, NULL, NULL);
+          real g = 1.0;
+          rc = material_r(opt, st, R->xf, R->Cf, x, C, &g, NULL, NULL);
           if (rc) { status |= (uint32_t)rc; break; }
           g_prev = g;
         } else {
@@ -775,30 +868,30 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
       }
       for (int k = 0; k < nleg; ++k) {
         size_t o = (size_t)i * Lmax + k;
-        if (sp_par) memcpy(sp_par + o * 6, rec[k].xp, 6 * sizeof(double));
-        if (sp_cov) memcpy(sp_cov + o * 36, rec[k].Cp, 36 * sizeof(double));
-        if (sf_par) memcpy(sf_par + o * 6, rec[k].xf, 6 * sizeof(double));
-        if (sf_cov) memcpy(sf_cov + o * 36, rec[k].Cf, 36 * sizeof(double));
+        if (sp_par) put(sp_par + o * 6, rec[k].xp, 6);
+        if (sp_cov) put(sp_cov + o * 36, rec[k].Cp, 36);
+        if (sf_par) put(sf_par + o * 6, rec[k].xf, 6);
+        if (sf_cov) put(sf_cov + o * 36, rec[k].Cf, 36);
       }
 
       /* C.2.6 RTS backward pass over the visited surfaces */
       if (opt->smooth && nleg > 0) {
-        double xs[6], Cs[36];
+        real xs[6], Cs[36];
         memcpy(xs, rec[nleg - 1].xf, sizeof(xs));
         memcpy(Cs, rec[nleg - 1].Cf, sizeof(Cs));
         size_t o = (size_t)i * Lmax + (nleg - 1);
-        if (ss_par) memcpy(ss_par + o * 6, xs, sizeof(xs));
-        if (ss_cov) memcpy(ss_cov + o * 36, Cs, sizeof(Cs));
+        if (ss_par) put(ss_par + o * 6, xs, 6);
+        if (ss_cov) put(ss_cov + o * 36, Cs, 36);
         for (int k = nleg - 2; k >= 0; --k) {
-          double xn[6], Cn[36];
-          int32_t rc = kfo_rts_step(rec[k].xf, rec[k].Cf, rec[k + 1].F, rec[k + 1].xp,
+          real xn[6], Cn[36];
+          int32_t rc = rts_step_r(rec[k].xf, rec[k].Cf, rec[k + 1].F, rec[k + 1].xp,
                                     rec[k + 1].Cp, xs, Cs, xn, Cn);
           if (rc) { /* fall back to the filtered states for the remaining surfaces */
             status |= (uint32_t)rc;
             for (int kk = k; kk >= 0; --kk) {
               size_t oo = (size_t)i * Lmax + kk;
-              if (ss_par) memcpy(ss_par + oo * 6, rec[kk].xf, 6 * sizeof(double));
-              if (ss_cov) memcpy(ss_cov + oo * 36, rec[kk].Cf, 36 * sizeof(double));
+              if (ss_par) put(ss_par + oo * 6, rec[kk].xf, 6);
+              if (ss_cov) put(ss_cov + oo * 36, rec[kk].Cf, 36);
             }
             memcpy(xs, rec[0].xf, sizeof(xs));
             memcpy(Cs, rec[0].Cf, sizeof(Cs));
@@ -807,8 +900,8 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
           memcpy(xs, xn, sizeof(xs));
           memcpy(Cs, Cn, sizeof(Cs));
           o = (size_t)i * Lmax + k;
-          if (ss_par) memcpy(ss_par + o * 6, xs, sizeof(xs));
-          if (ss_cov) memcpy(ss_cov + o * 36, Cs, sizeof(Cs));
+          if (ss_par) put(ss_par + o * 6, xs, 6);
+          if (ss_cov) put(ss_cov + o * 36, Cs, 36);
         }
         memcpy(first_x, xs, sizeof(first_x));
         memcpy(first_C, Cs, sizeof(first_C));
@@ -818,18 +911,19 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
 
     const int ndf = 2 * n_used - 5; /* time is never measured: 5, not 6 (reading U10) */
     if (ndf <= 0) status |= KFO_ST_NDF;
-    if (first_params) memcpy(first_params + i * 6, first_x, sizeof(first_x));
-    if (first_cov) memcpy(first_cov + i * 36, first_C, sizeof(first_C));
-    if (last_params) memcpy(last_params + i * 6, last_x, sizeof(last_x));
-    if (last_cov) memcpy(last_cov + i * 36, last_C, sizeof(last_C));
-    if (chi2_out) chi2_out[i] = chi2;
+    if (first_params) put(first_params + i * 6, first_x, 6);
+    if (first_cov) put(first_cov + i * 36, first_C, 36);
+    if (last_params) put(last_params + i * 6, last_x, 6);
+    if (last_cov) put(last_cov + i * 36, last_C, 36);
+    if (chi2_out) chi2_out[i] = (double)chi2;
     if (ndf_out) ndf_out[i] = ndf;
     if (status_out) status_out[i] = status;
     if (n_used_out) n_used_out[i] = n_used;
     if (n_out_out) n_out_out[i] = n_outl;
     if (n_holes_out) n_holes_out[i] = n_holes;
-    if (rk_err_max) rk_err_max[i] = errmax;
+    if (rk_err_max) rk_err_max[i] = (double)errmax;
   }
+  free(geom);
   return used_threads;
 }
 
@@ -838,25 +932,143 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
  * surface first_* of track i lives on.  A track whose extrapolation stops gets KFO_ST_PERIGEE OR-ed into
  * status[i] (plus FIELD_CLAMPED when a lookup was clamped) and NaN outputs. */
 int32_t kfo_perigee_batch(int64_t N, const double* first_params, const double* first_cov,
-                          const int32_t* on_surface, const double* geometry, const kfo_field* fld,
-                          const kfo_options* opt, const double line_c[3], const double line_a[3],
+                          const int32_t* on_surface, const double* geometry, const kfo_field* fld_in,
+                          const kfo_options* opt_in, const double line_c[3], const double line_a[3],
                           double* out_params, double* out_cov, uint32_t* status) {
-  if (N < 0 || !first_params || !first_cov || !on_surface || !geometry || !fld || !opt || !out_params || !out_cov)
+  if (N < 0 || !first_params || !first_cov || !on_surface || !geometry || !fld_in || !opt_in || !out_params || !out_cov)
     return -1;
+  const field_r fld = field_to_real(fld_in);
+  const options_r opt = options_to_real(opt_in);
+  const real lc[3] = {(real)line_c[0], (real)line_c[1], (real)line_c[2]};
+  const real la[3] = {(real)line_a[0], (real)line_a[1], (real)line_a[2]};
 #pragma omp parallel for schedule(static)
   for (int64_t i = 0; i < N; ++i) {
-    double J[36];
+    real x[6], C[36], sf[KFO_GEOM_STRIDE], xo[6], Co[36], J[36];
+    get(x, first_params + i * 6, 6);
+    get(C, first_cov + i * 36, 36);
+    get(sf, geometry + (size_t)on_surface[i] * KFO_GEOM_STRIDE, KFO_GEOM_STRIDE);
     int32_t clamped = 0;
-    const int32_t rc = kfo_to_line(fld, opt, first_params + i * 6, first_cov + i * 36,
-                                   geometry + (size_t)on_surface[i] * KFO_GEOM_STRIDE, line_c, line_a,
-                                   out_params + i * 6, out_cov + i * 36, J, &clamped);
+    const int32_t rc = to_line_r(&fld, &opt, x, C, sf, lc, la, xo, Co, J, &clamped);
     if (rc != 0) {
       fill_nan(out_params + i * 6, 6);
       fill_nan(out_cov + i * 36, 36);
       if (status) status[i] |= KFO_ST_PERIGEE;
+    } else {
+      put(out_params + i * 6, xo, 6);
+      put(out_cov + i * 36, Co, 36);
     }
     if (status && clamped) status[i] |= KFO_ST_FIELD_CLAMPED;
   }
   return 0;
 }
 
+/* ---- the step-level entry points of kf_oracle.h: double in, the step in `real`, double out ---------------- */
+void kfo_field_at(const kfo_field* fld_in, const double r[3], double b_tesla[3], int32_t* clamped) {
+  const field_r fld = field_to_real(fld_in);
+  real rr[3], b[3];
+  get(rr, r, 3);
+  field_at_r(&fld, rr, b, clamped);
+  put(b_tesla, b, 3);
+}
+
+void kfo_rkn4_step(const kfo_field* fld_in, double mass_gev, const double f[8], double h, double f_out[8],
+                   double Dstep[64], double* eps, int32_t* clamped) {
+  const field_r fld = field_to_real(fld_in);
+  real fr[8], fo[8], Ds[64], e = 0.0;
+  get(fr, f, 8);
+  rkn4_step_r(&fld, (real)mass_gev, fr, (real)h, fo, Dstep ? Ds : NULL, &e, clamped);
+  put(f_out, fo, 8);
+  if (Dstep) put(Dstep, Ds, 64);
+  if (eps) *eps = (double)e;
+}
+
+int32_t kfo_propagate(const kfo_field* fld_in, const kfo_options* opt_in, const double x[6],
+                      const double* surf_from, const double* surf_to, double x_out[6], double J[36],
+                      double free_out[8], double* rk_err, int32_t* clamped) {
+  const field_r fld = field_to_real(fld_in);
+  const options_r opt = options_to_real(opt_in);
+  real xr[6], sf[KFO_GEOM_STRIDE], st[KFO_GEOM_STRIDE], xo[6], Jr[36], fo[8], e = 0.0;
+  get(xr, x, 6);
+  get(sf, surf_from, KFO_GEOM_STRIDE);
+  get(st, surf_to, KFO_GEOM_STRIDE);
+  const int32_t rc = propagate_r(&fld, &opt, xr, sf, st, xo, Jr, fo, &e, clamped);
+  if (rc) return rc;
+  put(x_out, xo, 6);
+  put(J, Jr, 36);
+  if (free_out) put(free_out, fo, 8);
+  if (rk_err) *rk_err = (double)e;
+  return 0;
+}
+
+int32_t kfo_to_line(const kfo_field* fld_in, const kfo_options* opt_in, const double x[6], const double C[36],
+                    const double* surf_from, const double line_c[3], const double line_a[3], double x_out[6],
+                    double C_out[36], double J[36], int32_t* clamped) {
+  const field_r fld = field_to_real(fld_in);
+  const options_r opt = options_to_real(opt_in);
+  real xr[6], Cr[36], sf[KFO_GEOM_STRIDE], lc[3], la[3], xo[6], Co[36], Jr[36];
+  get(xr, x, 6);
+  get(Cr, C, 36);
+  get(sf, surf_from, KFO_GEOM_STRIDE);
+  get(lc, line_c, 3);
+  get(la, line_a, 3);
+  const int32_t rc = to_line_r(&fld, &opt, xr, Cr, sf, lc, la, xo, Co, Jr, clamped);
+  if (rc) return rc;
+  put(x_out, xo, 6);
+  put(C_out, Co, 36);
+  put(J, Jr, 36);
+  return 0;
+}
+
+int32_t kfo_update(const double xp[6], const double Cp[36], const double m[2], const double V[4], double xf[6],
+                   double Cf[36], double* chi2) {
+  real xpr[6], Cpr[36], mr[2], Vr[4], xfr[6], Cfr[36], c2 = 0.0;
+  get(xpr, xp, 6);
+  get(Cpr, Cp, 36);
+  get(mr, m, 2);
+  get(Vr, V, 4);
+  const int32_t rc = update_r(xpr, Cpr, mr, Vr, xfr, Cfr, &c2);
+  if (rc) return rc;
+  put(xf, xfr, 6);
+  put(Cf, Cfr, 36);
+  *chi2 = (double)c2;
+  return 0;
+}
+
+int32_t kfo_material(const kfo_options* opt_in, const double* surf, const double xf[6], const double Cf[36],
+                     double x_out[6], double C_out[36], double* g, double* theta0, double* dE_gev) {
+  const options_r opt = options_to_real(opt_in);
+  real sr[KFO_GEOM_STRIDE], xfr[6], Cfr[36], xo[6], Co[36], gr = 1.0, th = 0.0, dE = 0.0;
+  get(sr, surf, KFO_GEOM_STRIDE);
+  get(xfr, xf, 6);
+  get(Cfr, Cf, 36);
+  const int32_t rc = material_r(&opt, sr, xfr, Cfr, xo, Co, &gr, &th, &dE);
+  if (theta0) *theta0 = (double)th;
+  if (dE_gev) *dE_gev = (double)dE;
+  if (rc) return rc;
+  put(x_out, xo, 6);
+  put(C_out, Co, 36);
+  if (g) *g = (double)gr;
+  return 0;
+}
+
+int32_t kfo_rts_step(const double xf_k[6], const double Cf_k[36], const double F_k1[36], const double xp_k1[6],
+                     const double Cp_k1[36], const double xs_k1[6], const double Cs_k1[36], double xs_k[6],
+                     double Cs_k[36]) {
+  real xf[6], Cf[36], F[36], xp1[6], Cp1[36], xs1[6], Cs1[36], xs[6], Cs[36];
+  get(xf, xf_k, 6);
+  get(Cf, Cf_k, 36);
+  get(F, F_k1, 36);
+  get(xp1, xp_k1, 6);
+  get(Cp1, Cp_k1, 36);
+  get(xs1, xs_k1, 6);
+  get(Cs1, Cs_k1, 36);
+  const int32_t rc = rts_step_r(xf, Cf, F, xp1, Cp1, xs1, Cs1, xs, Cs);
+  if (rc) return rc;
+  put(xs_k, xs, 6);
+  put(Cs_k, Cs, 36);
+  return 0;
+}
+
+/* which arithmetic this build runs in: bytes of `real` and of the 6x6 solve's type */
+int32_t kfo_real_bytes(void) { return (int32_t)sizeof(real); }
+int32_t kfo_solve_real_bytes(void) { return (int32_t)sizeof(sreal); }

@@ -141,6 +141,12 @@ int32_t kfo_perigee_batch(int64_t n_tracks, const double* first_params, const do
                           const kfo_options* opt, const double line_c[3], const double line_a[3],
                           double* out_params, double* out_cov, uint32_t* status);
 
+/* Which arithmetic this build of the oracle runs in (kf_oracle.c "the arithmetic type"): sizeof the type of
+ * every operand (8 = double: the oracle; 16 = x87 long double: the arbiter; 4 = float: the paper's operating
+ * point) and of the smoother's 6x6 solve (8, 16, 8).  The interface is double in every build. */
+int32_t kfo_real_bytes(void);
+int32_t kfo_solve_real_bytes(void);
+
 #ifdef __cplusplus
 }
 #endif

@@ -93,3 +93,49 @@ def assert_parity(gpu, ref, states=False, sel=None, label="", loosen=1.0, offset
     bad = {k: v for k, v in rep.items() if not v <= loosen}
     assert not bad, f"{label}: tolerance exceeded (factor over the bar): {bad}; all: {rep}"
     return rep
+
+
+def arbitrated(gpu, ref64, ref_ld, states=False, sel=None, offsets=None, label="", slack=2.0):
+    """Parity where the conditioning of the inputs exceeds the north_star bars.
+
+    ref_ld is the long-double build of the oracle (the same algorithm with a 64-bit mantissa) on the same inputs: the
+    nearest thing to the exact result of the algorithm.  Every quantity is compared with IT; the bar of a quantity is
+    the north_star bar, widened only where -- and only as far as -- the DOUBLE oracle itself is away from the
+    long-double result:   factor(q) = max(1, slack * excess(ref64 vs ref_ld)(q)).
+    So the CUDA path may be at most `slack` times further from the exact result than the double oracle is, or inside
+    the north_star bar, whichever is wider.  Integers, flags and status stay exact (against both builds).
+    Returns (rep_gpu_vs_ld, rep_ref64_vs_ld)."""
+    e64 = compare(ref64, ref_ld, states=states, sel=sel, offsets=offsets)
+    rep = compare(gpu, ref_ld, states=states, sel=sel, offsets=offsets)
+    bad = {k: (v, max(1.0, slack * e64.get(k, 0.0))) for k, v in rep.items() if not v <= max(1.0, slack * e64.get(k, 0.0))}
+    assert not bad, f"{label}: further from the long-double result than allowed (excess, allowed): {bad}; gpu: {rep}; f64: {e64}"
+    return rep, e64
+
+
+def resolution_loss(low, ref, offsets, cut=0.0, guard=0.1):
+    """How far a reduced-precision fit `low` (float operands) is from the double fit `ref` of the same inputs, in the
+    units that matter for the physics: parameters in standard deviations of the reference, variances relative, chi2
+    absolute.  Tracks on which a discrete decision flipped (a hit whose chi2 is within `guard` of the outlier cut, a
+    status bit) are counted and left out of the value statistics.  Returns a dict."""
+    flipped = (low.status != ref.status) | (low.n_used != ref.n_used) | (low.n_outliers != ref.n_outliers)
+    if low.hit_flags is not None and ref.hit_flags is not None:
+        hit_track = np.repeat(np.arange(len(offsets) - 1), np.diff(offsets))
+        diff = low.hit_flags != ref.hit_flags
+        if cut > 0:  # a flip is only legitimate next to the cut
+            assert np.all(np.abs(ref.hit_chi2[diff] - cut) < guard), "a hit flag flipped far from the outlier cut"
+        flipped[np.unique(hit_track[diff])] = True
+    ok = ~flipped & ((ref.status & 7) == 0)
+    out = dict(flipped_tracks=int(flipped.sum()), tracks=int(ok.sum()))
+    worst_p, worst_v = 0.0, 0.0
+    for nm in ("first", "last"):
+        xa, xb = getattr(ref, nm + "_params")[ok], getattr(low, nm + "_params")[ok]
+        va = np.einsum("nii->ni", getattr(ref, nm + "_cov")[ok])
+        vb = np.einsum("nii->ni", getattr(low, nm + "_cov")[ok])
+        d = xb - xa
+        d[:, 2] = (d[:, 2] + np.pi) % (2 * np.pi) - np.pi
+        worst_p = max(worst_p, float(np.max(np.abs(d) / np.sqrt(va))))
+        worst_v = max(worst_v, float(np.max(np.abs(vb / va - 1.0))))
+        out[nm + "_params_sigma_rms"] = [float(v) for v in np.sqrt(np.mean((d / np.sqrt(va)) ** 2, axis=0))]
+    out["params_sigma"], out["var_rel"] = worst_p, worst_v
+    out["chi2_abs"] = float(np.max(np.abs(low.chi2[ok] - ref.chi2[ok])))
+    return out

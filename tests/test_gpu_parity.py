@@ -299,15 +299,24 @@ def test_options_parity(over):
     parity.assert_parity(got, ref, states=True, label=str(over))
 
 
-def test_inflated_prior_is_conditioning_limited():
-    """cov_inflation = 1e4 (the uninformative-prior variant of reading U10).  The gain-form update
-    C+ = (I - KH) C- cancels a 25 mm^2 prior against 1e-4 mm^2 hits and the RTS recursion cancels
-    C+ (prior-sized) against a 1e6 times smaller C^s, so round-off is amplified to ~1e-9..1e-8
-    relative in *both* implementations (measured against an 80-bit
-    reference).  The bars are widened 100x here; integers and flags stay exact."""
-    wl = W.make_config(3, n_tracks=2051, seed=77)
-    got, ref = both(wl, states=True, cov_inflation=1e4)
-    parity.assert_parity(got, ref, states=True, loosen=100.0)
+@pytest.mark.parametrize("cfg,n", [(1, 2000), (3, 2051)])
+@pytest.mark.parametrize("inflation", [1e2, 1e4])
+def test_inflated_prior_against_the_long_double_arbiter(cfg, n, inflation, variant):
+    """cov_inflation = 1e4 is the uninformative-prior variant of reading U10.  The gain-form update C+ = (I - KH) C-
+    cancels a 25 mm^2 prior against 1e-4 mm^2 hits and the RTS recursion cancels a prior-sized C+ against a 1e6
+    times smaller C^s: kappa ~ 1e6 digits are lost in ANY double-precision evaluation, the oracle's included
+    (tests/test_oracle_precision.py: the double oracle is up to 5x over the covariance bar there).  So the CUDA path
+    is compared with the LONG-DOUBLE evaluation of the algorithm, and a bar is widened only as far as the double
+    oracle itself is from that result (parity.arbitrated, slack 2).  At inflation 1e2 nothing is widened."""
+    wl = W.make_config(cfg, n_tracks=n, seed=77)
+    ref = oracle.fit_workload(wl, states=True, cov_inflation=inflation)
+    ref_ld = oracle.fit_workload(wl, states=True, cov_inflation=inflation, precision="ld")
+    got = kf.fit_workload(wl, states=True, cov_inflation=inflation, variant=variant)
+    rep, e64 = parity.arbitrated(got, ref, ref_ld, states=True, label=f"cfg{cfg} inflation {inflation}")
+    if inflation <= 1e2:
+        assert max(rep.values()) < 0.05 and max(e64.values()) < 0.05, (rep, e64)
+    else:
+        assert max(e64.values()) < 10.0 and max(rep.values()) < 10.0, (rep, e64)
 
 
 def test_filter_only_with_material_and_grid_field():
