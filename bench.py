@@ -79,6 +79,9 @@ def parse_args():
     ap.add_argument("--smoother", default="rts", choices=["rts", "bf"],
                     help="backward pass (kf_options.smoother): Rauch-Tung-Striebel (default, the north_star's) or the "
                          "Bryson-Frazier form of the same smoothed state (42-double records, no 6x6 solve)")
+    ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
+                    help="arithmetic (kf_options.precision): fp64 = the BASELINE.json metric (default); mixed = the paper's "
+                         "operating point, float operands and records with the 6x6 solve in double (PAPER.md:160-164, 272)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -236,7 +239,8 @@ def main():
     bf = args.smoother == "bf"
     # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit chi2 and flags (no RKN error diagnostic)
     out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
-    call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf))
+    mixed = args.precision == "mixed"
+    call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf), precision=int(mixed))
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -311,14 +315,14 @@ def main():
             barrier()
             return replicas.max_over_ranks(h0.elapsed_time(h1), dist, dev) / ke, ke
         # the public host-buffer call: chunks of 65,536 tracks over 3 streams (H2D, fit and D2H of different chunks overlap)
-        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf))
+        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf), precision=int(mixed))
         ms_e2e, ke = time_host(hc)
         e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
                    d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke, launches_per_step=int(hc.launches),
                    api="kf_fit_batch_host_pipelined (pinned host buffers; chunks of 65536 tracks on 3 streams: "
                        "H2D, forward, RTS, D2H per chunk)")
         del hc
-        hc = kf.HostCall(hb, dev, smoother=int(bf))  # context: the same through kf_fit_batch_host, everything in order on one stream
+        hc = kf.HostCall(hb, dev, smoother=int(bf), precision=int(mixed))  # context: the same through kf_fit_batch_host, everything in order on one stream
         ms_one, _ = time_host(hc)
         e2e["single_stream_ms_per_step"] = ms_one
         del hc
@@ -332,7 +336,7 @@ def main():
     fwd = float(np.mean(fwd_ms))
     rts = float(np.mean(rts_ms)) if smooth else 0.0
     fkind = hb.field_kind
-    rec_b = (42 * 8 if bf else REC_BYTES) if smooth else 0   # Bryson-Frazier record: 42 doubles, no flag byte
+    rec_b = (42 * 8 if bf else (55 * 4 + 1 if mixed else REC_BYTES)) if smooth else 0   # Bryson-Frazier record: 42 doubles, no flag byte; MIXED: 55 floats
     fwd_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 8) + N * (2 * 27 * 8 + 8 + 5 * 4) + M * 9
     rts_bytes = n_legs * rec_b + M * HIT_BYTES + N * (27 * 8 + 12)
     if bf:  # no hits re-read; the first-leg block (27 doubles) read, first_* written
@@ -342,7 +346,7 @@ def main():
     akey = "grid3" if fkind == "grid3" else ("const" if material else "const_nomat")
     alg = dict(kf_forward_kernel=ALGORITHMIC_FLOP_PER_LEG["forward"][akey], kf_rts_kernel=ALGORITHMIC_FLOP_PER_LEG["rts"])
     # the executed counts are of the capture's workload (constant field, material, RTS); other configs: null
-    exe_ok = fkind == "const" and material == 1 and smooth and not bf
+    exe_ok = fkind == "const" and material == 1 and smooth and not bf and not mixed
     fp64_nominal = 148 * FP64_LANES_PER_SM * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12  # TFLOP/s at max clock
     fp64_peak = float(fp64_probe)   # the DFMA-chain probe of THIS run (same box, same clocks, same power cap)
     hbm_peak = peaks["hbm_gbs"]
@@ -387,7 +391,7 @@ def main():
                         what="ALGORITHMIC bytes (records + hits + per-track in/out of this launch) / CUDA-event time",
                         fp64_pipe_frac=dom.get("fp64_pipe_frac"), fp64_pipe_pct_ncu=dom.get("fp64_pipe_pct_ncu"),
                         fp64_probe_tflops=fp64_peak, fp64_nominal_tflops=fp64_nominal)
-    if args.config == 2 and smooth and not bf:  # the capture is of this workload and of the RTS kernels; else null
+    if args.config == 2 and smooth and not bf and not mixed:  # the capture is of this workload and of the RTS kernels; else null
         roofline["traffic"] = NCU_TRAFFIC["bytes_per_leg"][dkey] * n_legs
         roofline["traffic_unit"] = "bytes per launch (ncu dram read+write per leg x legs of this launch)"
         roofline["traffic_source"] = NCU_TRAFFIC["source"]
@@ -405,13 +409,15 @@ def main():
 
     line = dict(
         metric=METRIC, value=value, unit=UNIT, n_gpus=world, steps=args.steps, warmup=max(args.warmup, 3),
-        ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None, dtype="f64",
+        ms_per_step=ms_step, higher_is_better=True, scaling="weak", vs_baseline=None,
+        dtype="f32 (6x6 solve f64)" if mixed else "f64",
         data="synthetic",
         config=dict(workload=W.WORKLOAD_NAMES[args.config], tracks=N, hits=M, legs=n_legs,
                     layers=hb.n_surfaces - 1, field=fkind, smooth=int(smooth),
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
                     parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant, smoother=args.smoother,
+                    precision=args.precision,
                     extra_untimed_warmup_steps=extra_warmup,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,

@@ -56,7 +56,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 105          /* major * 100 + minor */
+#define KF_VERSION 106          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -122,6 +122,19 @@ enum { KF_SORT_AUTO = 0, KF_SORT_OFF = 1, KF_SORT_ON = 2 };
  *        kappa * 1e-16 relative to it (an inflated prior), so it is an option, not the default.  Not with
  *        KF_STATES_SMOOTH, not with KF_VARIANT_LANES_PER_TRACK (KF_ERR_UNSUPPORTED). */
 enum { KF_SMOOTHER_RTS = 0, KF_SMOOTHER_BRYSON_FRAZIER = 1 };
+
+/* kf_options.precision: the arithmetic the fit runs in.
+ *   FP64   (default; the BASELINE.json metric) every operand IEEE double.
+ *   MIXED  the paper's operating point ("All the tests use single precision ... with the
+ *          exception of the matrix inversion"): inputs are rounded to float on load, the state, the Jacobians, the
+ *          covariances and the RTS records (half the workspace, half its HBM traffic) are float, the smoother's 6x6
+ *          solve runs in double, results are widened to the double arrays of kf_outputs.  The boundary does not
+ *          change.  The fitted parameters move by at most a few per cent of their own standard deviation against the
+ *          FP64 fit (resolution-loss table); a hit whose chi2 lies within ~0.05 of the
+ *          outlier cut may be classified differently.  Thread-per-track kernels, RTS smoother, at most 1024 surfaces
+ *          (KF_ERR_UNSUPPORTED with KF_VARIANT_LANES_PER_TRACK or KF_SMOOTHER_BRYSON_FRAZIER); the perigee
+ *          extrapolation of the result (kf_outputs.perigee_*) stays in double. */
+enum { KF_PRECISION_FP64 = 0, KF_PRECISION_MIXED = 1 };
 
 /* kf_options.output_states bitmask: which per-leg states to write to kf_outputs.state_* */
 enum { KF_STATES_PRED = 1, KF_STATES_FILT = 2, KF_STATES_SMOOTH = 4 };
@@ -193,6 +206,7 @@ typedef struct kf_options {
    * through perigee_center with UNIT direction perigee_axis (the beam axis; default origin, +z) */
   double perigee_center[3];
   double perigee_axis[3];
+  int32_t precision;      /* KF_PRECISION_* */
 } kf_options;
 
 /* (4) results -- PAPER.md:180: status, track states, fitted parameters */
@@ -224,11 +238,13 @@ typedef struct kf_outputs {
 } kf_outputs;
 
 /* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
- * no step tolerance, muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis through the origin. */
+ * no step tolerance, muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis
+ * through the origin, precision FP64. */
 void kf_default_options(kf_options* opt);
 
 /* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =
- * n_surfaces - 1 - start_surface legs per track: the RTS records and leg counts (only when smooth), then the
+ * n_surfaces - 1 - start_surface legs per track: the RTS records (55 values of the precision's type + a flag byte per
+ * leg and track) and leg counts (only when smooth), then the
  * length sort's permutation and counters (4.5 B per track).  A workspace that holds only the first part is
  * accepted: the batch is then fitted unsorted (KF_SORT_ON: KF_ERR_WORKSPACE). */
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt);

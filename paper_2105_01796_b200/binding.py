@@ -25,6 +25,7 @@ STATES_PRED, STATES_FILT, STATES_SMOOTH = 1, 2, 4
 VARIANT_AUTO, VARIANT_THREAD_PER_TRACK, VARIANT_LANES_PER_TRACK = 0, 1, 2
 SORT_AUTO, SORT_OFF, SORT_ON = 0, 1, 2
 SMOOTHER_RTS, SMOOTHER_BRYSON_FRAZIER = 0, 1
+PRECISION_FP64, PRECISION_MIXED = 0, 1
 _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .. 55
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",
@@ -57,7 +58,7 @@ class KfOptions(C.Structure):
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
                 ("cov_inflation", C.c_double), ("output_states", C.c_int32), ("variant", C.c_int32),
                 ("length_sort", C.c_int32), ("smoother", C.c_int32), ("step_tolerance_mm", C.c_double),
-                ("perigee_center", C.c_double * 3), ("perigee_axis", C.c_double * 3)]
+                ("perigee_center", C.c_double * 3), ("perigee_axis", C.c_double * 3), ("precision", C.c_int32)]
 
 
 KF_MAX_STREAMS = 8
@@ -137,9 +138,9 @@ def default_options() -> KfOptions:
 
 def make_options(smooth=1, material=0, outlier_chi2=0.0, n_corr_steps=2, max_step_mm=float("inf"),
                  mass_gev=0.1056583755, cov_inflation=1.0, output_states=0, variant=0,
-                 perigee_center=(0.0, 0.0, 0.0), perigee_axis=(0.0, 0.0, 1.0), length_sort=0, step_tolerance_mm=0.0, smoother=0, **_ignored) -> KfOptions:
+                 perigee_center=(0.0, 0.0, 0.0), perigee_axis=(0.0, 0.0, 1.0), length_sort=0, step_tolerance_mm=0.0, smoother=0, precision=0, **_ignored) -> KfOptions:
     o = KfOptions()
-    o.smoother = int(smoother)
+    o.smoother, o.precision = int(smoother), int(precision)
     o.length_sort, o.step_tolerance_mm = int(length_sort), float(step_tolerance_mm)
     for k in range(3):
         o.perigee_center[k], o.perigee_axis[k] = float(perigee_center[k]), float(perigee_axis[k])

@@ -40,60 +40,64 @@ __host__ __device__ constexpr int IX(int i, int j) { return i * 6 - (i * (i - 1)
 // symmetric access with any order
 __host__ __device__ constexpr int SX(int i, int j) { return i <= j ? IX(i, j) : IX(j, i); }
 
-struct FieldDesc {
-  double b[3];        // CONST: field already in GeV/(e mm)
-  double b2;          // CONST: |b|^2
-  double inv_spacing[3];  // GRID3: 1 / spacing
+template <typename R>
+struct FieldDescT {
+  R b[3];        // CONST: field already in GeV/(e mm)
+  R b2;          // CONST: |b|^2
+  R inv_spacing[3];  // GRID3: 1 / spacing
   int n[3];           // GRID3 nodes
-  double origin[3];
-  double spacing[3];
-  const double* grid; // [nz][ny][nx][3] tesla
+  R origin[3];
+  R spacing[3];
+  const double* grid; // [nz][ny][nx][3] tesla (the table as given: double)
 };
 
-struct MaterialDesc {
-  double mass;        // GeV
-  double inv_mass;    // 1 / mass
-  double rme;         // m_e / mass
-  double inv_I2;      // 1 / I^2, GeV^-2
-  double ZA;          // Z / A
-  double rho;         // g/cm^3
-  double I_gev;       // mean excitation energy, GeV
-  double log_hwp_I;   // ln(hbar omega_p / I)
+template <typename R>
+struct MaterialDescT {
+  R mass;        // GeV
+  R inv_mass;    // 1 / mass
+  R rme;         // m_e / mass
+  R inv_I2;      // 1 / I^2, GeV^-2
+  R ZA;          // Z / A
+  R rho;         // g/cm^3
+  R I_gev;       // mean excitation energy, GeV
+  R log_hwp_I;   // ln(hbar omega_p / I)
 };
 
 // ---- 3-vector helpers ----------------------------------------------------------------------------
-__device__ __forceinline__ void cross(const double a[3], const double b[3], double c[3]) {
+template <typename R>
+__device__ __forceinline__ void cross(const R a[3], const R b[3], R c[3]) {
   c[0] = a[1] * b[2] - a[2] * b[1];
   c[1] = a[2] * b[0] - a[0] * b[2];
   c[2] = a[0] * b[1] - a[1] * b[0];
 }
-__device__ __forceinline__ double dot(const double a[3], const double b[3]) {
+template <typename R>
+__device__ __forceinline__ R dot(const R a[3], const R b[3]) {
   return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
 }
 
 // ---- field --------------------------------------------------------------------------------------
 // B(r) in GeV/(e mm).  GRID3: trilinear, clamped outside (status bit 32).
-template <int FIELD>
-__device__ __forceinline__ void field_at(const FieldDesc& F, const double r[3], double B[3],
+template <int FIELD, typename R>
+__device__ __forceinline__ void field_at(const FieldDescT<R>& F, const R r[3], R B[3],
                                          unsigned& status) {
   if constexpr (FIELD == FIELD_CONST) {
     B[0] = F.b[0]; B[1] = F.b[1]; B[2] = F.b[2];
   } else {
     int idx[3];
-    double w[3];
+    R w[3];
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
       // correctly rounded quotient from the host-rounded reciprocal (Markstein): the cell index and the
       // clamp flag must not depend on a last-bit difference from a true division
-      const double num = r[a] - F.origin[a];
-      double f = num * F.inv_spacing[a];
+      const R num = r[a] - F.origin[a];
+      R f = num * F.inv_spacing[a];
       f = fma(fma(-f, F.spacing[a], num), F.inv_spacing[a], f);
-      double fl = floor(f);
-      fl = fmax(fl, 0.0);
-      fl = fmin(fl, (double)(F.n[a] - 2));
-      double ww = f - fl;
-      if (ww < 0.0) { ww = 0.0; status |= ST_FIELD_CLAMPED; }
-      if (ww > 1.0) { ww = 1.0; status |= ST_FIELD_CLAMPED; }
+      R fl = floor(f);
+      fl = fmax(fl, R(0.0));
+      fl = fmin(fl, (R)(F.n[a] - 2));
+      R ww = f - fl;
+      if (ww < R(0.0)) { ww = R(0.0); status |= ST_FIELD_CLAMPED; }
+      if (ww > R(1.0)) { ww = R(1.0); status |= ST_FIELD_CLAMPED; }
       idx[a] = (int)fl;
       w[a] = ww;
     }
@@ -101,25 +105,26 @@ __device__ __forceinline__ void field_at(const FieldDesc& F, const double r[3], 
     const size_t row = (size_t)nx * 3;
     const size_t slab = row * (size_t)F.n[1];
     const double* base = F.grid + (size_t)idx[2] * slab + (size_t)idx[1] * row + (size_t)idx[0] * 3;
-    double acc[3] = {0.0, 0.0, 0.0};
+    R acc[3] = {R(0.0), R(0.0), R(0.0)};
 #pragma unroll
     for (int dz = 0; dz < 2; ++dz)
 #pragma unroll
       for (int dy = 0; dy < 2; ++dy) {
         const double* nd = base + dz * slab + dy * row;  // two x-adjacent nodes: 6 contiguous doubles
-        const double wyz = (dy ? w[1] : 1.0 - w[1]) * (dz ? w[2] : 1.0 - w[2]);
-        const double w0 = (1.0 - w[0]) * wyz, w1 = w[0] * wyz;
+        const R wyz = (dy ? w[1] : R(1.0) - w[1]) * (dz ? w[2] : R(1.0) - w[2]);
+        const R w0 = (R(1.0) - w[0]) * wyz, w1 = w[0] * wyz;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) acc[c] += w0 * __ldg(nd + c) + w1 * __ldg(nd + 3 + c);
+        for (int c = 0; c < 3; ++c) acc[c] += w0 * R(__ldg(nd + c)) + w1 * R(__ldg(nd + 3 + c));
       }
 #pragma unroll
-    for (int c = 0; c < 3; ++c) B[c] = acc[c] * kTeslaToGeVPerMm;
+    for (int c = 0; c < 3; ++c) B[c] = acc[c] * R(kTeslaToGeVPerMm);
   }
 }
 
 // out[:, c] = lam * (X[:, c] x B) for the three columns of the row-major 3x3 X:  out = lam M(B) X
-__device__ __forceinline__ void cross_columns(const double X[9], const double B[3], double lam,
-                                              double out[9]) {
+template <typename R>
+__device__ __forceinline__ void cross_columns(const R X[9], const R B[3], R lam,
+                                              R out[9]) {
 #pragma unroll
   for (int c = 0; c < 3; ++c) {
     out[0 + c] = lam * (X[3 + c] * B[2] - X[6 + c] * B[1]);
@@ -131,40 +136,40 @@ __device__ __forceinline__ void cross_columns(const double X[9], const double B[
 // ---- one RKN4 step (DESIGN.md "The algorithm" A.2) -------------------------------------------------
 // Advances (r, t, T) by a step of length h and returns the step-Jacobian blocks
 //   A = dr'/dT, a = dr'/dlam, Bm = dT'/dT, b = dT'/dlam, tau = dt'/dlam   (dr'/dr = I, dT'/dr = 0).
-template <int FIELD>
+template <int FIELD, typename R>
 // dtds = sqrt(1 + m^2 lam^2) and tfac = m^2 lam / dtds are constant along a leg (lam is).
-__device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, double tfac, double r[3], double& t,
-                                          double T[3], double lam, double h, double A[9],
-                                          double a[3], double Bm[9], double b[3], double& tau,
-                                          double& eps, unsigned& status) {
-  double B1[3], B2[3], B3[3];
-  const double hh = 0.5 * h;
+__device__ __forceinline__ void rkn4_step(const FieldDescT<R>& F, R dtds, R tfac, R r[3], R& t,
+                                          R T[3], R lam, R h, R A[9],
+                                          R a[3], R Bm[9], R b[3], R& tau,
+                                          R& eps, unsigned& status) {
+  R B1[3], B2[3], B3[3];
+  const R hh = R(0.5) * h;
   // stage 1
   field_at<FIELD>(F, r, B1, status);
-  double l1[3], k1[3];
+  R l1[3], k1[3];
   cross(T, B1, l1);  // dk1/dlam
 #pragma unroll
   for (int i = 0; i < 3; ++i) k1[i] = lam * l1[i];
-  double d[9];  // current dk_i/dT
-  d[0] = 0.0;            d[1] = lam * B1[2];   d[2] = -lam * B1[1];
-  d[3] = -lam * B1[2];   d[4] = 0.0;           d[5] = lam * B1[0];
-  d[6] = lam * B1[1];    d[7] = -lam * B1[0];  d[8] = 0.0;
-  double SA[9], SB[9];  // d1+d2+d3 and d1+2d2+2d3+d4
+  R d[9];  // current dk_i/dT
+  d[0] = R(0.0);            d[1] = lam * B1[2];   d[2] = -lam * B1[1];
+  d[3] = -lam * B1[2];   d[4] = R(0.0);           d[5] = lam * B1[0];
+  d[6] = lam * B1[1];    d[7] = -lam * B1[0];  d[8] = R(0.0);
+  R SA[9], SB[9];  // d1+d2+d3 and d1+2d2+2d3+d4
 #pragma unroll
   for (int i = 0; i < 9; ++i) { SA[i] = d[i]; SB[i] = d[i]; }
-  double sa[3], sb[3];  // l1+l2+l3 and l1+2l2+2l3+l4
+  R sa[3], sb[3];  // l1+l2+l3 and l1+2l2+2l3+l4
 #pragma unroll
   for (int i = 0; i < 3; ++i) { sa[i] = l1[i]; sb[i] = l1[i]; }
 
   // stage 2 (midpoint)
-  double rm[3];
+  R rm[3];
 #pragma unroll
-  for (int i = 0; i < 3; ++i) rm[i] = r[i] + hh * T[i] + 0.125 * h * h * k1[i];
+  for (int i = 0; i < 3; ++i) rm[i] = r[i] + hh * T[i] + R(0.125) * h * h * k1[i];
   field_at<FIELD>(F, rm, B2, status);
-  double X[9], v[3], k2[3], l2[3];
+  R X[9], v[3], k2[3], l2[3];
 #pragma unroll
   for (int i = 0; i < 9; ++i) X[i] = hh * d[i];
-  X[0] += 1.0; X[4] += 1.0; X[8] += 1.0;
+  X[0] += R(1.0); X[4] += R(1.0); X[8] += R(1.0);
   cross_columns(X, B2, lam, d);  // d2
 #pragma unroll
   for (int i = 0; i < 3; ++i) v[i] = T[i] + hh * k1[i];
@@ -175,15 +180,15 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
 #pragma unroll
   for (int i = 0; i < 3; ++i) k2[i] *= lam;
 #pragma unroll
-  for (int i = 0; i < 9; ++i) { SA[i] += d[i]; SB[i] += 2.0 * d[i]; }
+  for (int i = 0; i < 9; ++i) { SA[i] += d[i]; SB[i] += R(2.0) * d[i]; }
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { sa[i] += l2[i]; sb[i] += 2.0 * l2[i]; }
+  for (int i = 0; i < 3; ++i) { sa[i] += l2[i]; sb[i] += R(2.0) * l2[i]; }
 
   // stage 3 (same field point)
-  double k3[3], l3[3];
+  R k3[3], l3[3];
 #pragma unroll
   for (int i = 0; i < 9; ++i) X[i] = hh * d[i];
-  X[0] += 1.0; X[4] += 1.0; X[8] += 1.0;
+  X[0] += R(1.0); X[4] += R(1.0); X[8] += R(1.0);
   cross_columns(X, B2, lam, d);  // d3
 #pragma unroll
   for (int i = 0; i < 3; ++i) v[i] = T[i] + hh * k2[i];
@@ -194,18 +199,18 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
 #pragma unroll
   for (int i = 0; i < 3; ++i) k3[i] *= lam;
 #pragma unroll
-  for (int i = 0; i < 9; ++i) { SA[i] += d[i]; SB[i] += 2.0 * d[i]; }
+  for (int i = 0; i < 9; ++i) { SA[i] += d[i]; SB[i] += R(2.0) * d[i]; }
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { sa[i] += l3[i]; sb[i] += 2.0 * l3[i]; }
+  for (int i = 0; i < 3; ++i) { sa[i] += l3[i]; sb[i] += R(2.0) * l3[i]; }
 
   // stage 4 (end point)
-  double re[3], k4[3], l4[3];
+  R re[3], k4[3], l4[3];
 #pragma unroll
-  for (int i = 0; i < 3; ++i) re[i] = r[i] + h * T[i] + 0.5 * h * h * k3[i];
+  for (int i = 0; i < 3; ++i) re[i] = r[i] + h * T[i] + R(0.5) * h * h * k3[i];
   field_at<FIELD>(F, re, B3, status);
 #pragma unroll
   for (int i = 0; i < 9; ++i) X[i] = h * d[i];
-  X[0] += 1.0; X[4] += 1.0; X[8] += 1.0;
+  X[0] += R(1.0); X[4] += R(1.0); X[8] += R(1.0);
   cross_columns(X, B3, lam, d);  // d4
 #pragma unroll
   for (int i = 0; i < 3; ++i) v[i] = T[i] + h * k3[i];
@@ -221,11 +226,11 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
   for (int i = 0; i < 3; ++i) sb[i] += l4[i];
 
   // Jacobian blocks
-  const double h6 = h * (1.0 / 6.0), h26 = h * h6;
+  const R h6 = h * (R(1.0) / R(6.0)), h26 = h * h6;
 #pragma unroll
   for (int i = 0; i < 9; ++i) { A[i] = h26 * SA[i]; Bm[i] = h6 * SB[i]; }
   A[0] += h; A[4] += h; A[8] += h;
-  Bm[0] += 1.0; Bm[4] += 1.0; Bm[8] += 1.0;
+  Bm[0] += R(1.0); Bm[4] += R(1.0); Bm[8] += R(1.0);
 #pragma unroll
   for (int i = 0; i < 3; ++i) { a[i] = h26 * sa[i]; b[i] = h6 * sb[i]; }
   tau = h * tfac;
@@ -235,13 +240,13 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
                  fabs(k1[2] - k2[2] - k3[2] + k4[2]));
 
   // state
-  double Tn[3];
+  R Tn[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     r[i] = r[i] + h * T[i] + h26 * (k1[i] + k2[i] + k3[i]);
-    Tn[i] = T[i] + h6 * (k1[i] + 2.0 * k2[i] + 2.0 * k3[i] + k4[i]);
+    Tn[i] = T[i] + h6 * (k1[i] + R(2.0) * k2[i] + R(2.0) * k3[i] + k4[i]);
   }
-  const double inrm = rsqrt_near_one(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
+  const R inrm = rsqrt_near_one(Tn[0] * Tn[0] + Tn[1] * Tn[1] + Tn[2] * Tn[2]);
 #pragma unroll
   for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
   t += h * dtds;
@@ -260,56 +265,58 @@ __device__ __forceinline__ void rkn4_step(const FieldDesc& F, double dtds, doubl
 // Same discrete step, same Jacobian as the general code path: only the arithmetic is regrouped.  All
 // step Jacobians commute, so the accumulated D keeps the form  P = P0 I + P1 M_B + P2 M_B^2 (dr/dT0),
 // Q = I + Q1 M_B + Q2 M_B^2 (dT/dT0): six scalars instead of two 3x3 matrices.
-struct PolyJac {
-  double P0, P1, P2, Q1, Q2;  // Q0 == 1
-  double p[3], q[3], sigma;   // dr/dlam, dT/dlam, dt/dlam
+template <typename R>
+struct PolyJacT {
+  R P0, P1, P2, Q1, Q2;  // Q0 == 1
+  R p[3], q[3], sigma;   // dr/dlam, dT/dlam, dt/dlam
 };
 
 // v -> c0 v + c1 (v x B) + c2 ((v x B) x B)
-__device__ __forceinline__ void poly_apply(const double B[3], double c0, double c1, double c2,
-                                           const double v[3], const double vx[3], const double vxx[3],
-                                           double out[3]) {
+template <typename R>
+__device__ __forceinline__ void poly_apply(const R B[3], R c0, R c1, R c2,
+                                           const R v[3], const R vx[3], const R vxx[3],
+                                           R out[3]) {
 #pragma unroll
   for (int i = 0; i < 3; ++i) out[i] = fma(c2, vxx[i], fma(c1, vx[i], c0 * v[i]));
 }
 
-template <bool FIRST>
-__device__ __forceinline__ void const_field_step(const double B[3], double b2, double dtds, double tfac,
-                                                 double lam, double h, double r[3], double& t, double T[3],
-                                                 PolyJac& D, double& errmax) {
-  const double u = h * lam, uu = u * u, s = uu * b2;
-  const double e = fma(s, -1.0 / 24.0, 0.5);
-  const double c1 = u * fma(s, -1.0 / 6.0, 1.0);
-  const double c2 = uu * e;
-  const double a1 = h * u * e;
-  const double a2 = h * uu * (1.0 / 6.0);
-  const double hh = h * h;
-  const double dc1 = h * fma(s, -0.5, 1.0), dc2 = h * c1;
-  const double da1 = hh * fma(s, -0.125, 0.5), da2 = hh * u * (1.0 / 3.0);
-  double w1[3], w2[3];
+template <bool FIRST, typename R>
+__device__ __forceinline__ void const_field_step(const R B[3], R b2, R dtds, R tfac,
+                                                 R lam, R h, R r[3], R& t, R T[3],
+                                                 PolyJacT<R>& D, R& errmax) {
+  const R u = h * lam, uu = u * u, s = uu * b2;
+  const R e = fma(s, -R(1.0) / R(24.0), R(0.5));
+  const R c1 = u * fma(s, -R(1.0) / R(6.0), R(1.0));
+  const R c2 = uu * e;
+  const R a1 = h * u * e;
+  const R a2 = h * uu * (R(1.0) / R(6.0));
+  const R hh = h * h;
+  const R dc1 = h * fma(s, -R(0.5), R(1.0)), dc2 = h * c1;
+  const R da1 = hh * fma(s, -R(0.125), R(0.5)), da2 = hh * u * (R(1.0) / R(3.0));
+  R w1[3], w2[3];
   cross(T, B, w1);
   cross(w1, B, w2);
-  double av[3], bv[3];
+  R av[3], bv[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     av[i] = fma(da2, w2[i], da1 * w1[i]);
     bv[i] = fma(dc2, w2[i], dc1 * w1[i]);
   }
-  const double eps = hh * fabs(lam) * 0.25 * s *
+  const R eps = hh * fabs(lam) * R(0.25) * s *
                      (fabs(fma(u, w2[0], w1[0])) + fabs(fma(u, w2[1], w1[1])) + fabs(fma(u, w2[2], w1[2])));
   errmax = fmax(errmax, eps);
   // state
-  double Tn[3];
+  R Tn[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     r[i] = fma(a2, w2[i], fma(a1, w1[i], fma(h, T[i], r[i])));
     Tn[i] = fma(c2, w2[i], fma(c1, w1[i], T[i]));
   }
-  const double inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+  const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
 #pragma unroll
   for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
   t = fma(h, dtds, t);
-  const double tau = h * tfac;
+  const R tau = h * tfac;
   // D <- Dstep D
   if constexpr (FIRST) {
     D.P0 = h; D.P1 = a1; D.P2 = a2; D.Q1 = c1; D.Q2 = c2;
@@ -317,7 +324,7 @@ __device__ __forceinline__ void const_field_step(const double B[3], double b2, d
     for (int i = 0; i < 3; ++i) { D.p[i] = av[i]; D.q[i] = bv[i]; }
     D.sigma = tau;
   } else {
-    double qx[3], qxx[3];
+    R qx[3], qxx[3];
     cross(D.q, B, qx);
     cross(qx, B, qxx);
 #pragma unroll
@@ -326,7 +333,7 @@ __device__ __forceinline__ void const_field_step(const double B[3], double b2, d
       D.q[i] += fma(c2, qxx[i], fma(c1, qx[i], bv[i]));
     }
     // polynomial products modulo M_B^3 = -b2 M_B:  P += A Q,  Q = Bm Q   (A0 = h, Bm0 = Q0 = 1)
-    const double Q1 = D.Q1, Q2 = D.Q2;
+    const R Q1 = D.Q1, Q2 = D.Q2;
     D.P0 += h;
     D.P1 += fma(h, Q1, a1) - b2 * fma(a1, Q2, a2 * Q1);
     D.P2 += fma(h, Q2, fma(a1, Q1, a2)) - b2 * (a2 * Q2);
@@ -337,93 +344,97 @@ __device__ __forceinline__ void const_field_step(const double B[3], double b2, d
 }
 
 // 3x3 row-major helpers (general field path)
-__device__ __forceinline__ void mat3_mul(const double A[9], const double B[9], double C[9]) {
+template <typename R>
+__device__ __forceinline__ void mat3_mul(const R A[9], const R B[9], R C[9]) {
 #pragma unroll
   for (int i = 0; i < 3; ++i)
 #pragma unroll
     for (int j = 0; j < 3; ++j)
       C[i * 3 + j] = A[i * 3 + 0] * B[0 + j] + A[i * 3 + 1] * B[3 + j] + A[i * 3 + 2] * B[6 + j];
 }
-__device__ __forceinline__ void mat3_vec(const double A[9], const double x[3], double y[3]) {
+template <typename R>
+__device__ __forceinline__ void mat3_vec(const R A[9], const R x[3], R y[3]) {
 #pragma unroll
   for (int i = 0; i < 3; ++i) y[i] = A[i * 3 + 0] * x[0] + A[i * 3 + 1] * x[1] + A[i * 3 + 2] * x[2];
 }
 
-struct MatJac {
-  double P[9], Q[9], p[3], q[3], sigma;
+template <typename R>
+struct MatJacT {
+  R P[9], Q[9], p[3], q[3], sigma;
 };
 
 // The bound-to-bound Jacobian, non-trivial part: Ja rows (loc0, loc1, phi, theta) x columns
 // (loc0, loc1, phi, theta, qp); Jt = row t over the same columns.  Row qp = e_qp, column t = e_t.
-struct BoundJacobian {
-  double Ja[4][5];
-  double Jt[5];
+template <typename R>
+struct BoundJacobianT {
+  R Ja[4][5];
+  R Jt[5];
 };
 
 // ---- propagate a bound state from surface sf to surface st (A.1 - A.3) ---------------------------
 // trig = (sin phi, cos phi, sin theta, cos theta) of x on entry; on success it holds the values of
 // the predicted (phi, theta), taken from the direction vector itself.  Returns 0 or the stopping bit.
-template <int FIELD>
-__device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, int n_corr,
-                                              double max_step, double step_tol, const double* __restrict__ sf,
-                                              const double* __restrict__ st, const double x[6],
-                                              double trig[4], double xo[6], BoundJacobian& J,
-                                              double& errmax, unsigned& status) {
-  const double sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
+template <int FIELD, typename R>
+__device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, int n_corr,
+                                              R max_step, R step_tol, const R* __restrict__ sf,
+                                              const R* __restrict__ st, const R x[6],
+                                              R trig[4], R xo[6], BoundJacobianT<R>& J,
+                                              R& errmax, unsigned& status) {
+  const R sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
   // A.1 bound -> free
-  double r[3], T[3];
+  R r[3], T[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) r[i] = fma(x[1], sf[6 + i], fma(x[0], sf[3 + i], sf[i]));
   T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
-  const double lam = x[4];
-  double t = x[5];
-  const double Tphi[3] = {-T[1], T[0], 0.0};
-  const double Tth[3] = {cphi * cth, sphi * cth, -sth};
-  const double nt[3] = {st[9], st[10], st[11]};
-  const double ct[3] = {st[0], st[1], st[2]};
-  const double ml = mass * lam;
-  double idtds;
-  const double dtds = sqrt_nr(fma(ml, ml, 1.0), idtds);  // dt/ds = sqrt(1 + m^2 lam^2)
-  const double tfac = mass * ml * idtds;                  // d(dt/ds)/dlam
+  const R lam = x[4];
+  R t = x[5];
+  const R Tphi[3] = {-T[1], T[0], R(0.0)};
+  const R Tth[3] = {cphi * cth, sphi * cth, -sth};
+  const R nt[3] = {st[9], st[10], st[11]};
+  const R ct[3] = {st[0], st[1], st[2]};
+  const R ml = mass * lam;
+  R idtds;
+  const R dtds = sqrt_nr(fma(ml, ml, R(1.0)), idtds);  // dt/ds = sqrt(1 + m^2 lam^2)
+  const R tfac = mass * ml * idtds;                  // d(dt/ds)/dlam
 
   // A.2 stepping: n_sub primary steps + n_corr correction steps, no accept/reject
   int n_sub = 1;
-  double nT = dot(nt, T);
-  if (!(nT > kNdotTMin)) return ST_PROPAGATION;
-  if (max_step > 0.0 || step_tol > 0.0) {
-    const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-    const double s0 = dot(nt, dr) / nT;
-    if (max_step > 0.0) {
-      double qn = ceil(fabs(s0) / max_step * (1.0 - 1e-12));
-      if (!(qn >= 1.0)) qn = 1.0;
-      if (qn > 1024.0) qn = 1024.0;
+  R nT = dot(nt, T);
+  if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+  if (max_step > R(0.0) || step_tol > R(0.0)) {
+    const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+    const R s0 = dot(nt, dr) / nT;
+    if (max_step > R(0.0)) {
+      R qn = ceil(fabs(s0) / max_step * (R(1.0) - R(1e-12)));
+      if (!(qn >= R(1.0))) qn = R(1.0);
+      if (qn > R(1024.0)) qn = R(1024.0);
       n_sub = (int)qn;
     }
-    if (step_tol > 0.0) {
+    if (step_tol > R(0.0)) {
       // adaptive step count (U31): the embedded error estimate of ONE trial step over the
       // whole leg fixes the number of primary steps, n = ceil((eps0 / tol)^(1/4)); the trial step is discarded
-      double e0;
+      R e0;
       if constexpr (FIELD == FIELD_CONST) {
         // closed form of h^2 |k1 - k2 - k3 + k4|_1 in a constant field (const_field_step)
-        const double u = s0 * lam, sq = u * u * F.b2;
-        double w1[3], w2[3];
+        const R u = s0 * lam, sq = u * u * F.b2;
+        R w1[3], w2[3];
         cross(T, F.b, w1);
         cross(w1, F.b, w2);
-        e0 = s0 * s0 * fabs(lam) * 0.25 * sq *
+        e0 = s0 * s0 * fabs(lam) * R(0.25) * sq *
              (fabs(fma(u, w2[0], w1[0])) + fabs(fma(u, w2[1], w1[1])) + fabs(fma(u, w2[2], w1[2])));
       } else {
-        double rr[3] = {r[0], r[1], r[2]}, TT[3] = {T[0], T[1], T[2]}, tt = t;
-        double A[9], a[3], Bm[9], b[3], tau;
+        R rr[3] = {r[0], r[1], r[2]}, TT[3] = {T[0], T[1], T[2]}, tt = t;
+        R A[9], a[3], Bm[9], b[3], tau;
         rkn4_step<FIELD>(F, dtds, tfac, rr, tt, TT, lam, s0, A, a, Bm, b, tau, e0, status);
       }
-      double qn = ceil(sqrt(sqrt(e0 / step_tol)) * (1.0 - 1e-12));
-      if (!(qn >= 1.0)) qn = 1.0;
-      if (qn > 1024.0) qn = 1024.0;
+      R qn = ceil(sqrt(sqrt(e0 / step_tol)) * (R(1.0) - R(1e-12)));
+      if (!(qn >= R(1.0))) qn = R(1.0);
+      if (qn > R(1024.0)) qn = R(1024.0);
       if ((int)qn > n_sub) n_sub = (int)qn;
     }
   }
   const int n_steps = n_sub + n_corr;
-  typename std::conditional<FIELD == FIELD_CONST, PolyJac, MatJac>::type D;
+  typename std::conditional<FIELD == FIELD_CONST, PolyJacT<R>, MatJacT<R>>::type D;
   bool fast = false;
   if constexpr (FIELD == FIELD_CONST) {
     // default policy (one primary + two correction steps) in a constant field: the three steps as one
@@ -435,30 +446,30 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
       for (int is = 0; is < 3; ++is) {
         if (is > 0) {
           nT = dot(nt, T);
-          bad = bad || !(nT > kNdotTMin);
+          bad = bad || !(nT > R(kNdotTMin));
         }
-        const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-        const double h = dot(nt, dr) * rcp_nr(nT);
+        const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+        const R h = dot(nt, dr) * rcp_nr(nT);
         if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
         else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
       }
-      const double fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
-      if (bad || !(fabs(fin) < 1.0e300)) return ST_PROPAGATION;  // non-finite values persist through the steps
+      const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
+      if (bad || !(fabs(fin) < big<R>())) return ST_PROPAGATION;  // non-finite values persist through the steps
     }
   }
   for (int is = 0; !fast && is < n_steps; ++is) {
     if (is > 0) {
       nT = dot(nt, T);
-      if (!(nT > kNdotTMin)) return ST_PROPAGATION;
+      if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
     }
-    const double dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-    double h = dot(nt, dr) * rcp_nr(nT);
-    if (is < n_sub - 1) h = h / (double)(n_sub - is);
+    const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+    R h = dot(nt, dr) * rcp_nr(nT);
+    if (is < n_sub - 1) h = h / (R)(n_sub - is);
     if constexpr (FIELD == FIELD_CONST) {
       if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
       else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
     } else {
-      double A[9], a[3], Bm[9], b[3], tau, eps;
+      R A[9], a[3], Bm[9], b[3], tau, eps;
       rkn4_step<FIELD>(F, dtds, tfac, r, t, T, lam, h, A, a, Bm, b, tau, eps, status);
       errmax = fmax(errmax, eps);
       if (is == 0) {
@@ -469,7 +480,7 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
         D.sigma = tau;
       } else {
         // D <- Dstep D:  P += A Q,  p += A q + a,  Q = Bm Q,  q = Bm q + b,  sigma += tau
-        double AQ[9], Aq[3], BQ[9], Bq[3];
+        R AQ[9], Aq[3], BQ[9], Bq[3];
         mat3_mul(A, D.Q, AQ);
         mat3_vec(A, D.q, Aq);
         mat3_mul(Bm, D.Q, BQ);
@@ -481,34 +492,34 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
         D.sigma += tau;
       }
     }
-    const double fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
-    if (!(fabs(fin) < 1.0e300)) return ST_PROPAGATION;  // catches NaN and Inf
+    const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
+    if (!(fabs(fin) < big<R>())) return ST_PROPAGATION;  // catches NaN and Inf
   }
 
   // A.3 free -> bound with the path-length correction  D~ = (I - f' w^T) D
   nT = dot(nt, T);
-  if (!(nT > kNdotTMin)) return ST_PROPAGATION;
-  double Bend[3], TxB[3];
+  if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+  R Bend[3], TxB[3];
   field_at<FIELD>(F, r, Bend, status);
   cross(T, Bend, TxB);
-  const double kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};  // dT/ds
-  const double inT = rcp_nr(nT);
-  const double w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
+  const R kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};  // dT/ds
+  const R inT = rcp_nr(nT);
+  const R w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
 
-  const double st2 = fma(T[0], T[0], T[1] * T[1]);
-  if (!(st2 > kSinThetaMin * kSinThetaMin)) return ST_THETA;
-  double isth;
-  const double sth2 = sqrt_nr(st2, isth);
-  const double cth2 = T[2];
-  const double cph2 = T[0] * isth, sph2 = T[1] * isth;
-  const double gphi[2] = {-sph2 * isth, cph2 * isth};
-  const double gth[3] = {cph2 * cth2, sph2 * cth2, -sth2};
-  const double* ut = st + 3;
-  const double* vt = st + 6;
+  const R st2 = fma(T[0], T[0], T[1] * T[1]);
+  if (!(st2 > R(kSinThetaMin) * R(kSinThetaMin))) return ST_THETA;
+  R isth;
+  const R sth2 = sqrt_nr(st2, isth);
+  const R cth2 = T[2];
+  const R cph2 = T[0] * isth, sph2 = T[1] * isth;
+  const R gphi[2] = {-sph2 * isth, cph2 * isth};
+  const R gth[3] = {cph2 * cth2, sph2 * cth2, -sth2};
+  const R* ut = st + 3;
+  const R* vt = st + 6;
 
   // columns of D J_b2f as (cr, ct_, cT); then c -= f' (w . cr); then rows of J_f2b
-  auto project = [&](int c, double cr[3], double ctime, double cT[3]) {
-    const double wd = dot(w, cr);
+  auto project = [&](int c, R cr[3], R ctime, R cT[3]) {
+    const R wd = dot(w, cr);
 #pragma unroll
     for (int i = 0; i < 3; ++i) { cr[i] = fma(-T[i], wd, cr[i]); cT[i] = fma(-kf_[i], wd, cT[i]); }
     J.Ja[0][c] = dot(ut, cr);
@@ -518,96 +529,97 @@ __device__ __forceinline__ unsigned propagate(const FieldDesc& F, double mass, i
     J.Jt[c] = fma(-dtds, wd, ctime);
   };
   {
-    double cr[3] = {sf[3], sf[4], sf[5]}, cT[3] = {0.0, 0.0, 0.0};
-    project(0, cr, 0.0, cT);
+    R cr[3] = {sf[3], sf[4], sf[5]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
+    project(0, cr, R(0.0), cT);
   }
   {
-    double cr[3] = {sf[6], sf[7], sf[8]}, cT[3] = {0.0, 0.0, 0.0};
-    project(1, cr, 0.0, cT);
+    R cr[3] = {sf[6], sf[7], sf[8]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
+    project(1, cr, R(0.0), cT);
   }
   if constexpr (FIELD == FIELD_CONST) {
     {
-      double vx[3], vxx[3], cr[3], cT[3];
+      R vx[3], vxx[3], cr[3], cT[3];
       cross(Tphi, F.b, vx);
       cross(vx, F.b, vxx);
       poly_apply(F.b, D.P0, D.P1, D.P2, Tphi, vx, vxx, cr);
-      poly_apply(F.b, 1.0, D.Q1, D.Q2, Tphi, vx, vxx, cT);
-      project(2, cr, 0.0, cT);
+      poly_apply(F.b, R(1.0), D.Q1, D.Q2, Tphi, vx, vxx, cT);
+      project(2, cr, R(0.0), cT);
     }
     {
-      double vx[3], vxx[3], cr[3], cT[3];
+      R vx[3], vxx[3], cr[3], cT[3];
       cross(Tth, F.b, vx);
       cross(vx, F.b, vxx);
       poly_apply(F.b, D.P0, D.P1, D.P2, Tth, vx, vxx, cr);
-      poly_apply(F.b, 1.0, D.Q1, D.Q2, Tth, vx, vxx, cT);
-      project(3, cr, 0.0, cT);
+      poly_apply(F.b, R(1.0), D.Q1, D.Q2, Tth, vx, vxx, cT);
+      project(3, cr, R(0.0), cT);
     }
   } else {
     {
-      double cr[3], cT[3];
+      R cr[3], cT[3];
       mat3_vec(D.P, Tphi, cr);
       mat3_vec(D.Q, Tphi, cT);
-      project(2, cr, 0.0, cT);
+      project(2, cr, R(0.0), cT);
     }
     {
-      double cr[3], cT[3];
+      R cr[3], cT[3];
       mat3_vec(D.P, Tth, cr);
       mat3_vec(D.Q, Tth, cT);
-      project(3, cr, 0.0, cT);
+      project(3, cr, R(0.0), cT);
     }
   }
   {
-    double cr[3] = {D.p[0], D.p[1], D.p[2]}, cT[3] = {D.q[0], D.q[1], D.q[2]};
+    R cr[3] = {D.p[0], D.p[1], D.p[2]}, cT[3] = {D.q[0], D.q[1], D.q[2]};
     project(4, cr, D.sigma, cT);
   }
 
-  const double dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
+  const R dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
   xo[0] = dot(ut, dr);
   xo[1] = dot(vt, dr);
   // phi' = atan2(Ty, Tx) and theta' = acos(Tz), taken as the input angle plus the rotation over the leg
   // (sin of the difference from the two direction vectors) whenever that rotation is small
   {
-    const double sdp = fma(sph2, cphi, -cph2 * sphi), cdp = fma(cph2, cphi, sph2 * sphi);
-    const double sdt = fma(sth2, cth, -cth2 * sth), cdt = fma(cth2, cth, sth2 * sth);
-    if (fabs(sdp) <= kSmallSine && cdp > 0.0 && fabs(sdt) <= kSmallSine && cdt > 0.0 && fabs(x[2]) <= kPi &&
-        x[3] > 0.0 && x[3] < kPi) {
-      double ph = x[2] + asin_small(sdp);
-      if (ph > kPi) ph -= 2.0 * kPi;
-      else if (ph <= -kPi) ph += 2.0 * kPi;
+    const R sdp = fma(sph2, cphi, -cph2 * sphi), cdp = fma(cph2, cphi, sph2 * sphi);
+    const R sdt = fma(sth2, cth, -cth2 * sth), cdt = fma(cth2, cth, sth2 * sth);
+    if (fabs(sdp) <= R(kSmallSine) && cdp > R(0.0) && fabs(sdt) <= R(kSmallSine) && cdt > R(0.0) && fabs(x[2]) <= R(kPi) &&
+        x[3] > R(0.0) && x[3] < R(kPi)) {
+      R ph = x[2] + asin_small(sdp);
+      if (ph > R(kPi)) ph -= R(2.0) * R(kPi);
+      else if (ph <= -R(kPi)) ph += R(2.0) * R(kPi);
       xo[2] = ph;
       xo[3] = x[3] + asin_small(sdt);
     } else {
       xo[2] = atan2(T[1], T[0]);
-      xo[3] = acos(fmin(fmax(T[2], -1.0), 1.0));
+      xo[3] = acos(fmin(fmax(T[2], -R(1.0)), R(1.0)));
     }
   }
   xo[4] = lam;
   xo[5] = t;
   trig[0] = sph2; trig[1] = cph2; trig[2] = sth2; trig[3] = cth2;
-  double chk = xo[0] + xo[1] + xo[5];
+  R chk = xo[0] + xo[1] + xo[5];
 #pragma unroll
   for (int c = 0; c < 5; ++c) chk += J.Ja[0][c] + J.Ja[1][c] + J.Ja[2][c] + J.Ja[3][c] + J.Jt[c];
-  if (!(fabs(chk) < 1.0e300)) return ST_PROPAGATION;
+  if (!(fabs(chk) < big<R>())) return ST_PROPAGATION;
   return 0u;
 }
 
 // ---- C- = J C J^T with the structure of J (A.4) -----------------------------------------------------
-__device__ __forceinline__ void transport_covariance(const BoundJacobian& J, const double C[21],
-                                                     double Cp[21]) {
+template <typename R>
+__device__ __forceinline__ void transport_covariance(const BoundJacobianT<R>& J, const R C[21],
+                                                     R Cp[21]) {
   // M = J C : rows a = 0..3 and t; row qp of M is row qp of C
-  double Ma[4][6], Mt[6];
+  R Ma[4][6], Mt[6];
 #pragma unroll
   for (int i = 0; i < 4; ++i)
 #pragma unroll
     for (int k = 0; k < 6; ++k) {
-      double s = J.Ja[i][0] * C[SX(0, k)];
+      R s = J.Ja[i][0] * C[SX(0, k)];
 #pragma unroll
       for (int l = 1; l < 5; ++l) s = fma(J.Ja[i][l], C[SX(l, k)], s);
       Ma[i][k] = s;
     }
 #pragma unroll
   for (int k = 0; k < 6; ++k) {
-    double s = C[SX(5, k)];
+    R s = C[SX(5, k)];
 #pragma unroll
     for (int l = 0; l < 5; ++l) s = fma(J.Jt[l], C[SX(l, k)], s);
     Mt[k] = s;
@@ -617,26 +629,26 @@ __device__ __forceinline__ void transport_covariance(const BoundJacobian& J, con
   for (int i = 0; i < 4; ++i) {
 #pragma unroll
     for (int j = i; j < 4; ++j) {
-      double s = Ma[i][0] * J.Ja[j][0];
+      R s = Ma[i][0] * J.Ja[j][0];
 #pragma unroll
       for (int l = 1; l < 5; ++l) s = fma(Ma[i][l], J.Ja[j][l], s);
       Cp[IX(i, j)] = s;
     }
     Cp[IX(i, 4)] = Ma[i][4];
-    double s = Ma[i][5];
+    R s = Ma[i][5];
 #pragma unroll
     for (int l = 0; l < 5; ++l) s = fma(Ma[i][l], J.Jt[l], s);
     Cp[IX(i, 5)] = s;
   }
   Cp[IX(4, 4)] = C[IX(4, 4)];
   {
-    double s = C[IX(4, 5)];  // M[qp][t]
+    R s = C[IX(4, 5)];  // M[qp][t]
 #pragma unroll
     for (int l = 0; l < 5; ++l) s = fma(C[SX(4, l)], J.Jt[l], s);
     Cp[IX(4, 5)] = s;
   }
   {
-    double s = Mt[5];
+    R s = Mt[5];
 #pragma unroll
     for (int l = 0; l < 5; ++l) s = fma(Mt[l], J.Jt[l], s);
     Cp[IX(5, 5)] = s;
@@ -645,18 +657,20 @@ __device__ __forceinline__ void transport_covariance(const BoundJacobian& J, con
 
 // ---- gain-matrix update with a 2-D hit (A.5) ----------------------------------------
 // Split in two so that the outlier test (on chi2) comes before any state is written.
-struct Gain {
-  double r0, r1, i00, i01, i11;
+template <typename R>
+struct GainT {
+  R r0, r1, i00, i01, i11;
 };
 // Returns false when S = H C- H^T + V is not positive definite.
-__device__ __forceinline__ bool gain_prepare(const double xp[6], const double Cp[21], double m0, double m1,
-                                             double v00, double v01, double v11, Gain& G, double& chi2) {
+template <typename R>
+__device__ __forceinline__ bool gain_prepare(const R xp[6], const R Cp[21], R m0, R m1,
+                                             R v00, R v01, R v11, GainT<R>& G, R& chi2) {
   G.r0 = m0 - xp[0];
   G.r1 = m1 - xp[1];
-  const double S00 = Cp[IX(0, 0)] + v00, S01 = Cp[IX(0, 1)] + v01, S11 = Cp[IX(1, 1)] + v11;
-  const double det = fma(S00, S11, -S01 * S01);
-  if (!(S00 > 0.0 && det > 0.0)) return false;
-  const double idet = rcp_nr(det);
+  const R S00 = Cp[IX(0, 0)] + v00, S01 = Cp[IX(0, 1)] + v01, S11 = Cp[IX(1, 1)] + v11;
+  const R det = fma(S00, S11, -S01 * S01);
+  if (!(S00 > R(0.0) && det > R(0.0))) return false;
+  const R idet = rcp_nr(det);
   G.i00 = S11 * idet;
   G.i01 = -S01 * idet;
   G.i11 = S00 * idet;
@@ -664,12 +678,13 @@ __device__ __forceinline__ bool gain_prepare(const double xp[6], const double Cp
   return true;
 }
 // x+ = x- + K r, C+ = (I - K H) C-  with K = C- H^T S^-1.  xf/Cf must not alias xp/Cp.
-__device__ __forceinline__ void gain_apply(const Gain& G, const double xp[6], const double Cp[21],
-                                           double xf[6], double Cf[21]) {
-  double K0[6], K1[6];
+template <typename R>
+__device__ __forceinline__ void gain_apply(const GainT<R>& G, const R xp[6], const R Cp[21],
+                                           R xf[6], R Cf[21]) {
+  R K0[6], K1[6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
-    const double c0 = Cp[SX(i, 0)], c1 = Cp[SX(i, 1)];
+    const R c0 = Cp[SX(i, 0)], c1 = Cp[SX(i, 1)];
     K0[i] = fma(c0, G.i00, c1 * G.i01);
     K1[i] = fma(c0, G.i01, c1 * G.i11);
     xf[i] = fma(K1[i], G.r1, fma(K0[i], G.r0, xp[i]));
@@ -684,47 +699,50 @@ __device__ __forceinline__ void gain_apply(const Gain& G, const double xp[6], co
 // ---- material at a surface, after the update (A.6) -----------------------------------
 // Highland theta0^2 and Bethe mean loss from the filtered state.  trig = sin/cos of the filtered
 // (phi, theta).  Returns false when the energy is exhausted (E' <= m).
-struct MaterialStep {
-  double lam_out, g, theta0sq_over_sin2, theta0sq;
+template <typename R>
+struct MaterialStepT {
+  R lam_out, g, theta0sq_over_sin2, theta0sq;
 };
-__device__ __forceinline__ bool material_prepare(const MaterialDesc& Mt, const double* __restrict__ surf,
-                                                 const double trig[4], double lam, MaterialStep& S) {
-  const double sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
-  const double m = Mt.mass;
-  const double al = fabs(lam);
-  const double p = rcp_nr(al);
-  double iE;
-  const double E = sqrt_nr(fma(p, p, m * m), iE);
-  const double ib2 = (E * al) * (E * al);  // 1 / beta^2
-  const double bg = p * Mt.inv_mass, gamma = E * Mt.inv_mass;
-  const double nT = surf[9] * (cphi * sth) + surf[10] * (sphi * sth) + surf[11] * cth;
-  const double cfac = rcp_nr(fabs(nT));  // path factor 1/|n.T|
+template <typename R>
+__device__ __forceinline__ bool material_prepare(const MaterialDescT<R>& Mt, const R* __restrict__ surf,
+                                                 const R trig[4], R lam, MaterialStepT<R>& S) {
+  const R sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
+  const R m = Mt.mass;
+  const R al = fabs(lam);
+  const R p = rcp_nr(al);
+  R iE;
+  const R E = sqrt_nr(fma(p, p, m * m), iE);
+  const R ib2 = (E * al) * (E * al);  // 1 / beta^2
+  const R bg = p * Mt.inv_mass, gamma = E * Mt.inv_mass;
+  const R nT = surf[9] * (cphi * sth) + surf[10] * (sphi * sth) + surf[11] * cth;
+  const R cfac = rcp_nr(fabs(nT));  // path factor 1/|n.T|
   // Highland: theta0 = 0.0136/(beta p) sqrt(X) (1 + 0.038 ln(X/beta^2)),  1/(beta p) = E lam^2
-  const double X = surf[14] * cfac;
-  const double theta0 = 0.0136 * (E * al * al) * sqrt_nr(X) * fma(0.038, log_pos(X * ib2), 1.0);
+  const R X = surf[14] * cfac;
+  const R theta0 = R(0.0136) * (E * al * al) * sqrt_nr(X) * fma(R(0.038), log_pos(X * ib2), R(1.0));
   // Bethe, asymptotic density correction
-  const double me = kElectronMass;
-  const double Wmax = 2.0 * me * bg * bg * rcp_nr(1.0 + 2.0 * gamma * Mt.rme + Mt.rme * Mt.rme);
-  const double dhalf = fmax(0.0, Mt.log_hwp_I + log_pos(bg) - 0.5);
-  const double b2 = (p * iE) * (p * iE);
-  const double dedx =
-      kBetheK * Mt.ZA * ib2 * (0.5 * log_pos(2.0 * me * bg * bg * Wmax * Mt.inv_I2) - b2 - dhalf);
-  const double dE = dedx * Mt.rho * 1e-3 * 0.1 * surf[15] * cfac;
-  const double E2 = E - dE;
+  const R me = R(kElectronMass);
+  const R Wmax = R(2.0) * me * bg * bg * rcp_nr(R(1.0) + R(2.0) * gamma * Mt.rme + Mt.rme * Mt.rme);
+  const R dhalf = fmax(R(0.0), Mt.log_hwp_I + log_pos(bg) - R(0.5));
+  const R b2 = (p * iE) * (p * iE);
+  const R dedx =
+      R(kBetheK) * Mt.ZA * ib2 * (R(0.5) * log_pos(R(2.0) * me * bg * bg * Wmax * Mt.inv_I2) - b2 - dhalf);
+  const R dE = dedx * Mt.rho * R(1e-3) * R(0.1) * surf[15] * cfac;
+  const R E2 = E - dE;
   if (!(E2 > m)) return false;
-  double ip2;
-  const double p2 = sqrt_nr(fma(E2, E2, -m * m), ip2);
+  R ip2;
+  const R p2 = sqrt_nr(fma(E2, E2, -m * m), ip2);
   (void)p2;
-  const double pr = p * ip2;
+  const R pr = p * ip2;
   S.g = pr * pr * pr * E2 * iE;  // dlam'/dlam = p^3 E' / (p'^3 E)
-  S.lam_out = (lam < 0.0 ? -ip2 : ip2);
-  const double t2 = theta0 * theta0;
+  S.lam_out = (lam < R(0.0) ? -ip2 : ip2);
+  const R t2 = theta0 * theta0;
   S.theta0sq = t2;
   S.theta0sq_over_sin2 = t2 * rcp_nr(sth * sth);
   return true;
 }
 // C <- G C G^T + Q : row/column qp scaled by g, Highland terms on the angle variances
-__device__ __forceinline__ void material_apply(const MaterialStep& S, double C[21]) {
+template <typename R>
+__device__ __forceinline__ void material_apply(const MaterialStepT<R>& S, R C[21]) {
 #pragma unroll
   for (int i = 0; i < 6; ++i)
     if (i != 4) C[SX(i, 4)] *= S.g;
@@ -734,8 +752,9 @@ __device__ __forceinline__ void material_apply(const MaterialStep& S, double C[2
 }
 
 // exact inverse of material_apply up to round-off (failure paths only)
-__device__ __forceinline__ void material_undo(const MaterialStep& S, double C[21]) {
-  const double ig = 1.0 / S.g;
+template <typename R>
+__device__ __forceinline__ void material_undo(const MaterialStepT<R>& S, R C[21]) {
+  const R ig = R(1.0) / S.g;
   C[IX(2, 2)] -= S.theta0sq_over_sin2;
   C[IX(3, 3)] -= S.theta0sq;
 #pragma unroll
@@ -743,5 +762,13 @@ __device__ __forceinline__ void material_undo(const MaterialStep& S, double C[21
     if (i != 4) C[SX(i, 4)] *= ig;
   C[IX(4, 4)] *= ig * ig;
 }
+
+// the FP64 path's names (kf_lanes.cuh, kf_perigee.cuh, kf_mbf.cuh are double only)
+using FieldDesc = FieldDescT<double>;
+using MaterialDesc = MaterialDescT<double>;
+using MatJac = MatJacT<double>;
+using BoundJacobian = BoundJacobianT<double>;
+using Gain = GainT<double>;
+using MaterialStep = MaterialStepT<double>;
 
 }  // namespace kf

@@ -49,7 +49,7 @@ struct WorkspaceLayout {
   long long n_tiles;
 };
 
-WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth, int mbf = 0) {
+WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth, int mbf = 0, int mixed = 0) {
   WorkspaceLayout w{};
   w.n_tiles = N > 0 ? (N + KF_TILE - 1) / KF_TILE : 0;
   if (N <= 0 || n_legs_max <= 0) return w;
@@ -58,7 +58,7 @@ WorkspaceLayout workspace_layout(long long N, int n_legs_max, int smooth, int mb
     w.rec_off = off;
     // RTS: Lmax tile-legs of kLegBytes; Bryson-Frazier: Lmax tile-legs of kMbfLegBytes + the first-leg block
     w.tile_stride = mbf ? (size_t)n_legs_max * kf::kMbfLegBytes + (size_t)kf::kMbfFirstDoubles * KF_TILE * sizeof(double)
-                        : (size_t)n_legs_max * kf::kLegBytes;
+                        : (size_t)n_legs_max * (mixed ? kf::leg_bytes<float>() : kf::leg_bytes<double>());
     off += align_up((size_t)w.n_tiles * w.tile_stride, 256);
     w.nleg_off = off;
     off += align_up((size_t)w.n_tiles * KF_TILE * sizeof(int), 256);
@@ -159,6 +159,11 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
   if (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER &&
       ((op->output_states & KF_STATES_SMOOTH) || op->variant == KF_VARIANT_LANES_PER_TRACK))
     return KF_ERR_UNSUPPORTED;
+  if (op->precision != KF_PRECISION_FP64 && op->precision != KF_PRECISION_MIXED) return KF_ERR_ARG;
+  if (op->precision == KF_PRECISION_MIXED &&
+      (op->variant == KF_VARIANT_LANES_PER_TRACK || (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER) ||
+       ge->n_surfaces > 1024))
+    return KF_ERR_UNSUPPORTED;
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)
     return KF_ERR_ARG;
@@ -184,12 +189,14 @@ void kf_default_options(kf_options* opt) {
   opt->perigee_axis[2] = 1.0;
   opt->length_sort = KF_SORT_AUTO;
   opt->smoother = KF_SMOOTHER_RTS;
+  opt->precision = KF_PRECISION_FP64;
 }
 
 size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options* opt) {
   const int smooth = opt ? opt->smooth : 1;
   const int mbf = smooth && opt && opt->smoother == KF_SMOOTHER_BRYSON_FRAZIER;
-  return workspace_layout(n_tracks, n_legs_max, smooth, mbf).total;
+  const int mixed = opt && opt->precision == KF_PRECISION_MIXED;
+  return workspace_layout(n_tracks, n_legs_max, smooth, mbf, mixed).total;
 }
 
 int kf_last_launch_count(void) { return g_launches; }
@@ -223,7 +230,8 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   const long long N = tr->n_tracks;
   const int Lmax = ge->n_surfaces - 1 - tr->start_surface;
   const int mbf = op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER;
-  const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth, mbf);
+  const int mixed = op->precision == KF_PRECISION_MIXED;
+  const WorkspaceLayout w = workspace_layout(N, Lmax, op->smooth, mbf, mixed);
   if (w.rec_total > 0 && (!workspace || workspace_bytes < w.rec_total)) return KF_ERR_WORKSPACE;
   // the sort's arrays come after the records: a workspace sized by kf_workspace_bytes always holds them; a
   // shorter one (records only) runs unsorted under AUTO and is refused under ON
@@ -264,6 +272,20 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
     P.mat.inv_I2 = 1.0 / (P.mat.I_gev * P.mat.I_gev);
     P.mat.log_hwp_I = log(28.816e-9 * sqrt(ge->mat_rho * P.mat.ZA) / P.mat.I_gev);
   }
+  // the same two descriptors rounded to float (the MIXED path's kernels read these)
+  for (int a = 0; a < 3; ++a) {
+    P.field_f.b[a] = (float)P.field.b[a];
+    P.field_f.inv_spacing[a] = (float)P.field.inv_spacing[a];
+    P.field_f.n[a] = P.field.n[a];
+    P.field_f.origin[a] = (float)P.field.origin[a];
+    P.field_f.spacing[a] = (float)P.field.spacing[a];
+  }
+  P.field_f.b2 = P.field_f.b[0] * P.field_f.b[0] + P.field_f.b[1] * P.field_f.b[1] + P.field_f.b[2] * P.field_f.b[2];
+  P.field_f.grid = P.field.grid;
+  P.mat_f.mass = (float)P.mat.mass; P.mat_f.inv_mass = (float)P.mat.inv_mass; P.mat_f.rme = (float)P.mat.rme;
+  P.mat_f.inv_I2 = (float)P.mat.inv_I2; P.mat_f.ZA = (float)P.mat.ZA; P.mat_f.rho = (float)P.mat.rho;
+  P.mat_f.I_gev = (float)P.mat.I_gev; P.mat_f.log_hwp_I = (float)P.mat.log_hwp_I;
+  P.mixed = mixed;
   P.smooth = op->smooth ? 1 : 0;
   P.n_corr = op->n_corr_steps;
   P.output_states = op->output_states;
@@ -280,7 +302,7 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (w.rec_total > 0) {
     char* base = static_cast<char*>(workspace);
     P.rec = base + w.rec_off;
-    P.leg_stride = mbf ? kf::kMbfLegBytes : kf::kLegBytes;
+    P.leg_stride = mbf ? kf::kMbfLegBytes : (mixed ? kf::leg_bytes<float>() : kf::leg_bytes<double>());
     P.tile_stride = w.tile_stride;
     P.mbf = mbf;
     P.first_off = (size_t)Lmax * kf::kMbfLegBytes;
@@ -311,7 +333,7 @@ kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
   return P;
 }
 
-// Enqueue the forward filter and, if asked for, the RTS pass over the tracks of P on `stream`.
+// Enqueue the forward filter over the tracks of P on `stream`.
 template <int LPT, int BLOCK, bool MBF, bool PLAIN = false>
 int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geom_smem, cudaStream_t stream) {
   using kf::FIELD_CONST;
@@ -331,6 +353,22 @@ int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geo
     case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
     case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
     default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
+  }
+}
+
+// The MIXED-precision forward filter (kf_options.precision): float operands and records, one thread per track,
+// geometry in shared memory (validate() refuses tables too large to stage).
+template <int BLOCK, bool PLAIN>
+int launch_forward_mixed(const kf::FitParams& P, bool grid3, bool material, cudaStream_t stream) {
+  using kf::FIELD_CONST;
+  using kf::FIELD_GRID3;
+  const size_t smem = kf::geom_smem_bytes<float>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK);
+  const char* nm = "kf_forward_kernel (mixed precision)";
+  switch ((grid3 ? 2 : 0) | (material ? 1 : 0)) {
+    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
+    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
+    case 2: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
+    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
   }
 }
 
@@ -358,10 +396,11 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
     g_launches += 3;
     P.perm = sort.perm;
   }
-  const bool lanes = !P.mbf && (variant == KF_VARIANT_LANES_PER_TRACK ||
-                                (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS));
-  const size_t geom_smem = P.geom_in_smem ? (size_t)P.n_surfaces * 20 * sizeof(double) : 0;
-  const size_t rts_smem = 2 * kf::kLegBytes + 2 * sizeof(unsigned long long);  // two record stages + mbarriers
+  const bool lanes = !P.mbf && !P.mixed && (variant == KF_VARIANT_LANES_PER_TRACK ||
+                                            (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS));
+  const size_t geom_smem = P.geom_in_smem ? kf::geom_smem_bytes<double>(P.n_surfaces) : 0;
+  // two record stages + mbarriers
+  const size_t rts_smem = 2 * (P.mixed ? kf::leg_bytes<float>() : kf::leg_bytes<double>()) + 2 * sizeof(unsigned long long);
   int rc;
   record_stage(0, stream);
   // 256-thread forward CTAs once a constant-field batch is more than one wave of 128-thread CTAs at two per SM
@@ -370,7 +409,13 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   // the plain instantiation: default stepping, per-surface resolutions, no per-leg PRED/FILT states, no RKN estimate
   const bool plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
                      !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
-  if (lanes) rc = launch_forward<kf::kLanes, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
+  if (P.mixed) {
+    const bool bigm = P.N > KF_FWD_BIG_MIN_TRACKS;
+    if (plain) rc = bigm ? launch_forward_mixed<KF_FWD_BLOCK, true>(P, grid3, material, stream)
+                         : launch_forward_mixed<KF_FWD_BLOCK_SMALL, true>(P, grid3, material, stream);
+    else rc = bigm ? launch_forward_mixed<KF_FWD_BLOCK, false>(P, grid3, material, stream)
+                   : launch_forward_mixed<KF_FWD_BLOCK_SMALL, false>(P, grid3, material, stream);
+  } else if (lanes) rc = launch_forward<kf::kLanes, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
   else if (P.mbf && plain) rc = big ? launch_forward<1, KF_FWD_BLOCK, true, true>(P, grid3, material, geom_smem, stream)
                                     : launch_forward<1, KF_FWD_BLOCK_SMALL, true, true>(P, grid3, material, geom_smem, stream);
   else if (P.mbf) rc = big ? launch_forward<1, KF_FWD_BLOCK, true>(P, grid3, material, geom_smem, stream)
@@ -383,6 +428,10 @@ int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3,
   record_stage(1, stream);
   if (P.smooth && P.mbf) {
     rc = launch(kf::kf_mbf_kernel, P, KF_TILE, kf::kMbfSmem, stream, "kf_mbf_kernel");
+  } else if (P.smooth && P.mixed) {
+    rc = (!P.var && !(P.output_states & kf::OUT_SMOOTH))
+             ? launch(kf::kf_rts_kernel<true, float>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel (mixed precision)")
+             : launch(kf::kf_rts_kernel<false, float>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel (mixed precision)");
   } else if (P.smooth) {
     rc = lanes ? launch(kf::kf_rts_lanes_kernel, P, kf::kRtsLanesBlock, kf::kRtsLanesSmem, stream, "kf_rts_lanes_kernel",
                         kf::kLanes)
@@ -526,7 +575,8 @@ ArenaLayout arena_layout(long long N, long long M, int nS, int start, const kf_f
   a.perigee_params = b.take(6 * N * D);
   a.perigee_cov = b.take(21 * N * D);
   a.workspace_bytes = workspace_layout(N, Lmax, op ? op->smooth : 1,
-                                       op && op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER).total;
+                                       op && op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER,
+                                       op && op->precision == KF_PRECISION_MIXED).total;
   a.workspace = b.take(a.workspace_bytes);
   a.total = b.off;
   return a;

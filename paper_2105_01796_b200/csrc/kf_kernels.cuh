@@ -48,7 +48,10 @@ constexpr int kMbfFirstDoubles = 27;  // x-(6) C-(21) of leg 0
 #define KF_FWD_BLOCK_SMALL 128
 #endif
 static_assert(KF_FWD_BLOCK % KF_TILE == 0 && KF_FWD_BLOCK_SMALL % KF_TILE == 0 && KF_TILE % 32 == 0, "a forward CTA covers whole tiles; a tile covers whole warps");
-constexpr size_t kLegBytes = (size_t)kRecDoubles * KF_TILE * sizeof(double) + KF_TILE;  // record + flags
+// bytes of one tile-leg: kRecDoubles values of the path's arithmetic type per track + one flag byte per track
+template <typename R>
+__host__ __device__ constexpr size_t leg_bytes() { return (size_t)kRecDoubles * KF_TILE * sizeof(R) + KF_TILE; }
+constexpr size_t kLegBytes = leg_bytes<double>();  // the FP64 path's record + flags
 #ifndef KF_FWD_MIN_BLOCKS
 #define KF_FWD_MIN_BLOCKS 1
 #endif
@@ -83,6 +86,8 @@ struct FitParams {
   int geom_in_smem;
   FieldDesc field;
   MaterialDesc mat;
+  FieldDescT<float> field_f;   // the same two descriptors rounded to float: what the MIXED-precision kernels read
+  MaterialDescT<float> mat_f;
   // options
   int smooth, n_corr, output_states;
   double outlier_chi2, max_step, step_tol, inflation;
@@ -101,20 +106,26 @@ struct FitParams {
   size_t tile_stride;   // = Lmax * kLegBytes
   int* nleg;            // [slots] legs the forward pass completed, by SLOT
   int mbf;              // 1: Bryson-Frazier records (kMbf*), 0: RTS records (kRec*)
+  int mixed;            // 1: float operands and records (kf_options.precision MIXED), 0: double
   size_t first_off;     // mbf: byte offset of a tile's first-leg block [kMbfFirstDoubles][KF_TILE] from its base
   // length sort of ragged batches (kf_sort.cuh): slot -> track.  Records and nleg are indexed by slot (the
   // position in launch order), every caller-visible array by track.  nullptr: slot == track.
   const int* perm;
 };
 
-__device__ __forceinline__ void store6(double* base, long long stride, long long i, const double v[6]) {
+template <typename R>
+__device__ __forceinline__ void store6(double* base, long long stride, long long i, const R v[6]) {
 #pragma unroll
-  for (int k = 0; k < 6; ++k) base[k * stride + i] = v[k];
+  for (int k = 0; k < 6; ++k) base[k * stride + i] = (double)v[k];
 }
-__device__ __forceinline__ void store21(double* base, long long stride, long long i, const double v[21]) {
+template <typename R>
+__device__ __forceinline__ void store21(double* base, long long stride, long long i, const R v[21]) {
 #pragma unroll
-  for (int k = 0; k < 21; ++k) base[k * stride + i] = v[k];
+  for (int k = 0; k < 21; ++k) base[k * stride + i] = (double)v[k];
 }
+// the descriptors of the kernel's arithmetic type
+template <typename R> __device__ __forceinline__ const FieldDescT<R>& field_of(const struct FitParams& P);
+template <typename R> __device__ __forceinline__ const MaterialDescT<R>& material_of(const struct FitParams& P);
 
 __device__ __forceinline__ unsigned smem_u32(const void* p) {
   return static_cast<unsigned>(__cvta_generic_to_shared(p));
@@ -133,11 +144,23 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // bytes of the forward kernel's hit staging area: two alternating slots of (loc0, loc1, surface) per thread
 constexpr size_t hit_stage_bytes(int block) { return (size_t)block * (2 * 2 * sizeof(double) + 2 * sizeof(int)); }
 
-// stage the geometry table in shared memory once per CTA (5 KB for 31 planes)
-__device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem) {
+template <> __device__ __forceinline__ const FieldDescT<double>& field_of<double>(const FitParams& P) { return P.field; }
+template <> __device__ __forceinline__ const FieldDescT<float>& field_of<float>(const FitParams& P) { return P.field_f; }
+template <> __device__ __forceinline__ const MaterialDescT<double>& material_of<double>(const FitParams& P) { return P.mat; }
+template <> __device__ __forceinline__ const MaterialDescT<float>& material_of<float>(const FitParams& P) { return P.mat_f; }
+
+// stage the geometry table in shared memory once per CTA (5 KB for 31 planes; half that in float), converted to the
+// kernel's arithmetic type
+template <typename R>
+__device__ __forceinline__ void stage_geometry(const FitParams& P, R* smem) {
   const int n = P.n_surfaces * 20;
-  for (int k = threadIdx.x; k < n; k += blockDim.x) smem[k] = P.geom[k];
+  for (int k = threadIdx.x; k < n; k += blockDim.x) smem[k] = (R)P.geom[k];
   __syncthreads();
+}
+// bytes the staged table takes (a multiple of 16: the hit slots behind it hold doubles)
+template <typename R>
+__host__ __device__ constexpr size_t geom_smem_bytes(int n_surfaces) {
+  return ((size_t)n_surfaces * 20 * sizeof(R) + 15) / 16 * 16;
 }
 
 
@@ -158,23 +181,38 @@ __device__ __forceinline__ void stage_geometry(const FitParams& P, double* smem)
 // PLAIN: the call uses the default stepping policy (one primary + two correction steps, no step cap, no tolerance),
 // per-surface resolutions, and asks for no per-leg predicted/filtered states and no RKN error estimate: those paths are
 // compiled out (measured on CFG2: 3.39 -> 3.15 ms; the run-time tests cost registers in a kernel that has none to spare).
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN>
-__global__ void __launch_bounds__(BLOCK, KF_FWD_MIN_BLOCKS)
+// R: the arithmetic type of the path.  double = the FP64 path (BASELINE.json metric).  float = the MIXED path
+// (kf_options.precision; "All the tests use single precision ... with the exception of the
+// matrix inversion"): inputs are rounded to float on load, every operand and the RTS record are float, outputs are
+// widened on store.  Thread-per-track only (LPT = 1), RTS records only, geometry in shared memory only.
+// The constant-field float instantiation is held to 128 registers (512 threads per SM resident: twice the FP64 path's
+// warps; no spills); the grid-field one needs 244 and is left alone.
+#ifndef KF_FWD_F32_THREADS_PER_SM
+#define KF_FWD_F32_THREADS_PER_SM 512
+#endif
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN, typename R = double>
+__global__ void __launch_bounds__(BLOCK, (std::is_same<R, float>::value && FIELD == FIELD_CONST) ? KF_FWD_F32_THREADS_PER_SM / BLOCK
+                                                                                                : KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
+  static_assert(std::is_same<R, double>::value || (LPT == 1 && !MBF && GEOM_SMEM), "the MIXED path: thread per track, RTS records");
   const int o_n_corr = PLAIN ? 2 : P.n_corr;
-  const double o_max_step = PLAIN ? 0.0 : P.max_step, o_step_tol = PLAIN ? 0.0 : P.step_tol;
+  const R o_max_step = PLAIN ? R(0.0) : (R)P.max_step, o_step_tol = PLAIN ? R(0.0) : (R)P.step_tol;
   const double* const o_var = PLAIN ? nullptr : P.var;
   const int o_states = PLAIN ? 0 : P.output_states;
   double* const o_rk_err = PLAIN ? nullptr : P.rk_err_max;
+  const R o_outlier = (R)P.outlier_chi2;
+  const FieldDescT<R>& Fd = field_of<R>(P);
+  const MaterialDescT<R>& Md = material_of<R>(P);
   static_assert(BLOCK % KF_TILE == 0, "a forward CTA covers whole tiles");
-  extern __shared__ double s_dyn[];
-  const double* __restrict__ G;
+  extern __shared__ __align__(16) unsigned char s_fwd_raw[];
+  const R* __restrict__ G;
   if constexpr (GEOM_SMEM) {
-    stage_geometry(P, s_dyn);
-    G = s_dyn;
+    stage_geometry<R>(P, reinterpret_cast<R*>(s_fwd_raw));
+    G = reinterpret_cast<const R*>(s_fwd_raw);
   } else {
-    G = P.geom;
+    G = reinterpret_cast<const R*>(P.geom);  // (double only, see the static_assert)
   }
+  double* const s_dyn = reinterpret_cast<double*>(s_fwd_raw + (GEOM_SMEM ? geom_smem_bytes<R>(P.n_surfaces) : 0));  // hit slots
   const long long tslot = ((long long)blockIdx.x * BLOCK + threadIdx.x) / LPT;
   if (tslot >= P.N) return;    // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
   const long long i = P.perm ? (long long)P.perm[tslot] : tslot;  // the track this slot fits
@@ -189,11 +227,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   // backwards is a malformed hit list (the track is not fitted and none of its per-hit outputs is touched)
   const bool offsets_ok = o0 >= 0 && o0 <= o1 && (long long)o1 <= P.M;
   if (!offsets_ok) o0 = o1 = 0;
-  double x[6], C[21];
+  R x[6], C[21];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) x[k] = P.params[k * N + i];
+  for (int k = 0; k < 6; ++k) x[k] = (R)P.params[k * N + i];
 #pragma unroll
-  for (int k = 0; k < 21; ++k) C[k] = P.inflation * P.cov[k * N + i];
+  for (int k = 0; k < 21; ++k) C[k] = (R)P.inflation * (R)P.cov[k * N + i];
 
   unsigned status = 0u;
   // the hit list must be strictly ascending in surface index, inside (start, n_surfaces)
@@ -212,7 +250,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   }
   // the next unconsumed hit is fetched one leg ahead of its use into this thread's own shared-memory
   // slot (two alternating slots), asynchronously
-  double* const s_hm = s_dyn + (GEOM_SMEM ? P.n_surfaces * 20 : 0) + threadIdx.x;  // [slot][2][BLOCK]
+  double* const s_hm = s_dyn + threadIdx.x;  // [slot][2][BLOCK] (the hits as given: doubles)
   int* const s_hs = reinterpret_cast<int*>(s_hm - threadIdx.x + 4 * BLOCK) + threadIdx.x;  // [slot][BLOCK]
   int slot = 0;
   auto fetch_hit = [&](int j, int sl) {
@@ -223,36 +261,36 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   };
   if (o0 < o1) fetch_hit(o0, 0);
 
-  double chi2 = 0.0, errmax = 0.0;
+  R chi2 = R(0.0), errmax = R(0.0);
   int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0, hp = o0;
-  double trig[4];
-  sincos(x[2], &trig[0], &trig[1]);
-  sincos(x[3], &trig[2], &trig[3]);
+  R trig[4];
+  sincos_lib(x[2], trig[0], trig[1]);
+  sincos_lib(x[3], trig[2], trig[3]);
   // this tile's records: [leg][kRecDoubles][KF_TILE] doubles + [KF_TILE] flag bytes per leg
   const int lane_in_tile = LPT == 1 ? threadIdx.x % KF_TILE : (int)(tslot % KF_TILE);
   char* __restrict__ tile_base = P.rec + (size_t)(tslot / KF_TILE) * P.tile_stride;
-  char* __restrict__ tile_rec = tile_base + (size_t)lane_in_tile * sizeof(double);
+  char* __restrict__ tile_rec = tile_base + (size_t)lane_in_tile * sizeof(R);
   unsigned char* __restrict__ tile_flag =
-      reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(double) + lane_in_tile;
+      reinterpret_cast<unsigned char*>(tile_base) + (size_t)kRecDoubles * KF_TILE * sizeof(R) + lane_in_tile;
 
   for (int l = 0; l < n_target; ++l) {
     const int s = P.start + 1 + l;
-    const double* __restrict__ sf = G + (s - 1) * 20;
-    const double* __restrict__ st = G + s * 20;
+    const R* __restrict__ sf = G + (s - 1) * 20;
+    const R* __restrict__ st = G + s * 20;
     // material of the previous surface, from its filtered state (U6, U16).  C is advanced through
     // the layer only after the propagation succeeded, so that a failed leg leaves (x, C) = last_*.
-    double g_prev = 1.0;
-    const double lam_filtered = x[4];
-    MaterialStep ms;
-    const bool mat_here = MATERIAL && l > 0 && sf[14] > 0.0;
+    R g_prev = R(1.0);
+    const R lam_filtered = x[4];
+    MaterialStepT<R> ms;
+    const bool mat_here = MATERIAL && l > 0 && sf[14] > R(0.0);
     if (mat_here) {
-      if (!material_prepare(P.mat, sf, trig, x[4], ms)) { status |= ST_ENERGY; break; }
+      if (!material_prepare(Md, sf, trig, x[4], ms)) { status |= ST_ENERGY; break; }
       x[4] = ms.lam_out;
       g_prev = ms.g;
     }
-    double xp[6];
-    BoundJacobian J;
-    const unsigned rc = propagate<FIELD>(P.field, P.mat.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig,
+    R xp[6];
+    BoundJacobianT<R> J;
+    const unsigned rc = propagate<FIELD>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig,
                                          xp, J, errmax, status);
     if (rc) {
       status |= rc;
@@ -261,15 +299,15 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     }
     // RTS record ("stored Jacobians"): x-, F = J G_prev, g_prev go out right away so that the
     // stores drain under the covariance transport; C- and the hit follow it
-    double* __restrict__ R = reinterpret_cast<double*>(tile_rec + (size_t)l * P.leg_stride);
+    R* __restrict__ Rk = reinterpret_cast<R*>(tile_rec + (size_t)l * P.leg_stride);
     if (P.smooth && lead) {
       // the F block sits at kRecFa (RTS record) or kMbfFa (Bryson-Frazier record); Ft and g follow it in both
-      double* __restrict__ RF = R + (size_t)(MBF ? kMbfFa : kRecFa) * KF_TILE;
+      R* __restrict__ RF = Rk + (size_t)(MBF ? kMbfFa : kRecFa) * KF_TILE;
       if (!MBF) {
 #pragma unroll
-        for (int k = 0; k < 6; ++k) KF_REC_STORE(&R[(kRecXp + k) * KF_TILE], xp[k]);
+        for (int k = 0; k < 6; ++k) KF_REC_STORE(&Rk[(kRecXp + k) * KF_TILE], xp[k]);
       } else if (l == 0) {
-        double* __restrict__ FB = reinterpret_cast<double*>(tile_rec + P.first_off);
+        R* __restrict__ FB = reinterpret_cast<R*>(tile_rec + P.first_off);
 #pragma unroll
         for (int k = 0; k < 6; ++k) KF_REC_STORE(&FB[k * KF_TILE], xp[k]);
       }
@@ -285,28 +323,28 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       KF_REC_STORE(&RF[(kRecG - kRecFa) * KF_TILE], g_prev);
     }
     if (mat_here) material_apply(ms, C);
-    double Cp[21];
+    R Cp[21];
     if constexpr (LPT == 1) transport_covariance(J, C, Cp);
     else transport_covariance_lanes(J, C, Cp, q, gbase, gmask);
 
     // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
     cp_async_wait_all();
     const bool has_hit = hp < o1 && s_hs[slot * BLOCK] == s;
-    const double m0 = has_hit ? s_hm[(slot * 2 + 0) * BLOCK] : 0.0;
-    const double m1 = has_hit ? s_hm[(slot * 2 + 1) * BLOCK] : 0.0;
+    const R m0 = has_hit ? (R)s_hm[(slot * 2 + 0) * BLOCK] : R(0.0);
+    const R m1 = has_hit ? (R)s_hm[(slot * 2 + 1) * BLOCK] : R(0.0);
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth && lead) {
       if (!MBF) {
 #pragma unroll
-        for (int k = 0; k < 21; ++k) KF_REC_STORE(&R[(kRecCp + k) * KF_TILE], Cp[k]);
-        KF_REC_STORE(&R[kRecM * KF_TILE], m0);
-        KF_REC_STORE(&R[(kRecM + 1) * KF_TILE], m1);
+        for (int k = 0; k < 21; ++k) KF_REC_STORE(&Rk[(kRecCp + k) * KF_TILE], Cp[k]);
+        KF_REC_STORE(&Rk[kRecM * KF_TILE], m0);
+        KF_REC_STORE(&Rk[(kRecM + 1) * KF_TILE], m1);
       } else {
 #pragma unroll
-        for (int k = 0; k < 11; ++k) KF_REC_STORE(&R[(kMbfCcol + k) * KF_TILE], Cp[k]);  // (0,0..5), (1,1..5)
+        for (int k = 0; k < 11; ++k) KF_REC_STORE(&Rk[(kMbfCcol + k) * KF_TILE], Cp[k]);  // (0,0..5), (1,1..5)
         if (l == 0) {
-          double* __restrict__ FB = reinterpret_cast<double*>(tile_rec + P.first_off);
+          R* __restrict__ FB = reinterpret_cast<R*>(tile_rec + P.first_off);
 #pragma unroll
           for (int k = 0; k < 21; ++k) KF_REC_STORE(&FB[(6 + k) * KF_TILE], Cp[k]);
         }
@@ -316,35 +354,35 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     // gain-matrix update with the surface's hit.  A hole or a flagged outlier runs the
     // same arithmetic with a zero gain (x+ = x-, C+ = C- exactly), so the leg has one code path.
     unsigned char flag = 0;
-    Gain gn;
-    gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
+    GainT<R> gn;
+    gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = R(0.0);
     if (has_hit) {
-      double v00, v11, v01 = 0.0;
+      R v00, v11, v01 = R(0.0);
       if (o_var) {
-        v00 = o_var[hp];
-        v11 = o_var[P.ldm + hp];
-        if (P.cov01) v01 = P.cov01[hp];
+        v00 = (R)o_var[hp];
+        v11 = (R)o_var[P.ldm + hp];
+        if (P.cov01) v01 = (R)P.cov01[hp];
       } else {
         v00 = st[16];
         v11 = st[17];
       }
-      double c2 = 0.0;
+      R c2 = R(0.0);
       if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
         status |= ST_NOT_POSITIVE;
         if (mat_here) material_undo(ms, C);
         x[4] = lam_filtered;
         break;
       }
-      if (P.outlier_chi2 > 0.0 && c2 > P.outlier_chi2) {  // strictly greater: flagged, not used (U9)
+      if (o_outlier > R(0.0) && c2 > o_outlier) {  // strictly greater: flagged, not used (U9)
         n_outl++;
         flag = 2;
-        gn.i00 = gn.i01 = gn.i11 = 0.0;
+        gn.i00 = gn.i01 = gn.i11 = R(0.0);
       } else {
         chi2 += c2;
         n_used++;
         flag = 1;
       }
-      if (P.hit_chi2 && lead) P.hit_chi2[hp] = c2;
+      if (P.hit_chi2 && lead) P.hit_chi2[hp] = (double)c2;
       if (P.hit_flags && lead) P.hit_flags[hp] = flag;
       hp++;
       slot ^= 1;
@@ -352,11 +390,11 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       n_holes++;
     }
     if (P.smooth && MBF && lead) {  // the gain as applied: zero for a hole or a flagged outlier
-      KF_REC_STORE(&R[(kMbfGain + 0) * KF_TILE], gn.r0);
-      KF_REC_STORE(&R[(kMbfGain + 1) * KF_TILE], gn.r1);
-      KF_REC_STORE(&R[(kMbfGain + 2) * KF_TILE], gn.i00);
-      KF_REC_STORE(&R[(kMbfGain + 3) * KF_TILE], gn.i01);
-      KF_REC_STORE(&R[(kMbfGain + 4) * KF_TILE], gn.i11);
+      KF_REC_STORE(&Rk[(kMbfGain + 0) * KF_TILE], gn.r0);
+      KF_REC_STORE(&Rk[(kMbfGain + 1) * KF_TILE], gn.r1);
+      KF_REC_STORE(&Rk[(kMbfGain + 2) * KF_TILE], gn.i00);
+      KF_REC_STORE(&Rk[(kMbfGain + 3) * KF_TILE], gn.i01);
+      KF_REC_STORE(&Rk[(kMbfGain + 4) * KF_TILE], gn.i11);
     }
     gain_apply(gn, xp, Cp, x, C);
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
@@ -379,9 +417,9 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 
   // (x, C) = filtered state of the last completed leg, before that layer's material (start state if none)
   if (MATERIAL && nleg == n_target && nleg > 0) {  // the last surface's material: status bit only
-    const double* __restrict__ sl = G + (P.start + nleg) * 20;
-    MaterialStep ms;
-    if (sl[14] > 0.0 && !material_prepare(P.mat, sl, trig, x[4], ms)) status |= ST_ENERGY;
+    const R* __restrict__ sl = G + (P.start + nleg) * 20;
+    MaterialStepT<R> ms;
+    if (sl[14] > R(0.0) && !material_prepare(Md, sl, trig, x[4], ms)) status |= ST_ENERGY;
   }
   if (!lead) return;
   store6(P.last_params, N, i, x);
@@ -393,13 +431,13 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
 
   const int ndf = 2 * n_used - 5;
   if (ndf <= 0) status |= ST_NDF;
-  P.chi2[i] = chi2;
+  P.chi2[i] = (double)chi2;
   P.ndf[i] = ndf;
   P.status[i] = status;
   P.n_used[i] = n_used;
   P.n_outliers[i] = n_outl;
   P.n_holes[i] = n_holes;
-  if (o_rk_err) o_rk_err[i] = errmax;
+  if (o_rk_err) o_rk_err[i] = (double)errmax;
   if (P.smooth) P.nleg[tslot] = nleg;
   for (int j = hp; j < o1; ++j) {  // hits never reached
     if (P.hit_chi2) P.hit_chi2[j] = 0.0;
@@ -461,37 +499,41 @@ __device__ __forceinline__ void bulk_prefetch_l2(const void* gmem_src, unsigned 
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(gmem_src), "r"(bytes) : "memory");
 }
 
-constexpr int kStageDoubles = (int)(kLegBytes / sizeof(double));
-static_assert(kLegBytes % 16 == 0, "a tile-leg must be a whole number of 16-byte units (bulk copy)");
+// values of type R per record stage in shared memory (the flag bytes included, rounded up)
+template <typename R>
+__host__ __device__ constexpr int stage_values() { return (int)(leg_bytes<R>() / sizeof(R)); }
+constexpr int kStageDoubles = stage_values<double>();
+static_assert(leg_bytes<double>() % 16 == 0 && leg_bytes<float>() % 16 == 0,
+              "a tile-leg must be a whole number of 16-byte units (bulk copy)");
 // record column of one thread inside a stage: component c at R[c * KF_TILE]
 #define KF_R(R, c) (R)[(c) * KF_TILE]
 
 // filtered state of a leg from its record column R exactly as the forward pass computed it:
 // the same gain routine on (x-, C-, hit); a hole or flagged outlier has x+ = x-, C+ = C-.
-template <bool PLAIN>
-__device__ __forceinline__ void refilter(const FitParams& P, const double* R, unsigned char flag, double gv0,
-                                         double gv1, int hp, double xf[6], double Cf[21]) {
+template <bool PLAIN, typename R>
+__device__ __forceinline__ void refilter(const FitParams& P, const R* Rc, unsigned char flag, R gv0,
+                                         R gv1, int hp, R xf[6], R Cf[21]) {
   const double* const var = PLAIN ? nullptr : P.var;
-  double xp[6], Cp[21];
+  R xp[6], Cp[21];
 #pragma unroll
-  for (int k = 0; k < 6; ++k) xp[k] = KF_R(R, kRecXp + k);
+  for (int k = 0; k < 6; ++k) xp[k] = KF_R(Rc, kRecXp + k);
 #pragma unroll
-  for (int k = 0; k < 21; ++k) Cp[k] = KF_R(R, kRecCp + k);
-  Gain gn;
-  gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = 0.0;
+  for (int k = 0; k < 21; ++k) Cp[k] = KF_R(Rc, kRecCp + k);
+  GainT<R> gn;
+  gn.r0 = gn.r1 = gn.i00 = gn.i01 = gn.i11 = R(0.0);
   if (flag == 1) {
-    const double m0 = KF_R(R, kRecM), m1 = KF_R(R, kRecM + 1);
-    double v00, v11, v01 = 0.0;
+    const R m0 = KF_R(Rc, kRecM), m1 = KF_R(Rc, kRecM + 1);
+    R v00, v11, v01 = R(0.0);
     if (var) {
-      v00 = var[hp];
-      v11 = var[P.ldm + hp];
-      if (P.cov01) v01 = P.cov01[hp];
+      v00 = (R)var[hp];
+      v11 = (R)var[P.ldm + hp];
+      if (P.cov01) v01 = (R)P.cov01[hp];
     } else {
       v00 = gv0;  // the surface's resolution (geometry table), fetched by the caller
       v11 = gv1;
     }
-    double c2;
-    if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) gn.i00 = gn.i01 = gn.i11 = 0.0;
+    R c2;
+    if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) gn.i00 = gn.i01 = gn.i11 = R(0.0);
   }
   gain_apply(gn, xp, Cp, xf, Cf);
 }
@@ -505,13 +547,19 @@ __device__ __forceinline__ void refilter(const FitParams& P, const double* R, un
 // dx = x^s_{k+1} - x-_{k+1} (phi wrapped into (-pi, pi]), dC -> scratch, Cholesky C-_{k+1} = L L^T without
 // pivoting (scale-invariant), L[i][j] (i >= j) kept at packed (j, i), inv = 1 / diag.
 // Returns false on a non-positive pivot.
-__device__ __forceinline__ bool rts_step_pre(double* R1, const double xs[6], const double Cs[21], double dx[6],
+//
+// The 6x6 solve (Cholesky factor and the two triangular solves per row of the gain) always runs in double, whatever the
+// operand type R: the paper keeps its matrix inversion in double "because of the difference in implementation of the
+// floating-point arithmetic between different hardware".
+template <typename R>
+__device__ __forceinline__ bool rts_step_pre(R* R1, const R xs[6], const R Cs[21], R dx[6],
                                              double L[21], double inv[6]) {
   bool ok = true;
 #pragma unroll
   for (int c = 0; c < 21; ++c) {
-    L[c] = KF_R(R1, kRecCp + c);
-    KF_R(R1, kRecCp + c) = Cs[c] - L[c];
+    const R cp = KF_R(R1, kRecCp + c);
+    L[c] = (double)cp;
+    KF_R(R1, kRecCp + c) = Cs[c] - cp;
   }
   // (fixed trip counts with compile-time guards: every index is a constant after unrolling)
 #pragma unroll
@@ -541,33 +589,34 @@ __device__ __forceinline__ bool rts_step_pre(double* R1, const double xs[6], con
 
 // Part 2: W = C+ F^T, A = W (L L^T)^-1, x^s_k = x+_k + A dx, C^s_k = C+_k + A dC A^T.
 // Returns false on a non-finite result (C+ is then still in the scratch F slots).
-__device__ __forceinline__ bool rts_step_post(double* R1, const double xf[6], const double Cf[21],
-                                              const double dx[6], const double L[21], const double inv[6],
-                                              double xs[6], double Cs[21]) {
+template <typename R>
+__device__ __forceinline__ bool rts_step_post(R* R1, const R xf[6], const R Cf[21],
+                                              const R dx[6], const double L[21], const double inv[6],
+                                              R xs[6], R Cs[21]) {
   // W = C+ F^T, streaming F (rows loc0, loc1, phi, theta over columns loc0..qp; row t; row qp = g e_qp)
-  double W[6][6];
+  R W[6][6];
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    double f[5];
+    R f[5];
 #pragma unroll
     for (int c = 0; c < 5; ++c) f[c] = KF_R(R1, kRecFa + j * 5 + c);
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-      double s = Cf[SX(i, 0)] * f[0];
+      R s = Cf[SX(i, 0)] * f[0];
 #pragma unroll
       for (int c = 1; c < 5; ++c) s = fma(Cf[SX(i, c)], f[c], s);
       W[i][j] = s;
     }
   }
   {
-    double f[5];
+    R f[5];
 #pragma unroll
     for (int c = 0; c < 5; ++c) f[c] = KF_R(R1, kRecFt + c);
-    const double g = KF_R(R1, kRecG);
+    const R g = KF_R(R1, kRecG);
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
       W[i][4] = Cf[SX(i, 4)] * g;
-      double s = Cf[SX(i, 5)];
+      R s = Cf[SX(i, 5)];
 #pragma unroll
       for (int c = 0; c < 5; ++c) s = fma(Cf[SX(i, c)], f[c], s);
       W[i][5] = s;
@@ -577,65 +626,73 @@ __device__ __forceinline__ bool rts_step_post(double* R1, const double xf[6], co
 #pragma unroll
   for (int c = 0; c < 21; ++c) KF_R(R1, kRecFa + c) = Cf[c];
 
-  // A = W (L L^T)^-1 row by row in place, x^s_k = x+_k + A dx
-  double chk = 0.0;
+  // A = W (L L^T)^-1 row by row (the two triangular solves in double), x^s_k = x+_k + A dx
+  R chk = R(0.0);
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
+    double y[6];
 #pragma unroll
     for (int r = 0; r < 6; ++r) {  // L y = w
-      double s = W[i][r];
+      double s = (double)W[i][r];
 #pragma unroll
-      for (int k = 0; k < r; ++k) s = fma(-L[IX(k, r)], W[i][k], s);
-      W[i][r] = s * inv[r];
+      for (int k = 0; k < r; ++k) s = fma(-L[IX(k, r)], y[k], s);
+      y[r] = s * inv[r];
     }
 #pragma unroll
     for (int r = 5; r >= 0; --r) {  // L^T a = y
-      double s = W[i][r];
+      double s = y[r];
 #pragma unroll
-      for (int k = r + 1; k < 6; ++k) s = fma(-L[IX(r, k)], W[i][k], s);
-      W[i][r] = s * inv[r];
+      for (int k = r + 1; k < 6; ++k) s = fma(-L[IX(r, k)], y[k], s);
+      y[r] = s * inv[r];
     }
-    double s = xf[i];
+#pragma unroll
+    for (int r = 0; r < 6; ++r) W[i][r] = (R)y[r];
+    R s = xf[i];
 #pragma unroll
     for (int j = 0; j < 6; ++j) s = fma(W[i][j], dx[j], s);
     xs[i] = s;
     chk += s;
   }
   // C^s_k = C+_k + A dC A^T  (dC and C+ back from scratch)
-  double dC[21];
+  R dC[21];
 #pragma unroll
   for (int c = 0; c < 21; ++c) dC[c] = KF_R(R1, kRecCp + c);
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
-    double T[6];
+    R T[6];
 #pragma unroll
     for (int j = 0; j < 6; ++j) {
-      double u = W[i][0] * dC[SX(0, j)];
+      R u = W[i][0] * dC[SX(0, j)];
 #pragma unroll
       for (int k = 1; k < 6; ++k) u = fma(W[i][k], dC[SX(k, j)], u);
       T[j] = u;
     }
 #pragma unroll
     for (int j = i; j < 6; ++j) {
-      double u = KF_R(R1, kRecFa + IX(i, j));
+      R u = KF_R(R1, kRecFa + IX(i, j));
 #pragma unroll
       for (int k = 0; k < 6; ++k) u = fma(T[k], W[j][k], u);
       Cs[IX(i, j)] = u;
       chk += u;
     }
   }
-  return fabs(chk) < 1.0e300;
+  return fabs(chk) < big<R>();
 }
 
 // PLAIN: per-surface resolutions and no per-leg smoothed states asked for: those paths are compiled out (2.68 -> 2.61 ms
 // on CFG2; like the forward kernel this one has no register to spare for run-time options).
-template <bool PLAIN>
+// R: the arithmetic type of the records and of every product (double, or float for the MIXED path); the 6x6 solve is
+// double in both (rts_step_pre / rts_step_post).
+template <bool PLAIN, typename R = double>
 __global__ void __launch_bounds__(KF_TILE, KF_RTS_MIN_BLOCKS)
 kf_rts_kernel(const __grid_constant__ FitParams P) {
+  constexpr unsigned kLeg = (unsigned)leg_bytes<R>();
+  constexpr int kStage = stage_values<R>();
   const double* const o_var = PLAIN ? nullptr : P.var;
   const int o_states = PLAIN ? 0 : P.output_states;
-  extern __shared__ __align__(128) double s_rec[];  // two stages of kStageDoubles, then two mbarriers
-  unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_rec + 2 * kStageDoubles);
+  extern __shared__ __align__(128) unsigned char s_rts_raw[];  // two stages of kLeg bytes, then two mbarriers
+  R* const s_rec = reinterpret_cast<R*>(s_rts_raw);
+  unsigned long long* bar = reinterpret_cast<unsigned long long*>(s_rts_raw + 2 * (size_t)kLeg);
   __shared__ int s_nmax;
   const int tid = threadIdx.x;
   const long long tslot = (long long)blockIdx.x * KF_TILE + tid;
@@ -657,12 +714,12 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
 
   const char* __restrict__ tile_base = P.rec + (size_t)blockIdx.x * P.tile_stride;
   if (tid == 0) {
-    mbar_expect_tx(&bar[(n - 1) & 1], (unsigned)kLegBytes);
-    bulk_load(s_rec + ((n - 1) & 1) * kStageDoubles, tile_base + (size_t)(n - 1) * P.leg_stride, (unsigned)kLegBytes,
+    mbar_expect_tx(&bar[(n - 1) & 1], kLeg);
+    bulk_load(s_rec + ((n - 1) & 1) * kStage, tile_base + (size_t)(n - 1) * P.leg_stride, kLeg,
               &bar[(n - 1) & 1]);
     if (n >= 2) {
-      mbar_expect_tx(&bar[(n - 2) & 1], (unsigned)kLegBytes);
-      bulk_load(s_rec + ((n - 2) & 1) * kStageDoubles, tile_base + (size_t)(n - 2) * P.leg_stride, (unsigned)kLegBytes,
+      mbar_expect_tx(&bar[(n - 2) & 1], kLeg);
+      bulk_load(s_rec + ((n - 2) & 1) * kStage, tile_base + (size_t)(n - 2) * P.leg_stride, kLeg,
                 &bar[(n - 2) & 1]);
     }
   }
@@ -675,32 +732,33 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
     while (hp >= o0 && P.surf_idx[hp] > P.start + nleg) hp--;
   }
 
-  double xs[6], Cs[21];
+  R xs[6], Cs[21];
   bool failed = false;
   unsigned phase = 0u;
   for (int k = n - 1; k >= 0; --k) {
     const int sc = k & 1, sn = sc ^ 1;
     // record k-2 is fetched at the end of the next iteration: start it towards L2 now
-    if (tid == 0 && k >= 2) bulk_prefetch_l2(tile_base + (size_t)(k - 2) * P.leg_stride, (unsigned)kLegBytes);
+    if (tid == 0 && k >= 2) bulk_prefetch_l2(tile_base + (size_t)(k - 2) * P.leg_stride, kLeg);
     // the surface's measurement variances come from L2: ask for them before waiting on the record
-    double gv0 = 0.0, gv1 = 0.0;
+    R gv0 = R(0.0), gv1 = R(0.0);
     if (!o_var) {
-      gv0 = __ldg(P.geom + (P.start + 1 + k) * 20 + 16);
-      gv1 = __ldg(P.geom + (P.start + 1 + k) * 20 + 17);
+      gv0 = (R)__ldg(P.geom + (P.start + 1 + k) * 20 + 16);
+      gv1 = (R)__ldg(P.geom + (P.start + 1 + k) * 20 + 17);
     }
-    const double* Rc = s_rec + sc * kStageDoubles + tid;
-    double* Rn = s_rec + sn * kStageDoubles + tid;
+    const R* Rc = s_rec + sc * kStage + tid;
+    R* Rn = s_rec + sn * kStage + tid;
     // everything that needs record k+1 only comes before the wait for record k
     const bool step = k < nleg - 1 && !failed;
-    double dx[6], L[21], inv[6];
+    R dx[6];
+    double L[21], inv[6];
     bool ok = true;
     if (step) ok = rts_step_pre(Rn, xs, Cs, dx, L, inv);
     mbar_wait(&bar[sc], (phase >> sc) & 1u);
     phase ^= 1u << sc;
     if (k < nleg) {
       const unsigned char flag =
-          reinterpret_cast<const unsigned char*>(s_rec + sc * kStageDoubles)[(size_t)kRecDoubles * KF_TILE * sizeof(double) + tid];
-      double xf[6], Cf[21];
+          reinterpret_cast<const unsigned char*>(s_rec + sc * kStage)[(size_t)kRecDoubles * KF_TILE * sizeof(R) + tid];
+      R xf[6], Cf[21];
       refilter<PLAIN>(P, Rc, flag, gv0, gv1, hp, xf, Cf);
       if (flag != 0) hp--;
       bool smoothed = false;
@@ -731,8 +789,8 @@ kf_rts_kernel(const __grid_constant__ FitParams P) {
       asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
       __syncthreads();
       if (tid == 0 && k >= 1) {
-        mbar_expect_tx(&bar[sn], (unsigned)kLegBytes);
-        bulk_load(s_rec + sn * kStageDoubles, tile_base + (size_t)(k - 1) * P.leg_stride, (unsigned)kLegBytes, &bar[sn]);
+        mbar_expect_tx(&bar[sn], kLeg);
+        bulk_load(s_rec + sn * kStage, tile_base + (size_t)(k - 1) * P.leg_stride, kLeg, &bar[sn]);
       }
     }
   }

@@ -37,16 +37,16 @@ def test_struct_sizes_match_the_header_layout():
     assert C.sizeof(B.KfMeasurements) == 48
     assert C.sizeof(B.KfGeometry) == 48
     assert C.sizeof(B.KfField) == 4 + 4 + 24 + 12 + 4 + 24 + 24 + 8
-    assert C.sizeof(B.KfOptions) == 56 + 8 + 8 + 48
+    assert C.sizeof(B.KfOptions) == 56 + 8 + 8 + 48 + 8  # ... perigee line (48), precision (int32 + padding)
     assert C.sizeof(B.KfOutputs) == 10 * 8 + 6 * 8 + 3 * 8 + 2 * 8
     assert C.sizeof(B.KfPipeline) == 8 + 8 * 8 + 9 * 8 + 8
 
 
 def test_defaults_and_version():
     L = B.lib()
-    assert L.kf_version() == 105
+    assert L.kf_version() == 106
     o = B.default_options()
-    assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort) == (1, 0, 2, 0, 0, 0)
+    assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort, o.precision) == (1, 0, 2, 0, 0, 0, 0)
     assert o.outlier_chi2 == 0.0 and np.isinf(o.max_step_mm) and o.cov_inflation == 1.0
     assert o.mass_gev == pytest.approx(0.1056583755)
     assert L.kf_status_string(0) == b"ok"
@@ -68,6 +68,11 @@ def test_workspace_bytes():
     o.smooth = 0
     assert B.workspace_bytes(n, L, o) == sort(n)
     o.smooth = 1
+    # MIXED precision: float records (55 floats + 1 flag byte per leg and track)
+    o.precision = B.PRECISION_MIXED
+    tiles = (n + B.TILE - 1) // B.TILE
+    assert B.workspace_bytes(n, L, o) == up(tiles * L * (B.REC_DOUBLES * 4 + 1) * B.TILE) + up(tiles * B.TILE * 4) + sort(n)
+    o.precision = B.PRECISION_FP64
     assert B.workspace_bytes(0, L, o) == 0
     # 1e6 tracks x 30 legs fits comfortably in 180 GB
     assert B.workspace_bytes(1_000_000, 30, o) < 14e9
@@ -132,6 +137,16 @@ def test_argument_validation_rejects_before_any_launch():
     d = _dummy_call()
     d["op"].variant = 99
     assert _call(d) == -1
+    # precision: FP64 | MIXED; MIXED is thread-per-track + RTS only
+    d = _dummy_call()
+    d["op"].precision = 5
+    assert _call(d) == -1
+    for bad in (dict(variant=B.VARIANT_LANES_PER_TRACK), dict(smoother=B.SMOOTHER_BRYSON_FRAZIER)):
+        d = _dummy_call()
+        d["op"].precision = B.PRECISION_MIXED
+        for k, v in bad.items():
+            setattr(d["op"], k, v)
+        assert _call(d) == -2
     # null descriptor
     assert B.lib().kf_fit_batch(None, None, None, None, None, None, None, 0, None) == -1
     # zero tracks: accepted, nothing enqueued
