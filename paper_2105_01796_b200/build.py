@@ -16,17 +16,23 @@ _ROOT = os.path.dirname(_HERE)
 CSRC = os.path.join(_HERE, "csrc")
 INCLUDE = os.path.join(_ROOT, "include")
 LIB_PATH = os.path.join(_HERE, "libkf_fit.so")
-SOURCES = [os.path.join(CSRC, "kf_fit.cu")]
+OBJ_DIR = os.path.join(_HERE, "build")  # git-ignored
+
+
+def sources() -> list:
+    """The translation units of the library: csrc/*.cu (kf_fit.cu = C ABI + host logic; the others one kernel family each)."""
+    return sorted(glob.glob(os.path.join(CSRC, "*.cu")))
 
 
 def headers() -> list:
-    """Every header the translation unit can include: csrc/*.cuh and include/*.h (globbed, so a new file is watched)."""
-    return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(INCLUDE, "*.h")))
+    """Every header a translation unit can include: csrc/*.cuh, csrc/*.h and include/*.h (globbed, so a new file is watched)."""
+    return sorted(glob.glob(os.path.join(CSRC, "*.cuh")) + glob.glob(os.path.join(CSRC, "*.h")) +
+                  glob.glob(os.path.join(INCLUDE, "*.h")))
 
 
 NVCC_FLAGS = [
     "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
-    "-Xcompiler", "-fPIC", "-shared",
+    "-Xcompiler", "-fPIC",
     # IEEE double throughout: no fast-math; FMA contraction stays on (DESIGN.md "Tolerances")
     "--fmad=true",
 ]
@@ -43,22 +49,48 @@ def is_stale() -> bool:
     if not os.path.exists(LIB_PATH):
         return True
     t = os.path.getmtime(LIB_PATH)
-    return any(os.path.getmtime(p) > t for p in SOURCES + headers())
+    return any(os.path.getmtime(p) > t for p in sources() + headers())
+
+
+def _run(cmd):
+    res = subprocess.run(cmd, capture_output=True, text=True)
+    if res.returncode != 0:
+        raise RuntimeError("nvcc failed: " + " ".join(cmd) + "\n" + res.stdout + res.stderr)
+    return res.stderr
 
 
 def build_library(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
+    """Compile every csrc/*.cu to an object (side by side, one nvcc each) and link them into libkf_fit.so.
+    An object is rebuilt when its source or any header is newer (or `force`, or other flags than last time)."""
     if not force and not is_stale():
         return LIB_PATH
-    cmd = [nvcc_path(), *NVCC_FLAGS, *extra_flags, "-I", INCLUDE, "-I", CSRC, "-o", LIB_PATH, *SOURCES]
+    from concurrent.futures import ThreadPoolExecutor
+    os.makedirs(OBJ_DIR, exist_ok=True)
+    nvcc = nvcc_path()
+    flags = [*NVCC_FLAGS, *extra_flags, "-I", INCLUDE, "-I", CSRC]
     if verbose:
-        cmd.insert(1, "-Xptxas")
-        cmd.insert(2, "-v")
-        print(" ".join(cmd), file=sys.stderr)
-    res = subprocess.run(cmd, capture_output=True, text=True)
-    if res.returncode != 0:
-        raise RuntimeError("nvcc failed:\n" + res.stdout + res.stderr)
+        flags = ["-Xptxas", "-v", *flags]
+    stamp = os.path.join(OBJ_DIR, "flags.txt")
+    same_flags = os.path.exists(stamp) and open(stamp).read() == " ".join(flags)
+    newest_header = max(os.path.getmtime(p) for p in headers())
+    jobs, objs = [], []
+    for src in sources():
+        obj = os.path.join(OBJ_DIR, os.path.splitext(os.path.basename(src))[0] + ".o")
+        objs.append(obj)
+        fresh = (not force and same_flags and os.path.exists(obj) and
+                 os.path.getmtime(obj) > max(os.path.getmtime(src), newest_header))
+        if not fresh:
+            jobs.append([nvcc, *flags, "-c", "-o", obj, src])
     if verbose:
-        print(res.stderr, file=sys.stderr)
+        for j in jobs:
+            print(" ".join(j), file=sys.stderr)
+    with ThreadPoolExecutor(max_workers=max(1, min(len(jobs), os.cpu_count() or 1))) as pool:
+        for log in pool.map(_run, jobs):
+            if verbose:
+                print(log, file=sys.stderr)
+    with open(stamp, "w") as f:
+        f.write(" ".join(flags))
+    _run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB_PATH, *objs])
     return LIB_PATH
 
 

@@ -14,18 +14,49 @@
 #include <vector>
 
 #include "kf_fit.h"
-#include "kf_kernels.cuh"
-#include "kf_perigee.cuh"
-#include "kf_sort.cuh"
-#include "kf_mbf.cuh"
+#include "kf_host.h"
+
+namespace kfh {
+thread_local char g_cuda_error[256] = "";
+thread_local int g_launches = 0;
+
+bool set_cuda_error(cudaError_t e, const char* where) {
+  if (e == cudaSuccess) return false;
+  snprintf(g_cuda_error, sizeof(g_cuda_error), "%s: %s", where, cudaGetErrorString(e));
+  return true;
+}
+
+// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel): set it the first time a kernel
+// asks for more than 48 KB on a device (or for more than it asked before), not on every launch
+bool raise_smem_limit(const void* kernel, size_t smem, const char* name) {
+  struct Entry { const void* fn; int dev; size_t bytes; };
+  static std::mutex mu;
+  static std::vector<Entry> seen;
+  int dev = 0;
+  if (set_cuda_error(cudaGetDevice(&dev), name)) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  for (Entry& e : seen)
+    if (e.fn == kernel && e.dev == dev) {
+      if (e.bytes >= smem) return true;
+      if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
+      e.bytes = smem;
+      return true;
+    }
+  if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
+  seen.push_back(Entry{kernel, dev, smem});
+  return true;
+}
+}  // namespace kfh
 
 namespace {
+
+using kfh::g_cuda_error;
+using kfh::g_launches;
+using kfh::set_cuda_error;
 
 // batches of more tracks than this take the 256-thread forward CTA (148 SMs x 2 CTAs x 128 threads = one wave)
 constexpr long long KF_FWD_BIG_MIN_TRACKS = 148LL * 2 * 128;
 
-thread_local char g_cuda_error[256] = "";
-thread_local int g_launches = 0;
 thread_local cudaEvent_t g_stage_events[3] = {nullptr, nullptr, nullptr};
 thread_local bool g_stage_events_on = false;
 
@@ -78,45 +109,6 @@ struct SortPlan {
   int* bins;
   int force;  // KF_SORT_ON: sort even when the lengths hardly differ
 };
-
-bool set_cuda_error(cudaError_t e, const char* where) {
-  if (e == cudaSuccess) return false;
-  snprintf(g_cuda_error, sizeof(g_cuda_error), "%s: %s", where, cudaGetErrorString(e));
-  return true;
-}
-
-// cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel): set it the first time a kernel
-// asks for more than 48 KB on a device (or for more than it asked before), not on every launch
-bool raise_smem_limit(const void* kernel, size_t smem, const char* name) {
-  struct Entry { const void* fn; int dev; size_t bytes; };
-  static std::mutex mu;
-  static std::vector<Entry> seen;
-  int dev = 0;
-  if (set_cuda_error(cudaGetDevice(&dev), name)) return false;
-  std::lock_guard<std::mutex> lock(mu);
-  for (Entry& e : seen)
-    if (e.fn == kernel && e.dev == dev) {
-      if (e.bytes >= smem) return true;
-      if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
-      e.bytes = smem;
-      return true;
-    }
-  if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem), name)) return false;
-  seen.push_back(Entry{kernel, dev, smem});
-  return true;
-}
-
-template <typename K>
-int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_t stream, const char* name,
-           int lanes_per_track = 1) {
-  if (smem > 48 * 1024 && !raise_smem_limit(reinterpret_cast<const void*>(kernel), smem, name)) return KF_ERR_CUDA;
-  // thread per track: forward KF_FWD_BLOCK tracks per CTA, RTS one CTA per tile; lanes per track: block / lanes tracks per CTA
-  const unsigned grid = (unsigned)((P.N * lanes_per_track + block - 1) / block);
-  kernel<<<grid, block, smem, stream>>>(P);
-  if (set_cuda_error(cudaGetLastError(), name)) return KF_ERR_CUDA;
-  g_launches++;
-  return KF_OK;
-}
 
 int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
              const kf_options* op, const kf_outputs* out) {
@@ -333,120 +325,45 @@ kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
   return P;
 }
 
-// Enqueue the forward filter over the tracks of P on `stream`.
-template <int LPT, int BLOCK, bool MBF, bool PLAIN = false>
-int launch_forward(const kf::FitParams& P, bool grid3, bool material, size_t geom_smem, cudaStream_t stream) {
-  using kf::FIELD_CONST;
-  using kf::FIELD_GRID3;
-  size_t smem = geom_smem + kf::hit_stage_bytes(BLOCK);
-#ifdef KF_FWD_EXTRA_SMEM
-  smem += KF_FWD_EXTRA_SMEM;
-#endif
-  const int sel = (grid3 ? 4 : 0) | (material ? 2 : 0) | (P.geom_in_smem ? 1 : 0);
-  const char* nm = "kf_forward_kernel";
-  switch (sel) {
-    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
-    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
-    case 2: return launch(kf::kf_forward_kernel<FIELD_CONST, true, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
-    case 3: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
-    case 4: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
-    case 5: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
-    case 6: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, false, LPT, BLOCK, MBF, false>, P, BLOCK, smem, stream, nm, LPT);
-    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, LPT, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, LPT);
-  }
-}
-
-// The MIXED-precision forward filter (kf_options.precision): float operands and records, one thread per track,
-// geometry in shared memory (validate() refuses tables too large to stage).
-template <int BLOCK, bool PLAIN>
-int launch_forward_mixed(const kf::FitParams& P, bool grid3, bool material, cudaStream_t stream) {
-  using kf::FIELD_CONST;
-  using kf::FIELD_GRID3;
-  const size_t smem = kf::geom_smem_bytes<float>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK);
-  const char* nm = "kf_forward_kernel (mixed precision)";
-  switch ((grid3 ? 2 : 0) | (material ? 1 : 0)) {
-    case 0: return launch(kf::kf_forward_kernel<FIELD_CONST, false, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
-    case 1: return launch(kf::kf_forward_kernel<FIELD_CONST, true, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
-    case 2: return launch(kf::kf_forward_kernel<FIELD_GRID3, false, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
-    default: return launch(kf::kf_forward_kernel<FIELD_GRID3, true, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream, nm);
-  }
-}
-
 // variant: KF_VARIANT_*.  AUTO is the measured choice: 8 lanes
 // per track while the batch is so small that every warp of either variant has an SM sub-partition to itself
 // (<= KF_AUTO_LANES_MAX_TRACKS: 6-9 % shorter latency), one thread per track above (up to 6.5x the throughput).
 //
 // sort.perm != nullptr: first the length sort of the range (kf_sort.cuh: zero the bin counters, histogram, scan,
 // scatter), then both kernels go through the slot -> track permutation.
-int enqueue_fit(const kf::FitParams& P0, const kf::PerigeeParams& G, bool grid3, bool material, int variant,
+int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, bool material, int variant,
                 SortPlan sort, cudaStream_t stream) {
   kf::FitParams P = P0;
   P.perm = nullptr;
+  int rc;
   if (sort.perm) {
-    kf::SortParams S{};
-    S.N = P.N; S.M = P.M; S.offsets = P.offsets; S.surf_idx = P.surf_idx; S.start = P.start;
-    S.lmax = P.n_surfaces - 1 - P.start;
-    S.bins = sort.bins; S.perm = sort.perm; S.force = sort.force;
-    if (set_cuda_error(cudaMemsetAsync(sort.bins, 0, kf::kSortBins * sizeof(int), stream), "length sort")) return KF_ERR_CUDA;
-    const unsigned grid = (unsigned)((P.N + kf::kSortBlock - 1) / kf::kSortBlock);
-    kf::kf_sort_hist_kernel<<<grid, kf::kSortBlock, 0, stream>>>(S);
-    kf::kf_sort_scan_kernel<<<1, 32, 0, stream>>>(sort.bins, S.lmax, S.force);
-    kf::kf_sort_scatter_kernel<<<grid, kf::kSortBlock, 0, stream>>>(S);
-    if (set_cuda_error(cudaGetLastError(), "length sort")) return KF_ERR_CUDA;
-    g_launches += 3;
+    rc = kfh::launch_length_sort(P, sort.perm, sort.bins, sort.force, stream);
+    if (rc != KF_OK) return rc;
     P.perm = sort.perm;
   }
   const bool lanes = !P.mbf && !P.mixed && (variant == KF_VARIANT_LANES_PER_TRACK ||
                                             (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS));
-  const size_t geom_smem = P.geom_in_smem ? kf::geom_smem_bytes<double>(P.n_surfaces) : 0;
-  // two record stages + mbarriers
-  const size_t rts_smem = 2 * (P.mixed ? kf::leg_bytes<float>() : kf::leg_bytes<double>()) + 2 * sizeof(unsigned long long);
-  int rc;
   record_stage(0, stream);
-  // 256-thread forward CTAs once a constant-field batch is more than one wave of 128-thread CTAs at two per SM
-  // (CFG2 3.47 -> 3.40 ms; the grid-field kernel, at 255 registers with spills, is slower that way: CFG4 5.87 -> 6.11 ms)
-  const bool big = !grid3 && P.N > KF_FWD_BIG_MIN_TRACKS;
+  kfh::ForwardChoice fc{};
+  fc.grid3 = grid3;
+  fc.material = material;
+  // 256-thread forward CTAs once a batch is more than one wave of 128-thread CTAs at two per SM (CFG2 3.47 -> 3.40 ms;
+  // the FP64 grid-field kernel is slower that way, CFG4 5.87 -> 6.11 ms, and always takes the small CTA)
+  fc.big = P.N > KF_FWD_BIG_MIN_TRACKS;
   // the plain instantiation: default stepping, per-surface resolutions, no per-leg PRED/FILT states, no RKN estimate
-  const bool plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
-                     !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
-  if (P.mixed) {
-    const bool bigm = P.N > KF_FWD_BIG_MIN_TRACKS;
-    if (plain) rc = bigm ? launch_forward_mixed<KF_FWD_BLOCK, true>(P, grid3, material, stream)
-                         : launch_forward_mixed<KF_FWD_BLOCK_SMALL, true>(P, grid3, material, stream);
-    else rc = bigm ? launch_forward_mixed<KF_FWD_BLOCK, false>(P, grid3, material, stream)
-                   : launch_forward_mixed<KF_FWD_BLOCK_SMALL, false>(P, grid3, material, stream);
-  } else if (lanes) rc = launch_forward<kf::kLanes, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
-  else if (P.mbf && plain) rc = big ? launch_forward<1, KF_FWD_BLOCK, true, true>(P, grid3, material, geom_smem, stream)
-                                    : launch_forward<1, KF_FWD_BLOCK_SMALL, true, true>(P, grid3, material, geom_smem, stream);
-  else if (P.mbf) rc = big ? launch_forward<1, KF_FWD_BLOCK, true>(P, grid3, material, geom_smem, stream)
-                           : launch_forward<1, KF_FWD_BLOCK_SMALL, true>(P, grid3, material, geom_smem, stream);
-  else if (plain) rc = big ? launch_forward<1, KF_FWD_BLOCK, false, true>(P, grid3, material, geom_smem, stream)
-                           : launch_forward<1, KF_FWD_BLOCK_SMALL, false, true>(P, grid3, material, geom_smem, stream);
-  else rc = big ? launch_forward<1, KF_FWD_BLOCK, false>(P, grid3, material, geom_smem, stream)
-                : launch_forward<1, KF_FWD_BLOCK_SMALL, false>(P, grid3, material, geom_smem, stream);
+  fc.plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
+             !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
+  fc.mbf = P.mbf != 0;
+  if (P.mixed) rc = kfh::launch_forward_mixed(P, fc, stream);
+  else if (lanes) rc = kfh::launch_forward_lanes(P, fc, stream);
+  else if (grid3) rc = kfh::launch_forward_grid(P, fc, stream);
+  else rc = kfh::launch_forward_const(P, fc, stream);
   if (rc != KF_OK) return rc;
   record_stage(1, stream);
-  if (P.smooth && P.mbf) {
-    rc = launch(kf::kf_mbf_kernel, P, KF_TILE, kf::kMbfSmem, stream, "kf_mbf_kernel");
-  } else if (P.smooth && P.mixed) {
-    rc = (!P.var && !(P.output_states & kf::OUT_SMOOTH))
-             ? launch(kf::kf_rts_kernel<true, float>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel (mixed precision)")
-             : launch(kf::kf_rts_kernel<false, float>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel (mixed precision)");
-  } else if (P.smooth) {
-    rc = lanes ? launch(kf::kf_rts_lanes_kernel, P, kf::kRtsLanesBlock, kf::kRtsLanesSmem, stream, "kf_rts_lanes_kernel",
-                        kf::kLanes)
-               : (!P.var && !(P.output_states & kf::OUT_SMOOTH))
-                     ? launch(kf::kf_rts_kernel<true>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel")
-                     : launch(kf::kf_rts_kernel<false>, P, KF_TILE, rts_smem, stream, "kf_rts_kernel");
-  }
+  if (P.smooth) rc = kfh::launch_backward(P, lanes, stream);
   record_stage(2, stream);
-  if (rc == KF_OK && G.params) {  // fitted parameters on the perigee surface: one more (small) kernel
-    const unsigned grid = (unsigned)((P.N + kf::kPerigeeBlock - 1) / kf::kPerigeeBlock);
-    if (grid3) kf::kf_perigee_kernel<kf::FIELD_GRID3><<<grid, kf::kPerigeeBlock, 0, stream>>>(P, G);
-    else kf::kf_perigee_kernel<kf::FIELD_CONST><<<grid, kf::kPerigeeBlock, 0, stream>>>(P, G);
-    if (set_cuda_error(cudaGetLastError(), "kf_perigee_kernel")) return KF_ERR_CUDA;
-    g_launches++;
-  }
+  // fitted parameters on the perigee surface: one more (small) kernel
+  if (rc == KF_OK && G.params) rc = kfh::launch_perigee(P, G, grid3, stream);
   return rc;
 }
 
@@ -465,9 +382,9 @@ SortPlan sort_for_range(const SortPlan& whole, const kf_options* op, long long t
   return r;
 }
 
-kf::PerigeeParams perigee_params(const kf_options* op, const kf_outputs* out, long long t0) {
-  kf::PerigeeParams G{};
-  for (int a = 0; a < 3; ++a) { G.line.c[a] = op->perigee_center[a]; G.line.a[a] = op->perigee_axis[a]; }
+kfh::PerigeeLine perigee_params(const kf_options* op, const kf_outputs* out, long long t0) {
+  kfh::PerigeeLine G{};
+  for (int a = 0; a < 3; ++a) { G.c[a] = op->perigee_center[a]; G.a[a] = op->perigee_axis[a]; }
   G.params = out->perigee_params ? out->perigee_params + t0 : nullptr;
   G.cov = out->perigee_cov ? out->perigee_cov + t0 : nullptr;
   return G;
@@ -495,30 +412,7 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
 
 double kf_probe_fp64_tflops(int iters, void* cuda_stream) {
   if (iters <= 0) return (double)KF_ERR_ARG;
-  cudaStream_t stream = static_cast<cudaStream_t>(cuda_stream);
-  int dev = 0, sms = 0;
-  if (set_cuda_error(cudaGetDevice(&dev), "cudaGetDevice")) return (double)KF_ERR_CUDA;
-  if (set_cuda_error(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev), "cudaDeviceGetAttribute"))
-    return (double)KF_ERR_CUDA;
-  const int block = 256, grid = sms * 8;
-  cudaEvent_t e0, e1;
-  if (set_cuda_error(cudaEventCreate(&e0), "cudaEventCreate")) return (double)KF_ERR_CUDA;
-  if (set_cuda_error(cudaEventCreate(&e1), "cudaEventCreate")) { cudaEventDestroy(e0); return (double)KF_ERR_CUDA; }
-  double best = 0.0;
-  for (int rep = 0; rep < 4; ++rep) {  // first repetition is the warm-up
-    cudaEventRecord(e0, stream);
-    kf::kf_dfma_probe_kernel<<<grid, block, 0, stream>>>(nullptr, iters, 1.0000001, 1e-9);
-    cudaEventRecord(e1, stream);
-    if (set_cuda_error(cudaEventSynchronize(e1), "kf_dfma_probe_kernel")) { best = (double)KF_ERR_CUDA; break; }
-    float ms = 0.f;
-    cudaEventElapsedTime(&ms, e0, e1);
-    const double flops = 2.0 * 8.0 * (double)iters * (double)block * (double)grid;
-    const double tf = flops / ((double)ms * 1e-3) * 1e-12;
-    if (rep > 0 && tf > best) best = tf;
-  }
-  cudaEventDestroy(e0);
-  cudaEventDestroy(e1);
-  return best;
+  return kfh::probe_fp64_tflops(iters, static_cast<cudaStream_t>(cuda_stream));
 }
 
 

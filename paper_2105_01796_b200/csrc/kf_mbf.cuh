@@ -16,11 +16,10 @@
 // in kf_rts_kernel.
 #pragma once
 
-#include "kf_kernels.cuh"
+#include "kf_rts.cuh"
 
 namespace kf {
 
-constexpr size_t kMbfLegBytes = (size_t)kMbfDoubles * KF_TILE * sizeof(double);
 constexpr double kMbfKappaMax = 1.0e6;  // ~30 eps kappa against the 1e-8 covariance bar
 constexpr int kMbfStages = 2;  // 43 KB per CTA: five CTAs (ten warps) per SM
 constexpr size_t kMbfSmem = kMbfStages * kMbfLegBytes + kMbfStages * sizeof(unsigned long long);

@@ -13,7 +13,7 @@
 // 27 out: this kernel is a footnote to the fit's cost (0.1 ms per 1e6 tracks against 6 ms).
 #pragma once
 
-#include "kf_kernels.cuh"
+#include "kf_common.cuh"
 
 namespace kf {
 

@@ -12,11 +12,10 @@
 // (PAPER.md:119), so the results do not depend on the slot a track runs in (tested bit for bit).
 #pragma once
 
-#include "kf_kernels.cuh"
+#include "kf_common.cuh"
 
 namespace kf {
 
-constexpr int kSortBins = 64;    // lengths are quantised into at most this many bins
 constexpr int kSortBlock = 256;
 
 struct SortParams {
