@@ -82,6 +82,9 @@ def parse_args():
     ap.add_argument("--precision", default="fp64", choices=["fp64", "mixed"],
                     help="arithmetic (kf_options.precision): fp64 = the BASELINE.json metric (default); mixed = the paper's "
                          "operating point, float operands and records with the 6x6 solve in double (PAPER.md:160-164, 272)")
+    ap.add_argument("--field-stage", action="store_true",
+                    help="grid field: pass the shared-memory staging hint (kf_field.stage_*, kf_field_stage_box): the acceptance "
+                         "box of the table is kept in shared memory instead of being read through L1/L2 (measured slower on cfg4)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -240,7 +243,8 @@ def main():
     # minimal outputs: first/last state, chi2, ndf, status, counters, per-hit chi2 and flags (no RKN error diagnostic)
     out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
     mixed = args.precision == "mixed"
-    call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf), precision=int(mixed))
+    call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf), precision=int(mixed),
+                      field_stage=args.field_stage)
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -315,14 +319,15 @@ def main():
             barrier()
             return replicas.max_over_ranks(h0.elapsed_time(h1), dist, dev) / ke, ke
         # the public host-buffer call: chunks of 65,536 tracks over 3 streams (H2D, fit and D2H of different chunks overlap)
-        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf), precision=int(mixed))
+        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf), precision=int(mixed),
+                         field_stage=args.field_stage)
         ms_e2e, ke = time_host(hc)
         e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
                    d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke, launches_per_step=int(hc.launches),
                    api="kf_fit_batch_host_pipelined (pinned host buffers; chunks of 65536 tracks on 3 streams: "
                        "H2D, forward, RTS, D2H per chunk)")
         del hc
-        hc = kf.HostCall(hb, dev, smoother=int(bf), precision=int(mixed))  # context: the same through kf_fit_batch_host, everything in order on one stream
+        hc = kf.HostCall(hb, dev, smoother=int(bf), precision=int(mixed), field_stage=args.field_stage)  # context: the same through kf_fit_batch_host, everything in order on one stream
         ms_one, _ = time_host(hc)
         e2e["single_stream_ms_per_step"] = ms_one
         del hc
@@ -417,7 +422,7 @@ def main():
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
                     parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant, smoother=args.smoother,
-                    precision=args.precision,
+                    precision=args.precision, field_stage=(fkind == "grid3" and args.field_stage),
                     extra_untimed_warmup_steps=extra_warmup,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,

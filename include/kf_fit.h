@@ -56,7 +56,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 106          /* major * 100 + minor */
+#define KF_VERSION 107          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -182,7 +182,22 @@ typedef struct kf_field {
   double spacing[3];   /* GRID3: mm, > 0 */
   const double* grid;  /* GRID3: double[nz][ny][nx][3] tesla, x fastest, component innermost.
                           Trilinear interpolation; outside the grid the clamped value is used. */
+  /* GRID3, optional hint (all zero = none): the box of nodes [stage_lo[a], stage_lo[a] + stage_n[a]) per axis that
+   * covers where the tracks of the batch go (the detector acceptance).  When it is well-formed (inside the grid,
+   * stage_n[a] >= 2) and fits (KF_FIELD_STAGE_MAX_BYTES), the thread-per-track forward kernel keeps that part of
+   * the table in shared memory ("position-specific field information ... stored and retrieved", PAPER.md:170;
+   * shared memory for the objects of a fit); a lookup outside the box reads the table in global
+   * memory.  Results do not depend on the hint (same values, same arithmetic).  kf_field_stage_box fills it. */
+  int32_t stage_lo[3];
+  int32_t stage_n[3];
 } kf_field;
+#define KF_FIELD_STAGE_MAX_BYTES (200 * 1024)
+
+/* Fill field->stage_lo / stage_n from a HOST copy of the geometry table: the smallest node box that contains every
+ * surface's rectangle (centre +- half lengths along u and v, record entries [12..13]) plus one cell of margin,
+ * clipped to the grid; the hint is cleared when the field is not GRID3, the table holds no half lengths, or the box
+ * would not fit in KF_FIELD_STAGE_MAX_BYTES of doubles.  Host-only arithmetic, no CUDA call.  Returns KF_OK / KF_ERR_ARG. */
+int kf_field_stage_box(const double* surfaces_host, int32_t n_surfaces, kf_field* field);
 
 /* (3) fit configuration -- PAPER.md:179 */
 typedef struct kf_options {

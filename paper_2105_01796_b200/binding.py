@@ -30,7 +30,7 @@ _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",
            "kf_fit_batch_host", "kf_fit_batch_host_pipelined", "kf_last_launch_count", "kf_set_stage_events", "kf_probe_fp64_tflops", "kf_status_string",
-           "kf_last_cuda_error", "kf_version")
+           "kf_last_cuda_error", "kf_version", "kf_field_stage_box")
 
 
 class KfTracksIn(C.Structure):
@@ -50,7 +50,8 @@ class KfGeometry(C.Structure):
 
 class KfField(C.Structure):
     _fields_ = [("kind", C.c_int32), ("b", C.c_double * 3), ("n", C.c_int32 * 3),
-                ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("grid", C.c_void_p)]
+                ("origin", C.c_double * 3), ("spacing", C.c_double * 3), ("grid", C.c_void_p),
+                ("stage_lo", C.c_int32 * 3), ("stage_n", C.c_int32 * 3)]
 
 
 class KfOptions(C.Structure):
@@ -96,6 +97,8 @@ def lib():
     L.kf_default_options.argtypes = [C.POINTER(KfOptions)]
     L.kf_workspace_bytes.restype = C.c_size_t
     L.kf_workspace_bytes.argtypes = [C.c_int64, C.c_int32, C.POINTER(KfOptions)]
+    L.kf_field_stage_box.restype = C.c_int
+    L.kf_field_stage_box.argtypes = [C.c_void_p, C.c_int32, C.POINTER(KfField)]
     L.kf_fit_batch.restype = C.c_int
     L.kf_fit_batch.argtypes = [C.POINTER(KfTracksIn), C.POINTER(KfMeasurements), C.POINTER(KfGeometry),
                                C.POINTER(KfField), C.POINTER(KfOptions), C.POINTER(KfOutputs),
@@ -226,7 +229,8 @@ class HostBatch:
             material=wl.material, options=wl.options)
 
 
-def _field_struct(hb: HostBatch, grid_ptr: int) -> KfField:
+def _field_struct(hb: HostBatch, grid_ptr: int, stage: bool = False) -> KfField:
+    """stage: let the library derive the shared-memory staging hint (kf_field.stage_*) from the host geometry table."""
     f = KfField()
     if hb.field_kind == "const":
         f.kind = 0
@@ -237,6 +241,11 @@ def _field_struct(hb: HostBatch, grid_ptr: int) -> KfField:
         f.origin[:] = [float(v) for v in hb.grid_origin]
         f.spacing[:] = [float(v) for v in hb.grid_spacing]
         f.grid = grid_ptr
+        if stage:
+            g = np.ascontiguousarray(hb.geometry, dtype=np.float64)
+            rc = lib().kf_field_stage_box(g.ctypes.data_as(C.c_void_p), int(hb.n_surfaces), C.byref(f))
+            if rc != 0:
+                raise KfError(rc)
     return f
 
 
@@ -368,8 +377,10 @@ class FitCall:
     This is what bench.py times; `fit_batch` below is the one-shot convenience."""
 
     def __init__(self, batch: DeviceBatch, out: Optional[DeviceOutputs] = None, workspace=None, perigee=None,
-                 **opt_over):
-        """perigee = (centre, unit axis): also return the fitted parameters on that line surface."""
+                 field_stage=False, **opt_over):
+        """perigee = (centre, unit axis): also return the fitted parameters on that line surface.
+        field_stage: pass the staging hint for a grid field (kf_field_stage_box): the acceptance box of the table is then
+        kept in shared memory.  Results do not depend on it; measured slower than the L1/L2 path on CFG4, so off."""
         hb = batch.host
         self.batch = batch
         if perigee is not None:
@@ -383,7 +394,7 @@ class FitCall:
         self.meas = KfMeasurements(hb.n_meas, _ptr(batch.offsets), _ptr(batch.surf_idx), _ptr(batch.loc),
                                    _ptr(batch.var) or None, _ptr(batch.cov01) or None)
         self.geom = _geom_struct(hb, _ptr(batch.geometry))
-        self.field = _field_struct(hb, _ptr(batch.grid))
+        self.field = _field_struct(hb, _ptr(batch.grid), stage=field_stage)
         self.outs = self.out.struct()
         self.launches = 0
 
@@ -427,7 +438,7 @@ class HostCall:
     enqueues.  h2d_bytes / d2h_bytes count the tensors the library copies per call."""
 
     def __init__(self, hb: HostBatch, device="cuda:0", per_hit=False, n_streams=0, chunk_tracks=0, perigee=None,
-                 **opt_over):
+                 field_stage=False, **opt_over):
         torch = _torch()
         self.hb, self.device = hb, torch.device(device)
         if perigee is not None:
@@ -472,7 +483,7 @@ class HostCall:
         self.meas = KfMeasurements(M, _ptr(self.h_offsets), _ptr(self.h_surf_idx), _ptr(self.h_loc),
                                    _ptr(self.h_var) or None, _ptr(self.h_cov01) or None)
         self.geom = _geom_struct(hb, _ptr(self.h_geometry))
-        self.field = _field_struct(hb, _ptr(self.h_grid))
+        self.field = _field_struct(hb, _ptr(self.h_grid), stage=field_stage)
         o = KfOutputs()
         for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status",
                      "n_used", "n_outliers", "n_holes", "hit_chi2", "hit_flags", "perigee_params", "perigee_cov"):

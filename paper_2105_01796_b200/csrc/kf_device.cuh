@@ -34,6 +34,10 @@ enum : unsigned {
 
 constexpr int FIELD_CONST = 0;
 constexpr int FIELD_GRID3 = 1;
+constexpr int FIELD_GRID3S = 2;  // GRID3 with a box of the table staged in shared memory (FieldDescT::box_*)
+
+// every kernel's dynamic shared memory starts here (all `extern __shared__` arrays of a kernel alias one base)
+extern __shared__ __align__(128) unsigned char kf_dyn_smem[];
 
 // packed upper-triangle index of a symmetric 6x6 (i <= j)
 __host__ __device__ constexpr int IX(int i, int j) { return i * 6 - (i * (i - 1)) / 2 + (j - i); }
@@ -49,6 +53,10 @@ struct FieldDescT {
   R origin[3];
   R spacing[3];
   const double* grid; // [nz][ny][nx][3] tesla (the table as given: double)
+  // GRID3S: nodes [box_lo, box_lo + box_n) per axis are held in shared memory as R[box_n[2]][box_n[1]][box_n[0]][3],
+  // box_off bytes behind the start of the kernel's dynamic shared memory; a lookup whose cell is not wholly inside
+  // reads the table in global memory
+  int box_lo[3], box_n[3], box_off;
 };
 
 template <typename R>
@@ -101,21 +109,43 @@ __device__ __forceinline__ void field_at(const FieldDescT<R>& F, const R r[3], R
       idx[a] = (int)fl;
       w[a] = ww;
     }
-    const int nx = F.n[0];
-    const size_t row = (size_t)nx * 3;
-    const size_t slab = row * (size_t)F.n[1];
-    const double* base = F.grid + (size_t)idx[2] * slab + (size_t)idx[1] * row + (size_t)idx[0] * 3;
     R acc[3] = {R(0.0), R(0.0), R(0.0)};
+    // the eight corners: four pairs of x-adjacent nodes (6 contiguous values each) at row / slab strides
+    auto corners = [&](auto base, int row, int slab, auto load6) {
 #pragma unroll
-    for (int dz = 0; dz < 2; ++dz)
+      for (int dz = 0; dz < 2; ++dz)
 #pragma unroll
-      for (int dy = 0; dy < 2; ++dy) {
-        const double* nd = base + dz * slab + dy * row;  // two x-adjacent nodes: 6 contiguous doubles
-        const R wyz = (dy ? w[1] : R(1.0) - w[1]) * (dz ? w[2] : R(1.0) - w[2]);
-        const R w0 = (R(1.0) - w[0]) * wyz, w1 = w[0] * wyz;
+        for (int dy = 0; dy < 2; ++dy) {
+          R nd[6];
+          load6(base + dz * slab + dy * row, nd);
+          const R wyz = (dy ? w[1] : R(1.0) - w[1]) * (dz ? w[2] : R(1.0) - w[2]);
+          const R w0 = (R(1.0) - w[0]) * wyz, w1 = w[0] * wyz;
 #pragma unroll
-        for (int c = 0; c < 3; ++c) acc[c] += w0 * R(__ldg(nd + c)) + w1 * R(__ldg(nd + 3 + c));
+          for (int c = 0; c < 3; ++c) acc[c] += w0 * nd[c] + w1 * nd[3 + c];
+        }
+    };
+    bool staged = false;
+    if constexpr (FIELD == FIELD_GRID3S) {
+      const int bi = idx[0] - F.box_lo[0], bj = idx[1] - F.box_lo[1], bk = idx[2] - F.box_lo[2];
+      staged = (unsigned)bi < (unsigned)(F.box_n[0] - 1) && (unsigned)bj < (unsigned)(F.box_n[1] - 1) &&
+               (unsigned)bk < (unsigned)(F.box_n[2] - 1);
+      if (staged) {
+        const int row = F.box_n[0] * 3, slab = row * F.box_n[1];
+        corners(reinterpret_cast<const R*>(kf_dyn_smem + F.box_off) + bk * slab + bj * row + bi * 3, row, slab,
+                [](const R* q, R nd[6]) {
+#pragma unroll
+                  for (int c = 0; c < 6; ++c) nd[c] = q[c];
+                });
       }
+    }
+    if (!staged) {
+      const int row = F.n[0] * 3, slab = row * F.n[1];
+      corners(F.grid + (size_t)idx[2] * slab + (size_t)idx[1] * row + (size_t)idx[0] * 3, row, slab,
+              [](const double* q, R nd[6]) {
+#pragma unroll
+                for (int c = 0; c < 6; ++c) nd[c] = R(__ldg(q + c));
+              });
+    }
 #pragma unroll
     for (int c = 0; c < 3; ++c) B[c] = acc[c] * R(kTeslaToGeVPerMm);
   }
@@ -363,6 +393,125 @@ struct MatJacT {
   R P[9], Q[9], p[3], q[3], sigma;
 };
 
+// ---- position-dependent field: the RKN4 step with the Jacobian carried as variational columns -------
+// In a grid field the step Jacobians do not commute, and accumulating them as 3x3 blocks (MatJacT: A, Bm per step,
+// then P += A Q, Q = Bm Q, then P Tphi, Q Tphi, ...) spends most of its arithmetic on matrix entries that only ever
+// act on three vectors.  Here the three non-trivial columns of D J_b2f themselves -- d(r, T)/d(phi), /d(theta),
+// /d(q/p) at the start of the leg -- are carried through the stages of every step (the variational equations of
+// the RKN4 scheme, the same discrete Jacobian as rkn4_step's blocks, regrouped):
+//   dk1 = lam dT x B1 (+ T x B1);  dT2 = dT + (h/2) dk1;  dk2 = lam dT2 x B2 (+ T2 x B2);  dT3 = dT + (h/2) dk2;
+//   dk3 = lam dT3 x B2 (+ T3 x B2);  dT4 = dT + h dk3;  dk4 = lam dT4 x B3 (+ T4 x B3)     [(+ ...): the q/p column]
+//   dr' = dr + h dT + (h^2/6)(dk1 + dk2 + dk3);   dT' = dT + (h/6)(dk1 + 2 dk2 + 2 dk3 + dk4).
+// The loc0 / loc1 columns stay (u, 0), (v, 0) while the field gradient is neglected (U4).
+// 19 numbers instead of 25, no 3x3 products, and the per-step blocks A, Bm never exist.
+template <typename R>
+struct ColJacT {
+  R dr[3][3], dT[3][3];  // [column: phi, theta, q/p][component]
+  R sigma;               // dt/dlam
+};
+
+// After a last step shorter than this, the field of that step's fourth stage (looked up at r + hT + (h^2/2) k3)
+// stands for the field at its end point r + hT + (h^2/6)(k1 + k2 + k3) in the path-length correction: the two points
+// are within h^2 |k| / 3 <= 1e-6 x 6e-3 / 3 = 2e-9 mm of each other (p >= 0.1 GeV in 2 T), which moves the Jacobian by
+// less than |k| |w.c| x |grad B|/|B| x 2e-9 <= 7e-3 x 0.2 x 2e-9 = 3e-12 relative for any grid of >= 10 mm spacing
+// (CFG4: 1e-14), far inside the 1e-8 covariance bar.  One lookup per leg saved.
+template <typename R> __device__ __forceinline__ constexpr R short_step() { return R(1.0e-3); }
+
+template <int FIELD, typename R>
+__device__ __forceinline__ void rkn4_step_cols(const FieldDescT<R>& F, R dtds, R tfac, R r[3], R& t, R T[3], R lam,
+                                               R h, ColJacT<R>& V, R Blast[3], R& eps, unsigned& status) {
+  const R hh = R(0.5) * h, h6 = h * (R(1.0) / R(6.0)), h26 = h * h6;
+  R B1[3], B2[3], B3[3];
+  // state and the q/p column together (the column's inhomogeneous terms are the stage vectors T_i x B_i)
+  R l1[3], l2[3], l3[3], l4[3], k1[3], k2[3], k3[3], k4[3], v[3];
+  R* const dTq = V.dT[2];
+  R* const drq = V.dr[2];
+  R q1[3], q2[3], q3[3], q4[3];
+  field_at<FIELD>(F, r, B1, status);
+  cross(T, B1, l1);
+  cross(dTq, B1, q1);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k1[i] = lam * l1[i]; q1[i] = fma(lam, q1[i], l1[i]); }
+  {
+    R rm[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) rm[i] = fma(R(0.125) * h * h, k1[i], fma(hh, T[i], r[i]));
+    field_at<FIELD>(F, rm, B2, status);
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k1[i], T[i]);
+  cross(v, B2, l2);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q1[i], dTq[i]);
+  cross(v, B2, q2);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k2[i] = lam * l2[i]; q2[i] = fma(lam, q2[i], l2[i]); }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k2[i], T[i]);
+  cross(v, B2, l3);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q2[i], dTq[i]);
+  cross(v, B2, q3);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k3[i] = lam * l3[i]; q3[i] = fma(lam, q3[i], l3[i]); }
+  {
+    R re[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) re[i] = fma(R(0.5) * h * h, k3[i], fma(h, T[i], r[i]));
+    field_at<FIELD>(F, re, B3, status);
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(h, k3[i], T[i]);
+  cross(v, B3, l4);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) v[i] = fma(h, q3[i], dTq[i]);
+  cross(v, B3, q4);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k4[i] = lam * l4[i]; q4[i] = fma(lam, q4[i], l4[i]); }
+  // the phi and theta columns: homogeneous, they need the three field values only
+#pragma unroll
+  for (int c = 0; c < 2; ++c) {
+    R* const dT = V.dT[c];
+    R* const dr = V.dr[c];
+    R d1[3], d2[3], d3[3], d4[3], w[3];
+    cross(dT, B1, d1);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { d1[i] *= lam; w[i] = fma(hh, d1[i], dT[i]); }
+    cross(w, B2, d2);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { d2[i] *= lam; w[i] = fma(hh, d2[i], dT[i]); }
+    cross(w, B2, d3);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { d3[i] *= lam; w[i] = fma(h, d3[i], dT[i]); }
+    cross(w, B3, d4);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      d4[i] *= lam;
+      dr[i] = fma(h26, d1[i] + d2[i] + d3[i], fma(h, dT[i], dr[i]));
+      dT[i] = fma(h6, (d1[i] + d4[i]) + R(2.0) * (d2[i] + d3[i]), dT[i]);
+    }
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    drq[i] = fma(h26, q1[i] + q2[i] + q3[i], fma(h, dTq[i], drq[i]));
+    dTq[i] = fma(h6, (q1[i] + q4[i]) + R(2.0) * (q2[i] + q3[i]), dTq[i]);
+  }
+  V.sigma = fma(h, tfac, V.sigma);
+  eps = h * h * (fabs(k1[0] - k2[0] - k3[0] + k4[0]) + fabs(k1[1] - k2[1] - k3[1] + k4[1]) +
+                 fabs(k1[2] - k2[2] - k3[2] + k4[2]));
+  // state
+  R Tn[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r[i] = fma(h26, k1[i] + k2[i] + k3[i], fma(h, T[i], r[i]));
+    Tn[i] = fma(h6, (k1[i] + k4[i]) + R(2.0) * (k2[i] + k3[i]), T[i]);
+  }
+  const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { T[i] = Tn[i] * inrm; Blast[i] = B3[i]; }
+  t = fma(h, dtds, t);
+}
+
 // The bound-to-bound Jacobian, non-trivial part: Ja rows (loc0, loc1, phi, theta) x columns
 // (loc0, loc1, phi, theta, qp); Jt = row t over the same columns.  Row qp = e_qp, column t = e_t.
 template <typename R>
@@ -434,7 +583,18 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
     }
   }
   const int n_steps = n_sub + n_corr;
-  typename std::conditional<FIELD == FIELD_CONST, PolyJacT<R>, MatJacT<R>>::type D;
+  typename std::conditional<FIELD == FIELD_CONST, PolyJacT<R>, ColJacT<R>>::type D;
+  R Bend[3];             // grid field: the field of the last step's fourth stage, used when that step was a short one
+  bool have_Bend = false;
+  if constexpr (FIELD != FIELD_CONST) {
+    // columns of J_b2f: d(r, T)/d(phi) = (0, Tphi), /d(theta) = (0, Tth), /d(q/p) = (0, 0)
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      D.dr[0][i] = D.dr[1][i] = D.dr[2][i] = R(0.0);
+      D.dT[0][i] = Tphi[i]; D.dT[1][i] = Tth[i]; D.dT[2][i] = R(0.0);
+    }
+    D.sigma = R(0.0);
+  }
   bool fast = false;
   if constexpr (FIELD == FIELD_CONST) {
     // default policy (one primary + two correction steps) in a constant field: the three steps as one
@@ -469,28 +629,10 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
       if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
       else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
     } else {
-      R A[9], a[3], Bm[9], b[3], tau, eps;
-      rkn4_step<FIELD>(F, dtds, tfac, r, t, T, lam, h, A, a, Bm, b, tau, eps, status);
+      R eps;
+      have_Bend = fabs(h) <= short_step<R>();  // (of the last step, when the loop ends)
+      rkn4_step_cols<FIELD>(F, dtds, tfac, r, t, T, lam, h, D, Bend, eps, status);
       errmax = fmax(errmax, eps);
-      if (is == 0) {
-#pragma unroll
-        for (int i = 0; i < 9; ++i) { D.P[i] = A[i]; D.Q[i] = Bm[i]; }
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { D.p[i] = a[i]; D.q[i] = b[i]; }
-        D.sigma = tau;
-      } else {
-        // D <- Dstep D:  P += A Q,  p += A q + a,  Q = Bm Q,  q = Bm q + b,  sigma += tau
-        R AQ[9], Aq[3], BQ[9], Bq[3];
-        mat3_mul(A, D.Q, AQ);
-        mat3_vec(A, D.q, Aq);
-        mat3_mul(Bm, D.Q, BQ);
-        mat3_vec(Bm, D.q, Bq);
-#pragma unroll
-        for (int i = 0; i < 9; ++i) { D.P[i] += AQ[i]; D.Q[i] = BQ[i]; }
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { D.p[i] += Aq[i] + a[i]; D.q[i] = Bq[i] + b[i]; }
-        D.sigma += tau;
-      }
     }
     const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
     if (!(fabs(fin) < big<R>())) return ST_PROPAGATION;  // catches NaN and Inf
@@ -499,9 +641,14 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   // A.3 free -> bound with the path-length correction  D~ = (I - f' w^T) D
   nT = dot(nt, T);
   if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
-  R Bend[3], TxB[3];
-  field_at<FIELD>(F, r, Bend, status);
-  cross(T, Bend, TxB);
+  R TxB[3];
+  if constexpr (FIELD == FIELD_CONST) {
+    cross(T, F.b, TxB);
+  } else {
+    // after a short last step (|h| <= short_step) the field of that step's last lookup stands for the field at the end point
+    if (!have_Bend) field_at<FIELD>(F, r, Bend, status);
+    cross(T, Bend, TxB);
+  }
   const R kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};  // dT/ds
   const R inT = rcp_nr(nT);
   const R w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
@@ -554,20 +701,11 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
       project(3, cr, R(0.0), cT);
     }
   } else {
-    {
-      R cr[3], cT[3];
-      mat3_vec(D.P, Tphi, cr);
-      mat3_vec(D.Q, Tphi, cT);
-      project(2, cr, R(0.0), cT);
-    }
-    {
-      R cr[3], cT[3];
-      mat3_vec(D.P, Tth, cr);
-      mat3_vec(D.Q, Tth, cT);
-      project(3, cr, R(0.0), cT);
-    }
+    project(2, D.dr[0], R(0.0), D.dT[0]);
+    project(3, D.dr[1], R(0.0), D.dT[1]);
+    project(4, D.dr[2], D.sigma, D.dT[2]);
   }
-  {
+  if constexpr (FIELD == FIELD_CONST) {
     R cr[3] = {D.p[0], D.p[1], D.p[2]}, cT[3] = {D.q[0], D.q[1], D.q[2]};
     project(4, cr, D.sigma, cT);
   }

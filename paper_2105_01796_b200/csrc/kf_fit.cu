@@ -253,6 +253,12 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
       P.field.inv_spacing[a] = 1.0 / fl->spacing[a];
     }
     P.field.grid = fl->grid;
+    // the staging hint, when well-formed (else ignored: results do not depend on it)
+    bool ok = true;
+    for (int a = 0; a < 3; ++a)
+      ok = ok && fl->stage_lo[a] >= 0 && fl->stage_n[a] >= 2 && fl->stage_lo[a] + fl->stage_n[a] <= fl->n[a];
+    if (ok && (size_t)fl->stage_n[0] * fl->stage_n[1] * fl->stage_n[2] * 3 * sizeof(double) <= KF_FIELD_STAGE_MAX_BYTES)
+      for (int a = 0; a < 3; ++a) { P.field.box_lo[a] = fl->stage_lo[a]; P.field.box_n[a] = fl->stage_n[a]; }
   }
   P.mat.mass = op->mass_gev;
   P.mat.inv_mass = 1.0 / op->mass_gev;
@@ -271,6 +277,8 @@ int build_params(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
     P.field_f.n[a] = P.field.n[a];
     P.field_f.origin[a] = (float)P.field.origin[a];
     P.field_f.spacing[a] = (float)P.field.spacing[a];
+    P.field_f.box_lo[a] = P.field.box_lo[a];
+    P.field_f.box_n[a] = P.field.box_n[a];
   }
   P.field_f.b2 = P.field_f.b[0] * P.field_f.b[0] + P.field_f.b[1] * P.field_f.b[1] + P.field_f.b[2] * P.field_f.b[2];
   P.field_f.grid = P.field.grid;
@@ -354,7 +362,20 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
   fc.plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
              !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
   fc.mbf = P.mbf != 0;
-  if (P.mixed) rc = kfh::launch_forward_mixed(P, fc, stream);
+  // grid field with the caller's box of the table in shared memory (kf_field.stage_*): thread per track, RTS records,
+  // when [geometry][hit slots][box] fit the CTA's shared memory
+  if (grid3 && !lanes && !P.mbf && P.geom_in_smem && P.field.box_n[0] >= 2) {
+    const size_t elem = P.mixed ? sizeof(float) : sizeof(double);
+    const size_t box = ((size_t)P.field.box_n[0] * P.field.box_n[1] * P.field.box_n[2] * 3 * elem + 15) / 16 * 16;
+    const size_t off = (P.mixed ? kf::geom_smem_bytes<float>(P.n_surfaces) : kf::geom_smem_bytes<double>(P.n_surfaces)) +
+                       kf::hit_stage_bytes(kfh::staged_block(box));
+    if (off + box <= 226 * 1024) {
+      fc.staged = true;
+      P.field.box_off = P.field_f.box_off = (int)off;
+    }
+  }
+  if (fc.staged) rc = kfh::launch_forward_staged(P, fc, stream);
+  else if (P.mixed) rc = kfh::launch_forward_mixed(P, fc, stream);
   else if (lanes) rc = kfh::launch_forward_lanes(P, fc, stream);
   else if (grid3) rc = kfh::launch_forward_grid(P, fc, stream);
   else rc = kfh::launch_forward_const(P, fc, stream);
@@ -408,6 +429,38 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   const int lmax = ge->n_surfaces - 1 - tr->start_surface;
   return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
                      sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream));
+}
+
+int kf_field_stage_box(const double* g, int32_t n_surfaces, kf_field* fl) {
+  if (!fl) return KF_ERR_ARG;
+  for (int a = 0; a < 3; ++a) fl->stage_lo[a] = fl->stage_n[a] = 0;
+  if (fl->kind != KF_FIELD_GRID3) return KF_OK;
+  if (!g || n_surfaces < 1) return KF_ERR_ARG;
+  for (int a = 0; a < 3; ++a)
+    if (fl->n[a] < 2 || !(fl->spacing[a] > 0.0)) return KF_ERR_ARG;
+  double lo[3] = {INFINITY, INFINITY, INFINITY}, hi[3] = {-INFINITY, -INFINITY, -INFINITY};
+  for (int s = 0; s < n_surfaces; ++s) {
+    const double* r = g + (size_t)s * KF_GEOM_STRIDE;
+    if (!(r[12] > 0.0 && r[13] > 0.0 && std::isfinite(r[12]) && std::isfinite(r[13]))) return KF_OK;  // no acceptance known
+    for (int a = 0; a < 3; ++a) {
+      const double e = std::fabs(r[3 + a]) * r[12] + std::fabs(r[6 + a]) * r[13];  // extent of the rectangle along axis a
+      lo[a] = std::min(lo[a], r[a] - e);
+      hi[a] = std::max(hi[a], r[a] + e);
+    }
+  }
+  int32_t blo[3], bn[3];
+  for (int a = 0; a < 3; ++a) {
+    // cells floor(f) - 1 .. floor(f) + 1 around both ends, clamped like the lookup clamps them
+    const double f0 = std::floor((lo[a] - fl->origin[a]) / fl->spacing[a]) - 1.0;
+    const double f1 = std::floor((hi[a] - fl->origin[a]) / fl->spacing[a]) + 1.0;
+    const int c0 = (int)std::min(std::max(f0, 0.0), (double)(fl->n[a] - 2));
+    const int c1 = (int)std::min(std::max(f1, 0.0), (double)(fl->n[a] - 2));
+    blo[a] = c0;
+    bn[a] = c1 - c0 + 2;  // nodes of cells c0 .. c1
+  }
+  if ((size_t)bn[0] * bn[1] * bn[2] * 3 * sizeof(double) > KF_FIELD_STAGE_MAX_BYTES) return KF_OK;
+  for (int a = 0; a < 3; ++a) { fl->stage_lo[a] = blo[a]; fl->stage_n[a] = bn[a]; }
+  return KF_OK;
 }
 
 double kf_probe_fp64_tflops(int iters, void* cuda_stream) {

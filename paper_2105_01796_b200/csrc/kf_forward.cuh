@@ -45,7 +45,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   const FieldDescT<R>& Fd = field_of<R>(P);
   const MaterialDescT<R>& Md = material_of<R>(P);
   static_assert(BLOCK % KF_TILE == 0, "a forward CTA covers whole tiles");
-  extern __shared__ __align__(16) unsigned char s_fwd_raw[];
+  unsigned char* const s_fwd_raw = kf_dyn_smem;
   const R* __restrict__ G;
   if constexpr (GEOM_SMEM) {
     stage_geometry<R>(P, reinterpret_cast<R*>(s_fwd_raw));
@@ -54,6 +54,18 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     G = reinterpret_cast<const R*>(P.geom);  // (double only, see the static_assert)
   }
   double* const s_dyn = reinterpret_cast<double*>(s_fwd_raw + (GEOM_SMEM ? geom_smem_bytes<R>(P.n_surfaces) : 0));  // hit slots
+  if constexpr (FIELD == FIELD_GRID3S) {
+    // the box of the field table the host chose (kf_field.stage_*) -> shared memory, once per CTA, as values of type R
+    R* const s_box = reinterpret_cast<R*>(kf_dyn_smem + Fd.box_off);
+    const int bx = Fd.box_n[0] * 3, by = Fd.box_n[1], bz = Fd.box_n[2];
+    const int rows = by * bz;
+    for (int e = threadIdx.x; e < rows * bx; e += BLOCK) {
+      const int rw = e / bx, c = e - rw * bx, k = rw / by, j = rw - k * by;
+      s_box[e] = (R)__ldg(Fd.grid + ((size_t)(Fd.box_lo[2] + k) * Fd.n[1] + (size_t)(Fd.box_lo[1] + j)) * ((size_t)Fd.n[0] * 3) +
+                          (size_t)Fd.box_lo[0] * 3 + c);
+    }
+    __syncthreads();
+  }
   const long long tslot = ((long long)blockIdx.x * BLOCK + threadIdx.x) / LPT;
   if (tslot >= P.N) return;    // LPT > 1: a group is 8 aligned lanes, so whole groups leave together
   const long long i = P.perm ? (long long)P.perm[tslot] : tslot;  // the track this slot fits

@@ -40,11 +40,16 @@ struct ForwardChoice {
   bool big;       // KF_FWD_BLOCK threads per CTA instead of KF_FWD_BLOCK_SMALL
   bool plain;     // default stepping, per-surface resolutions, no per-leg PRED/FILT states, no RKN estimate
   bool mbf;       // Bryson-Frazier records
+  bool staged;    // grid field with a box of the table in shared memory (FIELD_GRID3S; P.field.box_* set)
 };
 
 // kf_fwd_const.cu / kf_fwd_grid.cu: FP64, one thread per track
 int launch_forward_const(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
 int launch_forward_grid(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
+// kf_fwd_staged.cu: grid field with the staged box, FP64 and MIXED, one thread per track.  smem_box = bytes of the box
+int launch_forward_staged(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
+// threads per CTA the staged kernels take for a box of `box_bytes` (two 128-thread CTAs per SM while two boxes fit)
+int staged_block(size_t box_bytes);
 // kf_fwd_lanes.cu: FP64, 8 lanes per track
 int launch_forward_lanes(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
 // kf_fwd_mixed.cu: float operands and records (kf_options.precision MIXED)

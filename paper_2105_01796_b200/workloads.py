@@ -18,6 +18,8 @@ from __future__ import annotations
 from dataclasses import dataclass, field as _dc_field
 from typing import Optional
 
+import os
+
 import numpy as np
 
 # ---------------------------------------------------------------------------------------------
@@ -134,6 +136,8 @@ def _trilinear(grid, n, origin, spacing, pos):
         i = np.clip(np.floor(f), 0, n[a] - 2).astype(np.int64)
         idx.append(i)
         w.append(np.clip(f - i, 0.0, 1.0))
+    flat = grid.reshape(-1, 3)                      # node (k, j, i) at row (k * ny + j) * nx + i
+    base = (idx[2] * n[1] + idx[1]) * n[0] + idx[0]
     out = np.zeros((pos.shape[0], 3))
     for dz in (0, 1):
         wz = w[2] if dz else 1.0 - w[2]
@@ -141,7 +145,7 @@ def _trilinear(grid, n, origin, spacing, pos):
             wy = w[1] if dy else 1.0 - w[1]
             for dx in (0, 1):
                 wx = w[0] if dx else 1.0 - w[0]
-                out += (wz * wy * wx)[:, None] * grid[idx[2] + dz, idx[1] + dy, idx[0] + dx, :]
+                out += (wz * wy * wx)[:, None] * np.take(flat, base + ((dz * n[1] + dy) * n[0] + dx), axis=0)
     return out
 
 
@@ -193,45 +197,71 @@ def _rk4_to_x_plane(st: _Truth, x_plane: float, grid_desc, mass: float, max_step
     """Classical RK4 on (r, T) in the trilinear grid field with fixed steps <= max_step, then
     Newton-like landing steps onto x = x_plane (simulation only; U15 of SURVEY.md 8(c))."""
     n, origin, spacing, grid = grid_desc
-    r = np.stack([st.x, st.y, st.z], axis=1)
-    T = np.stack([np.cos(st.phi) * np.sin(st.theta), np.sin(st.phi) * np.sin(st.theta),
-                  np.cos(st.theta)], axis=1)
-    lam = st.lam
-    path = np.zeros_like(lam)
-
-    def acc(rr, TT):
-        B = _trilinear(grid, n, origin, spacing, rr) * TESLA
-        return lam[:, None] * np.cross(TT, B)
-
-    def step(h):
-        nonlocal r, T, path
-        hh = h[:, None]
-        k1r, k1t = T, acc(r, T)
-        k2r, k2t = T + 0.5 * hh * k1t, acc(r + 0.5 * hh * k1r, T + 0.5 * hh * k1t)
-        k3r, k3t = T + 0.5 * hh * k2t, acc(r + 0.5 * hh * k2r, T + 0.5 * hh * k2t)
-        k4r, k4t = T + hh * k3t, acc(r + hh * k3r, T + hh * k3t)
-        r = r + hh / 6.0 * (k1r + 2 * k2r + 2 * k3r + k4r)
-        T = T + hh / 6.0 * (k1t + 2 * k2t + 2 * k3t + k4t)
-        T = T / np.linalg.norm(T, axis=1, keepdims=True)
-        path = path + h
-
+    # only the particles still alive are transported (a stopped one makes no further hit); every operation below is
+    # element-wise per particle, so the values of the live ones do not depend on who else is in the arrays
+    live = np.flatnonzero(st.alive)
+    if live.size == 0:
+        st.x = np.full_like(st.x, x_plane)
+        return
+    r_all = np.stack([st.x[live], st.y[live], st.z[live]], axis=1)
+    T_all = np.stack([np.cos(st.phi[live]) * np.sin(st.theta[live]), np.sin(st.phi[live]) * np.sin(st.theta[live]),
+                      np.cos(st.theta[live])], axis=1)
+    lam_all = st.lam[live]
     with np.errstate(divide="ignore", invalid="ignore"):
-        n_big = int(np.ceil(np.nanmax(np.where(st.alive, (x_plane - r[:, 0]) / np.maximum(T[:, 0], 0.2), 0.0)) / max_step))
-        n_big = max(n_big, 1)
-        for i in range(n_big):
-            h = (x_plane - r[:, 0]) / T[:, 0] / (n_big - i)
-            h = np.where(st.alive & np.isfinite(h), h, 0.0)
-            step(h)
-        for _ in range(3):
-            h = (x_plane - r[:, 0]) / T[:, 0]
-            h = np.where(st.alive & np.isfinite(h), h, 0.0)
-            step(h)
-    st.alive &= T[:, 0] > 1e-3
+        n_big = int(np.ceil(np.nanmax((x_plane - r_all[:, 0]) / np.maximum(T_all[:, 0], 0.2)) / max_step))
+    n_big = max(n_big, 1)
+
+    def transport(sl):
+        """The particles of one slice through the n_big + 3 steps (every operation is per particle)."""
+        r, T, lam = r_all[sl], T_all[sl], lam_all[sl]
+        path = np.zeros_like(lam)
+
+        def acc(rr, TT):
+            B = _trilinear(grid, n, origin, spacing, rr) * TESLA
+            return lam[:, None] * np.cross(TT, B)
+
+        def step(h):
+            nonlocal r, T, path
+            hh = h[:, None]
+            k1r, k1t = T, acc(r, T)
+            k2r, k2t = T + 0.5 * hh * k1t, acc(r + 0.5 * hh * k1r, T + 0.5 * hh * k1t)
+            k3r, k3t = T + 0.5 * hh * k2t, acc(r + 0.5 * hh * k2r, T + 0.5 * hh * k2t)
+            k4r, k4t = T + hh * k3t, acc(r + hh * k3r, T + hh * k3t)
+            r = r + hh / 6.0 * (k1r + 2 * k2r + 2 * k3r + k4r)
+            T = T + hh / 6.0 * (k1t + 2 * k2t + 2 * k3t + k4t)
+            T = T / np.linalg.norm(T, axis=1, keepdims=True)
+            path = path + h
+
+        with np.errstate(divide="ignore", invalid="ignore"):
+            for i in range(n_big):
+                h = (x_plane - r[:, 0]) / T[:, 0] / (n_big - i)
+                h = np.where(np.isfinite(h), h, 0.0)
+                step(h)
+            for _ in range(3):
+                h = (x_plane - r[:, 0]) / T[:, 0]
+                h = np.where(np.isfinite(h), h, 0.0)
+                step(h)
+        return r, T, path
+
+    # slices of particles side by side on the host's cores (numpy releases the interpreter lock inside its loops)
+    chunk = 16384
+    slices = [slice(a, min(a + chunk, live.size)) for a in range(0, live.size, chunk)]
+    if len(slices) > 1:
+        from concurrent.futures import ThreadPoolExecutor
+        with ThreadPoolExecutor(max_workers=min(len(slices), os.cpu_count() or 1)) as pool:
+            parts = list(pool.map(transport, slices))
+    else:
+        parts = [transport(slices[0])]
+    r = np.concatenate([p[0] for p in parts])
+    T = np.concatenate([p[1] for p in parts])
+    path = np.concatenate([p[2] for p in parts])
+    lam = lam_all
+    st.alive[live] &= T[:, 0] > 1e-3
     st.x = np.full_like(st.x, x_plane)
-    st.y, st.z = r[:, 1].copy(), r[:, 2].copy()
-    st.phi = np.arctan2(T[:, 1], T[:, 0])
-    st.theta = np.arccos(np.clip(T[:, 2], -1.0, 1.0))
-    st.t = st.t + path * np.sqrt(1.0 + (mass * lam) ** 2)
+    st.y[live], st.z[live] = r[:, 1], r[:, 2]
+    st.phi[live] = np.arctan2(T[:, 1], T[:, 0])
+    st.theta[live] = np.arccos(np.clip(T[:, 2], -1.0, 1.0))
+    st.t[live] = st.t[live] + path * np.sqrt(1.0 + (mass * lam) ** 2)
 
 
 def highland_theta0(p, mass, x_over_X0_eff):

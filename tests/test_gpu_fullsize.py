@@ -94,9 +94,34 @@ def test_cfg3_full_size_ragged_with_outliers():
     assert got.n_outliers.sum() < 1.02 * n_true + 3e-3 * wl.n_meas
 
 
-def test_cfg4_field_map_large():
-    wl = W.make_config(4, n_tracks=60_000)
+def test_cfg4_full_size_field_map():
+    """BASELINE.json configs[4] at its full size (1,000,000 ragged tracks in the grid field, length-sorted): sampled
+    tracks against the oracle, properties on all; then the same batch with the field's acceptance box staged in shared
+    memory (kf_field.stage_*): every output bit for bit the same."""
+    import torch
+    wl = W.make_config(4)
+    assert wl.n_tracks == 1_000_000
     got = run_full(wl)
     sampled_parity(wl, got, 3000, 4)
     common_properties(wl, got)
-    assert np.any(got.status & 32)
+    assert np.any(got.status & 32)   # the planes beyond x = 400 mm lie outside the table: clamped lookups
+    lengths = got.n_used + got.n_outliers + got.n_holes
+    assert lengths.min() >= 0 and lengths.max() == 30 and 10 < lengths.mean() < 16
+    # pulls of the filtered state at the last visited layer against truth entering that layer: unit width
+    ok = ((got.status & 7) == 0) & (got.n_used >= 5)
+    last = np.clip(lengths - 1, 0, 29)
+    truth_last = wl.truth[np.arange(wl.n_tracks), last, :]
+    pull = (got.last_params - truth_last) / np.sqrt(np.einsum("nii->ni", got.last_cov))
+    assert np.all(np.abs(pull[ok][:, :5].mean(0)) < 0.02)
+    assert np.all(np.abs(pull[ok][:, :5].std(0) - 1.0) < 0.02)
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    hb = db.host
+    out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False)
+    call = kf.FitCall(db, out=out, field_stage=True)
+    assert call.field.stage_n[0] >= 2   # the hint was derived from the geometry's half lengths
+    call.run()
+    torch.cuda.synchronize()
+    staged = call.out.to_host()
+    for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status", "n_used", "n_outliers",
+                 "n_holes", "hit_chi2", "hit_flags"):
+        np.testing.assert_array_equal(getattr(staged, name), getattr(got, name), err_msg=name)

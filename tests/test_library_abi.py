@@ -36,7 +36,7 @@ def test_struct_sizes_match_the_header_layout():
     assert C.sizeof(B.KfTracksIn) == 32
     assert C.sizeof(B.KfMeasurements) == 48
     assert C.sizeof(B.KfGeometry) == 48
-    assert C.sizeof(B.KfField) == 4 + 4 + 24 + 12 + 4 + 24 + 24 + 8
+    assert C.sizeof(B.KfField) == 4 + 4 + 24 + 12 + 4 + 24 + 24 + 8 + 12 + 12
     assert C.sizeof(B.KfOptions) == 56 + 8 + 8 + 48 + 8  # ... perigee line (48), precision (int32 + padding)
     assert C.sizeof(B.KfOutputs) == 10 * 8 + 6 * 8 + 3 * 8 + 2 * 8
     assert C.sizeof(B.KfPipeline) == 8 + 8 * 8 + 9 * 8 + 8
@@ -44,7 +44,7 @@ def test_struct_sizes_match_the_header_layout():
 
 def test_defaults_and_version():
     L = B.lib()
-    assert L.kf_version() == 106
+    assert L.kf_version() == 107
     o = B.default_options()
     assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort, o.precision) == (1, 0, 2, 0, 0, 0, 0)
     assert o.outlier_chi2 == 0.0 and np.isinf(o.max_step_mm) and o.cov_inflation == 1.0
@@ -186,3 +186,35 @@ def test_product_path_never_imports_the_oracle():
                 src = open(os.path.join(dirpath, f)).read()
                 assert "import oracle" not in src and "from oracle" not in src, f
                 assert "kf_oracle" not in src, f
+
+
+def test_field_stage_box_from_the_host_geometry():
+    """kf_field_stage_box (host arithmetic only): the node box around every surface's rectangle plus one cell of margin,
+    clipped to the grid; cleared for a constant field, for a table without half lengths, for a box that does not fit."""
+    from paper_2105_01796_b200 import workloads as W
+    L = B.lib()
+    wl = W.make_config(4, n_tracks=16)
+    hb = B.HostBatch.from_workload(wl)
+    f = B._field_struct(hb, 0, stage=True)
+    # planes x = 0..900 mm, 100 x 100 mm; grid 41 x 21 x 21 nodes from (0, -100, -100), 10 mm: x is clipped to the whole
+    # axis, y and z cover cells 4..15 (-60..60 mm) -> nodes 4..17
+    assert list(f.stage_lo) == [0, 4, 4] and list(f.stage_n) == [41, 14, 14]
+    assert 41 * 14 * 14 * 3 * 8 <= 200 * 1024
+    g = np.ascontiguousarray(hb.geometry, dtype=np.float64)
+    # every corner of every rectangle lies in a cell whose nodes are all inside the box
+    for s in range(hb.n_surfaces):
+        c, u, v, hu, hv = g[s, 0:3], g[s, 3:6], g[s, 6:9], g[s, 12], g[s, 13]
+        for su in (-1, 1):
+            for sv in (-1, 1):
+                p = c + su * hu * u + sv * hv * v
+                for a in range(3):
+                    cell = int(np.clip(np.floor((p[a] - f.origin[a]) / f.spacing[a]), 0, f.n[a] - 2))
+                    assert f.stage_lo[a] <= cell and cell + 1 < f.stage_lo[a] + f.stage_n[a]
+    # no half lengths -> no hint; a finer grid -> the box no longer fits -> no hint; constant field -> no hint
+    g2 = g.copy(); g2[:, 12:14] = 0.0
+    assert L.kf_field_stage_box(g2.ctypes.data_as(C.c_void_p), hb.n_surfaces, C.byref(f)) == 0 and list(f.stage_n) == [0, 0, 0]
+    f.spacing[:] = [2.0, 2.0, 2.0]; f.n[:] = [201, 101, 101]
+    assert L.kf_field_stage_box(g.ctypes.data_as(C.c_void_p), hb.n_surfaces, C.byref(f)) == 0 and list(f.stage_n) == [0, 0, 0]
+    fc = B._field_struct(B.HostBatch.from_workload(W.make_config(0, n_tracks=4)), 0, stage=True)
+    assert fc.kind == 0 and list(fc.stage_n) == [0, 0, 0]
+    assert L.kf_field_stage_box(None, 3, None) == -1
