@@ -57,7 +57,8 @@ class _Options(C.Structure):
     _fields_ = [("smooth", C.c_int32), ("material", C.c_int32), ("outlier_chi2", C.c_double),
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
                 ("cov_inflation", C.c_double), ("mat_Z", C.c_double), ("mat_A", C.c_double),
-                ("mat_rho", C.c_double), ("mat_I_eV", C.c_double), ("step_tolerance_mm", C.c_double)]
+                ("mat_rho", C.c_double), ("mat_I_eV", C.c_double), ("step_tolerance_mm", C.c_double),
+                ("field_gradient", C.c_int32)]
 
 
 _libs = {}
@@ -111,9 +112,10 @@ def make_field(kind="const", b=(0.0, 0.0, 2.0), grid_n=None, grid_origin=None, g
 
 def make_options(smooth=1, material=0, outlier_chi2=0.0, n_corr_steps=2, max_step_mm=float("inf"),
                  mass_gev=0.1056583755, cov_inflation=1.0, Z=14.0, A=28.0855, rho=2.329,
-                 I_eV=173.0, step_tolerance_mm=0.0, **_ignored):
+                 I_eV=173.0, step_tolerance_mm=0.0, field_gradient=0, **_ignored):
     o = _Options()
     o.step_tolerance_mm = float(step_tolerance_mm)
+    o.field_gradient = int(field_gradient)
     o.smooth, o.material, o.outlier_chi2 = int(smooth), int(material), float(outlier_chi2)
     o.n_corr_steps, o.max_step_mm, o.mass_gev = int(n_corr_steps), float(max_step_mm), float(mass_gev)
     o.cov_inflation = float(cov_inflation)
@@ -140,11 +142,19 @@ def field_at(fld, r, precision="f64"):
     return b, cl.value
 
 
-def rkn4_step(fld, mass, f, h, precision="f64"):
+def field_gradient_at(fld, r, precision="f64"):
+    G = np.zeros((3, 3))
+    L = lib(precision)
+    L.kfo_field_gradient_at.restype = None
+    L.kfo_field_gradient_at(C.byref(fld), _d(_arr(r)), _d(G))
+    return G
+
+
+def rkn4_step(fld, mass, f, h, precision="f64", field_gradient=0):
     fo, Ds = np.zeros(8), np.zeros((8, 8))
     eps, cl = C.c_double(0), C.c_int32(0)
     lib(precision).kfo_rkn4_step(C.byref(fld), C.c_double(mass), _d(_arr(f)), C.c_double(h), _d(fo), _d(Ds),
-                        C.byref(eps), C.byref(cl))
+                        C.byref(eps), C.byref(cl), C.c_int32(int(field_gradient)))
     return fo, Ds, eps.value
 
 

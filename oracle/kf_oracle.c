@@ -59,6 +59,7 @@ typedef struct {
 typedef struct {
   int32_t smooth, material, n_corr_steps;
   real outlier_chi2, max_step_mm, mass_gev, cov_inflation, mat_Z, mat_A, mat_rho, mat_I_eV, step_tolerance_mm;
+  int32_t field_gradient; /* 1: the step Jacobian carries the dB/dr terms of a grid field (reading U32) */
 } options_r;
 
 /* ---- tiny dense helpers ------------------------------------------------------------------- */
@@ -147,6 +148,45 @@ static void field_internal(const field_r* fld, const real r[3], real B[3], int32
   for (int a = 0; a < 3; ++a) B[a] = bt[a] * TESLA_TO_GEV_PER_MM; /* dT/ds = lam T x B */
 }
 
+/* dB_c/dr_a of the trilinear interpolant at r, in GeV/(e mm) per mm: G[c * 3 + a].  Along an axis on which the
+ * lookup is clamped (r outside the grid) the interpolant is constant: zero derivative.  CONST field: zero. */
+static void field_gradient_internal(const field_r* fld, const real r[3], real G[9]) {
+  for (int i = 0; i < 9; ++i) G[i] = 0.0;
+  if (fld->kind == KFO_FIELD_CONST) return;
+  int idx[3], inside[3];
+  real w[3];
+  for (int a = 0; a < 3; ++a) {
+    real f = (r[a] - fld->origin[a]) / fld->spacing[a];
+    real fl = floor(f);
+    if (fl < 0.0) fl = 0.0;
+    if (fl > (real)(fld->n[a] - 2)) fl = (real)(fld->n[a] - 2);
+    real ww = f - fl;
+    inside[a] = 1;
+    if (ww < 0.0) { ww = 0.0; inside[a] = 0; }
+    if (ww > 1.0) { ww = 1.0; inside[a] = 0; }
+    idx[a] = (int)fl;
+    w[a] = ww;
+  }
+  const int nx = fld->n[0], ny = fld->n[1];
+  for (int a = 0; a < 3; ++a) {
+    if (!inside[a]) continue;
+    /* d/dr_a of sum_corners prod_b w_b(d_b) node: the factor of axis a becomes (+1 or -1) / spacing_a */
+    for (int dz = 0; dz < 2; ++dz)
+      for (int dy = 0; dy < 2; ++dy)
+        for (int dx = 0; dx < 2; ++dx) {
+          const int d[3] = {dx, dy, dz};
+          real wt = 1.0;
+          for (int b = 0; b < 3; ++b) {
+            if (b == a) wt *= (d[b] ? 1.0 : -1.0) / fld->spacing[a];
+            else wt *= (d[b] ? w[b] : 1.0 - w[b]);
+          }
+          const double* node =
+              fld->grid + 3 * ((size_t)(idx[2] + dz) * ny * nx + (size_t)(idx[1] + dy) * nx + (idx[0] + dx));
+          for (int c = 0; c < 3; ++c) G[c * 3 + a] += wt * (real)node[c] * TESLA_TO_GEV_PER_MM;
+        }
+  }
+}
+
 /* M(B) a := a x B */
 static void cross_matrix(const real B[3], real M[9]) {
   M[0] = 0.0;   M[1] = B[2];  M[2] = -B[1];
@@ -156,7 +196,7 @@ static void cross_matrix(const real B[3], real M[9]) {
 
 /* ---- C.2.2: one RKN4 step with its step Jacobian -------------------------------------------- */
 static void rkn4_step_r(const field_r* fld, real mass, const real f[8], real h, real fo[8],
-                   real Ds[64], real* eps, int32_t* clamped) {
+                   real Ds[64], real* eps, int32_t* clamped, int grad) {
   const real* r = f;
   const real t = f[3];
   const real* T = f + 4;
@@ -201,6 +241,55 @@ static void rkn4_step_r(const field_r* fld, real mass, const real f[8], real h, 
   if (eps) *eps = h * h * e;
 
   if (!Ds) return;
+  if (grad) {
+    /* Step Jacobian WITH the field-gradient terms (reading U32): the derivative of the stage arithmetic above,
+     * column by column.  For the variation (dr, dT, dlam) of the step's input, with G_i = dB/dr at stage point i:
+     *   dk1 = dlam (T x B1) + lam (dT x B1 + T x (G1 dr))
+     *   dr2 = dr + (h/2) dT + (h^2/8) dk1,  dT2 = dT + (h/2) dk1,  dk2 = dlam (T2 x B2) + lam (dT2 x B2 + T2 x (G2 dr2))
+     *   dT3 = dT + (h/2) dk2 (same point),                         dk3 = dlam (T3 x B2) + lam (dT3 x B2 + T3 x (G2 dr2))
+     *   dr4 = dr + h dT + (h^2/2) dk3,      dT4 = dT + h dk3,      dk4 = dlam (T4 x B3) + lam (dT4 x B3 + T4 x (G3 dr4))
+     *   dr' = dr + h dT + (h^2/6)(dk1 + dk2 + dk3),   dT' = dT + (h/6)(dk1 + 2 dk2 + 2 dk3 + dk4)
+     * (h fixed: the dependence of the step length on the state is the path-length correction's business; the
+     * normalisation of T' is left out as in the gradient-free Jacobian below). */
+    real G1[9], G2[9], G3[9];
+    field_gradient_internal(fld, r, G1);
+    field_gradient_internal(fld, rm, G2);
+    field_gradient_internal(fld, re, G3);
+    memset(Ds, 0, 64 * sizeof(real));
+    for (int col = 0; col < 8; ++col) {
+      real dr[3] = {0.0, 0.0, 0.0}, dT[3] = {0.0, 0.0, 0.0}, dlam = 0.0, dt = 0.0;
+      if (col < 3) dr[col] = 1.0;
+      else if (col == 3) dt = 1.0;
+      else if (col < 7) dT[col - 4] = 1.0;
+      else dlam = 1.0;
+      real dk1[3], dk2[3], dk3[3], dk4[3], dB[3], a1[3], a2[3], a3[3], drs[3], dTs[3];
+      /* stage 1 */
+      matmul(3, 3, 1, G1, dr, dB);
+      cross3(T, B1, a1); cross3(dT, B1, a2); cross3(T, dB, a3);
+      for (int a = 0; a < 3; ++a) dk1[a] = dlam * a1[a] + lam * (a2[a] + a3[a]);
+      /* stage 2 */
+      for (int a = 0; a < 3; ++a) { drs[a] = dr[a] + 0.5 * h * dT[a] + 0.125 * h * h * dk1[a]; dTs[a] = dT[a] + 0.5 * h * dk1[a]; }
+      matmul(3, 3, 1, G2, drs, dB);
+      cross3(T2, B2, a1); cross3(dTs, B2, a2); cross3(T2, dB, a3);
+      for (int a = 0; a < 3; ++a) dk2[a] = dlam * a1[a] + lam * (a2[a] + a3[a]);
+      /* stage 3: same point, direction T3 */
+      for (int a = 0; a < 3; ++a) dTs[a] = dT[a] + 0.5 * h * dk2[a];
+      cross3(T3, B2, a1); cross3(dTs, B2, a2); cross3(T3, dB, a3);
+      for (int a = 0; a < 3; ++a) dk3[a] = dlam * a1[a] + lam * (a2[a] + a3[a]);
+      /* stage 4 */
+      for (int a = 0; a < 3; ++a) { drs[a] = dr[a] + h * dT[a] + 0.5 * h * h * dk3[a]; dTs[a] = dT[a] + h * dk3[a]; }
+      matmul(3, 3, 1, G3, drs, dB);
+      cross3(T4, B3, a1); cross3(dTs, B3, a2); cross3(T4, dB, a3);
+      for (int a = 0; a < 3; ++a) dk4[a] = dlam * a1[a] + lam * (a2[a] + a3[a]);
+      for (int a = 0; a < 3; ++a) {
+        Ds[a * 8 + col] = dr[a] + h * dT[a] + h * h / 6.0 * (dk1[a] + dk2[a] + dk3[a]);
+        Ds[(4 + a) * 8 + col] = dT[a] + h / 6.0 * (dk1[a] + 2.0 * dk2[a] + 2.0 * dk3[a] + dk4[a]);
+      }
+      Ds[3 * 8 + col] = dt + h * mass * mass * lam / dtds * dlam;
+      Ds[7 * 8 + col] = dlam;
+    }
+    return;
+  }
   /* step Jacobian, field gradient neglected (reading U4) */
   real M1[9], M2[9], M3[9], d1[9], d2[9], d3[9], d4[9], P[9];
   cross_matrix(B1, M1);
@@ -250,26 +339,138 @@ static void rkn4_step_r(const field_r* fld, real mass, const real f[8], real h, 
   Ds[3 * 8 + 7] = h * mass * mass * lam / dtds; /* dt'/dlam */
 }
 
+/* ---- surfaces ("surfaces of different concrete types for different tracking detectors";
+ * DESIGN.md reading U33).  Record entry [18] = kind:
+ *   0 PLANE     centre c, orthonormal u, v, n = u x v;  r = c + loc0 u + loc1 v
+ *   1 CYLINDER  axis v through c, radius R = entry [12], azimuth alpha = loc0 / R measured from n towards u:
+ *               r = c + R (cos alpha n + sin alpha u) + loc1 v     (loc0 = R alpha: the arc length, loc1: along the axis)
+ *   2 DISC      the plane through c with normal n in polar coordinates: r = c + rho (cos alpha u + sin alpha v),
+ *               loc0 = rho > 0, loc1 = alpha in (-pi, pi]
+ * Each kind provides: local -> global with the tangent vectors dr/dloc; global -> local with the rows dloc/dr;
+ * the unit normal at a point; the straight-line path length from (r, T) to the surface. */
+enum { SURF_PLANE = 0, SURF_CYLINDER = 1, SURF_DISC = 2 };
+static int surf_kind(const real* s) { return (int)s[18]; }
+
+static void local_to_global(const real* s, real l0, real l1, real r[3], real e0[3], real e1[3]) {
+  const real *c = s, *u = s + 3, *v = s + 6, *n = s + 9;
+  const int kind = surf_kind(s);
+  if (kind == SURF_CYLINDER) {
+    const real R = s[12], al = l0 / R, ca = cos(al), sa = sin(al);
+    for (int a = 0; a < 3; ++a) {
+      r[a] = c[a] + R * (ca * n[a] + sa * u[a]) + l1 * v[a];
+      e0[a] = -sa * n[a] + ca * u[a]; /* dr/dloc0 = (1/R) dr/dalpha */
+      e1[a] = v[a];
+    }
+  } else if (kind == SURF_DISC) {
+    const real ca = cos(l1), sa = sin(l1);
+    for (int a = 0; a < 3; ++a) {
+      r[a] = c[a] + l0 * (ca * u[a] + sa * v[a]);
+      e0[a] = ca * u[a] + sa * v[a];          /* dr/drho */
+      e1[a] = l0 * (-sa * u[a] + ca * v[a]);  /* dr/dalpha */
+    }
+  } else {
+    for (int a = 0; a < 3; ++a) {
+      r[a] = c[a] + l0 * u[a] + l1 * v[a];
+      e0[a] = u[a];
+      e1[a] = v[a];
+    }
+  }
+}
+
+/* unit normal of the surface at the point r (which lies on it) */
+static void surface_normal(const real* s, const real r[3], real nrm[3]) {
+  const real *c = s, *v = s + 6, *n = s + 9;
+  if (surf_kind(s) == SURF_CYLINDER) {
+    real d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
+    const real z = dot3(d, v);
+    real dp[3] = {d[0] - z * v[0], d[1] - z * v[1], d[2] - z * v[2]};
+    const real rho = sqrt(dot3(dp, dp));
+    for (int a = 0; a < 3; ++a) nrm[a] = dp[a] / rho;
+  } else {
+    for (int a = 0; a < 3; ++a) nrm[a] = n[a];
+  }
+}
+
+/* local coordinates of the point r on the surface and the rows g0 = dloc0/dr, g1 = dloc1/dr */
+static void global_to_local(const real* s, const real r[3], real* l0, real* l1, real g0[3], real g1[3]) {
+  const real *c = s, *u = s + 3, *v = s + 6, *n = s + 9;
+  const real d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
+  const int kind = surf_kind(s);
+  if (kind == SURF_CYLINDER) {
+    const real R = s[12];
+    const real dn = dot3(d, n), du = dot3(d, u);
+    const real al = atan2(du, dn), rho2 = dn * dn + du * du;
+    *l0 = R * al;
+    *l1 = dot3(d, v);
+    for (int a = 0; a < 3; ++a) {
+      g0[a] = R * (dn * u[a] - du * n[a]) / rho2; /* R dalpha/dr */
+      g1[a] = v[a];
+    }
+  } else if (kind == SURF_DISC) {
+    const real du = dot3(d, u), dv = dot3(d, v);
+    const real rho = sqrt(du * du + dv * dv);
+    *l0 = rho;
+    *l1 = atan2(dv, du);
+    for (int a = 0; a < 3; ++a) {
+      g0[a] = (du * u[a] + dv * v[a]) / rho;
+      g1[a] = (du * v[a] - dv * u[a]) / (rho * rho);
+    }
+  } else {
+    *l0 = dot3(u, d);
+    *l1 = dot3(v, d);
+    for (int a = 0; a < 3; ++a) {
+      g0[a] = u[a];
+      g1[a] = v[a];
+    }
+  }
+}
+
+/* Straight-line path length h from (r, T) to the surface.  Planes and discs: h = n.(c - r)/(n.T), n.T > NT_MIN.
+ * Cylinder: with d, T projected on the plane normal to the axis, |d_p + h T_p|^2 = R^2, i.e. a h^2 + 2 b h + c0 = 0,
+ * a = |T_p|^2, b = d_p.T_p, c0 = |d_p|^2 - R^2; the root taken is h = -c0 / (b + sqrt(b^2 - a c0)): the crossing
+ * ahead for a track inside the cylinder (c0 < 0), and the near root in cancellation-free form once the track is
+ * within round-off of the surface and moving outwards.  Returns 0 when the surface cannot be reached. */
+static int path_to_surface(const real* s, const real r[3], const real T[3], real* h) {
+  const real *c = s, *v = s + 6, *n = s + 9;
+  if (surf_kind(s) == SURF_CYLINDER) {
+    const real R = s[12];
+    real d[3] = {r[0] - c[0], r[1] - c[1], r[2] - c[2]};
+    const real dz = dot3(d, v), tz = dot3(T, v);
+    real dp[3], tp[3];
+    for (int a = 0; a < 3; ++a) { dp[a] = d[a] - dz * v[a]; tp[a] = T[a] - tz * v[a]; }
+    const real a2 = dot3(tp, tp), b = dot3(dp, tp), c0 = dot3(dp, dp) - R * R;
+    const real disc = b * b - a2 * c0;
+    if (!(disc > 0.0)) return 0;
+    const real den = b + sqrt(disc);
+    if (!(den > NT_MIN * R)) return 0;
+    *h = -c0 / den;
+    return 1;
+  }
+  const real nT = dot3(n, T);
+  if (!(nT > NT_MIN)) return 0;
+  real dr[3] = {c[0] - r[0], c[1] - r[1], c[2] - r[2]};
+  *h = dot3(n, dr) / nT;
+  return 1;
+}
+
 /* ---- C.2.1 - C.2.3: bound -> bound propagation with the 6x6 Jacobian ------------------------ */
 static int32_t propagate_r(const field_r* fld, const options_r* opt, const real x[6],
                       const real* sf, const real* st, real xo[6], real J[36],
                       real free_out[8], real* rk_err, int32_t* clamped) {
-  const real *cf = sf, *uf = sf + 3, *vf = sf + 6;
-  const real *ct = st, *ut = st + 3, *vt = st + 6, *nt = st + 9;
   const real mass = opt->mass_gev;
 
   /* C.2.1 bound -> free on the start surface */
   const real sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
-  real f[8];
-  for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
+  real f[8], e0[3], e1[3];
+  local_to_global(sf, x[0], x[1], f, e0, e1);
   f[3] = x[5];
   f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
   f[7] = x[4];
   real Jb2f[48];
   memset(Jb2f, 0, sizeof(Jb2f));
   for (int a = 0; a < 3; ++a) {
-    Jb2f[a * 6 + 0] = uf[a];
-    Jb2f[a * 6 + 1] = vf[a];
+    Jb2f[a * 6 + 0] = e0[a];
+    Jb2f[a * 6 + 1] = e1[a];
   }
   Jb2f[3 * 6 + 5] = 1.0;
   Jb2f[4 * 6 + 2] = -sphi * sth; Jb2f[4 * 6 + 3] = cphi * cth;
@@ -284,10 +485,8 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   real errmax = 0.0;
   int n_sub = 1;
   {
-    real nT = dot3(nt, f + 4);
-    if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
-    real dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
-    real s0 = dot3(nt, dr) / nT;
+    real s0;
+    if (!path_to_surface(st, f, f + 4, &s0)) return KFO_ST_PROPAGATION;
     if (isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
       real q = ceil(fabs(s0) / opt->max_step_mm * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;
@@ -301,7 +500,7 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
      * per leg before any step is taken: no accept/reject loop. */
     if (isfinite(opt->step_tolerance_mm) && opt->step_tolerance_mm > 0.0) {
       real ft[8], Dt_[64], e0 = 0.0;
-      rkn4_step_r(fld, mass, f, s0, ft, Dt_, &e0, clamped);
+      rkn4_step_r(fld, mass, f, s0, ft, Dt_, &e0, clamped, 0);
       real q = ceil(sqrt(sqrt(e0 / opt->step_tolerance_mm)) * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;
       if (q > (real)MAX_SUBSTEPS) q = (real)MAX_SUBSTEPS;
@@ -310,13 +509,11 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   }
   const int n_steps = n_sub + opt->n_corr_steps;
   for (int is = 0; is < n_steps; ++is) {
-    real nT = dot3(nt, f + 4);
-    if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
-    real dr[3] = {ct[0] - f[0], ct[1] - f[1], ct[2] - f[2]};
-    real h = dot3(nt, dr) / nT;
-    if (is < n_sub) h = h / (real)(n_sub - is); /* the last primary step aims at the plane */
+    real h;
+    if (!path_to_surface(st, f, f + 4, &h)) return KFO_ST_PROPAGATION;
+    if (is < n_sub) h = h / (real)(n_sub - is); /* the last primary step aims at the surface */
     real fn[8], e = 0.0;
-    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped);
+    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped, opt->field_gradient);
     if (e > errmax) errmax = e;
     matmul(8, 8, 8, Ds, D, Dn);
     memcpy(D, Dn, sizeof(D));
@@ -329,6 +526,8 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   const real* r = f;
   const real* T = f + 4;
   const real lam = f[7];
+  real nt[3];
+  surface_normal(st, r, nt); /* planes, discs: the record's n; cylinder: the radial direction at r */
   const real nT = dot3(nt, T);
   if (!(nT > NT_MIN)) return KFO_ST_PROPAGATION;
   real B[3], TxB[3];
@@ -347,9 +546,8 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   const real phn = atan2(T[1], T[0]);
   const real s2 = sin(thn), c2 = cos(thn), sp = sin(phn), cp = cos(phn);
   if (!(s2 > SIN_THETA_MIN)) return KFO_ST_THETA;
-  real dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
-  xo[0] = dot3(ut, dr);
-  xo[1] = dot3(vt, dr);
+  real g0[3], g1[3];
+  global_to_local(st, r, &xo[0], &xo[1], g0, g1);
   xo[2] = phn;
   xo[3] = thn;
   xo[4] = lam;
@@ -357,8 +555,8 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   real Jf2b[48];
   memset(Jf2b, 0, sizeof(Jf2b));
   for (int a = 0; a < 3; ++a) {
-    Jf2b[0 * 8 + a] = ut[a];
-    Jf2b[1 * 8 + a] = vt[a];
+    Jf2b[0 * 8 + a] = g0[a];
+    Jf2b[1 * 8 + a] = g1[a];
   }
   Jf2b[2 * 8 + 4] = -sp / s2; Jf2b[2 * 8 + 5] = cp / s2; Jf2b[2 * 8 + 6] = 0.0;
   Jf2b[3 * 8 + 4] = cp * c2;  Jf2b[3 * 8 + 5] = sp * c2; Jf2b[3 * 8 + 6] = -s2;
@@ -391,19 +589,18 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
 static int32_t to_line_r(const field_r* fld, const options_r* opt, const real x[6], const real C[36],
                     const real* sf, const real lc[3], const real la[3], real xo[6], real Co[36],
                     real J[36], int32_t* clamped) {
-  const real *cf = sf, *uf = sf + 3, *vf = sf + 6;
   const real mass = opt->mass_gev;
   const real sphi = sin(x[2]), cphi = cos(x[2]), sth = sin(x[3]), cth = cos(x[3]);
-  real f[8];
-  for (int a = 0; a < 3; ++a) f[a] = cf[a] + x[0] * uf[a] + x[1] * vf[a];
+  real f[8], e0[3], e1[3];
+  local_to_global(sf, x[0], x[1], f, e0, e1);
   f[3] = x[5];
   f[4] = cphi * sth; f[5] = sphi * sth; f[6] = cth;
   f[7] = x[4];
   real Jb2f[48];
   memset(Jb2f, 0, sizeof(Jb2f));
   for (int a = 0; a < 3; ++a) {
-    Jb2f[a * 6 + 0] = uf[a];
-    Jb2f[a * 6 + 1] = vf[a];
+    Jb2f[a * 6 + 0] = e0[a];
+    Jb2f[a * 6 + 1] = e1[a];
   }
   Jb2f[3 * 6 + 5] = 1.0;
   Jb2f[4 * 6 + 2] = -sphi * sth; Jb2f[4 * 6 + 3] = cphi * cth;
@@ -439,7 +636,7 @@ static int32_t to_line_r(const field_r* fld, const options_r* opt, const real x[
     if (is >= n_sub + opt->n_corr_steps) break;
     if (is < n_sub) h = h / (real)(n_sub - is);
     real fn[8], e = 0.0;
-    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped);
+    rkn4_step_r(fld, mass, f, h, fn, Ds, &e, clamped, 0); /* the perigee extrapolation neglects dB/dr (U32) */
     matmul(8, 8, 8, Ds, D, Dn);
     memcpy(D, Dn, sizeof(D));
     memcpy(f, fn, sizeof(f));
@@ -529,7 +726,9 @@ static int32_t update_r(const real xp[6], const real Cp[36], const real m[2], co
 static int32_t material_r(const options_r* opt, const real* surf, const real xf[6],
                      const real Cf[36], real xo[6], real Co[36], real* g_out,
                      real* theta0_out, real* dE_out) {
-  const real* n = surf + 9;
+  real n[3], rpos[3], e0_[3], e1_[3];
+  local_to_global(surf, xf[0], xf[1], rpos, e0_, e1_);
+  surface_normal(surf, rpos, n); /* planes, discs: the record's n; cylinder: the radial direction at the state */
   const real xX0 = surf[14], thick = surf[15];
   const real m = opt->mass_gev;
   const real lam = xf[4];
@@ -708,6 +907,7 @@ static options_r options_to_real(const kfo_options* p) {
   o.outlier_chi2 = (real)p->outlier_chi2; o.max_step_mm = (real)p->max_step_mm; o.mass_gev = (real)p->mass_gev;
   o.cov_inflation = (real)p->cov_inflation; o.mat_Z = (real)p->mat_Z; o.mat_A = (real)p->mat_A;
   o.mat_rho = (real)p->mat_rho; o.mat_I_eV = (real)p->mat_I_eV; o.step_tolerance_mm = (real)p->step_tolerance_mm;
+  o.field_gradient = p->field_gradient;
   return o;
 }
 
@@ -971,12 +1171,20 @@ void kfo_field_at(const kfo_field* fld_in, const double r[3], double b_tesla[3],
   put(b_tesla, b, 3);
 }
 
+void kfo_field_gradient_at(const kfo_field* fld_in, const double r[3], double G_tesla_per_mm[9]) {
+  const field_r fld = field_to_real(fld_in);
+  real rr[3], G[9];
+  get(rr, r, 3);
+  field_gradient_internal(&fld, rr, G);
+  for (int i = 0; i < 9; ++i) G_tesla_per_mm[i] = (double)(G[i] / TESLA_TO_GEV_PER_MM);
+}
+
 void kfo_rkn4_step(const kfo_field* fld_in, double mass_gev, const double f[8], double h, double f_out[8],
-                   double Dstep[64], double* eps, int32_t* clamped) {
+                   double Dstep[64], double* eps, int32_t* clamped, int32_t field_gradient) {
   const field_r fld = field_to_real(fld_in);
   real fr[8], fo[8], Ds[64], e = 0.0;
   get(fr, f, 8);
-  rkn4_step_r(&fld, (real)mass_gev, fr, (real)h, fo, Dstep ? Ds : NULL, &e, clamped);
+  rkn4_step_r(&fld, (real)mass_gev, fr, (real)h, fo, Dstep ? Ds : NULL, &e, clamped, field_gradient);
   put(f_out, fo, 8);
   if (Dstep) put(Dstep, Ds, 64);
   if (eps) *eps = (double)e;

@@ -13,15 +13,22 @@
  * Pins (tests/test_oracle_*.py, run with -m "not gpu"): analytic helix, 4th-order convergence,
  * zero-field straight line, finite-difference Jacobian, noiseless recovery, weighted least
  * squares at zero field, KF+RTS == global linear least squares, covariance invariants,
- * chi2/pull statistics, the worked material table, trilinear exactness, option limits.
- * No function below is "parity unpinned".
+ * chi2/pull statistics, the worked material table, trilinear exactness, option limits; for the cylinder and disc
+ * surface kinds and the field-gradient terms of the step Jacobian (tests/test_oracle_surfaces.py): closed-form
+ * helix <-> cylinder, straight line <-> cylinder / disc, finite-difference Jacobians between every pair of kinds,
+ * chain rule through mixed kinds, disc = plane in polar coordinates, tangent-plane material, whole-fit pulls;
+ * gradient of the interpolant exact on a linear field, finite differences of the step and of the propagation in
+ * non-uniform tables.  No function below is "parity unpinned".
  *
  * Conventions:
  *   bound vector  x = (loc0, loc1, phi, theta, q/p, t)
  *   free  vector  f = (rx, ry, rz, t, Tx, Ty, Tz, q/p)          8 components
  *   units: mm, GeV, e; q/p in 1/GeV; t is c*t in mm; field in tesla at the interface
  *   geometry: packed table, 20 doubles per surface:
- *       center[3] u[3] v[3] n[3] half_len[2] x_over_X0 thickness_mm meas_var[2] pad[2]
+ *       center[3] u[3] v[3] n[3] half_len[2] x_over_X0 thickness_mm meas_var[2] kind pad
+ *       kind 0 = plane (loc = u, v coordinates), 1 = cylinder (axis v through the centre, radius = half_len[0],
+ *       loc0 = R alpha with alpha from n towards u, loc1 along the axis), 2 = disc (the plane in polar coordinates,
+ *       loc0 = rho, loc1 = alpha from u towards v)      -- PAPER.md:136-138, reading U33
  *   all matrices are dense row-major; all pointers are HOST pointers.
  */
 #ifndef KF_ORACLE_H
@@ -71,6 +78,7 @@ typedef struct {
   double cov_inflation;  /* multiplies the whole start covariance */
   double mat_Z, mat_A, mat_rho, mat_I_eV; /* one material for the batch (silicon in the configs) */
   double step_tolerance_mm; /* > 0: adaptive step count per leg (U31); <= 0 or inf: off */
+  int32_t field_gradient;   /* 1: the step Jacobian carries the dB/dr terms of a grid field (U32); 0: neglected (U4) */
 } kfo_options;
 
 /* --- step-level entry points (pinned one by one in tests/test_oracle_steps.py) ------------- */
@@ -78,12 +86,17 @@ typedef struct {
 /* B(r) in tesla; *clamped is OR-ed with 1 when r is outside the grid. */
 void kfo_field_at(const kfo_field* fld, const double r[3], double b_tesla[3], int32_t* clamped);
 
-/* One RKN4 step of length h on the free vector; Dstep is the 8x8 step Jacobian (field gradient
- * neglected), *eps the embedded error estimate h^2 |k1-k2-k3+k4|_1. */
-void kfo_rkn4_step(const kfo_field* fld, double mass_gev, const double f[8], double h,
-                   double f_out[8], double Dstep[64], double* eps, int32_t* clamped);
+/* dB_c/dr_a of the trilinear interpolant at r in tesla/mm, G[c * 3 + a]; zero along an axis on which the lookup is
+ * clamped, zero for a constant field. */
+void kfo_field_gradient_at(const kfo_field* fld, const double r[3], double G_tesla_per_mm[9]);
 
-/* bound state on surface `from` -> bound state on surface `to` with the 6x6 Jacobian.
+/* One RKN4 step of length h on the free vector; Dstep is the 8x8 step Jacobian (field gradient
+ * neglected, or with the dB/dr terms of the trilinear interpolant when field_gradient != 0),
+ * *eps the embedded error estimate h^2 |k1-k2-k3+k4|_1. */
+void kfo_rkn4_step(const kfo_field* fld, double mass_gev, const double f[8], double h,
+                   double f_out[8], double Dstep[64], double* eps, int32_t* clamped, int32_t field_gradient);
+
+/* bound state on surface `from` -> bound state on surface `to` (any kinds) with the 6x6 Jacobian.
  * Returns 0 or the status bit that stopped the propagation. */
 int32_t kfo_propagate(const kfo_field* fld, const kfo_options* opt, const double x[6],
                       const double* surf_from, const double* surf_to, double x_out[6],

@@ -286,14 +286,14 @@ def bethe_mean_dedx_mass(p, mass, mat):
         0.5 * np.log(2 * M_E * bg ** 2 * wmax / I ** 2) - beta ** 2 - dhalf)
 
 
-def _apply_material(st: _Truth, rng, x_over_X0, thickness_mm, mass, mat, g1, g2):
+def _apply_material(st: _Truth, rng, x_over_X0, thickness_mm, mass, mat, g1, g2, normal=None):
     """Gaussian multiple-scattering kick (two independent projected angles of width theta0 in the
     plane perpendicular to the direction) and mean energy loss, using the TRUE momentum before
-    the layer and the path factor 1/|n.T| (n = x axis)."""
+    the layer and the path factor 1/|n.T| (n = x axis, or the per-particle unit normals `normal` (N, 3))."""
     sth, cth = np.sin(st.theta), np.cos(st.theta)
     sph, cph = np.sin(st.phi), np.cos(st.phi)
     T = np.stack([cph * sth, sph * sth, cth], axis=1)
-    cfac = 1.0 / np.abs(T[:, 0])
+    cfac = 1.0 / np.abs(T[:, 0] if normal is None else np.sum(T * normal, axis=1))
     p = 1.0 / np.abs(st.lam)
     th0 = highland_theta0(p, mass, x_over_X0 * cfac)
     e_th = np.stack([cph * cth, sph * cth, -sth], axis=1)
@@ -424,6 +424,160 @@ def make_config(cfg: int, n_tracks: Optional[int] = None, seed: Optional[int] = 
         start_surface=0, params0=params0, cov0=cov0, offsets=offsets, surf_idx=surf_idx, loc=loc,
         options=options, material=mat, truth_start=truth_start, truth=truth,
         is_outlier=is_outlier, meta=dict(cfg=cfg, seed=c["seed"] if seed is None else seed),
+    )
+
+
+# ---------------------------------------------------------------------------------------------
+# non-planar surfaces ("surfaces of different concrete types"; U33): two small
+# tracker-shaped workloads for the cylinder and disc surface kinds.  Not BASELINE.json configs: they exist so that
+# the surface kinds are exercised by a whole fit (parity, pulls), not only step by step.
+# ---------------------------------------------------------------------------------------------
+SURF_PLANE, SURF_CYLINDER, SURF_DISC = 0, 1, 2
+
+
+def _sinc(a):
+    return np.sinc(a / np.pi)  # sin(a)/a, 1 at 0
+
+
+def _helix_advance(st: _Truth, s_t, bz_tesla, mass):
+    """Move every particle by the transverse arc length s_t along its helix in B = (0, 0, bz) (closed form, written with
+    sin(a)/a so that it stays exact for straight tracks)."""
+    sth = np.sin(st.theta)
+    kappa = -st.lam * (bz_tesla * TESLA) / sth
+    half = 0.5 * kappa * s_t
+    chord = s_t * _sinc(half)
+    st.x = st.x + chord * np.cos(st.phi + half)
+    st.y = st.y + chord * np.sin(st.phi + half)
+    st.z = st.z + s_t * np.cos(st.theta) / sth
+    st.phi = st.phi + kappa * s_t
+    st.t = st.t + (s_t / sth) * np.sqrt(1.0 + (mass * st.lam) ** 2)
+
+
+def _helix_to_cylinder(st: _Truth, R, bz_tesla, mass):
+    """To the cylinder of radius R around the z axis: Newton iteration on g(s_T) = x(s_T)^2 + y(s_T)^2 - R^2 with the
+    closed-form helix, started from the straight-line crossing (outward going)."""
+    sth = np.sin(st.theta)
+    kappa = -st.lam * (bz_tesla * TESLA) / sth
+    b = st.x * np.cos(st.phi) + st.y * np.sin(st.phi)
+    c0 = st.x ** 2 + st.y ** 2 - R * R
+    disc = b * b - c0
+    ok = disc > 0
+    s = np.where(ok, -c0 / (b + np.sqrt(np.where(ok, disc, 1.0))), 0.0)
+    for _ in range(8):
+        half = 0.5 * kappa * s
+        chord = s * _sinc(half)
+        x = st.x + chord * np.cos(st.phi + half)
+        y = st.y + chord * np.sin(st.phi + half)
+        ph = st.phi + kappa * s
+        g = x * x + y * y - R * R
+        dg = 2.0 * (x * np.cos(ph) + y * np.sin(ph))
+        with np.errstate(divide="ignore", invalid="ignore"):
+            s = np.where(ok & (dg > 0), s - g / dg, s)
+    st.alive &= ok & (s > 0)
+    _helix_advance(st, np.where(st.alive, s, 0.0), bz_tesla, mass)
+
+
+def _helix_to_z_plane(st: _Truth, z_plane, bz_tesla, mass):
+    cth = np.cos(st.theta)
+    ok = cth > 1e-3
+    s_t = np.where(ok, (z_plane - st.z) * np.sin(st.theta) / np.where(ok, cth, 1.0), 0.0)
+    st.alive &= ok & (s_t > 0)
+    _helix_advance(st, np.where(st.alive, s_t, 0.0), bz_tesla, mass)
+    st.z = np.where(st.alive, z_plane, st.z)
+
+
+def make_tracker(kind: str, n_tracks: int = 20_000, seed: Optional[int] = None, n_layers: int = 10, material: bool = True,
+                 p_range=(0.5, 10.0), smooth: bool = True) -> Workload:
+    """kind = "barrel": start plane x = 0, then n_layers cylinders around the z axis (radius 30 k mm, axis v = z,
+    azimuth from n = x towards u = y): bound (R alpha, z, phi, theta, q/p, t).
+    kind = "endcap": start plane z = 0 (u = x, v = y, n = z), then n_layers discs z = 30 k mm in polar coordinates:
+    bound (rho, alpha, phi, theta, q/p, t).
+    B = 2 T along z; truth = closed-form helix between surfaces, Highland kicks + Bethe mean loss per layer when
+    `material`; hits = truth local position + N(0, sigma), sigma = (10 um, 30 um) on cylinders (arc length, z) and
+    (10 um, 0.1 mrad) on discs (rho, alpha).  Start = truth on surface 0 smeared by the diagonal C0 of the configs."""
+    assert kind in ("barrel", "endcap")
+    N, L = int(n_tracks), int(n_layers)
+    rng = np.random.Generator(np.random.PCG64((6 if kind == "barrel" else 7) if seed is None else seed))
+    mass, mat, bz = M_MU, dict(SILICON), 2.0
+    x_over_X0, thick = (0.0032, 0.3) if material else (0.0, 0.0)
+    g = np.zeros((L + 1, GEOM_STRIDE), dtype=np.float64)
+    if kind == "barrel":
+        sig = np.array([0.010, 0.030])
+        for k in range(L + 1):
+            g[k, 0:3] = (0.0, 0.0, 0.0)
+            g[k, 3:6], g[k, 6:9], g[k, 9:12] = (0.0, 1.0, 0.0), (0.0, 0.0, 1.0), (1.0, 0.0, 0.0)
+            g[k, 12:14] = (30.0 * k, 500.0) if k > 0 else (50.0, 50.0)   # cylinder: radius, half length in z
+            g[k, 18] = SURF_CYLINDER if k > 0 else SURF_PLANE
+    else:
+        sig = np.array([0.010, 1.0e-4])
+        for k in range(L + 1):
+            g[k, 0:3] = (0.0, 0.0, 30.0 * k)
+            g[k, 3:6], g[k, 6:9], g[k, 9:12] = (1.0, 0.0, 0.0), (0.0, 1.0, 0.0), (0.0, 0.0, 1.0)
+            g[k, 12:14] = (200.0, 200.0)
+            g[k, 18] = SURF_DISC if k > 0 else SURF_PLANE
+    g[1:, 14], g[1:, 15] = x_over_X0, thick
+    g[:, 16:18] = sig[None, :] ** 2
+
+    charge = np.where(rng.random(N) < 0.5, -1.0, 1.0)
+    p = np.exp(rng.uniform(np.log(p_range[0]), np.log(p_range[1]), N))
+    st = _Truth(N)
+    if kind == "barrel":
+        st.phi = rng.uniform(-0.3, 0.3, N)
+        st.theta = np.pi / 2 + rng.uniform(-0.3, 0.3, N)
+    else:
+        st.phi = rng.uniform(-1.0, 1.0, N)
+        st.theta = rng.uniform(0.2, 0.5, N)
+    st.lam = charge / p
+
+    def bound(k):
+        if kind == "barrel":
+            if k == 0:
+                return np.stack([st.y, st.z, st.phi, st.theta, st.lam, st.t], axis=1)
+            return np.stack([30.0 * k * np.arctan2(st.y, st.x), st.z, st.phi, st.theta, st.lam, st.t], axis=1)
+        if k == 0:
+            return np.stack([st.x, st.y, st.phi, st.theta, st.lam, st.t], axis=1)
+        return np.stack([np.hypot(st.x, st.y), np.arctan2(st.y, st.x), st.phi, st.theta, st.lam, st.t], axis=1)
+
+    truth_start = bound(0)
+    truth = np.full((N, L, 6), np.nan)
+    hit_ok = np.zeros((N, L), dtype=bool)
+    hit_loc = np.zeros((N, L, 2))
+    for k in range(1, L + 1):
+        if kind == "barrel":
+            _helix_to_cylinder(st, 30.0 * k, bz, mass)
+        else:
+            _helix_to_z_plane(st, 30.0 * k, bz, mass)
+        b = bound(k)
+        truth[:, k - 1, :] = np.where(st.alive[:, None], b, np.nan)
+        hit_loc[:, k - 1, :] = b[:, :2] + rng.standard_normal((N, 2)) * sig[None, :]
+        hit_ok[:, k - 1] = st.alive
+        if material:
+            kicks = rng.standard_normal((N, 2))
+            if kind == "barrel":
+                rho = np.hypot(st.x, st.y)
+                nrm = np.stack([st.x / rho, st.y / rho, np.zeros(N)], axis=1)
+            else:
+                nrm = np.tile(np.array([0.0, 0.0, 1.0]), (N, 1))
+            _apply_material(st, rng, x_over_X0, thick, mass, mat, kicks[:, 0], kicks[:, 1], normal=nrm)
+
+    sig0 = np.stack([np.full(N, 0.05), np.full(N, 0.05), np.full(N, 1e-3), np.full(N, 1e-3),
+                     0.01 * np.abs(truth_start[:, 4]), np.full(N, C_MM_PER_NS)], axis=1)
+    params0 = truth_start + rng.standard_normal((N, 6)) * sig0
+    cov0 = np.zeros((N, 6, 6))
+    for a in range(6):
+        cov0[:, a, a] = sig0[:, a] ** 2
+    counts = hit_ok.sum(axis=1).astype(np.int32)
+    offsets = np.zeros(N + 1, dtype=np.int32)
+    np.cumsum(counts, out=offsets[1:])
+    tr, ly = np.nonzero(hit_ok)
+    options = dict(smooth=int(smooth), material=int(material), outlier_chi2=0.0, n_corr_steps=2,
+                   max_step_mm=float("inf"), mass_gev=mass, cov_inflation=1.0)
+    return Workload(
+        name=kind, n_tracks=N, n_layers=L, geometry=g, field_kind="const", field_b=np.array([0.0, 0.0, bz]),
+        grid_n=None, grid_origin=None, grid_spacing=None, grid=None, start_surface=0, params0=params0, cov0=cov0,
+        offsets=offsets, surf_idx=(ly + 1).astype(np.int32), loc=hit_loc[tr, ly, :].copy(), options=options,
+        material=mat, truth_start=truth_start, truth=truth, is_outlier=None,
+        meta=dict(kind=kind, surface_kinds=(1 << SURF_PLANE) | (1 << (SURF_CYLINDER if kind == "barrel" else SURF_DISC))),
     )
 
 

@@ -1,0 +1,446 @@
+"""Pins for the oracle's non-planar surfaces (cylinder, disc; reading U33) and for the
+field-gradient terms of the step Jacobian (reading U32).  Each check compares the oracle with
+something fixed independently of it: a closed form, a finite difference, a composition identity, a plane that must
+give the same answer, statistics of a whole fit.  CPU only.
+
+  PS1  helix <-> cylinder in B || axis: closed-form helix + scalar root of |r_T(s)|^2 = R^2
+  PS2  zero field: straight line <-> cylinder (quadratic) and <-> disc, arbitrary axis, closed form
+  PS3  finite-difference Jacobian for every pair of kinds (plane, cylinder, disc), general field direction
+  PS4  chain rule: A -> C directly = A -> B -> C with the Jacobians multiplied (mixed kinds)
+  PS5  a disc is the plane in polar coordinates: states and Jacobians related by the polar chart
+  PS6  material on a cylinder = material on the tangent plane at the same point
+  PS7  whole fits on the barrel and endcap workloads: noiseless recovery, chi2 = 2n, unit pulls
+  PG1  gradient of the trilinear interpolant: exact on a field linear in r, finite differences inside a cell, zero
+       along clamped axes
+  PG2  8x8 step Jacobian with the gradient terms against finite differences of the step in a non-uniform field;
+       without them the dT'/dr block is visibly wrong
+  PG3  bound-to-bound Jacobian in the CFG4 grid and in a strongly non-uniform grid: finite differences agree with
+       field_gradient = 1 (5e-6 / 1e-4 under a step cap), not with 0 (1.4e-2 / 0.13)
+  PG4  uniform table / constant field: field_gradient changes nothing
+  PG5  CFG4 fit with the gradient terms: unit pulls, and within a small fraction of a sigma of the fit without
+"""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2105_01796_b200 import workloads as W
+
+TESLA = 2.99792458e-4
+M_MU = 0.1056583755
+PLANE, CYL, DISC = 0, 1, 2
+
+
+def frame(u, v):
+    u = np.asarray(u, float) / np.linalg.norm(u)
+    v = np.asarray(v, float)
+    v = v - u * (u @ v)
+    v /= np.linalg.norm(v)
+    return u, v, np.cross(u, v)
+
+
+def surface(kind, center, u, v, radius=50.0, xX0=0.0, thick=0.0, var=(1e-4, 1e-4)):
+    u, v, n = frame(u, v)
+    s = np.zeros(20)
+    s[0:3], s[3:6], s[6:9], s[9:12] = center, u, v, n
+    s[12:14] = (radius, 500.0) if kind == CYL else (50.0, 50.0)
+    s[14], s[15], s[16:18], s[18] = xX0, thick, var, kind
+    return s
+
+
+def zcyl(R, center=(0.0, 0.0, 0.0)):
+    """cylinder around the z axis: axis v = z, azimuth from n = x towards u = y"""
+    return surface(CYL, center, (0, 1, 0), (0, 0, 1), radius=R)
+
+
+def local_point(s, l0, l1):
+    """the definition of the three charts, written out (test's own copy)"""
+    c, u, v, n = s[0:3], s[3:6], s[6:9], s[9:12]
+    if s[18] == CYL:
+        a = l0 / s[12]
+        return c + s[12] * (np.cos(a) * n + np.sin(a) * u) + l1 * v
+    if s[18] == DISC:
+        return c + l0 * (np.cos(l1) * u + np.sin(l1) * v)
+    return c + l0 * u + l1 * v
+
+
+def direction(phi, theta):
+    return np.array([np.cos(phi) * np.sin(theta), np.sin(phi) * np.sin(theta), np.cos(theta)])
+
+
+# ---- PS1 ---------------------------------------------------------------------------------------------------
+def helix_point(r0, phi, theta, lam, bz, s_t):
+    """closed-form helix in B = (0, 0, bz) after the transverse arc length s_t (sin(a)/a form)"""
+    kappa = -lam * bz * TESLA / np.sin(theta)
+    half = 0.5 * kappa * s_t
+    chord = s_t * np.sinc(half / np.pi)
+    return (np.array([r0[0] + chord * np.cos(phi + half), r0[1] + chord * np.sin(phi + half),
+                      r0[2] + s_t / np.tan(theta)]), phi + kappa * s_t)
+
+
+@pytest.mark.parametrize("p", [0.5, 1.0, 10.0, 100.0])
+@pytest.mark.parametrize("q", [-1.0, 1.0])
+def test_ps1_helix_to_cylinder_closed_form(p, q):
+    fld = oracle.make_field("const", (0, 0, 2.0))
+    opt = oracle.make_options(max_step_mm=2.0)   # RKN4 error ~ h^4: far below the comparison
+    sa, sb = zcyl(30.0), zcyl(75.0)
+    lam, phi, theta = q / p, 0.25, 1.35
+    x = np.array([30.0 * 0.1, -4.0, phi, theta, lam, 1.5])
+    r0 = local_point(sa, x[0], x[1])
+    # scalar root of g(s_T) = x^2 + y^2 - R^2 by bisection on the closed-form helix (no derivative, no oracle code)
+    lo, hi = 0.0, 200.0
+    for _ in range(200):
+        mid = 0.5 * (lo + hi)
+        pt, _ = helix_point(r0, phi, theta, lam, 2.0, mid)
+        lo, hi = (mid, hi) if pt[0] ** 2 + pt[1] ** 2 < 75.0 ** 2 else (lo, mid)
+    s_t = 0.5 * (lo + hi)
+    pt, phi1 = helix_point(r0, phi, theta, lam, 2.0, s_t)
+    r = oracle.propagate(fld, opt, x, sa, sb)
+    assert r.rc == 0
+    np.testing.assert_allclose(r.free[0:3], pt, atol=2e-9)
+    np.testing.assert_allclose(r.x[0], 75.0 * np.arctan2(pt[1], pt[0]), atol=2e-9)
+    np.testing.assert_allclose(r.x[1], pt[2], atol=2e-9)
+    np.testing.assert_allclose(r.x[2], phi1, atol=1e-10)
+    np.testing.assert_allclose(r.x[3], theta, atol=1e-12)
+    np.testing.assert_allclose(r.x[5], 1.5 + s_t / np.sin(theta) * np.sqrt(1 + (M_MU * lam) ** 2), atol=1e-8)
+    # default policy (one primary + two correction steps): on the surface to round-off, 4th-order accurate
+    r1 = oracle.propagate(fld, oracle.make_options(), x, sa, sb)
+    assert abs(np.hypot(r1.free[0], r1.free[1]) - 75.0) < 1e-11
+    assert np.linalg.norm(r1.free[0:3] - pt) < 2e-5 / p ** 3 + 1e-9
+
+
+# ---- PS2 ---------------------------------------------------------------------------------------------------
+def test_ps2_zero_field_straight_line_to_cylinder_and_disc():
+    fld = oracle.make_field("const", (0, 0, 0.0))
+    opt = oracle.make_options()
+    start = surface(PLANE, (1.0, -2.0, 0.5), (0.1, 1, 0), (0, 0.2, 1))
+    cyl = surface(CYL, (3.0, 1.0, -2.0), (0.1, 1.0, 0.05), (0.2, -0.1, 1.0), radius=60.0)   # tilted axis, off-origin
+    disc = surface(DISC, (80.0, 5.0, -3.0), (0.1, 1, 0.1), (-0.1, 0.05, 1))
+    x = np.array([1.5, -0.5, 0.1, 1.45, 0.7, 0.0])
+    r0, T = local_point(start, x[0], x[1]), direction(x[2], x[3])
+    # cylinder: |d_p + s T_p|^2 = R^2
+    c, u, v, n = cyl[0:3], cyl[3:6], cyl[6:9], cyl[9:12]
+    d = r0 - c
+    dp, tp = d - (d @ v) * v, T - (T @ v) * v
+    a, b, c0 = tp @ tp, dp @ tp, dp @ dp - 60.0 ** 2
+    s = (-b + np.sqrt(b * b - a * c0)) / a
+    pt = r0 + s * T
+    r = oracle.propagate(fld, opt, x, start, cyl)
+    assert r.rc == 0
+    np.testing.assert_allclose(r.free[0:3], pt, atol=1e-11)
+    dd = pt - c
+    np.testing.assert_allclose(r.x[0], 60.0 * np.arctan2(dd @ u, dd @ n), atol=1e-11)
+    np.testing.assert_allclose(r.x[1], dd @ v, atol=1e-11)
+    np.testing.assert_allclose(local_point(cyl, r.x[0], r.x[1]), pt, atol=1e-11)
+    np.testing.assert_allclose(r.x[2:5], x[2:5], atol=1e-14)
+    np.testing.assert_allclose(r.x[5], s * np.sqrt(1 + (M_MU * 0.7) ** 2), atol=1e-11)
+    # disc: plane crossing, then polar coordinates
+    c, u, v, n = disc[0:3], disc[3:6], disc[6:9], disc[9:12]
+    s = n @ (c - r0) / (n @ T)
+    pt = r0 + s * T
+    r = oracle.propagate(fld, opt, x, start, disc)
+    assert r.rc == 0
+    dd = pt - c
+    np.testing.assert_allclose(r.x[0], np.hypot(dd @ u, dd @ v), atol=1e-11)
+    np.testing.assert_allclose(r.x[1], np.arctan2(dd @ v, dd @ u), atol=1e-12)
+    np.testing.assert_allclose(local_point(disc, r.x[0], r.x[1]), pt, atol=1e-11)
+    # a track that cannot reach the cylinder (moving along its axis): stopped
+    xa = np.array([0.0, 0.0, np.arctan2(cyl[7], cyl[6]), np.arccos(cyl[8]), 0.7, 0.0])
+    assert oracle.propagate(fld, opt, xa, start, cyl).rc == 1
+
+
+# ---- PS3 ---------------------------------------------------------------------------------------------------
+def fd_jacobian(fld, opt, x, sa, sb, steps=(1e-4, 1e-4, 1e-6, 1e-6, 1e-6, 1e-3)):
+    J = np.zeros((6, 6))
+    for j in range(6):
+        xp_, xm_ = x.copy(), x.copy()
+        xp_[j] += steps[j]
+        xm_[j] -= steps[j]
+        a, b = oracle.propagate(fld, opt, xp_, sa, sb), oracle.propagate(fld, opt, xm_, sa, sb)
+        assert a.rc == 0 and b.rc == 0
+        J[:, j] = (a.x - b.x) / (2 * steps[j])
+    return J
+
+
+SURFS = {
+    "plane0": surface(PLANE, (0.0, 1.0, -2.0), (-0.2, 1, 0), (0.1, 0.1, 1)),
+    "cyl30": surface(CYL, (1.0, 0.5, 0.0), (0.05, 1, 0.02), (0.03, -0.02, 1), radius=30.0),
+    "cyl70": surface(CYL, (-1.0, 0.0, 2.0), (0, 1, 0.1), (0.1, 0, 1), radius=70.0),
+    "disc90": surface(DISC, (90.0, 3.0, -1.0), (0.1, 1, 0.1), (-0.1, 0.05, 1)),
+    "disc120": surface(DISC, (120.0, -6.0, 2.0), (0, 1, 0.05), (0.05, 0, 1)),
+    "plane150": surface(PLANE, (150.0, 0.0, 0.0), (0.1, 1, 0), (0, 0.1, 1)),
+}
+START = {   # a bound state on each start surface that moves roughly along +x
+    "plane0": [1.2, -0.7, 0.15, 1.45], "cyl30": [3.0, -4.0, 0.2, 1.4], "cyl70": [-5.0, 6.0, -0.1, 1.5],
+    "disc90": [12.0, 0.7, 0.1, 1.5], "disc120": [9.0, -2.0, -0.05, 1.6],
+}
+
+
+@pytest.mark.parametrize("legs", [("plane0", "cyl30"), ("cyl30", "cyl70"), ("cyl70", "disc90"), ("disc90", "disc120"),
+                                  ("disc120", "plane150"), ("plane0", "disc90"), ("cyl30", "plane150")])
+@pytest.mark.parametrize("p", [0.7, 5.0])
+def test_ps3_finite_difference_jacobian_between_surface_kinds(legs, p):
+    fld = oracle.make_field("const", (0.1, -0.05, 2.0))
+    # (legs up to 120 mm at 0.7 GeV: a step cap keeps the RKN4 discretisation error, which the analytic Jacobian of the
+    # flow does not follow, below the comparison)
+    opt = oracle.make_options(max_step_mm=10.0)
+    sa, sb = SURFS[legs[0]], SURFS[legs[1]]
+    x = np.array(START[legs[0]] + [-1.0 / p, 2.0])
+    r0 = oracle.propagate(fld, opt, x, sa, sb)
+    assert r0.rc == 0
+    Jfd = fd_jacobian(fld, opt, x, sa, sb)
+    scale = np.maximum(np.abs(r0.J), 1e-3)
+    assert np.max(np.abs(Jfd - r0.J) / scale) < 2e-6, np.abs(Jfd - r0.J) / scale
+    np.testing.assert_array_equal(r0.J[4], [0, 0, 0, 0, 1, 0])
+    np.testing.assert_array_equal(r0.J[:, 5], [0, 0, 0, 0, 0, 1])
+    # the landing point lies on the target surface and the local coordinates reproduce it
+    np.testing.assert_allclose(local_point(sb, r0.x[0], r0.x[1]), r0.free[0:3], atol=1e-10)
+
+
+# ---- PS4 ---------------------------------------------------------------------------------------------------
+def test_ps4_chain_rule_through_mixed_surface_kinds():
+    """The exact flow composes: A -> C = (B -> C) o (A -> B), states and Jacobians.  Small step caps take the RKN4
+    discretisation error out of the comparison."""
+    fld = oracle.make_field("const", (0.1, -0.05, 2.0))
+    opt = oracle.make_options(max_step_mm=1.0)
+    x = np.array(START["plane0"] + [1.0 / 0.9, 0.0])
+    chain = ["plane0", "cyl30", "cyl70", "disc90", "disc120", "plane150"]
+    xs, J = x, np.eye(6)
+    for a, b in zip(chain[:-1], chain[1:]):
+        r = oracle.propagate(fld, opt, xs, SURFS[a], SURFS[b])
+        assert r.rc == 0
+        xs, J = r.x, r.J @ J
+    direct = oracle.propagate(fld, opt, x, SURFS["plane0"], SURFS["plane150"])
+    assert direct.rc == 0
+    np.testing.assert_allclose(xs, direct.x, rtol=0, atol=5e-9)
+    np.testing.assert_allclose(J, direct.J, rtol=2e-7, atol=2e-7)
+
+
+# ---- PS5 ---------------------------------------------------------------------------------------------------
+def test_ps5_disc_is_the_plane_in_polar_coordinates():
+    fld = oracle.make_field("const", (0.1, -0.05, 2.0))
+    opt = oracle.make_options()
+    disc = SURFS["disc90"]
+    plane = disc.copy()
+    plane[18] = PLANE
+    x = np.array(START["plane0"] + [1.0 / 1.3, 0.0])
+    rp = oracle.propagate(fld, opt, x, SURFS["plane0"], plane)
+    rd = oracle.propagate(fld, opt, x, SURFS["plane0"], disc)
+    assert rp.rc == 0 and rd.rc == 0
+    a, b = rp.x[0], rp.x[1]
+    rho, al = np.hypot(a, b), np.arctan2(b, a)
+    np.testing.assert_allclose(rd.x, [rho, al, *rp.x[2:]], rtol=1e-14, atol=1e-13)
+    P = np.eye(6)   # d(rho, alpha)/d(a, b)
+    P[0, 0:2] = [a / rho, b / rho]
+    P[1, 0:2] = [-b / rho ** 2, a / rho ** 2]
+    np.testing.assert_allclose(rd.J, P @ rp.J, rtol=1e-12, atol=1e-13)
+    # and leaving from the disc = leaving from the plane at the same point: J_from_disc = J_from_plane d(a,b)/d(rho,alpha)
+    tgt = SURFS["plane150"]
+    fp = oracle.propagate(fld, opt, rp.x, plane, tgt)
+    fd = oracle.propagate(fld, opt, rd.x, disc, tgt)
+    np.testing.assert_allclose(fd.x, fp.x, rtol=1e-13, atol=1e-12)
+    Q = np.eye(6)
+    Q[0:2, 0] = [np.cos(al), np.sin(al)]
+    Q[0:2, 1] = [-rho * np.sin(al), rho * np.cos(al)]
+    np.testing.assert_allclose(fd.J, fp.J @ Q, rtol=1e-12, atol=1e-13)
+
+
+# ---- PS6 ---------------------------------------------------------------------------------------------------
+def test_ps6_material_on_a_cylinder_uses_the_normal_at_the_point():
+    opt = oracle.make_options(material=1)
+    cyl = zcyl(60.0)
+    cyl[14], cyl[15] = 0.0032, 0.3
+    xf = np.array([60.0 * 0.4, 3.0, 0.7, 1.3, 1.0 / 2.0, 0.0])
+    Cf = np.diag([1e-4, 1e-4, 1e-6, 1e-6, 1e-4, 1.0])
+    al = 0.4
+    er = np.array([np.cos(al), np.sin(al), 0.0])
+    # the tangent plane at the same point: same normal, so the same path factor, theta0, energy loss, G, Q
+    tang = surface(PLANE, local_point(cyl, xf[0], xf[1]), np.cross([0, 0, 1.0], er), (0, 0, 1), xX0=0.0032, thick=0.3)
+    np.testing.assert_allclose(tang[9:12], er, atol=1e-15)
+    xt = xf.copy()
+    xt[0:2] = 0.0
+    mc, mt = oracle.material(opt, cyl, xf, Cf), oracle.material(opt, tang, xt, Cf)
+    assert mc.rc == 0 and mt.rc == 0
+    np.testing.assert_allclose([mc.theta0, mc.dE, mc.g], [mt.theta0, mt.dE, mt.g], rtol=1e-14)
+    np.testing.assert_allclose(mc.C, mt.C, rtol=1e-14)
+    # and it is NOT the path factor of the record's n (the azimuth-zero direction)
+    T = direction(0.7, 1.3)
+    assert abs(1 / abs(er @ T) - 1 / abs(T[0])) > 0.05
+
+
+# ---- PS7 ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_ps7_whole_fit_on_cylinders_and_discs(kind):
+    wl = W.make_tracker(kind, n_tracks=6000)
+    assert set(np.unique(wl.geometry[:, 18])) == {0.0, 1.0 if kind == "barrel" else 2.0}
+    r = oracle.fit_workload(wl, states=True)
+    assert np.all(r.status == 0) and np.all(r.n_used == 10)
+    n = wl.n_tracks
+    assert abs(r.chi2.mean() - 20.0) < 4 * np.sqrt(40.0 / n)       # consistent prior: E[chi2] = 2n (U10)
+    for got, cov, truth in ((r.last_params, r.last_cov, wl.truth[:, -1, :]), (r.first_params, r.first_cov, wl.truth[:, 0, :])):
+        pull = (got - truth) / np.sqrt(np.einsum("nii->ni", cov))
+        assert np.all(np.abs(pull.mean(0)) < 5 / np.sqrt(n))
+        assert np.all(np.abs(pull.std(0) - 1.0) < 4 / np.sqrt(2 * n))
+    # noiseless hits, no material, exact start: the fit returns the truth on every surface
+    wl0 = W.make_tracker(kind, n_tracks=50, material=False)
+    tr, ly = np.repeat(np.arange(50), 10), np.tile(np.arange(10), 50)
+    wl0.loc[:] = wl0.truth[tr, ly, 0:2]
+    wl0.params0[:] = wl0.truth_start
+    r0 = oracle.fit_workload(wl0, states=True)
+    assert np.all(r0.status == 0)
+    np.testing.assert_allclose(r0.smooth_params, wl0.truth, rtol=0, atol=1e-5)   # RKN4 error of one ~35 mm step at 0.5 GeV
+    assert r0.chi2.max() < 1e-4
+
+
+# ---- PG1 ---------------------------------------------------------------------------------------------------
+def random_grid(seed, n=(9, 8, 7), spacing=(10.0, 12.0, 9.0), origin=(-5.0, -40.0, -30.0), smooth=True):
+    rng = np.random.default_rng(seed)
+    g = np.zeros((n[2], n[1], n[0], 3))
+    if smooth:   # a smooth non-uniform field sampled on the nodes (strong gradient: 30 % over the table)
+        xs = origin[0] + spacing[0] * np.arange(n[0])
+        ys = origin[1] + spacing[1] * np.arange(n[1])
+        zs = origin[2] + spacing[2] * np.arange(n[2])
+        Z, Y, X = np.meshgrid(zs, ys, xs, indexing="ij")
+        g[..., 2] = 2.0 * (1 - 0.3 * (X / 80.0) ** 2 + 0.1 * Y / 40.0)
+        g[..., 0] = 0.2 * Z / 30.0 + 0.05 * X * Y / 1600.0
+        g[..., 1] = -0.1 * X / 80.0 + 0.05 * np.sin(Z / 20.0)
+    else:
+        g[:] = rng.uniform(-2, 2, g.shape)
+    return oracle.make_field("grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=g), g
+
+
+def test_pg1_gradient_of_the_trilinear_interpolant():
+    n, spacing, origin = (6, 5, 4), (10.0, 8.0, 5.0), (-3.0, 2.0, 1.0)
+    A = np.array([[0.01, -0.02, 0.005], [0.0, 0.03, -0.01], [0.02, 0.01, -0.015]])
+    B0 = np.array([0.3, -0.2, 1.5])
+    xs = [origin[a] + spacing[a] * np.arange(n[a]) for a in range(3)]
+    Z, Y, X = np.meshgrid(xs[2], xs[1], xs[0], indexing="ij")
+    R = np.stack([X, Y, Z], axis=-1)
+    lin = oracle.make_field("grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=B0 + R @ A.T)
+    for r in ([5.0, 10.0, 3.0], [44.9, 33.9, 15.9], [12.3, 7.7, 9.1]):
+        np.testing.assert_allclose(oracle.field_gradient_at(lin, r), A, rtol=1e-12, atol=1e-15)   # exact on a linear field
+    fld, _ = random_grid(3, smooth=False)
+    rng = np.random.default_rng(4)
+    for _ in range(20):   # central differences inside one cell of a random table (tri-affine there: error O(d^2) = 0 + cross terms)
+        cell = [rng.integers(0, 8), rng.integers(0, 7), rng.integers(0, 6)]
+        r = np.array([-5.0 + 10.0 * (cell[0] + rng.uniform(0.2, 0.8)), -40.0 + 12.0 * (cell[1] + rng.uniform(0.2, 0.8)),
+                      -30.0 + 9.0 * (cell[2] + rng.uniform(0.2, 0.8))])
+        G = oracle.field_gradient_at(fld, r)
+        for a in range(3):
+            e = np.zeros(3)
+            e[a] = 1e-3
+            fd = (oracle.field_at(fld, r + e)[0] - oracle.field_at(fld, r - e)[0]) / 2e-3
+            np.testing.assert_allclose(G[:, a], fd, rtol=1e-9, atol=1e-11)   # exactly linear along one axis within a cell
+    # outside the table along x: clamped there, so dB/dx = 0 while the other axes still vary
+    G = oracle.field_gradient_at(fld, [-50.0, 0.0, 0.0])
+    assert np.all(G[:, 0] == 0) and np.any(G[:, 1] != 0) and np.any(G[:, 2] != 0)
+    assert np.all(oracle.field_gradient_at(oracle.make_field("const", (0, 0, 2.0)), [1.0, 2.0, 3.0]) == 0)
+
+
+# ---- PG2 ---------------------------------------------------------------------------------------------------
+def test_pg2_step_jacobian_with_gradient_terms_against_finite_differences():
+    fld, _ = random_grid(1)
+    ph, th, lam = 0.2, 1.3, 1 / 0.8
+    T = direction(ph, th)
+    f = np.concatenate([[12.0, 3.0, -4.0, 0.5], T, [lam]])
+    h = 21.0
+    fo, Dg, _ = oracle.rkn4_step(fld, M_MU, f, h, field_gradient=1)
+    _, D0, _ = oracle.rkn4_step(fld, M_MU, f, h, field_gradient=0)
+    P = np.eye(3) - np.outer(fo[4:7], fo[4:7])    # the step renormalises T; Dstep does not differentiate that
+
+    def fd_col(fp, fm, d):
+        return (oracle.rkn4_step(fld, M_MU, fp, h)[0] - oracle.rkn4_step(fld, M_MU, fm, h)[0]) / (2 * d)
+
+    def projected(col):
+        col = col.copy()
+        col[4:7] = P @ col[4:7]
+        return col
+
+    worst_without = 0.0
+    for j in (0, 1, 2, 7):       # r columns (the gradient's own) and the lam column
+        d = 1e-5 if j < 3 else 1e-6
+        fp, fm = f.copy(), f.copy()
+        fp[j] += d
+        fm[j] -= d
+        col = fd_col(fp, fm, d)
+        np.testing.assert_allclose(col, projected(Dg[:, j]), rtol=5e-7, atol=2e-9)
+        worst_without = max(worst_without, np.max(np.abs(col - projected(D0[:, j]))))
+    for e in (np.array([-np.sin(ph), np.cos(ph), 0.0]), np.array([np.cos(ph) * np.cos(th), np.sin(ph) * np.cos(th), -np.sin(th)])):
+        d = 1e-6
+        fp, fm = f.copy(), f.copy()
+        fp[4:7] = (T + d * e) / np.linalg.norm(T + d * e)
+        fm[4:7] = (T - d * e) / np.linalg.norm(T - d * e)
+        np.testing.assert_allclose(fd_col(fp, fm, d), projected(Dg[:, 4:7] @ e), rtol=5e-7, atol=2e-9)
+    # without the terms: dT'/dr is identically zero in Dstep, while the true derivative is ~ lam |grad B| h
+    assert np.all(D0[4:7, 0:3] == 0) and np.all(D0[0:3, 0:3] == np.eye(3))
+    assert worst_without > 1e-5
+    assert np.max(np.abs(Dg[4:7, 0:3])) > 1e-5
+
+
+# ---- PG3 ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg4", "strong"])
+def test_pg3_bound_jacobian_in_a_non_uniform_field(which):
+    if which == "cfg4":
+        n, origin, spacing, grid = W.cfg4_field_grid()
+        fld = oracle.make_field("grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+        sa = surface(PLANE, (300.0, 0, 0), (0, 1, 0), (0, 0, 1))
+        sb = surface(PLANE, (330.0, 0, 0), (0, 1, 0), (0, 0, 1))
+        x = np.array([3.3, -7.1, 0.15, np.pi / 2 + 0.12, -1.0 / 0.7, 2.0])   # stays inside single y, z cells
+    else:
+        fld, _ = random_grid(2)
+        sa = surface(PLANE, (2.0, 1.0, -2.0), (-0.1, 1, 0), (0.1, 0.1, 1))
+        sb = surface(PLANE, (47.0, 1.0, -2.0), (0.15, 1, 0), (0, -0.1, 1))
+        x = np.array([1.3, -0.7, 0.1, np.pi / 2 + 0.08, 1.0 / 0.6, 2.0])
+    # The analytic Jacobian is that of the flow (fixed-h step derivative + path-length correction with the flow's own
+    # f'); the finite difference differentiates the discrete map, which in a kinked (trilinear) field is only first
+    # order in the step where a step crosses a cell face.  A step cap brings the two together: measured
+    # with/without the terms  cfg4: 4.7e-5 / 1.4e-2 (one 30 mm step), 1.2e-6 / 1.4e-2 (0.25 mm);
+    # strong: 9.3e-3 / 0.13, 2.3e-5 / 0.13.
+    cap = dict(max_step_mm=0.25)
+    Jfd = fd_jacobian(fld, oracle.make_options(**cap), x, sa, sb, steps=(1e-3, 1e-3, 1e-5, 1e-5, 1e-5, 1e-3))
+    with_g = oracle.propagate(fld, oracle.make_options(field_gradient=1, **cap), x, sa, sb)
+    without = oracle.propagate(fld, oracle.make_options(field_gradient=0, **cap), x, sa, sb)
+    assert with_g.rc == 0 and without.rc == 0
+    np.testing.assert_array_equal(with_g.x, without.x)     # the state never depended on the Jacobian
+    scale = np.maximum(np.abs(with_g.J), 1e-3)
+    err1 = np.max(np.abs(Jfd - with_g.J) / scale)
+    err0 = np.max(np.abs(Jfd - without.J) / scale)
+    assert err1 < (5e-6 if which == "cfg4" else 1e-4), err1
+    assert err0 > (5e-3 if which == "cfg4" else 5e-2), err0    # U4's neglected term, visible at this level
+    # default policy (one step per leg): still two orders (cfg4) / one order (strong) nearer than without the terms
+    Jfd1 = fd_jacobian(fld, oracle.make_options(), x, sa, sb, steps=(1e-3, 1e-3, 1e-5, 1e-5, 1e-5, 1e-3))
+    g1 = oracle.propagate(fld, oracle.make_options(field_gradient=1), x, sa, sb)
+    g0 = oracle.propagate(fld, oracle.make_options(field_gradient=0), x, sa, sb)
+    s1 = np.maximum(np.abs(g1.J), 1e-3)
+    assert np.max(np.abs(Jfd1 - g1.J) / s1) < 0.1 * np.max(np.abs(Jfd1 - g0.J) / s1)
+
+
+# ---- PG4 ---------------------------------------------------------------------------------------------------
+def test_pg4_uniform_field_gradient_terms_vanish():
+    g = np.zeros((5, 5, 6, 3))
+    g[...] = (0.1, -0.05, 2.0)
+    uni = oracle.make_field("grid3", grid_n=(6, 5, 5), grid_origin=(-10.0, -40.0, -40.0), grid_spacing=(20.0, 20.0, 20.0), grid=g)
+    sa, sb = SURFS["plane0"], surface(PLANE, (45.0, 0, 0), (0.1, 1, 0), (0, 0.1, 1))
+    x = np.array(START["plane0"] + [1.0 / 0.9, 0.0])
+    a = oracle.propagate(uni, oracle.make_options(field_gradient=1), x, sa, sb)
+    b = oracle.propagate(uni, oracle.make_options(field_gradient=0), x, sa, sb)
+    c = oracle.propagate(oracle.make_field("const", (0.1, -0.05, 2.0)), oracle.make_options(field_gradient=1), x, sa, sb)
+    np.testing.assert_allclose(a.J, b.J, rtol=1e-13, atol=1e-15)   # two arrangements of the same sums
+    np.testing.assert_allclose(a.J, c.J, rtol=1e-12, atol=1e-14)
+    np.testing.assert_allclose(a.x, c.x, rtol=1e-13, atol=1e-13)
+
+
+# ---- PG5 ---------------------------------------------------------------------------------------------------
+def test_pg5_cfg4_fit_with_gradient_terms():
+    wl = W.make_config(4, n_tracks=4000)
+    r0 = oracle.fit_workload(wl)
+    r1 = oracle.fit_workload(wl, field_gradient=1)
+    np.testing.assert_array_equal(r0.status, r1.status)
+    np.testing.assert_array_equal(r0.n_used, r1.n_used)
+    ok = ((r1.status & 7) == 0) & (r1.n_used >= 5)
+    sig = np.sqrt(np.einsum("nii->ni", r0.first_cov))
+    shift = np.abs(r1.first_params - r0.first_params)[ok] / sig[ok]
+    assert 0 < shift.max() < 0.05          # a real but small effect in this mild field (0.2 % per cm)
+    lengths = r1.n_used + r1.n_holes
+    truth_last = wl.truth[np.arange(wl.n_tracks), np.clip(lengths - 1, 0, 29), :]
+    pull = ((r1.last_params - truth_last) / np.sqrt(np.einsum("nii->ni", r1.last_cov)))[ok]
+    assert np.all(np.abs(pull[:, :5].std(0) - 1.0) < 0.06)
