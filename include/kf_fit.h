@@ -56,7 +56,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 107          /* major * 100 + minor */
+#define KF_VERSION 108          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -158,10 +158,23 @@ typedef struct kf_measurements {
   const double* cov01;     /* double[M] per-hit covariance (needs var), or NULL: 0 */
 } kf_measurements;
 
-/* global data: detector geometry -- PAPER.md:168, 174, 182 (boundless planes).
+/* surface kinds (geometry record entry [18]; "surfaces of different concrete types for different
+ * tracking detectors"; reading U33).  The bound vector is (loc0, loc1, phi, theta, q/p, t) on every kind.
+ *   PLANE     r = c + loc0 u + loc1 v                                              (PAPER.md:182 boundless planes)
+ *   CYLINDER  axis v through c, radius R = entry [12]; azimuth alpha = loc0 / R measured from n towards u:
+ *             r = c + R (cos alpha n + sin alpha u) + loc1 v      (loc0 = arc length R alpha, loc1 = along the axis)
+ *             reached along the track's direction of motion from inside (navigation outwards)
+ *   DISC      the plane through c with normal n in polar coordinates: r = c + loc0 (cos loc1 u + sin loc1 v),
+ *             loc0 = rho > 0, loc1 = alpha in (-pi, pi]
+ * A measurement and the prediction it is compared with must lie on the same branch of an angular coordinate (the
+ * residual is not wrapped). */
+enum { KF_SURFACE_PLANE = 0, KF_SURFACE_CYLINDER = 1, KF_SURFACE_DISC = 2 };
+
+/* global data: detector geometry -- PAPER.md:168, 174, 182 (boundless planes), 136-138 (other kinds).
  * Surface record, KF_GEOM_STRIDE doubles:
- *   [0..2] centre  [3..5] u  [6..8] v  [9..11] n = u x v (orthonormal)  [12..13] half lengths (informational)
- *   [14] x/X0  [15] thickness in mm  [16..17] measurement variances (loc0, loc1)  [18..19] unused
+ *   [0..2] centre  [3..5] u  [6..8] v  [9..11] n = u x v (orthonormal)  [12..13] half lengths (informational; the
+ *   radius in [12] for a cylinder)  [14] x/X0 along the normal  [15] thickness in mm
+ *   [16..17] measurement variances (loc0, loc1)  [18] kind (KF_SURFACE_*, 0 = plane)  [19] unused
  * Navigation order = ascending surface index: a track visits start_surface+1, +2, ... up to the
  * surface of its last hit. */
 typedef struct kf_geometry {
@@ -170,6 +183,11 @@ typedef struct kf_geometry {
   double mat_Z, mat_A;     /* one material for the batch: atomic number, mass (g/mol) */
   double mat_rho;          /* density g/cm^3 */
   double mat_I_eV;         /* mean excitation energy */
+  int32_t surface_kinds;   /* bit k set = the table holds surfaces of kind k (the table itself is DEVICE memory, which
+                              the host-side dispatch does not read).  0 or 1 = planes only: entry [18] is then ignored
+                              and the plane-only kernels run.  Any other value selects the general-surface kernels:
+                              FP64, one thread per track, RTS smoother, at most 1024 surfaces
+                              (KF_ERR_UNSUPPORTED with MIXED precision, KF_VARIANT_LANES_PER_TRACK or Bryson-Frazier) */
 } kf_geometry;
 
 /* global data: magnetic field -- PAPER.md:170 (constant 3x1 vector; inhomogeneous fields need
@@ -222,6 +240,13 @@ typedef struct kf_options {
   double perigee_center[3];
   double perigee_axis[3];
   int32_t precision;      /* KF_PRECISION_* */
+  int32_t field_gradient; /* 1: the transported Jacobian carries the dB/dr terms of a GRID3 field (
+                             DESIGN.md reading U32): every stage derivative of the RKN4 step gains lam T_i x (G_i dr_i),
+                             G = gradient of the trilinear interpolant.  The states do not change, the covariances do
+                             (CFG4: up to a few per cent of a standard deviation on the fitted parameters).  0 (default):
+                             neglected (reading U4).  No effect in a constant field.  Runs in the general kernels (FP64,
+                             thread per track, RTS; KF_ERR_UNSUPPORTED otherwise); the perigee extrapolation neglects the
+                             terms either way */
 } kf_options;
 
 /* (4) results -- PAPER.md:180: status, track states, fitted parameters */
@@ -254,7 +279,7 @@ typedef struct kf_outputs {
 
 /* Fill `opt` with the defaults: smooth 1, material 0, outlier off, n_corr_steps 2, max_step inf,
  * no step tolerance, muon mass, inflation 1, no per-leg states, variant AUTO, length sort AUTO, perigee line = the z axis
- * through the origin, precision FP64. */
+ * through the origin, precision FP64, field gradient neglected. */
 void kf_default_options(kf_options* opt);
 
 /* Bytes of device workspace kf_fit_batch needs for n_tracks tracks and n_legs_max =

@@ -45,7 +45,7 @@ class KfMeasurements(C.Structure):
 
 class KfGeometry(C.Structure):
     _fields_ = [("n_surfaces", C.c_int32), ("surfaces", C.c_void_p), ("mat_Z", C.c_double),
-                ("mat_A", C.c_double), ("mat_rho", C.c_double), ("mat_I_eV", C.c_double)]
+                ("mat_A", C.c_double), ("mat_rho", C.c_double), ("mat_I_eV", C.c_double), ("surface_kinds", C.c_int32)]
 
 
 class KfField(C.Structure):
@@ -59,7 +59,8 @@ class KfOptions(C.Structure):
                 ("n_corr_steps", C.c_int32), ("max_step_mm", C.c_double), ("mass_gev", C.c_double),
                 ("cov_inflation", C.c_double), ("output_states", C.c_int32), ("variant", C.c_int32),
                 ("length_sort", C.c_int32), ("smoother", C.c_int32), ("step_tolerance_mm", C.c_double),
-                ("perigee_center", C.c_double * 3), ("perigee_axis", C.c_double * 3), ("precision", C.c_int32)]
+                ("perigee_center", C.c_double * 3), ("perigee_axis", C.c_double * 3), ("precision", C.c_int32),
+                ("field_gradient", C.c_int32)]
 
 
 KF_MAX_STREAMS = 8
@@ -141,8 +142,10 @@ def default_options() -> KfOptions:
 
 def make_options(smooth=1, material=0, outlier_chi2=0.0, n_corr_steps=2, max_step_mm=float("inf"),
                  mass_gev=0.1056583755, cov_inflation=1.0, output_states=0, variant=0,
-                 perigee_center=(0.0, 0.0, 0.0), perigee_axis=(0.0, 0.0, 1.0), length_sort=0, step_tolerance_mm=0.0, smoother=0, precision=0, **_ignored) -> KfOptions:
+                 perigee_center=(0.0, 0.0, 0.0), perigee_axis=(0.0, 0.0, 1.0), length_sort=0, step_tolerance_mm=0.0, smoother=0, precision=0, field_gradient=0,
+                 **_ignored) -> KfOptions:
     o = KfOptions()
+    o.field_gradient = int(field_gradient)
     o.smoother, o.precision = int(smoother), int(precision)
     o.length_sort, o.step_tolerance_mm = int(length_sort), float(step_tolerance_mm)
     for k in range(3):
@@ -254,6 +257,11 @@ def _geom_struct(hb: HostBatch, ptr: int) -> KfGeometry:
     g.n_surfaces, g.surfaces = hb.n_surfaces, ptr
     m = hb.material
     g.mat_Z, g.mat_A, g.mat_rho, g.mat_I_eV = float(m["Z"]), float(m["A"]), float(m["rho"]), float(m["I_eV"])
+    # which surface kinds the (host copy of the) table holds: the library's dispatch cannot read device memory
+    kinds = 0
+    for k in np.unique(np.asarray(hb.geometry)[:, 18]).astype(np.int64):
+        kinds |= 1 << int(k)
+    g.surface_kinds = int(kinds)
     return g
 
 

@@ -151,6 +151,74 @@ __device__ __forceinline__ void field_at(const FieldDescT<R>& F, const R r[3], R
   }
 }
 
+// B(r) and G[c][a] = dB_c/dr_a of the trilinear interpolant (GeV/(e mm) per mm), for the field-gradient terms of the
+// step Jacobian (U32).  Along an axis on which the lookup is clamped the interpolant is constant: zero
+// derivative.  A constant field has G = 0.  (Not a hot path: the eight corners are read once, plainly.)
+template <int FIELD, typename R>
+__device__ __forceinline__ void field_and_gradient_at(const FieldDescT<R>& F, const R r[3], R B[3], R G[9],
+                                                      unsigned& status) {
+#pragma unroll
+  for (int i = 0; i < 9; ++i) G[i] = R(0.0);
+  if constexpr (FIELD == FIELD_CONST) {
+    B[0] = F.b[0]; B[1] = F.b[1]; B[2] = F.b[2];
+  } else {
+    int idx[3];
+    R w[3];
+    bool inside[3];
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+      const R num = r[a] - F.origin[a];
+      R f = num * F.inv_spacing[a];
+      f = fma(fma(-f, F.spacing[a], num), F.inv_spacing[a], f);
+      R fl = floor(f);
+      fl = fmax(fl, R(0.0));
+      fl = fmin(fl, (R)(F.n[a] - 2));
+      R ww = f - fl;
+      inside[a] = true;
+      if (ww < R(0.0)) { ww = R(0.0); status |= ST_FIELD_CLAMPED; inside[a] = false; }
+      if (ww > R(1.0)) { ww = R(1.0); status |= ST_FIELD_CLAMPED; inside[a] = false; }
+      idx[a] = (int)fl;
+      w[a] = ww;
+    }
+    const int row = F.n[0] * 3, slab = row * F.n[1];
+    const double* base = F.grid + (size_t)idx[2] * slab + (size_t)idx[1] * row + (size_t)idx[0] * 3;
+    R nd[2][2][2][3];  // [dz][dy][dx][component]
+#pragma unroll
+    for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+      for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+        for (int dx = 0; dx < 2; ++dx)
+#pragma unroll
+          for (int c = 0; c < 3; ++c) nd[dz][dy][dx][c] = R(__ldg(base + dz * slab + dy * row + dx * 3 + c));
+    const R wx[2] = {R(1.0) - w[0], w[0]}, wy[2] = {R(1.0) - w[1], w[1]}, wz[2] = {R(1.0) - w[2], w[2]};
+#pragma unroll
+    for (int c = 0; c < 3; ++c) {
+      R b = R(0.0), gx = R(0.0), gy = R(0.0), gz = R(0.0);
+#pragma unroll
+      for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+        for (int dy = 0; dy < 2; ++dy) {
+#pragma unroll
+          for (int dx = 0; dx < 2; ++dx) b = fma(wz[dz] * wy[dy] * wx[dx], nd[dz][dy][dx][c], b);
+          gx = fma(wz[dz] * wy[dy], nd[dz][dy][1][c] - nd[dz][dy][0][c], gx);
+        }
+#pragma unroll
+      for (int dz = 0; dz < 2; ++dz)
+#pragma unroll
+        for (int dx = 0; dx < 2; ++dx) gy = fma(wz[dz] * wx[dx], nd[dz][1][dx][c] - nd[dz][0][dx][c], gy);
+#pragma unroll
+      for (int dy = 0; dy < 2; ++dy)
+#pragma unroll
+        for (int dx = 0; dx < 2; ++dx) gz = fma(wy[dy] * wx[dx], nd[1][dy][dx][c] - nd[0][dy][dx][c], gz);
+      B[c] = b * R(kTeslaToGeVPerMm);
+      G[c * 3 + 0] = inside[0] ? gx * F.inv_spacing[0] * R(kTeslaToGeVPerMm) : R(0.0);
+      G[c * 3 + 1] = inside[1] ? gy * F.inv_spacing[1] * R(kTeslaToGeVPerMm) : R(0.0);
+      G[c * 3 + 2] = inside[2] ? gz * F.inv_spacing[2] * R(kTeslaToGeVPerMm) : R(0.0);
+    }
+  }
+}
+
 // out[:, c] = lam * (X[:, c] x B) for the three columns of the row-major 3x3 X:  out = lam M(B) X
 template <typename R>
 __device__ __forceinline__ void cross_columns(const R X[9], const R B[3], R lam,
@@ -740,6 +808,333 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   return 0u;
 }
 
+// =====================================================================================================
+// General surfaces and the field-gradient terms: the path for geometries that are not all planes
+// (kf_geometry.surface_kinds) and for kf_options.field_gradient.  Not the hot path: one code path for
+// every field kind, library trigonometry, the five variational columns of D J_b2f carried through every step.
+//
+// Surface kinds (geometry record entry [18]; "surfaces of different concrete types"; U33):
+//   0 PLANE     r = c + loc0 u + loc1 v
+//   1 CYLINDER  axis v through c, radius R = entry [12], azimuth alpha = loc0 / R from n towards u:
+//               r = c + R (cos alpha n + sin alpha u) + loc1 v
+//   2 DISC      the plane through c with normal n in polar coordinates: r = c + loc0 (cos loc1 u + sin loc1 v)
+constexpr int SURF_PLANE = 0, SURF_CYLINDER = 1, SURF_DISC = 2;
+
+template <typename R>
+__device__ __forceinline__ void local_to_global(const R* __restrict__ s, R l0, R l1, R r[3], R e0[3], R e1[3]) {
+  const int kind = (int)s[18];
+  if (kind == SURF_CYLINDER) {
+    const R Rc = s[12];
+    R sa, ca;
+    sincos_lib(l0 / Rc, sa, ca);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      r[i] = s[i] + Rc * (ca * s[9 + i] + sa * s[3 + i]) + l1 * s[6 + i];
+      e0[i] = ca * s[3 + i] - sa * s[9 + i];
+      e1[i] = s[6 + i];
+    }
+  } else if (kind == SURF_DISC) {
+    R sa, ca;
+    sincos_lib(l1, sa, ca);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const R er = ca * s[3 + i] + sa * s[6 + i];
+      r[i] = fma(l0, er, s[i]);
+      e0[i] = er;
+      e1[i] = l0 * (ca * s[6 + i] - sa * s[3 + i]);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      r[i] = fma(l1, s[6 + i], fma(l0, s[3 + i], s[i]));
+      e0[i] = s[3 + i];
+      e1[i] = s[6 + i];
+    }
+  }
+}
+
+// unit normal at the point r of the surface (planes, discs: n; cylinder: the radial direction)
+template <typename R>
+__device__ __forceinline__ void surface_normal(const R* __restrict__ s, const R r[3], R nrm[3]) {
+  if ((int)s[18] == SURF_CYLINDER) {
+    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+    const R z = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+    R dp[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) dp[i] = fma(-z, s[6 + i], d[i]);
+    const R irho = R(1.0) / sqrt(dot(dp, dp));
+#pragma unroll
+    for (int i = 0; i < 3; ++i) nrm[i] = dp[i] * irho;
+  } else {
+    nrm[0] = s[9]; nrm[1] = s[10]; nrm[2] = s[11];
+  }
+}
+
+// local coordinates of the point r on the surface and the rows g0 = dloc0/dr, g1 = dloc1/dr
+template <typename R>
+__device__ __forceinline__ void global_to_local(const R* __restrict__ s, const R r[3], R& l0, R& l1, R g0[3], R g1[3]) {
+  const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+  const int kind = (int)s[18];
+  if (kind == SURF_CYLINDER) {
+    const R Rc = s[12];
+    const R dn = d[0] * s[9] + d[1] * s[10] + d[2] * s[11], du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
+    const R k = Rc / fma(dn, dn, du * du);
+    l0 = Rc * atan2(du, dn);
+    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      g0[i] = k * (dn * s[3 + i] - du * s[9 + i]);
+      g1[i] = s[6 + i];
+    }
+  } else if (kind == SURF_DISC) {
+    const R du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5], dv = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+    const R rho2 = fma(du, du, dv * dv), rho = sqrt(rho2);
+    l0 = rho;
+    l1 = atan2(dv, du);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      g0[i] = (du * s[3 + i] + dv * s[6 + i]) / rho;
+      g1[i] = (du * s[6 + i] - dv * s[3 + i]) / rho2;
+    }
+  } else {
+    l0 = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
+    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { g0[i] = s[3 + i]; g1[i] = s[6 + i]; }
+  }
+}
+
+// Straight-line path length from (r, T) to the surface; false when it cannot be reached.  Planes, discs:
+// n.(c - r)/(n.T) with n.T > 1e-6.  Cylinder: a h^2 + 2 b h + c0 = 0 for the components normal to the axis,
+// root h = -c0 / (b + sqrt(b^2 - a c0)): the crossing ahead of a track inside the cylinder, and the near root in
+// cancellation-free form once the track is within round-off of the surface (U33).
+template <typename R>
+__device__ __forceinline__ bool path_to_surface(const R* __restrict__ s, const R r[3], const R T[3], R& h) {
+  if ((int)s[18] == SURF_CYLINDER) {
+    const R Rc = s[12];
+    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+    const R dz = d[0] * s[6] + d[1] * s[7] + d[2] * s[8], tz = T[0] * s[6] + T[1] * s[7] + T[2] * s[8];
+    R dp[3], tp[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { dp[i] = fma(-dz, s[6 + i], d[i]); tp[i] = fma(-tz, s[6 + i], T[i]); }
+    const R a2 = dot(tp, tp), b = dot(dp, tp), c0 = dot(dp, dp) - Rc * Rc;
+    const R disc = fma(b, b, -a2 * c0);
+    if (!(disc > R(0.0))) return false;
+    const R den = b + sqrt(disc);
+    if (!(den > R(kNdotTMin) * Rc)) return false;
+    h = -c0 / den;
+    return true;
+  }
+  const R nT = T[0] * s[9] + T[1] * s[10] + T[2] * s[11];
+  if (!(nT > R(kNdotTMin))) return false;
+  h = ((s[0] - r[0]) * s[9] + (s[1] - r[1]) * s[10] + (s[2] - r[2]) * s[11]) / nT;
+  return true;
+}
+
+// the five variational columns d(r, T)/d(loc0, loc1, phi, theta, q/p) of D J_b2f and dt/dlam
+template <typename R>
+struct ColJac5T {
+  R dr[5][3], dT[5][3];
+  R sigma;
+};
+
+// One RKN4 step with the five columns carried through its stages (rkn4_step_cols with all columns; GRAD: plus the
+// field-gradient terms lam T_i x (G_i dr_i) in every stage derivative, U32 -- the derivative of the stage
+// arithmetic itself, h held fixed).
+template <int FIELD, bool GRAD, typename R>
+__device__ __forceinline__ void rkn4_step_cols5(const FieldDescT<R>& F, R dtds, R tfac, R r[3], R& t, R T[3], R lam,
+                                                R h, ColJac5T<R>& V, R Blast[3], R& eps, unsigned& status) {
+  const R hh = R(0.5) * h, h6 = h * (R(1.0) / R(6.0)), h26 = h * h6, h28 = R(0.125) * h * h, h22 = R(0.5) * h * h;
+  R B1[3], B2[3], B3[3], G1[9], G2[9], G3[9];
+  R T2[3], T3[3], T4[3], k1[3], k2[3], k3[3], k4[3], l1[3], l2[3], l3[3], l4[3];
+  auto lookup = [&](const R pos[3], R B[3], R G[9]) {
+    if constexpr (GRAD) field_and_gradient_at<FIELD>(F, pos, B, G, status);
+    else field_at<FIELD>(F, pos, B, status);
+  };
+  lookup(r, B1, G1);
+  cross(T, B1, l1);
+  R rm[3], re[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k1[i] = lam * l1[i]; rm[i] = fma(h28, k1[i], fma(hh, T[i], r[i])); T2[i] = fma(hh, k1[i], T[i]); }
+  lookup(rm, B2, G2);
+  cross(T2, B2, l2);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k2[i] = lam * l2[i]; T3[i] = fma(hh, k2[i], T[i]); }
+  cross(T3, B2, l3);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { k3[i] = lam * l3[i]; re[i] = fma(h22, k3[i], fma(h, T[i], r[i])); T4[i] = fma(h, k3[i], T[i]); }
+  lookup(re, B3, G3);
+  cross(T4, B3, l4);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) k4[i] = lam * l4[i];
+  // stage derivative of one column: dk = [q/p: T_i x B_i] + lam (dT_i x B_i + T_i x (G_i dr_i))
+  auto stage = [&](const R Ti[3], const R Bi[3], const R Gi[9], const R li[3], const R dTi[3], const R dri[3], bool qp,
+                   R dk[3]) {
+    R a[3];
+    cross(dTi, Bi, a);
+    if constexpr (GRAD) {
+      R dB[3], c[3];
+#pragma unroll
+      for (int i = 0; i < 3; ++i) dB[i] = fma(Gi[i * 3 + 2], dri[2], fma(Gi[i * 3 + 1], dri[1], Gi[i * 3] * dri[0]));
+      cross(Ti, dB, c);
+#pragma unroll
+      for (int i = 0; i < 3; ++i) a[i] += c[i];
+    }
+#pragma unroll
+    for (int i = 0; i < 3; ++i) dk[i] = qp ? fma(lam, a[i], li[i]) : lam * a[i];
+  };
+#pragma unroll
+  for (int c = 0; c < 5; ++c) {
+    const bool qp = c == 4;
+    R* const dr = V.dr[c];
+    R* const dT = V.dT[c];
+    R d1[3], d2[3], d3[3], d4[3], ds[3], dTs[3];
+    stage(T, B1, G1, l1, dT, dr, qp, d1);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { ds[i] = fma(h28, d1[i], fma(hh, dT[i], dr[i])); dTs[i] = fma(hh, d1[i], dT[i]); }
+    stage(T2, B2, G2, l2, dTs, ds, qp, d2);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) dTs[i] = fma(hh, d2[i], dT[i]);
+    stage(T3, B2, G2, l3, dTs, ds, qp, d3);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { ds[i] = fma(h22, d3[i], fma(h, dT[i], dr[i])); dTs[i] = fma(h, d3[i], dT[i]); }
+    stage(T4, B3, G3, l4, dTs, ds, qp, d4);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      dr[i] = fma(h26, d1[i] + d2[i] + d3[i], fma(h, dT[i], dr[i]));
+      dT[i] = fma(h6, (d1[i] + d4[i]) + R(2.0) * (d2[i] + d3[i]), dT[i]);
+    }
+  }
+  V.sigma = fma(h, tfac, V.sigma);
+  eps = h * h * (fabs(k1[0] - k2[0] - k3[0] + k4[0]) + fabs(k1[1] - k2[1] - k3[1] + k4[1]) +
+                 fabs(k1[2] - k2[2] - k3[2] + k4[2]));
+  R Tn[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r[i] = fma(h26, k1[i] + k2[i] + k3[i], fma(h, T[i], r[i]));
+    Tn[i] = fma(h6, (k1[i] + k4[i]) + R(2.0) * (k2[i] + k3[i]), T[i]);
+  }
+  const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { T[i] = Tn[i] * inrm; Blast[i] = B3[i]; }
+  t = fma(h, dtds, t);
+}
+
+// bound state on surface sf -> bound state on surface st, any kinds (A.1 - A.3 with the surface's own chart, normal and
+// path length).  Same contract as propagate().
+template <int FIELD, bool GRAD, typename R>
+__device__ __forceinline__ unsigned propagate_general(const FieldDescT<R>& F, R mass, int n_corr, R max_step, R step_tol,
+                                                      const R* __restrict__ sf, const R* __restrict__ st, const R x[6],
+                                                      R trig[4], R xo[6], BoundJacobianT<R>& J, R& errmax,
+                                                      unsigned& status) {
+  const R sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
+  R r[3], T[3];
+  ColJac5T<R> D;
+  local_to_global(sf, x[0], x[1], r, D.dr[0], D.dr[1]);
+  T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
+  const R lam = x[4];
+  R t = x[5];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { D.dT[0][i] = D.dT[1][i] = D.dT[4][i] = R(0.0); D.dr[2][i] = D.dr[3][i] = D.dr[4][i] = R(0.0); }
+  D.dT[2][0] = -T[1]; D.dT[2][1] = T[0]; D.dT[2][2] = R(0.0);
+  D.dT[3][0] = cphi * cth; D.dT[3][1] = sphi * cth; D.dT[3][2] = -sth;
+  D.sigma = R(0.0);
+  const R ml = mass * lam;
+  R idtds;
+  const R dtds = sqrt_nr(fma(ml, ml, R(1.0)), idtds);
+  const R tfac = mass * ml * idtds;
+
+  int n_sub = 1;
+  R h;
+  if (!path_to_surface(st, r, T, h)) return ST_PROPAGATION;
+  if (max_step > R(0.0)) {
+    R qn = ceil(fabs(h) / max_step * (R(1.0) - R(1e-12)));
+    if (!(qn >= R(1.0))) qn = R(1.0);
+    if (qn > R(1024.0)) qn = R(1024.0);
+    n_sub = (int)qn;
+  }
+  if (step_tol > R(0.0)) {  // adaptive step count (U31): the estimate of one trial step over the whole leg
+    R rr[3] = {r[0], r[1], r[2]}, TT[3] = {T[0], T[1], T[2]}, tt = t, e0;
+    R A[9], a[3], Bm[9], b[3], tau;
+    rkn4_step<(FIELD == FIELD_CONST ? FIELD_CONST : FIELD_GRID3)>(F, dtds, tfac, rr, tt, TT, lam, h, A, a, Bm, b, tau, e0, status);
+    R qn = ceil(sqrt(sqrt(e0 / step_tol)) * (R(1.0) - R(1e-12)));
+    if (!(qn >= R(1.0))) qn = R(1.0);
+    if (qn > R(1024.0)) qn = R(1024.0);
+    if ((int)qn > n_sub) n_sub = (int)qn;
+  }
+  const int n_steps = n_sub + n_corr;
+  R Bend[3];
+  bool have_Bend = false;
+  for (int is = 0; is < n_steps; ++is) {
+    if (is > 0 && !path_to_surface(st, r, T, h)) return ST_PROPAGATION;
+    if (is < n_sub - 1) h = h / (R)(n_sub - is);
+    R eps;
+    have_Bend = fabs(h) <= short_step<R>();
+    rkn4_step_cols5<FIELD, GRAD>(F, dtds, tfac, r, t, T, lam, h, D, Bend, eps, status);
+    errmax = fmax(errmax, eps);
+    const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
+    if (!(fabs(fin) < big<R>())) return ST_PROPAGATION;
+  }
+
+  // A.3 free -> bound with the path-length correction, w = normal / (normal . T)
+  R nt[3];
+  surface_normal(st, r, nt);
+  const R nT = dot(nt, T);
+  if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+  if (!have_Bend) field_at<FIELD>(F, r, Bend, status);
+  R TxB[3];
+  cross(T, Bend, TxB);
+  const R kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};
+  const R inT = R(1.0) / nT;
+  const R w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
+  const R st2 = fma(T[0], T[0], T[1] * T[1]);
+  if (!(st2 > R(kSinThetaMin) * R(kSinThetaMin))) return ST_THETA;
+  R isth;
+  const R sth2 = sqrt_nr(st2, isth);
+  const R cth2 = T[2];
+  const R cph2 = T[0] * isth, sph2 = T[1] * isth;
+  const R gphi[2] = {-sph2 * isth, cph2 * isth};
+  const R gth[3] = {cph2 * cth2, sph2 * cth2, -sth2};
+  R g0[3], g1[3];
+  global_to_local(st, r, xo[0], xo[1], g0, g1);
+#pragma unroll
+  for (int c = 0; c < 5; ++c) {
+    R* const cr = D.dr[c];
+    R* const cT = D.dT[c];
+    const R wd = dot(w, cr);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { cr[i] = fma(-T[i], wd, cr[i]); cT[i] = fma(-kf_[i], wd, cT[i]); }
+    J.Ja[0][c] = dot(g0, cr);
+    J.Ja[1][c] = dot(g1, cr);
+    J.Ja[2][c] = fma(gphi[0], cT[0], gphi[1] * cT[1]);
+    J.Ja[3][c] = dot(gth, cT);
+    J.Jt[c] = fma(-dtds, wd, c == 4 ? D.sigma : R(0.0));
+  }
+  {
+    const R sdp = fma(sph2, cphi, -cph2 * sphi), cdp = fma(cph2, cphi, sph2 * sphi);
+    const R sdt = fma(sth2, cth, -cth2 * sth), cdt = fma(cth2, cth, sth2 * sth);
+    if (fabs(sdp) <= R(kSmallSine) && cdp > R(0.0) && fabs(sdt) <= R(kSmallSine) && cdt > R(0.0) && fabs(x[2]) <= R(kPi) &&
+        x[3] > R(0.0) && x[3] < R(kPi)) {
+      R ph = x[2] + asin_small(sdp);
+      if (ph > R(kPi)) ph -= R(2.0) * R(kPi);
+      else if (ph <= -R(kPi)) ph += R(2.0) * R(kPi);
+      xo[2] = ph;
+      xo[3] = x[3] + asin_small(sdt);
+    } else {
+      xo[2] = atan2(T[1], T[0]);
+      xo[3] = acos(fmin(fmax(T[2], -R(1.0)), R(1.0)));
+    }
+  }
+  xo[4] = lam;
+  xo[5] = t;
+  trig[0] = sph2; trig[1] = cph2; trig[2] = sth2; trig[3] = cth2;
+  R chk = xo[0] + xo[1] + xo[5];
+#pragma unroll
+  for (int c = 0; c < 5; ++c) chk += J.Ja[0][c] + J.Ja[1][c] + J.Ja[2][c] + J.Ja[3][c] + J.Jt[c];
+  if (!(fabs(chk) < big<R>())) return ST_PROPAGATION;
+  return 0u;
+}
+
 // ---- C- = J C J^T with the structure of J (A.4) -----------------------------------------------------
 template <typename R>
 __device__ __forceinline__ void transport_covariance(const BoundJacobianT<R>& J, const R C[21],
@@ -841,9 +1236,11 @@ template <typename R>
 struct MaterialStepT {
   R lam_out, g, theta0sq_over_sin2, theta0sq;
 };
+// nrm: the unit normal of the surface at the state's position (planes: the record's n = surf + 9)
 template <typename R>
 __device__ __forceinline__ bool material_prepare(const MaterialDescT<R>& Mt, const R* __restrict__ surf,
-                                                 const R trig[4], R lam, MaterialStepT<R>& S) {
+                                                 const R* __restrict__ nrm, const R trig[4], R lam,
+                                                 MaterialStepT<R>& S) {
   const R sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
   const R m = Mt.mass;
   const R al = fabs(lam);
@@ -852,7 +1249,7 @@ __device__ __forceinline__ bool material_prepare(const MaterialDescT<R>& Mt, con
   const R E = sqrt_nr(fma(p, p, m * m), iE);
   const R ib2 = (E * al) * (E * al);  // 1 / beta^2
   const R bg = p * Mt.inv_mass, gamma = E * Mt.inv_mass;
-  const R nT = surf[9] * (cphi * sth) + surf[10] * (sphi * sth) + surf[11] * cth;
+  const R nT = nrm[0] * (cphi * sth) + nrm[1] * (sphi * sth) + nrm[2] * cth;
   const R cfac = rcp_nr(fabs(nT));  // path factor 1/|n.T|
   // Highland: theta0 = 0.0136/(beta p) sqrt(X) (1 + 0.038 ln(X/beta^2)),  1/(beta p) = E lam^2
   const R X = surf[14] * cfac;
@@ -877,6 +1274,20 @@ __device__ __forceinline__ bool material_prepare(const MaterialDescT<R>& Mt, con
   S.theta0sq = t2;
   S.theta0sq_over_sin2 = t2 * rcp_nr(sth * sth);
   return true;
+}
+template <typename R>
+__device__ __forceinline__ bool material_prepare(const MaterialDescT<R>& Mt, const R* __restrict__ surf,
+                                                 const R trig[4], R lam, MaterialStepT<R>& S) {
+  return material_prepare(Mt, surf, surf + 9, trig, lam, S);
+}
+// the same on a surface of any kind: the normal at the state's local position (l0, l1)
+template <typename R>
+__device__ __forceinline__ bool material_prepare_general(const MaterialDescT<R>& Mt, const R* __restrict__ surf, R l0,
+                                                         R l1, const R trig[4], R lam, MaterialStepT<R>& S) {
+  R r[3], e0[3], e1[3], nrm[3];
+  local_to_global(surf, l0, l1, r, e0, e1);
+  surface_normal(surf, r, nrm);
+  return material_prepare(Mt, surf, nrm, trig, lam, S);
 }
 // C <- G C G^T + Q : row/column qp scaled by g, Highland terms on the angle variances
 template <typename R>

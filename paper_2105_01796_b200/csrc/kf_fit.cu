@@ -156,6 +156,13 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
       (op->variant == KF_VARIANT_LANES_PER_TRACK || (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER) ||
        ge->n_surfaces > 1024))
     return KF_ERR_UNSUPPORTED;
+  if (op->field_gradient != 0 && op->field_gradient != 1) return KF_ERR_ARG;
+  if (ge->surface_kinds < 0 || ge->surface_kinds > 7) return KF_ERR_ARG;
+  // the general kernels (surfaces of any kind, field-gradient terms): FP64, thread per track, RTS, staged geometry
+  if (ge->surface_kinds > 1 || (op->field_gradient && fl->kind == KF_FIELD_GRID3))
+    if (op->precision != KF_PRECISION_FP64 || op->variant == KF_VARIANT_LANES_PER_TRACK ||
+        (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER) || ge->n_surfaces > 1024)
+      return KF_ERR_UNSUPPORTED;
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)
     return KF_ERR_ARG;
@@ -340,7 +347,7 @@ kf::FitParams sub_range(const kf::FitParams& F, long long t0, long long n) {
 // sort.perm != nullptr: first the length sort of the range (kf_sort.cuh: zero the bin counters, histogram, scan,
 // scatter), then both kernels go through the slot -> track permutation.
 int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, bool material, int variant,
-                SortPlan sort, cudaStream_t stream) {
+                SortPlan sort, cudaStream_t stream, int mode = 0) {
   kf::FitParams P = P0;
   P.perm = nullptr;
   int rc;
@@ -349,7 +356,7 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
     if (rc != KF_OK) return rc;
     P.perm = sort.perm;
   }
-  const bool lanes = !P.mbf && !P.mixed && (variant == KF_VARIANT_LANES_PER_TRACK ||
+  const bool lanes = mode == 0 && !P.mbf && !P.mixed && (variant == KF_VARIANT_LANES_PER_TRACK ||
                                             (variant == KF_VARIANT_AUTO && P.N <= KF_AUTO_LANES_MAX_TRACKS));
   record_stage(0, stream);
   kfh::ForwardChoice fc{};
@@ -362,9 +369,10 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
   fc.plain = P.n_corr == 2 && P.max_step == 0.0 && P.step_tol == 0.0 && !P.var && !P.rk_err_max &&
              !(P.output_states & (kf::OUT_PRED | kf::OUT_FILT));
   fc.mbf = P.mbf != 0;
+  fc.mode = mode;
   // grid field with the caller's box of the table in shared memory (kf_field.stage_*): thread per track, RTS records,
   // when [geometry][hit slots][box] fit the CTA's shared memory
-  if (grid3 && !lanes && !P.mbf && P.geom_in_smem && P.field.box_n[0] >= 2) {
+  if (mode == 0 && grid3 && !lanes && !P.mbf && P.geom_in_smem && P.field.box_n[0] >= 2) {
     const size_t elem = P.mixed ? sizeof(float) : sizeof(double);
     const size_t box = ((size_t)P.field.box_n[0] * P.field.box_n[1] * P.field.box_n[2] * 3 * elem + 15) / 16 * 16;
     const size_t off = (P.mixed ? kf::geom_smem_bytes<float>(P.n_surfaces) : kf::geom_smem_bytes<double>(P.n_surfaces)) +
@@ -374,7 +382,8 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
       P.field.box_off = P.field_f.box_off = (int)off;
     }
   }
-  if (fc.staged) rc = kfh::launch_forward_staged(P, fc, stream);
+  if (mode != 0) rc = kfh::launch_forward_general(P, fc, stream);
+  else if (fc.staged) rc = kfh::launch_forward_staged(P, fc, stream);
   else if (P.mixed) rc = kfh::launch_forward_mixed(P, fc, stream);
   else if (lanes) rc = kfh::launch_forward_lanes(P, fc, stream);
   else if (grid3) rc = kfh::launch_forward_grid(P, fc, stream);
@@ -386,6 +395,12 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
   // fitted parameters on the perigee surface: one more (small) kernel
   if (rc == KF_OK && G.params) rc = kfh::launch_perigee(P, G, grid3, stream);
   return rc;
+}
+
+// which forward path a call takes: 0 = the plane-only kernels; 1 = surfaces of any kind; 2 = + field-gradient terms
+int general_mode(const kf_geometry* ge, const kf_field* fl, const kf_options* op) {
+  if (op->field_gradient && fl->kind == KF_FIELD_GRID3) return 2;
+  return ge->surface_kinds > 1 ? 1 : 0;
 }
 
 // Does the range [t0, t0 + n) with n_hits hits get the length sort?  ON: yes.  AUTO: when its hit lists are not
@@ -428,7 +443,8 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   if (rc != KF_OK) return rc;
   const int lmax = ge->n_surfaces - 1 - tr->start_surface;
   return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
-                     sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream));
+                     sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream),
+                     general_mode(ge, fl, op));
 }
 
 int kf_field_stage_box(const double* g, int32_t n_surfaces, kf_field* fl) {
@@ -667,7 +683,7 @@ int host_impl(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geomet
     KF_TRY(h2d(a.cov01, ms->cov01, M, m0, nm, 1, D, st), "H2D cov01");
 
     const int frc = enqueue_fit(sub_range(F, t0, n), perigee_params(op, &dout, t0), grid3, op->material != 0, op->variant,
-                                sort_for_range(sort, op, t0, n, (long long)nm, Lmax), st);
+                                sort_for_range(sort, op, t0, n, (long long)nm, Lmax), st, general_mode(ge, fl, op));
     if (frc != KF_OK) return frc;
 
     KF_TRY(d2h(out->first_params, a.first_params, N, t0, n, 6, D, st), "D2H first_params");

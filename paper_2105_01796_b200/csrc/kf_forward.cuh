@@ -31,11 +31,15 @@ namespace kf {
 #ifndef KF_FWD_F32_THREADS_PER_SM
 #define KF_FWD_F32_THREADS_PER_SM 512
 #endif
-template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN, typename R = double>
+// MODE: 0 = planes only, field gradient neglected in the Jacobian (the hot path: propagate()); 1 = surfaces of any kind
+// (kf_geometry.surface_kinds: planes, cylinders, discs); 2 = any kind + the field-gradient terms of the
+// step Jacobian (kf_options.field_gradient).  1 and 2 take propagate_general().
+template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN, typename R = double, int MODE = 0>
 __global__ void __launch_bounds__(BLOCK, (std::is_same<R, float>::value && FIELD == FIELD_CONST) ? KF_FWD_F32_THREADS_PER_SM / BLOCK
                                                                                                 : KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   static_assert(std::is_same<R, double>::value || (LPT == 1 && !MBF && GEOM_SMEM), "the MIXED path: thread per track, RTS records");
+  static_assert(MODE == 0 || (std::is_same<R, double>::value && LPT == 1 && !MBF && GEOM_SMEM), "general surfaces / gradient terms: FP64, thread per track, RTS records");
   const int o_n_corr = PLAIN ? 2 : P.n_corr;
   const R o_max_step = PLAIN ? R(0.0) : (R)P.max_step, o_step_tol = PLAIN ? R(0.0) : (R)P.step_tol;
   const double* const o_var = PLAIN ? nullptr : P.var;
@@ -137,14 +141,18 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     MaterialStepT<R> ms;
     const bool mat_here = MATERIAL && l > 0 && sf[14] > R(0.0);
     if (mat_here) {
-      if (!material_prepare(Md, sf, trig, x[4], ms)) { status |= ST_ENERGY; break; }
+      bool ok_m;
+      if constexpr (MODE == 0) ok_m = material_prepare(Md, sf, trig, x[4], ms);
+      else ok_m = material_prepare_general(Md, sf, x[0], x[1], trig, x[4], ms);
+      if (!ok_m) { status |= ST_ENERGY; break; }
       x[4] = ms.lam_out;
       g_prev = ms.g;
     }
     R xp[6];
     BoundJacobianT<R> J;
-    const unsigned rc = propagate<FIELD>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig,
-                                         xp, J, errmax, status);
+    unsigned rc;
+    if constexpr (MODE == 0) rc = propagate<FIELD>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
+    else rc = propagate_general<FIELD, MODE == 2>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
     if (rc) {
       status |= rc;
       x[4] = lam_filtered;
@@ -272,7 +280,12 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   if (MATERIAL && nleg == n_target && nleg > 0) {  // the last surface's material: status bit only
     const R* __restrict__ sl = G + (P.start + nleg) * 20;
     MaterialStepT<R> ms;
-    if (sl[14] > R(0.0) && !material_prepare(Md, sl, trig, x[4], ms)) status |= ST_ENERGY;
+    if (sl[14] > R(0.0)) {
+      bool ok_m;
+      if constexpr (MODE == 0) ok_m = material_prepare(Md, sl, trig, x[4], ms);
+      else ok_m = material_prepare_general(Md, sl, x[0], x[1], trig, x[4], ms);
+      if (!ok_m) status |= ST_ENERGY;
+    }
   }
   if (!lead) return;
   store6(P.last_params, N, i, x);

@@ -41,6 +41,7 @@ struct ForwardChoice {
   bool plain;     // default stepping, per-surface resolutions, no per-leg PRED/FILT states, no RKN estimate
   bool mbf;       // Bryson-Frazier records
   bool staged;    // grid field with a box of the table in shared memory (FIELD_GRID3S; P.field.box_* set)
+  int mode;       // 0 planes only, gradient neglected; 1 surfaces of any kind; 2 any kind + field-gradient terms
 };
 
 // kf_fwd_const.cu / kf_fwd_grid.cu: FP64, one thread per track
@@ -50,6 +51,8 @@ int launch_forward_grid(const kf::FitParams& P, const ForwardChoice& c, cudaStre
 int launch_forward_staged(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
 // threads per CTA the staged kernels take for a box of `box_bytes` (two 128-thread CTAs per SM while two boxes fit)
 int staged_block(size_t box_bytes);
+// kf_fwd_general.cu: surfaces of any kind and / or the field-gradient terms (c.mode 1, 2), FP64, one thread per track
+int launch_forward_general(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
 // kf_fwd_lanes.cu: FP64, 8 lanes per track
 int launch_forward_lanes(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream);
 // kf_fwd_mixed.cu: float operands and records (kf_options.precision MIXED)

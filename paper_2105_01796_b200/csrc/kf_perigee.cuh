@@ -33,6 +33,8 @@ __device__ __forceinline__ unsigned propagate_to_line(const FieldDesc& F, double
   double r[3], T[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) r[i] = sf[i] + x[0] * sf[3 + i] + x[1] * sf[6 + i];
+  double e0[3] = {sf[3], sf[4], sf[5]}, e1[3] = {sf[6], sf[7], sf[8]};
+  if ((int)sf[18] != SURF_PLANE) local_to_global(sf, x[0], x[1], r, e0, e1);  // first_* on a cylinder or a disc (U33)
   T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
   const double lam = x[4];
   double t = x[5];
@@ -129,11 +131,11 @@ __device__ __forceinline__ unsigned propagate_to_line(const FieldDesc& F, double
     J.Jt[c] = ctime - dtds * wd;
   };
   {
-    double cr[3] = {sf[3], sf[4], sf[5]}, cT[3] = {0.0, 0.0, 0.0};
+    double cr[3] = {e0[0], e0[1], e0[2]}, cT[3] = {0.0, 0.0, 0.0};
     project(0, cr, 0.0, cT);
   }
   {
-    double cr[3] = {sf[6], sf[7], sf[8]}, cT[3] = {0.0, 0.0, 0.0};
+    double cr[3] = {e1[0], e1[1], e1[2]}, cT[3] = {0.0, 0.0, 0.0};
     project(1, cr, 0.0, cT);
   }
   {

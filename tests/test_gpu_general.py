@@ -1,0 +1,160 @@
+"""Parity of the general path of the CUDA library with the oracle: surfaces of any kind (planes, cylinders, discs;
+kf_geometry.surface_kinds, U33) and the field-gradient terms of the transported Jacobian
+(kf_options.field_gradient, U32).  Same bars as everywhere (tests/parity.py)."""
+import dataclasses
+
+import numpy as np
+import pytest
+
+import oracle
+import parity
+import paper_2105_01796_b200 as kf
+from paper_2105_01796_b200 import binding as B
+from paper_2105_01796_b200 import workloads as W
+
+pytestmark = pytest.mark.gpu
+
+Z_AXIS = ((0.0, 0.0, 0.0), (0.0, 0.0, 1.0))
+
+
+def both(wl, states=True, **over):
+    ref = oracle.fit_workload(wl, states=states, **over)
+    got = kf.fit_workload(wl, states=states, **over)
+    return got, ref
+
+
+def in_cfg4_grid(wl):
+    n, origin, spacing, grid = W.cfg4_field_grid()
+    return dataclasses.replace(wl, field_kind="grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+
+
+@pytest.mark.parametrize("kind,n", [("barrel", 5003), ("endcap", 5003), ("barrel", 130), ("endcap", 1)])
+def test_cylinders_and_discs_parity_all_states(kind, n):
+    wl = W.make_tracker(kind, n_tracks=n)
+    got, ref = both(wl, states=True)
+    rep = parity.assert_parity(got, ref, states=True, label=kind)
+    assert np.all(ref.status == 0)
+    assert max(rep.values()) < 0.05, rep
+    np.testing.assert_allclose(got.rk_err_max, ref.rk_err_max, rtol=1e-6, atol=1e-18)
+    if n > 1000:   # the GPU fit's own pulls against the truth on the last cylinder / disc
+        pull = (got.last_params - wl.truth[:, -1, :]) / np.sqrt(np.einsum("nii->ni", got.last_cov))
+        assert np.all(np.abs(pull.std(0) - 1.0) < 0.05)
+        assert abs(got.chi2.mean() - 20.0) < 0.5
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_general_surfaces_options_and_filter_only(kind):
+    wl = W.make_tracker(kind, n_tracks=1501, seed=21)
+    for over in (dict(smooth=0), dict(material=0), dict(max_step_mm=7.0), dict(step_tolerance_mm=1e-7), dict(n_corr_steps=3),
+                 dict(cov_inflation=100.0, outlier_chi2=12.0)):
+        got, ref = both(wl, states=True, **over)
+        loosen = 1.0
+        if "cov_inflation" in over:   # conditioning of the inflated prior: bars from the long-double arbiter
+            ld = oracle.fit_workload(wl, states=True, precision="ld", **over)
+            parity.arbitrated(got, ref, ld, states=True, label=f"{kind} {over}")
+            continue
+        rep = parity.assert_parity(got, ref, states=True, label=f"{kind} {over}", loosen=loosen)
+        assert max(rep.values()) < 0.1, (over, rep)
+
+
+def test_mixed_kinds_in_a_grid_field_with_holes_and_perigee():
+    """plane -> cylinders in the CFG4 table (lookups clamped beyond x = 400 mm... the barrel reaches 300 mm), hits missing
+    on random layers (CSR lists of different lengths, length sort under AUTO), perigee of the smoothed first state."""
+    wl = in_cfg4_grid(W.make_tracker("barrel", n_tracks=9001, seed=33))
+    rng = np.random.default_rng(5)
+    keep = rng.random(wl.n_meas) < 0.9
+    counts = np.add.reduceat(keep.astype(np.int64), wl.offsets[:-1])
+    off = np.zeros(wl.n_tracks + 1, np.int32)
+    np.cumsum(counts, out=off[1:])
+    wl = dataclasses.replace(wl, offsets=off, surf_idx=wl.surf_idx[keep].copy(), loc=wl.loc[keep].copy())
+    for over in (dict(), dict(field_gradient=1)):
+        ref = oracle.fit_workload(wl, states=True, perigee=Z_AXIS, **over)
+        got = kf.fit_workload(wl, states=True, perigee=Z_AXIS, **over)
+        rep = parity.assert_parity(got, ref, states=True, label=f"barrel in grid {over}")
+        assert max(rep.values()) < 0.1, rep
+        assert np.any(got.n_holes > 0)
+
+
+@pytest.mark.parametrize("cfg,n", [(4, 5003), (4, 257)])
+def test_field_gradient_terms_parity(cfg, n):
+    wl = W.make_config(cfg, n_tracks=n)
+    got, ref = both(wl, states=True, field_gradient=1)
+    rep = parity.assert_parity(got, ref, states=True, label="cfg4 with gradient terms")
+    assert max(rep.values()) < 0.05, rep
+    # the terms change the covariances (and through the gain the states), not the bookkeeping
+    plain = kf.fit_workload(wl, states=True)
+    np.testing.assert_array_equal(plain.n_used, got.n_used)
+    np.testing.assert_allclose(plain.pred_params[:, 0, :], got.pred_params[:, 0, :], rtol=1e-12, atol=1e-12)  # first leg: same state
+    assert np.nanmax(np.abs(plain.pred_cov[:, 0] - got.pred_cov[:, 0])) > 0
+    sig = np.sqrt(np.einsum("nii->ni", plain.first_cov))
+    ok = (plain.status & 7) == 0
+    assert 0 < np.max(np.abs(plain.first_params - got.first_params)[ok] / sig[ok]) < 0.05
+
+
+def test_field_gradient_in_a_strongly_non_uniform_table_and_constant_field():
+    wl = W.make_config(4, n_tracks=2001, seed=9)
+    n, origin, spacing, grid = W.cfg4_field_grid()
+    rng = np.random.default_rng(3)
+    grid = grid.copy()
+    grid[..., 0] = 0.3 * rng.standard_normal(grid.shape[:-1])     # node-to-node noise: kinks everywhere
+    grid[..., 1] = 0.3 * rng.standard_normal(grid.shape[:-1])
+    grid[..., 2] *= 1.0 + 0.2 * rng.standard_normal(grid.shape[:-1])
+    wl2 = dataclasses.replace(wl, grid=grid)
+    got, ref = both(wl2, states=True, field_gradient=1)
+    rep = parity.assert_parity(got, ref, states=True, label="noisy table with gradient terms")
+    assert max(rep.values()) < 0.2, rep
+    # constant field: the option is accepted and changes nothing (the plane-only kernels run)
+    wl1 = W.make_config(2, n_tracks=1001)
+    a = kf.fit_workload(wl1, field_gradient=1)
+    b = kf.fit_workload(wl1)
+    for name in ("first_params", "first_cov", "last_cov", "chi2"):
+        np.testing.assert_array_equal(getattr(a, name), getattr(b, name))
+
+
+def test_general_path_through_the_host_entry_points():
+    import torch
+    wl = W.make_tracker("barrel", n_tracks=3001, seed=12)
+    ref = oracle.fit_workload(wl, perigee=Z_AXIS)
+    for kw in (dict(), dict(n_streams=3, chunk_tracks=512)):
+        call = kf.HostCall(kf.HostBatch.from_workload(wl), per_hit=True, perigee=Z_AXIS, **kw)
+        call.run()
+        torch.cuda.synchronize()
+        got = call.to_host()
+        got.rk_err_max = None
+        parity.assert_parity(got, ref, label=f"host barrel {kw}")
+    wl4 = W.make_config(4, n_tracks=2001, seed=13)
+    ref = oracle.fit_workload(wl4, field_gradient=1)
+    call = kf.HostCall(kf.HostBatch.from_workload(wl4), per_hit=True, field_gradient=1)
+    call.run()
+    torch.cuda.synchronize()
+    got = call.to_host()
+    got.rk_err_max = None
+    parity.assert_parity(got, ref, label="host cfg4 gradient")
+
+
+def test_general_path_option_rules():
+    wl = W.make_tracker("endcap", n_tracks=300)
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    for over in (dict(precision=B.PRECISION_MIXED), dict(variant=2), dict(smoother=1)):
+        with pytest.raises(kf.KfError) as e:
+            kf.FitCall(db, **over).run()
+        assert e.value.rc == -2, over
+    with pytest.raises(kf.KfError) as e:
+        kf.FitCall(db, field_gradient=2).run()
+    assert e.value.rc == -1
+    wl4 = W.make_config(4, n_tracks=300)
+    db4 = kf.DeviceBatch(kf.HostBatch.from_workload(wl4))
+    for over in (dict(precision=B.PRECISION_MIXED), dict(variant=2), dict(smoother=1)):
+        with pytest.raises(kf.KfError) as e:
+            kf.FitCall(db4, field_gradient=1, **over).run()
+        assert e.value.rc == -2, over
+    # a small batch under AUTO takes the thread-per-track general kernels (not the lanes variant)
+    kf.FitCall(db).run()
+    assert B.lib().kf_last_launch_count() == 2
+    # a track that cannot reach the next cylinder (moving along the axis): stopped with bit 1, same on both sides
+    wlb = W.make_tracker("barrel", n_tracks=64, seed=3)
+    wlb.params0[5, 3] = 1e-9          # theta -> 0: along z, the cylinder axis
+    wlb.params0[9, 2] = np.pi         # heading back through the start plane: n.T < 0 ... the cylinder is still ahead
+    got, ref = both(wlb, states=False)
+    parity.assert_parity(got, ref, label="degenerate barrel")
+    assert got.status[5] & 1

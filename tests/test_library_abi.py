@@ -35,16 +35,16 @@ def test_struct_sizes_match_the_header_layout():
     # natural C layout of include/kf_fit.h on x86-64 / aarch64 (8-byte pointers and doubles)
     assert C.sizeof(B.KfTracksIn) == 32
     assert C.sizeof(B.KfMeasurements) == 48
-    assert C.sizeof(B.KfGeometry) == 48
+    assert C.sizeof(B.KfGeometry) == 48 + 8   # ... surface_kinds (int32 + padding)
     assert C.sizeof(B.KfField) == 4 + 4 + 24 + 12 + 4 + 24 + 24 + 8 + 12 + 12
-    assert C.sizeof(B.KfOptions) == 56 + 8 + 8 + 48 + 8  # ... perigee line (48), precision (int32 + padding)
+    assert C.sizeof(B.KfOptions) == 56 + 8 + 8 + 48 + 8  # ... perigee line (48), precision + field_gradient (2 x int32)
     assert C.sizeof(B.KfOutputs) == 10 * 8 + 6 * 8 + 3 * 8 + 2 * 8
     assert C.sizeof(B.KfPipeline) == 8 + 8 * 8 + 9 * 8 + 8
 
 
 def test_defaults_and_version():
     L = B.lib()
-    assert L.kf_version() == 107
+    assert L.kf_version() == 108
     o = B.default_options()
     assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort, o.precision) == (1, 0, 2, 0, 0, 0, 0)
     assert o.outlier_chi2 == 0.0 and np.isinf(o.max_step_mm) and o.cov_inflation == 1.0
