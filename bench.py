@@ -50,20 +50,20 @@ REC_BYTES = 55 * 8 + 1
 HIT_BYTES = 2 * 8 + 4
 ALGORITHMIC_FLOP_PER_LEG = dict(source="SURVEY.md 8(d) D.3 (hand count of the method)",
                                 forward={"const": 3450.0, "const_nomat": 3200.0, "grid3": 4000.0}, rts=1650.0 + 170.0)
-EXECUTED_PER_LEG = dict(source="profiles/r01p_ncu_summary.md (opcode table; 262,144 tracks x 30 legs = 7,864,320 legs per launch)",
+EXECUTED_PER_LEG = dict(source="profiles/r02_cfg2_ncu_summary.md (opcode table; 262,144 tracks x 30 legs = 7,864,320 legs per launch)",
                         flop=dict(kf_forward_kernel=(181.7e6 * 2 + 85.0e6 + 24.3e6) * 32 / 7864320,
                                   kf_rts_kernel=(183.7e6 * 2 + 44.6e6 + 14.1e6) * 32 / 7864320),
                         fp64_pipe_instr=dict(kf_forward_kernel=(181.7e6 + 85.0e6 + 24.3e6 + 7.1e6) * 32 / 7864320,
                                              kf_rts_kernel=(183.7e6 + 44.6e6 + 14.1e6 + 3.8e6) * 32 / 7864320),
-                        fp64_pipe_pct_ncu=dict(kf_forward_kernel=63.7, kf_rts_kernel=60.0),
+                        fp64_pipe_pct_ncu=dict(kf_forward_kernel=64.6, kf_rts_kernel=61.4),
                         workload="cfg2 (constant field, material, RTS)")
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x clock)
 # DRAM traffic per leg measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one launch
 # over 262,144 tracks x 30 legs of this workload, divided by the legs), from the committed capture below.
 # bench.py scales it to the launch it times; it is not re-measured live (never time under a profiler).
-NCU_TRAFFIC = dict(source="profiles/r01p_ncu_summary.md",
-                   bytes_per_leg={"kf_forward_kernel": (0.250662e9 + 3.624204e9) / 7864320,
-                                  "kf_rts_kernel": (3.475152e9 + 0.058937e9) / 7864320})
+NCU_TRAFFIC = dict(source="profiles/r02_cfg2_ncu_summary.md",
+                   bytes_per_leg={"kf_forward_kernel": (0.255249e9 + 3.627604e9) / 7864320,
+                                  "kf_rts_kernel": (3.474551e9 + 0.055275e9) / 7864320})
 
 
 def parse_args():
@@ -85,6 +85,20 @@ def parse_args():
     ap.add_argument("--field-stage", action="store_true",
                     help="grid field: pass the shared-memory staging hint (kf_field.stage_*, kf_field_stage_box): the acceptance "
                          "box of the table is kept in shared memory instead of being read through L1/L2 (measured slower on cfg4)")
+    ap.add_argument("--field-gradient", action="store_true",
+                    help="grid field: carry the dB/dr terms in the transported Jacobian (kf_options.field_gradient; the "
+                         "general kernels)")
+    ap.add_argument("--mode", default="batch", choices=["batch", "events", "pcie", "resolution"],
+                    help="batch (default): the bench line, one kf_fit_batch call over the whole workload per step.  "
+                         "events: the same workload cut into --events calls of equal size (event-at-a-time, SURVEY 8(f) #4; "
+                         "BASELINE configs[3]: 100 events x 10,000 tracks), issued round-robin on --streams streams, or all "
+                         "captured once in a CUDA graph (--graph) and replayed; one context line.  pcie: pinned-memory copy "
+                         "rates of this box (H2D alone, D2H alone, both at once): the floor of the e2e number; one context line.  "
+                         "resolution: the MIXED-precision fit against the FP64 fit of the same batch (both through the "
+                         "library): shifts of the fitted parameters in standard deviations, variances, chi2; one context line")
+    ap.add_argument("--events", type=int, default=100)
+    ap.add_argument("--streams", type=int, default=1)
+    ap.add_argument("--graph", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -218,10 +232,187 @@ def run_reference(args):
     return 0
 
 
+def run_events(args):
+    """Event-at-a-time (U20): the workload as --events independent kf_fit_batch calls
+    (resident inputs, one workspace and one output set per stream so that calls on different streams do not share
+    scratch), CUDA events around all of them; --graph: the calls of one step captured once, the graph replayed."""
+    import torch
+    import paper_2105_01796_b200 as kf
+    from paper_2105_01796_b200 import workloads as W
+    dev = torch.device("cuda", 0)
+    wl = W.make_config(args.config, n_tracks=args.tracks)
+    n_ev = args.events
+    per = wl.n_tracks // n_ev
+    assert per > 0
+    S = 1 if args.graph else max(1, args.streams)
+    calls = []
+    for e in range(n_ev):
+        sub = wl.subset(np.arange(e * per, (e + 1) * per))
+        hb = kf.HostBatch.from_workload(sub)
+        db = kf.DeviceBatch(hb, dev)
+        calls.append((db, hb))
+    # one output set + workspace per stream slot (calls on one stream run in order and may share them)
+    outs = [kf.DeviceOutputs(per, max(hb.n_meas for _, hb in calls), calls[0][1].n_legs_max, 0, per_hit=True, rk_err=False,
+                             device=dev) for _ in range(S)]
+    fits = []
+    for e, (db, hb) in enumerate(calls):
+        out = kf.DeviceOutputs(per, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev) if args.graph or S > 1 else outs[0]
+        fits.append(kf.FitCall(db, out=out))
+    streams = [torch.cuda.Stream(dev) for _ in range(S)]
+
+    def issue():
+        for e, f in enumerate(fits):
+            f.run(stream=streams[e % S])
+
+    main_stream = torch.cuda.current_stream(dev)
+
+    def step_plain():
+        for st in streams:
+            st.wait_stream(main_stream)
+        issue()
+        for st in streams:
+            main_stream.wait_stream(st)
+
+    graph = None
+    if args.graph:
+        for _ in range(3):
+            step_plain()
+        torch.cuda.synchronize()
+        graph = torch.cuda.CUDAGraph()
+        cap = torch.cuda.Stream(dev)
+        with torch.cuda.graph(graph, stream=cap):
+            for f in fits:
+                f.run(stream=torch.cuda.current_stream(dev))
+        step = graph.replay
+    else:
+        step = step_plain
+    for _ in range(max(args.warmup, 3)):
+        step()
+    torch.cuda.synchronize()
+    ev = [torch.cuda.Event(enable_timing=True) for _ in range(args.steps + 1)]
+    for k in range(args.steps):
+        ev[k].record()
+        step()
+    ev[args.steps].record()
+    torch.cuda.synchronize()
+    per_step = np.array([ev[k].elapsed_time(ev[k + 1]) for k in range(args.steps)])
+    launches = sum(f.launches for f in fits)
+    print(json.dumps(dict(mode="events", metric=METRIC, unit=UNIT, value=per * n_ev / (per_step.mean() * 1e-3),
+                          ms_per_step=float(per_step.mean()), median_ms=float(np.median(per_step)), steps=args.steps,
+                          config=dict(workload=W.WORKLOAD_NAMES[args.config], events=n_ev, tracks_per_event=per,
+                                      streams=S, cuda_graph=bool(args.graph)),
+                          ms_per_event=float(per_step.mean() / n_ev), gpu_launches=launches * args.steps,
+                          note="context line (event-at-a-time regime), not the bench line")))
+    return 0
+
+
+def run_pcie(args):
+    """Pinned-memory copy rates of this box with plain torch copies of the sizes the e2e call moves (820 MB in, 460 MB
+    out per 1e6-track CFG2 call): each direction alone and both at once on two streams."""
+    import torch
+    dev = torch.device("cuda", 0)
+    n_in, n_out = 820_000_000, 460_000_000
+    h_in = torch.empty(n_in, dtype=torch.uint8).pin_memory()
+    h_out = torch.empty(n_out, dtype=torch.uint8).pin_memory()
+    d_in = torch.empty(n_in, dtype=torch.uint8, device=dev)
+    d_out = torch.empty(n_out, dtype=torch.uint8, device=dev)
+    s1, s2 = torch.cuda.Stream(dev), torch.cuda.Stream(dev)
+
+    def timed(fn, reps=5):
+        fn()
+        torch.cuda.synchronize()
+        t = []
+        for _ in range(reps):
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            fn()
+            e1.record()
+            torch.cuda.synchronize()
+            t.append(e0.elapsed_time(e1))
+        return float(np.median(t))
+
+    def h2d():
+        d_in.copy_(h_in, non_blocking=True)
+
+    def d2h():
+        h_out.copy_(d_out, non_blocking=True)
+
+    def both():
+        cur = torch.cuda.current_stream(dev)
+        s1.wait_stream(cur)
+        s2.wait_stream(cur)
+        with torch.cuda.stream(s1):
+            d_in.copy_(h_in, non_blocking=True)
+        with torch.cuda.stream(s2):
+            h_out.copy_(d_out, non_blocking=True)
+        cur.wait_stream(s1)
+        cur.wait_stream(s2)
+
+    t_in, t_out, t_both = timed(h2d), timed(d2h), timed(both)
+    print(json.dumps(dict(mode="pcie", h2d_bytes=n_in, d2h_bytes=n_out, h2d_ms=t_in, d2h_ms=t_out, both_ms=t_both,
+                          h2d_gbs=n_in / t_in / 1e6, d2h_gbs=n_out / t_out / 1e6,
+                          both_total_gbs=(n_in + n_out) / t_both / 1e6,
+                          note="context line: plain pinned copies, no library call; the e2e number's floor is both_ms")))
+    return 0
+
+
+def run_resolution(args):
+    """PAPER.md:314-318 (float against double): the MIXED fit (float operands and records, 6x6 solve in double) against the
+    FP64 fit of the same batch, both by the library: |dx| / sigma of the fitted parameters (first_* and last_*), relative
+    change of their variances, |dchi2|, discrete decisions that differ; and the time of both."""
+    import torch
+    import paper_2105_01796_b200 as kf
+    from paper_2105_01796_b200 import workloads as W
+    dev = torch.device("cuda", 0)
+    wl = W.make_config(args.config, n_tracks=args.tracks or 200_000)
+    hb = kf.HostBatch.from_workload(wl)
+    db = kf.DeviceBatch(hb, dev)
+    res, ms = {}, {}
+    for name, prec in (("fp64", 0), ("mixed", 1)):
+        call = kf.FitCall(db, precision=prec)
+        for _ in range(3):
+            call.run()
+        torch.cuda.synchronize()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(args.steps):
+            call.run()
+        e1.record()
+        torch.cuda.synchronize()
+        ms[name] = e0.elapsed_time(e1) / args.steps
+        res[name] = call.out.to_host()
+    a, b = res["fp64"], res["mixed"]
+    same = (a.status == b.status) & (a.n_used == b.n_used) & (a.n_outliers == b.n_outliers)
+    ok = same & ((a.status & 7) == 0)
+    out = dict(mode="resolution", config=dict(workload=W.WORKLOAD_NAMES[args.config], tracks=int(wl.n_tracks)),
+               tracks_compared=int(ok.sum()), tracks_with_a_different_decision=int((~same).sum()),
+               ms_fp64=ms["fp64"], ms_mixed=ms["mixed"])
+    names = ["loc0", "loc1", "phi", "theta", "qp", "t"]
+    for nm in ("first", "last"):
+        va = np.einsum("nii->ni", getattr(a, nm + "_cov"))[ok]
+        vb = np.einsum("nii->ni", getattr(b, nm + "_cov"))[ok]
+        d = (getattr(b, nm + "_params") - getattr(a, nm + "_params"))[ok]
+        d[:, 2] = (d[:, 2] + np.pi) % (2 * np.pi) - np.pi
+        z = np.abs(d) / np.sqrt(va)
+        out[nm] = dict(rms_sigma={n_: float(v) for n_, v in zip(names, np.sqrt(np.mean(z ** 2, axis=0)))},
+                       max_sigma={n_: float(v) for n_, v in zip(names, z.max(axis=0))},
+                       max_var_rel=float(np.max(np.abs(vb / va - 1.0))))
+    out["max_abs_dchi2"] = float(np.max(np.abs(a.chi2 - b.chi2)[ok]))
+    out["mean_chi2"] = dict(fp64=float(a.chi2[ok].mean()), mixed=float(b.chi2[ok].mean()))
+    print(json.dumps(out))
+    return 0
+
+
 def main():
     args = parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.mode == "resolution":
+        return run_resolution(args)
+    if args.mode == "events":
+        return run_events(args)
+    if args.mode == "pcie":
+        return run_pcie(args)
 
     import torch
     import paper_2105_01796_b200 as kf
@@ -244,7 +435,7 @@ def main():
     out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False, device=dev)
     mixed = args.precision == "mixed"
     call = kf.FitCall(db, out=out, variant=variant, smoother=int(bf), precision=int(mixed),
-                      field_stage=args.field_stage)
+                      field_stage=args.field_stage, field_gradient=int(args.field_gradient))
     N, M = hb.n_tracks, hb.n_meas
     smooth = bool(hb.options.get("smooth", 1))
 
@@ -422,7 +613,7 @@ def main():
                     material=int(hb.options.get("material", 0)),
                     l2="inputs larger than L2 (RTS workspace %.1f GB per step)" % (n_legs * rec_b / 1e9),
                     parallelism="replicas only" if world > 1 else "1 GPU", variant=args.variant, smoother=args.smoother,
-                    precision=args.precision, field_stage=(fkind == "grid3" and args.field_stage),
+                    precision=args.precision, field_gradient=int(args.field_gradient), field_stage=(fkind == "grid3" and args.field_stage),
                     extra_untimed_warmup_steps=extra_warmup,
                     tracks_not_fitted=bad),
         clocks=clocks, e2e=e2e, gpu_launches=launches, roofline=roofline,

@@ -570,3 +570,44 @@ def test_pipelined_host_entry_point_matches_oracle(n_streams, chunk):
         torch.cuda.synchronize()
         again = call.to_host()
         assert np.array_equal(again.chi2, got.chi2) and np.array_equal(again.first_cov, got.first_cov)
+
+
+def test_cuda_graph_capture_of_the_fit_replays_to_the_same_bits():
+    """kf_fit_batch only enqueues (no allocation, no synchronisation, no host-side state of a fit): a call captured in a
+    CUDA graph replays the whole fit -- length sort, forward, RTS, perigee -- with results identical bit for bit to the
+    direct call, also after the inputs changed in place (the event-at-a-time regime, SURVEY 8(f) #4)."""
+    import torch
+    wl = W.make_config(3, n_tracks=20_001, seed=77)
+    hb = kf.HostBatch.from_workload(wl)
+    db = kf.DeviceBatch(hb)
+    direct = kf.FitCall(db, perigee=Z_AXIS)
+    direct.run()
+    torch.cuda.synchronize()
+    ref = direct.out.to_host()
+    call = kf.FitCall(db, perigee=Z_AXIS)
+    call.run()                       # warm-up outside the capture (one-time attribute calls)
+    torch.cuda.synchronize()
+    for t in (call.out.first_params, call.out.first_cov, call.out.chi2, call.out.perigee_params):
+        t.zero_()
+    graph = torch.cuda.CUDAGraph()
+    with torch.cuda.graph(graph):
+        call.run(stream=torch.cuda.current_stream())
+    torch.cuda.synchronize()
+    assert float(call.out.chi2.abs().sum()) == 0.0        # capture enqueued nothing
+    graph.replay()
+    torch.cuda.synchronize()
+    got = call.out.to_host()
+    for name in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf", "status", "n_used", "n_outliers",
+                 "n_holes", "perigee_params", "perigee_cov"):
+        np.testing.assert_array_equal(getattr(got, name), getattr(ref, name), err_msg=name)
+    # new hits in the same buffers, same graph
+    db.loc += 0.001
+    graph.replay()
+    torch.cuda.synchronize()
+    got2 = call.out.to_host()
+    direct.run()
+    torch.cuda.synchronize()
+    ref2 = direct.out.to_host()
+    assert not np.array_equal(ref2.chi2, ref.chi2)
+    for name in ("first_params", "first_cov", "chi2", "status", "perigee_params"):
+        np.testing.assert_array_equal(getattr(got2, name), getattr(ref2, name), err_msg=name)
