@@ -441,6 +441,49 @@ __device__ __forceinline__ void const_field_step(const R B[3], R b2, R dtds, R t
   }
 }
 
+// The same step to first order in h, for a correction step that starts within kFirstOrderStep of the surface (the second
+// correction step of the default policy: |h| = kappa |n x T| h1^2 / 2 <= 2e-6 mm down to 0.5 GeV).  Every dropped term of
+// const_field_step carries a further factor h or u = h lam: a1 w1 = h^2 lam |B| / 2 <= 1e-10 x 6e-3 / 2 = 3e-13 mm on
+// the position, c2 w2 = u^2 |B|^2 / 2 <= 2e-15 on the direction, <= 1e-13 relative on every entry of the accumulated
+// Jacobian -- below the last digit that survives the sums they enter, three orders inside the parity bars
+// (DESIGN.md "Tolerances").  A step longer than the threshold takes the full form.
+template <typename R> __device__ __forceinline__ constexpr R first_order_step();
+template <> __device__ __forceinline__ constexpr double first_order_step<double>() { return 1.0e-5; }
+template <> __device__ __forceinline__ constexpr float first_order_step<float>() { return 1.0e-3f; }
+
+template <typename R>
+__device__ __forceinline__ void const_field_step_first_order(const R B[3], R b2, R dtds, R tfac, R lam, R h, R r[3],
+                                                             R& t, R T[3], PolyJacT<R>& D) {
+  const R u = h * lam;
+  R w1[3];
+  cross(T, B, w1);
+  R Tn[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r[i] = fma(h, T[i], r[i]);
+    Tn[i] = fma(u, w1[i], T[i]);
+  }
+  const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
+  t = fma(h, dtds, t);
+  // D <- Dstep D with A = h I, Bm = I + u M_B, a = 0, b = h w1
+  R qx[3];
+  cross(D.q, B, qx);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    D.p[i] = fma(h, D.q[i], D.p[i]);
+    D.q[i] += fma(u, qx[i], h * w1[i]);
+  }
+  const R Q1 = D.Q1, Q2 = D.Q2;
+  D.P0 += h;
+  D.P1 = fma(h, Q1, D.P1);
+  D.P2 = fma(h, Q2, D.P2);
+  D.Q1 = (Q1 + u) - b2 * (u * Q2);
+  D.Q2 = fma(u, Q1, Q2);
+  D.sigma = fma(h, tfac, D.sigma);
+}
+
 // 3x3 row-major helpers (general field path)
 template <typename R>
 __device__ __forceinline__ void mat3_mul(const R A[9], const R B[9], R C[9]) {
@@ -580,6 +623,43 @@ __device__ __forceinline__ void rkn4_step_cols(const FieldDescT<R>& F, R dtds, R
   t = fma(h, dtds, t);
 }
 
+// The same step to first order in h (see const_field_step_first_order: a correction step that starts within
+// first_order_step() of the surface): the field is looked up once, at the start point -- over |h| <= 1e-5 mm it changes by
+// less than |grad B| h, which moves T' by <= |lam| |grad B| h^2 <= 6e-3 x 0.2 x 1e-10 = 1e-13 rad for any table of >= 10 mm
+// spacing -- and every term with a further factor h or h lam is dropped (<= 3e-13 mm, <= 1e-13 relative on the columns).
+// The field for the path-length correction is then looked up afresh at the end point (Blast is not set).
+template <int FIELD, typename R>
+__device__ __forceinline__ void rkn4_step_cols_first_order(const FieldDescT<R>& F, R dtds, R tfac, R r[3], R& t, R T[3],
+                                                           R lam, R h, ColJacT<R>& V, unsigned& status) {
+  const R u = h * lam;
+  R B1[3], w1[3];
+  field_at<FIELD>(F, r, B1, status);
+  cross(T, B1, w1);
+#pragma unroll
+  for (int c = 0; c < 3; ++c) {
+    R* const dT = V.dT[c];
+    R* const dr = V.dr[c];
+    R d1[3];
+    cross(dT, B1, d1);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      dr[i] = fma(h, dT[i], dr[i]);
+      dT[i] = fma(u, d1[i], c == 2 ? fma(h, w1[i], dT[i]) : dT[i]);
+    }
+  }
+  V.sigma = fma(h, tfac, V.sigma);
+  R Tn[3];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    r[i] = fma(h, T[i], r[i]);
+    Tn[i] = fma(u, w1[i], T[i]);
+  }
+  const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
+#pragma unroll
+  for (int i = 0; i < 3; ++i) T[i] = Tn[i] * inrm;
+  t = fma(h, dtds, t);
+}
+
 // The bound-to-bound Jacobian, non-trivial part: Ja rows (loc0, loc1, phi, theta) x columns
 // (loc0, loc1, phi, theta, qp); Jt = row t over the same columns.  Row qp = e_qp, column t = e_t.
 template <typename R>
@@ -679,6 +759,7 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
         const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
         const R h = dot(nt, dr) * rcp_nr(nT);
         if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
+        else if (is == 2 && fabs(h) <= first_order_step<R>()) const_field_step_first_order(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D);
         else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
       }
       const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
@@ -697,10 +778,15 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
       if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
       else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
     } else {
-      R eps;
-      have_Bend = fabs(h) <= short_step<R>();  // (of the last step, when the loop ends)
-      rkn4_step_cols<FIELD>(F, dtds, tfac, r, t, T, lam, h, D, Bend, eps, status);
-      errmax = fmax(errmax, eps);
+      if (is >= n_sub && is > 0 && fabs(h) <= first_order_step<R>()) {
+        have_Bend = false;
+        rkn4_step_cols_first_order<FIELD>(F, dtds, tfac, r, t, T, lam, h, D, status);
+      } else {
+        R eps;
+        have_Bend = fabs(h) <= short_step<R>();  // (of the last step, when the loop ends)
+        rkn4_step_cols<FIELD>(F, dtds, tfac, r, t, T, lam, h, D, Bend, eps, status);
+        errmax = fmax(errmax, eps);
+      }
     }
     const R fin = r[0] + r[1] + r[2] + T[0] + T[1] + T[2] + t;
     if (!(fabs(fin) < big<R>())) return ST_PROPAGATION;  // catches NaN and Inf
