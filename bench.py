@@ -51,19 +51,19 @@ HIT_BYTES = 2 * 8 + 4
 ALGORITHMIC_FLOP_PER_LEG = dict(source="SURVEY.md 8(d) D.3 (hand count of the method)",
                                 forward={"const": 3450.0, "const_nomat": 3200.0, "grid3": 4000.0}, rts=1650.0 + 170.0)
 EXECUTED_PER_LEG = dict(source="profiles/r02_cfg2_ncu_summary.md (opcode table; 262,144 tracks x 30 legs = 7,864,320 legs per launch)",
-                        flop=dict(kf_forward_kernel=(181.7e6 * 2 + 85.0e6 + 24.3e6) * 32 / 7864320,
+                        flop=dict(kf_forward_kernel=(172.2e6 * 2 + 78.8e6 + 22.8e6) * 32 / 7864320,
                                   kf_rts_kernel=(183.7e6 * 2 + 44.6e6 + 14.1e6) * 32 / 7864320),
-                        fp64_pipe_instr=dict(kf_forward_kernel=(181.7e6 + 85.0e6 + 24.3e6 + 7.1e6) * 32 / 7864320,
+                        fp64_pipe_instr=dict(kf_forward_kernel=(172.2e6 + 78.8e6 + 22.8e6 + 7.4e6) * 32 / 7864320,
                                              kf_rts_kernel=(183.7e6 + 44.6e6 + 14.1e6 + 3.8e6) * 32 / 7864320),
-                        fp64_pipe_pct_ncu=dict(kf_forward_kernel=64.6, kf_rts_kernel=61.4),
+                        fp64_pipe_pct_ncu=dict(kf_forward_kernel=62.1, kf_rts_kernel=61.4),
                         workload="cfg2 (constant field, material, RTS)")
 FP64_LANES_PER_SM = 64  # FP64 FMA lanes per SM on B200 (148 SMs x 64 x 2 flop x clock)
 # DRAM traffic per leg measured by ncu --set full (dram__bytes_read.sum + dram__bytes_write.sum of one launch
 # over 262,144 tracks x 30 legs of this workload, divided by the legs), from the committed capture below.
 # bench.py scales it to the launch it times; it is not re-measured live (never time under a profiler).
 NCU_TRAFFIC = dict(source="profiles/r02_cfg2_ncu_summary.md",
-                   bytes_per_leg={"kf_forward_kernel": (0.255249e9 + 3.627604e9) / 7864320,
-                                  "kf_rts_kernel": (3.474551e9 + 0.055275e9) / 7864320})
+                   bytes_per_leg={"kf_forward_kernel": (0.256866e9 + 3.625840e9) / 7864320,
+                                  "kf_rts_kernel": (3.474128e9 + 0.054606e9) / 7864320})
 
 
 def parse_args():
