@@ -71,7 +71,9 @@ def parse_args():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json configs index (default 2)")
+    ap.add_argument("--config", type=int, default=2,
+                    help="BASELINE.json configs index (default 2); 5 / 6: the barrel / endcap workloads of the cylinder and "
+                         "disc surface kinds (context, not BASELINE configs)")
     ap.add_argument("--tracks", type=int, default=None, help="override the number of tracks (testing)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--variant", default="auto", choices=["auto", "thread", "lanes"],
@@ -211,7 +213,7 @@ def run_reference(args):
     from paper_2105_01796_b200 import workloads as W
     cores = os.cpu_count() or 1
     n = int(min(args.tracks or 10**9, 1500 * cores, 100_000))
-    wl = W.make_config(args.config, n_tracks=n)
+    wl = W.make_workload(args.config, n_tracks=n)
     for _ in range(max(args.warmup, 1)):
         r = oracle.fit_workload(wl)
     t = time.perf_counter()
@@ -240,7 +242,7 @@ def run_events(args):
     import paper_2105_01796_b200 as kf
     from paper_2105_01796_b200 import workloads as W
     dev = torch.device("cuda", 0)
-    wl = W.make_config(args.config, n_tracks=args.tracks)
+    wl = W.make_workload(args.config, n_tracks=args.tracks)
     n_ev = args.events
     per = wl.n_tracks // n_ev
     assert per > 0
@@ -426,7 +428,7 @@ def main():
     dev = torch.device("cuda", torch.cuda.current_device())
     peaks = load_peaks()
 
-    wl = W.make_config(args.config, n_tracks=args.tracks)
+    wl = W.make_workload(args.config, n_tracks=args.tracks)
     hb = kf.HostBatch.from_workload(wl)
     db = kf.DeviceBatch(hb, dev)
     variant = {"auto": 0, "thread": 1, "lanes": 2}[args.variant]

@@ -668,10 +668,129 @@ struct BoundJacobianT {
   R Jt[5];
 };
 
+// ---- surface kinds (geometry record entry [18]; U33; described at "General surfaces" below) --
+constexpr int SURF_PLANE = 0, SURF_CYLINDER = 1, SURF_DISC = 2;
+
+template <typename R>
+__device__ __forceinline__ void local_to_global(const R* __restrict__ s, R l0, R l1, R r[3], R e0[3], R e1[3]) {
+  const int kind = (int)s[18];
+  if (kind == SURF_CYLINDER) {
+    const R Rc = s[12];
+    R sa, ca;
+    sincos_lib(l0 * rcp_nr(Rc), sa, ca);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      r[i] = s[i] + Rc * (ca * s[9 + i] + sa * s[3 + i]) + l1 * s[6 + i];
+      e0[i] = ca * s[3 + i] - sa * s[9 + i];
+      e1[i] = s[6 + i];
+    }
+  } else if (kind == SURF_DISC) {
+    R sa, ca;
+    sincos_lib(l1, sa, ca);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      const R er = ca * s[3 + i] + sa * s[6 + i];
+      r[i] = fma(l0, er, s[i]);
+      e0[i] = er;
+      e1[i] = l0 * (ca * s[6 + i] - sa * s[3 + i]);
+    }
+  } else {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      r[i] = fma(l1, s[6 + i], fma(l0, s[3 + i], s[i]));
+      e0[i] = s[3 + i];
+      e1[i] = s[6 + i];
+    }
+  }
+}
+
+// unit normal at the point r of the surface (planes, discs: n; cylinder: the radial direction)
+template <typename R>
+__device__ __forceinline__ void surface_normal(const R* __restrict__ s, const R r[3], R nrm[3]) {
+  if ((int)s[18] == SURF_CYLINDER) {
+    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+    const R z = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+    R dp[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) dp[i] = fma(-z, s[6 + i], d[i]);
+    const R irho = rsqrt_nr(dot(dp, dp));
+#pragma unroll
+    for (int i = 0; i < 3; ++i) nrm[i] = dp[i] * irho;
+  } else {
+    nrm[0] = s[9]; nrm[1] = s[10]; nrm[2] = s[11];
+  }
+}
+
+// local coordinates of the point r on the surface and the rows g0 = dloc0/dr, g1 = dloc1/dr
+template <typename R>
+__device__ __forceinline__ void global_to_local(const R* __restrict__ s, const R r[3], R& l0, R& l1, R g0[3], R g1[3]) {
+  const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+  const int kind = (int)s[18];
+  if (kind == SURF_CYLINDER) {
+    const R Rc = s[12];
+    const R dn = d[0] * s[9] + d[1] * s[10] + d[2] * s[11], du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
+    const R k = Rc * rcp_nr(fma(dn, dn, du * du));
+    l0 = Rc * atan2(du, dn);
+    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      g0[i] = k * (dn * s[3 + i] - du * s[9 + i]);
+      g1[i] = s[6 + i];
+    }
+  } else if (kind == SURF_DISC) {
+    const R du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5], dv = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+    const R rho2 = fma(du, du, dv * dv);
+    R irho;
+    const R rho = sqrt_nr(rho2, irho);
+    const R irho2 = irho * irho;
+    l0 = rho;
+    l1 = atan2(dv, du);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) {
+      g0[i] = (du * s[3 + i] + dv * s[6 + i]) * irho;
+      g1[i] = (du * s[6 + i] - dv * s[3 + i]) * irho2;
+    }
+  } else {
+    l0 = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
+    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { g0[i] = s[3 + i]; g1[i] = s[6 + i]; }
+  }
+}
+
+// Straight-line path length from (r, T) to the surface; false when it cannot be reached.  Planes, discs:
+// n.(c - r)/(n.T) with n.T > 1e-6.  Cylinder: a h^2 + 2 b h + c0 = 0 for the components normal to the axis,
+// root h = -c0 / (b + sqrt(b^2 - a c0)): the crossing ahead of a track inside the cylinder, and the near root in
+// cancellation-free form once the track is within round-off of the surface (DESIGN.md U33).
+template <typename R>
+__device__ __forceinline__ bool path_to_surface(const R* __restrict__ s, const R r[3], const R T[3], R& h) {
+  if ((int)s[18] == SURF_CYLINDER) {
+    const R Rc = s[12];
+    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
+    const R dz = d[0] * s[6] + d[1] * s[7] + d[2] * s[8], tz = T[0] * s[6] + T[1] * s[7] + T[2] * s[8];
+    R dp[3], tp[3];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { dp[i] = fma(-dz, s[6 + i], d[i]); tp[i] = fma(-tz, s[6 + i], T[i]); }
+    const R a2 = dot(tp, tp), b = dot(dp, tp), c0 = dot(dp, dp) - Rc * Rc;
+    const R disc = fma(b, b, -a2 * c0);
+    if (!(disc > R(0.0))) return false;
+    const R den = b + sqrt_nr(disc);
+    if (!(den > R(kNdotTMin) * Rc)) return false;
+    h = -c0 * rcp_nr(den);
+    return true;
+  }
+  const R nT = T[0] * s[9] + T[1] * s[10] + T[2] * s[11];
+  if (!(nT > R(kNdotTMin))) return false;
+  h = ((s[0] - r[0]) * s[9] + (s[1] - r[1]) * s[10] + (s[2] - r[2]) * s[11]) * rcp_nr(nT);
+  return true;
+}
+
 // ---- propagate a bound state from surface sf to surface st (A.1 - A.3) ---------------------------
 // trig = (sin phi, cos phi, sin theta, cos theta) of x on entry; on success it holds the values of
 // the predicted (phi, theta), taken from the direction vector itself.  Returns 0 or the stopping bit.
-template <int FIELD, typename R>
+// CURVED: the surfaces may be of any kind (the start surface's chart, the target's path length, normal and chart
+// through local_to_global / path_to_surface / surface_normal / global_to_local); else both are planes.
+template <int FIELD, typename R, bool CURVED = false>
 __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, int n_corr,
                                               R max_step, R step_tol, const R* __restrict__ sf,
                                               const R* __restrict__ st, const R x[6],
@@ -679,9 +798,13 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
                                               R& errmax, unsigned& status) {
   const R sphi = trig[0], cphi = trig[1], sth = trig[2], cth = trig[3];
   // A.1 bound -> free
-  R r[3], T[3];
+  R r[3], T[3], e0[3], e1[3];  // e0, e1 = dr/dloc0, dr/dloc1 on the start surface
+  if constexpr (CURVED) {
+    local_to_global(sf, x[0], x[1], r, e0, e1);
+  } else {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) r[i] = fma(x[1], sf[6 + i], fma(x[0], sf[3 + i], sf[i]));
+    for (int i = 0; i < 3; ++i) { r[i] = fma(x[1], sf[6 + i], fma(x[0], sf[3 + i], sf[i])); e0[i] = sf[3 + i]; e1[i] = sf[6 + i]; }
+  }
   T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
   const R lam = x[4];
   R t = x[5];
@@ -697,10 +820,20 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   // A.2 stepping: n_sub primary steps + n_corr correction steps, no accept/reject
   int n_sub = 1;
   R nT = dot(nt, T);
-  if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+  R h_first = R(0.0);  // CURVED: the first step's path length (also the reachability test)
+  if constexpr (CURVED) {
+    if (!path_to_surface(st, r, T, h_first)) return ST_PROPAGATION;
+  } else {
+    if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+  }
   if (max_step > R(0.0) || step_tol > R(0.0)) {
-    const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-    const R s0 = dot(nt, dr) / nT;
+    R s0;
+    if constexpr (CURVED) {
+      s0 = h_first;
+    } else {
+      const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+      s0 = dot(nt, dr) / nT;
+    }
     if (max_step > R(0.0)) {
       R qn = ceil(fabs(s0) / max_step * (R(1.0) - R(1e-12)));
       if (!(qn >= R(1.0))) qn = R(1.0);
@@ -752,12 +885,18 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
       bool bad = false;
 #pragma unroll
       for (int is = 0; is < 3; ++is) {
-        if (is > 0) {
-          nT = dot(nt, T);
-          bad = bad || !(nT > R(kNdotTMin));
+        R h;
+        if constexpr (CURVED) {
+          h = h_first;
+          if (is > 0) bad = !path_to_surface(st, r, T, h) || bad;
+        } else {
+          if (is > 0) {
+            nT = dot(nt, T);
+            bad = bad || !(nT > R(kNdotTMin));
+          }
+          const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+          h = dot(nt, dr) * rcp_nr(nT);
         }
-        const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-        const R h = dot(nt, dr) * rcp_nr(nT);
         if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
         else if (is == 2 && fabs(h) <= first_order_step<R>()) const_field_step_first_order(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D);
         else const_field_step<false>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
@@ -767,12 +906,18 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
     }
   }
   for (int is = 0; !fast && is < n_steps; ++is) {
-    if (is > 0) {
-      nT = dot(nt, T);
-      if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+    R h;
+    if constexpr (CURVED) {
+      h = h_first;
+      if (is > 0 && !path_to_surface(st, r, T, h)) return ST_PROPAGATION;
+    } else {
+      if (is > 0) {
+        nT = dot(nt, T);
+        if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
+      }
+      const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
+      h = dot(nt, dr) * rcp_nr(nT);
     }
-    const R dr[3] = {ct[0] - r[0], ct[1] - r[1], ct[2] - r[2]};
-    R h = dot(nt, dr) * rcp_nr(nT);
     if (is < n_sub - 1) h = h / (R)(n_sub - is);
     if constexpr (FIELD == FIELD_CONST) {
       if (is == 0) const_field_step<true>(F.b, F.b2, dtds, tfac, lam, h, r, t, T, D, errmax);
@@ -792,8 +937,10 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
     if (!(fabs(fin) < big<R>())) return ST_PROPAGATION;  // catches NaN and Inf
   }
 
-  // A.3 free -> bound with the path-length correction  D~ = (I - f' w^T) D
-  nT = dot(nt, T);
+  // A.3 free -> bound with the path-length correction  D~ = (I - f' w^T) D,  w = normal / (normal . T)
+  R nrm[3] = {nt[0], nt[1], nt[2]};
+  if constexpr (CURVED) surface_normal(st, r, nrm);  // cylinder: the radial direction at the landing point
+  nT = dot(nrm, T);
   if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
   R TxB[3];
   if constexpr (FIELD == FIELD_CONST) {
@@ -805,7 +952,7 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   }
   const R kf_[3] = {lam * TxB[0], lam * TxB[1], lam * TxB[2]};  // dT/ds
   const R inT = rcp_nr(nT);
-  const R w[3] = {nt[0] * inT, nt[1] * inT, nt[2] * inT};
+  const R w[3] = {nrm[0] * inT, nrm[1] * inT, nrm[2] * inT};
 
   const R st2 = fma(T[0], T[0], T[1] * T[1]);
   if (!(st2 > R(kSinThetaMin) * R(kSinThetaMin))) return ST_THETA;
@@ -815,8 +962,15 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   const R cph2 = T[0] * isth, sph2 = T[1] * isth;
   const R gphi[2] = {-sph2 * isth, cph2 * isth};
   const R gth[3] = {cph2 * cth2, sph2 * cth2, -sth2};
+  // rows dloc0/dr, dloc1/dr of the target's chart (planes: u, v) and, CURVED, the local coordinates themselves
   const R* ut = st + 3;
   const R* vt = st + 6;
+  R g0[3], g1[3];
+  if constexpr (CURVED) {
+    global_to_local(st, r, xo[0], xo[1], g0, g1);
+    ut = g0;
+    vt = g1;
+  }
 
   // columns of D J_b2f as (cr, ct_, cT); then c -= f' (w . cr); then rows of J_f2b
   auto project = [&](int c, R cr[3], R ctime, R cT[3]) {
@@ -830,11 +984,11 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
     J.Jt[c] = fma(-dtds, wd, ctime);
   };
   {
-    R cr[3] = {sf[3], sf[4], sf[5]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
+    R cr[3] = {e0[0], e0[1], e0[2]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
     project(0, cr, R(0.0), cT);
   }
   {
-    R cr[3] = {sf[6], sf[7], sf[8]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
+    R cr[3] = {e1[0], e1[1], e1[2]}, cT[3] = {R(0.0), R(0.0), R(0.0)};
     project(1, cr, R(0.0), cT);
   }
   if constexpr (FIELD == FIELD_CONST) {
@@ -864,9 +1018,11 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
     project(4, cr, D.sigma, cT);
   }
 
-  const R dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
-  xo[0] = dot(ut, dr);
-  xo[1] = dot(vt, dr);
+  if constexpr (!CURVED) {
+    const R dr[3] = {r[0] - ct[0], r[1] - ct[1], r[2] - ct[2]};
+    xo[0] = dot(ut, dr);
+    xo[1] = dot(vt, dr);
+  }
   // phi' = atan2(Ty, Tx) and theta' = acos(Tz), taken as the input angle plus the rotation over the leg
   // (sin of the difference from the two direction vectors) whenever that rotation is small
   {
@@ -904,119 +1060,6 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
 //   1 CYLINDER  axis v through c, radius R = entry [12], azimuth alpha = loc0 / R from n towards u:
 //               r = c + R (cos alpha n + sin alpha u) + loc1 v
 //   2 DISC      the plane through c with normal n in polar coordinates: r = c + loc0 (cos loc1 u + sin loc1 v)
-constexpr int SURF_PLANE = 0, SURF_CYLINDER = 1, SURF_DISC = 2;
-
-template <typename R>
-__device__ __forceinline__ void local_to_global(const R* __restrict__ s, R l0, R l1, R r[3], R e0[3], R e1[3]) {
-  const int kind = (int)s[18];
-  if (kind == SURF_CYLINDER) {
-    const R Rc = s[12];
-    R sa, ca;
-    sincos_lib(l0 / Rc, sa, ca);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      r[i] = s[i] + Rc * (ca * s[9 + i] + sa * s[3 + i]) + l1 * s[6 + i];
-      e0[i] = ca * s[3 + i] - sa * s[9 + i];
-      e1[i] = s[6 + i];
-    }
-  } else if (kind == SURF_DISC) {
-    R sa, ca;
-    sincos_lib(l1, sa, ca);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      const R er = ca * s[3 + i] + sa * s[6 + i];
-      r[i] = fma(l0, er, s[i]);
-      e0[i] = er;
-      e1[i] = l0 * (ca * s[6 + i] - sa * s[3 + i]);
-    }
-  } else {
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      r[i] = fma(l1, s[6 + i], fma(l0, s[3 + i], s[i]));
-      e0[i] = s[3 + i];
-      e1[i] = s[6 + i];
-    }
-  }
-}
-
-// unit normal at the point r of the surface (planes, discs: n; cylinder: the radial direction)
-template <typename R>
-__device__ __forceinline__ void surface_normal(const R* __restrict__ s, const R r[3], R nrm[3]) {
-  if ((int)s[18] == SURF_CYLINDER) {
-    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
-    const R z = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
-    R dp[3];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) dp[i] = fma(-z, s[6 + i], d[i]);
-    const R irho = R(1.0) / sqrt(dot(dp, dp));
-#pragma unroll
-    for (int i = 0; i < 3; ++i) nrm[i] = dp[i] * irho;
-  } else {
-    nrm[0] = s[9]; nrm[1] = s[10]; nrm[2] = s[11];
-  }
-}
-
-// local coordinates of the point r on the surface and the rows g0 = dloc0/dr, g1 = dloc1/dr
-template <typename R>
-__device__ __forceinline__ void global_to_local(const R* __restrict__ s, const R r[3], R& l0, R& l1, R g0[3], R g1[3]) {
-  const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
-  const int kind = (int)s[18];
-  if (kind == SURF_CYLINDER) {
-    const R Rc = s[12];
-    const R dn = d[0] * s[9] + d[1] * s[10] + d[2] * s[11], du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
-    const R k = Rc / fma(dn, dn, du * du);
-    l0 = Rc * atan2(du, dn);
-    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      g0[i] = k * (dn * s[3 + i] - du * s[9 + i]);
-      g1[i] = s[6 + i];
-    }
-  } else if (kind == SURF_DISC) {
-    const R du = d[0] * s[3] + d[1] * s[4] + d[2] * s[5], dv = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
-    const R rho2 = fma(du, du, dv * dv), rho = sqrt(rho2);
-    l0 = rho;
-    l1 = atan2(dv, du);
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      g0[i] = (du * s[3 + i] + dv * s[6 + i]) / rho;
-      g1[i] = (du * s[6 + i] - dv * s[3 + i]) / rho2;
-    }
-  } else {
-    l0 = d[0] * s[3] + d[1] * s[4] + d[2] * s[5];
-    l1 = d[0] * s[6] + d[1] * s[7] + d[2] * s[8];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) { g0[i] = s[3 + i]; g1[i] = s[6 + i]; }
-  }
-}
-
-// Straight-line path length from (r, T) to the surface; false when it cannot be reached.  Planes, discs:
-// n.(c - r)/(n.T) with n.T > 1e-6.  Cylinder: a h^2 + 2 b h + c0 = 0 for the components normal to the axis,
-// root h = -c0 / (b + sqrt(b^2 - a c0)): the crossing ahead of a track inside the cylinder, and the near root in
-// cancellation-free form once the track is within round-off of the surface (DESIGN.md U33).
-template <typename R>
-__device__ __forceinline__ bool path_to_surface(const R* __restrict__ s, const R r[3], const R T[3], R& h) {
-  if ((int)s[18] == SURF_CYLINDER) {
-    const R Rc = s[12];
-    const R d[3] = {r[0] - s[0], r[1] - s[1], r[2] - s[2]};
-    const R dz = d[0] * s[6] + d[1] * s[7] + d[2] * s[8], tz = T[0] * s[6] + T[1] * s[7] + T[2] * s[8];
-    R dp[3], tp[3];
-#pragma unroll
-    for (int i = 0; i < 3; ++i) { dp[i] = fma(-dz, s[6 + i], d[i]); tp[i] = fma(-tz, s[6 + i], T[i]); }
-    const R a2 = dot(tp, tp), b = dot(dp, tp), c0 = dot(dp, dp) - Rc * Rc;
-    const R disc = fma(b, b, -a2 * c0);
-    if (!(disc > R(0.0))) return false;
-    const R den = b + sqrt(disc);
-    if (!(den > R(kNdotTMin) * Rc)) return false;
-    h = -c0 / den;
-    return true;
-  }
-  const R nT = T[0] * s[9] + T[1] * s[10] + T[2] * s[11];
-  if (!(nT > R(kNdotTMin))) return false;
-  h = ((s[0] - r[0]) * s[9] + (s[1] - r[1]) * s[10] + (s[2] - r[2]) * s[11]) / nT;
-  return true;
-}
-
 // the five variational columns d(r, T)/d(loc0, loc1, phi, theta, q/p) of D J_b2f and dt/dlam
 template <typename R>
 struct ColJac5T {

@@ -33,7 +33,8 @@ namespace kf {
 #endif
 // MODE: 0 = planes only, field gradient neglected in the Jacobian (the hot path: propagate()); 1 = surfaces of any kind
 // (kf_geometry.surface_kinds: planes, cylinders, discs); 2 = any kind + the field-gradient terms of the
-// step Jacobian (kf_options.field_gradient).  1 and 2 take propagate_general().
+// step Jacobian (kf_options.field_gradient).  1 takes propagate<.., CURVED> (the hot path's closed-form
+// / column steps with the surfaces' own charts), 2 takes propagate_general() (five columns with the gradient terms).
 template <int FIELD, bool MATERIAL, bool GEOM_SMEM, int LPT, int BLOCK, bool MBF, bool PLAIN, typename R = double, int MODE = 0>
 __global__ void __launch_bounds__(BLOCK, (std::is_same<R, float>::value && FIELD == FIELD_CONST) ? KF_FWD_F32_THREADS_PER_SM / BLOCK
                                                                                                 : KF_FWD_MIN_BLOCKS)
@@ -152,7 +153,8 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     BoundJacobianT<R> J;
     unsigned rc;
     if constexpr (MODE == 0) rc = propagate<FIELD>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
-    else rc = propagate_general<FIELD, MODE == 2>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
+    else if constexpr (MODE == 1) rc = propagate<FIELD, R, true>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
+    else rc = propagate_general<FIELD, true>(Fd, Md.mass, o_n_corr, o_max_step, o_step_tol, sf, st, x, trig, xp, J, errmax, status);
     if (rc) {
       status |= rc;
       x[4] = lam_filtered;

@@ -587,4 +587,14 @@ WORKLOAD_NAMES = {
     2: "cfg2 telescope 30 layers with material, filter+RTS, 1e6 tracks",
     3: "cfg3 ragged 100 events x 1e4 tracks, 30 layers material, eff 0.95, 1% outliers, filter+RTS",
     4: "cfg4 field-map 30 layers material, trilinear grid field, acceptance stop, filter+RTS",
+    # not BASELINE.json configs: the two tracker-shaped workloads of the cylinder and disc surface kinds (make_tracker)
+    5: "barrel: start plane + 10 cylinders around z, material, constant field, filter+RTS",
+    6: "endcap: start plane + 10 discs in polar coordinates, material, constant field, filter+RTS",
 }
+
+
+def make_workload(cfg: int, n_tracks: Optional[int] = None, seed: Optional[int] = None) -> Workload:
+    """BASELINE.json configs[cfg] for cfg 0..4; 5 / 6: the barrel / endcap workloads (default 1,000,000 tracks)."""
+    if cfg in (5, 6):
+        return make_tracker("barrel" if cfg == 5 else "endcap", n_tracks=n_tracks or 1_000_000, seed=seed)
+    return make_config(cfg, n_tracks=n_tracks, seed=seed)
