@@ -158,3 +158,110 @@ def test_general_path_option_rules():
     got, ref = both(wlb, states=False)
     parity.assert_parity(got, ref, label="degenerate barrel")
     assert got.status[5] & 1
+
+
+# ---- randomised trackers: mixed kinds, tilted axes, random fields, holes, options -------------------------------------
+def _frame(u, v):
+    u = np.asarray(u, float) / np.linalg.norm(u)
+    v = np.asarray(v, float)
+    v = v - u * (u @ v)
+    v /= np.linalg.norm(v)
+    return u, v, np.cross(u, v)
+
+
+def random_tracker(seed):
+    """Start plane near x = 0, then surfaces of random kinds ordered so that a track along +x meets them in index order:
+    cylinders of growing radius around a slightly tilted, slightly off-origin axis ~ z; planes and discs with normal ~ x
+    at growing x (the disc's centre far off in -y so that rho stays well above zero and alpha away from +-pi)."""
+    rng = np.random.default_rng(7000 + seed)
+    L = int(rng.integers(3, 12))
+    g = np.zeros((L + 1, 20))
+    reach = 0.0
+    for k in range(L + 1):
+        kind = 0 if k == 0 else int(rng.choice([0, 1, 2], p=[0.25, 0.45, 0.3]))
+        reach += rng.uniform(15.0, 40.0) if k else 0.0
+        t1, t2 = rng.uniform(-0.08, 0.08, 2)
+        if kind == 1:      # cylinder: axis ~ z, azimuth zero along ~ x
+            u, v, n = _frame((t1, 1.0, t2), (t2, -t1, 1.0))
+            g[k, 0:3] = (rng.uniform(-1, 1), rng.uniform(-1, 1), rng.uniform(-1, 1))
+            g[k, 12:14] = (reach, 500.0)
+        elif kind == 2:    # disc: normal ~ x, centre displaced along -y: rho ~ 150 mm, alpha ~ +pi/2
+            u, v, n = _frame((t1, 1.0, 0.0), (t2, 0.0, 1.0))
+            g[k, 0:3] = (reach, -150.0 + rng.uniform(-5, 5), rng.uniform(-2, 2))
+            g[k, 12:14] = 300.0
+        else:
+            u, v, n = _frame((t1, 1.0, 0.0), (t2, 0.0, 1.0))
+            g[k, 0:3] = (reach, rng.uniform(-2, 2), rng.uniform(-2, 2))
+            g[k, 12:14] = 50.0
+        g[k, 3:6], g[k, 6:9], g[k, 9:12], g[k, 18] = u, v, n, kind
+        if k and rng.random() < 0.7:
+            g[k, 14] = rng.uniform(5e-4, 1e-2)
+            g[k, 15] = g[k, 14] * 93.7
+        g[k, 16:18] = (rng.uniform(0.005, 0.05) ** 2, (rng.uniform(0.005, 0.05) if kind != 2 else rng.uniform(5e-5, 3e-4)) ** 2)
+    fkind = rng.choice(["const", "grid3"], p=[0.6, 0.4])
+    if fkind == "grid3":
+        n = np.array([int(rng.integers(8, 16)), int(rng.integers(5, 9)), int(rng.integers(5, 9))])
+        origin = np.array([-30.0, -70.0, -70.0])
+        spacing = np.array([(reach + 80.0) / (n[0] - 1), 140.0 / (n[1] - 1), 140.0 / (n[2] - 1)])
+        grid = rng.uniform(-0.2, 0.2, (n[2], n[1], n[0], 3))
+        grid[..., 2] += rng.uniform(1.0, 2.5)
+        field = dict(field_kind="grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+        fld = oracle.make_field("grid3", grid_n=n, grid_origin=origin, grid_spacing=spacing, grid=grid)
+    else:
+        b = tuple(rng.uniform(-0.4, 0.4, 2)) + (rng.choice([-1, 1]) * rng.uniform(0.5, 3.0),)
+        field = dict(field_kind="const", field_b=b)
+        fld = oracle.make_field("const", b)
+    N = int(rng.integers(40, 400))
+    p = np.exp(rng.uniform(np.log(0.6), np.log(40.0), N))
+    x0 = np.stack([rng.uniform(-3, 3, N), rng.uniform(-3, 3, N), rng.uniform(-0.15, 0.15, N),
+                   np.pi / 2 + rng.uniform(-0.15, 0.15, N), rng.choice([-1.0, 1.0], N) / p, rng.uniform(0, 50, N)], axis=1)
+    sig = np.array([0.1, 0.1, 2e-3, 2e-3, 0.0, 300.0])[None, :].repeat(N, 0)
+    sig[:, 4] = 0.03 * np.abs(x0[:, 4])
+    cov0 = np.zeros((N, 6, 6))
+    for a in range(6):
+        cov0[:, a, a] = sig[:, a] ** 2
+    opts = dict(smooth=int(rng.random() < 0.8), material=int(rng.random() < 0.7), outlier_chi2=float(rng.choice([0.0, 15.0])),
+                n_corr_steps=int(rng.integers(1, 4)), max_step_mm=float(rng.choice([np.inf, np.inf, 11.0])),
+                step_tolerance_mm=float(rng.choice([0.0, 0.0, 1e-6])), mass_gev=0.1056583755, cov_inflation=float(rng.choice([1.0, 4.0])),
+                field_gradient=int(fkind == "grid3" and rng.random() < 0.5))
+    opt0 = oracle.make_options()
+    offsets, surf, loc = [0], [], []
+    eff = rng.uniform(0.8, 1.0)
+    for i in range(N):
+        x = x0[i].copy()
+        for k in range(0, L):
+            pr = oracle.propagate(fld, opt0, x, g[k], g[k + 1])     # truth hits: input generation only
+            if pr.rc != 0:
+                break
+            x = pr.x
+            if rng.random() < eff:
+                surf.append(k + 1)
+                loc.append(x[:2] + rng.standard_normal(2) * np.sqrt(g[k + 1, 16:18]))
+        offsets.append(len(surf))
+    params0 = x0 + rng.standard_normal((N, 6)) * sig * 0.7
+    return dict(params0=params0, cov0=cov0, offsets=np.array(offsets, np.int32), surf_idx=np.array(surf, np.int32),
+                loc=np.array(loc).reshape(-1, 2), geom=g, field=field, fld=fld, opts=opts, kinds=sorted(set(g[:, 18].astype(int))))
+
+
+@pytest.mark.parametrize("seed", range(16))
+def test_random_tracker_parity(seed):
+    c = random_tracker(seed)
+    opt = oracle.make_options(**c["opts"])
+    ref = oracle.fit_batch(c["params0"], c["cov0"], 0, c["offsets"], c["surf_idx"], c["loc"], c["geom"], c["fld"], opt, states=True)
+    oracle.perigee_batch(ref, c["geom"], 0, c["fld"], opt, *Z_AXIS)
+    hb = kf.HostBatch.from_arrays(c["params0"], c["cov0"], 0, c["offsets"], c["surf_idx"], c["loc"], c["geom"],
+                                  options=c["opts"], **c["field"])
+    smooth = c["opts"]["smooth"]
+    states = B.STATES_PRED | B.STATES_FILT | (B.STATES_SMOOTH if smooth else 0)
+    for sort in (B.SORT_OFF, B.SORT_ON):
+        out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, states, perigee=True)
+        call = kf.FitCall(kf.DeviceBatch(hb), out=out, perigee=Z_AXIS, length_sort=sort, output_states=states)
+        got = call.run().to_host()
+        label = f"tracker seed {seed} kinds {c['kinds']} sort {sort} opts {c['opts']}"
+        # tracks whose fit ran away (a hit list that stops constraining a low-momentum track) carry no digits
+        with np.errstate(invalid="ignore"):
+            wide = np.nan_to_num(np.einsum("nlii->nli", ref.pred_cov)[..., :2], nan=0.0, posinf=1e99).max(axis=(1, 2)) > 1e4
+        ok = ~wide
+        rep = parity.assert_parity(got, ref, states=True, sel=ok, label=label, offsets=c["offsets"])
+        assert max(rep.values()) < 0.5, (label, rep)
+    assert (ref.status[ok] & 7 == 0).mean() > 0.9
