@@ -14,13 +14,15 @@
  *   "global data shared by different tracks" (geometry, field) are kf_geometry / kf_field.
  *   The exact arithmetic (the paper prints none) is stated in DESIGN.md "The algorithm".
  *
- * All of it runs in hand-written sm_100a CUDA kernels in IEEE double precision.  There is no CPU
+ * All of it runs in hand-written sm_100a CUDA kernels, in IEEE double precision by default (kf_options.precision
+ * MIXED: float operands with the smoother's 6x6 solve in double, the paper's own operating point).  There is no CPU
  * fallback: without a CUDA device every compute entry point returns KF_ERR_CUDA.
  *
  * Conventions
  *   units      mm, GeV, e.  q/p in 1/GeV.  t is c*t in mm (1 ns = 299.792458 mm).  Field in tesla.
  *   bound      x = (loc0, loc1, phi, theta, q/p, t) on a plane with centre c and orthonormal
- *              u, v, n = u x v:  r = c + loc0 u + loc1 v,  T = (cos phi sin theta, sin phi sin theta, cos theta).
+ *              u, v, n = u x v:  r = c + loc0 u + loc1 v,  T = (cos phi sin theta, sin phi sin theta, cos theta);
+ *              on a cylinder or a disc (loc0, loc1) are the chart of that kind (KF_SURFACE_* below).
  *   SoA        per-track arrays are component-major: element (component k, track i) of a
  *              double[K][N] array lives at [k * N + i].
  *   cov        6x6 symmetric, packed upper triangle row-major, 21 values:

@@ -1,4 +1,5 @@
-// kf_device.cuh -- device-side arithmetic of the per-track Kalman fit (sm_100a, IEEE double).
+// kf_device.cuh -- device-side arithmetic of the per-track Kalman fit (sm_100a; templated on the real type R: IEEE
+// double, or float for the MIXED-precision path).
 //
 // One thread owns one track; every matrix below is a fully unrolled register array.  The
 // structure the method guarantees is exploited everywhere:
@@ -533,89 +534,113 @@ __device__ __forceinline__ void rkn4_step_cols(const FieldDescT<R>& F, R dtds, R
                                                R h, ColJacT<R>& V, R Blast[3], R& eps, unsigned& status) {
   const R hh = R(0.5) * h, h6 = h * (R(1.0) / R(6.0)), h26 = h * h6;
   R B1[3], B2[3], B3[3];
-  // state and the q/p column together (the column's inhomogeneous terms are the stage vectors T_i x B_i)
-  R l1[3], l2[3], l3[3], l4[3], k1[3], k2[3], k3[3], k4[3], v[3];
+  // State and the q/p column together (the column's inhomogeneous terms are the stage vectors T_i x B_i).  The stage
+  // slopes are folded into running sums as they appear -- sA = k1 + k2 + k3 (position), sB = k1 + 2 k2 + 2 k3 + k4
+  // (direction), sE = k1 - k2 - k3 + k4 (error estimate), likewise qA, qB for the column -- so that no slope outlives
+  // the next stage (registers: the kernel has none to spare).
   R* const dTq = V.dT[2];
   R* const drq = V.dr[2];
-  R q1[3], q2[3], q3[3], q4[3];
+  R l[3], k[3], q[3], v[3], sA[3], sB[3], sE[3], qA[3], qB[3];
   field_at<FIELD>(F, r, B1, status);
-  cross(T, B1, l1);
-  cross(dTq, B1, q1);
+  cross(T, B1, l);
+  cross(dTq, B1, q);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { k1[i] = lam * l1[i]; q1[i] = fma(lam, q1[i], l1[i]); }
+  for (int i = 0; i < 3; ++i) {
+    k[i] = lam * l[i];
+    q[i] = fma(lam, q[i], l[i]);
+    sA[i] = k[i]; sB[i] = k[i]; sE[i] = k[i];
+    qA[i] = q[i]; qB[i] = q[i];
+  }
   {
     R rm[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) rm[i] = fma(R(0.125) * h * h, k1[i], fma(hh, T[i], r[i]));
+    for (int i = 0; i < 3; ++i) rm[i] = fma(R(0.125) * h * h, k[i], fma(hh, T[i], r[i]));
     field_at<FIELD>(F, rm, B2, status);
   }
+  // stage 2
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k1[i], T[i]);
-  cross(v, B2, l2);
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k[i], T[i]);
+  cross(v, B2, l);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q1[i], dTq[i]);
-  cross(v, B2, q2);
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q[i], dTq[i]);
+  cross(v, B2, q);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { k2[i] = lam * l2[i]; q2[i] = fma(lam, q2[i], l2[i]); }
+  for (int i = 0; i < 3; ++i) {
+    k[i] = lam * l[i];
+    q[i] = fma(lam, q[i], l[i]);
+    sA[i] += k[i]; sB[i] = fma(R(2.0), k[i], sB[i]); sE[i] -= k[i];
+    qA[i] += q[i]; qB[i] = fma(R(2.0), q[i], qB[i]);
+  }
+  // stage 3 (same field point)
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k2[i], T[i]);
-  cross(v, B2, l3);
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, k[i], T[i]);
+  cross(v, B2, l);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q2[i], dTq[i]);
-  cross(v, B2, q3);
+  for (int i = 0; i < 3; ++i) v[i] = fma(hh, q[i], dTq[i]);
+  cross(v, B2, q);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { k3[i] = lam * l3[i]; q3[i] = fma(lam, q3[i], l3[i]); }
+  for (int i = 0; i < 3; ++i) {
+    k[i] = lam * l[i];
+    q[i] = fma(lam, q[i], l[i]);
+    sA[i] += k[i]; sB[i] = fma(R(2.0), k[i], sB[i]); sE[i] -= k[i];
+    qA[i] += q[i]; qB[i] = fma(R(2.0), q[i], qB[i]);
+  }
   {
     R re[3];
 #pragma unroll
-    for (int i = 0; i < 3; ++i) re[i] = fma(R(0.5) * h * h, k3[i], fma(h, T[i], r[i]));
+    for (int i = 0; i < 3; ++i) re[i] = fma(R(0.5) * h * h, k[i], fma(h, T[i], r[i]));
     field_at<FIELD>(F, re, B3, status);
   }
+  // stage 4
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(h, k3[i], T[i]);
-  cross(v, B3, l4);
+  for (int i = 0; i < 3; ++i) v[i] = fma(h, k[i], T[i]);
+  cross(v, B3, l);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) v[i] = fma(h, q3[i], dTq[i]);
-  cross(v, B3, q4);
+  for (int i = 0; i < 3; ++i) v[i] = fma(h, q[i], dTq[i]);
+  cross(v, B3, q);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) { k4[i] = lam * l4[i]; q4[i] = fma(lam, q4[i], l4[i]); }
+  for (int i = 0; i < 3; ++i) {
+    k[i] = lam * l[i];
+    q[i] = fma(lam, q[i], l[i]);
+    sB[i] += k[i]; sE[i] += k[i];
+    qB[i] += q[i];
+  }
   // the phi and theta columns: homogeneous, they need the three field values only
 #pragma unroll
   for (int c = 0; c < 2; ++c) {
     R* const dT = V.dT[c];
     R* const dr = V.dr[c];
-    R d1[3], d2[3], d3[3], d4[3], w[3];
-    cross(dT, B1, d1);
+    R d[3], w[3], dA[3], dB[3];
+    cross(dT, B1, d);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) { d1[i] *= lam; w[i] = fma(hh, d1[i], dT[i]); }
-    cross(w, B2, d2);
+    for (int i = 0; i < 3; ++i) { d[i] *= lam; dA[i] = d[i]; dB[i] = d[i]; w[i] = fma(hh, d[i], dT[i]); }
+    cross(w, B2, d);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) { d2[i] *= lam; w[i] = fma(hh, d2[i], dT[i]); }
-    cross(w, B2, d3);
+    for (int i = 0; i < 3; ++i) { d[i] *= lam; dA[i] += d[i]; dB[i] = fma(R(2.0), d[i], dB[i]); w[i] = fma(hh, d[i], dT[i]); }
+    cross(w, B2, d);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) { d3[i] *= lam; w[i] = fma(h, d3[i], dT[i]); }
-    cross(w, B3, d4);
+    for (int i = 0; i < 3; ++i) { d[i] *= lam; dA[i] += d[i]; dB[i] = fma(R(2.0), d[i], dB[i]); w[i] = fma(h, d[i], dT[i]); }
+    cross(w, B3, d);
 #pragma unroll
     for (int i = 0; i < 3; ++i) {
-      d4[i] *= lam;
-      dr[i] = fma(h26, d1[i] + d2[i] + d3[i], fma(h, dT[i], dr[i]));
-      dT[i] = fma(h6, (d1[i] + d4[i]) + R(2.0) * (d2[i] + d3[i]), dT[i]);
+      dB[i] = fma(lam, d[i], dB[i]);
+      dr[i] = fma(h26, dA[i], fma(h, dT[i], dr[i]));
+      dT[i] = fma(h6, dB[i], dT[i]);
     }
   }
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    drq[i] = fma(h26, q1[i] + q2[i] + q3[i], fma(h, dTq[i], drq[i]));
-    dTq[i] = fma(h6, (q1[i] + q4[i]) + R(2.0) * (q2[i] + q3[i]), dTq[i]);
+    drq[i] = fma(h26, qA[i], fma(h, dTq[i], drq[i]));
+    dTq[i] = fma(h6, qB[i], dTq[i]);
   }
   V.sigma = fma(h, tfac, V.sigma);
-  eps = h * h * (fabs(k1[0] - k2[0] - k3[0] + k4[0]) + fabs(k1[1] - k2[1] - k3[1] + k4[1]) +
-                 fabs(k1[2] - k2[2] - k3[2] + k4[2]));
+  eps = h * h * (fabs(sE[0]) + fabs(sE[1]) + fabs(sE[2]));
   // state
   R Tn[3];
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    r[i] = fma(h26, k1[i] + k2[i] + k3[i], fma(h, T[i], r[i]));
-    Tn[i] = fma(h6, (k1[i] + k4[i]) + R(2.0) * (k2[i] + k3[i]), T[i]);
+    r[i] = fma(h26, sA[i], fma(h, T[i], r[i]));
+    Tn[i] = fma(h6, sB[i], T[i]);
   }
   const R inrm = rsqrt_near_one(fma(Tn[0], Tn[0], fma(Tn[1], Tn[1], Tn[2] * Tn[2])));
 #pragma unroll

@@ -1,7 +1,7 @@
 // kf_fit.cu -- host side of libkf_fit.so: the C ABI declared in include/kf_fit.h.
 //
-// Validates the descriptors, lays out the workspace, and enqueues the sm_100a kernels of
-// kf_kernels.cuh on the caller's stream.  No allocation, no synchronisation, no global state
+// Validates the descriptors, lays out the workspace, decides which kernel family a call takes and enqueues it on the
+// caller's stream through the launchers of kf_host.h (one translation unit per family: kf_fwd_*.cu, kf_bwd.cu).  No allocation, no synchronisation, no global state
 // (apart from thread-local error text / launch counter).  There is no CPU fallback: every compute
 // entry point ends in a kernel launch and reports KF_ERR_CUDA if that fails.
 #include <cuda_runtime.h>

@@ -444,3 +444,21 @@ def test_pg5_cfg4_fit_with_gradient_terms():
     truth_last = wl.truth[np.arange(wl.n_tracks), np.clip(lengths - 1, 0, 29), :]
     pull = ((r1.last_params - truth_last) / np.sqrt(np.einsum("nii->ni", r1.last_cov)))[ok]
     assert np.all(np.abs(pull[:, :5].std(0) - 1.0) < 0.06)
+
+
+def test_tracker_workloads_are_seeded_and_well_formed():
+    """the two generators behind PS7 and the GPU parity tests: deterministic, CSR-consistent, hits on every layer,
+    kinds as documented, truth on the surfaces (radius / z of the chart)"""
+    for cfg, kind, k in ((5, "barrel", 1.0), (6, "endcap", 2.0)):
+        a, b = W.make_workload(cfg, n_tracks=300), W.make_tracker(kind, n_tracks=300)
+        for name in ("params0", "cov0", "offsets", "surf_idx", "loc", "geometry", "truth"):
+            np.testing.assert_array_equal(getattr(a, name), getattr(b, name), err_msg=name)
+        assert a.offsets[0] == 0 and a.offsets[-1] == a.n_meas and np.all(np.diff(a.offsets) == 10)
+        assert np.all(a.geometry[1:, 18] == k) and a.geometry[0, 18] == 0
+        assert np.all(np.diff(a.surf_idx.reshape(300, 10), axis=1) == 1)
+        if kind == "barrel":    # loc0 = R alpha: |alpha| < 0.5 rad for tracks within +-0.3 rad of the x axis
+            R = a.geometry[1:, 12]
+            assert np.all(np.abs(a.truth[:, :, 0] / R[None, :]) < 0.6)
+        else:                   # loc0 = rho > 0, loc1 = alpha in (-pi, pi)
+            assert np.all(a.truth[:, :, 0] > 0) and np.all(np.abs(a.truth[:, :, 1]) < np.pi)
+    assert W.make_workload(1, n_tracks=10).name == "cfg1"
