@@ -188,8 +188,8 @@ typedef struct kf_geometry {
   int32_t surface_kinds;   /* bit k set = the table holds surfaces of kind k (the table itself is DEVICE memory, which
                               the host-side dispatch does not read).  0 or 1 = planes only: entry [18] is then ignored
                               and the plane-only kernels run.  Any other value selects the general-surface kernels:
-                              FP64, one thread per track, RTS smoother, at most 1024 surfaces
-                              (KF_ERR_UNSUPPORTED with MIXED precision, KF_VARIANT_LANES_PER_TRACK or Bryson-Frazier) */
+                              one thread per track, RTS smoother, at most 1024 surfaces, FP64 or MIXED precision
+                              (KF_ERR_UNSUPPORTED with KF_VARIANT_LANES_PER_TRACK or Bryson-Frazier) */
 } kf_geometry;
 
 /* global data: magnetic field -- PAPER.md:170 (constant 3x1 vector; inhomogeneous fields need
@@ -247,8 +247,8 @@ typedef struct kf_options {
                              G = gradient of the trilinear interpolant.  The states do not change, the covariances do
                              (CFG4: up to a few per cent of a standard deviation on the fitted parameters).  0 (default):
                              neglected (reading U4).  No effect in a constant field.  Runs in the general kernels (FP64,
-                             thread per track, RTS; KF_ERR_UNSUPPORTED otherwise); the perigee extrapolation neglects the
-                             terms either way */
+                             thread per track, RTS; KF_ERR_UNSUPPORTED with MIXED precision, the lanes variant or
+                             Bryson-Frazier); the perigee extrapolation neglects the terms either way */
 } kf_options;
 
 /* (4) results -- PAPER.md:180: status, track states, fitted parameters */

@@ -158,10 +158,12 @@ int validate(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometr
     return KF_ERR_UNSUPPORTED;
   if (op->field_gradient != 0 && op->field_gradient != 1) return KF_ERR_ARG;
   if (ge->surface_kinds < 0 || ge->surface_kinds > 7) return KF_ERR_ARG;
-  // the general kernels (surfaces of any kind, field-gradient terms): FP64, thread per track, RTS, staged geometry
+  // the general kernels (surfaces of any kind, field-gradient terms): thread per track, RTS, staged geometry; the
+  // field-gradient terms in FP64 only
   if (ge->surface_kinds > 1 || (op->field_gradient && fl->kind == KF_FIELD_GRID3))
-    if (op->precision != KF_PRECISION_FP64 || op->variant == KF_VARIANT_LANES_PER_TRACK ||
-        (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER) || ge->n_surfaces > 1024)
+    if (op->variant == KF_VARIANT_LANES_PER_TRACK || (op->smooth && op->smoother == KF_SMOOTHER_BRYSON_FRAZIER) ||
+        ge->n_surfaces > 1024 ||
+        (op->precision != KF_PRECISION_FP64 && op->field_gradient && fl->kind == KF_FIELD_GRID3))
       return KF_ERR_UNSUPPORTED;
   if (op->variant != KF_VARIANT_AUTO && op->variant != KF_VARIANT_THREAD_PER_TRACK &&
       op->variant != KF_VARIANT_LANES_PER_TRACK)

@@ -40,7 +40,8 @@ __global__ void __launch_bounds__(BLOCK, (std::is_same<R, float>::value && FIELD
                                                                                                 : KF_FWD_MIN_BLOCKS)
 kf_forward_kernel(const __grid_constant__ FitParams P) {
   static_assert(std::is_same<R, double>::value || (LPT == 1 && !MBF && GEOM_SMEM), "the MIXED path: thread per track, RTS records");
-  static_assert(MODE == 0 || (std::is_same<R, double>::value && LPT == 1 && !MBF && GEOM_SMEM), "general surfaces / gradient terms: FP64, thread per track, RTS records");
+  static_assert(MODE == 0 || (LPT == 1 && !MBF && GEOM_SMEM), "general surfaces / gradient terms: thread per track, RTS records");
+  static_assert(MODE != 2 || std::is_same<R, double>::value, "the field-gradient terms: FP64");
   const int o_n_corr = PLAIN ? 2 : P.n_corr;
   const R o_max_step = PLAIN ? R(0.0) : (R)P.max_step, o_step_tol = PLAIN ? R(0.0) : (R)P.step_tol;
   const double* const o_var = PLAIN ? nullptr : P.var;

@@ -8,16 +8,18 @@
 namespace kfh {
 
 namespace {
-template <int FIELD, bool MATERIAL, int MODE, int BLOCK, bool PLAIN>
+template <int FIELD, bool MATERIAL, int MODE, int BLOCK, bool PLAIN, typename R = double>
 int go(const kf::FitParams& P, cudaStream_t stream) {
-  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, double, MODE>, P, BLOCK,
-                kf::geom_smem_bytes<double>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK), stream,
+  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, R, MODE>, P, BLOCK,
+                kf::geom_smem_bytes<R>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK), stream,
                 MODE == 2 ? "kf_forward_kernel (general surfaces, field-gradient terms)" : "kf_forward_kernel (general surfaces)");
 }
 // MODE 1 follows the plane-only kernels' choices: 256-thread CTAs for large constant-field batches, PLAIN when the call
 // asks for nothing optional
 template <int FIELD, bool MATERIAL>
 int pick1(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream) {
+  if (P.mixed)   // MIXED precision (float operands and records): the 128-thread CTA, the general instantiation
+    return go<FIELD, MATERIAL, 1, KF_FWD_BLOCK_SMALL, false, float>(P, stream);
   if (FIELD == kf::FIELD_CONST && c.big)
     return c.plain ? go<FIELD, MATERIAL, 1, KF_FWD_BLOCK, true>(P, stream) : go<FIELD, MATERIAL, 1, KF_FWD_BLOCK, false>(P, stream);
   return c.plain ? go<FIELD, MATERIAL, 1, KF_FWD_BLOCK_SMALL, true>(P, stream) : go<FIELD, MATERIAL, 1, KF_FWD_BLOCK_SMALL, false>(P, stream);

@@ -135,7 +135,7 @@ def test_general_path_through_the_host_entry_points():
 def test_general_path_option_rules():
     wl = W.make_tracker("endcap", n_tracks=300)
     db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
-    for over in (dict(precision=B.PRECISION_MIXED), dict(variant=2), dict(smoother=1)):
+    for over in (dict(variant=2), dict(smoother=1)):
         with pytest.raises(kf.KfError) as e:
             kf.FitCall(db, **over).run()
         assert e.value.rc == -2, over
@@ -265,3 +265,62 @@ def test_random_tracker_parity(seed):
         rep = parity.assert_parity(got, ref, states=True, sel=ok, label=label, offsets=c["offsets"])
         assert max(rep.values()) < 0.5, (label, rep)
     assert (ref.status[ok] & 7 == 0).mean() > 0.9
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_cylinders_and_discs_in_mixed_precision(kind):
+    """kf_options.precision = MIXED on surfaces of other kinds: against the float build of the oracle and the double oracle,
+    with the bars of tests/test_gpu_mixed.py (sigma units; widened only as far as the float oracle itself is from the
+    double fit)."""
+    import test_gpu_mixed as TM
+    wl = W.make_tracker(kind, n_tracks=5003, seed=5)
+    ref64 = oracle.fit_workload(wl, states=True)
+    ref32 = oracle.fit_workload(wl, states=True, precision="f32")
+    got = kf.fit_workload(wl, states=True, precision=B.PRECISION_MIXED)
+    assert B.lib().kf_last_launch_count() == 2
+    a, b, o = TM.check(got, ref64, ref32, wl.offsets, label=kind)
+
+    def per_leg(x):   # worst |dx| / sigma and worst relative change of a variance over all per-leg states, against the double fit
+        wp, wv = 0.0, 0.0
+        for nm in ("pred", "filt", "smooth"):
+            d = getattr(x, nm + "_params") - getattr(ref64, nm + "_params")
+            d[..., 2] = (d[..., 2] + np.pi) % (2 * np.pi) - np.pi
+            va = np.einsum("nlii->nli", getattr(ref64, nm + "_cov"))
+            wp = max(wp, float(np.nanmax(np.abs(d) / np.sqrt(va))))
+            wv = max(wv, float(np.nanmax(np.abs(np.einsum("nlii->nli", getattr(x, nm + "_cov")) / va - 1.0))))
+        return wp, wv
+
+    (gp, gv), (op_, ov) = per_leg(got), per_leg(ref32)
+    # the same rule as TM.check: the fixed bars, widened only as far as twice the float ORACLE's own distance from the double
+    # fit (the polar chart of a disc divides by rho: its alpha variance is the most sensitive entry)
+    assert gp < max(0.05, 2.0 * op_) and gv < max(1e-3, 2.0 * ov), (gp, gv, op_, ov)
+    np.testing.assert_array_equal(got.first_cov, got.first_cov.astype(np.float32).astype(np.float64))
+    pull = (got.last_params - wl.truth[:, -1, :]) / np.sqrt(np.einsum("nii->ni", got.last_cov))
+    assert np.all(np.abs(pull.std(0) - 1.0) < 0.05)
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_tracker_workloads_at_a_million_tracks(kind):
+    """the launch configuration `bench.py --config 5|6` times: sampled tracks re-fitted by the oracle, properties on all"""
+    import torch
+    wl = W.make_tracker(kind, n_tracks=1_000_000)
+    db = kf.DeviceBatch(kf.HostBatch.from_workload(wl))
+    hb = db.host
+    out = kf.DeviceOutputs(hb.n_tracks, hb.n_meas, hb.n_legs_max, 0, per_hit=True, rk_err=False)
+    call = kf.FitCall(db, out=out)
+    call.run()
+    torch.cuda.synchronize()
+    assert call.launches == 2
+    got = call.out.to_host()
+    rng = np.random.default_rng(8)
+    idx = np.unique(np.concatenate([rng.choice(wl.n_tracks, 2000, replace=False), np.arange(40), np.arange(wl.n_tracks - 40, wl.n_tracks)]))
+    ref = oracle.fit_workload(wl.subset(idx))
+    from types import SimpleNamespace
+    g = SimpleNamespace(**{k: getattr(got, k)[idx] for k in ("first_params", "first_cov", "last_params", "last_cov", "chi2", "ndf",
+                                                             "status", "n_used", "n_outliers", "n_holes")}, hit_flags=None, hit_chi2=None)
+    ref.hit_flags = ref.hit_chi2 = None
+    parity.assert_parity(g, ref, label=kind + " 1e6")
+    assert np.all(got.status == 0) and np.all(got.n_used == 10)
+    assert abs(got.chi2.mean() - 20.0) < 4 * np.sqrt(40.0 / wl.n_tracks)
+    pull = (got.last_params - wl.truth[:, -1, :]) / np.sqrt(np.einsum("nii->ni", got.last_cov))
+    assert np.all(np.abs(pull[:, :5].mean(0)) < 0.01) and np.all(np.abs(pull[:, :5].std(0) - 1.0) < 0.01)
