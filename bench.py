@@ -101,6 +101,8 @@ def parse_args():
     ap.add_argument("--events", type=int, default=100)
     ap.add_argument("--streams", type=int, default=1)
     ap.add_argument("--graph", action="store_true")
+    ap.add_argument("--e2e-chunk", type=int, default=65536, help="tracks per chunk of the pipelined host call (e2e)")
+    ap.add_argument("--e2e-streams", type=int, default=3, help="streams of the pipelined host call (e2e)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     return ap.parse_args()
@@ -511,13 +513,13 @@ def main():
             h1.record()
             barrier()
             return replicas.max_over_ranks(h0.elapsed_time(h1), dist, dev) / ke, ke
-        # the public host-buffer call: chunks of 65,536 tracks over 3 streams (H2D, fit and D2H of different chunks overlap)
-        hc = kf.HostCall(hb, dev, n_streams=3, chunk_tracks=65536, smoother=int(bf), precision=int(mixed),
+        # the public host-buffer call: chunks of whole CTAs over a few streams (H2D, fit and D2H of different chunks overlap)
+        hc = kf.HostCall(hb, dev, n_streams=args.e2e_streams, chunk_tracks=args.e2e_chunk, smoother=int(bf), precision=int(mixed),
                          field_stage=args.field_stage)
         ms_e2e, ke = time_host(hc)
         e2e = dict(value=world * N / (ms_e2e * 1e-3), unit=UNIT, h2d_bytes_per_step=int(hc.h2d_bytes),
                    d2h_bytes_per_step=int(hc.d2h_bytes), ms_per_step=ms_e2e, steps=ke, launches_per_step=int(hc.launches),
-                   api="kf_fit_batch_host_pipelined (pinned host buffers; chunks of 65536 tracks on 3 streams: "
+                   api=f"kf_fit_batch_host_pipelined (pinned host buffers; chunks of {args.e2e_chunk} tracks on {args.e2e_streams} streams: "
                        "H2D, forward, RTS, D2H per chunk)")
         del hc
         hc = kf.HostCall(hb, dev, smoother=int(bf), precision=int(mixed), field_stage=args.field_stage)  # context: the same through kf_fit_batch_host, everything in order on one stream
