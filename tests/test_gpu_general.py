@@ -243,7 +243,7 @@ def random_tracker(seed):
                 loc=np.array(loc).reshape(-1, 2), geom=g, field=field, fld=fld, opts=opts, kinds=sorted(set(g[:, 18].astype(int))))
 
 
-@pytest.mark.parametrize("seed", range(16))
+@pytest.mark.parametrize("seed", range(int(__import__("os").environ.get("KF_TRACKER_SEEDS", "16"))))
 def test_random_tracker_parity(seed):
     c = random_tracker(seed)
     opt = oracle.make_options(**c["opts"])
