@@ -1,5 +1,5 @@
 // kf_common.cuh -- what the two global kernels of the fit share: record layout, parameter block, small device helpers.
-// (kf_forward.cuh: kf_forward_kernel; kf_rts.cuh: kf_rts_kernel, kf_rts_lanes_kernel; kf_kernels.cuh includes all three.)
+// (kf_forward.cuh: kf_forward_kernel; kf_rts.cuh: kf_rts_kernel, kf_rts_lanes_kernel.)
 //
 //   kf_forward_kernel : one thread = one track.  Kalman step loop of PAPER.md:55-60: propagate
 //                       (RKN4 + free-Jacobian transport), C- = J C J^T, gain-matrix
