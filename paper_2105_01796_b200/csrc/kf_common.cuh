@@ -145,7 +145,11 @@ __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commi
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
 // bytes of the forward kernel's hit staging area: two alternating slots of (loc0, loc1, surface) per thread
-constexpr size_t hit_stage_bytes(int block) { return (size_t)block * (2 * 2 * sizeof(double) + 2 * sizeof(int)); }
+__host__ __device__ constexpr size_t hit_stage_bytes(int block) { return (size_t)block * (2 * 2 * sizeof(double) + 2 * sizeof(int)); }
+
+// bytes of the grid-field kernels' parking area for the covariance (kf_forward.cuh): 21 values per thread behind the hit slots
+template <typename R>
+__host__ __device__ constexpr size_t cov_park_bytes(int block) { return (size_t)block * 21 * sizeof(R); }
 
 template <> __device__ __forceinline__ const FieldDescT<double>& field_of<double>(const FitParams& P) { return P.field; }
 template <> __device__ __forceinline__ const FieldDescT<float>& field_of<float>(const FitParams& P) { return P.field_f; }

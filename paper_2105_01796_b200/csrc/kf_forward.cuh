@@ -120,6 +120,24 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   };
   if (o0 < o1) fetch_hit(o0, 0);
 
+  // Grid field, thread per track: the covariance is dead weight while the propagation runs (255 registers, spills): it is
+  // parked in a shared-memory column of the thread between the gain update of one leg and the covariance transport of the
+  // next ([21][BLOCK] values behind the hit slots; conflict-free).
+  constexpr bool kParkC = FIELD == FIELD_GRID3 && LPT == 1 && MODE != 2 && std::is_same<R, double>::value;
+  R* const s_C = reinterpret_cast<R*>(reinterpret_cast<unsigned char*>(s_dyn) + hit_stage_bytes(BLOCK)) + threadIdx.x;
+  auto park_C = [&]() {
+    if constexpr (kParkC) {
+#pragma unroll
+      for (int k = 0; k < 21; ++k) s_C[k * BLOCK] = C[k];
+    }
+  };
+  auto fetch_C = [&]() {
+    if constexpr (kParkC) {
+#pragma unroll
+      for (int k = 0; k < 21; ++k) C[k] = s_C[k * BLOCK];
+    }
+  };
+  park_C();
   R chi2 = R(0.0), errmax = R(0.0);
   int n_used = 0, n_outl = 0, n_holes = 0, nleg = 0, hp = o0;
   R trig[4];
@@ -186,6 +204,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       KF_REC_STORE(&RF[(kRecFt - kRecFa + 4) * KF_TILE], J.Jt[4] * g_prev);
       KF_REC_STORE(&RF[(kRecG - kRecFa) * KF_TILE], g_prev);
     }
+    fetch_C();
     if (mat_here) material_apply(ms, C);
     R Cp[21];
     if constexpr (LPT == 1) transport_covariance(J, C, Cp);
@@ -233,7 +252,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       R c2 = R(0.0);
       if (!gain_prepare(xp, Cp, m0, m1, v00, v01, v11, gn, c2)) {
         status |= ST_NOT_POSITIVE;
-        if (mat_here) material_undo(ms, C);
+        if (mat_here && !kParkC) material_undo(ms, C);   // (parked: the column still holds C before the layer)
         x[4] = lam_filtered;
         break;
       }
@@ -261,6 +280,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
       KF_REC_STORE(&Rk[(kMbfGain + 4) * KF_TILE], gn.i11);
     }
     gain_apply(gn, xp, Cp, x, C);
+    park_C();
     // trig holds the angles of x-: rotate by the gain's correction (zero for a hole)
     rotate_trig(trig, x[2], x[2] - xp[2], x[3], x[3] - xp[3]);
     if (P.smooth && !MBF && lead) tile_flag[(size_t)l * P.leg_stride] = flag;
@@ -292,6 +312,7 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
   }
   if (!lead) return;
   store6(P.last_params, N, i, x);
+  fetch_C();
   store21(P.last_cov, N, i, C);
   if (nleg == 0) {
     store6(P.first_params, N, i, x);

@@ -12,9 +12,9 @@ int go(const kf::FitParams& P, cudaStream_t stream) {
   const char* nm = "kf_forward_kernel (grid field)";
   if (P.geom_in_smem)
     return launch(kf::kf_forward_kernel<kf::FIELD_GRID3, MATERIAL, true, 1, BLOCK, MBF, PLAIN>, P, BLOCK,
-                  kf::geom_smem_bytes<double>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK), stream, nm);
+                  kf::geom_smem_bytes<double>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK) + kf::cov_park_bytes<double>(BLOCK), stream, nm);
   return launch(kf::kf_forward_kernel<kf::FIELD_GRID3, MATERIAL, false, 1, BLOCK, MBF, false>, P, BLOCK,
-                kf::hit_stage_bytes(BLOCK), stream, nm);
+                kf::hit_stage_bytes(BLOCK) + kf::cov_park_bytes<double>(BLOCK), stream, nm);
 }
 template <bool MATERIAL, bool MBF>
 int pick(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream) {
