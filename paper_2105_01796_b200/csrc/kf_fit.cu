@@ -46,6 +46,24 @@ bool raise_smem_limit(const void* kernel, size_t smem, const char* name) {
   seen.push_back(Entry{kernel, dev, smem});
   return true;
 }
+bool prefer_carveout(const void* kernel, int percent, const char* name) {
+  struct Entry { const void* fn; int dev; int pct; };
+  static std::mutex mu;
+  static std::vector<Entry> seen;
+  int dev = 0;
+  if (set_cuda_error(cudaGetDevice(&dev), name)) return false;
+  std::lock_guard<std::mutex> lock(mu);
+  for (Entry& e : seen)
+    if (e.fn == kernel && e.dev == dev) {
+      if (e.pct == percent) return true;
+      if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, percent), name)) return false;
+      e.pct = percent;
+      return true;
+    }
+  if (set_cuda_error(cudaFuncSetAttribute(kernel, cudaFuncAttributePreferredSharedMemoryCarveout, percent), name)) return false;
+  seen.push_back(Entry{kernel, dev, percent});
+  return true;
+}
 }  // namespace kfh
 
 namespace {

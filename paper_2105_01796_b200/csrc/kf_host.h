@@ -20,12 +20,16 @@ extern thread_local int g_launches;
 bool set_cuda_error(cudaError_t e, const char* where);  // true when e is an error (text kept)
 // cudaFuncAttributeMaxDynamicSharedMemorySize is a property of (device, kernel): raised once, not per launch
 bool raise_smem_limit(const void* kernel, size_t smem, const char* name);
+// cudaFuncAttributePreferredSharedMemoryCarveout (per cent of the SM's 256 KB unified L1 / shared memory), set once per
+// (device, kernel): a kernel that gathers from a table through L1 asks for no more shared memory than its CTAs use
+bool prefer_carveout(const void* kernel, int percent, const char* name);
 
 // one launch over the tracks of P: thread per track (block tracks per CTA) or lanes per track (block / lanes)
 template <typename K>
 int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_t stream, const char* name,
-           int lanes_per_track = 1) {
+           int lanes_per_track = 1, int carveout_pct = -1) {
   if (smem > 48 * 1024 && !raise_smem_limit(reinterpret_cast<const void*>(kernel), smem, name)) return KF_ERR_CUDA;
+  if (carveout_pct >= 0 && !prefer_carveout(reinterpret_cast<const void*>(kernel), carveout_pct, name)) return KF_ERR_CUDA;
   const unsigned grid = (unsigned)((P.N * lanes_per_track + block - 1) / block);
   kernel<<<grid, block, smem, stream>>>(P);
   if (set_cuda_error(cudaGetLastError(), name)) return KF_ERR_CUDA;
