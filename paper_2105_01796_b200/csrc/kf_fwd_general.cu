@@ -10,10 +10,12 @@ namespace kfh {
 namespace {
 template <int FIELD, bool MATERIAL, int MODE, int BLOCK, bool PLAIN, typename R = double>
 int go(const kf::FitParams& P, cudaStream_t stream) {
-  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, R, MODE>, P, BLOCK,
-                kf::geom_smem_bytes<R>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK) +
-                    (FIELD == kf::FIELD_GRID3 && MODE == 1 && sizeof(R) == 8 ? kf::cov_park_bytes<double>(BLOCK) : 0), stream,
-                MODE == 2 ? "kf_forward_kernel (general surfaces, field-gradient terms)" : "kf_forward_kernel (general surfaces)");
+  const size_t smem = kf::geom_smem_bytes<R>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK) +
+                      (FIELD == kf::FIELD_GRID3 && MODE == 1 && sizeof(R) == 8 ? kf::cov_park_bytes<double>(BLOCK) : 0);
+  const int pct = FIELD == kf::FIELD_GRID3 ? carveout_for(smem, 256 / BLOCK) : -1;   // grid field: the rest of the SM to L1
+  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, R, MODE>, P, BLOCK, smem, stream,
+                MODE == 2 ? "kf_forward_kernel (general surfaces, field-gradient terms)" : "kf_forward_kernel (general surfaces)",
+                1, pct);
 }
 // MODE 1 follows the plane-only kernels' choices: 256-thread CTAs for large constant-field batches, PLAIN when the call
 // asks for nothing optional

@@ -1,7 +1,5 @@
 // kf_fwd_grid.cu -- kf_forward_kernel instantiations for a 3-D grid field (trilinear), FP64, one thread per track.
 // Always KF_FWD_BLOCK_SMALL threads per CTA (measured: the 256-thread CTA is slower for this kernel).
-#include <algorithm>
-
 #include "kf_host.h"
 #include "kf_forward.cuh"
 
@@ -16,7 +14,7 @@ int go(const kf::FitParams& P, cudaStream_t stream) {
     // the table is gathered through L1: ask for just the shared memory two resident CTAs use (+ 1 KB each that the
     // system reserves), leaving the rest of the SM's 256 KB to L1 (CFG4 forward 1.256 -> 1.224 ms per 262,144 tracks)
     const size_t smem = kf::geom_smem_bytes<double>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK) + kf::cov_park_bytes<double>(BLOCK);
-    const int pct = (int)std::min<size_t>(100, (2 * (smem + 1024) * 100 + 256 * 1024 - 1) / (256 * 1024));
+    const int pct = carveout_for(smem, 2);
     return launch(kf::kf_forward_kernel<kf::FIELD_GRID3, MATERIAL, true, 1, BLOCK, MBF, PLAIN>, P, BLOCK, smem, stream, nm, 1, pct);
   }
   return launch(kf::kf_forward_kernel<kf::FIELD_GRID3, MATERIAL, false, 1, BLOCK, MBF, false>, P, BLOCK,

@@ -9,9 +9,12 @@ namespace kfh {
 namespace {
 template <int FIELD, bool MATERIAL, int BLOCK, bool PLAIN>
 int go(const kf::FitParams& P, cudaStream_t stream) {
-  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK,
-                kf::geom_smem_bytes<float>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK), stream,
-                "kf_forward_kernel (mixed precision)");
+  const size_t smem = kf::geom_smem_bytes<float>(P.n_surfaces) + kf::hit_stage_bytes(BLOCK);
+  // grid field: the table is gathered through L1 -- leave it all the SM's memory the resident CTAs do not use
+  // (224-236 registers: 256 threads per SM)
+  const int pct = FIELD == kf::FIELD_GRID3 ? carveout_for(smem, 256 / BLOCK) : -1;
+  return launch(kf::kf_forward_kernel<FIELD, MATERIAL, true, 1, BLOCK, false, PLAIN, float>, P, BLOCK, smem, stream,
+                "kf_forward_kernel (mixed precision)", 1, pct);
 }
 template <int FIELD, bool MATERIAL>
 int pick(const kf::FitParams& P, const ForwardChoice& c, cudaStream_t stream) {

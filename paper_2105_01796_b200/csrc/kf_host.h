@@ -37,6 +37,14 @@ int launch(K kernel, const kf::FitParams& P, int block, size_t smem, cudaStream_
   return KF_OK;
 }
 
+// carve-out (per cent of the SM's 256 KB) that `ctas` resident CTAs of `smem` dynamic bytes (+ 1 KB each reserved by the
+// system) need: what the kernels that gather the field table through L1 ask for, leaving the rest to L1
+inline int carveout_for(size_t smem, int ctas) {
+  const size_t need = (size_t)ctas * (smem + 1024);
+  const size_t pct = (need * 100 + 256 * 1024 - 1) / (256 * 1024);
+  return (int)(pct > 100 ? 100 : pct);
+}
+
 // which forward-kernel instantiation a call takes (decided in kf_fit.cu: enqueue_fit)
 struct ForwardChoice {
   bool grid3;     // field kind
