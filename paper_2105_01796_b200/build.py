@@ -95,4 +95,7 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
 
 
 if __name__ == "__main__":
-    print(build_library(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    # python build.py [--force] [-v] [-DNAME=VALUE ...]   (-D flags go to nvcc: the tuning macros KF_FWD_BLOCK,
+    # KF_FWD_BLOCK_SMALL, KF_FWD_MIN_BLOCKS, KF_RTS_MIN_BLOCKS, KF_TILE, ... of csrc/kf_common.cuh)
+    defines = [a for a in sys.argv[1:] if a.startswith("-D")]
+    print(build_library(force="--force" in sys.argv or bool(defines), verbose="-v" in sys.argv, extra_flags=defines))
