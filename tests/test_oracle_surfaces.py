@@ -10,6 +10,7 @@ give the same answer, statistics of a whole fit.  CPU only.
   PS5  a disc is the plane in polar coordinates: states and Jacobians related by the polar chart
   PS6  material on a cylinder = material on the tangent plane at the same point
   PS7  whole fits on the barrel and endcap workloads: noiseless recovery, chi2 = 2n, unit pulls
+  PS8  KF + RTS == dense global least squares on both workloads (P7 with the cylinder / disc charts)
   PG1  gradient of the trilinear interpolant: exact on a field linear in r, finite differences inside a cell, zero
        along clamped axes
   PG2  8x8 step Jacobian with the gradient terms against finite differences of the step in a non-uniform field;
@@ -462,3 +463,22 @@ def test_tracker_workloads_are_seeded_and_well_formed():
         else:                   # loc0 = rho > 0, loc1 = alpha in (-pi, pi)
             assert np.all(a.truth[:, :, 0] > 0) and np.all(np.abs(a.truth[:, :, 1]) < np.pi)
     assert W.make_workload(1, n_tracks=10).name == "cfg1"
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_ps8_kf_rts_equals_global_least_squares_on_cylinders_and_discs(kind):
+    """P7 on the other surface kinds: the smoothed states of the recursive fit are the solution of the dense linear
+    least-squares problem over (x_0, scattering angles per layer) built from the same step functions and Jacobians --
+    the update and smoother algebra, F = J G and the process-noise placement with the cylinder / disc charts."""
+    import test_oracle_fit as TF
+    wl = W.make_tracker(kind, n_tracks=10, n_layers=8)
+    r = oracle.fit_workload(wl, states=True)
+    assert np.all(r.status == 0)
+    floors = np.array([1.0, 1.0, 0.1, 1.0, 0.01, 1.0])
+    for i in range(wl.n_tracks):
+        xs_, Cs_ = TF._global_lsq(wl, i, r, True)
+        dx = np.abs(r.smooth_params[i] - xs_) / np.maximum(np.abs(xs_), floors)
+        assert dx.max() < 1e-9, dx.max()
+        sd = np.sqrt(np.einsum("kii->ki", Cs_))
+        dC = np.abs(r.smooth_cov[i] - Cs_) / (sd[:, :, None] * sd[:, None, :])
+        assert dC.max() < 1e-7, dC.max()
