@@ -482,3 +482,27 @@ def test_ps8_kf_rts_equals_global_least_squares_on_cylinders_and_discs(kind):
         sd = np.sqrt(np.einsum("kii->ki", Cs_))
         dC = np.abs(r.smooth_cov[i] - Cs_) / (sd[:, :, None] * sd[:, None, :])
         assert dC.max() < 1e-7, dC.max()
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_ps9_covariance_invariants_on_cylinders_and_discs(kind):
+    """P8 on the other kinds: symmetric positive definite covariances, filtered <= predicted (rank <= 2 update),
+    smoothed <= filtered, last smoothed = last filtered."""
+    wl = W.make_tracker(kind, n_tracks=300)
+    r = oracle.fit_workload(wl, states=True)
+    assert np.all(r.status == 0)
+    diag = lambda C: np.einsum("...ii->...i", C)
+    for i in range(wl.n_tracks):
+        Cp, Cf, Cs = r.pred_cov[i], r.filt_cov[i], r.smooth_cov[i]
+        for C in (Cp, Cf, Cs):
+            assert np.array_equal(C, np.swapaxes(C, 1, 2))
+            s = np.sqrt(diag(C))
+            assert np.linalg.eigvalsh(C / (s[:, :, None] * s[:, None, :])).min() > 0
+        s = np.sqrt(diag(Cp))
+        d1 = (Cp - Cf) / (s[:, :, None] * s[:, None, :])
+        assert np.linalg.eigvalsh(d1).min() > -1e-10
+        assert np.all(np.sum(np.linalg.eigvalsh(d1) > 1e-9, axis=1) <= 2)
+        s = np.sqrt(diag(Cf))
+        assert np.linalg.eigvalsh((Cf - Cs) / (s[:, :, None] * s[:, None, :])).min() > -1e-9
+        assert np.array_equal(r.smooth_params[i, -1], r.filt_params[i, -1])
+    assert np.all(r.ndf == 2 * r.n_used - 5)
