@@ -168,8 +168,8 @@ typedef struct kf_measurements {
  *             reached along the track's direction of motion from inside (navigation outwards)
  *   DISC      the plane through c with normal n in polar coordinates: r = c + loc0 (cos loc1 u + sin loc1 v),
  *             loc0 = rho > 0, loc1 = alpha in (-pi, pi]
- * A measurement and the prediction it is compared with must lie on the same branch of an angular coordinate (the
- * residual is not wrapped). */
+ * The angular coordinates are periodic (R alpha: 2 pi R; alpha: 2 pi): a hit is taken on the branch nearest the
+ * prediction before the update. */
 enum { KF_SURFACE_PLANE = 0, KF_SURFACE_CYLINDER = 1, KF_SURFACE_DISC = 2 };
 
 /* global data: detector geometry -- PAPER.md:168, 174, 182 (boundless planes), 136-138 (other kinds).

@@ -1023,7 +1023,19 @@ int32_t kfo_fit_batch(int64_t N, const double* params0, const double* cov0, int3
             V[0] = st[16]; V[3] = st[17]; V[1] = V[2] = 0.0;
           }
           real c2 = 0.0, xf[6], Cf[36];
-          const real m[2] = {(real)loc[(size_t)hp * 2 + 0], (real)loc[(size_t)hp * 2 + 1]};
+          real m[2] = {(real)loc[(size_t)hp * 2 + 0], (real)loc[(size_t)hp * 2 + 1]};
+          /* angular local coordinates (reading U33): the hit is taken on the branch nearest the prediction -- the arc
+             length R alpha of a cylinder has period 2 pi R, the azimuth of a disc 2 pi.  A residual already inside
+             (-P/2, P/2] leaves the hit untouched. */
+          {
+            const int kind = surf_kind(st);
+            const int a = kind == SURF_CYLINDER ? 0 : 1;
+            const real period = kind == SURF_CYLINDER ? 2.0 * PI * st[12] : (kind == SURF_DISC ? 2.0 * PI : 0.0);
+            if (period > 0.0) {
+              const real d = m[a] - R->xp[a];
+              if (d > 0.5 * period || d <= -0.5 * period) m[a] = m[a] - period * ceil((d - 0.5 * period) / period);
+            }
+          }
           rc = update_r(R->xp, R->Cp, m, V, xf, Cf, &c2);
           if (rc) { status |= (uint32_t)rc; break; }
           if (opt->outlier_chi2 > 0.0 && c2 > opt->outlier_chi2) { /* reading U9: strictly greater */

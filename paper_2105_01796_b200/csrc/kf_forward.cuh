@@ -213,8 +213,20 @@ kf_forward_kernel(const __grid_constant__ FitParams P) {
     // hit of this surface, if any (fetched during the previous leg); start fetching the one after it
     cp_async_wait_all();
     const bool has_hit = hp < o1 && s_hs[slot * BLOCK] == s;
-    const R m0 = has_hit ? (R)s_hm[(slot * 2 + 0) * BLOCK] : R(0.0);
-    const R m1 = has_hit ? (R)s_hm[(slot * 2 + 1) * BLOCK] : R(0.0);
+    R m0 = has_hit ? (R)s_hm[(slot * 2 + 0) * BLOCK] : R(0.0);
+    R m1 = has_hit ? (R)s_hm[(slot * 2 + 1) * BLOCK] : R(0.0);
+    if constexpr (MODE != 0) {
+      // angular local coordinates (U33): the hit is taken on the branch nearest the prediction (period 2 pi R for
+      // the arc length on a cylinder, 2 pi for the azimuth on a disc); the record keeps the hit as used, so the RTS kernel's
+      // re-filtering sees the same residual
+      const int kind = (int)st[18];
+      if (has_hit && kind != SURF_PLANE) {
+        const R period = kind == SURF_CYLINDER ? R(2.0) * R(kPi) * st[12] : R(2.0) * R(kPi);
+        R& m = kind == SURF_CYLINDER ? m0 : m1;
+        const R d = m - (kind == SURF_CYLINDER ? xp[0] : xp[1]);
+        if (d > R(0.5) * period || d <= -R(0.5) * period) m = m - period * ceil((d - R(0.5) * period) / period);
+      }
+    }
     if (has_hit && hp + 1 < o1) fetch_hit(hp + 1, slot ^ 1);
 
     if (P.smooth && lead) {

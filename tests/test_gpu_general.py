@@ -324,3 +324,25 @@ def test_tracker_workloads_at_a_million_tracks(kind):
     assert abs(got.chi2.mean() - 20.0) < 4 * np.sqrt(40.0 / wl.n_tracks)
     pull = (got.last_params - wl.truth[:, -1, :]) / np.sqrt(np.einsum("nii->ni", got.last_cov))
     assert np.all(np.abs(pull[:, :5].mean(0)) < 0.01) and np.all(np.abs(pull[:, :5].std(0) - 1.0) < 0.01)
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_hits_across_the_branch_cut_of_an_angular_coordinate(kind):
+    """U33: a hit is taken on the branch of its periodic coordinate nearest the prediction, in the forward kernel and -- through
+    the record, which keeps the hit as used -- in the RTS kernel's re-filtering.  The chart turned by pi (tracks cross at
+    alpha ~ +-pi) with a third of the hits given a whole period off, against the oracle and against the original chart."""
+    from test_oracle_surfaces import across_the_branch_cut
+    wl = W.make_tracker(kind, n_tracks=3001, seed=17)
+    wl2 = across_the_branch_cut(wl, kind)
+    ang = 0 if kind == "barrel" else 1
+    shift = (2 * np.pi * wl.geometry[wl2.surf_idx, 12]) if kind == "barrel" else np.full(wl2.n_meas, 2 * np.pi)
+    wl2.loc[::3, ang] += shift[::3]
+    wl2.loc[1::7, ang] -= 2 * shift[1::7]
+    got, ref = both(wl2, states=True)
+    rep = parity.assert_parity(got, ref, states=True, label=kind + " across the cut")
+    assert max(rep.values()) < 0.1, rep
+    assert np.all(got.status == 0) and np.all(got.n_used == 10)
+    base = kf.fit_workload(wl, states=True)
+    np.testing.assert_allclose(got.chi2, base.chi2, rtol=1e-8, atol=1e-8)
+    other = [k for k in range(6) if k != ang]
+    np.testing.assert_allclose(got.first_params[:, other], base.first_params[:, other], rtol=1e-8, atol=1e-9)

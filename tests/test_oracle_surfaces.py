@@ -11,6 +11,8 @@ give the same answer, statistics of a whole fit.  CPU only.
   PS6  material on a cylinder = material on the tangent plane at the same point
   PS7  whole fits on the barrel and endcap workloads: noiseless recovery, chi2 = 2n, unit pulls
   PS8  KF + RTS == dense global least squares on both workloads (P7 with the cylinder / disc charts)
+  PS9  covariance invariants on both workloads (P8)
+  PS10 periodic local coordinates: the chart turned by pi and hits whole periods off give the original fit
   PG1  gradient of the trilinear interpolant: exact on a field linear in r, finite differences inside a cell, zero
        along clamped axes
   PG2  8x8 step Jacobian with the gradient terms against finite differences of the step in a non-uniform field;
@@ -506,3 +508,58 @@ def test_ps9_covariance_invariants_on_cylinders_and_discs(kind):
         assert np.linalg.eigvalsh((Cf - Cs) / (s[:, :, None] * s[:, None, :])).min() > -1e-9
         assert np.array_equal(r.smooth_params[i, -1], r.filt_params[i, -1])
     assert np.all(r.ndf == 2 * r.n_used - 5)
+
+
+def across_the_branch_cut(wl, kind):
+    """The same detector with the angular chart of every cylinder / disc turned by pi about its axis / normal (u -> -u,
+    and n -> -n on a cylinder, v -> -v on a disc): the same surfaces in space, but the tracks, which cross at alpha ~ 0 in
+    the original chart, now cross at alpha ~ +-pi, where a hit and its prediction can lie on opposite sides of the cut."""
+    import dataclasses
+    g = wl.geometry.copy()
+    loc = wl.loc.copy()
+    wrap = lambda a: a - 2 * np.pi * np.ceil((a - np.pi) / (2 * np.pi))
+    if kind == "barrel":
+        g[1:, 3:6] *= -1.0
+        g[1:, 9:12] *= -1.0
+        R = g[wl.surf_idx, 12]
+        loc[:, 0] = R * wrap(loc[:, 0] / R + np.pi)
+    else:
+        g[1:, 3:6] *= -1.0
+        g[1:, 6:9] *= -1.0
+        loc[:, 1] = wrap(loc[:, 1] + np.pi)
+    return dataclasses.replace(wl, geometry=g, loc=loc)
+
+
+@pytest.mark.parametrize("kind", ["barrel", "endcap"])
+def test_ps10_hits_are_taken_on_the_branch_nearest_the_prediction(kind):
+    """U33: angular local coordinates are periodic (2 pi R on a cylinder, 2 pi on a disc).  A fit across the branch cut
+    gives the fit of the original chart: same chi2, same parameters, the angular coordinate shifted by half a period."""
+    wl = W.make_tracker(kind, n_tracks=400, seed=17)
+    wl2 = across_the_branch_cut(wl, kind)
+    a, b = oracle.fit_workload(wl, states=True), oracle.fit_workload(wl2, states=True)
+    assert np.all(a.status == 0) and np.all(b.status == 0)
+    ang = 0 if kind == "barrel" else 1
+    period = 2 * np.pi * wl.geometry[1:, 12][None, :] if kind == "barrel" else 2 * np.pi
+    # the cut really is crossed: some hits lie more than half a period from their prediction before they are wrapped (the
+    # few tracks that pass within a hit resolution of alpha = 0 in the original chart; the whole-period shifts below
+    # exercise the rule on a third of all hits)
+    tr = np.repeat(np.arange(wl.n_tracks), np.diff(wl.offsets))
+    raw = wl2.loc[:, ang] - b.pred_params[tr, wl2.surf_idx - 1, ang]
+    half = (np.pi * wl.geometry[wl2.surf_idx, 12]) if kind == "barrel" else np.pi
+    assert np.sum(np.abs(raw) > half) >= 1
+    np.testing.assert_allclose(b.chi2, a.chi2, rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(b.hit_chi2, a.hit_chi2, rtol=1e-8, atol=1e-9)
+    for name in ("pred_params", "filt_params", "smooth_params"):
+        xa, xb = getattr(a, name), getattr(b, name)
+        other = [k for k in range(6) if k != ang]
+        np.testing.assert_allclose(xb[..., other], xa[..., other], rtol=1e-9, atol=1e-9)
+        d = (xb[..., ang] - xa[..., ang]) / period          # half a period apart, modulo whole periods
+        np.testing.assert_allclose(d - np.round(d - 0.5), 0.5, atol=1e-9)
+    np.testing.assert_allclose(b.smooth_cov, a.smooth_cov, rtol=1e-7, atol=1e-18)
+    # a hit given a whole period off is the same hit
+    wl3 = across_the_branch_cut(wl, kind)
+    shift = (2 * np.pi * wl.geometry[wl3.surf_idx, 12]) if kind == "barrel" else 2 * np.pi
+    wl3.loc[::3, ang] += shift[::3] if kind == "barrel" else shift
+    c = oracle.fit_workload(wl3)
+    np.testing.assert_allclose(c.chi2, b.chi2, rtol=1e-9, atol=1e-9)
+    np.testing.assert_allclose(c.first_params, b.first_params, rtol=1e-9, atol=1e-9)
