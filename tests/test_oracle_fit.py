@@ -372,3 +372,4 @@ def test_rts_phi_difference_is_wrapped_over_any_number_of_turns():
     assert rc != 0
     bad[2] = 1e300
     rc, x, C = oracle.rts_step(xf, Cf, F, xp1, Cp1, bad, Cs1)  # returns (the loop form never did)
+
