@@ -31,7 +31,8 @@
  *              the descriptor structs themselves are small HOST structs read during the call.
  *
  * Ownership and ordering
- *   The caller owns every buffer including the workspace.  The library allocates no device or
+ *   The caller owns every buffer including the workspace (kf_fit_batch_static alone uses a fixed array inside
+ *   the library image instead; see there).  The library allocates no device or
  *   pinned memory, never frees and never synchronises: kf_fit_batch validates the descriptors on
  *   the host, enqueues its kernels on `cuda_stream` (a cudaStream_t; NULL = the legacy default
  *   stream) and returns.  Inputs are read-only.  Buffers must stay valid until the stream has run
@@ -58,7 +59,7 @@
 extern "C" {
 #endif
 
-#define KF_VERSION 108          /* major * 100 + minor */
+#define KF_VERSION 109          /* major * 100 + minor */
 #define KF_GEOM_STRIDE 20       /* doubles per surface record */
 #define KF_MAX_SUBSTEPS 1024    /* cap on primary RKN sub-steps per leg (max_step_mm) */
 
@@ -68,7 +69,8 @@ enum {
   KF_ERR_ARG = -1,        /* null / ill-formed descriptor */
   KF_ERR_UNSUPPORTED = -2,/* unsupported option combination */
   KF_ERR_WORKSPACE = -3,  /* workspace too small (see kf_workspace_bytes) */
-  KF_ERR_CUDA = -4        /* CUDA error at launch (text: kf_last_cuda_error) */
+  KF_ERR_CUDA = -4,       /* CUDA error at launch (text: kf_last_cuda_error) */
+  KF_ERR_STATIC_LIMIT = -5 /* kf_fit_batch_static only: the batch needs more scratch than KF_STATIC_WORKSPACE_BYTES */
 };
 
 /* per-track status bits (never fail the call) */
@@ -295,6 +297,46 @@ size_t kf_workspace_bytes(int64_t n_tracks, int32_t n_legs_max, const kf_options
 int kf_fit_batch(const kf_tracks_in* tracks, const kf_measurements* meas, const kf_geometry* geom,
                  const kf_field* field, const kf_options* opt, const kf_outputs* out,
                  void* workspace, size_t workspace_bytes, void* cuda_stream);
+
+/* The same fit for a caller that has no device memory to give as workspace and may not allocate any.
+ *
+ * Who that is: kf_fit_batch leaves the RTS records, leg counts and length-sort arrays to a caller-owned workspace,
+ * which assumes the caller can get one.  Some cannot.  A reconstruction module plugged into an experiment's event
+ * framework gets its input and output buffers from the framework's device-memory pool and is forbidden to call the
+ * CUDA allocator itself (the pool is the memory budget).  An online-trigger or other latency-bound thread may not
+ * call cudaMalloc / cudaFree once the run has started, because those calls take driver-wide locks and cudaFree
+ * waits for the whole device: one late allocation stalls every stream.  A process on a GPU whose memory is already
+ * handed out to its neighbours cannot count on a late cudaMalloc succeeding at all.
+ *
+ * What it does: the workspace lives in a KF_STATIC_WORKSPACE_BYTES array that is part of the library image
+ * (a file-scope `static __device__ __align__(256)` array in kf_fit.cu).  The call allocates nothing, frees nothing and
+ * calls no allocating library routine; apart from the workspace it is kf_fit_batch argument for argument (same
+ * validation, same kernels, same results bit for bit), with `tracks`, `meas`, `geom`, `field`, `out` still the
+ * caller's DEVICE buffers.
+ *
+ * Limit: the batch must satisfy kf_workspace_bytes(n_tracks, n_legs_max, opt) <= KF_STATIC_WORKSPACE_BYTES (64 MiB:
+ * about 5,000 tracks x 30 legs in FP64 with smoothing, 10,000 in MIXED precision; any number without smoothing up
+ * to the sort arrays' 4.5 B per track).  A larger batch is refused with KF_ERR_STATIC_LIMIT before anything is
+ * enqueued, outputs untouched: split it, or use kf_fit_batch with a workspace.  The price of the array: every GPU
+ * on which this process uses the library gives up those 64 MiB from the moment the library's code is loaded onto it
+ * until the process exits, whether or not this entry point is ever called.
+ *
+ * First call on a device: the first call made while a given device is current looks up the array's device address
+ * on that device (cudaGetSymbolAddress, which may also load the library's module there) and remembers it; later
+ * calls on that device reuse it.  Make that first call with the device current, outside any stream capture, e.g.
+ * once at start-up with n_tracks = 0 (which does the look-up and enqueues nothing).  A failed look-up returns
+ * KF_ERR_CUDA and is retried by the next call.
+ *
+ * One array, shared: every call on a device, from whatever thread or stream, uses the same bytes, and the array
+ * keeps what the previous call left in it.  Nothing in it has to be cleared by the caller: the only part that must
+ * start at zero, the length sort's counters, is cleared on `cuda_stream` by the call itself (as in kf_fit_batch),
+ * and every record and leg count is written by the forward kernel before the backward pass reads it.  But two calls
+ * whose kernels can run at the same time on one GPU (different streams without an ordering between them, or two
+ * host threads) overwrite each other's records and give wrong results without any error: order them on one
+ * stream, or with events.  Calls on different GPUs do not interfere (each GPU has its own copy of the array). */
+#define KF_STATIC_WORKSPACE_BYTES (64u * 1024u * 1024u)
+int kf_fit_batch_static(const kf_tracks_in* tracks, const kf_measurements* meas, const kf_geometry* geom,
+                        const kf_field* field, const kf_options* opt, const kf_outputs* out, void* cuda_stream);
 
 /* End-to-end variant for HOST buffers (the paper's offload runtime):
  * every array pointer in tracks/meas/geom/field/out is a HOST pointer (pinned memory for

@@ -30,7 +30,8 @@ _TRIU = np.triu_indices(6)  # packed upper triangle, row-major: 00 01 .. 05 11 .
 
 EXPORTS = ("kf_default_options", "kf_workspace_bytes", "kf_fit_batch", "kf_host_arena_bytes",
            "kf_fit_batch_host", "kf_fit_batch_host_pipelined", "kf_last_launch_count", "kf_set_stage_events", "kf_probe_fp64_tflops", "kf_status_string",
-           "kf_last_cuda_error", "kf_version", "kf_field_stage_box")
+           "kf_last_cuda_error", "kf_version", "kf_field_stage_box", "kf_fit_batch_static")
+STATIC_WORKSPACE_BYTES = 64 * 1024 * 1024  # KF_STATIC_WORKSPACE_BYTES
 
 
 class KfTracksIn(C.Structure):
@@ -104,6 +105,8 @@ def lib():
     L.kf_fit_batch.argtypes = [C.POINTER(KfTracksIn), C.POINTER(KfMeasurements), C.POINTER(KfGeometry),
                                C.POINTER(KfField), C.POINTER(KfOptions), C.POINTER(KfOutputs),
                                C.c_void_p, C.c_size_t, C.c_void_p]
+    L.kf_fit_batch_static.restype = C.c_int
+    L.kf_fit_batch_static.argtypes = L.kf_fit_batch.argtypes[:6] + [C.c_void_p]
     L.kf_host_arena_bytes.restype = C.c_size_t
     L.kf_host_arena_bytes.argtypes = [C.c_int64, C.c_int64, C.c_int32, C.c_int32, C.POINTER(KfField),
                                       C.POINTER(KfOptions), C.c_int, C.c_int]
@@ -412,6 +415,41 @@ class FitCall:
         rc = lib().kf_fit_batch(C.byref(self.tracks), C.byref(self.meas), C.byref(self.geom),
                                 C.byref(self.field), C.byref(self.opt), C.byref(self.outs),
                                 _ptr(self.workspace), self.workspace.numel(), C.c_void_p(s.cuda_stream))
+        if rc != 0:
+            raise KfError(rc)
+        self.launches = lib().kf_last_launch_count()
+        return self.out
+
+
+class StaticFitCall(FitCall):
+    """A prepared kf_fit_batch_static call: the fit for callers that cannot allocate device memory for a workspace.
+
+    Meant for code that receives its input and output buffers from somebody else's memory pool and is not allowed
+    to call the CUDA allocator itself (a plug-in inside an event-processing framework), or that must not allocate
+    once its latency-critical loop runs (cudaMalloc / cudaFree take driver-wide locks; cudaFree waits for the device).
+    The RTS records and sort arrays then live in a 64 MiB array inside the library image (STATIC_WORKSPACE_BYTES)
+    instead of a caller-owned workspace, so the batch must need no more than that (about 5,000 tracks x 30 legs in
+    FP64): a larger one raises KfError with rc = -5 and nothing is enqueued.  Results are those of FitCall, bit for
+    bit.  All calls on one GPU share that array: calls that could overlap on the GPU (two streams with no ordering
+    between them) corrupt each other, so keep them on one stream or order them with events.  The first run() on a
+    device also looks up the array's address there; do it once at start-up, outside any stream capture.
+
+    Here torch still allocates the inputs and outputs (this is a test and example harness); the library call
+    itself allocates nothing."""
+
+    def __init__(self, batch: DeviceBatch, out: Optional[DeviceOutputs] = None, perigee=None, **opt_over):
+        torch = _torch()
+        # an empty tensor stands in for FitCall's workspace so that none is allocated
+        super().__init__(batch, out=out, workspace=torch.empty(0, dtype=torch.uint8, device=batch.device),
+                         perigee=perigee, **opt_over)
+
+    def run(self, stream=None):
+        torch = _torch()
+        s = stream if stream is not None else torch.cuda.current_stream(self.batch.device)
+        with torch.cuda.device(self.batch.device):  # the static array is looked up on the CURRENT device
+            rc = lib().kf_fit_batch_static(C.byref(self.tracks), C.byref(self.meas), C.byref(self.geom),
+                                           C.byref(self.field), C.byref(self.opt), C.byref(self.outs),
+                                           C.c_void_p(s.cuda_stream))
         if rc != 0:
             raise KfError(rc)
         self.launches = lib().kf_last_launch_count()

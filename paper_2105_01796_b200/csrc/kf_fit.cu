@@ -234,6 +234,9 @@ const char* kf_status_string(int rc) {
     case KF_ERR_UNSUPPORTED: return "unsupported option combination";
     case KF_ERR_WORKSPACE: return "workspace too small";
     case KF_ERR_CUDA: return "CUDA error (see kf_last_cuda_error)";
+    case KF_ERR_STATIC_LIMIT:
+      return "batch needs more scratch than the 64 MiB static workspace of kf_fit_batch_static holds "
+             "(kf_workspace_bytes > KF_STATIC_WORKSPACE_BYTES): split the batch or use kf_fit_batch with a workspace";
     default: return "unknown return code";
   }
 }
@@ -462,6 +465,74 @@ int kf_fit_batch(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geo
   rc = build_params(tr, ms, ge, fl, op, out, workspace, workspace_bytes, P, sort);
   if (rc != KF_OK) return rc;
   const int lmax = ge->n_surfaces - 1 - tr->start_surface;
+  return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
+                     sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream),
+                     general_mode(ge, fl, op));
+}
+
+// ---- kf_fit_batch_static: the fit for callers that may not allocate (include/kf_fit.h) ----------------------
+}  // extern "C"
+
+namespace {
+
+// The workspace of kf_fit_batch_static.  It is part of the library image: each GPU gets its own copy when the module
+// of this file is loaded there and keeps it until the process ends.  In HOST code the name below is only a handle
+// for cudaGetSymbolAddress -- it is not a device address and must never be handed to a kernel.
+static __device__ __align__(256) unsigned char g_static_workspace[KF_STATIC_WORKSPACE_BYTES];
+
+constexpr int kMaxStaticDevices = 64;
+
+// Device address of g_static_workspace on the CURRENT device, looked up once per device and kept.  The look-up is
+// the set-up step that the header asks callers to get out of the way before any stream capture.
+int static_workspace_on_current_device(void** ptr) {
+  static std::mutex mu;
+  static void* addr[kMaxStaticDevices] = {};
+  int dev = 0;
+  if (set_cuda_error(cudaGetDevice(&dev), "kf_fit_batch_static: cudaGetDevice")) return KF_ERR_CUDA;
+  if (dev < 0 || dev >= kMaxStaticDevices) {
+    snprintf(g_cuda_error, sizeof(g_cuda_error), "kf_fit_batch_static: device ordinal %d beyond the %d supported", dev,
+             kMaxStaticDevices);
+    return KF_ERR_CUDA;
+  }
+  std::lock_guard<std::mutex> lock(mu);
+  if (!addr[dev]) {
+    void* p = nullptr;
+    if (set_cuda_error(cudaGetSymbolAddress(&p, g_static_workspace), "kf_fit_batch_static: cudaGetSymbolAddress"))
+      return KF_ERR_CUDA;
+    if (!p) {
+      snprintf(g_cuda_error, sizeof(g_cuda_error), "kf_fit_batch_static: cudaGetSymbolAddress returned a null address");
+      return KF_ERR_CUDA;
+    }
+    addr[dev] = p;
+  }
+  *ptr = addr[dev];
+  return KF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int kf_fit_batch_static(const kf_tracks_in* tr, const kf_measurements* ms, const kf_geometry* ge, const kf_field* fl,
+                        const kf_options* op, const kf_outputs* out, void* cuda_stream) {
+  g_launches = 0;
+  int rc = validate(tr, ms, ge, fl, op, out);
+  if (rc != KF_OK) return rc;
+  // the size test is host arithmetic and comes before any CUDA call: a batch that does not fit changes nothing
+  const int lmax = ge->n_surfaces - 1 - tr->start_surface;
+  const size_t need = kf_workspace_bytes(tr->n_tracks, lmax, op);
+  if (need > (size_t)KF_STATIC_WORKSPACE_BYTES) return KF_ERR_STATIC_LIMIT;
+  void* workspace = nullptr;
+  rc = static_workspace_on_current_device(&workspace);  // first call on this device: the one-time address look-up
+  if (rc != KF_OK) return rc;
+  if (tr->n_tracks == 0) return KF_OK;
+  // from here on this is kf_fit_batch with the static array as a full-size workspace.  What must start at zero in
+  // it (the length sort's counters) is cleared on the stream by launch_length_sort; the rest of the last call's
+  // contents is overwritten by the forward kernel before anything reads it.
+  kf::FitParams P;
+  SortPlan sort;
+  rc = build_params(tr, ms, ge, fl, op, out, workspace, (size_t)KF_STATIC_WORKSPACE_BYTES, P, sort);
+  if (rc != KF_OK) return rc;
   return enqueue_fit(P, perigee_params(op, out, 0), fl->kind == KF_FIELD_GRID3, op->material != 0, op->variant,
                      sort_for_range(sort, op, 0, tr->n_tracks, ms->n_meas, lmax), static_cast<cudaStream_t>(cuda_stream),
                      general_mode(ge, fl, op));

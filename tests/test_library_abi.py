@@ -44,7 +44,7 @@ def test_struct_sizes_match_the_header_layout():
 
 def test_defaults_and_version():
     L = B.lib()
-    assert L.kf_version() == 108
+    assert L.kf_version() == 109
     o = B.default_options()
     assert (o.smooth, o.material, o.n_corr_steps, o.output_states, o.variant, o.length_sort, o.precision) == (1, 0, 2, 0, 0, 0, 0)
     assert o.outlier_chi2 == 0.0 and np.isinf(o.max_step_mm) and o.cov_inflation == 1.0
