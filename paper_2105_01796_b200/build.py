@@ -45,8 +45,36 @@ def nvcc_path() -> str:
     raise RuntimeError("nvcc not found: libkf_fit.so cannot be built (there is no CPU fallback)")
 
 
-def is_stale() -> bool:
+STAMP = os.path.join(OBJ_DIR, "flags.txt")
+
+
+def flag_stamp(extra_flags=()) -> str:
+    """What the stamp file of a build holds: the path-independent nvcc flags, tuning -D macros included (the -I paths
+    are left out: the repository sits at another path on the GPU box)."""
+    return " ".join([*NVCC_FLAGS, *extra_flags])
+
+
+def built_flags():
+    """The flag stamp of the library that is there now (None: no stamp)."""
+    try:
+        with open(STAMP) as f:
+            return f.read()
+    except OSError:
+        return None
+
+
+def built_defines() -> list:
+    """The -D macros the library that is there now was built with ([] for the default build)."""
+    return [w for w in (built_flags() or "").split() if w.startswith("-D")]
+
+
+def is_stale(extra_flags=()) -> bool:
+    """True when the library is missing, older than a source or header, or was built with other flags than
+    `extra_flags` asks for: a tuning build (`python build.py -DKF_FWD_MIN_BLOCKS=2`) is stale for every later default
+    call (lib(), tests, bench, __graft_entry__.build), which therefore rebuilds instead of silently using it."""
     if not os.path.exists(LIB_PATH):
+        return True
+    if built_flags() != flag_stamp(extra_flags):
         return True
     t = os.path.getmtime(LIB_PATH)
     return any(os.path.getmtime(p) > t for p in sources() + headers())
@@ -62,7 +90,7 @@ def _run(cmd):
 def build_library(force: bool = False, verbose: bool = False, extra_flags=()) -> str:
     """Compile every csrc/*.cu to an object (side by side, one nvcc each) and link them into libkf_fit.so.
     An object is rebuilt when its source or any header is newer (or `force`, or other flags than last time)."""
-    if not force and not is_stale():
+    if not force and not is_stale(extra_flags):
         return LIB_PATH
     from concurrent.futures import ThreadPoolExecutor
     os.makedirs(OBJ_DIR, exist_ok=True)
@@ -70,8 +98,7 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
     flags = [*NVCC_FLAGS, *extra_flags, "-I", INCLUDE, "-I", CSRC]
     if verbose:
         flags = ["-Xptxas", "-v", *flags]
-    stamp = os.path.join(OBJ_DIR, "flags.txt")
-    same_flags = os.path.exists(stamp) and open(stamp).read() == " ".join(flags)
+    same_flags = built_flags() == flag_stamp(extra_flags)
     newest_header = max(os.path.getmtime(p) for p in headers())
     jobs, objs = [], []
     for src in sources():
@@ -88,9 +115,11 @@ def build_library(force: bool = False, verbose: bool = False, extra_flags=()) ->
         for log in pool.map(_run, jobs):
             if verbose:
                 print(log, file=sys.stderr)
-    with open(stamp, "w") as f:
-        f.write(" ".join(flags))
+    if os.path.exists(STAMP):
+        os.remove(STAMP)  # a build that fails half-way leaves no stamp: the next call starts over
     _run([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB_PATH, *objs])
+    with open(STAMP, "w") as f:
+        f.write(flag_stamp(extra_flags))
     return LIB_PATH
 
 

@@ -31,6 +31,26 @@ def test_library_builds_and_exports_every_declared_symbol():
         assert hasattr(lib, n), f"{n} declared in include/kf_fit.h but not exported"
 
 
+def test_a_build_with_other_flags_is_stale_for_the_default_build():
+    """build.py: a tuning build (`python build.py -DKF_FWD_MIN_BLOCKS=2`) must not be picked up silently by a later default
+    call (lib(), tests, bench): staleness compares the flag stamp of the library that is there, not only file times."""
+    kbuild.build_library()
+    assert not kbuild.is_stale()
+    assert kbuild.built_flags() == kbuild.flag_stamp() and kbuild.built_defines() == []
+    assert kbuild.is_stale(extra_flags=("-DKF_FWD_MIN_BLOCKS=2",))
+    assert "-DKF_FWD_MIN_BLOCKS=2" in kbuild.flag_stamp(("-DKF_FWD_MIN_BLOCKS=2",))
+    assert ROOT not in kbuild.flag_stamp()   # path-free: the repository sits elsewhere on the GPU box
+    saved = kbuild.built_flags()
+    try:
+        with open(kbuild.STAMP, "w") as f:
+            f.write(saved + " -DKF_FWD_MIN_BLOCKS=2")   # as a tuning build would leave it
+        assert kbuild.is_stale() and kbuild.built_defines() == ["-DKF_FWD_MIN_BLOCKS=2"]
+    finally:
+        with open(kbuild.STAMP, "w") as f:
+            f.write(saved)
+    assert not kbuild.is_stale()
+
+
 def test_struct_sizes_match_the_header_layout():
     # natural C layout of include/kf_fit.h on x86-64 / aarch64 (8-byte pointers and doubles)
     assert C.sizeof(B.KfTracksIn) == 32
