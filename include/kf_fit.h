@@ -188,8 +188,11 @@ typedef struct kf_geometry {
   double mat_rho;          /* density g/cm^3 */
   double mat_I_eV;         /* mean excitation energy */
   int32_t surface_kinds;   /* bit k set = the table holds surfaces of kind k (the table itself is DEVICE memory, which
-                              the host-side dispatch does not read).  0 or 1 = planes only: entry [18] is then ignored
-                              and the plane-only kernels run.  Any other value selects the general-surface kernels:
+                              the host-side dispatch does not read).  0 or 1 = planes only: the plane-only kernels run
+                              and entry [18] is then ignored by the fit AND by the perigee extrapolation (one exception:
+                              kf_options.field_gradient with a GRID3 field runs the general kernels, which read entry
+                              [18] of every record -- keep it 0 for planes there).  Any other value selects the
+                              general-surface kernels:
                               one thread per track, RTS smoother, at most 1024 surfaces, FP64 or MIXED precision
                               (KF_ERR_UNSUPPORTED with KF_VARIANT_LANES_PER_TRACK or Bryson-Frazier) */
 } kf_geometry;

@@ -39,8 +39,9 @@ int launch_length_sort(const kf::FitParams& P, int* perm, int* bins, int force, 
   return KF_OK;
 }
 
-int launch_perigee(const kf::FitParams& P, const PerigeeLine& line, bool grid3, cudaStream_t stream) {
+int launch_perigee(const kf::FitParams& P, const PerigeeLine& line, bool grid3, bool any_kind, cudaStream_t stream) {
   kf::PerigeeParams G{};
+  G.any_kind = any_kind ? 1 : 0;
   for (int a = 0; a < 3; ++a) { G.line.c[a] = line.c[a]; G.line.a[a] = line.a[a]; }
   G.params = line.params;
   G.cov = line.cov;

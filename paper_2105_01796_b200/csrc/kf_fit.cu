@@ -416,7 +416,9 @@ int enqueue_fit(const kf::FitParams& P0, const kfh::PerigeeLine& G, bool grid3, 
   if (P.smooth) rc = kfh::launch_backward(P, lanes, stream);
   record_stage(2, stream);
   // fitted parameters on the perigee surface: one more (small) kernel
-  if (rc == KF_OK && G.params) rc = kfh::launch_perigee(P, G, grid3, stream);
+  // (the perigee kernel reads the chart of the first surface the way the forward kernel did: entry [18] only when the
+  // general kernels ran)
+  if (rc == KF_OK && G.params) rc = kfh::launch_perigee(P, G, grid3, mode != 0, stream);
   return rc;
 }
 

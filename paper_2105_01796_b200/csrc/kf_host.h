@@ -79,7 +79,8 @@ struct PerigeeLine {
 };
 int launch_backward(const kf::FitParams& P, bool lanes, cudaStream_t stream);
 int launch_length_sort(const kf::FitParams& P, int* perm, int* bins, int force, cudaStream_t stream);
-int launch_perigee(const kf::FitParams& P, const PerigeeLine& line, bool grid3, cudaStream_t stream);
+// any_kind: the geometry table may hold cylinders / discs (kf_geometry.surface_kinds > 1); false: entry [18] is not read
+int launch_perigee(const kf::FitParams& P, const PerigeeLine& line, bool grid3, bool any_kind, cudaStream_t stream);
 double probe_fp64_tflops(int iters, cudaStream_t stream);
 
 }  // namespace kfh

@@ -21,9 +21,12 @@ struct LineSurface {
   double c[3], a[3];
 };
 
-// (x on plane sf) -> (xo on the line, J).  Returns 0 or the stopping bit; `status` collects FIELD_CLAMPED.
+// (x on surface sf) -> (xo on the line, J).  Returns 0 or the stopping bit; `status` collects FIELD_CLAMPED.
+// any_kind: the call runs in the general-surface kernels (kf_geometry.surface_kinds > 1), so record entry [18] says
+// which chart sf has; false: planes only, entry [18] is NOT read (include/kf_fit.h: "entry [18] is then ignored").
 template <int FIELD>
 __device__ __forceinline__ unsigned propagate_to_line(const FieldDesc& F, double mass, int n_corr, double max_step,
+                                                      bool any_kind,
                                                       const double* __restrict__ sf, const LineSurface& Ln,
                                                       const double x[6], double xo[6], BoundJacobian& J,
                                                       unsigned& status) {
@@ -34,7 +37,7 @@ __device__ __forceinline__ unsigned propagate_to_line(const FieldDesc& F, double
 #pragma unroll
   for (int i = 0; i < 3; ++i) r[i] = sf[i] + x[0] * sf[3 + i] + x[1] * sf[6 + i];
   double e0[3] = {sf[3], sf[4], sf[5]}, e1[3] = {sf[6], sf[7], sf[8]};
-  if ((int)sf[18] != SURF_PLANE) local_to_global(sf, x[0], x[1], r, e0, e1);  // first_* on a cylinder or a disc (U33)
+  if (any_kind && (int)sf[18] != SURF_PLANE) local_to_global(sf, x[0], x[1], r, e0, e1);  // first_* on a cylinder or a disc (U33)
   T[0] = cphi * sth; T[1] = sphi * sth; T[2] = cth;
   const double lam = x[4];
   double t = x[5];
@@ -173,6 +176,7 @@ struct PerigeeParams {
   LineSurface line;
   double* params;  // [6][ldn]
   double* cov;     // [21][ldn]
+  int any_kind;    // 1: the fit ran in the general-surface kernels, geometry entry [18] is the surface kind; 0: planes
 };
 
 constexpr int kPerigeeBlock = 128;
@@ -194,7 +198,7 @@ kf_perigee_kernel(const __grid_constant__ FitParams P, const __grid_constant__ P
   unsigned status = 0u;
   double xo[6], Co[21];
   BoundJacobian J;
-  const unsigned rc = propagate_to_line<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, sf, G.line, x, xo, J, status);
+  const unsigned rc = propagate_to_line<FIELD>(P.field, P.mat.mass, P.n_corr, P.max_step, G.any_kind != 0, sf, G.line, x, xo, J, status);
   bool ok = rc == 0u;
   if (ok) {
     transport_covariance(J, C, Co);

@@ -57,6 +57,26 @@ def test_perigee_parameters_parity(cfg, n, line):
         assert np.all(np.abs(pull.mean(axis=0)) < 4.5 / np.sqrt(n)) and np.all(np.abs(pull.std(axis=0) - 1.0) < 0.05)
 
 
+def test_planes_only_table_ignores_the_kind_entry_also_in_the_perigee_extrapolation():
+    """include/kf_fit.h, kf_geometry.surface_kinds: with 0 or 1 the plane-only kernels run and record entry [18] is
+    ignored -- by the fit and by the perigee kernel alike (it once took the first surface's chart from [18] whatever
+    the dispatch said).  Junk in [18..19] must not change a bit of the result."""
+    import dataclasses
+    wl = W.make_config(2, n_tracks=700, seed=61)
+    hb = kf.HostBatch.from_workload(wl)
+    ref = kf.FitCall(kf.DeviceBatch(hb), perigee=TILTED_AXIS).run().to_host()
+    geo = hb.geometry.copy()
+    geo[:, 18] = np.where(np.arange(geo.shape[0]) % 2 == 0, 1.0, 2.0)   # "cylinder", "disc"
+    geo[:, 19] = 12345.0
+    call = kf.FitCall(kf.DeviceBatch(dataclasses.replace(hb, geometry=geo)), perigee=TILTED_AXIS)
+    assert call.geom.surface_kinds > 1      # what the binding derives from the host copy of the table ...
+    call.geom.surface_kinds = 1             # ... and what this caller declares instead: planes only
+    got = call.run().to_host()
+    assert np.all(np.isfinite(got.perigee_params[(got.status & 128) == 0]))
+    for name in ("perigee_params", "perigee_cov", "first_params", "first_cov", "last_params", "last_cov", "chi2", "status"):
+        np.testing.assert_array_equal(getattr(got, name), getattr(ref, name), err_msg=name)
+
+
 def test_perigee_failing_tracks_and_options(variant):
     """tracks that never start (bad hit lists, NaN input), moving along the axis, stepping options."""
     wl = W.make_config(2, n_tracks=400, seed=33)
