@@ -139,3 +139,82 @@ def resolution_loss(low, ref, offsets, cut=0.0, guard=0.1):
     out["params_sigma"], out["var_rel"] = worst_p, worst_v
     out["chi2_abs"] = float(np.max(np.abs(low.chi2[ok] - ref.chi2[ok])))
     return out
+
+
+# ---- whole-population comparison at full size (first_*, last_*, chi2, ndf, counters, status for ALL
+# tracks; per-surface states for a 1 % sample) --------------------------------------------------------------------------
+def per_track_factors(gpu, ref):
+    """Per track, the largest factor of the tolerance used by each floating-point quantity (same bars as compare())."""
+    out = {}
+    for name in ("first_params", "last_params"):
+        g, r = np.asarray(getattr(gpu, name)), np.asarray(getattr(ref, name))
+        tol = PARAM_RTOL * np.maximum(np.abs(r), PARAM_FLOOR)
+        with np.errstate(invalid="ignore"):
+            ex = np.abs(g - r) / tol
+        ex = np.where(np.isnan(r) & np.isnan(g), 0.0, np.where(np.isnan(ex), np.inf, ex))
+        out[name] = ex.max(axis=1)
+    for name in ("first_cov", "last_cov"):
+        g, r = np.asarray(getattr(gpu, name)), np.asarray(getattr(ref, name))
+        d = np.sqrt(np.abs(np.einsum("nii->ni", r)))
+        with np.errstate(invalid="ignore", divide="ignore"):
+            ex = np.abs(g - r) / (COV_RTOL * d[:, :, None] * d[:, None, :])
+        ex = np.where((np.isnan(r) & np.isnan(g)) | (g == r), 0.0, np.where(np.isnan(ex), np.inf, ex))
+        out[name] = ex.reshape(ex.shape[0], -1).max(axis=1)
+    g, r = np.asarray(gpu.chi2), np.asarray(ref.chi2)
+    out["chi2"] = np.abs(g - r) / (CHI2_RTOL * np.maximum(np.abs(r), 1.0))
+    return out
+
+
+def whole_population(wl, gpu, label, **oracle_over):
+    """Every track of `wl` re-fitted by the oracle (all host cores) and compared with the CUDA result `gpu` (host arrays of
+    DeviceOutputs.to_host()).  Discrete results (ndf, counters, status, per-hit flags) must agree on every track: a track
+    that differs is LISTED in the failure message, none is excluded.  Floating-point results: the worst factor of the
+    north_star bars and the 99.99th percentile over tracks are printed per quantity; the worst must be <= 1."""
+    import oracle
+    ref = oracle.fit_workload(wl, **oracle_over)
+    n = wl.n_tracks
+    flipped = np.zeros(n, bool)
+    for name in ("ndf", "n_used", "n_outliers", "n_holes"):
+        flipped |= np.asarray(getattr(gpu, name)) != np.asarray(getattr(ref, name))
+    flipped |= np.asarray(gpu.status).astype(np.uint32) != np.asarray(ref.status).astype(np.uint32)
+    hit_diff = 0
+    if gpu.hit_flags is not None and ref.hit_flags is not None:
+        bad_hits = np.asarray(gpu.hit_flags) != np.asarray(ref.hit_flags)
+        hit_diff = int(bad_hits.sum())
+        if hit_diff:
+            flipped[np.unique(np.searchsorted(wl.offsets, np.flatnonzero(bad_hits), side="right") - 1)] = True
+    idx = np.flatnonzero(flipped)
+    listing = [dict(track=int(i), status=(int(gpu.status[i]), int(ref.status[i])), n_used=(int(gpu.n_used[i]), int(ref.n_used[i])),
+                    n_outliers=(int(gpu.n_outliers[i]), int(ref.n_outliers[i])), n_holes=(int(gpu.n_holes[i]), int(ref.n_holes[i])))
+               for i in idx[:20]]
+    fac = per_track_factors(gpu, ref)
+    if gpu.hit_chi2 is not None and ref.hit_chi2 is not None:
+        g, r = np.asarray(gpu.hit_chi2), np.asarray(ref.hit_chi2)
+        fac["hit_chi2"] = np.abs(g - r) / (CHI2_RTOL * np.maximum(np.abs(r), 1.0))
+    rep = {k: dict(worst=float(v.max()) if v.size else 0.0, p9999=float(np.percentile(v, 99.99)) if v.size else 0.0,
+                   at=int(np.argmax(v)) if v.size else -1) for k, v in fac.items()}
+    print(f"\n[whole population] {label}: {n} tracks, {wl.n_meas} hits against the oracle; discrete decisions differing on "
+          f"{idx.size} tracks ({hit_diff} hit flags)")
+    for k, v in rep.items():
+        print(f"    {k:13s} worst factor of the bar {v['worst']:.3e} (element {v['at']}), 99.99th percentile {v['p9999']:.3e}")
+    assert idx.size == 0, f"{label}: discrete decisions differ on {idx.size} of {n} tracks (first 20 listed): {listing}"
+    over = {k: v for k, v in rep.items() if not v["worst"] <= 1.0}
+    assert not over, f"{label}: tolerance exceeded: {over}"
+    return rep, ref
+
+
+def state_sample(wl, label, fraction=0.01, seed=0, **over):
+    """Per-surface PRED / FILT / SMOOTH states of a `fraction` sample of the tracks (first and last tile included): the
+    sample is fitted by both sides with all per-leg states out and compared element by element."""
+    import oracle
+    import paper_2105_01796_b200 as kf
+    rng = np.random.default_rng(seed)
+    n = wl.n_tracks
+    idx = np.unique(np.concatenate([rng.choice(n, max(1, int(n * fraction)), replace=False), np.arange(min(64, n)),
+                                    np.arange(max(0, n - 64), n)]))
+    sub = wl.subset(idx)
+    ref = oracle.fit_workload(sub, states=True, **over)
+    got = kf.fit_workload(sub, states=True, **over)
+    rep = assert_parity(got, ref, states=True, label=label + f" (per-leg states, {idx.size} tracks)")
+    print(f"[state sample] {label}: {idx.size} tracks, worst factor {max(rep.values()):.3e}")
+    return rep
