@@ -132,6 +132,12 @@ def test_random_configuration_parity(seed):
         wide = np.nan_to_num(np.einsum("nlii->nli", ref.pred_cov)[..., :2], nan=0.0, posinf=1e99).max(axis=(1, 2)) > 1e4
         odd = ~np.all(np.isfinite(np.nan_to_num(ref.last_params, nan=0.0)), axis=1)
     runaway = far | wide | odd
+    # such tracks are counted and listed, not silently dropped.  Over the 48 seeds the criterion (a
+    # function of the ORACLE's result only) marks 1,112 of 15,391 tracks, at most a third of a case
+    n_run = int(runaway.sum())
+    print(f"\n[fuzz seed {seed}] runaway tracks (values not compared, discrete results counted below): {n_run} of {runaway.size}"
+          f"{': ' + str(np.flatnonzero(runaway)[:12].tolist()) if n_run else ''}")
+    assert n_run <= 0.4 * runaway.size, (seed, n_run, runaway.size)
     for variant in (B.VARIANT_THREAD_PER_TRACK, B.VARIANT_LANES_PER_TRACK):
         for sort in (B.SORT_OFF, B.SORT_ON):
             db = kf.DeviceBatch(hb)
@@ -149,6 +155,14 @@ def test_random_configuration_parity(seed):
             np.testing.assert_array_equal(got.hit_flags[keep_hits], ref.hit_flags[keep_hits], err_msg=label + " hit_flags")
             np.testing.assert_array_equal(got.status[~runaway], ref.status[~runaway], err_msg=label)
             np.testing.assert_array_equal(got.status[runaway] & np.uint32(64), ref.status[runaway] & np.uint32(64), err_msg=label)
+            # how many of the runaway tracks really took another discrete decision than the oracle (listed; the bar is that
+            # they stay the exception even inside this group)
+            flip = runaway & ((got.status != ref.status) | (got.n_used != ref.n_used) | (got.n_outliers != ref.n_outliers) |
+                              (got.n_holes != ref.n_holes))
+            if n_run:
+                print(f"    variant {variant} sort {sort}: {int(flip.sum())} of {n_run} runaway tracks differ in status or counters"
+                      f"{': ' + str([(int(i), int(got.status[i]), int(ref.status[i])) for i in np.flatnonzero(flip)[:8]]) if flip.any() else ''}")
+            assert flip.sum() <= 2, (label, int(flip.sum()), n_run)   # measured on B200 over the 48 seeds: 0 everywhere
             # values: every track that stayed a track and whose discrete decisions agree in double and long double
             same = ~runaway & (ref.status == ref_ld.status) & (ref.n_used == ref_ld.n_used) & (ref.n_outliers == ref_ld.n_outliers)
             well = same & (kappa <= 1e5)
