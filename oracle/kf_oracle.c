@@ -487,6 +487,12 @@ static int32_t propagate_r(const field_r* fld, const options_r* opt, const real 
   {
     real s0;
     if (!path_to_surface(st, f, f + 4, &s0)) return KFO_ST_PROPAGATION;
+    /* A cylinder is reached from inside (kf_fit.h KF_SURFACE_CYLINDER; reading U33): the first aim of a leg
+     * must lie ahead.  A start point outside the cylinder and moving away from it has its chosen root behind it
+     * (s0 <= 0) -- that is "cannot be reached", not a step backwards.  (Moving inwards from outside, the chosen root's
+     * denominator is negative and path_to_surface has already refused.)  Later aims of the same leg may be slightly
+     * negative: they are corrections around the surface. */
+    if (surf_kind(st) == SURF_CYLINDER && !(s0 > 0.0)) return KFO_ST_PROPAGATION;
     if (isfinite(opt->max_step_mm) && opt->max_step_mm > 0.0) {
       real q = ceil(fabs(s0) / opt->max_step_mm * (1.0 - 1e-12));
       if (!(q >= 1.0)) q = 1.0;

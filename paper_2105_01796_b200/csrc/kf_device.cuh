@@ -10,7 +10,11 @@
 //   * H selects loc0, loc1; covariances are packed upper triangles (21 numbers).
 // Citations: PAPER.md:55-62 (Kalman step, RTS with stored Jacobians), PAPER.md:128 (RKN transport,
 // local<->global Jacobians), PAPER.md:119 (8x8 global covariance), PAPER.md:168 (material).
-// This file shares nothing with oracle/ (its own constants, its own formulas' arrangement).
+// This file shares no code with oracle/ (its own constants, its own formulas' arrangement).  One caveat: the four
+// general-surface helpers below (local_to_global, surface_normal, global_to_local, path_to_surface) decompose reading
+// U33 the way the oracle does, so GPU-vs-oracle parity on cylinders and discs checks their transcription; what pins
+// U33 itself is independent of both: the oracle-side pins PS1-PS11 and the GPU-side closed-form test
+// tests/test_gpu_general.py::test_gpu_helix_to_cylinder_closed_form_without_the_oracle.
 #pragma once
 
 #include <cstdint>
@@ -848,6 +852,9 @@ __device__ __forceinline__ unsigned propagate(const FieldDescT<R>& F, R mass, in
   R h_first = R(0.0);  // CURVED: the first step's path length (also the reachability test)
   if constexpr (CURVED) {
     if (!path_to_surface(st, r, T, h_first)) return ST_PROPAGATION;
+    // a cylinder is reached from inside: a first aim that lies behind the start point (outside, moving away) is
+    // "cannot be reached", not a step backwards; later aims of the leg are corrections and may have either sign
+    if ((int)st[18] == SURF_CYLINDER && !(h_first > R(0.0))) return ST_PROPAGATION;
   } else {
     if (!(nT > R(kNdotTMin))) return ST_PROPAGATION;
   }
@@ -1201,6 +1208,7 @@ __device__ __forceinline__ unsigned propagate_general(const FieldDescT<R>& F, R 
   int n_sub = 1;
   R h;
   if (!path_to_surface(st, r, T, h)) return ST_PROPAGATION;
+  if ((int)st[18] == SURF_CYLINDER && !(h > R(0.0))) return ST_PROPAGATION;  // first aim behind the start point (see propagate<>)
   if (max_step > R(0.0)) {
     R qn = ceil(fabs(h) / max_step * (R(1.0) - R(1e-12)));
     if (!(qn >= R(1.0))) qn = R(1.0);

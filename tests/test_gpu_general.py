@@ -341,3 +341,97 @@ def test_hits_across_the_branch_cut_of_an_angular_coordinate(kind):
     other = [k for k in range(6) if k != ang]
     np.testing.assert_allclose(got.first_params[:, other], base.first_params[:, other], rtol=1e-8, atol=1e-9)
 
+
+def test_cylinder_behind_the_start_point_stops_the_track_like_the_oracle():
+    """kf_fit.h KF_SURFACE_CYLINDER "reached ... from inside" (pin PS11 on the oracle side): tracks that start outside the
+    first cylinder -- moving away, moving inwards, missing it -- stop with KF_ST_PROPAGATION on both sides instead of
+    stepping backwards; the tracks that start inside are fitted as before.  Status and counters exact, values at the bars."""
+    rng = np.random.default_rng(77)
+    def rec(kind, radius):
+        s = np.zeros(20)
+        s[3:6], s[6:9], s[9:12] = (0, 1, 0), (0, 0, 1), (1, 0, 0)   # plane x = 0: loc0 = y, loc1 = z; cylinders: axis z
+        s[12:14], s[16:18], s[18] = (radius, 500.0), (1e-4, 1e-4), kind
+        return s
+    geom = np.stack([rec(0, 50.0), rec(1, 60.0), rec(1, 80.0)])
+    n = 640
+    y0 = np.where(np.arange(n) % 4 == 0, rng.uniform(-20, 20, n), rng.uniform(90, 120, n))      # a quarter starts inside
+    phi = np.choose(np.arange(n) % 4, [rng.uniform(-0.3, 0.3, n), np.full(n, np.pi / 2), np.full(n, -np.pi / 2),
+                                       rng.uniform(-0.05, 0.05, n)])                           # ahead, away, inwards, missing
+    params0 = np.stack([y0, rng.uniform(-5, 5, n), phi, np.pi / 2 + rng.uniform(-0.1, 0.1, n),
+                        rng.choice([-1.0, 1.0], n) / rng.uniform(0.5, 5.0, n), np.zeros(n)], axis=1)
+    cov0 = np.tile(np.diag([0.05, 0.05, 1e-3, 1e-3, 0.01 * 0.5, 1.0]) ** 2, (n, 1, 1))
+    offsets = np.arange(0, 2 * n + 1, 2, dtype=np.int32)
+    surf_idx = np.tile(np.array([1, 2], np.int32), n)
+    loc = rng.normal(0.0, 5.0, (2 * n, 2))
+    opts = dict(smooth=1, material=0)
+    hb = kf.HostBatch.from_arrays(params0, cov0, 0, offsets, surf_idx, loc, geom, field_kind="const", field_b=(0, 0, 2.0),
+                                  options=opts)
+    got = kf.FitCall(kf.DeviceBatch(hb)).run().to_host()
+    ref = oracle.fit_batch(params0, cov0, 0, offsets, surf_idx, loc, geom, oracle.make_field("const", (0, 0, 2.0)),
+                           oracle.make_options(**opts))
+    outside = np.arange(n) % 4 != 0
+    assert np.all(ref.status[outside] & 1) and np.all(ref.n_used[outside] == 0)
+    assert np.all(ref.status[~outside] & 1 == 0) and np.all(ref.n_used[~outside] == 2)
+    parity.assert_parity(got, ref, label="cylinder behind the start point")
+
+
+def test_gpu_helix_to_cylinder_closed_form_without_the_oracle():
+    """A pin of the CUDA path's cylinder chart, crossing and landing that does not go through the oracle (whose surface
+    helpers follow the same decomposition as the kernel's): in B = (0, 0, 2 T) the per-leg PRED state on a cylinder
+    around z must be the closed-form helix from the previous state, with the crossing found here by bisection on
+    |r_T(s)| = R.  Leg 0 starts from the start parameters on a plane; leg 1 starts from the kernel's own FILTERED state on
+    the first cylinder, mapped to space with the chart's definition written out below (include/kf_fit.h KF_SURFACE_CYLINDER)."""
+    TESLA, M_MU, BZ = 2.99792458e-4, 0.1056583755, 2.0
+    rng = np.random.default_rng(5)
+    n = 3000
+    def rec(kind, radius):
+        s = np.zeros(20)
+        s[3:6], s[6:9], s[9:12] = (0, 1, 0), (0, 0, 1), (1, 0, 0)   # plane x = 0: loc0 = y, loc1 = z; cylinders: axis z
+        s[12:14], s[16:18], s[18] = (radius, 500.0), (1e-4, 1e-4), kind
+        return s
+    R1, R2 = 40.0, 75.0
+    geom = np.stack([rec(0, 50.0), rec(1, R1), rec(1, R2)])
+
+    def helix(x0, y0, z0, phi, theta, lam, s):
+        kappa = -lam * BZ * TESLA / np.sin(theta)
+        half = 0.5 * kappa * s
+        chord = s * np.sinc(half / np.pi)
+        return x0 + chord * np.cos(phi + half), y0 + chord * np.sin(phi + half), z0 + s / np.tan(theta), phi + kappa * s
+
+    def to_cylinder(x0, y0, z0, phi, theta, lam, t, R):
+        lo, hi = np.zeros_like(x0), np.full_like(x0, 300.0)
+        for _ in range(80):
+            mid = 0.5 * (lo + hi)
+            x, y, _, _ = helix(x0, y0, z0, phi, theta, lam, mid)
+            inside = x * x + y * y < R * R
+            lo, hi = np.where(inside, mid, lo), np.where(inside, hi, mid)
+        s = 0.5 * (lo + hi)
+        x, y, z, phi1 = helix(x0, y0, z0, phi, theta, lam, s)
+        t1 = t + s / np.sin(theta) * np.sqrt(1.0 + (M_MU * lam) ** 2)
+        return np.stack([R * np.arctan2(y, x), z, phi1, theta, lam, t1], axis=1)
+
+    y0, z0 = rng.uniform(-10, 10, n), rng.uniform(-5, 5, n)
+    phi, theta = rng.uniform(-0.5, 0.5, n), rng.uniform(1.2, 1.9, n)
+    lam = rng.choice([-1.0, 1.0], n) / np.exp(rng.uniform(np.log(0.5), np.log(10.0), n))
+    params0 = np.stack([y0, z0, phi, theta, lam, np.full(n, 1.5)], axis=1)
+    want0 = to_cylinder(np.zeros(n), y0, z0, phi, theta, lam, params0[:, 5], R1)
+    hit1 = want0[:, :2] + rng.normal(0, 0.01, (n, 2))
+    hit2 = to_cylinder(np.zeros(n), y0, z0, phi, theta, lam, params0[:, 5], R2)[:, :2] + rng.normal(0, 0.01, (n, 2))
+    cov0 = np.tile(np.diag([0.05, 0.05, 1e-3, 1e-3, 0.01 * 0.5, 1.0]) ** 2, (n, 1, 1))
+    offsets = np.arange(0, 2 * n + 1, 2, dtype=np.int32)
+    loc = np.stack([hit1, hit2], axis=1).reshape(-1, 2)
+    hb = kf.HostBatch.from_arrays(params0, cov0, 0, offsets, np.tile(np.array([1, 2], np.int32), n), loc, geom,
+                                  field_kind="const", field_b=(0, 0, BZ), options=dict(smooth=1, material=0, max_step_mm=2.0))
+    call = kf.FitCall(kf.DeviceBatch(hb), output_states=B.STATES_PRED | B.STATES_FILT)
+    assert call.geom.surface_kinds == 0b11
+    got = call.run().to_host()
+    assert np.all(got.status & 7 == 0)
+    tol = np.array([2e-9, 2e-9, 1e-10, 1e-12, 1e-15, 1e-8])
+    d0 = np.abs(got.pred_params[:, 0, :] - want0)
+    assert np.all(d0 <= tol), d0.max(axis=0)
+    # leg 1: from the kernel's filtered state on cylinder 1 (chart: alpha = loc0 / R from n = x towards u = y)
+    f = got.filt_params[:, 0, :]
+    a = f[:, 0] / R1
+    want1 = to_cylinder(R1 * np.cos(a), R1 * np.sin(a), f[:, 1], f[:, 2], f[:, 3], f[:, 4], f[:, 5], R2)
+    d1 = np.abs(got.pred_params[:, 1, :] - want1)
+    assert np.all(d1 <= tol), d1.max(axis=0)

@@ -563,3 +563,30 @@ def test_ps10_hits_are_taken_on_the_branch_nearest_the_prediction(kind):
     c = oracle.fit_workload(wl3)
     np.testing.assert_allclose(c.chi2, b.chi2, rtol=1e-9, atol=1e-9)
     np.testing.assert_allclose(c.first_params, b.first_params, rtol=1e-9, atol=1e-9)
+
+
+# ---- PS11: a cylinder is reached from inside ------------------------------------------------------------------
+def test_ps11_a_cylinder_behind_the_start_point_is_not_reached_by_stepping_backwards():
+    """kf_fit.h KF_SURFACE_CYLINDER: "reached along the track's direction of motion from inside".  Straight lines
+    (zero field) from a plane through the origin to the z cylinder of radius 60: from inside the crossing ahead is
+    the textbook root; from a point outside, moving away, there is no crossing ahead (both roots are behind: the
+    oracle once returned the nearer of them, a step backwards, without a status bit); from outside moving inwards,
+    and on a line that misses the cylinder, the leg is refused as well."""
+    fld, opt = oracle.make_field("const", (0, 0, 0.0)), oracle.make_options()
+    start = surface(PLANE, (0.0, 0.0, 0.0), (0, 1, 0), (0, 0, 1))     # the plane x = 0: loc0 = y, loc1 = z
+    cyl = zcyl(60.0)
+    th = 1.45
+    inside = oracle.propagate(fld, opt, np.array([10.0, 1.0, np.pi / 2, th, 0.5, 0.0]), start, cyl)      # from y = 10 along +y
+    assert inside.rc == 0
+    s_t = np.sqrt(60.0 ** 2 - 0.0) - 10.0                                # transverse path to y = 60 on the line x = 0
+    np.testing.assert_allclose(inside.free[:3], [0.0, 60.0, 1.0 + s_t / np.tan(th)], atol=1e-11)
+    away = oracle.propagate(fld, opt, np.array([100.0, 1.0, np.pi / 2, th, 0.5, 0.0]), start, cyl)       # y = 100, along +y
+    assert away.rc == 1, "a start outside the cylinder moving away must stop with KF_ST_PROPAGATION"
+    inwards = oracle.propagate(fld, opt, np.array([100.0, 1.0, -np.pi / 2, th, 0.5, 0.0]), start, cyl)   # y = 100, along -y
+    assert inwards.rc == 1
+    misses = oracle.propagate(fld, opt, np.array([100.0, 1.0, 0.05, th, 0.5, 0.0]), start, cyl)          # y = 100, along +x
+    assert misses.rc == 1
+    # in a field, from inside, nothing changes: PS1's helix crossing (|r_T| = R at the end point)
+    fld2 = oracle.make_field("const", (0, 0, 2.0))
+    r = oracle.propagate(fld2, opt, np.array([10.0, 1.0, 0.3, th, 0.8, 0.0]), start, cyl)
+    assert r.rc == 0 and abs(np.hypot(r.free[0], r.free[1]) - 60.0) < 1e-9
