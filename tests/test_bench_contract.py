@@ -41,3 +41,42 @@ def test_our_arm_refuses_to_run_without_a_gpu():
         pytest.skip("a GPU is present")
     r = run_bench("--steps", "1", "--warmup", "1", "--tracks", "100")
     assert r.returncode != 0 and "no CPU fallback" in (r.stderr + r.stdout)
+
+
+def test_roofline_constants_are_the_numbers_of_the_committed_capture():
+    """bench.py's executed-flop, FP64-pipe and DRAM-traffic constants (CAPTURE_COUNTS) are typed in from an ncu capture
+    summarised under profiles/.  This re-reads that file -- the counter table's dram__bytes_* and FP64-pipe rows and the
+    opcode table -- so that a refreshed capture and the constants cannot drift apart; and the hash that bench.py compares
+    the built sources with must be the hash of csrc/ as committed (else the bench line reports the counts as null)."""
+    import re
+    sys.path.insert(0, ROOT)
+    import bench
+    cc = bench.CAPTURE_COUNTS
+    txt = open(os.path.join(ROOT, cc["source"])).read()
+    rows = {}
+    for line in txt.splitlines():
+        m = re.match(r"\| `([^`]+)` \| ([^|]*) \| (.*) \|$", line)
+        if m and m.group(1) not in rows:
+            rows[m.group(1)] = (m.group(2).strip(), [c.strip() for c in m.group(3).split(" | ")])
+    kernels = rows["Kernel Name"][1]
+    col = {k: [i for i, n in enumerate(kernels) if k in n][0] for k in ("kf_forward_kernel", "kf_rts_kernel")}
+    for k, i in col.items():
+        assert rows["dram__bytes_read.sum"][0] == "Gbyte" and rows["dram__bytes_write.sum"][0] == "Gbyte"
+        got = (float(rows["dram__bytes_read.sum"][1][i]), float(rows["dram__bytes_write.sum"][1][i]))
+        assert got == pytest.approx(cc["dram_gbyte"][k], rel=1e-6), (k, got)
+        pct = float(rows["sm__pipe_fp64_cycles_active.avg.pct_of_peak_sustained_active"][1][i])
+        assert abs(pct - cc["fp64_pipe_pct"][k]) < 0.06, (k, pct)
+        # opcode table: "    void kf::<kernel><...>: ..." followed by "      DFMA    172.182 M ..."
+        blk = txt[txt.index("void kf::" + k):]
+        blk = blk[:blk.index("\n\n")]
+        for op, want in cc["opcodes_M"][k].items():
+            m = re.search(r"^\s+%s\s+([0-9.]+) M" % op, blk, flags=re.M)
+            assert m and float(m.group(1)) == pytest.approx(want, abs=5e-4), (k, op, m and m.group(1))
+    # the derived per-leg figures are those of the opcode counts (DFMA = 2 flop)
+    f = cc["opcodes_M"]["kf_forward_kernel"]
+    assert bench.EXECUTED_PER_LEG["flop"]["kf_forward_kernel"] == pytest.approx(
+        (2 * f["DFMA"] + f["DMUL"] + f["DADD"]) * 1e6 * 32 / (262144 * 30))
+    assert 1800 < bench.EXECUTED_PER_LEG["flop"]["kf_forward_kernel"] < 1830
+    assert bench.NCU_TRAFFIC["bytes_per_leg"]["kf_rts_kernel"] == pytest.approx(441.0, rel=0.02)
+    assert bench.CAPTURE["sources_sha16"] == bench.kernel_sources_sha16(), \
+        "csrc/ changed since the capture bench.py's roofline constants come from: refresh " + cc["source"]
