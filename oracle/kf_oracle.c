@@ -427,9 +427,10 @@ static void global_to_local(const real* s, const real r[3], real* l0, real* l1, 
 
 /* Straight-line path length h from (r, T) to the surface.  Planes and discs: h = n.(c - r)/(n.T), n.T > NT_MIN.
  * Cylinder: with d, T projected on the plane normal to the axis, |d_p + h T_p|^2 = R^2, i.e. a h^2 + 2 b h + c0 = 0,
- * a = |T_p|^2, b = d_p.T_p, c0 = |d_p|^2 - R^2; the root taken is h = -c0 / (b + sqrt(b^2 - a c0)): the crossing
- * ahead for a track inside the cylinder (c0 < 0), and the near root in cancellation-free form once the track is
- * within round-off of the surface and moving outwards.  Returns 0 when the surface cannot be reached. */
+ * a = |T_p|^2, b = d_p.T_p, c0 = |d_p|^2 - R^2; the root taken is the larger of the two textbook roots
+ * (-b -+ sqrt(b^2 - a c0)) / a: the crossing ahead for a track inside the cylinder (c0 < 0), and the root next to the
+ * point once the track is within round-off of the surface and moving outwards.  Returns 0 when the surface cannot
+ * be reached. */
 static int path_to_surface(const real* s, const real r[3], const real T[3], real* h) {
   const real *c = s, *v = s + 6, *n = s + 9;
   if (surf_kind(s) == SURF_CYLINDER) {
@@ -440,10 +441,16 @@ static int path_to_surface(const real* s, const real r[3], const real T[3], real
     for (int a = 0; a < 3; ++a) { dp[a] = d[a] - dz * v[a]; tp[a] = T[a] - tz * v[a]; }
     const real a2 = dot3(tp, tp), b = dot3(dp, tp), c0 = dot3(dp, dp) - R * R;
     const real disc = b * b - a2 * c0;
-    if (!(disc > 0.0)) return 0;
-    const real den = b + sqrt(disc);
-    if (!(den > NT_MIN * R)) return 0;
-    *h = -c0 / den;
+    if (!(disc > 0.0)) return 0;            /* the line misses the cylinder, or runs along its axis (a = 0) */
+    const real sq = sqrt(disc);
+    if (!(b + sq > NT_MIN * R)) return 0;   /* reading U33: grazing, or moving inwards from on / outside the surface */
+    /* the textbook roots (-b -+ sqrt(b^2 - a c0)) / a, both formed; sq > 0 and a > 0, so root_hi > root_lo.  Inside the
+     * cylinder (c0 < 0) they straddle zero and root_hi is the crossing ahead; on the surface to round-off and moving
+     * outwards root_hi is the one next to the point (the correction), root_lo the crossing far behind.  Either way
+     * the larger root.  (Its cancellation next to the surface is an absolute error of eps b / a ~ 1e-14 mm in h: no
+     * stable rearrangement is needed at the 1e-10 bars, and none is used -- the kernel's form is not copied here.) */
+    const real root_lo = (-b - sq) / a2, root_hi = (-b + sq) / a2;
+    *h = root_hi > root_lo ? root_hi : root_lo;
     return 1;
   }
   const real nT = dot3(n, T);
